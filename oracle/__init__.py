@@ -1,0 +1,165 @@
+"""ctypes front end of the CPU oracle (oracle/skv_oracle.c).
+
+TEST INFRASTRUCTURE ONLY: imported by tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs.  The product package never imports this module.
+
+All arrays are numpy, one request at a time, contiguous, in the oracle's canonical layouts:
+  K, V : float16 [L][n][Hkv][d]      Q : float16 [L][Hq][w][d]
+  I    : float32 [L][n]              tier : uint8 [L][n]  (16 / 8 / 4 / 0)
+"""
+import ctypes as C
+from dataclasses import dataclass
+
+import numpy as np
+
+from . import build as _build
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(_build.build())
+        _lib.orc_half_to_float.restype = C.c_float
+        _lib.orc_half_to_float.argtypes = [C.c_uint16]
+        _lib.orc_float_to_half.restype = C.c_uint16
+        _lib.orc_float_to_half.argtypes = [C.c_float]
+        _lib.orc_blob_bytes.restype = C.c_uint64
+        _lib.orc_max_threads.restype = C.c_int
+    return _lib
+
+
+def _p(a):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def _c(a, dtype):
+    a = np.ascontiguousarray(a)
+    assert a.dtype == dtype, (a.dtype, dtype)
+    return a
+
+
+@dataclass(frozen=True)
+class Counts:
+    n16: int
+    n8: int
+    n4: int
+    n0: int
+    budget_q4: int
+    spent_q4: int
+
+    def arr(self):
+        return (C.c_int64 * 6)(self.n16, self.n8, self.n4, self.n0, self.budget_q4, self.spent_q4)
+
+
+def half_to_float(bits: int) -> float:
+    return float(lib().orc_half_to_float(int(bits)))
+
+
+def float_to_half(x: float) -> int:
+    return int(lib().orc_float_to_half(C.c_float(x)))
+
+
+def max_threads() -> int:
+    return int(lib().orc_max_threads())
+
+
+def set_threads(t: int) -> None:
+    lib().orc_set_threads(C.c_int(int(t)))
+
+
+def tier_counts(n, b, n_sink=0, ranges=(), allow_int4=True):
+    """O2.  Returns (Counts, protected bitmap uint8[n]).  Raises ValueError on infeasible/invalid."""
+    rng = np.asarray(ranges, dtype=np.int32).reshape(-1, 2)
+    out = (C.c_int64 * 6)()
+    prot = np.zeros(int(n), dtype=np.uint8)
+    rc = lib().orc_tier_counts(C.c_int64(int(n)), C.c_double(float(b)), C.c_int32(int(n_sink)),
+                               C.c_int32(len(rng)), _p(np.ascontiguousarray(rng)),
+                               C.c_int32(1 if allow_int4 else 0), out, _p(prot))
+    if rc != 0:
+        raise ValueError(f"orc_tier_counts rc={rc}")
+    return Counts(*[int(v) for v in out]), prot
+
+
+def importance(K, Q, causal=True, lam=0.0):
+    """O1.  K [L][n][Hkv][d] f16, Q [L][Hq][w][d] f16 -> I [L][n] f32."""
+    K = _c(K, np.float16)
+    Q = _c(Q, np.float16)
+    L, n, Hkv, d = K.shape
+    L2, Hq, w, d2 = Q.shape
+    assert L == L2 and d == d2 and Hq % Hkv == 0 and 1 <= w <= n
+    I = np.empty((L, n), dtype=np.float32)
+    lib().orc_importance(C.c_int32(L), C.c_int32(Hq), C.c_int32(Hkv), C.c_int32(d), C.c_int64(n),
+                         C.c_int32(w), C.c_int32(1 if causal else 0), C.c_double(float(lam)),
+                         _p(K), _p(Q), _p(I))
+    return I
+
+
+def importance_kvnorm(K, lam=0.0):
+    K = _c(K, np.float16)
+    L, n, Hkv, d = K.shape
+    I = np.empty((L, n), dtype=np.float32)
+    lib().orc_importance_kvnorm(C.c_int32(L), C.c_int32(Hkv), C.c_int32(d), C.c_int64(n),
+                                C.c_double(float(lam)), _p(K), _p(I))
+    return I
+
+
+def assign(I, prot, counts: Counts):
+    """O3.  I [L][n] f32, prot uint8[n] -> tier uint8 [L][n]."""
+    I = _c(I, np.float32)
+    prot = _c(prot, np.uint8)
+    L, n = I.shape
+    tier = np.empty((L, n), dtype=np.uint8)
+    c4 = (C.c_int64 * 4)(counts.n16, counts.n8, counts.n4, counts.n0)
+    lib().orc_assign(C.c_int32(L), C.c_int64(n), _p(I), _p(prot), c4, _p(tier))
+    return tier
+
+
+def blob_bytes(L, Hkv, d, n, counts: Counts) -> int:
+    c4 = (C.c_int64 * 4)(counts.n16, counts.n8, counts.n4, counts.n0)
+    return int(lib().orc_blob_bytes(C.c_int32(L), C.c_int32(Hkv), C.c_int32(d), C.c_int64(n), c4))
+
+
+def pack(K, V, tier, counts: Counts, allow_int4=True):
+    """O4+O5.  Returns the SKV1 blob as uint8[total_bytes]."""
+    K = _c(K, np.float16)
+    V = _c(V, np.float16)
+    tier = _c(tier, np.uint8)
+    L, n, Hkv, d = K.shape
+    assert V.shape == K.shape and tier.shape == (L, n)
+    blob = np.empty(blob_bytes(L, Hkv, d, n, counts), dtype=np.uint8)
+    rc = lib().orc_pack(C.c_int32(L), C.c_int32(Hkv), C.c_int32(d), C.c_int64(n), _p(K), _p(V),
+                        _p(tier), counts.arr(), C.c_int32(1 if allow_int4 else 0), _p(blob))
+    if rc != 0:
+        raise ValueError(f"orc_pack rc={rc} (tier map does not match counts)")
+    return blob
+
+
+def unpack(blob, L, Hkv, d, n):
+    """O6.  Returns (K, V, tier) dense."""
+    blob = _c(blob, np.uint8)
+    K = np.empty((L, n, Hkv, d), dtype=np.float16)
+    V = np.empty((L, n, Hkv, d), dtype=np.float16)
+    tier = np.empty((L, n), dtype=np.uint8)
+    rc = lib().orc_unpack(_p(blob), C.c_uint64(blob.size), C.c_int32(L), C.c_int32(Hkv), C.c_int32(d),
+                          C.c_int64(n), _p(K), _p(V), _p(tier))
+    if rc != 0:
+        raise ValueError(f"orc_unpack rc={rc} (bad blob)")
+    return K, V, tier
+
+
+def quantize_vector(x, qmax):
+    """O4 on one vector.  x float16[d] -> (amax_bits, int8[d])."""
+    x = _c(x, np.float16)
+    q = np.empty(x.size, dtype=np.int8)
+    ab = C.c_uint16(0)
+    lib().orc_quantize_vector(_p(x), C.c_int32(x.size), C.c_int32(int(qmax)), C.byref(ab), _p(q))
+    return int(ab.value), q
+
+
+def dequantize_vector(q, qmax, amax_bits):
+    q = _c(q, np.int8)
+    y = np.empty(q.size, dtype=np.float16)
+    lib().orc_dequantize_vector(_p(q), C.c_int32(q.size), C.c_int32(int(qmax)), C.c_uint16(int(amax_bits)), _p(y))
+    return y

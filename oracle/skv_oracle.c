@@ -1,0 +1,500 @@
+/*
+ * skv_oracle.c -- plain, slow, obviously-correct CPU ORACLE for the SpectrumKV
+ * per-token mixed-precision KV transfer path (arxiv/paper_2606_08635).
+ *
+ * TEST INFRASTRUCTURE ONLY.  Nothing in the product path (paper_2606_08635_b200/)
+ * may import, call, link or execute this file; only tests/, __graft_entry__.smoke()
+ * and bench.py's cpu_baseline / --impl reference legs may.  It shares no code,
+ * header, table or constant generator with the CUDA path.
+ *
+ * Written from /root/reference/PAPER.md and the readings P1..P14 recorded in
+ * DESIGN.md (the paper is silent on every byte-level detail).  Citations are
+ * PAPER.md:<line> plus the section / equation.  No blocking, fusion or
+ * reordering beyond what the cited definition states; the OpenMP pragmas only
+ * split INDEPENDENT layers across threads (no arithmetic is reordered).
+ *
+ * Canonical layouts of this oracle (one request at a time, all contiguous):
+ *   K, V : fp16 bits (uint16_t) [L][n][Hkv][d]     (token-major)
+ *   Q    : fp16 bits            [L][Hq][w][d]      (window query i is at position n-w+i)
+ *   I    : float32              [L][n]
+ *   tier : uint8                [L][n]  values 16, 8, 4, 0 (0 = dropped)
+ *
+ * Parity pins (tests/test_oracle_*.py, -m "not gpu"):
+ *   half<->float conversion : exhaustive against numpy float16
+ *   importance              : sum_j A_j = 1, K==0 closed forms, one-hot key, decay closed form,
+ *                             float64 torch.softmax(QK^T/sqrt d) on CPU
+ *   tier counts             : Eq. 14-15 fractions, PAPER.md:301 (b=0.3 -> 80% INT4), :543 (60% sent)
+ *   selection               : O(n^2) brute-force rank, Prop. 1 monotonicity, sinks FP16
+ *   quantizer               : worked examples W1..W5 (hand-computed), error bound <= scale/2
+ *   wire format             : W6 layout, hand-written blob, Eq. 1 byte identity
+ *   pack/unpack             : b=1 identity round trip
+ * PARITY UNPINNED (conventions of this build with no external fixture):
+ *   group size = one head vector, fp16 amax scale record, reciprocal multiply,
+ *   nibble order, segment order/alignment, tie direction, causal default,
+ *   mean normalisation, per-layer map.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+/* ------------------------------------------------------------------------ */
+/* IEEE-754 binary16 <-> binary32, written out bit by bit.                  */
+/* ------------------------------------------------------------------------ */
+
+/* binary16 -> binary32 is exact: 1 sign, 5 exponent (bias 15), 10 fraction bits. */
+float orc_half_to_float(uint16_t h)
+{
+    uint32_t sign = (uint32_t)(h >> 15) & 1u;
+    uint32_t exp  = (uint32_t)(h >> 10) & 0x1Fu;
+    uint32_t frac = (uint32_t)h & 0x3FFu;
+    double v;
+    if (exp == 0)        v = ldexp((double)frac, -24);              /* subnormal / zero: frac * 2^-24 */
+    else if (exp == 31)  v = frac ? (double)NAN : (double)INFINITY; /* not expected on the path       */
+    else                 v = ldexp((double)(1024u + frac), (int)exp - 25); /* (1+frac/1024)*2^(exp-15) */
+    return (float)(sign ? -v : v);
+}
+
+/* binary32 -> binary16, round to nearest, ties to even (the value is finite on the path). */
+uint16_t orc_float_to_half(float f)
+{
+    uint16_t sign = (uint16_t)(signbit(f) ? 0x8000u : 0u);
+    double a = fabs((double)f);
+    if (isnan(f)) return (uint16_t)(sign | 0x7E00u);
+    if (a == 0.0) return sign;
+    /* choose the binary16 quantum (ulp) for the binade of a; smallest quantum is 2^-24 */
+    int e;
+    (void)frexp(a, &e);          /* a = m * 2^e, m in [0.5,1)  => a in [2^(e-1), 2^e) */
+    int q = e - 11;              /* 11 significant bits => ulp = 2^(e-1-10)           */
+    if (q < -24) q = -24;        /* subnormal range                                    */
+    double scaled = ldexp(a, -q);         /* exact */
+    double r = nearbyint(scaled);         /* default FE_TONEAREST: ties to even */
+    double v = ldexp(r, q);
+    if (v >= 65520.0) return (uint16_t)(sign | 0x7C00u);   /* overflow to inf (never on the path) */
+    /* re-encode v (exactly representable in binary16) */
+    if (v < ldexp(1.0, -14))              /* subnormal: frac = v / 2^-24 */
+        return (uint16_t)(sign | (uint16_t)ldexp(v, 24));
+    (void)frexp(v, &e);                   /* v in [2^(e-1), 2^e) */
+    uint32_t exp  = (uint32_t)(e - 1 + 15);
+    uint32_t frac = (uint32_t)(ldexp(v, 10 - (e - 1))) - 1024u;
+    return (uint16_t)(sign | (exp << 10) | frac);
+}
+
+/* ------------------------------------------------------------------------ */
+/* O1. Importance  (Eq. 13; logits q^T k / sqrt(d) PAPER.md:109; */
+/*     Alg. 1 step 2 PAPER.md:239; readings P1, P2, P4 in DESIGN.md)          */
+/* ------------------------------------------------------------------------ */
+/*
+ * For layer l, query head h (KV head g = h / (Hq/Hkv)), window query i at position
+ * pos_i = n-w+i :  z_j = (sum_c Q[l,h,i,c] K[l,j,g,c]) / sqrt(d);  causal => keys j > pos_i excluded;
+ * p = softmax(z);  A[l,j] = (1/(Hq*w)) sum_{h,i} p_{h,i,j};  I[l,j] = A[l,j] * exp(-lambda*(n-1-j)).
+ * All in float64; result cast to float32 (RN).
+ */
+void orc_importance(int32_t L, int32_t Hq, int32_t Hkv, int32_t d, int64_t n, int32_t w,
+                    int32_t causal, double lambda,
+                    const uint16_t *K, const uint16_t *Q, float *I)
+{
+    const int32_t G = Hq / Hkv;
+    const double inv_sqrt_d = 1.0 / sqrt((double)d);
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int32_t l = 0; l < L; ++l) {
+        double *A = (double *)calloc((size_t)n, sizeof(double));
+        double *z = (double *)malloc((size_t)n * sizeof(double));
+        double *kq = (double *)malloc((size_t)d * sizeof(double));
+        for (int32_t h = 0; h < Hq; ++h) {
+            const int32_t g = h / G;
+            for (int32_t i = 0; i < w; ++i) {
+                const int64_t pos = n - w + i;
+                const int64_t last = causal ? pos : n - 1;      /* keys 0..last take part */
+                const uint16_t *q = Q + (((size_t)l * Hq + h) * w + i) * d;
+                for (int32_t c = 0; c < d; ++c) kq[c] = (double)orc_half_to_float(q[c]);
+                double zmax = -INFINITY;
+                for (int64_t j = 0; j <= last; ++j) {
+                    const uint16_t *k = K + (((size_t)l * n + j) * Hkv + g) * d;
+                    double dot = 0.0;
+                    for (int32_t c = 0; c < d; ++c) dot += kq[c] * (double)orc_half_to_float(k[c]);
+                    z[j] = dot * inv_sqrt_d;
+                    if (z[j] > zmax) zmax = z[j];
+                }
+                double Z = 0.0;
+                for (int64_t j = 0; j <= last; ++j) { z[j] = exp(z[j] - zmax); Z += z[j]; }
+                for (int64_t j = 0; j <= last; ++j) A[j] += z[j] / Z;
+            }
+        }
+        const double norm = 1.0 / ((double)Hq * (double)w);
+        for (int64_t j = 0; j < n; ++j) {
+            double delta = (double)(n - 1 - j);                 /* P4: 0-based recency distance */
+            I[(size_t)l * n + j] = (float)(A[j] * norm * exp(-lambda * delta));
+        }
+        free(A); free(z); free(kq);
+    }
+}
+
+/* ------------------------------------------------------------------------ */
+/* O2. Tier counts (PAPER.md:51-58 Eq. 2-3, :220-228 Eq. 14-15, :230        */
+/*     SinkProtect, :543 two-tier drop; reading P5)                          */
+/* ------------------------------------------------------------------------ */
+/*
+ * Quarter-units: cost 4/2/1/0 for tiers 16/8/4/0.  Q = floor(4*b*n + 1e-6).
+ * prot (nullable, [n]) receives the protected bitmap = [0,s) U ranges.
+ * out = {n16, n8, n4, n0, Q, spent}.  Returns 0, -1 invalid argument, -3 infeasible.
+ */
+int orc_tier_counts(int64_t n, double b, int32_t n_sink, int32_t n_ranges, const int32_t *ranges,
+                    int32_t allow_int4, int64_t out[6], uint8_t *prot)
+{
+    if (n <= 0 || !(b > 0.0) || n_sink < 0 || n_ranges < 0) return -1;
+    if (b > 1.0) b = 1.0;
+    uint8_t *p = prot ? prot : (uint8_t *)malloc((size_t)n);
+    memset(p, 0, (size_t)n);
+    for (int64_t j = 0; j < n && j < n_sink; ++j) p[j] = 1;
+    for (int32_t r = 0; r < n_ranges; ++r) {
+        int64_t beg = ranges[2 * r], end = ranges[2 * r + 1];
+        if (beg < 0 || end > n || beg > end) { if (!prot) free(p); return -1; }
+        for (int64_t j = beg; j < end; ++j) p[j] = 1;
+    }
+    int64_t P = 0;
+    for (int64_t j = 0; j < n; ++j) P += p[j];
+    if (!prot) free(p);
+
+    const int64_t Q = (int64_t)floor(4.0 * b * (double)n + 1e-6);
+    const int64_t m = n - P;
+    const int64_t R = Q - 4 * P;             /* budget left after paying FP16 for the protected set */
+    if (R < 0) return -3;
+    int64_t n16 = P, n8 = 0, n4 = 0, n0 = 0;
+    if (R >= 4 * m) {                        /* everything FP16 (Eq. 15 at b = 1) */
+        n16 = n;
+    } else if (R >= 2 * m) {                 /* FP16 + INT8 mix (Eq. 15) */
+        int64_t extra = (R - 2 * m) / 2;     /* each FP16 upgrade over INT8 costs 2 quarter-units */
+        n16 = P + extra;
+        n8 = m - extra;
+    } else if (allow_int4) {
+        if (R >= m) {                        /* INT8 + INT4 mix (Eq. 14) */
+            n8 = R - m;                      /* each INT8 upgrade over INT4 costs 1 */
+            n4 = m - n8;
+        } else {                             /* below b = 0.25: INT4 + drop (by analogy with :543) */
+            n4 = R;
+            n0 = m - R;
+        }
+    } else {                                 /* 2-tier: INT8 + drop */
+        n8 = R / 2;
+        n0 = m - n8;
+    }
+    out[0] = n16; out[1] = n8; out[2] = n4; out[3] = n0;
+    out[4] = Q;   out[5] = 4 * n16 + 2 * n8 + n4;
+    return 0;
+}
+
+/* ------------------------------------------------------------------------ */
+/* O3. Selection (PAPER.md:216 "pinned before ranking", :240 Alg. 1 step 3, */
+/*     Prop. 1; tie-break reading P6)                           */
+/* ------------------------------------------------------------------------ */
+typedef struct { float key; int64_t pos; } orc_item;
+
+static int orc_item_cmp(const void *a, const void *b)
+{
+    const orc_item *x = (const orc_item *)a, *y = (const orc_item *)b;
+    if (x->key > y->key) return -1;          /* higher importance first            */
+    if (x->key < y->key) return 1;
+    if (x->pos < y->pos) return -1;          /* P6: equal scores => lower position first */
+    if (x->pos > y->pos) return 1;
+    return 0;
+}
+
+/* One layer: I[n], prot[n] -> tier[n]; counts = {n16,n8,n4,n0} from orc_tier_counts. */
+void orc_assign_layer(int64_t n, const float *I, const uint8_t *prot, const int64_t counts[4],
+                      uint8_t *tier)
+{
+    orc_item *it = (orc_item *)malloc((size_t)n * sizeof(orc_item));
+    int64_t m = 0, P = 0;
+    for (int64_t j = 0; j < n; ++j) {
+        if (prot[j]) { tier[j] = 16; ++P; continue; }
+        float key = I[j];
+        if (!(key > 0.0f)) key = 0.0f;       /* NaN, negative, -0 -> +0 (lowest rank) */
+        it[m].key = key; it[m].pos = j; ++m;
+    }
+    qsort(it, (size_t)m, sizeof(orc_item), orc_item_cmp);
+    const int64_t c16 = counts[0] - P, c8 = counts[1], c4 = counts[2];
+    for (int64_t r = 0; r < m; ++r) {
+        uint8_t t;
+        if (r < c16) t = 16;
+        else if (r < c16 + c8) t = 8;
+        else if (r < c16 + c8 + c4) t = 4;
+        else t = 0;
+        tier[it[r].pos] = t;
+    }
+    free(it);
+}
+
+void orc_assign(int32_t L, int64_t n, const float *I, const uint8_t *prot, const int64_t counts[4],
+                uint8_t *tier)
+{
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int32_t l = 0; l < L; ++l)
+        orc_assign_layer(n, I + (size_t)l * n, prot, counts, tier + (size_t)l * n);
+}
+
+/* ------------------------------------------------------------------------ */
+/* O5. Wire format SKV1 (paper: "mixed-precision payload" PAPER.md:241;     */
+/*     layout is reading P9, DESIGN.md / docs in include/skv.h)              */
+/* ------------------------------------------------------------------------ */
+typedef struct {
+    uint64_t tier_map_off, layer0_off, layer_stride, seg_off[10], seg_bytes[10], total_bytes;
+} orc_layout_t;
+
+static uint64_t pad256(uint64_t x) { return (x + 255u) / 256u * 256u; }
+
+/* segment order: K16 V16 K8 V8 K4 V4 SK8 SV8 SK4 SV4 */
+void orc_layout(int32_t L, int32_t Hkv, int32_t d, int64_t n, const int64_t counts[4], orc_layout_t *lo)
+{
+    const uint64_t n16 = (uint64_t)counts[0], n8 = (uint64_t)counts[1], n4 = (uint64_t)counts[2];
+    const uint64_t H = (uint64_t)Hkv, D = (uint64_t)d;
+    const uint64_t raw[10] = {
+        n16 * H * D * 2, n16 * H * D * 2,      /* K16, V16 : f16            */
+        n8 * H * D,      n8 * H * D,           /* K8,  V8  : i8             */
+        n4 * H * D / 2,  n4 * H * D / 2,       /* K4,  V4  : two codes/byte */
+        n8 * H * 2,      n8 * H * 2,           /* SK8, SV8 : f16 amax       */
+        n4 * H * 2,      n4 * H * 2 };         /* SK4, SV4 : f16 amax       */
+    lo->tier_map_off = 256;
+    lo->layer0_off = 256 + pad256((uint64_t)L * (uint64_t)n);
+    uint64_t off = 0;
+    for (int s = 0; s < 10; ++s) { lo->seg_off[s] = off; lo->seg_bytes[s] = raw[s]; off += pad256(raw[s]); }
+    lo->layer_stride = off;
+    lo->total_bytes = lo->layer0_off + (uint64_t)L * lo->layer_stride;
+}
+
+uint64_t orc_blob_bytes(int32_t L, int32_t Hkv, int32_t d, int64_t n, const int64_t counts[4])
+{
+    orc_layout_t lo; orc_layout(L, Hkv, d, n, counts, &lo); return lo.total_bytes;
+}
+
+static void put_u32(uint8_t *p, uint32_t v) { for (int i = 0; i < 4; ++i) p[i] = (uint8_t)(v >> (8 * i)); }
+static void put_u64(uint8_t *p, uint64_t v) { for (int i = 0; i < 8; ++i) p[i] = (uint8_t)(v >> (8 * i)); }
+static uint32_t get_u32(const uint8_t *p) { uint32_t v = 0; for (int i = 0; i < 4; ++i) v |= (uint32_t)p[i] << (8 * i); return v; }
+static uint64_t get_u64(const uint8_t *p) { uint64_t v = 0; for (int i = 0; i < 8; ++i) v |= (uint64_t)p[i] << (8 * i); return v; }
+
+/* ------------------------------------------------------------------------ */
+/* O4. Quantizer ("standard symmetric INT4" PAPER.md:583; K and V quantized */
+/*     independently PAPER.md:241; readings P7, P8)                          */
+/* ------------------------------------------------------------------------ */
+/*
+ * One group = one head vector of d fp16 values.  qmax = 127 (INT8) / 7 (INT4).
+ * amax = max|x| (an fp16 value, stored losslessly as the 2-byte scale record).
+ * inv = fl32(qmax / amax), scale = fl32(amax / qmax) (0 when amax = 0).
+ * q = clamp(rint(fl32(x * inv)), -qmax, qmax), rint = round half to even.
+ */
+static uint16_t orc_amax_bits(const uint16_t *x, int32_t d)
+{
+    uint16_t best = 0;                                   /* |x| as fp16 bits: monotone for finite values */
+    for (int32_t c = 0; c < d; ++c) { uint16_t a = (uint16_t)(x[c] & 0x7FFFu); if (a > best) best = a; }
+    return best;
+}
+
+void orc_quantize_vector(const uint16_t *x, int32_t d, int32_t qmax, uint16_t *amax_out, int8_t *q)
+{
+    const uint16_t ab = orc_amax_bits(x, d);
+    const float amax = orc_half_to_float(ab);
+    volatile float inv = 0.0f;                           /* volatile: force a rounded binary32 at each step */
+    if (amax != 0.0f) inv = (float)qmax / amax;
+    for (int32_t c = 0; c < d; ++c) {
+        volatile float t = orc_half_to_float(x[c]) * inv;
+        float r = rintf(t);                              /* FE_TONEAREST: ties to even */
+        if (r > (float)qmax) r = (float)qmax;
+        if (r < -(float)qmax) r = -(float)qmax;
+        q[c] = (int8_t)r;
+    }
+    *amax_out = ab;
+}
+
+/* y = f16_rn(fl32(float(q) * scale)), scale = fl32(amax / qmax).  ("table lookup") */
+void orc_dequantize_vector(const int8_t *q, int32_t d, int32_t qmax, uint16_t amax_bits, uint16_t *y)
+{
+    const float amax = orc_half_to_float(amax_bits);
+    volatile float scale = 0.0f;
+    if (amax != 0.0f) scale = amax / (float)qmax;
+    for (int32_t c = 0; c < d; ++c) {
+        volatile float v = (float)q[c] * scale;
+        y[c] = orc_float_to_half(v);
+    }
+}
+
+/* ------------------------------------------------------------------------ */
+/* O5/O4. Pack (Alg. 1 step 4)                                 */
+/* ------------------------------------------------------------------------ */
+/* counts6 = {n16,n8,n4,n0,Q,spent}; blob must hold orc_blob_bytes(); written completely
+ * (every pad byte zero).  Returns 0, or -1 if a layer's tier map disagrees with counts. */
+int orc_pack(int32_t L, int32_t Hkv, int32_t d, int64_t n, const uint16_t *K, const uint16_t *V,
+             const uint8_t *tier, const int64_t counts6[6], int32_t allow_int4, uint8_t *blob)
+{
+    orc_layout_t lo; orc_layout(L, Hkv, d, n, counts6, &lo);
+    memset(blob, 0, (size_t)lo.total_bytes);
+    put_u32(blob + 0, 0x31564B53u);  put_u32(blob + 4, 1u);
+    put_u32(blob + 8, (uint32_t)L);  put_u32(blob + 12, (uint32_t)Hkv);
+    put_u32(blob + 16, (uint32_t)d); put_u32(blob + 20, (uint32_t)n);
+    put_u32(blob + 24, (uint32_t)counts6[0]); put_u32(blob + 28, (uint32_t)counts6[1]);
+    put_u32(blob + 32, (uint32_t)counts6[2]); put_u32(blob + 36, (uint32_t)counts6[3]);
+    put_u32(blob + 40, allow_int4 ? 1u : 0u); put_u32(blob + 44, 0u);
+    put_u64(blob + 48, (uint64_t)counts6[4]);
+    put_u64(blob + 56, lo.tier_map_off); put_u64(blob + 64, lo.layer0_off); put_u64(blob + 72, lo.layer_stride);
+    for (int s = 0; s < 10; ++s) put_u64(blob + 80 + 8 * s, lo.seg_off[s]);
+    put_u64(blob + 160, lo.total_bytes);
+    memcpy(blob + lo.tier_map_off, tier, (size_t)L * (size_t)n);
+
+    int bad = 0;
+    const size_t row = (size_t)Hkv * (size_t)d;          /* elements in one token's K (or V) row */
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int32_t l = 0; l < L; ++l) {
+        uint8_t *base = blob + lo.layer0_off + (size_t)l * lo.layer_stride;
+        int8_t *q = (int8_t *)malloc((size_t)d);
+        int64_t slot16 = 0, slot8 = 0, slot4 = 0;        /* stable compaction: ascending position */
+        for (int64_t j = 0; j < n; ++j) {
+            const uint8_t t = tier[(size_t)l * n + j];
+            for (int kv = 0; kv < 2; ++kv) {
+                const uint16_t *src = (kv ? V : K) + ((size_t)l * n + j) * row;
+                if (t == 16) {
+                    uint8_t *dst = base + lo.seg_off[0 + kv] + (size_t)slot16 * row * 2;
+                    for (size_t e = 0; e < row; ++e) { dst[2 * e] = (uint8_t)src[e]; dst[2 * e + 1] = (uint8_t)(src[e] >> 8); }
+                } else if (t == 8) {
+                    uint8_t *dst = base + lo.seg_off[2 + kv] + (size_t)slot8 * row;
+                    uint8_t *sc  = base + lo.seg_off[6 + kv] + (size_t)slot8 * Hkv * 2;
+                    for (int32_t h = 0; h < Hkv; ++h) {
+                        uint16_t ab;
+                        orc_quantize_vector(src + (size_t)h * d, d, 127, &ab, q);
+                        for (int32_t c = 0; c < d; ++c) dst[(size_t)h * d + c] = (uint8_t)q[c];
+                        sc[2 * h] = (uint8_t)ab; sc[2 * h + 1] = (uint8_t)(ab >> 8);
+                    }
+                } else if (t == 4) {
+                    uint8_t *dst = base + lo.seg_off[4 + kv] + (size_t)slot4 * row / 2;
+                    uint8_t *sc  = base + lo.seg_off[8 + kv] + (size_t)slot4 * Hkv * 2;
+                    for (int32_t h = 0; h < Hkv; ++h) {
+                        uint16_t ab;
+                        orc_quantize_vector(src + (size_t)h * d, d, 7, &ab, q);
+                        for (int32_t c = 0; c < d; c += 2)   /* element 2i low nibble, 2i+1 high nibble */
+                            dst[((size_t)h * d + c) / 2] = (uint8_t)((q[c] & 0xF) | ((q[c + 1] & 0xF) << 4));
+                        sc[2 * h] = (uint8_t)ab; sc[2 * h + 1] = (uint8_t)(ab >> 8);
+                    }
+                }                                        /* t == 0: dropped, no bytes */
+            }
+            if (t == 16) ++slot16; else if (t == 8) ++slot8; else if (t == 4) ++slot4;
+        }
+        free(q);
+        if (slot16 != counts6[0] || slot8 != counts6[1] || slot4 != counts6[2]) {
+#pragma omp atomic write
+            bad = 1;
+        }
+    }
+    return bad ? -1 : 0;
+}
+
+/* ------------------------------------------------------------------------ */
+/* O6. Unpack (decode side; dropped -> +0.0 fill, reading P10) */
+/* ------------------------------------------------------------------------ */
+/* Parses the header (dims must match the arguments), returns 0 or -5 (bad blob). */
+int orc_unpack(const uint8_t *blob, uint64_t blob_bytes, int32_t L, int32_t Hkv, int32_t d, int64_t n,
+               uint16_t *K, uint16_t *V, uint8_t *tier_out)
+{
+    if (blob_bytes < 256) return -5;
+    if (get_u32(blob) != 0x31564B53u || get_u32(blob + 4) != 1u) return -5;
+    if (get_u32(blob + 8) != (uint32_t)L || get_u32(blob + 12) != (uint32_t)Hkv ||
+        get_u32(blob + 16) != (uint32_t)d || get_u32(blob + 20) != (uint32_t)n) return -5;
+    int64_t counts[4] = { get_u32(blob + 24), get_u32(blob + 28), get_u32(blob + 32), get_u32(blob + 36) };
+    if (counts[0] + counts[1] + counts[2] + counts[3] != n) return -5;
+    orc_layout_t lo; orc_layout(L, Hkv, d, n, counts, &lo);
+    if (get_u64(blob + 56) != lo.tier_map_off || get_u64(blob + 64) != lo.layer0_off ||
+        get_u64(blob + 72) != lo.layer_stride || get_u64(blob + 160) != lo.total_bytes ||
+        lo.total_bytes != blob_bytes) return -5;
+    for (int s = 0; s < 10; ++s) if (get_u64(blob + 80 + 8 * s) != lo.seg_off[s]) return -5;
+    const uint8_t *tier = blob + lo.tier_map_off;
+    if (tier_out) memcpy(tier_out, tier, (size_t)L * (size_t)n);
+
+    const size_t row = (size_t)Hkv * (size_t)d;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int32_t l = 0; l < L; ++l) {
+        const uint8_t *base = blob + lo.layer0_off + (size_t)l * lo.layer_stride;
+        int8_t *q = (int8_t *)malloc((size_t)d);
+        int64_t slot16 = 0, slot8 = 0, slot4 = 0;
+        for (int64_t j = 0; j < n; ++j) {
+            const uint8_t t = tier[(size_t)l * n + j];
+            for (int kv = 0; kv < 2; ++kv) {
+                uint16_t *dst = (kv ? V : K) + ((size_t)l * n + j) * row;
+                if (t == 16) {
+                    const uint8_t *src = base + lo.seg_off[0 + kv] + (size_t)slot16 * row * 2;
+                    for (size_t e = 0; e < row; ++e) dst[e] = (uint16_t)(src[2 * e] | (src[2 * e + 1] << 8));
+                } else if (t == 8) {
+                    const uint8_t *src = base + lo.seg_off[2 + kv] + (size_t)slot8 * row;
+                    const uint8_t *sc  = base + lo.seg_off[6 + kv] + (size_t)slot8 * Hkv * 2;
+                    for (int32_t h = 0; h < Hkv; ++h) {
+                        for (int32_t c = 0; c < d; ++c) q[c] = (int8_t)src[(size_t)h * d + c];
+                        orc_dequantize_vector(q, d, 127, (uint16_t)(sc[2 * h] | (sc[2 * h + 1] << 8)), dst + (size_t)h * d);
+                    }
+                } else if (t == 4) {
+                    const uint8_t *src = base + lo.seg_off[4 + kv] + (size_t)slot4 * row / 2;
+                    const uint8_t *sc  = base + lo.seg_off[8 + kv] + (size_t)slot4 * Hkv * 2;
+                    for (int32_t h = 0; h < Hkv; ++h) {
+                        for (int32_t c = 0; c < d; ++c) {
+                            uint8_t byte = src[((size_t)h * d + c) / 2];
+                            int nib = (c & 1) ? (byte >> 4) : (byte & 0xF);
+                            q[c] = (int8_t)(nib >= 8 ? nib - 16 : nib);      /* 4-bit two's complement */
+                        }
+                        orc_dequantize_vector(q, d, 7, (uint16_t)(sc[2 * h] | (sc[2 * h + 1] << 8)), dst + (size_t)h * d);
+                    }
+                } else {
+                    for (size_t e = 0; e < row; ++e) dst[e] = 0;             /* P10: dropped => +0.0 */
+                }
+            }
+            if (t == 16) ++slot16; else if (t == 8) ++slot8; else if (t == 4) ++slot4;
+        }
+        free(q);
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------ */
+/* NEXT-1: KV-norm fallback score ("or a KV-norm          */
+/* fallback").  Reading P15: A_j = mean over KV heads of the L2 norm of the  */
+/* key vector, normalised to sum 1 over j; then the same decay.  UNPINNED.   */
+/* ------------------------------------------------------------------------ */
+void orc_importance_kvnorm(int32_t L, int32_t Hkv, int32_t d, int64_t n, double lambda,
+                           const uint16_t *K, float *I)
+{
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int32_t l = 0; l < L; ++l) {
+        double *A = (double *)malloc((size_t)n * sizeof(double));
+        double total = 0.0;
+        for (int64_t j = 0; j < n; ++j) {
+            double acc = 0.0;
+            for (int32_t g = 0; g < Hkv; ++g) {
+                const uint16_t *k = K + (((size_t)l * n + j) * Hkv + g) * d;
+                double ss = 0.0;
+                for (int32_t c = 0; c < d; ++c) { double v = (double)orc_half_to_float(k[c]); ss += v * v; }
+                acc += sqrt(ss);
+            }
+            A[j] = acc / (double)Hkv;
+            total += A[j];
+        }
+        for (int64_t j = 0; j < n; ++j) {
+            double a = total > 0.0 ? A[j] / total : 1.0 / (double)n;
+            I[(size_t)l * n + j] = (float)(a * exp(-lambda * (double)(n - 1 - j)));
+        }
+        free(A);
+    }
+}
+
+int orc_max_threads(void)
+{
+#ifdef _OPENMP
+    extern int omp_get_max_threads(void);
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+void orc_set_threads(int t)
+{
+#ifdef _OPENMP
+    extern void omp_set_num_threads(int);
+    omp_set_num_threads(t);
+#else
+    (void)t;
+#endif
+}

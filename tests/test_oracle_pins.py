@@ -1,0 +1,541 @@
+"""Pins for the CPU oracle (oracle/skv_oracle.c) against what the paper and the mathematics fix.
+
+None of these tests touches the CUDA path.  Each pin is chosen so that a plausible mistake in the
+oracle (dropped term, wrong sign/index, transposed operand, wrong rounding) fails it.
+"""
+import os
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from conftest import read_golden
+
+GOLD = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+# ----------------------------------------------------------------------------------------------
+# fp16 <-> fp32 conversion: pinned exhaustively against numpy's float16 (an independent library)
+# ----------------------------------------------------------------------------------------------
+def test_half_to_float_exhaustive():
+    bits = np.arange(65536, dtype=np.uint16)
+    ref = bits.view(np.float16).astype(np.float32)
+    got = np.array([oracle.half_to_float(int(b)) for b in bits], dtype=np.float32)
+    nan = np.isnan(ref)
+    assert np.array_equal(np.isnan(got), nan)
+    assert np.array_equal(got[~nan].view(np.uint32), ref[~nan].view(np.uint32))
+
+
+def test_float_to_half_rne_against_numpy():
+    rng = np.random.default_rng(0)
+    halves = np.arange(0, 0x7C00, dtype=np.uint16).view(np.float16).astype(np.float64)
+    mids = ((halves[:-1] + halves[1:]) / 2).astype(np.float32)          # exact ties between neighbours
+    near = np.concatenate([np.nextafter(mids, np.float32(np.inf)), np.nextafter(mids, np.float32(-np.inf))])
+    rand = np.concatenate([rng.standard_normal(20000) * s for s in (1e-7, 1e-4, 1.0, 100.0, 3e4)]).astype(np.float32)
+    edge = np.array([0.0, -0.0, 65504.0, 65519.0, 5.96e-8, 2.98e-8, 2.9802322e-8, 6.1e-5, 6.1035156e-5], dtype=np.float32)
+    xs = np.concatenate([mids, near, rand, edge, -mids[::7]])
+    xs = xs[np.abs(xs) < 65520.0]
+    ref = xs.astype(np.float16).view(np.uint16)
+    got = np.array([oracle.float_to_half(float(x)) for x in xs], dtype=np.uint16)
+    assert np.array_equal(got, ref)
+
+
+# ----------------------------------------------------------------------------------------------
+# O2 tier counts
+# ----------------------------------------------------------------------------------------------
+def test_tier_fractions_from_paper():
+    for b, a4, n16, n8, n4, n0 in read_golden(os.path.join(GOLD, "tier_fractions.txt")):
+        c, prot = oracle.tier_counts(10000, float(b), 0, [], bool(int(a4)))
+        assert (c.n16, c.n8, c.n4, c.n0) == (int(n16), int(n8), int(n4), int(n0)), b
+        assert prot.sum() == 0
+
+
+def test_tier_counts_invariants_sweep():
+    rng = np.random.default_rng(1)
+    for _ in range(3000):
+        n = int(rng.integers(1, 5000))
+        b = float(rng.choice([rng.uniform(0.01, 1.2), rng.integers(1, 41) / 40.0]))
+        s = int(rng.integers(0, min(n, 9)))
+        rngs = []
+        for _r in range(int(rng.integers(0, 3))):
+            a = int(rng.integers(0, n + 1)); e = int(rng.integers(a, n + 1)); rngs.append((a, e))
+        a4 = bool(rng.integers(0, 2))
+        prot_ref = np.zeros(n, bool); prot_ref[:s] = True
+        for a, e in rngs:
+            prot_ref[a:e] = True
+        P = int(prot_ref.sum())
+        Q = int(np.floor(4 * min(b, 1.0) * n + 1e-6))
+        try:
+            c, prot = oracle.tier_counts(n, b, s, rngs, a4)
+        except ValueError:
+            assert 4 * P > Q            # only infeasible budgets are refused
+            continue
+        assert 4 * P <= Q
+        assert np.array_equal(prot.astype(bool), prot_ref)
+        assert c.budget_q4 == Q
+        assert c.n16 + c.n8 + c.n4 + c.n0 == n and min(c.n16, c.n8, c.n4, c.n0) >= 0
+        assert c.spent_q4 == 4 * c.n16 + 2 * c.n8 + c.n4 <= Q          # Eq. 3: never over budget
+        assert c.n16 >= P
+        if c.n16 < n:
+            assert Q - c.spent_q4 <= 1                                  # budget used up to rounding
+        # at most two ADJACENT tiers among the non-protected tokens (Eq. 14-15 structure)
+        pops = [c.n16 - P > 0, c.n8 > 0, c.n4 > 0, c.n0 > 0]
+        idx = [i for i, p in enumerate(pops) if p]
+        assert len(idx) <= 2 and (len(idx) < 2 or idx[1] - idx[0] == 1 or (not a4 and idx == [1, 3]))
+        if not a4:
+            assert c.n4 == 0
+
+
+def test_tier_counts_config_table():
+    # (n, b, s, ranges, allow_int4) -> counts; closed form of DESIGN.md reading P5 evaluated by hand
+    # e.g. C3 b=0.3: Q=floor(4*.3*4096)=4915, P=68, m=4028, R=4915-272=4643 in [m,2m): n8=R-m=615, n4=2m-R=3413
+    table = [
+        (256, 0.5, 4, [], True, (4, 244, 8, 0)),
+        (4096, 0.3, 4, [], False, (4, 2449, 0, 1643)),
+        (4096, 0.5, 4, [], False, (4, 4088, 0, 4)),
+        (4096, 0.3, 4, [(4032, 4096)], True, (68, 615, 3413, 0)),
+        (4096, 0.5, 4, [(4032, 4096)], True, (68, 3892, 136, 0)),
+        (4096, 0.5, 4, [], True, (4, 4084, 8, 0)),
+        (32768, 0.3, 4, [], True, (4, 6541, 26223, 0)),
+        (32768, 0.4, 4, [], True, (4, 19648, 13116, 0)),
+        (32768, 0.5, 4, [], True, (4, 32756, 8, 0)),
+        (32768, 0.75, 4, [], True, (16384, 16384, 0, 0)),
+        (32768, 1.0, 4, [], True, (32768, 0, 0, 0)),
+    ]
+    for n, b, s, r, a4, want in table:
+        c, _ = oracle.tier_counts(n, b, s, r, a4)
+        assert (c.n16, c.n8, c.n4, c.n0) == want, (n, b)
+
+
+def test_overlapping_ranges_counted_once_and_b_clamped():
+    c, prot = oracle.tier_counts(100, 1.7, 4, [(2, 10), (8, 12), (50, 50)], True)
+    assert prot.sum() == 12 and c.n16 == 100 and c.budget_q4 == 400
+    with pytest.raises(ValueError):
+        oracle.tier_counts(100, 0.1, 20, [], True)          # 4P = 80 > Q = 40
+    with pytest.raises(ValueError):
+        oracle.tier_counts(100, 0.5, 0, [(10, 101)], True)  # range outside [0, n]
+
+
+# ----------------------------------------------------------------------------------------------
+# O3 selection
+# ----------------------------------------------------------------------------------------------
+def _brute_force_tiers(I, prot, counts):
+    """rank_j = #{k : I_k > I_j or (I_k == I_j and k < j)} over non-protected tokens, O(n^2)."""
+    n = len(I)
+    key = np.where(I > 0, I, np.float32(0)).astype(np.float32)
+    key[np.isnan(I)] = 0
+    tier = np.zeros(n, np.uint8)
+    P = int(prot.sum())
+    for j in range(n):
+        if prot[j]:
+            tier[j] = 16
+            continue
+        rank = 0
+        for k in range(n):
+            if prot[k] or k == j:
+                continue
+            if key[k] > key[j] or (key[k] == key[j] and k < j):
+                rank += 1
+        c16 = counts.n16 - P
+        tier[j] = 16 if rank < c16 else 8 if rank < c16 + counts.n8 else 4 if rank < c16 + counts.n8 + counts.n4 else 0
+    return tier
+
+
+@pytest.mark.parametrize("n,b,s,ranges,a4", [
+    (64, 0.4, 4, [], True), (97, 0.3, 2, [(90, 97)], True), (50, 0.3, 4, [], False),
+    (33, 0.75, 0, [(5, 9)], True), (40, 0.2, 1, [], True), (31, 1.0, 4, [], True)])
+def test_selection_matches_brute_force(n, b, s, ranges, a4):
+    rng = np.random.default_rng(n)
+    I = rng.random((2, n)).astype(np.float32)
+    I[0, 5] = I[0, 20] = I[0, 21]        # exact ties
+    I[1, 3] = np.nan; I[1, 9] = -1.0; I[1, 10] = -0.0; I[1, 11] = 0.0
+    c, prot = oracle.tier_counts(n, b, s, ranges, a4)
+    tier = oracle.assign(I, prot, c)
+    for l in range(2):
+        assert np.array_equal(tier[l], _brute_force_tiers(I[l], prot, c))
+        assert [(tier[l] == t).sum() for t in (16, 8, 4, 0)] == [c.n16, c.n8, c.n4, c.n0]
+
+
+def test_selection_monotone_and_sinks_fp16():
+    # Prop. 1: higher importance never gets a lower tier; sinks FP16 whatever their score
+    rng = np.random.default_rng(7)
+    n = 2000
+    I = (rng.random((3, n)) ** 6).astype(np.float32)
+    I[:, :4] = 0.0                                           # sinks with the lowest possible score
+    c, prot = oracle.tier_counts(n, 0.35, 4, [(1900, 1910)], True)
+    tier = oracle.assign(I, prot, c).astype(np.int32)
+    assert (tier[:, :4] == 16).all() and (tier[:, 1900:1910] == 16).all()
+    for l in range(3):
+        free = ~prot.astype(bool)
+        order = np.argsort(-I[l][free], kind="stable")
+        t = tier[l][free][order]
+        assert (np.diff(t) <= 0).all()                       # non-increasing tier along decreasing importance
+
+
+def test_selection_tie_break_lower_position_first():
+    I = np.full((1, 10), 0.5, np.float32)
+    c, prot = oracle.tier_counts(10, 0.4, 0, [], True)       # Q=16, m=10: n8=6, n4=4
+    assert (c.n8, c.n4) == (6, 4)
+    tier = oracle.assign(I, prot, c)
+    assert tier[0].tolist() == [8] * 6 + [4] * 4
+
+
+# ----------------------------------------------------------------------------------------------
+# O4 quantizer
+# ----------------------------------------------------------------------------------------------
+def test_quantizer_worked_examples():
+    rows = read_golden(os.path.join(GOLD, "quantizer_worked.txt"))
+    groups = {}
+    for name, qmax, x, code, ybits in rows:
+        groups.setdefault((name, int(qmax)), []).append((float(x), int(code), int(ybits, 16)))
+    assert len(groups) == 4
+    for (name, qmax), items in groups.items():
+        x = np.zeros(128, np.float16)
+        x[:len(items)] = [it[0] for it in items]
+        assert all(float(np.float16(it[0])) == it[0] for it in items)      # fixtures are exact fp16 values
+        ab, q = oracle.quantize_vector(x, qmax)
+        assert ab == int(np.abs(x).max().view(np.uint16)), name
+        assert q[:len(items)].tolist() == [it[1] for it in items], name
+        assert (q[len(items):] == 0).all()
+        y = oracle.dequantize_vector(q, qmax, ab)
+        assert y[:len(items)].view(np.uint16).tolist() == [it[2] for it in items], name
+
+
+def test_quantizer_special_cases():
+    z = np.zeros(64, np.float16); z[3] = -0.0
+    ab, q = oracle.quantize_vector(z, 127)
+    assert ab == 0 and (q == 0).all()
+    assert (oracle.dequantize_vector(q, 127, ab).view(np.uint16) == 0).all()     # +0.0
+    big = np.full(64, 65504.0, np.float16); big[1] = -65504.0
+    for qmax in (127, 7):
+        ab, q = oracle.quantize_vector(big, qmax)
+        assert q[0] == qmax and q[1] == -qmax
+        assert np.array_equal(oracle.dequantize_vector(q, qmax, ab), big)        # no overflow
+    sub = np.zeros(64, np.float16); sub[0] = np.float16(5.96e-8); sub[1] = -sub[0]
+    ab, q = oracle.quantize_vector(sub, 127)
+    assert ab == 1 and q[0] == 127 and q[1] == -127
+    assert np.array_equal(oracle.dequantize_vector(q, 127, ab), sub)
+
+
+@pytest.mark.parametrize("qmax", [127, 7])
+def test_quantizer_error_bound(qmax):
+    # BASELINE north_star: per-element dequantization error <= scale/2 (on the fp32 product, with the
+    # reciprocal-multiply slack derived in DESIGN.md; + half an fp16 ulp on the stored output).
+    rng = np.random.default_rng(3)
+    for scale_mag in (1e-3, 1.0, 50.0):
+        x = (rng.standard_normal((200, 128)) * scale_mag).astype(np.float16)
+        x[:, :6] *= 10
+        x = np.clip(x, -65504, 65504).astype(np.float16)
+        for v in x:
+            ab, q = oracle.quantize_vector(v, qmax)
+            amax = float(np.uint16(ab).view(np.float16))
+            assert amax == float(np.abs(v).max())
+            scale = amax / qmax
+            assert np.abs(q).max() == qmax                                     # the amax element hits +-qmax
+            err = np.abs(q.astype(np.float64) * scale - v.astype(np.float64))
+            assert err.max() <= scale / 2 * (1 + 1e-4)
+            y = oracle.dequantize_vector(q, qmax, ab).astype(np.float64)
+            ulp = np.spacing(np.abs(y).astype(np.float16)).astype(np.float64)
+            assert (np.abs(y - v.astype(np.float64)) <= scale / 2 * (1 + 1e-4) + ulp / 2 + 1e-12).all()
+            assert (np.sign(q) * np.sign(v.astype(np.float64)) >= 0).all()     # symmetric: sign preserved
+
+
+def test_quantizer_cosine_band():
+    # Table 8: INT8 cosine > 0.9999, INT4 0.96-0.99 on real KV; on N(0,1) vectors the
+    # same quantizer must land in the same regime (statistical sanity, not a bit-level pin).
+    rng = np.random.default_rng(4)
+    x = rng.standard_normal((500, 128)).astype(np.float16)
+    for qmax, lo, hi in ((127, 0.9999, 1.0), (7, 0.985, 0.998)):
+        cs = []
+        for v in x:
+            ab, q = oracle.quantize_vector(v, qmax)
+            y = oracle.dequantize_vector(q, qmax, ab).astype(np.float64)
+            v64 = v.astype(np.float64)
+            cs.append(y @ v64 / np.linalg.norm(y) / np.linalg.norm(v64))
+        assert lo < np.mean(cs) <= hi, (qmax, np.mean(cs))
+
+
+# ----------------------------------------------------------------------------------------------
+# O5 wire format
+# ----------------------------------------------------------------------------------------------
+def _u32(b, off):
+    return int.from_bytes(bytes(b[off:off + 4]), "little")
+
+
+def _u64(b, off):
+    return int.from_bytes(bytes(b[off:off + 8]), "little")
+
+
+def _w6_inputs():
+    rows = read_golden(os.path.join(GOLD, "quantizer_worked.txt"))
+    w1 = [r for r in rows if r[0] == "W1"]
+    w3 = [r for r in rows if r[0] == "W3"]
+    K = np.zeros((1, 4, 1, 64), np.float16)
+    V = np.zeros((1, 4, 1, 64), np.float16)
+    K[0, 0, 0, :] = np.arange(64) / 8.0 - 3.0                 # FP16 token: copied verbatim
+    V[0, 0, 0, :] = -np.arange(64) / 16.0
+    K[0, 1, 0, :len(w1)] = [float(r[2]) for r in w1]          # INT8 token, W1 vector
+    V[0, 1, 0, :2] = [1.0, 0.5]                               # W2: amax 1.0 -> codes 127, 64
+    K[0, 2, 0, :len(w3)] = [float(r[2]) for r in w3]          # INT4 token, W3 vector
+    V[0, 2, 0, :3] = [1.0, 0.5, -0.25]                        # W4: codes 7, 4, -2
+    K[0, 3] = 9.0; V[0, 3] = -9.0                             # dropped token: leaves no bytes
+    tier = np.array([[16, 8, 4, 0]], np.uint8)
+    return K, V, tier, w1, w3
+
+
+def test_w6_layout_and_hand_written_blob():
+    g = {r[0]: r[1:] for r in read_golden(os.path.join(GOLD, "w6_layout.txt"))}
+    K, V, tier, w1, w3 = _w6_inputs()
+    counts = oracle.Counts(1, 1, 1, 1, 7, 7)
+    blob = oracle.pack(K, V, tier, counts, allow_int4=True)
+    assert blob.size == int(g["total_bytes"][0]) == oracle.blob_bytes(1, 1, 64, 4, counts)
+    # header, field by field
+    assert bytes(blob[0:4]) == b"SKV1" and _u32(blob, 4) == 1
+    assert [_u32(blob, o) for o in (8, 12, 16, 20)] == [1, 1, 64, 4]
+    assert [_u32(blob, o) for o in (24, 28, 32, 36)] == [1, 1, 1, 1]
+    assert _u32(blob, 40) == 1 and _u32(blob, 44) == 0 and _u64(blob, 48) == 7
+    assert _u64(blob, 56) == int(g["tier_map_off"][0]) and _u64(blob, 64) == int(g["layer0_off"][0])
+    assert _u64(blob, 72) == int(g["layer_stride"][0]) and _u64(blob, 160) == int(g["total_bytes"][0])
+    seg = [int(v) for v in g["seg_off"]]
+    assert [_u64(blob, 80 + 8 * i) for i in range(10)] == seg
+    assert not blob[168:256].any()
+    # expected blob written by hand from the format text and the worked codes
+    want = np.zeros(3072, np.uint8)
+    want[:256] = blob[:256]                                    # header checked field by field above
+    want[256:260] = [16, 8, 4, 0]
+    base = 512
+    want[base + seg[0]: base + seg[0] + 128] = K[0, 0, 0].view(np.uint8)
+    want[base + seg[1]: base + seg[1] + 128] = V[0, 0, 0].view(np.uint8)
+    k8 = np.zeros(64, np.int8); k8[:len(w1)] = [int(r[3]) for r in w1]
+    v8 = np.zeros(64, np.int8); v8[:2] = [127, 64]
+    want[base + seg[2]: base + seg[2] + 64] = k8.view(np.uint8)
+    want[base + seg[3]: base + seg[3] + 64] = v8.view(np.uint8)
+    k4 = [int(r[3]) for r in w3] + [0] * (64 - len(w3))
+    v4 = [7, 4, -2] + [0] * 61
+    for s, codes in ((4, k4), (5, v4)):
+        want[base + seg[s]: base + seg[s] + 32] = [(codes[2 * i] & 0xF) | ((codes[2 * i + 1] & 0xF) << 4) for i in range(32)]
+    for s, amax in ((6, 1.984375), (7, 1.0), (8, 1.75), (9, 1.0)):
+        want[base + seg[s]: base + seg[s] + 2] = np.array([amax], np.float16).view(np.uint8)
+    assert np.array_equal(blob, want)
+    # W5 nibble packing
+    vec = np.zeros(64, np.float16); vec[:6] = [1.75, -1.0, 0.0, -0.25, 0.5, -1.75]   # codes 7,-4,0,-1,2,-7
+    ab, q = oracle.quantize_vector(vec, 7)
+    assert q[:6].tolist() == [7, -4, 0, -1, 2, -7]
+    K2 = np.zeros((1, 1, 1, 64), np.float16); K2[0, 0, 0] = vec
+    b2 = oracle.pack(K2, K2, np.array([[4]], np.uint8), oracle.Counts(0, 0, 1, 0, 1, 1))
+    off = _u64(b2, 64) + _u64(b2, 80 + 8 * 4)
+    assert bytes(b2[off:off + 3]).hex().upper() == "".join(g["nibbles"])
+    # decode side: unpack reproduces FP16 row, dequantised rows, zeros for the dropped token
+    K3, V3, t3 = oracle.unpack(blob, 1, 1, 64, 4)
+    assert np.array_equal(t3, tier)
+    assert np.array_equal(K3[0, 0], K[0, 0]) and np.array_equal(V3[0, 0], V[0, 0])
+    assert K3[0, 1, 0, :len(w1)].view(np.uint16).tolist() == [int(r[4], 16) for r in w1]
+    assert K3[0, 2, 0, :len(w3)].view(np.uint16).tolist() == [int(r[4], 16) for r in w3]
+    assert not K3[0, 3].view(np.uint16).any() and not V3[0, 3].view(np.uint16).any()
+
+
+def test_blob_bytes_closed_form_and_eq1_identity():
+    # payload bytes (segments without pads/scales/map/header) == Bytes_FP16 * spent / (4 n)   (Eq. 1-3)
+    for (L, Hkv, d, n, b, s, a4) in [(3, 4, 128, 1000, 0.3, 4, True), (2, 8, 256, 257, 0.5, 4, True),
+                                     (5, 4, 128, 4096, 0.3, 4, False), (1, 2, 64, 250, 0.8, 0, True)]:
+        c, prot = oracle.tier_counts(n, b, s, [], a4)
+        bytes_fp16 = 2 * L * Hkv * d * n * 2
+        payload = L * 2 * Hkv * d * (2 * c.n16 + c.n8 + c.n4 // 2) if c.n4 % 2 == 0 else None
+        if payload is not None:
+            assert payload * 4 * n == bytes_fp16 * c.spent_q4
+        pad = lambda x: (x + 255) // 256 * 256
+        segs = [c.n16 * Hkv * d * 2] * 2 + [c.n8 * Hkv * d] * 2 + [c.n4 * Hkv * d // 2] * 2 + \
+               [c.n8 * Hkv * 2] * 2 + [c.n4 * Hkv * 2] * 2
+        total = 256 + pad(L * n) + L * sum(pad(x) for x in segs)
+        assert oracle.blob_bytes(L, Hkv, d, n, c) == total
+
+
+# ----------------------------------------------------------------------------------------------
+# O5/O6 pack + unpack
+# ----------------------------------------------------------------------------------------------
+def _rand_kv(L, n, Hkv, d, seed):
+    rng = np.random.default_rng(seed)
+    K = rng.standard_normal((L, n, Hkv, d)).astype(np.float16)
+    K[..., :3] *= 10
+    V = rng.standard_normal((L, n, Hkv, d)).astype(np.float16)
+    return K, V
+
+
+def test_b1_identity_round_trip():
+    L, n, Hkv, d = 2, 77, 2, 64
+    K, V = _rand_kv(L, n, Hkv, d, 5)
+    c, prot = oracle.tier_counts(n, 1.0, 4, [], True)
+    I = np.random.default_rng(0).random((L, n)).astype(np.float32)
+    tier = oracle.assign(I, prot, c)
+    assert (tier == 16).all()
+    blob = oracle.pack(K, V, tier, c)
+    K2, V2, t2 = oracle.unpack(blob, L, Hkv, d, n)
+    assert np.array_equal(K2.view(np.uint16), K.view(np.uint16)) and np.array_equal(V2.view(np.uint16), V.view(np.uint16))
+    # Eq. 1: payload of an all-FP16 blob is exactly Bytes_FP16
+    assert blob.size >= 2 * L * Hkv * d * n * 2
+
+
+def test_round_trip_matches_vector_quantizer_and_positions():
+    L, n, Hkv, d = 2, 130, 2, 128
+    K, V = _rand_kv(L, n, Hkv, d, 6)
+    c, prot = oracle.tier_counts(n, 0.22, 3, [(100, 104)], True)     # exercises 16 / 4 / drop
+    c2, _ = oracle.tier_counts(n, 0.45, 3, [(100, 104)], True)       # exercises 16 / 8 / 4
+    I = np.random.default_rng(1).random((L, n)).astype(np.float32)
+    for cc in (c, c2):
+        tier = oracle.assign(I, prot, cc)
+        blob = oracle.pack(K, V, tier, cc)
+        K2, V2, t2 = oracle.unpack(blob, L, Hkv, d, n)
+        assert np.array_equal(t2, tier)
+        for X, X2 in ((K, K2), (V, V2)):
+            for l in range(L):
+                for j in range(n):
+                    t = tier[l, j]
+                    if t == 16:
+                        assert np.array_equal(X2[l, j].view(np.uint16), X[l, j].view(np.uint16))
+                    elif t == 0:
+                        assert not X2[l, j].view(np.uint16).any()
+                    else:
+                        qmax = 127 if t == 8 else 7
+                        for h in range(Hkv):
+                            ab, q = oracle.quantize_vector(X[l, j, h], qmax)
+                            assert np.array_equal(X2[l, j, h].view(np.uint16),
+                                                  oracle.dequantize_vector(q, qmax, ab).view(np.uint16))
+
+
+def test_pack_rejects_mismatched_counts_and_unpack_rejects_bad_header():
+    L, n, Hkv, d = 1, 16, 1, 64
+    K, V = _rand_kv(L, n, Hkv, d, 8)
+    c, prot = oracle.tier_counts(n, 0.5, 0, [], True)
+    tier = np.full((L, n), 8, np.uint8)
+    blob = oracle.pack(K, V, tier, c)
+    bad_tier = tier.copy(); bad_tier[0, 0] = 4
+    with pytest.raises(ValueError):
+        oracle.pack(K, V, bad_tier, c)
+    for off in (0, 4, 8, 20, 24, 64, 160):
+        b = blob.copy(); b[off] ^= 1
+        with pytest.raises(ValueError):
+            oracle.unpack(b, L, Hkv, d, n)
+
+
+def test_value_error_bound_eq5_and_logit_bound_eq10():
+    # Eq. 5: ||y - y~|| <= sum_j p_j ||e_j||;  Eq. 10: e^{-2 eta} p <= p~ <= e^{2 eta} p.
+    # Sanity that unpacked rows land at the right positions with the right magnitudes.
+    L, n, Hkv, d = 1, 300, 1, 128
+    K, V = _rand_kv(L, n, Hkv, d, 9)
+    c, prot = oracle.tier_counts(n, 0.3, 4, [], True)
+    I = np.random.default_rng(2).random((L, n)).astype(np.float32)
+    tier = oracle.assign(I, prot, c)
+    K2, V2, _ = oracle.unpack(oracle.pack(K, V, tier, c), L, Hkv, d, n)
+    q = np.random.default_rng(3).standard_normal(d)
+    k, k2 = K[0, :, 0].astype(np.float64), K2[0, :, 0].astype(np.float64)
+    v, v2 = V[0, :, 0].astype(np.float64), V2[0, :, 0].astype(np.float64)
+    z, z2 = k @ q / np.sqrt(d), k2 @ q / np.sqrt(d)
+    p = np.exp(z - z.max()); p /= p.sum()
+    p2 = np.exp(z2 - z2.max()); p2 /= p2.sum()
+    eta = np.abs(z2 - z).max()
+    assert (p2 <= np.exp(2 * eta) * p * (1 + 1e-9)).all() and (p2 >= np.exp(-2 * eta) * p * (1 - 1e-9)).all()
+    e = np.linalg.norm(v - v2, axis=1)
+    assert np.linalg.norm(p @ v - p @ v2) <= (p * e).sum() * (1 + 1e-9)
+    assert (e[tier[0] == 16] == 0).all() and e[tier[0] == 4].mean() > e[tier[0] == 8].mean() > 0
+
+
+def test_drop_tail_mass_lemma1():
+    # Lemma 1: dropping a set of mass eps with renormalisation moves y by <= 2 eps V.
+    L, n, Hkv, d = 1, 200, 1, 64
+    K, V = _rand_kv(L, n, Hkv, d, 10)
+    c, prot = oracle.tier_counts(n, 0.3, 4, [], False)          # 2-tier: INT8 + drop
+    assert c.n0 > 0
+    rng = np.random.default_rng(4)
+    p = rng.random(n) ** 8; p /= p.sum()
+    I = p[None].astype(np.float32)
+    tier = oracle.assign(I, prot, c)
+    keep = tier[0] != 0
+    eps = p[~keep].sum()
+    v = V[0, :, 0].astype(np.float64)
+    y = p @ v
+    yhat = (p[keep] / (1 - eps)) @ v[keep]
+    Vmax = np.linalg.norm(v, axis=1).max()
+    assert np.linalg.norm(y - yhat) <= 2 * eps * Vmax
+    # the dropped set is the lowest-importance one: its mass is below the mass of any equal-size kept set
+    assert eps <= np.sort(p[~prot.astype(bool)])[: c.n0].sum() * (1 + 1e-6)
+
+
+# ----------------------------------------------------------------------------------------------
+# O1 importance
+# ----------------------------------------------------------------------------------------------
+def _rand_qk(L, Hq, Hkv, d, n, w, seed):
+    rng = np.random.default_rng(seed)
+    K = rng.standard_normal((L, n, Hkv, d)).astype(np.float16)
+    Q = rng.standard_normal((L, Hq, w, d)).astype(np.float16)
+    return K, Q
+
+
+@pytest.mark.parametrize("causal", [True, False])
+def test_importance_sums_to_one(causal):
+    K, Q = _rand_qk(2, 4, 2, 64, 90, 7, 11)
+    I = oracle.importance(K, Q, causal=causal, lam=0.0)
+    assert I.shape == (2, 90) and (I >= 0).all()
+    assert np.allclose(I.astype(np.float64).sum(axis=1), 1.0, atol=1e-6)
+
+
+def test_importance_zero_keys_closed_forms():
+    L, Hq, Hkv, d, n, w = 1, 2, 1, 64, 40, 8
+    K = np.zeros((L, n, Hkv, d), np.float16)
+    Q = np.random.default_rng(0).standard_normal((L, Hq, w, d)).astype(np.float16)
+    I = oracle.importance(K, Q, causal=False)
+    assert np.allclose(I, 1.0 / n, rtol=1e-6)
+    I = oracle.importance(K, Q, causal=True)
+    pos = np.arange(n - w, n)
+    want = np.array([(1.0 / (pos[pos >= j] + 1)).sum() / w for j in range(n)])
+    assert np.allclose(I[0], want, rtol=1e-6)
+
+
+def test_importance_dominant_key_and_gqa_mapping():
+    # KV head g serves query heads [g*G, (g+1)*G) (integer division, HF repeat_kv convention).
+    L, Hq, Hkv, d, n, w = 1, 4, 2, 64, 50, 4
+    K = np.zeros((L, n, Hkv, d), np.float16)
+    Q = np.zeros((L, Hq, w, d), np.float16)
+    Q[..., 0] = 8.0
+    K[0, 10, 0, 0] = 30.0           # KV head 0: key 10 dominates  (logit 8*30/8 = 30)
+    K[0, 20, 1, 0] = 30.0           # KV head 1: key 20 dominates
+    I = oracle.importance(K, Q, causal=True)
+    assert abs(I[0, 10] - 0.5) < 1e-6 and abs(I[0, 20] - 0.5) < 1e-6
+    Q[0, 2:, :, 0] = 0.0            # query heads 2,3 (-> KV head 1) become uniform
+    I = oracle.importance(K, Q, causal=False)
+    assert abs(I[0, 10] - (0.5 + 0.5 / n)) < 1e-4 and abs(I[0, 20] - 0.5 / n) < 1e-4
+
+
+def test_importance_decay_closed_form():
+    K, Q = _rand_qk(1, 2, 1, 64, 120, 5, 12)
+    I0 = oracle.importance(K, Q, lam=0.0).astype(np.float64)
+    for lam in (0.001, 0.005, 0.010):                       # the values the paper prints (Table 15)
+        I = oracle.importance(K, Q, lam=lam).astype(np.float64)
+        ratio = I[0] / I0[0]
+        want = np.exp(-lam * (120 - 1 - np.arange(120)))    # newest token: Delta = 0
+        assert np.allclose(ratio, want, rtol=1e-5)
+    assert abs(ratio[-1] - 1.0) < 1e-6
+
+
+@pytest.mark.parametrize("causal", [True, False])
+def test_importance_matches_textbook_softmax(causal):
+    L, Hq, Hkv, d, n, w = 2, 6, 2, 128, 150, 9
+    K, Q = _rand_qk(L, Hq, Hkv, d, n, w, 13)
+    I = oracle.importance(K, Q, causal=causal)
+    Kt = torch.from_numpy(K).double().permute(0, 2, 1, 3)              # [L][Hkv][n][d]
+    Kt = Kt.repeat_interleave(Hq // Hkv, dim=1)                        # repeat_kv
+    Qt = torch.from_numpy(Q).double()                                  # [L][Hq][w][d]
+    z = torch.matmul(Qt, Kt.transpose(-1, -2)) / d ** 0.5              # [L][Hq][w][n]
+    if causal:
+        pos = torch.arange(n - w, n)[:, None]
+        z = z.masked_fill(torch.arange(n)[None, :] > pos, float("-inf"))
+    A = torch.softmax(z, dim=-1).mean(dim=(1, 2))
+    assert np.allclose(I, A.numpy(), rtol=1e-6, atol=1e-12)
+
+
+def test_kvnorm_fallback_shape_and_normalisation():
+    K, _ = _rand_qk(2, 2, 2, 64, 33, 3, 14)
+    I = oracle.importance_kvnorm(K)
+    assert np.allclose(I.astype(np.float64).sum(axis=1), 1.0, atol=1e-6)
+    nrm = np.linalg.norm(K.astype(np.float64), axis=-1).mean(axis=-1)
+    assert np.allclose(I, nrm / nrm.sum(axis=1, keepdims=True), rtol=1e-6)
