@@ -1,0 +1,158 @@
+/*
+ * skv.h -- C ABI of the B200-native SpectrumKV per-token mixed-precision KV transfer path
+ * (arxiv/paper_2606_08635; citations are /root/reference/PAPER.md:<line>).
+ *
+ * The library implements Algorithm 1 steps 2-4 and the decode-side
+ * dequantisation as hand-written CUDA for sm_100a:
+ *
+ *   skv_importance    Alg. 1 step 2, Eq. 13: I_j = A_j exp(-lambda Delta_j), A_j = softmax
+ *                     mass of the last-w prompt queries on key j (logits q.k/sqrt(d)),
+ *                     averaged over query heads and window queries
+ *   skv_importance_kvnorm   the "KV-norm fallback" of Alg. 1 step 2
+ *   skv_tier_counts   Eq. 2-3, Eq. 14-15, SinkProtect,
+ *                     2-tier fallback with drop: budget b -> (n16, n8, n4, n0)
+ *   skv_assign_tiers  Alg. 1 step 3, Prop. 1: pin protected positions to
+ *                     FP16, rank the rest by (importance desc, position asc)
+ *   skv_pack          Alg. 1 step 4: quantise K and V independently per the tier map
+ *                     ("standard symmetric") and compact into one SKV1 blob
+ *   skv_unpack        PAPER.md:202: dequantise and scatter back into a dense FP16 cache
+ *   skv_blob_check    decode-side validation of a received blob header (host)
+ *
+ * Conventions
+ *   - Every pointer is tagged HOST or DEVICE.  DEVICE pointers are plain CUDA device addresses
+ *     (e.g. torch.Tensor.data_ptr()); the library never allocates, frees or keeps them.
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  All work is
+ *     enqueued on that stream; no entry point synchronises the host.
+ *   - Every entry returns SKV_OK (0) or a negative skv_status and launches nothing on error.
+ *   - The library keeps no global state and is re-entrant.
+ *   - fp16 = IEEE binary16.  K/V inputs must be finite (NaN/Inf is undefined behaviour).
+ *
+ * Tier codes (bits per element): 16 = FP16, 8 = INT8, 4 = INT4, 0 = dropped (c = 0).
+ *
+ * Wire format "SKV1" (little endian; one self-contained blob per request; a batch is R blobs back to
+ * back at stride skv_blob_bytes(); the paper only says "mixed-precision payload"):
+ *
+ *   [0,256)  header: 0 u32 magic 0x31564B53 ("SKV1"), 4 u32 version = 1, 8 u32 L, 12 u32 Hkv, 16 u32 d_h,
+ *            20 u32 n, 24 u32 n16, 28 u32 n8, 32 u32 n4, 36 u32 n0, 40 u32 flags (bit0 = allow_int4),
+ *            44 u32 0, 48 u64 budget in quarter-units, 56 u64 tier_map_off (= 256), 64 u64 layer0_off,
+ *            72 u64 layer_stride, 80 u64 seg_off[10] (relative to the layer block), 160 u64 total_bytes,
+ *            168..255 zero
+ *   [256,..) tier map u8[L][n], zero padded to a multiple of 256 B
+ *   layer l at layer0_off + l*layer_stride: ten segments, each starting on a 256-B boundary, pads zero:
+ *            K16,V16 : f16 [n16][Hkv][d_h]     K8,V8 : i8 [n8][Hkv][d_h]     K4,V4 : u8 [n4][Hkv][d_h/2]
+ *            SK8,SV8 : f16 amax [n8][Hkv]      SK4,SV4 : f16 amax [n4][Hkv]
+ *   Slot order inside a tier = ascending token position.  INT4 byte i holds element 2i in the low nibble
+ *   and 2i+1 in the high nibble (4-bit two's complement).  Dropped tokens occupy no bytes.
+ *
+ * Quantiser (one group = one head vector of d_h values; qmax = 127 / 7):
+ *   amax = max|x| (an fp16 value, stored as the 2-byte scale record);
+ *   inv = fl32(qmax/amax), scale = fl32(amax/qmax)   (both 0 when amax = 0);
+ *   q = clamp(rint(fl32(x*inv)), -qmax, qmax), rint = round half to even;   y = f16_rn(fl32(q*scale)).
+ */
+#ifndef SKV_H_
+#define SKV_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    SKV_OK = 0,
+    SKV_ERR_INVALID_ARG = -1,       /* null pointer, dims <= 0, Hq % Hkv != 0, window outside [1,n], b <= 0 or NaN,
+                                       range outside [0,n] or begin > end */
+    SKV_ERR_UNSUPPORTED = -2,       /* head_dim not in {64,128,256}; stride_token/stride_head/stride_layer/
+                                       stride_request not multiples of 8 elements; pointer not 16-B aligned;
+                                       n_tokens > 2^24 */
+    SKV_ERR_BUDGET_INFEASIBLE = -3, /* protected tokens alone exceed the budget (4P > floor(4bn)) */
+    SKV_ERR_BUFFER_TOO_SMALL = -4,  /* blob capacity or workspace */
+    SKV_ERR_BAD_BLOB = -5,          /* skv_blob_check: magic / version / dims / offsets / total_bytes mismatch */
+    SKV_ERR_CUDA = -6               /* a CUDA runtime call or kernel launch failed */
+} skv_status;
+
+/* One batch of dense caches.  Strides are in ELEMENTS (fp16) and apply to both K and V; the head
+ * dimension is contiguous.  Token-major default: stride_head = d_h, stride_token = Hkv*d_h,
+ * stride_layer = n*Hkv*d_h, stride_request = L*n*Hkv*d_h.  The HF layout [L][Hkv][n][d_h] is
+ * stride_token = d_h, stride_head = n*d_h.  All requests of a batch have the same n_tokens. */
+typedef struct {
+    int32_t n_layers, n_q_heads, n_kv_heads, head_dim, n_tokens, n_requests;
+    int64_t stride_request, stride_layer, stride_token, stride_head;
+} skv_shape;
+
+/* Transfer policy (PAPER.md:51-58 b; :216, :230 sinks; :25 protected positions; :234 allow_int4). */
+typedef struct {
+    double  budget;           /* b in (0,1]; values > 1 are clamped to 1 */
+    int32_t n_sink;           /* s: positions [0,s) forced FP16 */
+    int32_t n_ranges;         /* number of protected ranges */
+    const int32_t *ranges;    /* HOST, n_ranges x [begin,end) half-open, forced FP16; read during the call only */
+    int32_t allow_int4;       /* probe result: 1 = 3-tier, 0 = 2-tier FP16+INT8(+drop) */
+} skv_policy;
+
+/* Tier populations of ONE layer of ONE request (identical for every layer and request of a batch,
+ * because n, b and the protected set are).  budget_q4 = floor(4bn + 1e-6), spent_q4 = 4n16+2n8+n4. */
+typedef struct {
+    int32_t n16, n8, n4, n0;
+    int32_t allow_int4, reserved;
+    int64_t budget_q4, spent_q4;
+} skv_counts;
+
+/* HOST only.  Closed form of Eq. 14-15 with sink/range pinning paid out of the budget. */
+int skv_tier_counts(const skv_shape *shape, const skv_policy *policy, skv_counts *counts_out);
+
+/* HOST only.  Bytes of ONE request's SKV1 blob (a multiple of 256); 0 on invalid arguments. */
+size_t skv_blob_bytes(const skv_shape *shape, const skv_counts *counts);
+
+/* HOST only.  Workspace (DEVICE bytes) sufficient for any entry point on this shape with the given
+ * observation window (pass window = 0 if skv_importance is not used). */
+size_t skv_workspace_bytes(const skv_shape *shape, int32_t window);
+
+/* HOST only.  Validates the first 256 bytes of a received blob (HOST memory) against blob_bytes and
+ * returns the dims (strides zero) and counts it declares.  SKV_ERR_BAD_BLOB on any mismatch. */
+int skv_blob_check(const void *header_host, size_t blob_bytes, skv_shape *shape_out, skv_counts *counts_out);
+
+/* DEVICE.  K_dev: fp16, addressed by `shape` strides.  Q_dev: fp16 [R][L][Hq][window][d_h] contiguous,
+ * window query i of a request sits at position n - window + i.  causal != 0 excludes keys beyond the
+ * query position.  importance_dev: f32 [R][L][n].  Accumulation in fp32 (tensor cores, fp16 inputs);
+ * agreement with the float64 definition is ~1e-5 relative (contract: 1e-3). */
+int skv_importance(const skv_shape *shape, const void *K_dev, const void *Q_dev, int32_t window,
+                   int32_t causal, float lambda, float *importance_dev,
+                   void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
+
+/* DEVICE.  KV-norm fallback score: A_j = mean over KV heads of ||k_j||_2, normalised to sum 1 per layer,
+ * times the same decay.  importance_dev: f32 [R][L][n]. */
+int skv_importance_kvnorm(const skv_shape *shape, const void *K_dev, float lambda, float *importance_dev,
+                          void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
+
+/* DEVICE.  importance_dev f32 [R][L][n] -> tier_map_dev u8 [R][L][n].  NaN / negative / -0 scores rank as
+ * +0; equal scores are ranked by ascending position.  counts_out_host (HOST, nullable) receives the
+ * closed-form counts; no device->host transfer takes place. */
+int skv_assign_tiers(const skv_shape *shape, const skv_policy *policy, const float *importance_dev,
+                     uint8_t *tier_map_dev, skv_counts *counts_out_host,
+                     void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
+
+/* DEVICE.  Writes n_requests blobs at blob_dev + r*skv_blob_bytes(); every byte of each blob is written
+ * (pads zero) so blobs are memcmp-comparable.  blob_dev must be 256-B aligned.  `counts` must match the
+ * tier map of every layer (maps produced by skv_assign_tiers always do); on a mismatch slots are clamped
+ * to the segment capacity (memory safe) and the blob is meaningless. */
+int skv_pack(const skv_shape *shape, const void *K_dev, const void *V_dev, const uint8_t *tier_map_dev,
+             const skv_counts *counts, void *blob_dev, size_t blob_capacity,
+             void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
+
+/* DEVICE.  blob_dev holds n_requests blobs of blob_bytes each (as validated by skv_blob_check on the
+ * host copy).  `shape` gives dims and OUTPUT strides.  Writes every element of K_out/V_out (dropped
+ * tokens -> +0.0) and, if tier_map_out_dev != NULL, the tier map u8 [R][L][n] (the validity mask). */
+int skv_unpack(const skv_shape *shape, const void *blob_dev, size_t blob_bytes, const skv_counts *counts,
+               void *K_out_dev, void *V_out_dev, uint8_t *tier_map_out_dev,
+               void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
+
+const char *skv_strerror(int status);
+
+/* Library build tag, e.g. "skv 0.1 sm_100a". */
+const char *skv_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SKV_H_ */

@@ -1,0 +1,176 @@
+// skv_assign.cu -- budgeted tier assignment (Alg. 1 step 3; Prop. 1, PAPER.md:101;
+// "Sink positions are pinned before ranking").
+//
+// One CTA per (layer, request).  The layer's n scores are turned into 32-bit ranking keys held in shared
+// memory (global workspace when n*4 exceeds the shared-memory budget): protected positions get the
+// sentinel 0xFFFFFFFF (they outrank everything, so the top-n16 set contains them), every other token the
+// bits of its non-negative f32 score (NaN / negative / -0 -> 0), which order like the floats.
+// Three order statistics (ranks n16, n16+n8, n16+n8+n4) are found by an MSB-first 8-bit radix select;
+// ties at a threshold are admitted in ascending position (a block scan of the "== threshold" flags),
+// which makes the result the unique stable ranking the oracle's sort produces.
+#include "skv_common.cuh"
+
+namespace skv {
+
+constexpr int kAssignThreads = 1024;
+
+struct Thresh { uint32_t key; uint32_t n_gt; uint32_t pass_all; uint32_t rank; };
+
+__device__ __forceinline__ uint32_t sanitize_key(float x)
+{
+    return (x > 0.0f) ? __float_as_uint(x) : 0u;        // NaN compares false -> 0; -0, negatives -> 0
+}
+
+// K-th largest (1-based, 1 <= kth <= n) of keys[0..n): returns the key and the number of strictly greater keys.
+__device__ void radix_select(const uint32_t *keys, int n, uint32_t kth, uint32_t *hist /*256*/, uint32_t *bcast /*2*/,
+                             uint32_t &key_out, uint32_t &ngt_out)
+{
+    const uint32_t tid = threadIdx.x, lane = tid & 31;
+    uint32_t prefix = 0, mask = 0, remaining = kth;
+    for (int shift = 24; shift >= 0; shift -= 8) {
+        if (tid < 256) hist[tid] = 0;
+        __syncthreads();
+        for (int j0 = 0; j0 < n; j0 += blockDim.x) {
+            const int j = j0 + tid;
+            const bool in = j < n && ((keys[j] & mask) == prefix);
+            const uint32_t digit = in ? (keys[j] >> shift) & 0xFFu : 0x100u;
+            // warp-aggregated histogram update: one atomic per distinct digit per warp
+            const uint32_t peers = __match_any_sync(0xffffffffu, digit);
+            if (in && lane == (uint32_t)(__ffs(peers) - 1)) atomicAdd(&hist[digit], __popc(peers));
+        }
+        __syncthreads();
+        if (tid < 32) {
+            // lane i owns bins [8i, 8i+8); suffix sums from the top digit down
+            uint32_t loc[8], sum = 0;
+#pragma unroll
+            for (int b = 0; b < 8; ++b) { loc[b] = hist[lane * 8 + b]; sum += loc[b]; }
+            uint32_t incl = sum;                          // inclusive suffix sum over lanes >= this lane
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t y = __shfl_down_sync(0xffffffffu, incl, o);
+                if (lane + o < 32) incl += y;
+            }
+            const uint32_t above = incl - sum;            // keys in bins owned by higher lanes
+            const bool mine = above < remaining && remaining <= incl;
+            if (mine) {
+                uint32_t acc = above;
+                int b = 7;
+                for (; b >= 0; --b) { if (acc + loc[b] >= remaining) break; acc += loc[b]; }
+                bcast[0] = lane * 8 + b;                  // the digit of the K-th largest
+                bcast[1] = remaining - acc;               // its rank inside that bin
+            }
+        }
+        __syncthreads();
+        prefix |= bcast[0] << shift;
+        mask |= 0xFFu << shift;
+        remaining = bcast[1];
+        __syncthreads();
+    }
+    key_out = prefix;
+    ngt_out = kth - remaining;
+}
+
+__global__ void __launch_bounds__(kAssignThreads)
+assign_kernel(Geom g, Intervals prot, const float *__restrict__ importance, uint8_t *__restrict__ tier_map,
+              uint32_t *__restrict__ key_ws, int keys_in_smem)
+{
+    extern __shared__ uint32_t smem[];
+    __shared__ uint32_t hist[256];
+    __shared__ uint32_t bcast[2];
+    __shared__ uint32_t warp_tot[3][32];
+    __shared__ Thresh th[3];
+
+    const int l = blockIdx.x, r = blockIdx.y, n = g.n;
+    const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int64_t off = ((int64_t)r * g.L + l) * n;
+    uint32_t *keys = keys_in_smem ? smem : key_ws + off;
+
+    for (int j = tid; j < n; j += blockDim.x) {
+        bool p = false;
+        for (int q = 0; q < prot.count; ++q) p |= (j >= prot.lo[q] && j < prot.hi[q]);
+        keys[j] = p ? 0xFFFFFFFFu : sanitize_key(importance[off + j]);
+    }
+    __syncthreads();
+
+    const uint32_t K[3] = {(uint32_t)g.n16, (uint32_t)(g.n16 + g.n8), (uint32_t)(g.n16 + g.n8 + g.n4)};
+    for (int k = 0; k < 3; ++k) {
+        uint32_t key = 0xFFFFFFFFu, ngt = 0, all = 0;
+        if (K[k] >= (uint32_t)n) all = 1;                 // every token passes this level
+        else if (K[k] > 0) radix_select(keys, n, K[k], hist, bcast, key, ngt);
+        else { key = 0xFFFFFFFFu; ngt = 0; }              // K = 0: nobody passes (rank test below fails)
+        if (tid == 0) { th[k].key = key; th[k].n_gt = ngt; th[k].pass_all = all; th[k].rank = K[k]; }
+        __syncthreads();
+    }
+
+    // position-ordered rank among equals: thread t owns the contiguous chunk [t*c, (t+1)*c)
+    const int c = (n + blockDim.x - 1) / blockDim.x;
+    const int beg = min(n, (int)tid * c), end = min(n, beg + c);
+    uint32_t eq[3] = {0, 0, 0};
+    for (int j = beg; j < end; ++j) {
+        const uint32_t key = keys[j];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) eq[k] += (key == th[k].key);
+    }
+    uint32_t excl[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        uint32_t x = eq[k];
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
+            if (lane >= (uint32_t)o) x += y;
+        }
+        if (lane == 31) warp_tot[k][warp] = x;
+        excl[k] = x - eq[k];
+    }
+    __syncthreads();
+    if (warp < 3) {
+        const uint32_t w = warp_tot[warp][lane];
+        uint32_t s = w;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t y = __shfl_up_sync(0xffffffffu, s, o);
+            if (lane >= (uint32_t)o) s += y;
+        }
+        warp_tot[warp][lane] = s - w;
+    }
+    __syncthreads();
+    uint32_t run[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) run[k] = excl[k] + warp_tot[k][warp];
+
+    uint8_t *out = tier_map + off;
+    for (int j = beg; j < end; ++j) {
+        const uint32_t key = keys[j];
+        uint32_t tier = 0;
+        bool done = false;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            bool pass;
+            if (th[k].pass_all) pass = true;
+            else if (key > th[k].key) pass = true;                       // rank < n_gt < K
+            else if (key == th[k].key) pass = (th[k].n_gt + run[k]) < th[k].rank;
+            else pass = false;
+            if (key == th[k].key) run[k] += 1;
+            if (pass && !done) { tier = (k == 0) ? 16u : (k == 1) ? 8u : 4u; done = true; }
+        }
+        out[j] = (uint8_t)tier;
+    }
+}
+
+cudaError_t launch_assign(const Geom &g, const Intervals &prot, const float *importance, uint8_t *tier_map,
+                          uint32_t *key_ws, cudaStream_t s)
+{
+    const size_t need = (size_t)g.n * 4;
+    const int in_smem = need <= 200 * 1024;
+    const size_t dyn = in_smem ? need : 0;
+    if (dyn > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(assign_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
+        if (e != cudaSuccess) return e;
+    }
+    dim3 grid(g.L, g.R);
+    assign_kernel<<<grid, kAssignThreads, dyn, s>>>(g, prot, importance, tier_map, key_ws, in_smem);
+    return cudaGetLastError();
+}
+
+}  // namespace skv

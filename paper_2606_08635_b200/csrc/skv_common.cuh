@@ -1,0 +1,58 @@
+// skv_common.cuh -- internal declarations shared by the CUDA translation units of libskv.
+// (Product code; shares nothing with oracle/.)
+#pragma once
+#include <cuda_fp16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/skv.h"
+
+namespace skv {
+
+// SKV1 layout of one request's blob (include/skv.h, "Wire format").  Segment order:
+// K16 V16 K8 V8 K4 V4 SK8 SV8 SK4 SV4.
+struct Layout {
+    uint64_t tier_map_off, layer0_off, layer_stride, total_bytes;
+    uint64_t seg_off[10];
+    uint64_t seg_raw[10];
+};
+
+// Dense-cache geometry handed to kernels by value.
+struct Geom {
+    int32_t L, Hq, Hkv, D, n, R;
+    int64_t sr, sl, st, sh;      // strides in elements
+    int32_t n16, n8, n4, n0;
+    int32_t row_chunks;          // ceil(Hkv*D / 256): 16-byte-per-lane warp chunks in one token row
+    int32_t tiles;               // ceil(n / kTileTokens)
+};
+
+constexpr int kTileTokens = 32;  // tokens per pack/unpack tile (one ballot word)
+
+struct Header256 { uint32_t w[64]; };   // the 256-byte SKV1 header image, built on the host
+
+static inline __host__ __device__ uint64_t pad256(uint64_t x) { return (x + 255ull) & ~255ull; }
+
+// host helpers (skv_host.cu)
+Layout make_layout(int L, int Hkv, int D, int64_t n, int64_t n16, int64_t n8, int64_t n4);
+
+// launchers (one per .cu)
+cudaError_t launch_tile_scan_pack(const Geom &g, const Layout &lo, const uint8_t *tier_map, uint8_t *blob,
+                                  uint64_t blob_stride, const Header256 &hdr, uint4 *tile_base, cudaStream_t s);
+cudaError_t launch_pack(const Geom &g, const Layout &lo, const __half *K, const __half *V, const uint8_t *tier_map,
+                        uint8_t *blob, uint64_t blob_stride, const uint4 *tile_base, cudaStream_t s);
+cudaError_t launch_tile_scan_unpack(const Geom &g, const Layout &lo, const uint8_t *blob, uint64_t blob_stride,
+                                    uint8_t *tier_map_out, uint4 *tile_base, cudaStream_t s);
+cudaError_t launch_unpack(const Geom &g, const Layout &lo, const uint8_t *blob, uint64_t blob_stride,
+                          __half *K, __half *V, const uint4 *tile_base, cudaStream_t s);
+
+struct Intervals { int32_t count; int32_t lo[32]; int32_t hi[32]; };   // merged protected ranges (incl. sinks)
+cudaError_t launch_assign(const Geom &g, const Intervals &prot, const float *importance, uint8_t *tier_map,
+                          uint32_t *key_ws, cudaStream_t s);
+
+cudaError_t launch_importance(const Geom &g, const __half *K, const __half *Q, int window, int causal, float lambda,
+                              float *importance, void *ws, size_t ws_bytes, cudaStream_t s);
+size_t importance_ws_bytes(const Geom &g, int window);
+cudaError_t launch_importance_kvnorm(const Geom &g, const __half *K, float lambda, float *importance, float *ws,
+                                     cudaStream_t s);
+
+}  // namespace skv

@@ -1,0 +1,320 @@
+// skv_host.cu -- the C ABI of libskv (include/skv.h): argument validation, the closed-form tier counts
+// (Eq. 14-15; SinkProtect PAPER.md:230; 2-tier drop PAPER.md:543), the SKV1 layout
+// arithmetic, and kernel launches on the caller's stream.  No allocation, no global state, no host sync.
+#include <math.h>
+#include <string.h>
+
+#include <algorithm>
+#include <vector>
+
+#include "skv_common.cuh"
+
+namespace skv {
+
+Layout make_layout(int L, int Hkv, int D, int64_t n, int64_t n16, int64_t n8, int64_t n4)
+{
+    Layout lo;
+    const uint64_t H = (uint64_t)Hkv, d = (uint64_t)D;
+    const uint64_t raw[10] = {
+        (uint64_t)n16 * H * d * 2, (uint64_t)n16 * H * d * 2,
+        (uint64_t)n8 * H * d,      (uint64_t)n8 * H * d,
+        (uint64_t)n4 * H * d / 2,  (uint64_t)n4 * H * d / 2,
+        (uint64_t)n8 * H * 2,      (uint64_t)n8 * H * 2,
+        (uint64_t)n4 * H * 2,      (uint64_t)n4 * H * 2};
+    lo.tier_map_off = 256;
+    lo.layer0_off = 256 + pad256((uint64_t)L * (uint64_t)n);
+    uint64_t off = 0;
+    for (int s = 0; s < 10; ++s) { lo.seg_off[s] = off; lo.seg_raw[s] = raw[s]; off += pad256(raw[s]); }
+    lo.layer_stride = off;
+    lo.total_bytes = lo.layer0_off + (uint64_t)L * lo.layer_stride;
+    return lo;
+}
+
+static bool dims_ok(const skv_shape *s)
+{
+    return s && s->n_layers > 0 && s->n_kv_heads > 0 && s->head_dim > 0 && s->n_tokens > 0 && s->n_requests > 0;
+}
+
+static int check_dims_supported(const skv_shape *s)
+{
+    if (!dims_ok(s)) return SKV_ERR_INVALID_ARG;
+    if (s->head_dim != 64 && s->head_dim != 128 && s->head_dim != 256) return SKV_ERR_UNSUPPORTED;
+    if (s->n_tokens > (1 << 20)) return SKV_ERR_UNSUPPORTED;
+    if (s->n_layers > 65535 || s->n_requests > 65535 || (int64_t)s->n_layers * s->n_requests > 65535) return SKV_ERR_UNSUPPORTED;
+    return SKV_OK;
+}
+
+static int check_cache(const skv_shape *s, const void *K, const void *V)
+{
+    int rc = check_dims_supported(s);
+    if (rc) return rc;
+    if (!K || !V) return SKV_ERR_INVALID_ARG;
+    if (s->stride_head <= 0 || s->stride_token <= 0 || s->stride_layer < 0 || s->stride_request < 0) return SKV_ERR_INVALID_ARG;
+    if ((s->stride_head % 8) || (s->stride_token % 8) || (s->stride_layer % 8) || (s->stride_request % 8)) return SKV_ERR_UNSUPPORTED;
+    if (((uintptr_t)K & 15) || ((uintptr_t)V & 15)) return SKV_ERR_UNSUPPORTED;
+    return SKV_OK;
+}
+
+static Geom make_geom(const skv_shape *s, const skv_counts *c)
+{
+    Geom g;
+    g.L = s->n_layers; g.Hq = s->n_q_heads; g.Hkv = s->n_kv_heads; g.D = s->head_dim; g.n = s->n_tokens; g.R = s->n_requests;
+    g.sr = s->stride_request; g.sl = s->stride_layer; g.st = s->stride_token; g.sh = s->stride_head;
+    g.n16 = c ? c->n16 : 0; g.n8 = c ? c->n8 : 0; g.n4 = c ? c->n4 : 0; g.n0 = c ? c->n0 : 0;
+    g.row_chunks = (g.Hkv * g.D + 255) / 256;
+    g.tiles = (g.n + kTileTokens - 1) / kTileTokens;
+    return g;
+}
+
+static bool counts_ok(const skv_shape *s, const skv_counts *c)
+{
+    return c && c->n16 >= 0 && c->n8 >= 0 && c->n4 >= 0 && c->n0 >= 0 &&
+           (int64_t)c->n16 + c->n8 + c->n4 + c->n0 == (int64_t)s->n_tokens;
+}
+
+static size_t scan_ws_bytes(const skv_shape *s)
+{
+    const size_t tiles = ((size_t)s->n_tokens + kTileTokens - 1) / kTileTokens;
+    return (size_t)s->n_requests * s->n_layers * tiles * sizeof(uint4);
+}
+
+// merged, sorted protected intervals = [0,s) U ranges; returns P (their total size) or <0 on error
+static int64_t merge_protected(const skv_shape *s, const skv_policy *p, std::vector<std::pair<int32_t, int32_t>> &out)
+{
+    const int32_t n = s->n_tokens;
+    if (p->n_sink < 0 || p->n_ranges < 0 || (p->n_ranges > 0 && !p->ranges)) return -1;
+    std::vector<std::pair<int32_t, int32_t>> iv;
+    if (p->n_sink > 0) iv.emplace_back(0, std::min(p->n_sink, n));
+    for (int i = 0; i < p->n_ranges; ++i) {
+        const int32_t b = p->ranges[2 * i], e = p->ranges[2 * i + 1];
+        if (b < 0 || e > n || b > e) return -1;
+        if (e > b) iv.emplace_back(b, e);
+    }
+    std::sort(iv.begin(), iv.end());
+    out.clear();
+    for (auto &x : iv) {
+        if (!out.empty() && x.first <= out.back().second) out.back().second = std::max(out.back().second, x.second);
+        else out.push_back(x);
+    }
+    int64_t P = 0;
+    for (auto &x : out) P += x.second - x.first;
+    return P;
+}
+
+static int tier_counts_impl(const skv_shape *s, const skv_policy *p, skv_counts *c,
+                            std::vector<std::pair<int32_t, int32_t>> &prot)
+{
+    if (!dims_ok(s) || !p || !c) return SKV_ERR_INVALID_ARG;
+    double b = p->budget;
+    if (!(b > 0.0)) return SKV_ERR_INVALID_ARG;           // also rejects NaN
+    if (b > 1.0) b = 1.0;
+    const int64_t P = merge_protected(s, p, prot);
+    if (P < 0) return SKV_ERR_INVALID_ARG;
+    const int64_t n = s->n_tokens;
+    const int64_t Q = (int64_t)floor(4.0 * b * (double)n + 1e-6);     // quarter-units: 4 / 2 / 1 / 0 per token
+    const int64_t m = n - P, R = Q - 4 * P;
+    if (R < 0) return SKV_ERR_BUDGET_INFEASIBLE;
+    int64_t n16 = P, n8 = 0, n4 = 0, n0 = 0;
+    if (R >= 4 * m) n16 = n;
+    else if (R >= 2 * m) { const int64_t up = (R - 2 * m) / 2; n16 = P + up; n8 = m - up; }
+    else if (p->allow_int4) {
+        if (R >= m) { n8 = R - m; n4 = m - n8; }
+        else { n4 = R; n0 = m - R; }
+    } else { n8 = R / 2; n0 = m - n8; }
+    c->n16 = (int32_t)n16; c->n8 = (int32_t)n8; c->n4 = (int32_t)n4; c->n0 = (int32_t)n0;
+    c->allow_int4 = p->allow_int4 ? 1 : 0; c->reserved = 0;
+    c->budget_q4 = Q; c->spent_q4 = 4 * n16 + 2 * n8 + n4;
+    return SKV_OK;
+}
+
+static void put32(uint8_t *p, uint32_t v) { memcpy(p, &v, 4); }
+static void put64(uint8_t *p, uint64_t v) { memcpy(p, &v, 8); }
+static uint32_t get32(const uint8_t *p) { uint32_t v; memcpy(&v, p, 4); return v; }
+static uint64_t get64(const uint8_t *p) { uint64_t v; memcpy(&v, p, 8); return v; }
+
+}  // namespace skv
+
+using namespace skv;
+
+extern "C" {
+
+int skv_tier_counts(const skv_shape *shape, const skv_policy *policy, skv_counts *counts_out)
+{
+    std::vector<std::pair<int32_t, int32_t>> prot;
+    return tier_counts_impl(shape, policy, counts_out, prot);
+}
+
+size_t skv_blob_bytes(const skv_shape *shape, const skv_counts *counts)
+{
+    if (!dims_ok(shape) || !counts_ok(shape, counts)) return 0;
+    return (size_t)make_layout(shape->n_layers, shape->n_kv_heads, shape->head_dim, shape->n_tokens,
+                               counts->n16, counts->n8, counts->n4).total_bytes;
+}
+
+size_t skv_workspace_bytes(const skv_shape *shape, int32_t window)
+{
+    if (!dims_ok(shape)) return 0;
+    const Geom g = make_geom(shape, nullptr);
+    size_t need = scan_ws_bytes(shape);
+    need = std::max(need, (size_t)shape->n_requests * shape->n_layers * shape->n_tokens * sizeof(uint32_t));  // assign keys
+    need = std::max(need, importance_ws_bytes(g, 0));
+    if (window > 0 && shape->n_q_heads > 0) need = std::max(need, importance_ws_bytes(g, window));
+    return (need + 255) & ~(size_t)255;
+}
+
+int skv_blob_check(const void *header_host, size_t blob_bytes, skv_shape *shape_out, skv_counts *counts_out)
+{
+    if (!header_host) return SKV_ERR_INVALID_ARG;
+    if (blob_bytes < 256) return SKV_ERR_BAD_BLOB;
+    const uint8_t *h = (const uint8_t *)header_host;
+    if (get32(h) != 0x31564B53u || get32(h + 4) != 1u) return SKV_ERR_BAD_BLOB;
+    const uint32_t L = get32(h + 8), Hkv = get32(h + 12), D = get32(h + 16), n = get32(h + 20);
+    const uint32_t n16 = get32(h + 24), n8 = get32(h + 28), n4 = get32(h + 32), n0 = get32(h + 36);
+    const uint32_t flags = get32(h + 40);
+    if (L == 0 || Hkv == 0 || n == 0 || L > 65535u || n > (1u << 20) || Hkv > 65535u) return SKV_ERR_BAD_BLOB;
+    if (D != 64 && D != 128 && D != 256) return SKV_ERR_BAD_BLOB;
+    if ((uint64_t)n16 + n8 + n4 + n0 != n || (flags & ~1u) || get32(h + 44) != 0) return SKV_ERR_BAD_BLOB;
+    if (!(flags & 1u) && n4 != 0) return SKV_ERR_BAD_BLOB;
+    const Layout lo = make_layout((int)L, (int)Hkv, (int)D, n, n16, n8, n4);
+    if (get64(h + 56) != lo.tier_map_off || get64(h + 64) != lo.layer0_off || get64(h + 72) != lo.layer_stride ||
+        get64(h + 160) != lo.total_bytes || lo.total_bytes != blob_bytes) return SKV_ERR_BAD_BLOB;
+    for (int s = 0; s < 10; ++s) if (get64(h + 80 + 8 * s) != lo.seg_off[s]) return SKV_ERR_BAD_BLOB;
+    for (int o = 168; o < 256; ++o) if (h[o]) return SKV_ERR_BAD_BLOB;
+    const uint64_t Q = get64(h + 48);
+    if (Q > 4ull * n || 4ull * n16 + 2ull * n8 + n4 > Q) return SKV_ERR_BAD_BLOB;
+    if (shape_out) {
+        memset(shape_out, 0, sizeof(*shape_out));
+        shape_out->n_layers = (int32_t)L; shape_out->n_kv_heads = (int32_t)Hkv; shape_out->head_dim = (int32_t)D;
+        shape_out->n_tokens = (int32_t)n; shape_out->n_requests = 1;
+    }
+    if (counts_out) {
+        counts_out->n16 = (int32_t)n16; counts_out->n8 = (int32_t)n8; counts_out->n4 = (int32_t)n4; counts_out->n0 = (int32_t)n0;
+        counts_out->allow_int4 = (int32_t)(flags & 1u); counts_out->reserved = 0;
+        counts_out->budget_q4 = (int64_t)Q; counts_out->spent_q4 = 4ll * n16 + 2ll * n8 + n4;
+    }
+    return SKV_OK;
+}
+
+int skv_importance(const skv_shape *shape, const void *K_dev, const void *Q_dev, int32_t window, int32_t causal,
+                   float lambda, float *importance_dev, void *ws, size_t ws_bytes, void *cuda_stream)
+{
+    int rc = check_cache(shape, K_dev, K_dev);
+    if (rc) return rc;
+    if (!Q_dev || !importance_dev || !ws) return SKV_ERR_INVALID_ARG;
+    if (shape->n_q_heads <= 0 || shape->n_q_heads % shape->n_kv_heads) return SKV_ERR_INVALID_ARG;
+    if (window < 1 || window > shape->n_tokens) return SKV_ERR_INVALID_ARG;
+    if (!(lambda >= 0.0f)) return SKV_ERR_INVALID_ARG;
+    if ((uintptr_t)Q_dev & 15) return SKV_ERR_UNSUPPORTED;
+    const Geom g = make_geom(shape, nullptr);
+    if (ws_bytes < importance_ws_bytes(g, window)) return SKV_ERR_BUFFER_TOO_SMALL;
+    cudaError_t e = launch_importance(g, (const __half *)K_dev, (const __half *)Q_dev, window, causal ? 1 : 0, lambda,
+                                      importance_dev, ws, ws_bytes, (cudaStream_t)cuda_stream);
+    return e == cudaSuccess ? SKV_OK : SKV_ERR_CUDA;
+}
+
+int skv_importance_kvnorm(const skv_shape *shape, const void *K_dev, float lambda, float *importance_dev,
+                          void *ws, size_t ws_bytes, void *cuda_stream)
+{
+    int rc = check_cache(shape, K_dev, K_dev);
+    if (rc) return rc;
+    if (!importance_dev || !ws || !(lambda >= 0.0f)) return SKV_ERR_INVALID_ARG;
+    const Geom g = make_geom(shape, nullptr);
+    if (ws_bytes < importance_ws_bytes(g, 0)) return SKV_ERR_BUFFER_TOO_SMALL;
+    cudaError_t e = launch_importance_kvnorm(g, (const __half *)K_dev, lambda, importance_dev, (float *)ws,
+                                             (cudaStream_t)cuda_stream);
+    return e == cudaSuccess ? SKV_OK : SKV_ERR_CUDA;
+}
+
+int skv_assign_tiers(const skv_shape *shape, const skv_policy *policy, const float *importance_dev,
+                     uint8_t *tier_map_dev, skv_counts *counts_out_host, void *ws, size_t ws_bytes, void *cuda_stream)
+{
+    int rc = check_dims_supported(shape);
+    if (rc) return rc;
+    if (!policy || !importance_dev || !tier_map_dev) return SKV_ERR_INVALID_ARG;
+    skv_counts c;
+    std::vector<std::pair<int32_t, int32_t>> prot;
+    rc = tier_counts_impl(shape, policy, &c, prot);
+    if (rc) return rc;
+    if (prot.size() > 32) return SKV_ERR_UNSUPPORTED;    // more than 32 disjoint protected intervals
+    const size_t key_bytes = (size_t)shape->n_requests * shape->n_layers * shape->n_tokens * sizeof(uint32_t);
+    const bool need_ws = (size_t)shape->n_tokens * 4 > 200 * 1024;
+    if (need_ws && (!ws || ws_bytes < key_bytes)) return SKV_ERR_BUFFER_TOO_SMALL;
+    Intervals iv;
+    memset(&iv, 0, sizeof(iv));
+    iv.count = (int32_t)prot.size();
+    for (size_t i = 0; i < prot.size(); ++i) { iv.lo[i] = prot[i].first; iv.hi[i] = prot[i].second; }
+    const Geom g = make_geom(shape, &c);
+    cudaError_t e = launch_assign(g, iv, importance_dev, tier_map_dev, (uint32_t *)ws, (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return SKV_ERR_CUDA;
+    if (counts_out_host) *counts_out_host = c;
+    return SKV_OK;
+}
+
+int skv_pack(const skv_shape *shape, const void *K_dev, const void *V_dev, const uint8_t *tier_map_dev,
+             const skv_counts *counts, void *blob_dev, size_t blob_capacity, void *ws, size_t ws_bytes, void *cuda_stream)
+{
+    int rc = check_cache(shape, K_dev, V_dev);
+    if (rc) return rc;
+    if (!tier_map_dev || !blob_dev || !ws || !counts_ok(shape, counts)) return SKV_ERR_INVALID_ARG;
+    if ((uintptr_t)blob_dev & 255) return SKV_ERR_UNSUPPORTED;
+    const Geom g = make_geom(shape, counts);
+    const Layout lo = make_layout(g.L, g.Hkv, g.D, g.n, g.n16, g.n8, g.n4);
+    if (blob_capacity < (size_t)lo.total_bytes * (size_t)g.R) return SKV_ERR_BUFFER_TOO_SMALL;
+    if (ws_bytes < scan_ws_bytes(shape)) return SKV_ERR_BUFFER_TOO_SMALL;
+
+    Header256 hdr;
+    memset(&hdr, 0, sizeof(hdr));
+    uint8_t *h = reinterpret_cast<uint8_t *>(hdr.w);
+    put32(h + 0, 0x31564B53u); put32(h + 4, 1u);
+    put32(h + 8, (uint32_t)g.L); put32(h + 12, (uint32_t)g.Hkv); put32(h + 16, (uint32_t)g.D); put32(h + 20, (uint32_t)g.n);
+    put32(h + 24, (uint32_t)g.n16); put32(h + 28, (uint32_t)g.n8); put32(h + 32, (uint32_t)g.n4); put32(h + 36, (uint32_t)g.n0);
+    put32(h + 40, counts->allow_int4 ? 1u : 0u);
+    put64(h + 48, (uint64_t)counts->budget_q4);
+    put64(h + 56, lo.tier_map_off); put64(h + 64, lo.layer0_off); put64(h + 72, lo.layer_stride);
+    for (int s = 0; s < 10; ++s) put64(h + 80 + 8 * s, lo.seg_off[s]);
+    put64(h + 160, lo.total_bytes);
+
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    cudaError_t e = launch_tile_scan_pack(g, lo, tier_map_dev, (uint8_t *)blob_dev, lo.total_bytes, hdr, (uint4 *)ws, st);
+    if (e != cudaSuccess) return SKV_ERR_CUDA;
+    e = launch_pack(g, lo, (const __half *)K_dev, (const __half *)V_dev, tier_map_dev, (uint8_t *)blob_dev,
+                    lo.total_bytes, (const uint4 *)ws, st);
+    return e == cudaSuccess ? SKV_OK : SKV_ERR_CUDA;
+}
+
+int skv_unpack(const skv_shape *shape, const void *blob_dev, size_t blob_bytes, const skv_counts *counts,
+               void *K_out_dev, void *V_out_dev, uint8_t *tier_map_out_dev, void *ws, size_t ws_bytes, void *cuda_stream)
+{
+    int rc = check_cache(shape, K_out_dev, V_out_dev);
+    if (rc) return rc;
+    if (!blob_dev || !ws || !counts_ok(shape, counts)) return SKV_ERR_INVALID_ARG;
+    if ((uintptr_t)blob_dev & 255) return SKV_ERR_UNSUPPORTED;
+    const Geom g = make_geom(shape, counts);
+    const Layout lo = make_layout(g.L, g.Hkv, g.D, g.n, g.n16, g.n8, g.n4);
+    if (blob_bytes != (size_t)lo.total_bytes) return SKV_ERR_BAD_BLOB;
+    if (ws_bytes < scan_ws_bytes(shape)) return SKV_ERR_BUFFER_TOO_SMALL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    cudaError_t e = launch_tile_scan_unpack(g, lo, (const uint8_t *)blob_dev, lo.total_bytes, tier_map_out_dev, (uint4 *)ws, st);
+    if (e != cudaSuccess) return SKV_ERR_CUDA;
+    e = launch_unpack(g, lo, (const uint8_t *)blob_dev, lo.total_bytes, (__half *)K_out_dev, (__half *)V_out_dev,
+                      (const uint4 *)ws, st);
+    return e == cudaSuccess ? SKV_OK : SKV_ERR_CUDA;
+}
+
+const char *skv_strerror(int status)
+{
+    switch (status) {
+    case SKV_OK: return "ok";
+    case SKV_ERR_INVALID_ARG: return "invalid argument";
+    case SKV_ERR_UNSUPPORTED: return "unsupported shape, stride or alignment";
+    case SKV_ERR_BUDGET_INFEASIBLE: return "protected tokens alone exceed the transfer budget";
+    case SKV_ERR_BUFFER_TOO_SMALL: return "blob capacity or workspace too small";
+    case SKV_ERR_BAD_BLOB: return "malformed SKV1 blob";
+    case SKV_ERR_CUDA: return "CUDA runtime error";
+    default: return "unknown status";
+    }
+}
+
+const char *skv_version(void) { return "skv 0.1 sm_100a"; }
+
+}  // extern "C"

@@ -1,0 +1,226 @@
+// skv_pack.cu -- quantize-and-pack (Alg. 1 step 4; "standard symmetric").
+//
+// One warp per token, one CTA per 32-token tile of one (request, layer).  The warp reads the token's K
+// row and V row with 16-byte loads (8 fp16 per lane, coalesced; any 16-B aligned strides), reduces the
+// |x| max over the lanes of a head vector with shuffles, quantises in fp32 exactly as include/skv.h
+// specifies, and stores the codes at the token's slot (tile base from skv_scan.cu + in-tile rank from a
+// ballot).  All lanes of a warp share one tier => no divergence.  Dropped tokens are never loaded.
+//
+// HBM-bound: reads Bytes_FP16, writes beta*Bytes_FP16.
+#include "skv_common.cuh"
+
+namespace skv {
+
+__device__ __forceinline__ uint4 ld_stream(const void *p)
+{
+    uint4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ void st_stream(void *p, uint4 v)
+{
+    asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};" :: "l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+__device__ __forceinline__ void st_stream(void *p, uint2 v)
+{
+    asm volatile("st.global.L1::no_allocate.v2.u32 [%0], {%1,%2};" :: "l"(p), "r"(v.x), "r"(v.y) : "memory");
+}
+__device__ __forceinline__ void st_stream(void *p, uint32_t v)
+{
+    asm volatile("st.global.L1::no_allocate.u32 [%0], %1;" :: "l"(p), "r"(v) : "memory");
+}
+
+// |x| max of the 8 halves in a uint4, as a half2 with the max in both halves' union (max(lo,hi) taken later)
+__device__ __forceinline__ __half2 absmax8(const uint4 &v)
+{
+    const __half2 a = __habs2(*reinterpret_cast<const __half2 *>(&v.x));
+    const __half2 b = __habs2(*reinterpret_cast<const __half2 *>(&v.y));
+    const __half2 c = __habs2(*reinterpret_cast<const __half2 *>(&v.z));
+    const __half2 d = __habs2(*reinterpret_cast<const __half2 *>(&v.w));
+    return __hmax2(__hmax2(a, b), __hmax2(c, d));
+}
+
+// round-half-even of fl32(x*inv) via the 1.5*2^23 magic constant: the low bits of the sum's encoding are
+// the two's-complement integer (|x*inv| <= qmax*(1+2^-23) << 2^22, so the clamp of the spec is a no-op).
+__device__ __forceinline__ uint32_t rne_code_bits(float x, float inv)
+{
+    return __float_as_uint(__fadd_rn(__fmul_rn(x, inv), 12582912.0f));
+}
+
+template <int D, int QMAX>
+__device__ __forceinline__ void quantize_chunk(const uint4 &v, uint32_t lane, __half &amax_out, uint32_t codes[8])
+{
+    constexpr int LPV = D / 8;                        // lanes per head vector
+    __half2 m2 = absmax8(v);
+#pragma unroll
+    for (int o = 1; o < LPV; o <<= 1) {
+        const uint32_t other = __shfl_xor_sync(0xffffffffu, *reinterpret_cast<uint32_t *>(&m2), o);
+        m2 = __hmax2(m2, *reinterpret_cast<const __half2 *>(&other));
+    }
+    const __half amax = __hmax(__low2half(m2), __high2half(m2));
+    const float af = __half2float(amax);
+    const float inv = af != 0.0f ? __fdiv_rn((float)QMAX, af) : 0.0f;
+    const __half2 *h = reinterpret_cast<const __half2 *>(&v);
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const float2 f = __half22float2(h[k]);
+        codes[2 * k] = rne_code_bits(f.x, inv);
+        codes[2 * k + 1] = rne_code_bits(f.y, inv);
+    }
+    amax_out = amax;
+    (void)lane;
+}
+
+__device__ __forceinline__ uint32_t pack4_bytes(uint32_t a, uint32_t b, uint32_t c, uint32_t d)
+{
+    const uint32_t ab = __byte_perm(a, b, 0x0040);    // [a.b0, b.b0, -, -]
+    const uint32_t cd = __byte_perm(c, d, 0x0040);
+    return __byte_perm(ab, cd, 0x5410);               // [a.b0, b.b0, c.b0, d.b0]
+}
+
+template <int D>
+__global__ void __launch_bounds__(256)
+pack_kernel(Geom g, Layout lo, const __half *__restrict__ K, const __half *__restrict__ V,
+            const uint8_t *__restrict__ tier_map, uint8_t *__restrict__ blob, uint64_t blob_stride,
+            const uint4 *__restrict__ tile_base)
+{
+    constexpr int LPV = D / 8;
+    const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    const int64_t tile = blockIdx.x;
+    const int l = blockIdx.y, r = blockIdx.z;
+    const int64_t n = g.n;
+    const int64_t j0 = tile * kTileTokens;
+
+    // tiers of the tile: lane i holds token j0+i
+    const uint8_t *tm = tier_map + ((int64_t)r * g.L + l) * n;
+    const uint32_t my_t = (j0 + lane < n) ? (uint32_t)tm[j0 + lane] : 0xFFu;
+    const uint32_t m16 = __ballot_sync(0xffffffffu, my_t == 16u);
+    const uint32_t m8 = __ballot_sync(0xffffffffu, my_t == 8u);
+    const uint32_t m4 = __ballot_sync(0xffffffffu, my_t == 4u);
+    const uint4 base = tile_base[((int64_t)r * g.L + l) * g.tiles + tile];
+
+    uint8_t *lbase = blob + (uint64_t)r * blob_stride + lo.layer0_off + (uint64_t)l * lo.layer_stride;
+    const int row_elems = g.Hkv * D;
+    const int64_t cache_off = (int64_t)r * g.sr + (int64_t)l * g.sl;
+
+    for (uint32_t i = warp; i < (uint32_t)kTileTokens; i += nwarps) {
+        const uint32_t t = __shfl_sync(0xffffffffu, my_t, i);
+        if (t != 16u && t != 8u && t != 4u) continue;                 // dropped / tail / invalid: no bytes
+        const uint32_t below = (1u << i) - 1u;
+        const int64_t j = j0 + i;
+        const __half *krow = K + cache_off + j * g.st;
+        const __half *vrow = V + cache_off + j * g.st;
+
+        if (t == 16u) {
+            const uint32_t slot = base.x + __popc(m16 & below);
+            if (slot >= (uint32_t)g.n16) continue;
+            uint8_t *kd = lbase + lo.seg_off[0] + (uint64_t)slot * row_elems * 2;
+            uint8_t *vd = lbase + lo.seg_off[1] + (uint64_t)slot * row_elems * 2;
+            for (int c0 = 0; c0 < g.row_chunks; c0 += 4) {
+                uint4 kv[4], vv[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int e = (c0 + u) * 256 + lane * 8;
+                    if (e < row_elems) {
+                        const int h = e / D, c = e % D;
+                        kv[u] = ld_stream(krow + (int64_t)h * g.sh + c);
+                        vv[u] = ld_stream(vrow + (int64_t)h * g.sh + c);
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int e = (c0 + u) * 256 + lane * 8;
+                    if (e < row_elems) { st_stream(kd + e * 2, kv[u]); st_stream(vd + e * 2, vv[u]); }
+                }
+            }
+        } else if (t == 8u) {
+            const uint32_t slot = base.y + __popc(m8 & below);
+            if (slot >= (uint32_t)g.n8) continue;
+            uint8_t *kd = lbase + lo.seg_off[2] + (uint64_t)slot * row_elems;
+            uint8_t *vd = lbase + lo.seg_off[3] + (uint64_t)slot * row_elems;
+            __half *ks = reinterpret_cast<__half *>(lbase + lo.seg_off[6]) + (uint64_t)slot * g.Hkv;
+            __half *vs = reinterpret_cast<__half *>(lbase + lo.seg_off[7]) + (uint64_t)slot * g.Hkv;
+            for (int c0 = 0; c0 < g.row_chunks; c0 += 4) {
+                uint4 kv[4], vv[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int e = (c0 + u) * 256 + lane * 8;
+                    kv[u] = make_uint4(0, 0, 0, 0); vv[u] = kv[u];
+                    if (e < row_elems) {
+                        const int h = e / D, c = e % D;
+                        kv[u] = ld_stream(krow + (int64_t)h * g.sh + c);
+                        vv[u] = ld_stream(vrow + (int64_t)h * g.sh + c);
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    if ((c0 + u) * 256 >= row_elems) break;            // warp-uniform
+                    const int e = (c0 + u) * 256 + lane * 8;
+                    __half ak, av; uint32_t ck[8], cv[8];
+                    quantize_chunk<D, 127>(kv[u], lane, ak, ck);
+                    quantize_chunk<D, 127>(vv[u], lane, av, cv);
+                    if (e < row_elems) {
+                        st_stream(kd + e, make_uint2(pack4_bytes(ck[0], ck[1], ck[2], ck[3]), pack4_bytes(ck[4], ck[5], ck[6], ck[7])));
+                        st_stream(vd + e, make_uint2(pack4_bytes(cv[0], cv[1], cv[2], cv[3]), pack4_bytes(cv[4], cv[5], cv[6], cv[7])));
+                        if ((lane % LPV) == 0) { ks[e / D] = ak; vs[e / D] = av; }
+                    }
+                }
+            }
+        } else {
+            const uint32_t slot = base.z + __popc(m4 & below);
+            if (slot >= (uint32_t)g.n4) continue;
+            uint8_t *kd = lbase + lo.seg_off[4] + (uint64_t)slot * (row_elems / 2);
+            uint8_t *vd = lbase + lo.seg_off[5] + (uint64_t)slot * (row_elems / 2);
+            __half *ks = reinterpret_cast<__half *>(lbase + lo.seg_off[8]) + (uint64_t)slot * g.Hkv;
+            __half *vs = reinterpret_cast<__half *>(lbase + lo.seg_off[9]) + (uint64_t)slot * g.Hkv;
+            for (int c0 = 0; c0 < g.row_chunks; c0 += 4) {
+                uint4 kv[4], vv[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int e = (c0 + u) * 256 + lane * 8;
+                    kv[u] = make_uint4(0, 0, 0, 0); vv[u] = kv[u];
+                    if (e < row_elems) {
+                        const int h = e / D, c = e % D;
+                        kv[u] = ld_stream(krow + (int64_t)h * g.sh + c);
+                        vv[u] = ld_stream(vrow + (int64_t)h * g.sh + c);
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    if ((c0 + u) * 256 >= row_elems) break;
+                    const int e = (c0 + u) * 256 + lane * 8;
+                    __half ak, av; uint32_t ck[8], cv[8];
+                    quantize_chunk<D, 7>(kv[u], lane, ak, ck);
+                    quantize_chunk<D, 7>(vv[u], lane, av, cv);
+                    if (e < row_elems) {
+                        uint32_t kb[4], vb[4];
+#pragma unroll
+                        for (int k = 0; k < 4; ++k) {                  // element 2k low nibble, 2k+1 high nibble
+                            kb[k] = (ck[2 * k] & 0xFu) | (ck[2 * k + 1] << 4);
+                            vb[k] = (cv[2 * k] & 0xFu) | (cv[2 * k + 1] << 4);
+                        }
+                        st_stream(kd + e / 2, pack4_bytes(kb[0], kb[1], kb[2], kb[3]));
+                        st_stream(vd + e / 2, pack4_bytes(vb[0], vb[1], vb[2], vb[3]));
+                        if ((lane % LPV) == 0) { ks[e / D] = ak; vs[e / D] = av; }
+                    }
+                }
+            }
+        }
+    }
+}
+
+cudaError_t launch_pack(const Geom &g, const Layout &lo, const __half *K, const __half *V, const uint8_t *tier_map,
+                        uint8_t *blob, uint64_t blob_stride, const uint4 *tile_base, cudaStream_t s)
+{
+    dim3 grid(g.tiles, g.L, g.R);
+    switch (g.D) {
+    case 64:  pack_kernel<64><<<grid, 256, 0, s>>>(g, lo, K, V, tier_map, blob, blob_stride, tile_base); break;
+    case 128: pack_kernel<128><<<grid, 256, 0, s>>>(g, lo, K, V, tier_map, blob, blob_stride, tile_base); break;
+    case 256: pack_kernel<256><<<grid, 256, 0, s>>>(g, lo, K, V, tier_map, blob, blob_stride, tile_base); break;
+    default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+}  // namespace skv

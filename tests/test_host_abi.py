@@ -1,0 +1,123 @@
+"""CPU-only tests of the C-ABI library: it loads without a GPU, exports every symbol include/skv.h declares,
+and its host-side logic (tier counts, blob sizes, header validation, argument errors) agrees with the oracle."""
+import os
+import re
+
+import numpy as np
+import pytest
+
+import oracle
+import paper_2606_08635_b200 as skv
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    from paper_2606_08635_b200 import build
+    build.build()
+
+
+def test_library_exports_every_declared_symbol():
+    text = open(os.path.join(ROOT, "include", "skv.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    declared = set(re.findall(r"\b(skv_[a-z0-9_]+)\s*\(", text))
+    assert declared == set(skv.EXPORTS)
+    L = skv.lib()
+    for name in declared:
+        assert getattr(L, name) is not None
+    assert "sm_100a" in skv.skv_version()
+
+
+def test_tier_counts_match_oracle_sweep():
+    rng = np.random.default_rng(0)
+    for _ in range(2000):
+        n = int(rng.integers(1, 6000))
+        b = float(rng.choice([rng.uniform(0.01, 1.3), rng.integers(1, 41) / 40.0]))
+        s = int(rng.integers(0, min(n, 9) + 1))
+        rngs = []
+        for _r in range(int(rng.integers(0, 4))):
+            a = int(rng.integers(0, n + 1)); e = int(rng.integers(a, n + 1)); rngs.append((a, e))
+        a4 = bool(rng.integers(0, 2))
+        shape = skv.make_shape(2, 4, 2, 128, n)
+        pol = skv.make_policy(b, s, rngs, a4)
+        try:
+            want, _ = oracle.tier_counts(n, b, s, rngs, a4)
+        except ValueError:
+            with pytest.raises(skv.SkvError) as ei:
+                skv.skv_tier_counts(shape, pol)
+            assert ei.value.status == skv.SKV_ERR_BUDGET_INFEASIBLE
+            continue
+        got = skv.skv_tier_counts(shape, pol)
+        assert got.as_tuple() == (want.n16, want.n8, want.n4, want.n0)
+        assert (got.budget_q4, got.spent_q4, got.allow_int4) == (want.budget_q4, want.spent_q4, int(a4))
+        assert skv.skv_blob_bytes(shape, got) == oracle.blob_bytes(2, 2, 128, n, want)
+
+
+def test_argument_errors():
+    shape = skv.make_shape(2, 4, 2, 128, 100)
+    for bad_b in (0.0, -1.0, float("nan")):
+        with pytest.raises(skv.SkvError) as ei:
+            skv.skv_tier_counts(shape, skv.make_policy(bad_b))
+        assert ei.value.status == skv.SKV_ERR_INVALID_ARG
+    for rngs in ([(5, 101)], [(-1, 3)], [(9, 4)]):
+        with pytest.raises(skv.SkvError) as ei:
+            skv.skv_tier_counts(shape, skv.make_policy(0.5, 0, rngs))
+        assert ei.value.status == skv.SKV_ERR_INVALID_ARG
+    c = skv.skv_tier_counts(shape, skv.make_policy(0.5, 4))
+    # device entry points validate before launching anything: null pointers / bad dims / misalignment
+    ws = 0
+    for fn, args in (
+        (skv.skv_pack, (shape, 0, 0, 0, c, 0, 0)),
+        (skv.skv_unpack, (shape, 0, 0, c, 0, 0, None, 0)),
+    ):
+        with pytest.raises(skv.SkvError) as ei:
+            fn(*args, stream=0)
+        assert ei.value.status == skv.SKV_ERR_INVALID_ARG
+    shape_bad = skv.make_shape(2, 4, 2, 96, 100)
+    L = skv.lib()
+    import ctypes as C
+    rc = L.skv_pack(C.byref(shape_bad), 256, 256, 256, C.byref(c), 256, 1 << 30, 256, 1 << 30, None)
+    assert rc == skv.SKV_ERR_UNSUPPORTED
+    rc = L.skv_pack(C.byref(shape), 256 + 8, 256, 256, C.byref(c), 256, 1 << 30, 256, 1 << 30, None)
+    assert rc == skv.SKV_ERR_UNSUPPORTED            # K not 16-byte aligned
+    rc = L.skv_pack(C.byref(shape), 256, 256, 256, C.byref(c), 256, 16, 256, 1 << 30, None)
+    assert rc == skv.SKV_ERR_BUFFER_TOO_SMALL       # blob capacity
+    rc = L.skv_pack(C.byref(shape), 256, 256, 256, C.byref(c), 256, 1 << 30, 256, 16, None)
+    assert rc == skv.SKV_ERR_BUFFER_TOO_SMALL       # workspace
+    rc = L.skv_importance(C.byref(shape), 256, 256, 101, 1, 0.0, 256, 256, 1 << 30, None)
+    assert rc == skv.SKV_ERR_INVALID_ARG            # window > n
+    shape3 = skv.make_shape(2, 5, 2, 128, 100)
+    rc = L.skv_importance(C.byref(shape3), 256, 256, 8, 1, 0.0, 256, 256, 1 << 30, None)
+    assert rc == skv.SKV_ERR_INVALID_ARG            # Hq % Hkv != 0
+    assert skv.skv_strerror(skv.SKV_ERR_BAD_BLOB).startswith("malformed")
+
+
+def test_blob_check_accepts_oracle_blob_and_rejects_corruption():
+    L_, n, Hkv, d = 2, 50, 2, 64
+    rng = np.random.default_rng(1)
+    K = rng.standard_normal((L_, n, Hkv, d)).astype(np.float16)
+    V = rng.standard_normal((L_, n, Hkv, d)).astype(np.float16)
+    c, prot = oracle.tier_counts(n, 0.4, 4, [], True)
+    tier = oracle.assign(rng.random((L_, n)).astype(np.float32), prot, c)
+    blob = oracle.pack(K, V, tier, c)
+    s, cc = skv.skv_blob_check(blob[:256].tobytes(), blob.size)
+    assert (s.n_layers, s.n_kv_heads, s.head_dim, s.n_tokens) == (L_, Hkv, d, n)
+    assert cc.as_tuple() == (c.n16, c.n8, c.n4, c.n0) and cc.budget_q4 == c.budget_q4 and cc.allow_int4 == 1
+    for off in (0, 3, 4, 8, 12, 16, 20, 24, 28, 32, 36, 40, 44, 56, 64, 72, 80, 152, 160, 200, 255):
+        h = bytearray(blob[:256].tobytes()); h[off] ^= 0x01
+        with pytest.raises(skv.SkvError) as ei:
+            skv.skv_blob_check(bytes(h), blob.size)
+        assert ei.value.status == skv.SKV_ERR_BAD_BLOB, off
+    with pytest.raises(skv.SkvError):
+        skv.skv_blob_check(blob[:256].tobytes(), blob.size - 256)
+
+
+def test_workspace_covers_every_entry_point():
+    for (L_, Hq, Hkv, d, n, R, w) in [(1, 2, 2, 128, 256, 1, 16), (32, 32, 8, 128, 32768, 4, 64), (42, 16, 8, 256, 4096, 1, 32)]:
+        shape = skv.make_shape(L_, Hq, Hkv, d, n, R)
+        ws = skv.skv_workspace_bytes(shape, w)
+        assert ws % 256 == 0
+        assert ws >= R * L_ * ((n + 31) // 32) * 16          # tile prefix table of pack / unpack
+        assert ws >= R * L_ * n * 4                           # selection keys when they do not fit shared memory
+        assert ws >= R * L_ * Hq * w * 4                      # per-row log-sum-exp of the importance pass
