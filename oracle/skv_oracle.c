@@ -101,6 +101,10 @@ void orc_importance(int32_t L, int32_t Hq, int32_t Hkv, int32_t d, int64_t n, in
         double *A = (double *)calloc((size_t)n, sizeof(double));
         double *z = (double *)malloc((size_t)n * sizeof(double));
         double *kq = (double *)malloc((size_t)d * sizeof(double));
+        /* the layer's keys converted to double once (exact), [n][Hkv][d] */
+        double *Kd = (double *)malloc((size_t)n * Hkv * d * sizeof(double));
+        for (size_t e = 0; e < (size_t)n * Hkv * d; ++e)
+            Kd[e] = (double)orc_half_to_float(K[(size_t)l * n * Hkv * d + e]);
         for (int32_t h = 0; h < Hq; ++h) {
             const int32_t g = h / G;
             for (int32_t i = 0; i < w; ++i) {
@@ -110,9 +114,9 @@ void orc_importance(int32_t L, int32_t Hq, int32_t Hkv, int32_t d, int64_t n, in
                 for (int32_t c = 0; c < d; ++c) kq[c] = (double)orc_half_to_float(q[c]);
                 double zmax = -INFINITY;
                 for (int64_t j = 0; j <= last; ++j) {
-                    const uint16_t *k = K + (((size_t)l * n + j) * Hkv + g) * d;
+                    const double *k = Kd + ((size_t)j * Hkv + g) * d;
                     double dot = 0.0;
-                    for (int32_t c = 0; c < d; ++c) dot += kq[c] * (double)orc_half_to_float(k[c]);
+                    for (int32_t c = 0; c < d; ++c) dot += kq[c] * k[c];
                     z[j] = dot * inv_sqrt_d;
                     if (z[j] > zmax) zmax = z[j];
                 }
@@ -126,7 +130,7 @@ void orc_importance(int32_t L, int32_t Hq, int32_t Hkv, int32_t d, int64_t n, in
             double delta = (double)(n - 1 - j);                 /* P4: 0-based recency distance */
             I[(size_t)l * n + j] = (float)(A[j] * norm * exp(-lambda * delta));
         }
-        free(A); free(z); free(kq);
+        free(A); free(z); free(kq); free(Kd);
     }
 }
 
