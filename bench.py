@@ -309,9 +309,10 @@ def oracle_sample(cfg, b, target_seconds):
     nbytes, tp, tu = run(layers)
     per_layer = (tp + tu) / layers
     want = int(min(cfg.L, max(layers, target_seconds / max(per_layer, 1e-9))))
-    want = max(threads, (want // threads) * threads) if want >= threads else want
-    if want > layers * 2:
-        layers = min(cfg.L, want)
+    if want >= threads:
+        want = (want // threads) * threads
+    if want > layers:
+        layers = want
         nbytes, tp, tu = run(layers)
     gbs = nbytes / (tp + tu) / 1e9
     sample = (f"oracle pack+unpack of {layers} of {cfg.L} layers of 1 request ({nbytes / 2**20:.0f} MiB FP16 KV), "
