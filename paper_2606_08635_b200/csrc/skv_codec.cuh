@@ -1,0 +1,187 @@
+// skv_codec.cuh -- device helpers shared by the pack and unpack kernels: streaming loads/stores, the
+// per-vector absmax machinery and the exact fp32 quantise / dequantise steps of include/skv.h.
+#pragma once
+#include "skv_common.cuh"
+
+namespace skv {
+
+__device__ __forceinline__ uint4 ld_stream(const void *p)
+{
+    uint4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ uint2 ld_stream8(const void *p)
+{
+    uint2 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v2.u32 {%0,%1}, [%2];" : "=r"(r.x), "=r"(r.y) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ uint32_t ld_stream4(const void *p)
+{
+    uint32_t r;
+    asm volatile("ld.global.nc.L1::no_allocate.u32 %0, [%1];" : "=r"(r) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ void st_stream(void *p, uint4 v)
+{
+    asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};" :: "l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+__device__ __forceinline__ void st_stream(void *p, uint2 v)
+{
+    asm volatile("st.global.L1::no_allocate.v2.u32 [%0], {%1,%2};" :: "l"(p), "r"(v.x), "r"(v.y) : "memory");
+}
+__device__ __forceinline__ void st_stream(void *p, uint32_t v)
+{
+    asm volatile("st.global.L1::no_allocate.u32 [%0], %1;" :: "l"(p), "r"(v) : "memory");
+}
+
+__device__ __forceinline__ uint32_t h2u(__half2 h) { return *reinterpret_cast<uint32_t *>(&h); }
+__device__ __forceinline__ __half2 u2h(uint32_t u) { return *reinterpret_cast<__half2 *>(&u); }
+
+// |x| max of the 8 halves in a uint4 as one half
+__device__ __forceinline__ __half absmax8_scalar(const uint4 &v)
+{
+    const __half2 m = __hmax2(__hmax2(__habs2(u2h(v.x)), __habs2(u2h(v.y))), __hmax2(__habs2(u2h(v.z)), __habs2(u2h(v.w))));
+    return __hmax(__low2half(m), __high2half(m));
+}
+
+// round-half-even of fl32(x*inv) via the 1.5*2^23 magic constant: the low bits of the sum's encoding are
+// the two's-complement integer (|x*inv| <= qmax*(1+2^-23) << 2^22, so the clamp of the spec is a no-op).
+__device__ __forceinline__ uint32_t rne_code_bits(float x, float inv)
+{
+    return __float_as_uint(__fadd_rn(__fmul_rn(x, inv), 12582912.0f));
+}
+
+__device__ __forceinline__ uint32_t pack4_bytes(uint32_t a, uint32_t b, uint32_t c, uint32_t d)
+{
+    const uint32_t ab = __byte_perm(a, b, 0x0040);    // [a.b0, b.b0, -, -]
+    const uint32_t cd = __byte_perm(c, d, 0x0040);
+    return __byte_perm(ab, cd, 0x5410);               // [a.b0, b.b0, c.b0, d.b0]
+}
+
+// 8 fp16 -> 8 INT8 codes (two words)
+__device__ __forceinline__ uint2 quant8_int8(const uint4 &v, float inv)
+{
+    const float2 a = __half22float2(u2h(v.x)), b = __half22float2(u2h(v.y));
+    const float2 c = __half22float2(u2h(v.z)), d = __half22float2(u2h(v.w));
+    return make_uint2(pack4_bytes(rne_code_bits(a.x, inv), rne_code_bits(a.y, inv), rne_code_bits(b.x, inv), rne_code_bits(b.y, inv)),
+                      pack4_bytes(rne_code_bits(c.x, inv), rne_code_bits(c.y, inv), rne_code_bits(d.x, inv), rne_code_bits(d.y, inv)));
+}
+
+// 8 fp16 -> 8 INT4 codes (one word; element 2k in the low nibble of byte k)
+__device__ __forceinline__ uint32_t quant8_int4(const uint4 &v, float inv)
+{
+    const float2 a = __half22float2(u2h(v.x)), b = __half22float2(u2h(v.y));
+    const float2 c = __half22float2(u2h(v.z)), d = __half22float2(u2h(v.w));
+    const uint32_t b0 = (rne_code_bits(a.x, inv) & 0xFu) | (rne_code_bits(a.y, inv) << 4);
+    const uint32_t b1 = (rne_code_bits(b.x, inv) & 0xFu) | (rne_code_bits(b.y, inv) << 4);
+    const uint32_t b2 = (rne_code_bits(c.x, inv) & 0xFu) | (rne_code_bits(c.y, inv) << 4);
+    const uint32_t b3 = (rne_code_bits(d.x, inv) & 0xFu) | (rne_code_bits(d.y, inv) << 4);
+    return pack4_bytes(b0, b1, b2, b3);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Transposed group reduction.  A head vector spans LPV lanes; a warp holds NCH chunks (K and V amax of a
+// chunk packed in one half2).  Instead of NCH full butterflies, the first log2(NCH) steps halve the set
+// of chunks a lane keeps, so the whole reduction costs NCH-1 + log2(LPV/NCH) shuffles.  Afterwards lane
+// holds the reduced value of chunk held_chunk(lane); src_lane(lane, u) is a lane that holds chunk u.
+// ------------------------------------------------------------------------------------------------
+template <int LPV, int NCH>
+__device__ __forceinline__ int held_chunk(uint32_t lane)
+{
+    if (NCH == 4) return (int)(((lane / (LPV / 2)) & 1) * 2 + ((lane / (LPV / 4)) & 1));
+    if (NCH == 2) return (int)((lane / (LPV / 2)) & 1);
+    return 0;
+}
+template <int LPV, int NCH>
+__device__ __forceinline__ int src_lane(uint32_t lane, int u)
+{
+    const int base = (int)(lane & ~(uint32_t)(LPV - 1));
+    if (NCH == 4) return base + (u >> 1) * (LPV / 2) + (u & 1) * (LPV / 4);
+    if (NCH == 2) return base + u * (LPV / 2);
+    return base;
+}
+template <int LPV, int NCH>
+__device__ __forceinline__ __half2 group_absmax(__half2 (&m)[NCH], uint32_t lane)
+{
+    __half2 v;
+    int o = LPV / 2;
+    if (NCH == 4) {
+        const bool hi = (lane / (LPV / 2)) & 1;
+        const __half2 keep0 = hi ? m[2] : m[0], keep1 = hi ? m[3] : m[1];
+        const __half2 send0 = hi ? m[0] : m[2], send1 = hi ? m[1] : m[3];
+        const __half2 k0 = __hmax2(keep0, u2h(__shfl_xor_sync(0xffffffffu, h2u(send0), LPV / 2)));
+        const __half2 k1 = __hmax2(keep1, u2h(__shfl_xor_sync(0xffffffffu, h2u(send1), LPV / 2)));
+        const bool hi2 = (lane / (LPV / 4)) & 1;
+        const __half2 keep = hi2 ? k1 : k0, send = hi2 ? k0 : k1;
+        v = __hmax2(keep, u2h(__shfl_xor_sync(0xffffffffu, h2u(send), LPV / 4)));
+        o = LPV / 8;
+    } else if (NCH == 2) {
+        const bool hi = (lane / (LPV / 2)) & 1;
+        const __half2 keep = hi ? m[1] : m[0], send = hi ? m[0] : m[1];
+        v = __hmax2(keep, u2h(__shfl_xor_sync(0xffffffffu, h2u(send), LPV / 2)));
+        o = LPV / 4;
+    } else {
+        v = m[0];
+    }
+#pragma unroll
+    for (; o >= 1; o >>= 1) v = __hmax2(v, u2h(__shfl_xor_sync(0xffffffffu, h2u(v), o)));
+    return v;
+}
+
+// ------------------------------------------------------------------------------------------------
+// dequantise: biased bytes -> f16_rn(fl32(float(q) * scale)); int->float through the 2^23 exponent trick
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t h2_bits(float a, float b) { return h2u(__floats2half2_rn(a, b)); }
+
+template <int BIAS>
+__device__ __forceinline__ void dequant4(uint32_t w, float scale, uint32_t &o0, uint32_t &o1)
+{
+    constexpr float kOff = 8388608.0f + (float)BIAS;                  // 2^23 + BIAS, exact
+    const float f0 = __fsub_rn(__uint_as_float(__byte_perm(w, 0x4B000000u, 0x7540)), kOff);
+    const float f1 = __fsub_rn(__uint_as_float(__byte_perm(w, 0x4B000000u, 0x7541)), kOff);
+    const float f2 = __fsub_rn(__uint_as_float(__byte_perm(w, 0x4B000000u, 0x7542)), kOff);
+    const float f3 = __fsub_rn(__uint_as_float(__byte_perm(w, 0x4B000000u, 0x7543)), kOff);
+    o0 = h2_bits(__fmul_rn(f0, scale), __fmul_rn(f1, scale));
+    o1 = h2_bits(__fmul_rn(f2, scale), __fmul_rn(f3, scale));
+}
+__device__ __forceinline__ uint4 dequant_int8(uint2 w, float scale)
+{
+    uint4 o;
+    dequant4<128>(w.x ^ 0x80808080u, scale, o.x, o.y);
+    dequant4<128>(w.y ^ 0x80808080u, scale, o.z, o.w);
+    return o;
+}
+__device__ __forceinline__ uint4 dequant_int4(uint32_t w, float scale)
+{
+    w ^= 0x88888888u;                                   // every nibble becomes q+8
+    const uint32_t even = w & 0x0F0F0F0Fu;              // elements 0,2,4,6
+    const uint32_t odd = (w >> 4) & 0x0F0F0F0Fu;        // elements 1,3,5,7
+    constexpr float kOff = 8388608.0f + 8.0f;
+    float f[8];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        f[2 * k] = __fsub_rn(__uint_as_float(__byte_perm(even, 0x4B000000u, 0x7540 + k)), kOff);
+        f[2 * k + 1] = __fsub_rn(__uint_as_float(__byte_perm(odd, 0x4B000000u, 0x7540 + k)), kOff);
+    }
+    uint4 o;
+    o.x = h2_bits(__fmul_rn(f[0], scale), __fmul_rn(f[1], scale));
+    o.y = h2_bits(__fmul_rn(f[2], scale), __fmul_rn(f[3], scale));
+    o.z = h2_bits(__fmul_rn(f[4], scale), __fmul_rn(f[5], scale));
+    o.w = h2_bits(__fmul_rn(f[6], scale), __fmul_rn(f[7], scale));
+    return o;
+}
+__device__ __forceinline__ float scale_of(__half amax, float qmax)
+{
+    const float af = __half2float(amax);
+    return af != 0.0f ? __fdiv_rn(af, qmax) : 0.0f;
+}
+__device__ __forceinline__ float inv_of(__half amax, float qmax)
+{
+    const float af = __half2float(amax);
+    return af != 0.0f ? __fdiv_rn(qmax, af) : 0.0f;
+}
+
+}  // namespace skv

@@ -7,29 +7,9 @@
 // ballot).  All lanes of a warp share one tier => no divergence.  Dropped tokens are never loaded.
 //
 // HBM-bound: reads Bytes_FP16, writes beta*Bytes_FP16.
-#include "skv_common.cuh"
+#include "skv_codec.cuh"
 
 namespace skv {
-
-__device__ __forceinline__ uint4 ld_stream(const void *p)
-{
-    uint4 r;
-    asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
-                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
-    return r;
-}
-__device__ __forceinline__ void st_stream(void *p, uint4 v)
-{
-    asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};" :: "l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
-}
-__device__ __forceinline__ void st_stream(void *p, uint2 v)
-{
-    asm volatile("st.global.L1::no_allocate.v2.u32 [%0], {%1,%2};" :: "l"(p), "r"(v.x), "r"(v.y) : "memory");
-}
-__device__ __forceinline__ void st_stream(void *p, uint32_t v)
-{
-    asm volatile("st.global.L1::no_allocate.u32 [%0], %1;" :: "l"(p), "r"(v) : "memory");
-}
 
 // |x| max of the 8 halves in a uint4, as a half2 with the max in both halves' union (max(lo,hi) taken later)
 __device__ __forceinline__ __half2 absmax8(const uint4 &v)
@@ -39,13 +19,6 @@ __device__ __forceinline__ __half2 absmax8(const uint4 &v)
     const __half2 c = __habs2(*reinterpret_cast<const __half2 *>(&v.z));
     const __half2 d = __habs2(*reinterpret_cast<const __half2 *>(&v.w));
     return __hmax2(__hmax2(a, b), __hmax2(c, d));
-}
-
-// round-half-even of fl32(x*inv) via the 1.5*2^23 magic constant: the low bits of the sum's encoding are
-// the two's-complement integer (|x*inv| <= qmax*(1+2^-23) << 2^22, so the clamp of the spec is a no-op).
-__device__ __forceinline__ uint32_t rne_code_bits(float x, float inv)
-{
-    return __float_as_uint(__fadd_rn(__fmul_rn(x, inv), 12582912.0f));
 }
 
 template <int D, int QMAX>
@@ -70,13 +43,6 @@ __device__ __forceinline__ void quantize_chunk(const uint4 &v, uint32_t lane, __
     }
     amax_out = amax;
     (void)lane;
-}
-
-__device__ __forceinline__ uint32_t pack4_bytes(uint32_t a, uint32_t b, uint32_t c, uint32_t d)
-{
-    const uint32_t ab = __byte_perm(a, b, 0x0040);    // [a.b0, b.b0, -, -]
-    const uint32_t cd = __byte_perm(c, d, 0x0040);
-    return __byte_perm(ab, cd, 0x5410);               // [a.b0, b.b0, c.b0, d.b0]
 }
 
 template <int D>
@@ -210,17 +176,141 @@ pack_kernel(Geom g, Layout lo, const __half *__restrict__ K, const __half *__res
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Fast path: the token row is a whole number of NCH-chunk batches (row_elems % (256*NCH) == 0).
+// Fully unrolled; the K and V absmax of the NCH chunks are reduced together by the transposed group
+// reduction (skv_codec.cuh): NCH-1+log2(LPV/NCH) shuffles and TWO divisions per lane per batch instead
+// of 2*NCH*log2(LPV) shuffles and 2*NCH divisions; the reciprocals are then broadcast with 2*NCH shuffles.
+// ------------------------------------------------------------------------------------------------
+template <int D, int NCH, int MINB>
+__global__ void __launch_bounds__(256, MINB)
+pack_fast_kernel(Geom g, Layout lo, const __half *__restrict__ K, const __half *__restrict__ V,
+                 const uint8_t *__restrict__ tier_map, uint8_t *__restrict__ blob, uint64_t blob_stride,
+                 const uint4 *__restrict__ tile_base)
+{
+    constexpr int LPV = D / 8;                 // lanes per head vector
+    constexpr int HPC = 256 / D;               // head vectors per 256-element chunk
+    const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t tile = blockIdx.x;
+    const int l = blockIdx.y, r = blockIdx.z;
+    const int64_t n = g.n;
+    const int64_t j0 = tile * kTileTokens;
+
+    const uint8_t *tm = tier_map + ((int64_t)r * g.L + l) * n;
+    const uint32_t my_t = (j0 + lane < n) ? (uint32_t)tm[j0 + lane] : 0xFFu;
+    const uint32_t m16 = __ballot_sync(0xffffffffu, my_t == 16u);
+    const uint32_t m8 = __ballot_sync(0xffffffffu, my_t == 8u);
+    const uint32_t m4 = __ballot_sync(0xffffffffu, my_t == 4u);
+    const uint4 base = tile_base[((int64_t)r * g.L + l) * g.tiles + tile];
+
+    uint8_t *lbase = blob + (uint64_t)r * blob_stride + lo.layer0_off + (uint64_t)l * lo.layer_stride;
+    const int row_elems = g.Hkv * D;
+    const __half *Kb = K + (int64_t)r * g.sr + (int64_t)l * g.sl;
+    const __half *Vb = V + (int64_t)r * g.sr + (int64_t)l * g.sl;
+    const int lane_h = (int)(lane * 8) / D, lane_c = (int)(lane * 8) % D;
+    const int my_chunk = held_chunk<LPV, NCH>(lane);
+    const bool scale_writer = (lane % (LPV / NCH)) == 0;
+
+    for (uint32_t i = warp; i < (uint32_t)kTileTokens; i += 8) {
+        const uint32_t t = __shfl_sync(0xffffffffu, my_t, i);
+        if (t != 16u && t != 8u && t != 4u) continue;                 // dropped / tail / invalid: no bytes
+        const uint32_t below = (1u << i) - 1u;
+        const int64_t j = j0 + i;
+        const __half *krow = Kb + j * g.st + lane_c;
+        const __half *vrow = Vb + j * g.st + lane_c;
+        const uint32_t slot = (t == 16u) ? base.x + __popc(m16 & below)
+                            : (t == 8u)  ? base.y + __popc(m8 & below) : base.z + __popc(m4 & below);
+        const uint32_t cap = (t == 16u) ? (uint32_t)g.n16 : (t == 8u) ? (uint32_t)g.n8 : (uint32_t)g.n4;
+        if (slot >= cap) continue;                                    // foreign map that disagrees with counts
+
+        for (int cb = 0; cb < g.row_chunks; cb += NCH) {
+            uint4 kv[NCH], vv[NCH];
+#pragma unroll
+            for (int u = 0; u < NCH; ++u) {
+                const int64_t off = (int64_t)((cb + u) * HPC + lane_h) * g.sh;
+                kv[u] = ld_stream(krow + off);
+                vv[u] = ld_stream(vrow + off);
+            }
+            if (t == 16u) {
+                uint8_t *kd = lbase + lo.seg_off[0] + ((uint64_t)slot * row_elems + cb * 256 + lane * 8) * 2;
+                uint8_t *vd = lbase + lo.seg_off[1] + ((uint64_t)slot * row_elems + cb * 256 + lane * 8) * 2;
+#pragma unroll
+                for (int u = 0; u < NCH; ++u) { st_stream(kd + u * 512, kv[u]); st_stream(vd + u * 512, vv[u]); }
+                continue;
+            }
+            __half2 m[NCH];
+#pragma unroll
+            for (int u = 0; u < NCH; ++u) m[u] = __halves2half2(absmax8_scalar(kv[u]), absmax8_scalar(vv[u]));
+            const __half2 a2 = group_absmax<LPV, NCH>(m, lane);      // (K amax, V amax) of chunk cb + my_chunk
+            const bool is8 = (t == 8u);
+            const float qmax = is8 ? 127.0f : 7.0f;
+            const float invK = inv_of(__low2half(a2), qmax), invV = inv_of(__high2half(a2), qmax);
+            if (scale_writer) {
+                const int head = (cb + my_chunk) * HPC + (int)(lane / LPV);
+                __half *ks = reinterpret_cast<__half *>(lbase + lo.seg_off[is8 ? 6 : 8]) + (uint64_t)slot * g.Hkv;
+                __half *vs = reinterpret_cast<__half *>(lbase + lo.seg_off[is8 ? 7 : 9]) + (uint64_t)slot * g.Hkv;
+                ks[head] = __low2half(a2);
+                vs[head] = __high2half(a2);
+            }
+            if (is8) {
+                uint8_t *kd = lbase + lo.seg_off[2] + (uint64_t)slot * row_elems + cb * 256 + lane * 8;
+                uint8_t *vd = lbase + lo.seg_off[3] + (uint64_t)slot * row_elems + cb * 256 + lane * 8;
+#pragma unroll
+                for (int u = 0; u < NCH; ++u) {
+                    const int src = src_lane<LPV, NCH>(lane, u);
+                    const float ik = __shfl_sync(0xffffffffu, invK, src), iv = __shfl_sync(0xffffffffu, invV, src);
+                    st_stream(kd + u * 256, quant8_int8(kv[u], ik));
+                    st_stream(vd + u * 256, quant8_int8(vv[u], iv));
+                }
+            } else {
+                uint8_t *kd = lbase + lo.seg_off[4] + (uint64_t)slot * (row_elems / 2) + cb * 128 + lane * 4;
+                uint8_t *vd = lbase + lo.seg_off[5] + (uint64_t)slot * (row_elems / 2) + cb * 128 + lane * 4;
+#pragma unroll
+                for (int u = 0; u < NCH; ++u) {
+                    const int src = src_lane<LPV, NCH>(lane, u);
+                    const float ik = __shfl_sync(0xffffffffu, invK, src), iv = __shfl_sync(0xffffffffu, invV, src);
+                    st_stream(kd + u * 128, quant8_int4(kv[u], ik));
+                    st_stream(vd + u * 128, quant8_int4(vv[u], iv));
+                }
+            }
+        }
+    }
+}
+
+template <int D, int NCH>
+static cudaError_t launch_pack_fast(const Geom &g, const Layout &lo, const __half *K, const __half *V,
+                                    const uint8_t *tier_map, uint8_t *blob, uint64_t blob_stride,
+                                    const uint4 *tile_base, cudaStream_t s)
+{
+    dim3 grid(g.tiles, g.L, g.R);
+    pack_fast_kernel<D, NCH, 3><<<grid, 256, 0, s>>>(g, lo, K, V, tier_map, blob, blob_stride, tile_base);
+    return cudaGetLastError();
+}
+
+template <int D>
+static cudaError_t launch_pack_d(const Geom &g, const Layout &lo, const __half *K, const __half *V,
+                                 const uint8_t *tier_map, uint8_t *blob, uint64_t blob_stride,
+                                 const uint4 *tile_base, cudaStream_t s)
+{
+    if ((g.Hkv * D) % 256 == 0) {
+        if (g.row_chunks % 4 == 0) return launch_pack_fast<D, 4>(g, lo, K, V, tier_map, blob, blob_stride, tile_base, s);
+        if (g.row_chunks % 2 == 0) return launch_pack_fast<D, 2>(g, lo, K, V, tier_map, blob, blob_stride, tile_base, s);
+        return launch_pack_fast<D, 1>(g, lo, K, V, tier_map, blob, blob_stride, tile_base, s);
+    }
+    dim3 grid(g.tiles, g.L, g.R);
+    pack_kernel<D><<<grid, 256, 0, s>>>(g, lo, K, V, tier_map, blob, blob_stride, tile_base);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_pack(const Geom &g, const Layout &lo, const __half *K, const __half *V, const uint8_t *tier_map,
                         uint8_t *blob, uint64_t blob_stride, const uint4 *tile_base, cudaStream_t s)
 {
-    dim3 grid(g.tiles, g.L, g.R);
     switch (g.D) {
-    case 64:  pack_kernel<64><<<grid, 256, 0, s>>>(g, lo, K, V, tier_map, blob, blob_stride, tile_base); break;
-    case 128: pack_kernel<128><<<grid, 256, 0, s>>>(g, lo, K, V, tier_map, blob, blob_stride, tile_base); break;
-    case 256: pack_kernel<256><<<grid, 256, 0, s>>>(g, lo, K, V, tier_map, blob, blob_stride, tile_base); break;
+    case 64:  return launch_pack_d<64>(g, lo, K, V, tier_map, blob, blob_stride, tile_base, s);
+    case 128: return launch_pack_d<128>(g, lo, K, V, tier_map, blob, blob_stride, tile_base, s);
+    case 256: return launch_pack_d<256>(g, lo, K, V, tier_map, blob, blob_stride, tile_base, s);
     default: return cudaErrorInvalidValue;
     }
-    return cudaGetLastError();
 }
 
 }  // namespace skv

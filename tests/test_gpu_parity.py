@@ -65,7 +65,7 @@ def test_c5_shaped_two_requests_b_sweep(b):
 
 
 @pytest.mark.parametrize("n", [250, 257, 1000, 4097, 31, 33])
-@pytest.mark.parametrize("d,Hkv,Hq", [(128, 2, 4), (64, 3, 3), (256, 1, 2)])
+@pytest.mark.parametrize("d,Hkv,Hq", [(128, 2, 4), (64, 3, 3), (256, 1, 2), (64, 8, 8), (64, 16, 16), (256, 2, 2)])
 def test_ragged_token_counts_and_head_dims(n, d, Hkv, Hq):
     cfg = skv_synth.Config("ragged", L=2, Hq=Hq, Hkv=Hkv, d=d, n=n, w=min(8, n), R=1, k_dist="outlier",
                            n_sink=2, ranges=((n - 5, n - 1),), seed=n + d)
