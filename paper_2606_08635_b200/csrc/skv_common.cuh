@@ -52,6 +52,9 @@ cudaError_t launch_assign(const Geom &g, const Intervals &prot, const float *imp
 cudaError_t launch_importance(const Geom &g, const __half *K, const __half *Q, int window, int causal, float lambda,
                               float *importance, void *ws, size_t ws_bytes, cudaStream_t s);
 size_t importance_ws_bytes(const Geom &g, int window);
+cudaError_t launch_importance_tc(const Geom &g, const __half *K, const __half *Q, int window, int causal, float lambda,
+                                 float *importance, void *ws, cudaStream_t s);
+size_t importance_tc_ws_bytes(const Geom &g, int window);
 cudaError_t launch_importance_kvnorm(const Geom &g, const __half *K, float lambda, float *importance, float *ws,
                                      cudaStream_t s);
 

@@ -12,6 +12,10 @@
 //                      no atomics), scaled by 1/(Hq*w) and the recency decay.
 // fp16 operands, fp32 accumulation (mma.sync.m16n8k16), operands staged in XOR-swizzled shared memory by
 // cp.async and fetched with ldmatrix.
+#include <stdlib.h>
+
+#include <algorithm>
+
 #include "skv_common.cuh"
 
 namespace skv {
@@ -357,7 +361,8 @@ size_t importance_ws_bytes(const Geom &g, int window)
     const size_t rows = (size_t)g.R * g.L * g.Hq * window;
     const size_t a = rows * nc * sizeof(float2) + rows * sizeof(float) + 256;
     const size_t b = (size_t)g.R * g.L * g.n * sizeof(float);
-    return a > b ? a : b;
+    const size_t c = importance_tc_ws_bytes(g, window);
+    return std::max(a, std::max(b, c));
 }
 
 template <int D>
@@ -393,6 +398,13 @@ static cudaError_t launch_importance_t(const Geom &g, const __half *K, const __h
 cudaError_t launch_importance(const Geom &g, const __half *K, const __half *Q, int window, int causal, float lambda,
                               float *importance, void *ws, size_t, cudaStream_t s)
 {
+    // tcgen05 / TMEM / TMA path (skv_importance_tc.cu).  The mma.sync kernels below remain as the fallback for
+    // drivers that cannot build the tensor maps, and for A/B comparison (SKV_IMPORTANCE=mma).
+    const char *sel = getenv("SKV_IMPORTANCE");
+    if (!(sel && sel[0] == 'm')) {
+        const cudaError_t e = launch_importance_tc(g, K, Q, window, causal, lambda, importance, ws, s);
+        if (e != cudaErrorNotSupported) return e;
+    }
     switch (g.D) {
     case 64:  return launch_importance_t<64>(g, K, Q, window, causal, lambda, importance, ws, s);
     case 128: return launch_importance_t<128>(g, K, Q, window, causal, lambda, importance, ws, s);
