@@ -4,7 +4,7 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl skv|reference] [--workload C5] [--budget 0.5]
 
 A "step" is one pass of the whole hot path over one batch of synthetic requests:
-    skv_importance -> skv_assign_tiers -> skv_pack -> skv_unpack      (8 kernel launches)
+    skv_importance -> skv_assign_tiers -> skv_pack -> skv_unpack      (9 kernel launches)
 `value` = FP16 KV bytes of the batch / (time in skv_pack + skv_unpack), inputs resident in HBM, timed with CUDA
 events on the launching stream.  `e2e` = the same bytes / the time of the whole path driven from pinned HOST
 buffers (H2D of K,V,Q; the pinned-host D2H+H2D hop of the blob that stands in for the network; D2H of the
@@ -33,7 +33,7 @@ FALLBACK_HBM_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallba
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="skv", choices=["skv", "reference"])
     ap.add_argument("--workload", default="C5")
@@ -52,6 +52,22 @@ def measured_peak():
             return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
     except Exception:
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic(workload, b, R, kernel):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` ("pack" | "unpack"), as captured by
+    `ncu --set full` and recorded in profiles/r1_traffic.csv (workload,budget,n_requests,kernel,dram_bytes);
+    None when no capture of this exact workload is on file."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "r1_traffic.csv")) as f:
+            for ln in f:
+                fld = [x.strip() for x in ln.split(",")]
+                if len(fld) >= 5 and fld[0] == workload and fld[3] == kernel:
+                    if abs(float(fld[1]) - b) < 1e-9 and int(fld[2]) == R:
+                        return float(fld[4])
+    except Exception:
+        pass
+    return None
 
 
 def config_json(cfg, b, R, extra=None):
@@ -79,7 +95,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
@@ -88,9 +104,15 @@ class ClockSampler:
 
     def _read(self):
         for line in self.proc.stdout:
-            self.lines.append(line.strip())
+            self.lines.append((time.time(), line.strip()))
 
-    def stop(self):
+    def wait_first_sample(self, timeout=5.0):
+        t_end = time.time() + timeout
+        while self.proc and not self.lines and time.time() < t_end:
+            time.sleep(0.01)
+
+    def stop(self, t0=None, t1=None):
+        """Summary of the samples that arrived in [t0, t1] (the timed region; all samples if none did)."""
         if not self.proc:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         time.sleep(0.15)
@@ -101,7 +123,8 @@ class ClockSampler:
             self.proc.kill()
         sm, mx, reasons, pw = [], [], set(), []
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for ln in self.lines:
+        inside = [ln for (t, ln) in self.lines if t0 is not None and t0 <= t <= t1 + 0.05]
+        for ln in (inside or [ln for (_, ln) in self.lines]):
             f = [x.strip() for x in ln.split(",")]
             if len(f) < 8:
                 continue
@@ -114,7 +137,8 @@ class ClockSampler:
                     reasons.add(name)
         sm.sort()
         return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "samples_in_timed_region": len(inside),
+                "reasons": sorted(reasons)}
 
 
 # ----------------------------------------------------------------------------------------------------
@@ -146,6 +170,12 @@ def aggregate_over_ranks(ms_local, bytes_local, device="cpu"):
     return [float(x) for x in t.tolist()], float(b.item())
 
 
+def rank_request_ids(rank, R):
+    """Requests are independent: rank k owns the global request ids [k*R, (k+1)*R) -- its own
+    seeds, its own blobs, no exchange with any other rank."""
+    return list(range(rank * R, (rank + 1) * R))
+
+
 def barrier():
     import torch.distributed as dist
     if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
@@ -156,7 +186,7 @@ def barrier():
 # the CUDA arm
 # ----------------------------------------------------------------------------------------------------
 STAGES = ("importance", "assign", "pack", "unpack")
-LAUNCHES_PER_STEP = 3 + 1 + 2 + 2     # rowstats, combine, colsum | assign | tile_scan, pack | tile_scan, unpack
+LAUNCHES_PER_STEP = 4 + 1 + 2 + 2     # imp_tc<1>, combine, imp_tc<2>, finish | assign | tile_scan, pack | tile_scan, unpack
 
 
 class DeviceProblem:
@@ -169,9 +199,9 @@ class DeviceProblem:
         self.K = torch.empty((R, L, cfg.n, cfg.Hkv, cfg.d), dtype=torch.float16, device=dev)
         self.V = torch.empty_like(self.K)
         self.Q = torch.empty((R, L, cfg.Hq, cfg.w, cfg.d), dtype=torch.float16, device=dev)
-        for r in range(R):
-            self.K[r], self.V[r] = skv_synth.make_kv(cfg, r + rank * R, device=dev)
-            self.Q[r] = skv_synth.make_q(cfg, r + rank * R, device=dev)
+        for r, rid in enumerate(rank_request_ids(rank, R)):
+            self.K[r], self.V[r] = skv_synth.make_kv(cfg, rid, device=dev)
+            self.Q[r] = skv_synth.make_q(cfg, rid, device=dev)
         self.shape = skv.make_shape(L, cfg.Hq, cfg.Hkv, cfg.d, cfg.n, R)
         self.policy = skv.make_policy(b, cfg.n_sink, cfg.ranges, cfg.allow_int4)
         self.counts = skv.skv_tier_counts(self.shape, self.policy)
@@ -369,13 +399,15 @@ def main():
     barrier()
     torch.cuda.synchronize()
     sampler.start()
+    sampler.wait_first_sample()
     t_wall0 = time.perf_counter()
+    t_abs0 = time.time()
     for k in range(K):
         prob.step(ev[k])
     torch.cuda.synchronize()
     barrier()
     t_wall = time.perf_counter() - t_wall0
-    clocks = sampler.stop()
+    clocks = sampler.stop(t_abs0, time.time())
 
     total_ms = ev[0][0].elapsed_time(ev[K - 1][4])
     stage_ms = [sum(ev[k][i].elapsed_time(ev[k][i + 1]) for k in range(K)) / K for i in range(4)]
@@ -402,14 +434,7 @@ def main():
     dom = "pack" if ms_pack >= ms_unpack else "unpack"
     dom_ms = max(ms_pack, ms_unpack)
     achieved = alg[dom] / (dom_ms * 1e-3) / 1e9
-    traffic = None
-    try:
-        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            tj = json.load(f)
-        if tj.get("workload") == args.workload and abs(tj.get("budget", -1) - b) < 1e-9 and tj.get("n_requests") == R:
-            traffic = tj.get(dom + "_kernel_dram_bytes")
-    except Exception:
-        pass
+    traffic = ncu_traffic(args.workload, b, R, dom)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
