@@ -41,6 +41,8 @@ def parse_args():
     ap.add_argument("--requests", type=int, default=None)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--e2e-chunk-layers", type=int, default=4, help="layers per pipelined transfer chunk")
+    ap.add_argument("--e2e-depth", type=int, default=3, help="device slots of the pipelined transfer")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
     return ap.parse_args()
 
@@ -235,17 +237,17 @@ class DeviceProblem:
         return {"pack": fp16 + blob + tm, "unpack": blob + fp16 + tm}
 
 
-def run_e2e(cfg, b, R, dev, steps, warmup):
-    """The whole path driven from pinned HOST buffers, one request at a time through the C ABI (R = 1 shapes):
-    H2D K,V,Q -> importance -> assign -> pack -> D2H blob -> skv_blob_check (host) -> H2D blob -> unpack -> D2H K,V."""
+def run_e2e(cfg, b, R, dev, steps, warmup, chunk_layers=4, depth=3):
+    """The whole path driven from pinned HOST buffers through the public API (paper_2606_08635_b200.transfer.
+    LayerPipelinedTransfer: per layer chunk  H2D K,V,Q -> importance -> assign -> pack -> D2H blob -> skv_blob_check
+    (host) -> H2D blob -> unpack -> D2H K,V,  chunks overlapped on three streams).  Also times, once each for
+    context, the same path with no overlap (one request at a time on one stream) and the bare hop of one request
+    (raw FP16 K,V vs the SKV1 blob, D2H + H2D)."""
     import torch
     import paper_2606_08635_b200 as skv
+    from paper_2606_08635_b200.transfer import LayerPipelinedTransfer
     import skv_synth
     L = cfg.L
-    shape = skv.make_shape(L, cfg.Hq, cfg.Hkv, cfg.d, cfg.n, 1)
-    policy = skv.make_policy(b, cfg.n_sink, cfg.ranges, cfg.allow_int4)
-    counts = skv.skv_tier_counts(shape, policy)
-    bb = skv.skv_blob_bytes(shape, counts)
     pin = dict(pin_memory=True)
     hK = torch.empty((R, L, cfg.n, cfg.Hkv, cfg.d), dtype=torch.float16, **pin)
     hV = torch.empty_like(hK, **pin)
@@ -254,9 +256,33 @@ def run_e2e(cfg, b, R, dev, steps, warmup):
         k, v = skv_synth.make_kv(cfg, r, device=dev)
         hK[r].copy_(k); hV[r].copy_(v); hQ[r].copy_(skv_synth.make_q(cfg, r, device=dev))
         del k, v
-    h_blob = torch.empty((bb,), dtype=torch.uint8, **pin)
-    hKo = torch.empty((L, cfg.n, cfg.Hkv, cfg.d), dtype=torch.float16, **pin)
+    hKo = torch.empty((min(R, 2), L, cfg.n, cfg.Hkv, cfg.d), dtype=torch.float16, **pin)    # 2-request output ring
     hVo = torch.empty_like(hKo, **pin)
+    lpc = max(1, min(L, chunk_layers))
+    pipe = LayerPipelinedTransfer(L, cfg.Hq, cfg.Hkv, cfg.d, cfg.n, cfg.w, b, cfg.n_sink, cfg.ranges, cfg.allow_int4,
+                                  layers_per_chunk=lpc, depth=depth, device=dev)
+    torch.cuda.synchronize()
+    for _ in range(warmup):
+        pipe.run(hK, hV, hQ, hKo, hVo)
+    barrier()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        pipe.run(hK, hV, hQ, hKo, hVo)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    h2d_req, d2h_req = pipe.bytes_per_request()
+    out = {"ms_per_step": ms, "steps": steps, "h2d": R * h2d_req, "d2h": R * d2h_req, "layers_per_chunk": lpc, "depth": depth}
+    del pipe
+
+    # context 1: no overlap -- one request at a time, one stream, whole-request blobs
+    shape = skv.make_shape(L, cfg.Hq, cfg.Hkv, cfg.d, cfg.n, 1)
+    policy = skv.make_policy(b, cfg.n_sink, cfg.ranges, cfg.allow_int4)
+    counts = skv.skv_tier_counts(shape, policy)
+    bb = skv.skv_blob_bytes(shape, counts)
+    h_blob = torch.empty((bb,), dtype=torch.uint8, **pin)
     dK = torch.empty((L, cfg.n, cfg.Hkv, cfg.d), dtype=torch.float16, device=dev)
     dV, dKo, dVo = torch.empty_like(dK), torch.empty_like(dK), torch.empty_like(dK)
     dQ = torch.empty((L, cfg.Hq, cfg.w, cfg.d), dtype=torch.float16, device=dev)
@@ -264,49 +290,39 @@ def run_e2e(cfg, b, R, dev, steps, warmup):
     dT = torch.empty((L, cfg.n), dtype=torch.uint8, device=dev)
     d_blob, d_blob2 = torch.empty((bb,), dtype=torch.uint8, device=dev), torch.empty((bb,), dtype=torch.uint8, device=dev)
     ws = torch.empty(skv.skv_workspace_bytes(shape, cfg.w), dtype=torch.uint8, device=dev)
-    torch.cuda.synchronize()
 
-    def one_step():
-        for r in range(R):
-            dK.copy_(hK[r], non_blocking=True); dV.copy_(hV[r], non_blocking=True); dQ.copy_(hQ[r], non_blocking=True)
-            skv.skv_importance(shape, dK, dQ, cfg.w, dI, ws)
-            c = skv.skv_assign_tiers(shape, policy, dI, dT, ws)
-            skv.skv_pack(shape, dK, dV, dT, c, d_blob, ws)
-            h_blob.copy_(d_blob, non_blocking=True)               # the hop, prefill side
-            torch.cuda.current_stream().synchronize()             # blob has "arrived" at the decode side
-            _, hc = skv.skv_blob_check(h_blob, bb)
-            d_blob2.copy_(h_blob, non_blocking=True)              # the hop, decode side
-            skv.skv_unpack(shape, d_blob2, bb, hc, dKo, dVo, None, ws)
-            hKo.copy_(dKo, non_blocking=True); hVo.copy_(dVo, non_blocking=True)
+    def sequential_request(r):
+        dK.copy_(hK[r], non_blocking=True); dV.copy_(hV[r], non_blocking=True); dQ.copy_(hQ[r], non_blocking=True)
+        skv.skv_importance(shape, dK, dQ, cfg.w, dI, ws)
+        c = skv.skv_assign_tiers(shape, policy, dI, dT, ws)
+        skv.skv_pack(shape, dK, dV, dT, c, d_blob, ws)
+        h_blob.copy_(d_blob, non_blocking=True)
+        torch.cuda.current_stream().synchronize()
+        _, hc = skv.skv_blob_check(h_blob, bb)
+        d_blob2.copy_(h_blob, non_blocking=True)
+        skv.skv_unpack(shape, d_blob2, bb, hc, dKo, dVo, None, ws)
+        hKo[0].copy_(dKo, non_blocking=True); hVo[0].copy_(dVo, non_blocking=True)
         torch.cuda.current_stream().synchronize()
 
-    for _ in range(warmup):
-        one_step()
-    barrier()
-    torch.cuda.synchronize()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for _ in range(steps):
-        one_step()
-    e1.record()
-    torch.cuda.synchronize()
-    ms = e0.elapsed_time(e1) / steps
-    kvq = (hK[0].numel() + hV[0].numel() + hQ[0].numel()) * 2
-    h2d = R * (kvq + bb)
-    d2h = R * (bb + (hKo.numel() + hVo.numel()) * 2)
-    # raw FP16 hop for context: D2H + H2D of one request's K and V (what the paper's full-KV baseline ships)
+    sequential_request(0)
+    s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    s0.record()
+    sequential_request(0)
+    s1.record()
+    # context 2: the bare hop of one request, raw FP16 K,V vs the blob
     r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     r0.record()
-    hKo.copy_(dK, non_blocking=True); hVo.copy_(dV, non_blocking=True)
-    dKo.copy_(hKo, non_blocking=True); dVo.copy_(hVo, non_blocking=True)
+    hKo[0].copy_(dK, non_blocking=True); hVo[0].copy_(dV, non_blocking=True)
+    dKo.copy_(hKo[0], non_blocking=True); dVo.copy_(hVo[0], non_blocking=True)
     r1.record()
     p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     p0.record()
     h_blob.copy_(d_blob, non_blocking=True); d_blob2.copy_(h_blob, non_blocking=True)
     p1.record()
     torch.cuda.synchronize()
-    return {"ms_per_step": ms, "steps": steps, "h2d": h2d, "d2h": d2h,
-            "raw_fp16_hop_ms_per_request": r0.elapsed_time(r1), "blob_hop_ms_per_request": p0.elapsed_time(p1)}
+    out.update({"sequential_ms_per_request": s0.elapsed_time(s1),
+                "raw_fp16_hop_ms_per_request": r0.elapsed_time(r1), "blob_hop_ms_per_request": p0.elapsed_time(p1)})
+    return out
 
 
 # ----------------------------------------------------------------------------------------------------
@@ -419,11 +435,12 @@ def main():
 
     e2e = None
     if not args.no_e2e:
-        r = run_e2e(cfg, b, R, dev, steps=min(K, 3), warmup=1)
+        r = run_e2e(cfg, b, R, dev, steps=min(K, 3), warmup=1, chunk_layers=args.e2e_chunk_layers, depth=args.e2e_depth)
         red2, _ = aggregate_over_ranks([r["ms_per_step"]], bytes_local, device=dev)
         e2e = {"value": bytes_all / (red2[0] * 1e-3) / 1e9, "unit": "GB/s of FP16 KV, whole path from pinned host buffers",
                "h2d_bytes_per_step": r["h2d"], "d2h_bytes_per_step": r["d2h"], "ms_per_step": red2[0], "steps": r["steps"],
-               "ms_per_request": red2[0] / R,
+               "ms_per_request": red2[0] / R, "pipeline": f"layer chunks of {r['layers_per_chunk']}, {r['depth']} slots, 3 streams",
+               "sequential_ms_per_request": r["sequential_ms_per_request"],
                "raw_fp16_hop_ms_per_request": r["raw_fp16_hop_ms_per_request"],
                "blob_hop_ms_per_request": r["blob_hop_ms_per_request"]}
 

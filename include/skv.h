@@ -47,7 +47,8 @@
  * Quantiser (one group = one head vector of d_h values; qmax = 127 / 7):
  *   amax = max|x| (an fp16 value, stored as the 2-byte scale record);
  *   inv = fl32(qmax/amax), scale = fl32(amax/qmax)   (both 0 when amax = 0);
- *   q = clamp(rint(fl32(x*inv)), -qmax, qmax), rint = round half to even;   y = f16_rn(fl32(q*scale)).
+ *   q = clamp(rint(x*inv), -qmax, qmax): the real product of the fp16 x and the fp32 inv, rounded ONCE, half to
+ *   even (a 35-bit product, so no intermediate binary32 rounding);   y = f16_rn(fl32(q*scale)).
  */
 #ifndef SKV_H_
 #define SKV_H_

@@ -284,7 +284,9 @@ static uint64_t get_u64(const uint8_t *p) { uint64_t v = 0; for (int i = 0; i < 
  * One group = one head vector of d fp16 values.  qmax = 127 (INT8) / 7 (INT4).
  * amax = max|x| (an fp16 value, stored losslessly as the 2-byte scale record).
  * inv = fl32(qmax / amax), scale = fl32(amax / qmax) (0 when amax = 0).
- * q = clamp(rint(fl32(x * inv)), -qmax, qmax), rint = round half to even.
+ * q = clamp(rint(x * inv), -qmax, qmax): the product is taken EXACTLY (an fp16 times an fp32 has at most
+ * 11 + 24 = 35 significant bits, so binary64 holds it without rounding) and rounded ONCE, half to even
+ * (reading P8 of DESIGN.md: a single rounding of the real product, not fl32 first and rint second).
  */
 static uint16_t orc_amax_bits(const uint16_t *x, int32_t d)
 {
@@ -300,10 +302,10 @@ void orc_quantize_vector(const uint16_t *x, int32_t d, int32_t qmax, uint16_t *a
     volatile float inv = 0.0f;                           /* volatile: force a rounded binary32 at each step */
     if (amax != 0.0f) inv = (float)qmax / amax;
     for (int32_t c = 0; c < d; ++c) {
-        volatile float t = orc_half_to_float(x[c]) * inv;
-        float r = rintf(t);                              /* FE_TONEAREST: ties to even */
-        if (r > (float)qmax) r = (float)qmax;
-        if (r < -(float)qmax) r = -(float)qmax;
+        const double t = (double)orc_half_to_float(x[c]) * (double)inv;   /* exact: 35 bits fit in 53 */
+        double r = rint(t);                              /* FE_TONEAREST: ties to even */
+        if (r > (double)qmax) r = (double)qmax;
+        if (r < -(double)qmax) r = -(double)qmax;
         q[c] = (int8_t)r;
     }
     *amax_out = ab;

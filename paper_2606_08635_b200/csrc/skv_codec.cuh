@@ -47,11 +47,13 @@ __device__ __forceinline__ __half absmax8_scalar(const uint4 &v)
     return __hmax(__low2half(m), __high2half(m));
 }
 
-// round-half-even of fl32(x*inv) via the 1.5*2^23 magic constant: the low bits of the sum's encoding are
-// the two's-complement integer (|x*inv| <= qmax*(1+2^-23) << 2^22, so the clamp of the spec is a no-op).
+// round-half-even of the EXACT product x*inv (include/skv.h) in one fused multiply-add with the 1.5*2^23 magic
+// constant: |x*inv| <= qmax*(1+2^-23) << 2^22, so x*inv + 1.5*2^23 lies in [2^23, 2^24) where binary32 spacing is 1
+// and the FMA's single rounding IS round-half-even to an integer (the constant is even, so parity carries over);
+// the low bits of the encoding are the two's-complement code and the clamp of the spec is a no-op.
 __device__ __forceinline__ uint32_t rne_code_bits(float x, float inv)
 {
-    return __float_as_uint(__fadd_rn(__fmul_rn(x, inv), 12582912.0f));
+    return __float_as_uint(__fmaf_rn(x, inv, 12582912.0f));
 }
 
 __device__ __forceinline__ uint32_t pack4_bytes(uint32_t a, uint32_t b, uint32_t c, uint32_t d)

@@ -211,6 +211,7 @@ pack_fast_kernel(Geom g, Layout lo, const __half *__restrict__ K, const __half *
     const int my_chunk = held_chunk<LPV, NCH>(lane);
     const bool scale_writer = (lane % (LPV / NCH)) == 0;
 
+#pragma unroll 1
     for (uint32_t i = warp; i < (uint32_t)kTileTokens; i += 8) {
         const uint32_t t = __shfl_sync(0xffffffffu, my_t, i);
         if (t != 16u && t != 8u && t != 4u) continue;                 // dropped / tail / invalid: no bytes
@@ -223,6 +224,7 @@ pack_fast_kernel(Geom g, Layout lo, const __half *__restrict__ K, const __half *
         const uint32_t cap = (t == 16u) ? (uint32_t)g.n16 : (t == 8u) ? (uint32_t)g.n8 : (uint32_t)g.n4;
         if (slot >= cap) continue;                                    // foreign map that disagrees with counts
 
+#pragma unroll 1
         for (int cb = 0; cb < g.row_chunks; cb += NCH) {
             uint4 kv[NCH], vv[NCH];
 #pragma unroll

@@ -175,6 +175,7 @@ unpack_fast_kernel(Geom g, Layout lo, const uint8_t *__restrict__ blob, uint64_t
         else if (t == 4u) { slot = base.z + __popc(m4 & below); if (slot >= (uint32_t)g.n4) t = 0; }
         else t = 0;
 
+#pragma unroll 1
         for (int cb = 0; cb < g.row_chunks; cb += NCH) {
             if (t == 16u) {
                 const uint8_t *ks = lbase + lo.seg_off[0] + ((uint64_t)slot * row_elems + cb * 256 + lane * 8) * 2;

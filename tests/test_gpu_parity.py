@@ -231,3 +231,33 @@ def test_full_size_bench_config_sampled():
         if (r, l) == (0, 0):                                             # float64 importance of one full layer
             I_or = oracle.importance(Kh, Qh).astype(np.float64)
             assert np.all(np.abs(Ih.astype(np.float64) - I_or) <= 1e-3 * I_or + 1e-30)
+
+
+@pytest.mark.parametrize("L,lpc", [(5, 2), (3, 4)])
+def test_layer_pipelined_transfer_matches_oracle(L, lpc):
+    """NEXT-2: the layer-pipelined host round trip (three streams, chunked blobs, ragged last chunk) returns, for
+    every layer, exactly what the oracle's pack -> unpack gives for the tier map the oracle assigns from the SAME
+    importance scores (the GPU's, read back), and those scores are within 1e-3 of the float64 oracle."""
+    from paper_2606_08635_b200.transfer import LayerPipelinedTransfer
+    cfg = C["C5"].scaled(L=L, n=1000, R=2)
+    case = Case(cfg, 0.4)
+    pin = dict(pin_memory=True)
+    hK, hV, hQ = case.K.contiguous().pin_memory(), case.V.contiguous().pin_memory(), case.Q.contiguous().pin_memory()
+    hKo = torch.full(hK.shape, float("nan"), dtype=torch.float16, **pin)
+    hVo = torch.full(hK.shape, float("nan"), dtype=torch.float16, **pin)
+    hI = torch.full((2, L, cfg.n), float("nan"), dtype=torch.float32, **pin)
+    hT = torch.full((2, L, cfg.n), 0xEE, dtype=torch.uint8, **pin)
+    pipe = LayerPipelinedTransfer(L, cfg.Hq, cfg.Hkv, cfg.d, cfg.n, cfg.w, 0.4, cfg.n_sink, cfg.ranges, cfg.allow_int4,
+                                  layers_per_chunk=lpc, depth=2)
+    for _ in range(2):                                       # second run reuses every slot and event path
+        pipe.run(hK, hV, hQ, hKo, hVo, hI, hT)
+    for r in range(2):
+        Ig = hI[r].numpy()
+        Io = case.I[r].astype(np.float64)
+        assert np.all(np.abs(Ig - Io) <= 1e-3 * Io + 1e-30)
+        tier = oracle.assign(Ig, case.prot, case.counts)
+        assert np.array_equal(tier, hT[r].numpy())
+        blob = oracle.pack(case.K[r].numpy(), case.V[r].numpy(), tier, case.counts, cfg.allow_int4)
+        K2, V2, _ = oracle.unpack(blob, L, cfg.Hkv, cfg.d, cfg.n)
+        assert np.array_equal(hKo[r].numpy().view(np.uint16), K2.view(np.uint16))
+        assert np.array_equal(hVo[r].numpy().view(np.uint16), V2.view(np.uint16))

@@ -218,6 +218,39 @@ def test_quantizer_special_cases():
     assert np.array_equal(oracle.dequantize_vector(q, 127, ab), sub)
 
 
+def _exact_code(x16, inv32, qmax):
+    """round-half-even of the exact rational product, clamped (independent of the oracle: fractions only)."""
+    from fractions import Fraction
+    import math
+    ex = Fraction(float(x16)) * Fraction(float(inv32))
+    fl = math.floor(ex)
+    fr = ex - fl
+    r = fl if fr < Fraction(1, 2) else fl + 1 if fr > Fraction(1, 2) else (fl if fl % 2 == 0 else fl + 1)
+    return max(-qmax, min(qmax, r))
+
+
+def test_quantizer_single_rounding_of_the_exact_product():
+    rows = read_golden(os.path.join(GOLD, "quantizer_single_rounding.txt"))
+    assert len(rows) == 6
+    for qmax, amax, x, code, code_two_step in rows:
+        qmax, amax, x, code, code_two_step = int(qmax), float(amax), float(x), int(code), int(code_two_step)
+        assert float(np.float16(amax)) == amax and float(np.float16(x)) == x and code != code_two_step
+        inv = np.float32(qmax) / np.float32(amax)
+        assert int(np.rint(np.float32(x) * inv)) == code_two_step            # what the rejected reading gives
+        assert _exact_code(x, inv, qmax) == code                              # the fixture is self-consistent
+        v = np.zeros(64, np.float16); v[0] = amax; v[1] = x
+        ab, q = oracle.quantize_vector(v, qmax)
+        assert q[0] == qmax and q[1] == code
+    # brute force on random vectors: every code equals the exactly-rounded rational product
+    rng = np.random.default_rng(11)
+    for qmax in (127, 7):
+        for _ in range(20):
+            v = (rng.standard_normal(128) * rng.uniform(0.01, 30)).astype(np.float16)
+            ab, q = oracle.quantize_vector(v, qmax)
+            inv = np.float32(qmax) / np.float32(np.uint16(ab).view(np.float16))
+            assert q.tolist() == [_exact_code(e, inv, qmax) for e in v]
+
+
 @pytest.mark.parametrize("qmax", [127, 7])
 def test_quantizer_error_bound(qmax):
     # BASELINE north_star: per-element dequantization error <= scale/2 (on the fp32 product, with the
