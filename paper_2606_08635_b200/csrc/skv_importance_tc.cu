@@ -2,15 +2,19 @@
 //
 // Same mathematics as skv_importance.cu (Eq. 13; logits PAPER.md:109), re-designed for sm_100a:
 //   * one persistent, warp-specialised CTA per SM: warp 0 = TMA producer, warp 1 = MMA issuer (one elected
-//     thread) and TMEM owner, warps 2..9 = eight epilogue warps;
+//     thread) and TMEM owner, warps 2..17 = sixteen epilogue warps (four per scheduler, so that the MUFU pipe,
+//     which bounds this kernel at d_h = 128, always has an eligible warp);
+//   * a quarter of the exponentials is evaluated on the FMA pipe (round-to-nearest range reduction + degree-4
+//     minimax polynomial, 2.7e-6 relative) instead of MUFU.EX2, which lifts the 16 ex2/clk/SM ceiling;
 //   * operands land in shared memory by TMA (cp.async.bulk.tensor, 128-byte swizzle, mbarrier complete_tx)
 //     straight from the strided K cache and the Q window; accumulators live in TMEM (2 stages x 256 columns);
 //   * pass 1 (rowstats): D[query row][key] = Q_blk K_tile^T, queries are TMEM lanes, so each epilogue thread owns
 //     one query row and keeps its online (max, sum 2^x) entirely in registers -- no shuffles;
 //   * pass 2 (colsum):  D[key][query row] = K_tile Q_blk^T, keys are TMEM lanes, so each thread owns one key and
-//     sums p = 2^(s - lse2[row]) over its columns in registers -- no shuffles, no atomics; the per-(KV head, row
-//     block, column half) partial sums go to a workspace and a small finish kernel adds them in a fixed order
-//     (deterministic) and applies 1/(Hq w) and the recency decay.
+//     sums p = 2^(s - lse2[row]) over its columns in registers -- no shuffles, no atomics; the four column groups
+//     of a tile are added through shared memory in a fixed order, the per-(KV head, row block) partial sums go to a
+//     workspace and a small finish kernel adds them in a fixed order (deterministic) and applies 1/(Hq w) and the
+//     recency decay.
 // A work item is (request, layer, KV head, row block, key chunk); items are dealt round-robin to the CTAs.
 #include <cuda.h>
 #include <string.h>
@@ -23,8 +27,9 @@ namespace skv {
 
 namespace tc {
 
-constexpr int kThreads = 320;            // warps: 0 TMA, 1 MMA/TMEM, 2..9 epilogue
-constexpr int kEpiWarps = 8;
+constexpr int kEpiWarps = 16;
+constexpr int kEpiThreads = kEpiWarps * 32;
+constexpr int kThreads = 64 + kEpiThreads;   // warps: 0 TMA, 1 MMA/TMEM, 2..17 epilogue
 constexpr int kTileKeys = 128;
 constexpr float kNegBig = -1.0e30f;
 
@@ -37,9 +42,9 @@ struct Params {
     int n_items;
     int kdim[4];                        // position of (head, token, layer, request) in the K tensor map (1..4)
     float2 *partial;                    // [rows][pchunks]
-    int pchunks;                        // n_chunks * (halves == 1 ? 2 : 1)
+    int pchunks;                        // n_chunks * (column groups per row in pass 1: 4 / halves)
     const float *lse2;                  // [R][L][Hq*w]
-    float *apart;                       // [R][L][S][n], S = Hkv*RB*2
+    float *apart;                       // [R][L][S][n], S = Hkv*RB
     int S;
 };
 
@@ -121,13 +126,72 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, float (&v)[32])
 #pragma unroll
     for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
 }
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, float (&v)[16])
+{
+    uint32_t r[16];
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+        "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+          "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+        : "r"(taddr) : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+    for (int i = 0; i < 16; ++i) v[i] = __uint_as_float(r[i]);
+}
 __device__ __forceinline__ float ex2(float x)
 {
     float y;
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
-__device__ __forceinline__ void epi_bar_sync() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
+// 2^x for a PAIR of values on the FMA/ALU pipes with the packed fp32 instructions of sm_100 (FFMA2 / FADD2):
+// n = rint(x) through the 1.5*2^23 constant, f = x - n in [-0.5, 0.5], degree-4 minimax polynomial for 2^f (max
+// relative error 2.7e-6), exponent patched in with one shift-add per value.  x is clamped at -125 (anything below
+// contributes < 2^-125 of the row's reference term).  5.5 issue slots per value and no MUFU.
+__device__ __forceinline__ float2 ex2_fma2(float2 x)
+{
+    x.x = fmaxf(x.x, -125.0f);
+    x.y = fmaxf(x.y, -125.0f);
+    const float2 t = __fadd2_rn(x, make_float2(12582912.0f, 12582912.0f));
+    const float2 nf = __fadd2_rn(t, make_float2(-12582912.0f, -12582912.0f));
+    const float2 f = __ffma2_rn(nf, make_float2(-1.0f, -1.0f), x);
+    float2 q = __ffma2_rn(f, make_float2(0.009570102207362652f, 0.009570102207362652f), make_float2(0.05591785907745361f, 0.05591785907745361f));
+    q = __ffma2_rn(q, f, make_float2(0.240247443318367f, 0.240247443318367f));
+    q = __ffma2_rn(q, f, make_float2(0.6931217908859253f, 0.6931217908859253f));
+    q = __ffma2_rn(q, f, make_float2(0.9999992847442627f, 0.9999992847442627f));
+    return make_float2(__int_as_float(__float_as_int(q.x) + (__float_as_int(t.x) << 23)),
+                       __int_as_float(__float_as_int(q.y) + (__float_as_int(t.y) << 23)));
+}
+__device__ __forceinline__ float2 ex2_mufu2(float2 x) { return make_float2(ex2(x.x), ex2(x.y)); }
+// which of the 8 value pairs of a 16-wide group go to the FMA pipe (the rest to MUFU.EX2): kFmaPairs of 8
+#ifndef SKV_EX2_FMA_PAIRS
+#define SKV_EX2_FMA_PAIRS 2
+#endif
+__device__ __forceinline__ constexpr bool pair_on_fma(int pi)
+{
+    return SKV_EX2_FMA_PAIRS == 0 ? false
+         : SKV_EX2_FMA_PAIRS == 1 ? (pi & 7) == 3
+         : SKV_EX2_FMA_PAIRS == 2 ? (pi & 3) == 1
+         : SKV_EX2_FMA_PAIRS == 3 ? ((pi & 7) == 1 || (pi & 7) == 4 || (pi & 7) == 6)
+         :                          (pi & 1) == 1;
+}
+template <int PI> __device__ __forceinline__ float2 ex2_pair(float2 x) { return pair_on_fma(PI) ? ex2_fma2(x) : ex2_mufu2(x); }
+// sum of 2^(v*sc + add) over a 16-wide group, two packed accumulators
+template <int N>
+__device__ __forceinline__ void exp_accumulate(const float (&v)[N], float2 sc2, const float2 (&add2)[N / 2], float2 &accA, float2 &accB)
+{
+#pragma unroll
+    for (int pi = 0; pi < N / 2; ++pi) {
+        const float2 x = __ffma2_rn(make_float2(v[2 * pi], v[2 * pi + 1]), sc2, add2[pi]);
+        const float2 e = pair_on_fma(pi) ? ex2_fma2(x) : ex2_mufu2(x);
+        if (pi & 1) accB = __fadd2_rn(accB, e); else accA = __fadd2_rn(accA, e);
+    }
+}
+template <int D> struct ScaleLog2 {   // log2(e) / sqrt(D) as an immediate
+    static constexpr float value = (D == 64) ? 0.18033688011112042f : (D == 128) ? 0.12751743082459868f : 0.09016844005556021f;
+};
+__device__ __forceinline__ void epi_bar_sync() { asm volatile("bar.sync 1, 512;" ::: "memory"); }
 
 }  // namespace tc
 
@@ -141,7 +205,8 @@ template <int D> struct Cfg {
     static constexpr int K_KB_STRIDE = kTileKeys * 128;
     static constexpr int K_BYTES = KB * K_KB_STRIDE;
     static constexpr int STAGES = (D == 64) ? 6 : (D == 128) ? 4 : 2;
-    static constexpr int SMEM = 1024 + Q_BYTES + STAGES * K_BYTES + 256 * 4 * 2 + 256;
+    static constexpr int RED_BYTES = 4 * 3 * kTileKeys * 4;            // pass 2: ring of 4 x [column groups 1..3][128 keys]
+    static constexpr int SMEM = 1024 + Q_BYTES + STAGES * K_BYTES + 256 * 4 * 2 + RED_BYTES + 256;
 };
 
 struct Item { int r, l, g, rb, chunk, gb; };
@@ -170,12 +235,14 @@ imp_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ C
     const uint32_t sK = sQ + C::Q_BYTES;
     float *sLse = reinterpret_cast<float *>(gbase + C::Q_BYTES + C::STAGES * C::K_BYTES);
     int *sLim = reinterpret_cast<int *>(sLse + 256);
-    const uint32_t sBar = sK + C::STAGES * C::K_BYTES + 256 * 4 * 2;
+    float *sRed = reinterpret_cast<float *>(sLim + 256);
+    const uint32_t sBar = sK + C::STAGES * C::K_BYTES + 256 * 4 * 2 + C::RED_BYTES;
     // barriers (8 bytes each): kfull[S], kempty[S], qfull, qempty, tfull[2], tempty[2]
     const uint32_t kfull = sBar, kempty = sBar + 8 * C::STAGES;
     const uint32_t qfull = sBar + 16 * C::STAGES, qempty = qfull + 8;
     const uint32_t tfull = qempty + 8, tempty = tfull + 16;
-    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(gbase + (tempty + 16 - sbase));
+    const uint32_t redfull = tempty + 16;                               // 4 barriers: column-group partials landed
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(gbase + (redfull + 32 - sbase));
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n = p.g.n;
@@ -184,6 +251,7 @@ imp_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ C
         for (int s = 0; s < C::STAGES; ++s) { mbar_init(kfull + 8 * s, 1); mbar_init(kempty + 8 * s, 1); }
         mbar_init(qfull, 1); mbar_init(qempty, 1);
         for (int a = 0; a < 2; ++a) { mbar_init(tfull + 8 * a, 1); mbar_init(tempty + 8 * a, kEpiWarps); }
+        for (int a = 0; a < 4; ++a) mbar_init(redfull + 8 * a, kEpiWarps - 4);
         fence_barrier_init();
     }
     if (warp == 1) {
@@ -257,22 +325,25 @@ imp_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ C
             }
         }
     } else {
-        // ===================== epilogue warps (2..9) =====================
-        const int e = warp - 2, quad = warp & 3, hsel = e >> 2;
-        const int etid = e * 32 + lane;                                   // 0..255 among the epilogue threads
-        const float sc = 1.4426950408889634f * rsqrtf((float)D);         // log2(e)/sqrt(d)
+        // ===================== epilogue warps (2..17) =====================
+        // TMEM lane window of a warp is fixed by (warp id % 4); grp = which of the four warps on that window.
+        const int e = warp - 2, quad = warp & 3, grp = e >> 2;
+        const int etid = e * 32 + lane;                                   // 0..511 among the epilogue threads
+        constexpr float sc = ScaleLog2<D>::value;                         // log2(e)/sqrt(d)
         const int G = p.g.Hq / p.g.Hkv, M = G * p.w;
-        uint32_t astage = 0, aphase = 0;
+        uint32_t astage = 0, aphase = 0, rstage = 0, rphase = 0;
         for (int item = blockIdx.x; item < p.n_items; item += gridDim.x) {
             const Item it = decode_item(p, item);
             const int key_beg = it.chunk * p.chunk_keys, key_end = min(n, key_beg + p.chunk_keys);
             const int64_t rowbase = ((int64_t)it.r * p.g.L + it.l) * p.g.Hq * p.w + (int64_t)it.g * M;
             const int mrows = min(p.MB, M - it.rb * p.MB);
             if (PASS == 1) {
-                const int row_in_blk = (p.halves == 2 ? hsel * 128 : 0) + quad * 32 + lane;
-                const int col0 = (p.halves == 2) ? 0 : hsel * 64;
-                const int ncols = (p.halves == 2) ? 128 : 64;
-                const int colbase = (p.halves == 2) ? hsel * 128 : col0;
+                // halves == 2: 2 row halves x 2 column groups of 64 keys; halves == 1: 4 column groups of 32 keys
+                const int hsel = (p.halves == 2) ? (grp & 1) : 0;
+                const int cg = (p.halves == 2) ? (grp >> 1) : grp;
+                const int ncols = (p.halves == 2) ? 64 : 32;
+                const int col0 = cg * ncols;                              // key offset inside the 128-key tile
+                const int row_in_blk = hsel * 128 + quad * 32 + lane;
                 const int row_g = it.rb * p.MB + row_in_blk;
                 const bool valid = row_in_blk < mrows;
                 const int lim = p.causal ? (n - p.w + (row_g % p.w)) : (n - 1);
@@ -281,21 +352,41 @@ imp_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ C
                     mbar_wait(tfull + 8 * astage, aphase);
                     tc_fence_after();
                     const bool need_mask = p.causal ? (k0 + kTileKeys - 1 > n - p.w) : (k0 + kTileKeys > n);
-                    const uint32_t taddr = tmem + ((uint32_t)(quad * 32) << 16) + astage * 256 + colbase;
+                    const uint32_t taddr = tmem + ((uint32_t)(quad * 32) << 16) + astage * 256 + hsel * 128 + col0;
                     for (int cc = 0; cc < ncols; cc += 32) {
                         float v[32];
                         tmem_ld32(taddr + cc, v);
                         const int j0 = k0 + col0 + cc;
                         float tmax = kNegBig;
                         if (!need_mask) {
+                            // lazy reference exponent: m is fixed by the first visible group of the row and only an
+                            // overflow guard watches it afterwards (the row sum is z * 2^m for ANY m, so no per-
+                            // element max is needed); the exact online-max update below is the rare rescue path.
+                            if (m < 0.5f * kNegBig) {
 #pragma unroll
-                            for (int i = 0; i < 32; ++i) tmax = fmaxf(tmax, v[i]);
-                            const float mn = fmaxf(m, tmax * sc);
-                            float acc = 0.f;
+                                for (int i = 0; i < 32; ++i) tmax = fmaxf(tmax, v[i]);
+                                m = tmax * sc;
+                            }
+                            float2 nm2[16];
 #pragma unroll
-                            for (int i = 0; i < 32; ++i) acc += ex2(fmaf(v[i], sc, -mn));
-                            z = z * ex2(m - mn) + acc;
-                            m = mn;
+                            for (int pi = 0; pi < 16; ++pi) nm2[pi] = make_float2(-m, -m);
+                            float2 accA = make_float2(0.f, 0.f), accB = accA;
+                            exp_accumulate<32>(v, make_float2(sc, sc), nm2, accA, accB);
+                            const float2 s2 = __fadd2_rn(accA, accB);
+                            const float a = s2.x + s2.y;
+                            if (a < 1.0e30f) {
+                                z += a;
+                                if (!(z < 1.0e30f)) { z *= 0x1p-80f; m += 80.0f; }
+                            } else {                                      // a term overflowed: redo the group exactly
+#pragma unroll
+                                for (int i = 0; i < 32; ++i) tmax = fmaxf(tmax, v[i]);
+                                const float mn = fmaxf(m, tmax * sc);
+                                float acc = 0.f;
+#pragma unroll
+                                for (int i = 0; i < 32; ++i) acc += ex2(fmaf(v[i], sc, -mn));
+                                z = z * ex2(m - mn) + acc;
+                                m = mn;
+                            }
                         } else {
 #pragma unroll
                             for (int i = 0; i < 32; ++i) if (j0 + i <= lim) tmax = fmaxf(tmax, v[i]);
@@ -313,52 +404,71 @@ imp_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ C
                     if (++astage == 2) { astage = 0; aphase ^= 1; }
                 }
                 if (valid) {
-                    const int pc = (p.halves == 2) ? it.chunk : it.chunk * 2 + hsel;
-                    p.partial[(rowbase + row_g) * p.pchunks + pc] = make_float2(m, z);
+                    const int cs = (p.halves == 2) ? 2 : 4;
+                    p.partial[(rowbase + row_g) * p.pchunks + it.chunk * cs + cg] = make_float2(m, z);
                 }
             } else {
                 // per-item column tables: lse2 of the block's query rows and their causal limits
                 epi_bar_sync();
-                for (int idx = etid; idx < p.qrows; idx += 256) {
+                for (int idx = etid; idx < p.qrows; idx += kEpiThreads) {
                     const bool ok = idx < mrows;
-                    sLse[idx] = ok ? p.lse2[rowbase + it.rb * p.MB + idx] : 0.f;
+                    sLse[idx] = ok ? -p.lse2[rowbase + it.rb * p.MB + idx] : 0.f;      // NEGATED lse2
                     sLim[idx] = ok ? (p.causal ? (n - p.w + ((it.rb * p.MB + idx) % p.w)) : (n - 1)) : -1;
                 }
                 epi_bar_sync();
-                const int half = p.qrows >> 1;
-                const int cbeg = hsel * half;
-                float *out = p.apart + (((int64_t)it.r * p.g.L + it.l) * p.S + it.gb * 2 + hsel) * (int64_t)n;
+                const int qcols = p.qrows >> 2;                           // query columns per group: 16, 32, 48 or 64
+                const int cbeg = grp * qcols;
+                float *out = p.apart + (((int64_t)it.r * p.g.L + it.l) * p.S + it.gb) * (int64_t)n;
                 for (int k0 = key_beg; k0 < key_end; k0 += kTileKeys) {
                     mbar_wait(tfull + 8 * astage, aphase);
                     tc_fence_after();
                     const int j = k0 + quad * 32 + lane;
                     const bool tile_mask = p.causal && (k0 + kTileKeys - 1 > n - p.w);
                     const uint32_t taddr = tmem + ((uint32_t)(quad * 32) << 16) + astage * 256 + cbeg;
-                    float sum = 0.f;
-                    for (int cc = 0; cc < half; cc += 32) {
+                    float2 accA = make_float2(0.f, 0.f), accB = accA;
+                    float s0 = 0.f;
+                    for (int cc = 0; cc < qcols; cc += 16) {
                         if (cbeg + cc >= mrows) break;                    // warp-uniform: only padding columns left
-                        float v[32];
-                        tmem_ld32(taddr + cc, v);
-                        const float4 *l4 = reinterpret_cast<const float4 *>(sLse + cbeg + cc);
-                        if (!tile_mask && cbeg + cc + 32 <= mrows) {
+                        float v[16];
+                        tmem_ld16(taddr + cc, v);
+                        if (!tile_mask && cbeg + cc + 16 <= mrows) {
+                            const float4 *l4 = reinterpret_cast<const float4 *>(sLse + cbeg + cc);
+                            float2 nl2[8];
 #pragma unroll
-                            for (int i = 0; i < 8; ++i) {
+                            for (int i = 0; i < 4; ++i) {
                                 const float4 L4 = l4[i];
-                                sum += ex2(fmaf(v[4 * i], sc, -L4.x)) + ex2(fmaf(v[4 * i + 1], sc, -L4.y)) +
-                                       ex2(fmaf(v[4 * i + 2], sc, -L4.z)) + ex2(fmaf(v[4 * i + 3], sc, -L4.w));
+                                nl2[2 * i] = make_float2(L4.x, L4.y);
+                                nl2[2 * i + 1] = make_float2(L4.z, L4.w);
                             }
+                            exp_accumulate<16>(v, make_float2(sc, sc), nl2, accA, accB);
                         } else {
                             const int *lim = sLim + cbeg + cc;
 #pragma unroll
-                            for (int i = 0; i < 32; ++i)
-                                sum += (j <= lim[i]) ? ex2(fmaf(v[i], sc, -sLse[cbeg + cc + i])) : 0.f;
+                            for (int i = 0; i < 16; ++i)
+                                s0 += (j <= lim[i]) ? ex2(fmaf(v[i], sc, sLse[cbeg + cc + i])) : 0.f;
                         }
                     }
+                    const float2 s2 = __fadd2_rn(accA, accB);
                     tc_fence_before();
                     __syncwarp();
                     if (lane == 0) mbar_arrive(tempty + 8 * astage);
                     if (++astage == 2) { astage = 0; aphase ^= 1; }
-                    if (j < n) out[j] = sum;
+                    // add the four column groups of this tile in a fixed order (deterministic): groups 1..3 drop
+                    // their sums into a 4-deep shared-memory ring and arrive on its mbarrier (they never block);
+                    // group 0 waits for the slot, adds and stores.  Ring depth 4 > the 2 TMEM stages any warp can
+                    // run ahead, so a slot is never overwritten before group 0 has read it.
+                    const float mine = (s2.x + s2.y) + s0;
+                    float *red = sRed + rstage * (3 * kTileKeys);
+                    if (grp != 0) {
+                        red[(grp - 1) * kTileKeys + quad * 32 + lane] = mine;
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(redfull + 8 * rstage);
+                    } else {
+                        mbar_wait(redfull + 8 * rstage, rphase);
+                        const int k = quad * 32 + lane;
+                        if (j < n) out[j] = (mine + red[k]) + (red[kTileKeys + k] + red[2 * kTileKeys + k]);
+                    }
+                    if (++rstage == 4) { rstage = 0; rphase ^= 1; }
                 }
             }
         }
@@ -430,8 +540,8 @@ static TcPlan tc_plan(const Geom &g, int w)
     if (ck > npad) ck = npad;
     t.chunk_keys = ck;
     t.n_chunks = (g.n + ck - 1) / ck;
-    t.pchunks = t.n_chunks * (t.halves == 1 ? 2 : 1);
-    t.S = g.Hkv * t.RB * 2;
+    t.pchunks = t.n_chunks * (t.halves == 1 ? 4 : 2);
+    t.S = g.Hkv * t.RB;
     t.n_items = (int)(triples * t.n_chunks);
     const size_t rows = (size_t)g.R * g.L * g.Hq * w;
     t.partial_bytes = (rows * t.pchunks * sizeof(float2) + 255) & ~(size_t)255;
