@@ -261,3 +261,85 @@ def test_layer_pipelined_transfer_matches_oracle(L, lpc):
         K2, V2, _ = oracle.unpack(blob, L, cfg.Hkv, cfg.d, cfg.n)
         assert np.array_equal(hKo[r].numpy().view(np.uint16), K2.view(np.uint16))
         assert np.array_equal(hVo[r].numpy().view(np.uint16), V2.view(np.uint16))
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("name,b", [("C2", 0.3), ("C2", 0.5), ("C3", 0.3), ("C3", 0.5), ("C4", 0.5)])
+def test_full_size_model_shaped_configs(name, b):
+    """BASELINE configs C2-C4 at FULL size (all layers): importance on the GPU, then tier map, every blob byte and
+    every dequantised fp16 element compared with the oracle run on the same importance scores; the float64 oracle
+    importance is compared on two sampled layers."""
+    cfg = C[name]
+    dev = torch.device("cuda:0")
+    L = cfg.L
+    K, V = skv_synth.make_kv(cfg, 0)
+    Q = skv_synth.make_q(cfg, 0)
+    Kd, Vd, Qd = K.to(dev)[None], V.to(dev)[None], Q.to(dev)[None]
+    shape = skv.make_shape(L, cfg.Hq, cfg.Hkv, cfg.d, cfg.n, 1)
+    pol = skv.make_policy(b, cfg.n_sink, cfg.ranges, cfg.allow_int4)
+    ws = torch.empty(skv.skv_workspace_bytes(shape, cfg.w), dtype=torch.uint8, device=dev)
+    I = torch.empty((1, L, cfg.n), dtype=torch.float32, device=dev)
+    tier = torch.empty((1, L, cfg.n), dtype=torch.uint8, device=dev)
+    skv.skv_importance(shape, Kd, Qd, cfg.w, I, ws)
+    counts = skv.skv_assign_tiers(shape, pol, I, tier, ws)
+    bb = skv.skv_blob_bytes(shape, counts)
+    blob = torch.full((bb,), 0xAB, dtype=torch.uint8, device=dev)
+    skv.skv_pack(shape, Kd, Vd, tier, counts, blob, ws)
+    Ko = torch.full_like(Kd, float("nan")); Vo = torch.full_like(Vd, float("nan"))
+    skv.skv_unpack(shape, blob, bb, counts, Ko, Vo, None, ws)
+    torch.cuda.synchronize()
+
+    oc, prot = oracle.tier_counts(cfg.n, b, cfg.n_sink, cfg.ranges, cfg.allow_int4)
+    assert counts.as_tuple() == (oc.n16, oc.n8, oc.n4, oc.n0)
+    Ih = I[0].cpu().numpy()
+    t_or = oracle.assign(Ih, prot, oc)
+    assert np.array_equal(t_or, tier[0].cpu().numpy())
+    Kn, Vn = K.numpy(), V.numpy()
+    blob_or = oracle.pack(Kn, Vn, t_or, oc, cfg.allow_int4)
+    assert blob_or.size == bb and np.array_equal(blob.cpu().numpy(), blob_or)
+    K2, V2, _ = oracle.unpack(blob_or, L, cfg.Hkv, cfg.d, cfg.n)
+    assert np.array_equal(Ko[0].cpu().numpy().view(np.uint16), K2.view(np.uint16))
+    assert np.array_equal(Vo[0].cpu().numpy().view(np.uint16), V2.view(np.uint16))
+    for l in (0, L - 1):
+        I_or = oracle.importance(Kn[l:l + 1], Q.numpy()[l:l + 1]).astype(np.float64)
+        assert np.all(np.abs(Ih[l:l + 1].astype(np.float64) - I_or) <= 1e-3 * I_or + 1e-30)
+
+
+@pytest.mark.parametrize("n,d,Hkv,Hq,w", [(257, 128, 2, 4, 16), (1000, 64, 3, 3, 8), (4097, 256, 1, 2, 32)])
+def test_guard_zones_around_every_output(n, d, Hkv, Hq, w):
+    """compute-sanitizer is closed on this GPU pool, so out-of-bounds writes are hunted with canaries: every output
+    and the workspace sit inside a larger allocation whose margins must come back untouched, and the workspace is
+    exactly skv_workspace_bytes() long."""
+    dev = torch.device("cuda:0")
+    cfg = C["C1"].scaled(L=2, Hq=Hq, Hkv=Hkv, d=d, n=n, w=w, R=2, k_dist="outlier")
+    case = Case(cfg, 0.4, with_importance=False)
+    G = 4096                                                     # guard bytes on each side (multiple of 256)
+
+    def guarded(nbytes, dtype):
+        raw = torch.full((G + nbytes + G,), 0x5A, dtype=torch.uint8, device=dev)
+        return raw, raw[G:G + nbytes].view(dtype)
+
+    shape, pol = case.shape(), case.policy()
+    R, L = case.R, case.L
+    Kd, Vd, Qd = case.K.to(dev), case.V.to(dev), case.Q.to(dev)
+    raws = []
+    r_ws, ws = guarded((skv.skv_workspace_bytes(shape, w) + 255) // 256 * 256, torch.uint8); raws.append(r_ws)
+    r_I, I = guarded(R * L * n * 4, torch.float32); raws.append(r_I)
+    n_pad = (R * L * n + 255) // 256 * 256
+    r_t, tier_raw = guarded(n_pad, torch.uint8); raws.append(r_t)
+    tier = tier_raw[:R * L * n]
+    skv.skv_importance(shape, Kd, Qd, w, I, ws)
+    counts = skv.skv_assign_tiers(shape, pol, I, tier, ws)
+    bb = skv.skv_blob_bytes(shape, counts)
+    r_b, blob = guarded(R * bb, torch.uint8); raws.append(r_b)
+    skv.skv_pack(shape, Kd, Vd, tier, counts, blob, ws)
+    r_k, Ko = guarded(Kd.numel() * 2, torch.float16); raws.append(r_k)
+    r_v, Vo = guarded(Vd.numel() * 2, torch.float16); raws.append(r_v)
+    r_to, to_raw = guarded(n_pad, torch.uint8); raws.append(r_to)
+    skv.skv_unpack(shape, blob, bb, counts, Ko, Vo, to_raw[:R * L * n], ws)
+    skv.skv_importance_kvnorm(shape, Kd, I, ws)
+    torch.cuda.synchronize()
+    for raw in raws:
+        assert bool((raw[:G] == 0x5A).all()) and bool((raw[-G:] == 0x5A).all())
+    assert bool((tier_raw[R * L * n:] == 0x5A).all()) and bool((to_raw[R * L * n:] == 0x5A).all())
+    assert torch.equal(to_raw[:R * L * n], tier)
