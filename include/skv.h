@@ -17,6 +17,7 @@
  *                     ("standard symmetric") and compact into one SKV1 blob
  *   skv_unpack        PAPER.md:202: dequantise and scatter back into a dense FP16 cache
  *   skv_blob_check    decode-side validation of a received blob header (host)
+ *   skv_unpack_patch  cold-tier precision upgrade: apply an upgrade blob to a dense cache in place
  *
  * Conventions
  *   - Every pointer is tagged HOST or DEVICE.  DEVICE pointers are plain CUDA device addresses
@@ -147,6 +148,25 @@ int skv_pack(const skv_shape *shape, const void *K_dev, const void *V_dev, const
 int skv_unpack(const skv_shape *shape, const void *blob_dev, size_t blob_bytes, const skv_counts *counts,
                void *K_out_dev, void *V_out_dev, uint8_t *tier_map_out_dev,
                void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
+
+/* DEVICE.  Cold-tier precision upgrade, decode side ("a cold-tier fetch only needs to
+ * upgrade the precision"; described there, never implemented).  The prefill side builds an UPGRADE
+ * blob with skv_pack() from an upgrade map u8 [R][L][n] that holds the new tier (normally 16) at the tokens to
+ * upgrade and 0 everywhere else, with counts from skv_counts_from_populations() (the same number of upgraded
+ * tokens in every layer).  skv_unpack_patch() applies it in place: tokens the blob carries are overwritten in
+ * K_inout/V_inout exactly as skv_unpack() would write them, tokens it does not carry (tier 0 in the blob) are left
+ * untouched, and tier_map_inout_dev (nullable) is updated at the carried tokens only.  The replacement rows are
+ * shipped whole (2 B per element at tier 16): a lossless residual against the INT4 codes does not fit the paper's
+ * s16 - s4 figure (NEXT-3). */
+int skv_unpack_patch(const skv_shape *shape, const void *blob_dev, size_t blob_bytes, const skv_counts *counts,
+                     void *K_inout_dev, void *V_inout_dev, uint8_t *tier_map_inout_dev,
+                     void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
+
+/* HOST only.  Counts for explicit tier populations (upgrade blobs, ablation policies): n0 = n - n16 - n8 - n4,
+ * budget_q4 = spent_q4 = 4 n16 + 2 n8 + n4.  SKV_ERR_INVALID_ARG if the populations exceed n or n4 > 0 without
+ * allow_int4. */
+int skv_counts_from_populations(const skv_shape *shape, int32_t n16, int32_t n8, int32_t n4, int32_t allow_int4,
+                                skv_counts *counts_out);
 
 const char *skv_strerror(int status);
 

@@ -149,6 +149,21 @@ def unpack(blob, L, Hkv, d, n):
     return K, V, tier
 
 
+def unpack_patch(blob, K, V, tier):
+    """NEXT-3 cold-tier upgrade: applies an upgrade blob to COPIES of the dense cache K, V [L][n][Hkv][d] and of the
+    tier map [L][n]; returns (K, V, tier)."""
+    blob = _c(blob, np.uint8)
+    K = np.array(K, dtype=np.float16, order="C", copy=True)
+    V = np.array(V, dtype=np.float16, order="C", copy=True)
+    tier = np.array(tier, dtype=np.uint8, order="C", copy=True)
+    L, n, Hkv, d = K.shape
+    rc = lib().orc_unpack_patch(_p(blob), C.c_uint64(blob.size), C.c_int32(L), C.c_int32(Hkv), C.c_int32(d),
+                                C.c_int64(n), _p(K), _p(V), _p(tier))
+    if rc != 0:
+        raise ValueError(f"orc_unpack_patch rc={rc} (bad blob)")
+    return K, V, tier
+
+
 def quantize_vector(x, qmax):
     """O4 on one vector.  x float16[d] -> (amax_bits, int8[d])."""
     x = _c(x, np.float16)

@@ -395,8 +395,8 @@ int orc_pack(int32_t L, int32_t Hkv, int32_t d, int64_t n, const uint16_t *K, co
 /* O6. Unpack (decode side; dropped -> +0.0 fill, reading P10) */
 /* ------------------------------------------------------------------------ */
 /* Parses the header (dims must match the arguments), returns 0 or -5 (bad blob). */
-int orc_unpack(const uint8_t *blob, uint64_t blob_bytes, int32_t L, int32_t Hkv, int32_t d, int64_t n,
-               uint16_t *K, uint16_t *V, uint8_t *tier_out)
+static int orc_unpack_impl(const uint8_t *blob, uint64_t blob_bytes, int32_t L, int32_t Hkv, int32_t d, int64_t n,
+                           uint16_t *K, uint16_t *V, uint8_t *tier_out, int patch)
 {
     if (blob_bytes < 256) return -5;
     if (get_u32(blob) != 0x31564B53u || get_u32(blob + 4) != 1u) return -5;
@@ -410,7 +410,9 @@ int orc_unpack(const uint8_t *blob, uint64_t blob_bytes, int32_t L, int32_t Hkv,
         lo.total_bytes != blob_bytes) return -5;
     for (int s = 0; s < 10; ++s) if (get_u64(blob + 80 + 8 * s) != lo.seg_off[s]) return -5;
     const uint8_t *tier = blob + lo.tier_map_off;
-    if (tier_out) memcpy(tier_out, tier, (size_t)L * (size_t)n);
+    if (tier_out && !patch) memcpy(tier_out, tier, (size_t)L * (size_t)n);
+    if (tier_out && patch)                               /* upgrade: only the shipped tokens change tier */
+        for (size_t i = 0; i < (size_t)L * (size_t)n; ++i) if (tier[i] != 0) tier_out[i] = tier[i];
 
     const size_t row = (size_t)Hkv * (size_t)d;
 #pragma omp parallel for schedule(dynamic, 1)
@@ -443,15 +445,31 @@ int orc_unpack(const uint8_t *blob, uint64_t blob_bytes, int32_t L, int32_t Hkv,
                         }
                         orc_dequantize_vector(q, d, 7, (uint16_t)(sc[2 * h] | (sc[2 * h + 1] << 8)), dst + (size_t)h * d);
                     }
-                } else {
+                } else if (!patch) {
                     for (size_t e = 0; e < row; ++e) dst[e] = 0;             /* P10: dropped => +0.0 */
-                }
+                }                                                            /* patch: not shipped => untouched */
             }
             if (t == 16) ++slot16; else if (t == 8) ++slot8; else if (t == 4) ++slot4;
         }
         free(q);
     }
     return 0;
+}
+
+int orc_unpack(const uint8_t *blob, uint64_t blob_bytes, int32_t L, int32_t Hkv, int32_t d, int64_t n,
+               uint16_t *K, uint16_t *V, uint8_t *tier_out)
+{
+    return orc_unpack_impl(blob, blob_bytes, L, Hkv, d, n, K, V, tier_out, 0);
+}
+
+/* NEXT-3: cold-tier precision upgrade ("a cold-tier fetch only needs to upgrade the
+ * precision").  An upgrade blob is an ordinary SKV1 blob packed from an upgrade map (new tier at the tokens to
+ * upgrade, 0 elsewhere); applying it overwrites exactly the shipped tokens of the dense cache K, V (in place) and
+ * of the tier map, and touches nothing else. */
+int orc_unpack_patch(const uint8_t *blob, uint64_t blob_bytes, int32_t L, int32_t Hkv, int32_t d, int64_t n,
+                     uint16_t *K_inout, uint16_t *V_inout, uint8_t *tier_inout)
+{
+    return orc_unpack_impl(blob, blob_bytes, L, Hkv, d, n, K_inout, V_inout, tier_inout, 1);
 }
 
 /* ------------------------------------------------------------------------ */

@@ -7,7 +7,8 @@ the import of any entry point raises.
 
 Entry points mirror the C ABI one to one (see include/skv.h for semantics and citations):
     skv_tier_counts, skv_blob_bytes, skv_workspace_bytes, skv_blob_check,
-    skv_importance, skv_importance_kvnorm, skv_assign_tiers, skv_pack, skv_unpack, skv_strerror
+    skv_importance, skv_importance_kvnorm, skv_assign_tiers, skv_pack, skv_unpack, skv_unpack_patch,
+    skv_counts_from_populations, skv_strerror
 """
 import ctypes as C
 import os
@@ -56,7 +57,8 @@ class skv_counts(C.Structure):
 
 
 EXPORTS = ("skv_tier_counts", "skv_blob_bytes", "skv_workspace_bytes", "skv_blob_check", "skv_importance",
-           "skv_importance_kvnorm", "skv_assign_tiers", "skv_pack", "skv_unpack", "skv_strerror", "skv_version")
+           "skv_importance_kvnorm", "skv_assign_tiers", "skv_pack", "skv_unpack", "skv_unpack_patch",
+           "skv_counts_from_populations", "skv_strerror", "skv_version")
 
 _lib = None
 
@@ -81,6 +83,8 @@ def lib():
         L.skv_assign_tiers.argtypes = [P(skv_shape), P(skv_policy), V, V, P(skv_counts), V, C.c_size_t, V]
         L.skv_pack.argtypes = [P(skv_shape), V, V, V, P(skv_counts), V, C.c_size_t, V, C.c_size_t, V]
         L.skv_unpack.argtypes = [P(skv_shape), V, C.c_size_t, P(skv_counts), V, V, V, V, C.c_size_t, V]
+        L.skv_unpack_patch.argtypes = L.skv_unpack.argtypes
+        L.skv_counts_from_populations.argtypes = [P(skv_shape), C.c_int32, C.c_int32, C.c_int32, C.c_int32, P(skv_counts)]
         L.skv_strerror.argtypes = [C.c_int]
         L.skv_strerror.restype = C.c_char_p
         L.skv_version.restype = C.c_char_p
@@ -213,3 +217,16 @@ def skv_pack(shape, K, V, tier_map, counts, blob, workspace, stream=None):
 def skv_unpack(shape, blob, blob_bytes, counts, K_out, V_out, tier_map_out, workspace, stream=None):
     _check(lib().skv_unpack(C.byref(shape), _ptr(blob), int(blob_bytes), C.byref(counts), _ptr(K_out), _ptr(V_out),
                             _ptr(tier_map_out), _ptr(workspace), _nbytes(workspace), _stream(stream)), "skv_unpack")
+
+
+def skv_unpack_patch(shape, blob, blob_bytes, counts, K_inout, V_inout, tier_map_inout, workspace, stream=None):
+    _check(lib().skv_unpack_patch(C.byref(shape), _ptr(blob), int(blob_bytes), C.byref(counts), _ptr(K_inout),
+                                  _ptr(V_inout), _ptr(tier_map_inout), _ptr(workspace), _nbytes(workspace),
+                                  _stream(stream)), "skv_unpack_patch")
+
+
+def skv_counts_from_populations(shape, n16, n8=0, n4=0, allow_int4=True):
+    c = skv_counts()
+    _check(lib().skv_counts_from_populations(C.byref(shape), int(n16), int(n8), int(n4), 1 if allow_int4 else 0,
+                                             C.byref(c)), "skv_counts_from_populations")
+    return c

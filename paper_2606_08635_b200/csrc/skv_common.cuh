@@ -24,6 +24,7 @@ struct Geom {
     int32_t n16, n8, n4, n0;
     int32_t row_chunks;          // ceil(Hkv*D / 256): 16-byte-per-lane warp chunks in one token row
     int32_t tiles;               // ceil(n / kTileTokens)
+    int32_t patch;               // unpack only: 1 = tokens the blob does not carry (tier 0) are left untouched
 };
 
 constexpr int kTileTokens = 32;  // tokens per pack/unpack tile (one ballot word)

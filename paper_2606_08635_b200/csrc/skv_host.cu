@@ -63,6 +63,7 @@ static Geom make_geom(const skv_shape *s, const skv_counts *c)
     g.n16 = c ? c->n16 : 0; g.n8 = c ? c->n8 : 0; g.n4 = c ? c->n4 : 0; g.n0 = c ? c->n0 : 0;
     g.row_chunks = (g.Hkv * g.D + 255) / 256;
     g.tiles = (g.n + kTileTokens - 1) / kTileTokens;
+    g.patch = 0;
     return g;
 }
 
@@ -282,14 +283,16 @@ int skv_pack(const skv_shape *shape, const void *K_dev, const void *V_dev, const
     return e == cudaSuccess ? SKV_OK : SKV_ERR_CUDA;
 }
 
-int skv_unpack(const skv_shape *shape, const void *blob_dev, size_t blob_bytes, const skv_counts *counts,
-               void *K_out_dev, void *V_out_dev, uint8_t *tier_map_out_dev, void *ws, size_t ws_bytes, void *cuda_stream)
+static int unpack_impl(const skv_shape *shape, const void *blob_dev, size_t blob_bytes, const skv_counts *counts,
+                       void *K_out_dev, void *V_out_dev, uint8_t *tier_map_out_dev, void *ws, size_t ws_bytes,
+                       void *cuda_stream, int patch)
 {
     int rc = check_cache(shape, K_out_dev, V_out_dev);
     if (rc) return rc;
     if (!blob_dev || !ws || !counts_ok(shape, counts)) return SKV_ERR_INVALID_ARG;
     if ((uintptr_t)blob_dev & 255) return SKV_ERR_UNSUPPORTED;
-    const Geom g = make_geom(shape, counts);
+    Geom g = make_geom(shape, counts);
+    g.patch = patch;
     const Layout lo = make_layout(g.L, g.Hkv, g.D, g.n, g.n16, g.n8, g.n4);
     if (blob_bytes != (size_t)lo.total_bytes) return SKV_ERR_BAD_BLOB;
     if (ws_bytes < scan_ws_bytes(shape)) return SKV_ERR_BUFFER_TOO_SMALL;
@@ -299,6 +302,33 @@ int skv_unpack(const skv_shape *shape, const void *blob_dev, size_t blob_bytes, 
     e = launch_unpack(g, lo, (const uint8_t *)blob_dev, lo.total_bytes, (__half *)K_out_dev, (__half *)V_out_dev,
                       (const uint4 *)ws, st);
     return e == cudaSuccess ? SKV_OK : SKV_ERR_CUDA;
+}
+
+int skv_unpack(const skv_shape *shape, const void *blob_dev, size_t blob_bytes, const skv_counts *counts,
+               void *K_out_dev, void *V_out_dev, uint8_t *tier_map_out_dev, void *ws, size_t ws_bytes, void *cuda_stream)
+{
+    return unpack_impl(shape, blob_dev, blob_bytes, counts, K_out_dev, V_out_dev, tier_map_out_dev, ws, ws_bytes, cuda_stream, 0);
+}
+
+int skv_unpack_patch(const skv_shape *shape, const void *blob_dev, size_t blob_bytes, const skv_counts *counts,
+                     void *K_inout_dev, void *V_inout_dev, uint8_t *tier_map_inout_dev, void *ws, size_t ws_bytes,
+                     void *cuda_stream)
+{
+    return unpack_impl(shape, blob_dev, blob_bytes, counts, K_inout_dev, V_inout_dev, tier_map_inout_dev, ws, ws_bytes, cuda_stream, 1);
+}
+
+int skv_counts_from_populations(const skv_shape *shape, int32_t n16, int32_t n8, int32_t n4, int32_t allow_int4,
+                                skv_counts *counts_out)
+{
+    if (!dims_ok(shape) || !counts_out || n16 < 0 || n8 < 0 || n4 < 0) return SKV_ERR_INVALID_ARG;
+    if ((int64_t)n16 + n8 + n4 > (int64_t)shape->n_tokens || (n4 > 0 && !allow_int4)) return SKV_ERR_INVALID_ARG;
+    memset(counts_out, 0, sizeof(*counts_out));
+    counts_out->n16 = n16; counts_out->n8 = n8; counts_out->n4 = n4;
+    counts_out->n0 = shape->n_tokens - n16 - n8 - n4;
+    counts_out->allow_int4 = allow_int4 ? 1 : 0;
+    counts_out->spent_q4 = 4LL * n16 + 2LL * n8 + n4;
+    counts_out->budget_q4 = counts_out->spent_q4;
+    return SKV_OK;
 }
 
 const char *skv_strerror(int status)

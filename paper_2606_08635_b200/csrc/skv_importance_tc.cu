@@ -147,12 +147,13 @@ __device__ __forceinline__ float ex2(float x)
 }
 // 2^x for a PAIR of values on the FMA/ALU pipes with the packed fp32 instructions of sm_100 (FFMA2 / FADD2):
 // n = rint(x) through the 1.5*2^23 constant, f = x - n in [-0.5, 0.5], degree-4 minimax polynomial for 2^f (max
-// relative error 2.7e-6), exponent patched in with one shift-add per value.  x is clamped at -125 (anything below
-// contributes < 2^-125 of the row's reference term).  5.5 issue slots per value and no MUFU.
+// relative error 2.7e-6), exponent patched in with one shift-add per value.  x is clamped to [-125, 128]: anything
+// below contributes < 2^-125 of the row's reference term, anything above yields a value the caller's overflow guard
+// (a < 1e30 is false for huge, Inf and NaN) rejects.  6 issue slots per value and no MUFU.
 __device__ __forceinline__ float2 ex2_fma2(float2 x)
 {
-    x.x = fmaxf(x.x, -125.0f);
-    x.y = fmaxf(x.y, -125.0f);
+    x.x = fminf(fmaxf(x.x, -125.0f), 128.0f);            // upper clamp: x >= 128 must come out as >= 2^127 / Inf / NaN
+    x.y = fminf(fmaxf(x.y, -125.0f), 128.0f);            // (never a wrapped exponent), so the overflow guard sees it
     const float2 t = __fadd2_rn(x, make_float2(12582912.0f, 12582912.0f));
     const float2 nf = __fadd2_rn(t, make_float2(-12582912.0f, -12582912.0f));
     const float2 f = __ffma2_rn(nf, make_float2(-1.0f, -1.0f), x);

@@ -107,7 +107,11 @@ tile_scan_kernel(Geom g, Layout lo, const uint8_t *__restrict__ tier_in /* pack:
         }
     } else if (tier_out != nullptr) {
         uint8_t *tm = tier_out + ((int64_t)r * g.L + l) * n;
-        for (int64_t j = tid; j < n; j += blockDim.x) tm[j] = tier[j];
+        if (g.patch) {                                                   // patch mode: only shipped tokens change tier
+            for (int64_t j = tid; j < n; j += blockDim.x) { const uint8_t t = tier[j]; if (t != 0) tm[j] = t; }
+        } else {
+            for (int64_t j = tid; j < n; j += blockDim.x) tm[j] = tier[j];
+        }
     }
 }
 

@@ -45,6 +45,7 @@ unpack_kernel(Geom g, Layout lo, const uint8_t *__restrict__ blob, uint64_t blob
         else if (t == 8u) { slot = base.y + __popc(m8 & below); if (slot >= (uint32_t)g.n8) t = 0; }
         else if (t == 4u) { slot = base.z + __popc(m4 & below); if (slot >= (uint32_t)g.n4) t = 0; }
         else t = 0;
+        if (t == 0u && g.patch) continue;                             // patch mode (skv_unpack_patch): keep what is there
 
         if (t == 16u) {
             const uint8_t *ks = lbase + lo.seg_off[0] + (uint64_t)slot * row_elems * 2;
@@ -174,6 +175,7 @@ unpack_fast_kernel(Geom g, Layout lo, const uint8_t *__restrict__ blob, uint64_t
         else if (t == 8u) { slot = base.y + __popc(m8 & below); if (slot >= (uint32_t)g.n8) t = 0; }
         else if (t == 4u) { slot = base.z + __popc(m4 & below); if (slot >= (uint32_t)g.n4) t = 0; }
         else t = 0;
+        if (t == 0u && g.patch) continue;                             // patch mode (skv_unpack_patch): keep what is there
 
 #pragma unroll 1
         for (int cb = 0; cb < g.row_chunks; cb += NCH) {

@@ -343,3 +343,73 @@ def test_guard_zones_around_every_output(n, d, Hkv, Hq, w):
         assert bool((raw[:G] == 0x5A).all()) and bool((raw[-G:] == 0x5A).all())
     assert bool((tier_raw[R * L * n:] == 0x5A).all()) and bool((to_raw[R * L * n:] == 0x5A).all())
     assert torch.equal(to_raw[:R * L * n], tier)
+
+
+@pytest.mark.parametrize("order", ["small_then_huge", "huge_then_small", "alternating_blocks"])
+def test_importance_extreme_logit_range(order):
+    """Logits that jump by thousands of log2 units inside a row: the lazily chosen reference exponent of pass 1 must
+    take its overflow-rescue path (and, the other way round, let negligible terms underflow) without leaving the
+    1e-3 band of the float64 oracle.  Keys are scaled per token block; queries are all-positive so that the big
+    keys really dominate."""
+    cfg = skv_synth.Config("xrange", L=1, Hq=4, Hkv=2, d=128, n=1536, w=32, R=1, n_sink=2, seed=21)
+    K, V = skv_synth.make_kv(cfg, 0)
+    Q = skv_synth.make_q(cfg, 0).abs() * 4.0
+    scale = torch.ones(cfg.n)
+    blk = torch.arange(cfg.n) // 128
+    if order == "small_then_huge":
+        scale[:] = 0.01; scale[cfg.n // 2:] = 6.0
+    elif order == "huge_then_small":
+        scale[:] = 6.0; scale[cfg.n // 2:] = 0.01
+    else:
+        scale[:] = torch.where(blk % 2 == 0, torch.tensor(0.01), torch.tensor(6.0))
+    K = (K.float().abs() * scale[None, :, None, None]).half()
+    dev = torch.device("cuda:0")
+    shape = skv.make_shape(1, cfg.Hq, cfg.Hkv, cfg.d, cfg.n, 1)
+    ws = torch.empty(skv.skv_workspace_bytes(shape, cfg.w), dtype=torch.uint8, device=dev)
+    for causal in (True, False):
+        I = torch.full((1, 1, cfg.n), float("nan"), dtype=torch.float32, device=dev)
+        skv.skv_importance(shape, K.to(dev)[None], Q.to(dev)[None], cfg.w, I, ws, causal=causal)
+        Ig = I[0].cpu().numpy().astype(np.float64)
+        Io = oracle.importance(K.numpy(), Q.numpy(), causal=causal).astype(np.float64)
+        assert np.isfinite(Ig).all() and abs(Ig.sum() - 1.0) < 1e-4
+        assert np.all(np.abs(Ig - Io) <= 1e-3 * Io + 1e-30), np.max(np.abs(Ig - Io) / (Io + 1e-30))
+
+
+def test_cold_tier_upgrade_patch():
+    """NEXT-3: upgrade blobs built by skv_pack from an upgrade map and applied in place by skv_unpack_patch, against
+    the oracle: blob bytes, patched K/V and the merged tier map bit-exact; first an FP16 upgrade of some INT4 tokens,
+    then an INT8 'half upgrade' of others on top of it."""
+    dev = torch.device("cuda:0")
+    cfg = C["C3"].scaled(L=3, n=1000, R=2, ranges=())
+    case = Case(cfg, 0.3, with_importance=False)
+    out = gpu_pipeline(case, run_importance=False)
+    shape = case.shape()
+    ws = torch.empty(skv.skv_workspace_bytes(shape, cfg.w), dtype=torch.uint8, device=dev)
+    Kd, Vd = case.K.to(dev), case.V.to(dev)
+    Kc, Vc = torch.from_numpy(out["K2"]).to(dev), torch.from_numpy(out["V2"]).to(dev)      # decode-side dense cache
+    tc = torch.from_numpy(out["tier"]).to(dev)
+    K_or = [case.K2[r].copy() for r in range(case.R)]; V_or = [case.V2[r].copy() for r in range(case.R)]
+    t_or = [case.tier[r].copy() for r in range(case.R)]
+    rng = np.random.default_rng(3)
+    for new_tier, k in ((16, 37), (8, 64)):
+        up = np.zeros((case.R, case.L, cfg.n), np.uint8)
+        for r in range(case.R):
+            for l in range(case.L):
+                cand = np.flatnonzero(t_or[r][l] == 4)
+                up[r, l, rng.choice(cand, size=k, replace=False)] = new_tier
+        pops = (k, 0, 0) if new_tier == 16 else (0, k, 0)
+        uc = skv.skv_counts_from_populations(shape, *pops)
+        assert uc.as_tuple() == (pops[0], pops[1], 0, cfg.n - k)
+        bb = skv.skv_blob_bytes(shape, uc)
+        ublob = torch.full((case.R * bb,), 0xAB, dtype=torch.uint8, device=dev)
+        skv.skv_pack(shape, Kd, Vd, torch.from_numpy(up).to(dev), uc, ublob, ws)
+        skv.skv_unpack_patch(shape, ublob, bb, uc, Kc, Vc, tc, ws)
+        torch.cuda.synchronize()
+        oc = oracle.Counts(pops[0], pops[1], 0, cfg.n - k, uc.budget_q4, uc.spent_q4)
+        for r in range(case.R):
+            blob_or = oracle.pack(case.K[r].numpy(), case.V[r].numpy(), up[r], oc, True)
+            assert np.array_equal(ublob[r * bb:(r + 1) * bb].cpu().numpy(), blob_or)
+            K_or[r], V_or[r], t_or[r] = oracle.unpack_patch(blob_or, K_or[r], V_or[r], t_or[r])
+            assert np.array_equal(Kc[r].cpu().numpy().view(np.uint16), K_or[r].view(np.uint16))
+            assert np.array_equal(Vc[r].cpu().numpy().view(np.uint16), V_or[r].view(np.uint16))
+            assert np.array_equal(tc[r].cpu().numpy(), t_or[r])

@@ -572,3 +572,43 @@ def test_kvnorm_fallback_shape_and_normalisation():
     assert np.allclose(I.astype(np.float64).sum(axis=1), 1.0, atol=1e-6)
     nrm = np.linalg.norm(K.astype(np.float64), axis=-1).mean(axis=-1)
     assert np.allclose(I, nrm / nrm.sum(axis=1, keepdims=True), rtol=1e-6)
+
+
+# ----------------------------------------------------------------------------------------------
+# NEXT-3 cold-tier precision upgrade
+# ----------------------------------------------------------------------------------------------
+def test_upgrade_patch_restores_exact_rows_and_touches_nothing_else():
+    """Pins that need no implementation: (i) an upgraded token's K/V rows equal the original FP16 rows bit for bit,
+    (ii) every other row and tier entry is untouched, (iii) upgrading every non-FP16 token reaches the b = 1 identity
+    in two hops, (iv) the upgrade payload is 2 B per element (Eq. 1 restricted to the upgraded tokens)."""
+    L, n, Hkv, d = 3, 200, 2, 64
+    rng = np.random.default_rng(5)
+    K = rng.standard_normal((L, n, Hkv, d)).astype(np.float16)
+    V = rng.standard_normal((L, n, Hkv, d)).astype(np.float16)
+    counts, prot = oracle.tier_counts(n, 0.3, 4, [], True)
+    I = rng.random((L, n)).astype(np.float32)
+    tier = oracle.assign(I, prot, counts)
+    K1, V1, t1 = oracle.unpack(oracle.pack(K, V, tier, counts, True), L, Hkv, d, n)
+    # upgrade the k highest-scored INT4 tokens of every layer to FP16
+    k = 17
+    up = np.zeros((L, n), np.uint8)
+    for l in range(L):
+        cand = np.flatnonzero(tier[l] == 4)
+        up[l, cand[np.argsort(-I[l, cand], kind="stable")[:k]]] = 16
+    uc = oracle.Counts(k, 0, 0, n - k, 4 * k, 4 * k)
+    ublob = oracle.pack(K, V, up, uc, True)
+    payload = 2 * L * k * Hkv * d * 2
+    assert payload <= ublob.size <= payload + 256 + (L * n + 255) // 256 * 256 + L * 10 * 256     # 2 B/elem + framing
+    K2, V2, t2 = oracle.unpack_patch(ublob, K1, V1, t1)
+    m = up == 16
+    assert np.array_equal(K2[m].view(np.uint16), K[m].view(np.uint16)) and np.array_equal(V2[m].view(np.uint16), V[m].view(np.uint16))
+    assert np.array_equal(K2[~m].view(np.uint16), K1[~m].view(np.uint16)) and np.array_equal(V2[~m].view(np.uint16), V1[~m].view(np.uint16))
+    assert (t2[m] == 16).all() and np.array_equal(t2[~m], t1[~m])
+    assert not np.array_equal(K2[m].view(np.uint16), K1[m].view(np.uint16))                  # the INT4 rows really differed
+    # upgrade everything that is not FP16 yet -> identity
+    up_all = np.where(tier != 16, 16, 0).astype(np.uint8)
+    k_all = int((up_all[0] == 16).sum())
+    ac = oracle.Counts(k_all, 0, 0, n - k_all, 4 * k_all, 4 * k_all)
+    K3, V3, t3 = oracle.unpack_patch(oracle.pack(K, V, up_all, ac, True), K1, V1, t1)
+    assert np.array_equal(K3.view(np.uint16), K.view(np.uint16)) and np.array_equal(V3.view(np.uint16), V.view(np.uint16))
+    assert (t3 == 16).all()
