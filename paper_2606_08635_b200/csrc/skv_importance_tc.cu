@@ -591,7 +591,7 @@ static cudaError_t launch_tc_t(const Geom &g, const CUtensorMap &tmK, const CUte
     return cudaGetLastError();
 }
 
-// Returns cudaErrorNotSupported when the tensor maps cannot be built (caller falls back to the mma.sync kernels).
+// Returns cudaErrorNotSupported when the tensor maps cannot be built (reported as SKV_ERR_CUDA; there is no other path).
 cudaError_t launch_importance_tc(const Geom &g, const __half *K, const __half *Q, int window, int causal, float lambda,
                                  float *importance, void *ws, cudaStream_t s)
 {
