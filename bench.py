@@ -41,6 +41,7 @@ def parse_args():
     ap.add_argument("--requests", type=int, default=None)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-next", action="store_true", help="skip the timings of the NEXT rows (kvnorm score, upgrade)")
     ap.add_argument("--e2e-chunk-layers", type=int, default=4, help="layers per pipelined transfer chunk")
     ap.add_argument("--e2e-depth", type=int, default=3, help="device slots of the pipelined transfer")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
@@ -235,6 +236,43 @@ class DeviceProblem:
         blob = self.blob_bytes * self.R
         tm = self.cfg.L * self.cfg.n * self.R
         return {"pack": fp16 + blob + tm, "unpack": blob + fp16 + tm}
+
+
+def run_next_rows(prob, steps):
+    """SURVEY.md 8(f) rows at the same workload, outside the timed step: NEXT-1 KV-norm fallback score (reads K once)
+    and NEXT-3 cold-tier upgrade (FP16 upgrade blob of 1024 tokens per layer: skv_pack + skv_unpack_patch)."""
+    import torch
+    skv, cfg, R = prob.skv, prob.cfg, prob.R
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    out = {}
+    a, b_ = ev(), ev()
+    skv.skv_importance_kvnorm(prob.shape, prob.K, prob.I, prob.ws)
+    a.record()
+    for _ in range(steps):
+        skv.skv_importance_kvnorm(prob.shape, prob.K, prob.I, prob.ws)
+    b_.record(); torch.cuda.synchronize()
+    ms = a.elapsed_time(b_) / steps
+    kbytes = cfg.bytes_fp16 * R // 2
+    out["kvnorm"] = {"ms": ms, "algorithmic_bytes": kbytes, "GBps": kbytes / (ms * 1e-3) / 1e9}
+    k = min(1024, cfg.n // 4)
+    up = torch.zeros((R, cfg.L, cfg.n), dtype=torch.uint8, device=prob.dev)
+    up[:, :, cfg.n // 2:cfg.n // 2 + 2 * k:2] = 16                      # every other token of a 2k window
+    uc = skv.skv_counts_from_populations(prob.shape, k)
+    bb = skv.skv_blob_bytes(prob.shape, uc)
+    ublob = torch.empty((R, bb), dtype=torch.uint8, device=prob.dev)
+    def once():
+        skv.skv_pack(prob.shape, prob.K, prob.V, up, uc, ublob, prob.ws)
+        skv.skv_unpack_patch(prob.shape, ublob, bb, uc, prob.Ko, prob.Vo, prob.tier_out, prob.ws)
+    once()
+    a.record()
+    for _ in range(steps):
+        once()
+    b_.record(); torch.cuda.synchronize()
+    ms = a.elapsed_time(b_) / steps
+    moved = 2 * R * bb                                                  # rows read + blob written, blob read + rows written
+    out["upgrade"] = {"tokens_per_layer": k, "blob_bytes_per_request": bb, "ms_pack_plus_patch": ms,
+                      "GBps": 2 * moved / (ms * 1e-3) / 1e9}
+    return out
 
 
 def run_e2e(cfg, b, R, dev, steps, warmup, chunk_layers=4, depth=3):
@@ -433,6 +471,7 @@ def main():
     ms_step, (ms_imp, ms_asg, ms_pack, ms_unpack) = red[0], red[1:]
     value = bytes_all / ((ms_pack + ms_unpack) * 1e-3) / 1e9
 
+    next_rows = None if args.no_next else run_next_rows(prob, min(K, 10))
     e2e = None
     if not args.no_e2e:
         r = run_e2e(cfg, b, R, dev, steps=min(K, 3), warmup=1, chunk_layers=args.e2e_chunk_layers, depth=args.e2e_depth)
@@ -472,6 +511,10 @@ def main():
                        "note": "two-pass: the contraction and the exponentials run twice"},
         "clocks": clocks, "gpu_launches": LAUNCHES_PER_STEP * K, "wall_s_timed_region": t_wall,
     }
+    if next_rows is not None:
+        for v in next_rows.values():
+            v["frac_of_hbm_peak"] = v["GBps"] / peak
+        line["next_rows"] = next_rows
     if e2e is not None:
         line["e2e"] = e2e
     if not args.no_cpu_baseline and world == 1:

@@ -20,26 +20,46 @@ kvnorm_kernel(Geom g, const __half *__restrict__ K, float *__restrict__ raw /*[R
 {
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int l = blockIdx.y, r = blockIdx.z;
-    const int64_t j = (int64_t)blockIdx.x * 8 + warp;
+    const int lpv = g.D / 8;
+    const int hpc = 256 / g.D;                                           // head vectors per 256-element chunk
+    const int lane_h = (int)(lane * 8) / g.D, lane_c = (int)(lane * 8) % g.D;   // D is 64, 128 or 256: once per thread
+    const int64_t lane_off = (int64_t)lane_h * g.sh + lane_c, chunk_stride = (int64_t)hpc * g.sh;
+    // 64 tokens per CTA (8 per warp, interleaved so that the warps of a CTA stream adjacent rows): fat enough that
+    // the grid is not CTA-launch-bound
+    for (int it = 0; it < 8; ++it) {
+    const int64_t j = (int64_t)blockIdx.x * 64 + it * 8 + warp;
     if (j >= g.n) return;
     const __half *row = K + (int64_t)r * g.sr + (int64_t)l * g.sl + j * g.st;
-    const int lpv = g.D / 8;
     float acc = 0.f;
-    for (int e0 = 0; e0 < g.Hkv * g.D; e0 += 256) {
-        const int e = e0 + lane * 8;
-        float ss = 0.f;
-        if (e < g.Hkv * g.D) {
-            const uint4 v = *reinterpret_cast<const uint4 *>(row + (int64_t)(e / g.D) * g.sh + (e % g.D));
-            const __half2 *h = reinterpret_cast<const __half2 *>(&v);
+    const int row_elems = g.Hkv * g.D;
+    for (int e0 = 0; e0 < row_elems; e0 += 1024) {                       // four 16-byte loads in flight per lane
+        uint4 v[4];
 #pragma unroll
-            for (int k = 0; k < 4; ++k) { const float2 f = __half22float2(h[k]); ss += f.x * f.x + f.y * f.y; }
+        for (int u = 0; u < 4; ++u) {
+            const int e = e0 + u * 256 + lane * 8;
+            v[u] = make_uint4(0, 0, 0, 0);
+            if (e < row_elems) {
+                const __half *p = row + (int64_t)((e0 >> 8) + u) * chunk_stride + lane_off;
+                asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+                             : "=r"(v[u].x), "=r"(v[u].y), "=r"(v[u].z), "=r"(v[u].w) : "l"(p));
+            }
         }
-        for (int o = 1; o < lpv; o <<= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
-        if ((lane % lpv) == 0 && e < g.Hkv * g.D) acc += sqrtf(ss);
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int e = e0 + u * 256 + lane * 8;
+            const __half2 *h = reinterpret_cast<const __half2 *>(&v[u]);
+            float2 s2 = make_float2(0.f, 0.f);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) { const float2 f = __half22float2(h[k]); s2 = __ffma2_rn(f, f, s2); }
+            float ss = s2.x + s2.y;
+            for (int o = 1; o < lpv; o <<= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
+            if ((lane % lpv) == 0 && e < row_elems) acc += sqrtf(ss);
+        }
     }
 #pragma unroll
     for (int o = 16; o >= 1; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
     if (lane == 0) raw[((int64_t)r * g.L + l) * g.n + j] = acc / (float)g.Hkv;
+    }
 }
 
 __global__ void __launch_bounds__(1024)
@@ -92,7 +112,7 @@ cudaError_t launch_importance(const Geom &g, const __half *K, const __half *Q, i
 cudaError_t launch_importance_kvnorm(const Geom &g, const __half *K, float lambda, float *importance, float *ws,
                                      cudaStream_t s)
 {
-    dim3 g1((g.n + 7) / 8, g.L, g.R);
+    dim3 g1((g.n + 63) / 64, g.L, g.R);
     kvnorm_kernel<<<g1, 256, 0, s>>>(g, K, ws);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
