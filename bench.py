@@ -48,6 +48,15 @@ def parse_args():
     return ap.parse_args()
 
 
+def measured_tensor_peak():
+    """(sustained dense bf16/fp16 TFLOP/s, source) -- the importance kernels run inside a long step."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["bf16_tflops_sustained"]), "measured (MEASURED_PEAKS.json bf16_tflops_sustained)"
+    except Exception:
+        return 1400.0, "fallback (B200_PROFILING.md, sustained)"
+
+
 def measured_peak():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     try:
@@ -538,7 +547,11 @@ def main():
                      "frac_of_nominal_8TBs": achieved / 8000.0},
         "importance": {"ms": ms_imp, "useful_tflops": 2.0 * cfg.L * cfg.Hq * cfg.w * cfg.n * cfg.d * R / (ms_imp * 1e-3) / 1e12,
                        "executed_tflops": 4.0 * cfg.L * cfg.Hq * cfg.w * cfg.n * cfg.d * R / (ms_imp * 1e-3) / 1e12,
-                       "note": "two-pass: the contraction and the exponentials run twice"},
+                       "note": "two-pass: the contraction and the exponentials run twice; bound by the MUFU ex2 / FMA / "
+                               "tensor pipe mix at d_h = 128 (profiles/r1_full_v3_ncu.md), not by the tensor pipe alone",
+                       "tensor_peak_tflops": measured_tensor_peak()[0], "tensor_peak_source": measured_tensor_peak()[1],
+                       "useful_frac_of_tensor_peak": 2.0 * cfg.L * cfg.Hq * cfg.w * cfg.n * cfg.d * R / (ms_imp * 1e-3) / 1e12 / measured_tensor_peak()[0],
+                       "executed_frac_of_tensor_peak": 4.0 * cfg.L * cfg.Hq * cfg.w * cfg.n * cfg.d * R / (ms_imp * 1e-3) / 1e12 / measured_tensor_peak()[0]},
         "clocks": clocks, "gpu_launches": LAUNCHES_PER_STEP * K, "wall_s_timed_region": t_wall,
     }
     if next_rows is not None:
