@@ -413,3 +413,34 @@ def test_cold_tier_upgrade_patch():
             assert np.array_equal(Kc[r].cpu().numpy().view(np.uint16), K_or[r].view(np.uint16))
             assert np.array_equal(Vc[r].cpu().numpy().view(np.uint16), V_or[r].view(np.uint16))
             assert np.array_equal(tc[r].cpu().numpy(), t_or[r])
+
+
+def test_layer_pipelined_transfer_ragged_batch():
+    """NEXT-2, ragged batch: three requests of different lengths through one pipeline (slots sized for the longest);
+    each comes back exactly as the oracle's pack -> unpack of the tier map assigned from the GPU's own scores."""
+    from paper_2606_08635_b200.transfer import LayerPipelinedTransfer
+    base = C["C5"].scaled(L=3, R=1)
+    ns = (1000, 257, 640)
+    pipe = LayerPipelinedTransfer(3, base.Hq, base.Hkv, base.d, max(ns), base.w, 0.4, base.n_sink, (), base.allow_int4,
+                                  layers_per_chunk=2, depth=2)
+    reqs, cases = [], []
+    for r, n in enumerate(ns):
+        cfg = base.scaled(n=n, seed=30 + r)
+        K, V = skv_synth.make_kv(cfg, 0)
+        Q = skv_synth.make_q(cfg, 0)
+        cases.append((cfg, K, V, Q))
+        nan = lambda t: torch.full(t.shape, float("nan"), dtype=torch.float16, pin_memory=True)
+        reqs.append(dict(K=K.pin_memory(), V=V.pin_memory(), Q=Q.pin_memory(), Ko=nan(K), Vo=nan(V),
+                         I=torch.full((3, n), float("nan"), dtype=torch.float32, pin_memory=True),
+                         T=torch.full((3, n), 0xEE, dtype=torch.uint8, pin_memory=True)))
+    pipe.run_ragged(reqs)
+    for (cfg, K, V, Q), req in zip(cases, reqs):
+        counts, prot = oracle.tier_counts(cfg.n, 0.4, cfg.n_sink, (), cfg.allow_int4)
+        Ig = req["I"].numpy()
+        Io = oracle.importance(K.numpy(), Q.numpy()).astype(np.float64)
+        assert np.all(np.abs(Ig - Io) <= 1e-3 * Io + 1e-30)
+        tier = oracle.assign(Ig, prot, counts)
+        assert np.array_equal(tier, req["T"].numpy())
+        K2, V2, _ = oracle.unpack(oracle.pack(K.numpy(), V.numpy(), tier, counts, cfg.allow_int4), 3, cfg.Hkv, cfg.d, cfg.n)
+        assert np.array_equal(req["Ko"].numpy().view(np.uint16), K2.view(np.uint16))
+        assert np.array_equal(req["Vo"].numpy().view(np.uint16), V2.view(np.uint16))
