@@ -444,3 +444,16 @@ def test_layer_pipelined_transfer_ragged_batch():
         K2, V2, _ = oracle.unpack(oracle.pack(K.numpy(), V.numpy(), tier, counts, cfg.allow_int4), 3, cfg.Hkv, cfg.d, cfg.n)
         assert np.array_equal(req["Ko"].numpy().view(np.uint16), K2.view(np.uint16))
         assert np.array_equal(req["Vo"].numpy().view(np.uint16), V2.view(np.uint16))
+
+
+@pytest.mark.parametrize("n,b,a4", [(70001, 0.4, True), (131072, 0.3, False)])
+def test_long_sequences_beyond_the_shared_memory_selection_path(n, b, a4):
+    """n > 51200 tokens: the selection kernel keeps its keys in the global workspace instead of shared memory (and
+    the scan walks > 2000 tiles per layer); seeded stand-in scores with many exact duplicates, bit-exact against the
+    oracle through assign -> pack -> unpack."""
+    cfg = skv_synth.Config("long", L=2, Hq=2, Hkv=1, d=64, n=n, w=8, R=1, n_sink=4, seed=41, allow_int4=a4)
+    rng = np.random.default_rng(n)
+    I = rng.integers(0, 5000, size=(1, 2, n)).astype(np.float32) * np.float32(1e-5)      # ~14-26 duplicates per value
+    case = Case(cfg, b, with_importance=False, importance_override=I)
+    out = gpu_pipeline(case, run_importance=False)
+    assert_bit_exact(case, out)
