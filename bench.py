@@ -281,6 +281,25 @@ def run_next_rows(prob, steps):
     moved = 2 * R * bb                                                  # rows read + blob written, blob read + rows written
     out["upgrade"] = {"tokens_per_layer": k, "blob_bytes_per_request": bb, "ms_pack_plus_patch": ms,
                       "GBps": 2 * moved / (ms * 1e-3) / 1e9}
+    del ublob, up
+    # NEXT-4: the same caches with an asymmetric 2-bit low tier at b = 0.2 (INT8 + 2-bit mix, budget in eighths)
+    pol2 = skv.make_policy(0.2, cfg.n_sink, cfg.ranges, 2)
+    c2 = skv.skv_assign_tiers(prob.shape, pol2, prob.I, prob.tier, prob.ws)
+    bb2 = skv.skv_blob_bytes(prob.shape, c2)
+    blob2 = torch.empty((R, bb2), dtype=torch.uint8, device=prob.dev)
+    def once2():
+        skv.skv_pack(prob.shape, prob.K, prob.V, prob.tier, c2, blob2, prob.ws)
+        skv.skv_unpack(prob.shape, blob2, bb2, c2, prob.Ko, prob.Vo, prob.tier_out, prob.ws)
+    once2()
+    a.record()
+    for _ in range(steps):
+        once2()
+    b_.record(); torch.cuda.synchronize()
+    ms = a.elapsed_time(b_) / steps
+    moved2 = 2 * (cfg.bytes_fp16 * R + R * bb2 + cfg.L * cfg.n * R)
+    out["two_bit_low_tier"] = {"budget": 0.2, "counts": list(c2.as_tuple()), "blob_bytes_per_request": bb2,
+                               "ms_pack_plus_unpack": ms, "GBps": moved2 / (ms * 1e-3) / 1e9,
+                               "GBps_of_fp16_kv": cfg.bytes_fp16 * R / (ms * 1e-3) / 1e9}
     return out
 
 

@@ -34,7 +34,7 @@
  * back at stride skv_blob_bytes(); the paper only says "mixed-precision payload"):
  *
  *   [0,256)  header: 0 u32 magic 0x31564B53 ("SKV1"), 4 u32 version = 1, 8 u32 L, 12 u32 Hkv, 16 u32 d_h,
- *            20 u32 n, 24 u32 n16, 28 u32 n8, 32 u32 n4, 36 u32 n0, 40 u32 flags (bit0 = allow_int4),
+ *            20 u32 n, 24 u32 n16, 28 u32 n8, 32 u32 n4, 36 u32 n0, 40 u32 flags (bit0 = allow_int4, bit1 = 2-bit low tier),
  *            44 u32 0, 48 u64 budget in quarter-units, 56 u64 tier_map_off (= 256), 64 u64 layer0_off,
  *            72 u64 layer_stride, 80 u64 seg_off[10] (relative to the layer block), 160 u64 total_bytes,
  *            168..255 zero
@@ -44,6 +44,14 @@
  *            SK8,SV8 : f16 amax [n8][Hkv]      SK4,SV4 : f16 amax [n4][Hkv]
  *   Slot order inside a tier = ascending token position.  INT4 byte i holds element 2i in the low nibble
  *   and 2i+1 in the high nibble (4-bit two's complement).  Dropped tokens occupy no bytes.
+ *
+ * 2-bit low tier (NEXT-4; "the INT4 tier could use KIVI-style asymmetric 2-bit quantization"): with
+ * allow_int4 = 2 the low tier of a blob is coded in 2 bits instead of 4.  Its tier code is 2, header flags = 3,
+ * K4/V4 hold four codes per byte (element 4i+k in bits 2k..2k+1 of byte i), SK4/SV4 hold an fp16 (lo, hi) pair per
+ * head vector, and the budget runs in EIGHTH-units (8 / 4 / 1 / 0 per token; budget_q4 and spent_q4 are then
+ * eighths).  Quantiser: lo = min x, hi = max x (a zero of either sign recorded as +0), r = fl32(hi - lo),
+ * inv = fl32(3/r), step = fl32(r/3) (0 when r = 0); q = clamp(rint(fl32(x - lo) * inv), 0, 3), the product exact and
+ * rounded once, half to even; y = f16_rn(fma(q, step, lo)).
  *
  * Quantiser (one group = one head vector of d_h values; qmax = 127 / 7):
  *   amax = max|x| (an fp16 value, stored as the 2-byte scale record);
@@ -89,11 +97,13 @@ typedef struct {
     int32_t n_sink;           /* s: positions [0,s) forced FP16 */
     int32_t n_ranges;         /* number of protected ranges */
     const int32_t *ranges;    /* HOST, n_ranges x [begin,end) half-open, forced FP16; read during the call only */
-    int32_t allow_int4;       /* probe result: 1 = 3-tier, 0 = 2-tier FP16+INT8(+drop) */
+    int32_t allow_int4;       /* probe result: 1 = 3-tier, 0 = 2-tier FP16+INT8(+drop);
+                                 2 = 3-tier whose low tier is asymmetric 2-bit (NEXT-4) */
 } skv_policy;
 
 /* Tier populations of ONE layer of ONE request (identical for every layer and request of a batch,
- * because n, b and the protected set are).  budget_q4 = floor(4bn + 1e-6), spent_q4 = 4n16+2n8+n4. */
+ * because n, b and the protected set are).  budget_q4 = floor(4bn + 1e-6), spent_q4 = 4n16+2n8+n4; with
+ * allow_int4 = 2, n4 is the population of the 2-bit tier and both are in eighths: floor(8bn + 1e-6), 8n16+4n8+n4. */
 typedef struct {
     int32_t n16, n8, n4, n0;
     int32_t allow_int4, reserved;

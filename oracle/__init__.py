@@ -26,6 +26,7 @@ def lib():
         _lib.orc_float_to_half.restype = C.c_uint16
         _lib.orc_float_to_half.argtypes = [C.c_float]
         _lib.orc_blob_bytes.restype = C.c_uint64
+        _lib.orc_blob_bytes_low.restype = C.c_uint64
         _lib.orc_max_threads.restype = C.c_int
     return _lib
 
@@ -46,8 +47,9 @@ class Counts:
     n8: int
     n4: int
     n0: int
-    budget_q4: int
+    budget_q4: int            # quarter-units; EIGHTH-units when low_bits == 2
     spent_q4: int
+    low_bits: int = 4         # 4 = symmetric INT4 low tier (tier code 4); 2 = asymmetric 2-bit (tier code 2, NEXT-4)
 
     def arr(self):
         return (C.c_int64 * 6)(self.n16, self.n8, self.n4, self.n0, self.budget_q4, self.spent_q4)
@@ -69,6 +71,11 @@ def set_threads(t: int) -> None:
     lib().orc_set_threads(C.c_int(int(t)))
 
 
+def _mode(allow_int4):
+    """allow_int4: False/0 = 2-tier, True/1 = symmetric INT4 low tier, 2 = asymmetric 2-bit low tier (NEXT-4)."""
+    return 2 if (allow_int4 == 2 and allow_int4 is not True) else (1 if allow_int4 else 0)
+
+
 def tier_counts(n, b, n_sink=0, ranges=(), allow_int4=True):
     """O2.  Returns (Counts, protected bitmap uint8[n]).  Raises ValueError on infeasible/invalid."""
     rng = np.asarray(ranges, dtype=np.int32).reshape(-1, 2)
@@ -76,10 +83,10 @@ def tier_counts(n, b, n_sink=0, ranges=(), allow_int4=True):
     prot = np.zeros(int(n), dtype=np.uint8)
     rc = lib().orc_tier_counts(C.c_int64(int(n)), C.c_double(float(b)), C.c_int32(int(n_sink)),
                                C.c_int32(len(rng)), _p(np.ascontiguousarray(rng)),
-                               C.c_int32(1 if allow_int4 else 0), out, _p(prot))
+                               C.c_int32(_mode(allow_int4)), out, _p(prot))
     if rc != 0:
         raise ValueError(f"orc_tier_counts rc={rc}")
-    return Counts(*[int(v) for v in out]), prot
+    return Counts(*[int(v) for v in out], low_bits=2 if _mode(allow_int4) == 2 else 4), prot
 
 
 def importance(K, Q, causal=True, lam=0.0):
@@ -112,13 +119,14 @@ def assign(I, prot, counts: Counts):
     L, n = I.shape
     tier = np.empty((L, n), dtype=np.uint8)
     c4 = (C.c_int64 * 4)(counts.n16, counts.n8, counts.n4, counts.n0)
-    lib().orc_assign(C.c_int32(L), C.c_int64(n), _p(I), _p(prot), c4, _p(tier))
+    lib().orc_assign_low(C.c_int32(L), C.c_int64(n), _p(I), _p(prot), c4, C.c_int32(counts.low_bits), _p(tier))
     return tier
 
 
 def blob_bytes(L, Hkv, d, n, counts: Counts) -> int:
     c4 = (C.c_int64 * 4)(counts.n16, counts.n8, counts.n4, counts.n0)
-    return int(lib().orc_blob_bytes(C.c_int32(L), C.c_int32(Hkv), C.c_int32(d), C.c_int64(n), c4))
+    return int(lib().orc_blob_bytes_low(C.c_int32(L), C.c_int32(Hkv), C.c_int32(d), C.c_int64(n), c4,
+                                        C.c_int32(counts.low_bits)))
 
 
 def pack(K, V, tier, counts: Counts, allow_int4=True):
@@ -130,7 +138,7 @@ def pack(K, V, tier, counts: Counts, allow_int4=True):
     assert V.shape == K.shape and tier.shape == (L, n)
     blob = np.empty(blob_bytes(L, Hkv, d, n, counts), dtype=np.uint8)
     rc = lib().orc_pack(C.c_int32(L), C.c_int32(Hkv), C.c_int32(d), C.c_int64(n), _p(K), _p(V),
-                        _p(tier), counts.arr(), C.c_int32(1 if allow_int4 else 0), _p(blob))
+                        _p(tier), counts.arr(), C.c_int32(2 if counts.low_bits == 2 else _mode(allow_int4)), _p(blob))
     if rc != 0:
         raise ValueError(f"orc_pack rc={rc} (tier map does not match counts)")
     return blob
@@ -162,6 +170,22 @@ def unpack_patch(blob, K, V, tier):
     if rc != 0:
         raise ValueError(f"orc_unpack_patch rc={rc} (bad blob)")
     return K, V, tier
+
+
+def quantize2_vector(x):
+    """NEXT-4 asymmetric 2-bit quantizer on one vector.  x float16[d] -> (lo_bits, hi_bits, uint8[d] codes 0..3)."""
+    x = _c(x, np.float16)
+    q = np.empty(x.size, dtype=np.uint8)
+    lo, hi = C.c_uint16(0), C.c_uint16(0)
+    lib().orc_quantize2_vector(_p(x), C.c_int32(x.size), C.byref(lo), C.byref(hi), _p(q))
+    return int(lo.value), int(hi.value), q
+
+
+def dequantize2_vector(q, lo_bits, hi_bits):
+    q = _c(q, np.uint8)
+    y = np.empty(q.size, dtype=np.float16)
+    lib().orc_dequantize2_vector(_p(q), C.c_int32(q.size), C.c_uint16(int(lo_bits)), C.c_uint16(int(hi_bits)), _p(y))
+    return y
 
 
 def quantize_vector(x, qmax):

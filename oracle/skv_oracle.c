@@ -160,6 +160,21 @@ int orc_tier_counts(int64_t n, double b, int32_t n_sink, int32_t n_ranges, const
     for (int64_t j = 0; j < n; ++j) P += p[j];
     if (!prot) free(p);
 
+    if (allow_int4 == 2) {
+        /* NEXT-4 ("the INT4 tier could use KIVI-style asymmetric 2-bit quantization"): the low tier
+         * costs c = 1/8, so the same greedy ladder runs in EIGHTH-units, 8 / 4 / 1 / 0 per token (reading P18). */
+        const int64_t Q8 = (int64_t)floor(8.0 * b * (double)n + 1e-6);
+        const int64_t m8 = n - P, R8 = Q8 - 8 * P;
+        if (R8 < 0) return -3;
+        int64_t a16 = P, a8 = 0, a2 = 0, a0 = 0;
+        if (R8 >= 8 * m8) a16 = n;
+        else if (R8 >= 4 * m8) { int64_t extra = (R8 - 4 * m8) / 4; a16 = P + extra; a8 = m8 - extra; }
+        else if (R8 >= m8) { a8 = (R8 - m8) / 3; a2 = m8 - a8; }      /* each INT8 upgrade over 2-bit costs 3 */
+        else { a2 = R8; a0 = m8 - R8; }
+        out[0] = a16; out[1] = a8; out[2] = a2; out[3] = a0;
+        out[4] = Q8;  out[5] = 8 * a16 + 4 * a8 + a2;
+        return 0;
+    }
     const int64_t Q = (int64_t)floor(4.0 * b * (double)n + 1e-6);
     const int64_t m = n - P;
     const int64_t R = Q - 4 * P;             /* budget left after paying FP16 for the protected set */
@@ -205,8 +220,8 @@ static int orc_item_cmp(const void *a, const void *b)
 }
 
 /* One layer: I[n], prot[n] -> tier[n]; counts = {n16,n8,n4,n0} from orc_tier_counts. */
-void orc_assign_layer(int64_t n, const float *I, const uint8_t *prot, const int64_t counts[4],
-                      uint8_t *tier)
+static void orc_assign_layer_code(int64_t n, const float *I, const uint8_t *prot, const int64_t counts[4],
+                                  uint8_t low_code, uint8_t *tier)
 {
     orc_item *it = (orc_item *)malloc((size_t)n * sizeof(orc_item));
     int64_t m = 0, P = 0;
@@ -222,19 +237,32 @@ void orc_assign_layer(int64_t n, const float *I, const uint8_t *prot, const int6
         uint8_t t;
         if (r < c16) t = 16;
         else if (r < c16 + c8) t = 8;
-        else if (r < c16 + c8 + c4) t = 4;
+        else if (r < c16 + c8 + c4) t = low_code;      /* 4 (symmetric INT4) or 2 (asymmetric 2-bit, NEXT-4) */
         else t = 0;
         tier[it[r].pos] = t;
     }
     free(it);
 }
 
-void orc_assign(int32_t L, int64_t n, const float *I, const uint8_t *prot, const int64_t counts[4],
-                uint8_t *tier)
+void orc_assign_layer(int64_t n, const float *I, const uint8_t *prot, const int64_t counts[4],
+                      uint8_t *tier)
+{
+    orc_assign_layer_code(n, I, prot, counts, 4, tier);
+}
+
+/* low_bits: 4 = the low tier is symmetric INT4 (tier code 4); 2 = asymmetric 2-bit (tier code 2). */
+void orc_assign_low(int32_t L, int64_t n, const float *I, const uint8_t *prot, const int64_t counts[4],
+                    int32_t low_bits, uint8_t *tier)
 {
 #pragma omp parallel for schedule(dynamic, 1)
     for (int32_t l = 0; l < L; ++l)
-        orc_assign_layer(n, I + (size_t)l * n, prot, counts, tier + (size_t)l * n);
+        orc_assign_layer_code(n, I + (size_t)l * n, prot, counts, (uint8_t)(low_bits == 2 ? 2 : 4), tier + (size_t)l * n);
+}
+
+void orc_assign(int32_t L, int64_t n, const float *I, const uint8_t *prot, const int64_t counts[4],
+                uint8_t *tier)
+{
+    orc_assign_low(L, n, I, prot, counts, 4, tier);
 }
 
 /* ------------------------------------------------------------------------ */
@@ -247,17 +275,20 @@ typedef struct {
 
 static uint64_t pad256(uint64_t x) { return (x + 255u) / 256u * 256u; }
 
-/* segment order: K16 V16 K8 V8 K4 V4 SK8 SV8 SK4 SV4 */
-void orc_layout(int32_t L, int32_t Hkv, int32_t d, int64_t n, const int64_t counts[4], orc_layout_t *lo)
+/* segment order: K16 V16 K8 V8 K4 V4 SK8 SV8 SK4 SV4.  With low_bits = 2 (NEXT-4) the low-tier segments hold four
+ * 2-bit codes per byte and a (lo, hi) pair of fp16 records per head vector. */
+void orc_layout_low(int32_t L, int32_t Hkv, int32_t d, int64_t n, const int64_t counts[4], int32_t low_bits,
+                    orc_layout_t *lo)
 {
     const uint64_t n16 = (uint64_t)counts[0], n8 = (uint64_t)counts[1], n4 = (uint64_t)counts[2];
     const uint64_t H = (uint64_t)Hkv, D = (uint64_t)d;
+    const uint64_t cpb = (low_bits == 2) ? 4 : 2, rec = (low_bits == 2) ? 4 : 2;
     const uint64_t raw[10] = {
         n16 * H * D * 2, n16 * H * D * 2,      /* K16, V16 : f16            */
         n8 * H * D,      n8 * H * D,           /* K8,  V8  : i8             */
-        n4 * H * D / 2,  n4 * H * D / 2,       /* K4,  V4  : two codes/byte */
+        n4 * H * D / cpb, n4 * H * D / cpb,    /* K4,  V4  : two (INT4) or four (2-bit) codes per byte */
         n8 * H * 2,      n8 * H * 2,           /* SK8, SV8 : f16 amax       */
-        n4 * H * 2,      n4 * H * 2 };         /* SK4, SV4 : f16 amax       */
+        n4 * H * rec,    n4 * H * rec };       /* SK4, SV4 : f16 amax, or f16 (lo, hi) for 2-bit */
     lo->tier_map_off = 256;
     lo->layer0_off = 256 + pad256((uint64_t)L * (uint64_t)n);
     uint64_t off = 0;
@@ -266,9 +297,19 @@ void orc_layout(int32_t L, int32_t Hkv, int32_t d, int64_t n, const int64_t coun
     lo->total_bytes = lo->layer0_off + (uint64_t)L * lo->layer_stride;
 }
 
+void orc_layout(int32_t L, int32_t Hkv, int32_t d, int64_t n, const int64_t counts[4], orc_layout_t *lo)
+{
+    orc_layout_low(L, Hkv, d, n, counts, 4, lo);
+}
+
+uint64_t orc_blob_bytes_low(int32_t L, int32_t Hkv, int32_t d, int64_t n, const int64_t counts[4], int32_t low_bits)
+{
+    orc_layout_t lo; orc_layout_low(L, Hkv, d, n, counts, low_bits, &lo); return lo.total_bytes;
+}
+
 uint64_t orc_blob_bytes(int32_t L, int32_t Hkv, int32_t d, int64_t n, const int64_t counts[4])
 {
-    orc_layout_t lo; orc_layout(L, Hkv, d, n, counts, &lo); return lo.total_bytes;
+    return orc_blob_bytes_low(L, Hkv, d, n, counts, 4);
 }
 
 static void put_u32(uint8_t *p, uint32_t v) { for (int i = 0; i < 4; ++i) p[i] = (uint8_t)(v >> (8 * i)); }
@@ -323,6 +364,46 @@ void orc_dequantize_vector(const int8_t *q, int32_t d, int32_t qmax, uint16_t am
     }
 }
 
+/*
+ * NEXT-4: asymmetric 2-bit quantizer for the low tier ("the INT4 tier could use KIVI-style asymmetric 2-bit
+ * quantization instead of standard symmetric INT4"; reading P19 of DESIGN.md -- the paper gives no
+ * arithmetic).  One group = one head vector.  lo = min x, hi = max x (fp16 values, stored losslessly as the two
+ * 2-byte records; a zero of either sign is stored as +0).  r = fl32(hi - lo), step = fl32(r / 3), inv = fl32(3 / r)
+ * (both 0 when r = 0).  q = clamp(rint(fl32(x - lo) * inv), 0, 3), the product exact and rounded once, half to even
+ * (as P8).  y = f16_rn(fma(q, step, lo)), the fused multiply-add rounded once to binary32.
+ */
+void orc_quantize2_vector(const uint16_t *x, int32_t d, uint16_t *lo_out, uint16_t *hi_out, uint8_t *q)
+{
+    float lo = orc_half_to_float(x[0]), hi = lo;
+    for (int32_t c = 1; c < d; ++c) { const float v = orc_half_to_float(x[c]); if (v < lo) lo = v; if (v > hi) hi = v; }
+    if (lo == 0.0f) lo = 0.0f * 0.0f;                    /* -0 -> +0 (0*0 = +0) */
+    if (hi == 0.0f) hi = 0.0f * 0.0f;
+    volatile float r = hi - lo;
+    volatile float inv = 0.0f;
+    if (r != 0.0f) inv = 3.0f / r;
+    for (int32_t c = 0; c < d; ++c) {
+        volatile float dx = orc_half_to_float(x[c]) - lo;                    /* one binary32 rounding */
+        double t = rint((double)dx * (double)inv);                           /* exact product, rounded once */
+        if (t > 3.0) t = 3.0;
+        if (t < 0.0) t = 0.0;
+        q[c] = (uint8_t)t;
+    }
+    *lo_out = orc_float_to_half(lo);                     /* exact: lo, hi are fp16 values */
+    *hi_out = orc_float_to_half(hi);
+}
+
+void orc_dequantize2_vector(const uint8_t *q, int32_t d, uint16_t lo_bits, uint16_t hi_bits, uint16_t *y)
+{
+    const float lo = orc_half_to_float(lo_bits), hi = orc_half_to_float(hi_bits);
+    volatile float r = hi - lo;
+    volatile float step = 0.0f;
+    if (r != 0.0f) step = r / 3.0f;
+    for (int32_t c = 0; c < d; ++c) {
+        volatile float v = fmaf((float)q[c], step, lo);                      /* correctly rounded fused multiply-add */
+        y[c] = orc_float_to_half(v);
+    }
+}
+
 /* ------------------------------------------------------------------------ */
 /* O5/O4. Pack (Alg. 1 step 4)                                 */
 /* ------------------------------------------------------------------------ */
@@ -331,14 +412,15 @@ void orc_dequantize_vector(const int8_t *q, int32_t d, int32_t qmax, uint16_t am
 int orc_pack(int32_t L, int32_t Hkv, int32_t d, int64_t n, const uint16_t *K, const uint16_t *V,
              const uint8_t *tier, const int64_t counts6[6], int32_t allow_int4, uint8_t *blob)
 {
-    orc_layout_t lo; orc_layout(L, Hkv, d, n, counts6, &lo);
+    const int low2 = (allow_int4 == 2);                  /* NEXT-4: the low tier is asymmetric 2-bit, tier code 2 */
+    orc_layout_t lo; orc_layout_low(L, Hkv, d, n, counts6, low2 ? 2 : 4, &lo);
     memset(blob, 0, (size_t)lo.total_bytes);
     put_u32(blob + 0, 0x31564B53u);  put_u32(blob + 4, 1u);
     put_u32(blob + 8, (uint32_t)L);  put_u32(blob + 12, (uint32_t)Hkv);
     put_u32(blob + 16, (uint32_t)d); put_u32(blob + 20, (uint32_t)n);
     put_u32(blob + 24, (uint32_t)counts6[0]); put_u32(blob + 28, (uint32_t)counts6[1]);
     put_u32(blob + 32, (uint32_t)counts6[2]); put_u32(blob + 36, (uint32_t)counts6[3]);
-    put_u32(blob + 40, allow_int4 ? 1u : 0u); put_u32(blob + 44, 0u);
+    put_u32(blob + 40, (allow_int4 ? 1u : 0u) | (low2 ? 2u : 0u)); put_u32(blob + 44, 0u);   /* flags: bit0 low tier allowed, bit1 it is 2-bit */
     put_u64(blob + 48, (uint64_t)counts6[4]);
     put_u64(blob + 56, lo.tier_map_off); put_u64(blob + 64, lo.layer0_off); put_u64(blob + 72, lo.layer_stride);
     for (int s = 0; s < 10; ++s) put_u64(blob + 80 + 8 * s, lo.seg_off[s]);
@@ -368,7 +450,7 @@ int orc_pack(int32_t L, int32_t Hkv, int32_t d, int64_t n, const uint16_t *K, co
                         for (int32_t c = 0; c < d; ++c) dst[(size_t)h * d + c] = (uint8_t)q[c];
                         sc[2 * h] = (uint8_t)ab; sc[2 * h + 1] = (uint8_t)(ab >> 8);
                     }
-                } else if (t == 4) {
+                } else if (t == 4 && !low2) {
                     uint8_t *dst = base + lo.seg_off[4 + kv] + (size_t)slot4 * row / 2;
                     uint8_t *sc  = base + lo.seg_off[8 + kv] + (size_t)slot4 * Hkv * 2;
                     for (int32_t h = 0; h < Hkv; ++h) {
@@ -378,9 +460,20 @@ int orc_pack(int32_t L, int32_t Hkv, int32_t d, int64_t n, const uint16_t *K, co
                             dst[((size_t)h * d + c) / 2] = (uint8_t)((q[c] & 0xF) | ((q[c + 1] & 0xF) << 4));
                         sc[2 * h] = (uint8_t)ab; sc[2 * h + 1] = (uint8_t)(ab >> 8);
                     }
+                } else if (t == 2 && low2) {
+                    uint8_t *dst = base + lo.seg_off[4 + kv] + (size_t)slot4 * row / 4;
+                    uint8_t *sc  = base + lo.seg_off[8 + kv] + (size_t)slot4 * Hkv * 4;
+                    for (int32_t h = 0; h < Hkv; ++h) {
+                        uint16_t lb, hb;
+                        orc_quantize2_vector(src + (size_t)h * d, d, &lb, &hb, (uint8_t *)q);
+                        for (int32_t c = 0; c < d; c += 4)   /* element 4i+k in bits 2k..2k+1 of byte i */
+                            dst[((size_t)h * d + c) / 4] = (uint8_t)((q[c] & 3) | ((q[c + 1] & 3) << 2) | ((q[c + 2] & 3) << 4) | ((q[c + 3] & 3) << 6));
+                        sc[4 * h] = (uint8_t)lb; sc[4 * h + 1] = (uint8_t)(lb >> 8);
+                        sc[4 * h + 2] = (uint8_t)hb; sc[4 * h + 3] = (uint8_t)(hb >> 8);
+                    }
                 }                                        /* t == 0: dropped, no bytes */
             }
-            if (t == 16) ++slot16; else if (t == 8) ++slot8; else if (t == 4) ++slot4;
+            if (t == 16) ++slot16; else if (t == 8) ++slot8; else if (t == (low2 ? 2 : 4)) ++slot4;
         }
         free(q);
         if (slot16 != counts6[0] || slot8 != counts6[1] || slot4 != counts6[2]) {
@@ -404,7 +497,10 @@ static int orc_unpack_impl(const uint8_t *blob, uint64_t blob_bytes, int32_t L, 
         get_u32(blob + 16) != (uint32_t)d || get_u32(blob + 20) != (uint32_t)n) return -5;
     int64_t counts[4] = { get_u32(blob + 24), get_u32(blob + 28), get_u32(blob + 32), get_u32(blob + 36) };
     if (counts[0] + counts[1] + counts[2] + counts[3] != n) return -5;
-    orc_layout_t lo; orc_layout(L, Hkv, d, n, counts, &lo);
+    const uint32_t flags = get_u32(blob + 40);
+    if (flags & ~3u) return -5;
+    const int low2 = (flags & 2u) != 0;                  /* NEXT-4: the low tier is asymmetric 2-bit */
+    orc_layout_t lo; orc_layout_low(L, Hkv, d, n, counts, low2 ? 2 : 4, &lo);
     if (get_u64(blob + 56) != lo.tier_map_off || get_u64(blob + 64) != lo.layer0_off ||
         get_u64(blob + 72) != lo.layer_stride || get_u64(blob + 160) != lo.total_bytes ||
         lo.total_bytes != blob_bytes) return -5;
@@ -434,7 +530,16 @@ static int orc_unpack_impl(const uint8_t *blob, uint64_t blob_bytes, int32_t L, 
                         for (int32_t c = 0; c < d; ++c) q[c] = (int8_t)src[(size_t)h * d + c];
                         orc_dequantize_vector(q, d, 127, (uint16_t)(sc[2 * h] | (sc[2 * h + 1] << 8)), dst + (size_t)h * d);
                     }
-                } else if (t == 4) {
+                } else if (t == 2 && low2) {
+                    const uint8_t *src = base + lo.seg_off[4 + kv] + (size_t)slot4 * row / 4;
+                    const uint8_t *sc  = base + lo.seg_off[8 + kv] + (size_t)slot4 * Hkv * 4;
+                    for (int32_t h = 0; h < Hkv; ++h) {
+                        for (int32_t c = 0; c < d; ++c)
+                            q[c] = (int8_t)((src[((size_t)h * d + c) / 4] >> (2 * (c & 3))) & 3);
+                        orc_dequantize2_vector((const uint8_t *)q, d, (uint16_t)(sc[4 * h] | (sc[4 * h + 1] << 8)),
+                                               (uint16_t)(sc[4 * h + 2] | (sc[4 * h + 3] << 8)), dst + (size_t)h * d);
+                    }
+                } else if (t == 4 && !low2) {
                     const uint8_t *src = base + lo.seg_off[4 + kv] + (size_t)slot4 * row / 2;
                     const uint8_t *sc  = base + lo.seg_off[8 + kv] + (size_t)slot4 * Hkv * 2;
                     for (int32_t h = 0; h < Hkv; ++h) {
@@ -449,7 +554,7 @@ static int orc_unpack_impl(const uint8_t *blob, uint64_t blob_bytes, int32_t L, 
                     for (size_t e = 0; e < row; ++e) dst[e] = 0;             /* P10: dropped => +0.0 */
                 }                                                            /* patch: not shipped => untouched */
             }
-            if (t == 16) ++slot16; else if (t == 8) ++slot8; else if (t == 4) ++slot4;
+            if (t == 16) ++slot16; else if (t == 8) ++slot8; else if (t == (low2 ? 2 : 4)) ++slot4;
         }
         free(q);
     }

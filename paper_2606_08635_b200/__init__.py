@@ -117,10 +117,15 @@ def make_shape(n_layers, n_q_heads, n_kv_heads, head_dim, n_tokens, n_requests=1
     return s
 
 
+def _low_mode(allow_int4):
+    """False/0 = 2-tier, True/1 = symmetric INT4 low tier, 2 = asymmetric 2-bit low tier (NEXT-4)."""
+    return 2 if (allow_int4 == 2 and allow_int4 is not True) else (1 if allow_int4 else 0)
+
+
 def make_policy(budget, n_sink=0, ranges=(), allow_int4=True):
     flat = [int(v) for r in ranges for v in r]
     arr = (C.c_int32 * max(1, len(flat)))(*flat)
-    p = skv_policy(float(budget), int(n_sink), len(flat) // 2, C.cast(arr, C.POINTER(C.c_int32)), 1 if allow_int4 else 0)
+    p = skv_policy(float(budget), int(n_sink), len(flat) // 2, C.cast(arr, C.POINTER(C.c_int32)), _low_mode(allow_int4))
     p._keepalive = arr
     return p
 
@@ -227,6 +232,6 @@ def skv_unpack_patch(shape, blob, blob_bytes, counts, K_inout, V_inout, tier_map
 
 def skv_counts_from_populations(shape, n16, n8=0, n4=0, allow_int4=True):
     c = skv_counts()
-    _check(lib().skv_counts_from_populations(C.byref(shape), int(n16), int(n8), int(n4), 1 if allow_int4 else 0,
+    _check(lib().skv_counts_from_populations(C.byref(shape), int(n16), int(n8), int(n4), _low_mode(allow_int4),
                                              C.byref(c)), "skv_counts_from_populations")
     return c

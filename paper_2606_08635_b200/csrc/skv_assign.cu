@@ -152,7 +152,7 @@ assign_kernel(Geom g, Intervals prot, const float *__restrict__ importance, uint
             else if (key == th[k].key) pass = (th[k].n_gt + run[k]) < th[k].rank;
             else pass = false;
             if (key == th[k].key) run[k] += 1;
-            if (pass && !done) { tier = (k == 0) ? 16u : (k == 1) ? 8u : 4u; done = true; }
+            if (pass && !done) { tier = (k == 0) ? 16u : (k == 1) ? 8u : (uint32_t)g.low_code; done = true; }
         }
         out[j] = (uint8_t)tier;
     }

@@ -175,6 +175,68 @@ __device__ __forceinline__ uint4 dequant_int4(uint32_t w, float scale)
     o.w = h2_bits(__fmul_rn(f[6], scale), __fmul_rn(f[7], scale));
     return o;
 }
+// ------------------------------------------------------------------------------------------------
+// NEXT-4: asymmetric 2-bit low tier (include/skv.h "2-bit quantiser")
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint16_t ld_stream2(const void *p)
+{
+    uint16_t r;
+    asm volatile("ld.global.nc.L1::no_allocate.u16 %0, [%1];" : "=h"(r) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ void st_stream2(void *p, uint16_t v)
+{
+    asm volatile("st.global.L1::no_allocate.u16 [%0], %1;" :: "l"(p), "h"(v) : "memory");
+}
+// (max, -min) of the 8 halves in a uint4: both halves of the result reduce with hmax2
+__device__ __forceinline__ __half2 max_negmin8(const uint4 &v)
+{
+    const __half2 a = u2h(v.x), b = u2h(v.y), c = u2h(v.z), d = u2h(v.w);
+    const __half2 mx = __hmax2(__hmax2(a, b), __hmax2(c, d));
+    const __half2 mn = __hmin2(__hmin2(a, b), __hmin2(c, d));
+    return __halves2half2(__hmax(__low2half(mx), __high2half(mx)), __hneg(__hmin(__low2half(mn), __high2half(mn))));
+}
+// canonical records from a reduced (max, -min): a zero of either sign is stored as +0
+__device__ __forceinline__ void lohi_of(__half2 m, __half &lo, __half &hi)
+{
+    hi = __low2half(m);
+    lo = __hneg(__high2half(m));
+    const __half z = __ushort_as_half((unsigned short)0);
+    if (__heq(hi, z)) hi = z;
+    if (__heq(lo, z)) lo = z;
+}
+__device__ __forceinline__ float range_of(__half lo, __half hi) { return __fsub_rn(__half2float(hi), __half2float(lo)); }
+__device__ __forceinline__ float inv3_of(float r) { return r != 0.0f ? __fdiv_rn(3.0f, r) : 0.0f; }
+__device__ __forceinline__ float step3_of(float r) { return r != 0.0f ? __fdiv_rn(r, 3.0f) : 0.0f; }
+// 8 fp16 -> 8 two-bit codes (16 bits; element k in bits 2k..2k+1).  q_k = rint(fl32(x_k - lo) * inv), the product exact
+// and rounded once: the whole word is built in the mantissa of one float by a chain of fused multiply-adds,
+//     a <- fma(dx_k, inv, a)      adds q_k (a is an even integer in [2^23, 2^24), so the FMA's rounding is RNE of the product)
+//     a <- fma(a, 4, -3*M)        shifts the partial word two bits up (exact), M = 1.5 * 2^23
+__device__ __forceinline__ uint32_t quant8_int2(const uint4 &v, float lo, float inv)
+{
+    const float2 p0 = __half22float2(u2h(v.x)), p1 = __half22float2(u2h(v.y));
+    const float2 p2 = __half22float2(u2h(v.z)), p3 = __half22float2(u2h(v.w));
+    const float x[8] = {p0.x, p0.y, p1.x, p1.y, p2.x, p2.y, p3.x, p3.y};
+    float a = __fmaf_rn(__fsub_rn(x[7], lo), inv, 12582912.0f);
+#pragma unroll
+    for (int k = 6; k >= 0; --k) {
+        a = __fmaf_rn(a, 4.0f, -37748736.0f);
+        a = __fmaf_rn(__fsub_rn(x[k], lo), inv, a);
+    }
+    return __float_as_uint(a) & 0xFFFFu;
+}
+// 16 bits of two-bit codes -> 8 fp16: y = f16_rn(fma(q, step, lo))
+__device__ __forceinline__ uint4 dequant_int2(uint32_t w, float step, float lo)
+{
+    float f[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k)                          // int -> float through the 2^23 exponent trick (exact)
+        f[k] = __fmaf_rn(__fsub_rn(__uint_as_float(0x4B000000u | ((w >> (2 * k)) & 3u)), 8388608.0f), step, lo);
+    uint4 o;
+    o.x = h2_bits(f[0], f[1]); o.y = h2_bits(f[2], f[3]); o.z = h2_bits(f[4], f[5]); o.w = h2_bits(f[6], f[7]);
+    return o;
+}
+
 __device__ __forceinline__ float scale_of(__half amax, float qmax)
 {
     const float af = __half2float(amax);

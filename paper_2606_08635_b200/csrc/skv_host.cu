@@ -11,16 +11,19 @@
 
 namespace skv {
 
-Layout make_layout(int L, int Hkv, int D, int64_t n, int64_t n16, int64_t n8, int64_t n4)
+// low_bits: 4 = the low tier holds symmetric INT4 codes (two per byte, one fp16 amax record per head vector);
+// 2 = asymmetric 2-bit codes (four per byte, an fp16 (lo, hi) pair per head vector) -- NEXT-4.
+Layout make_layout(int L, int Hkv, int D, int64_t n, int64_t n16, int64_t n8, int64_t n4, int low_bits)
 {
     Layout lo;
     const uint64_t H = (uint64_t)Hkv, d = (uint64_t)D;
+    const uint64_t cpb = low_bits == 2 ? 4 : 2, rec = low_bits == 2 ? 4 : 2;
     const uint64_t raw[10] = {
         (uint64_t)n16 * H * d * 2, (uint64_t)n16 * H * d * 2,
         (uint64_t)n8 * H * d,      (uint64_t)n8 * H * d,
-        (uint64_t)n4 * H * d / 2,  (uint64_t)n4 * H * d / 2,
+        (uint64_t)n4 * H * d / cpb, (uint64_t)n4 * H * d / cpb,
         (uint64_t)n8 * H * 2,      (uint64_t)n8 * H * 2,
-        (uint64_t)n4 * H * 2,      (uint64_t)n4 * H * 2};
+        (uint64_t)n4 * H * rec,    (uint64_t)n4 * H * rec};
     lo.tier_map_off = 256;
     lo.layer0_off = 256 + pad256((uint64_t)L * (uint64_t)n);
     uint64_t off = 0;
@@ -64,6 +67,7 @@ static Geom make_geom(const skv_shape *s, const skv_counts *c)
     g.row_chunks = (g.Hkv * g.D + 255) / 256;
     g.tiles = (g.n + kTileTokens - 1) / kTileTokens;
     g.patch = 0;
+    g.low_code = (c && c->allow_int4 == 2) ? 2 : 4;
     return g;
 }
 
@@ -112,6 +116,22 @@ static int tier_counts_impl(const skv_shape *s, const skv_policy *p, skv_counts 
     const int64_t P = merge_protected(s, p, prot);
     if (P < 0) return SKV_ERR_INVALID_ARG;
     const int64_t n = s->n_tokens;
+    if (p->allow_int4 != 0 && p->allow_int4 != 1 && p->allow_int4 != 2) return SKV_ERR_INVALID_ARG;
+    if (p->allow_int4 == 2) {
+        // NEXT-4: 2-bit low tier, c = 1/8 -> the same greedy ladder in EIGHTH-units, 8 / 4 / 1 / 0 per token
+        const int64_t Q8 = (int64_t)floor(8.0 * b * (double)n + 1e-6);
+        const int64_t m8 = n - P, R8 = Q8 - 8 * P;
+        if (R8 < 0) return SKV_ERR_BUDGET_INFEASIBLE;
+        int64_t a16 = P, a8 = 0, a2 = 0, a0 = 0;
+        if (R8 >= 8 * m8) a16 = n;
+        else if (R8 >= 4 * m8) { const int64_t up = (R8 - 4 * m8) / 4; a16 = P + up; a8 = m8 - up; }
+        else if (R8 >= m8) { a8 = (R8 - m8) / 3; a2 = m8 - a8; }
+        else { a2 = R8; a0 = m8 - R8; }
+        c->n16 = (int32_t)a16; c->n8 = (int32_t)a8; c->n4 = (int32_t)a2; c->n0 = (int32_t)a0;
+        c->allow_int4 = 2; c->reserved = 0;
+        c->budget_q4 = Q8; c->spent_q4 = 8 * a16 + 4 * a8 + a2;
+        return SKV_OK;
+    }
     const int64_t Q = (int64_t)floor(4.0 * b * (double)n + 1e-6);     // quarter-units: 4 / 2 / 1 / 0 per token
     const int64_t m = n - P, R = Q - 4 * P;
     if (R < 0) return SKV_ERR_BUDGET_INFEASIBLE;
@@ -149,7 +169,7 @@ size_t skv_blob_bytes(const skv_shape *shape, const skv_counts *counts)
 {
     if (!dims_ok(shape) || !counts_ok(shape, counts)) return 0;
     return (size_t)make_layout(shape->n_layers, shape->n_kv_heads, shape->head_dim, shape->n_tokens,
-                               counts->n16, counts->n8, counts->n4).total_bytes;
+                               counts->n16, counts->n8, counts->n4, counts->allow_int4 == 2 ? 2 : 4).total_bytes;
 }
 
 size_t skv_workspace_bytes(const skv_shape *shape, int32_t window)
@@ -174,15 +194,18 @@ int skv_blob_check(const void *header_host, size_t blob_bytes, skv_shape *shape_
     const uint32_t flags = get32(h + 40);
     if (L == 0 || Hkv == 0 || n == 0 || L > 65535u || n > (1u << 20) || Hkv > 65535u) return SKV_ERR_BAD_BLOB;
     if (D != 64 && D != 128 && D != 256) return SKV_ERR_BAD_BLOB;
-    if ((uint64_t)n16 + n8 + n4 + n0 != n || (flags & ~1u) || get32(h + 44) != 0) return SKV_ERR_BAD_BLOB;
+    if ((uint64_t)n16 + n8 + n4 + n0 != n || (flags & ~3u) || flags == 2u || get32(h + 44) != 0) return SKV_ERR_BAD_BLOB;
     if (!(flags & 1u) && n4 != 0) return SKV_ERR_BAD_BLOB;
-    const Layout lo = make_layout((int)L, (int)Hkv, (int)D, n, n16, n8, n4);
+    const bool low2 = (flags & 2u) != 0;                    // bit1: the low tier is asymmetric 2-bit (budget in eighths)
+    const Layout lo = make_layout((int)L, (int)Hkv, (int)D, n, n16, n8, n4, low2 ? 2 : 4);
     if (get64(h + 56) != lo.tier_map_off || get64(h + 64) != lo.layer0_off || get64(h + 72) != lo.layer_stride ||
         get64(h + 160) != lo.total_bytes || lo.total_bytes != blob_bytes) return SKV_ERR_BAD_BLOB;
     for (int s = 0; s < 10; ++s) if (get64(h + 80 + 8 * s) != lo.seg_off[s]) return SKV_ERR_BAD_BLOB;
     for (int o = 168; o < 256; ++o) if (h[o]) return SKV_ERR_BAD_BLOB;
     const uint64_t Q = get64(h + 48);
-    if (Q > 4ull * n || 4ull * n16 + 2ull * n8 + n4 > Q) return SKV_ERR_BAD_BLOB;
+    const uint64_t unit = low2 ? 8ull : 4ull;
+    const uint64_t spent = unit * n16 + (unit / 2) * n8 + n4;
+    if (Q > unit * n || spent > Q) return SKV_ERR_BAD_BLOB;
     if (shape_out) {
         memset(shape_out, 0, sizeof(*shape_out));
         shape_out->n_layers = (int32_t)L; shape_out->n_kv_heads = (int32_t)Hkv; shape_out->head_dim = (int32_t)D;
@@ -190,8 +213,8 @@ int skv_blob_check(const void *header_host, size_t blob_bytes, skv_shape *shape_
     }
     if (counts_out) {
         counts_out->n16 = (int32_t)n16; counts_out->n8 = (int32_t)n8; counts_out->n4 = (int32_t)n4; counts_out->n0 = (int32_t)n0;
-        counts_out->allow_int4 = (int32_t)(flags & 1u); counts_out->reserved = 0;
-        counts_out->budget_q4 = (int64_t)Q; counts_out->spent_q4 = 4ll * n16 + 2ll * n8 + n4;
+        counts_out->allow_int4 = low2 ? 2 : (int32_t)(flags & 1u); counts_out->reserved = 0;
+        counts_out->budget_q4 = (int64_t)Q; counts_out->spent_q4 = (int64_t)spent;
     }
     return SKV_OK;
 }
@@ -259,7 +282,7 @@ int skv_pack(const skv_shape *shape, const void *K_dev, const void *V_dev, const
     if (!tier_map_dev || !blob_dev || !ws || !counts_ok(shape, counts)) return SKV_ERR_INVALID_ARG;
     if ((uintptr_t)blob_dev & 255) return SKV_ERR_UNSUPPORTED;
     const Geom g = make_geom(shape, counts);
-    const Layout lo = make_layout(g.L, g.Hkv, g.D, g.n, g.n16, g.n8, g.n4);
+    const Layout lo = make_layout(g.L, g.Hkv, g.D, g.n, g.n16, g.n8, g.n4, g.low_code);
     if (blob_capacity < (size_t)lo.total_bytes * (size_t)g.R) return SKV_ERR_BUFFER_TOO_SMALL;
     if (ws_bytes < scan_ws_bytes(shape)) return SKV_ERR_BUFFER_TOO_SMALL;
 
@@ -269,7 +292,7 @@ int skv_pack(const skv_shape *shape, const void *K_dev, const void *V_dev, const
     put32(h + 0, 0x31564B53u); put32(h + 4, 1u);
     put32(h + 8, (uint32_t)g.L); put32(h + 12, (uint32_t)g.Hkv); put32(h + 16, (uint32_t)g.D); put32(h + 20, (uint32_t)g.n);
     put32(h + 24, (uint32_t)g.n16); put32(h + 28, (uint32_t)g.n8); put32(h + 32, (uint32_t)g.n4); put32(h + 36, (uint32_t)g.n0);
-    put32(h + 40, counts->allow_int4 ? 1u : 0u);
+    put32(h + 40, (counts->allow_int4 ? 1u : 0u) | (counts->allow_int4 == 2 ? 2u : 0u));
     put64(h + 48, (uint64_t)counts->budget_q4);
     put64(h + 56, lo.tier_map_off); put64(h + 64, lo.layer0_off); put64(h + 72, lo.layer_stride);
     for (int s = 0; s < 10; ++s) put64(h + 80 + 8 * s, lo.seg_off[s]);
@@ -293,7 +316,7 @@ static int unpack_impl(const skv_shape *shape, const void *blob_dev, size_t blob
     if ((uintptr_t)blob_dev & 255) return SKV_ERR_UNSUPPORTED;
     Geom g = make_geom(shape, counts);
     g.patch = patch;
-    const Layout lo = make_layout(g.L, g.Hkv, g.D, g.n, g.n16, g.n8, g.n4);
+    const Layout lo = make_layout(g.L, g.Hkv, g.D, g.n, g.n16, g.n8, g.n4, g.low_code);
     if (blob_bytes != (size_t)lo.total_bytes) return SKV_ERR_BAD_BLOB;
     if (ws_bytes < scan_ws_bytes(shape)) return SKV_ERR_BUFFER_TOO_SMALL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -325,8 +348,9 @@ int skv_counts_from_populations(const skv_shape *shape, int32_t n16, int32_t n8,
     memset(counts_out, 0, sizeof(*counts_out));
     counts_out->n16 = n16; counts_out->n8 = n8; counts_out->n4 = n4;
     counts_out->n0 = shape->n_tokens - n16 - n8 - n4;
-    counts_out->allow_int4 = allow_int4 ? 1 : 0;
-    counts_out->spent_q4 = 4LL * n16 + 2LL * n8 + n4;
+    if (allow_int4 < 0 || allow_int4 > 2) return SKV_ERR_INVALID_ARG;
+    counts_out->allow_int4 = allow_int4;
+    counts_out->spent_q4 = allow_int4 == 2 ? 8LL * n16 + 4LL * n8 + n4 : 4LL * n16 + 2LL * n8 + n4;
     counts_out->budget_q4 = counts_out->spent_q4;
     return SKV_OK;
 }

@@ -63,7 +63,8 @@ pack_kernel(Geom g, Layout lo, const __half *__restrict__ K, const __half *__res
     const uint32_t my_t = (j0 + lane < n) ? (uint32_t)tm[j0 + lane] : 0xFFu;
     const uint32_t m16 = __ballot_sync(0xffffffffu, my_t == 16u);
     const uint32_t m8 = __ballot_sync(0xffffffffu, my_t == 8u);
-    const uint32_t m4 = __ballot_sync(0xffffffffu, my_t == 4u);
+    const uint32_t low = (uint32_t)g.low_code;                       // 4: symmetric INT4, 2: asymmetric 2-bit (NEXT-4)
+    const uint32_t m4 = __ballot_sync(0xffffffffu, my_t == low);
     const uint4 base = tile_base[((int64_t)r * g.L + l) * g.tiles + tile];
 
     uint8_t *lbase = blob + (uint64_t)r * blob_stride + lo.layer0_off + (uint64_t)l * lo.layer_stride;
@@ -72,7 +73,7 @@ pack_kernel(Geom g, Layout lo, const __half *__restrict__ K, const __half *__res
 
     for (uint32_t i = warp; i < (uint32_t)kTileTokens; i += nwarps) {
         const uint32_t t = __shfl_sync(0xffffffffu, my_t, i);
-        if (t != 16u && t != 8u && t != 4u) continue;                 // dropped / tail / invalid: no bytes
+        if (t != 16u && t != 8u && t != low) continue;                // dropped / tail / invalid: no bytes
         const uint32_t below = (1u << i) - 1u;
         const int64_t j = j0 + i;
         const __half *krow = K + cache_off + j * g.st;
@@ -133,6 +134,37 @@ pack_kernel(Geom g, Layout lo, const __half *__restrict__ K, const __half *__res
                     }
                 }
             }
+        } else if (low == 2u) {
+            const uint32_t slot = base.z + __popc(m4 & below);
+            if (slot >= (uint32_t)g.n4) continue;
+            uint8_t *kd = lbase + lo.seg_off[4] + (uint64_t)slot * (row_elems / 4);
+            uint8_t *vd = lbase + lo.seg_off[5] + (uint64_t)slot * (row_elems / 4);
+            __half2 *ks = reinterpret_cast<__half2 *>(lbase + lo.seg_off[8]) + (uint64_t)slot * g.Hkv;
+            __half2 *vs = reinterpret_cast<__half2 *>(lbase + lo.seg_off[9]) + (uint64_t)slot * g.Hkv;
+            for (int c0 = 0; c0 < g.row_chunks; ++c0) {
+                const int e = c0 * 256 + lane * 8;
+                const bool in = e < row_elems;
+                uint4 kv = make_uint4(0, 0, 0, 0), vv = kv;
+                if (in) {
+                    const int h = e / D, c = e % D;
+                    kv = ld_stream(krow + (int64_t)h * g.sh + c);
+                    vv = ld_stream(vrow + (int64_t)h * g.sh + c);
+                }
+                // lanes past the row hold zeros: they sit in head-vector groups of their own (row_elems % D == 0)
+                __half2 mk = max_negmin8(kv), mv = max_negmin8(vv);
+#pragma unroll
+                for (int o = 1; o < LPV; o <<= 1) {
+                    mk = __hmax2(mk, u2h(__shfl_xor_sync(0xffffffffu, h2u(mk), o)));
+                    mv = __hmax2(mv, u2h(__shfl_xor_sync(0xffffffffu, h2u(mv), o)));
+                }
+                __half loK, hiK, loV, hiV;
+                lohi_of(mk, loK, hiK); lohi_of(mv, loV, hiV);
+                if (in) {
+                    st_stream2(kd + e / 4, (uint16_t)quant8_int2(kv, __half2float(loK), inv3_of(range_of(loK, hiK))));
+                    st_stream2(vd + e / 4, (uint16_t)quant8_int2(vv, __half2float(loV), inv3_of(range_of(loV, hiV))));
+                    if ((lane % LPV) == 0) { ks[e / D] = __halves2half2(loK, hiK); vs[e / D] = __halves2half2(loV, hiV); }
+                }
+            }
         } else {
             const uint32_t slot = base.z + __popc(m4 & below);
             if (slot >= (uint32_t)g.n4) continue;
@@ -182,7 +214,8 @@ pack_kernel(Geom g, Layout lo, const __half *__restrict__ K, const __half *__res
 // reduction (skv_codec.cuh): NCH-1+log2(LPV/NCH) shuffles and TWO divisions per lane per batch instead
 // of 2*NCH*log2(LPV) shuffles and 2*NCH divisions; the reciprocals are then broadcast with 2*NCH shuffles.
 // ------------------------------------------------------------------------------------------------
-template <int D, int NCH, int MINB>
+// LOW2 = false: the low tier is symmetric INT4 (tier code 4).  LOW2 = true (NEXT-4): asymmetric 2-bit (tier code 2).
+template <int D, int NCH, int MINB, bool LOW2>
 __global__ void __launch_bounds__(256, MINB)
 pack_fast_kernel(Geom g, Layout lo, const __half *__restrict__ K, const __half *__restrict__ V,
                  const uint8_t *__restrict__ tier_map, uint8_t *__restrict__ blob, uint64_t blob_stride,
@@ -200,7 +233,8 @@ pack_fast_kernel(Geom g, Layout lo, const __half *__restrict__ K, const __half *
     const uint32_t my_t = (j0 + lane < n) ? (uint32_t)tm[j0 + lane] : 0xFFu;
     const uint32_t m16 = __ballot_sync(0xffffffffu, my_t == 16u);
     const uint32_t m8 = __ballot_sync(0xffffffffu, my_t == 8u);
-    const uint32_t m4 = __ballot_sync(0xffffffffu, my_t == 4u);
+    constexpr uint32_t kLow = LOW2 ? 2u : 4u;
+    const uint32_t m4 = __ballot_sync(0xffffffffu, my_t == kLow);
     const uint4 base = tile_base[((int64_t)r * g.L + l) * g.tiles + tile];
 
     uint8_t *lbase = blob + (uint64_t)r * blob_stride + lo.layer0_off + (uint64_t)l * lo.layer_stride;
@@ -214,7 +248,7 @@ pack_fast_kernel(Geom g, Layout lo, const __half *__restrict__ K, const __half *
 #pragma unroll 1
     for (uint32_t i = warp; i < (uint32_t)kTileTokens; i += 8) {
         const uint32_t t = __shfl_sync(0xffffffffu, my_t, i);
-        if (t != 16u && t != 8u && t != 4u) continue;                 // dropped / tail / invalid: no bytes
+        if (t != 16u && t != 8u && t != kLow) continue;               // dropped / tail / invalid: no bytes
         const uint32_t below = (1u << i) - 1u;
         const int64_t j = j0 + i;
         const __half *krow = Kb + j * g.st + lane_c;
@@ -238,6 +272,36 @@ pack_fast_kernel(Geom g, Layout lo, const __half *__restrict__ K, const __half *
                 uint8_t *vd = lbase + lo.seg_off[1] + ((uint64_t)slot * row_elems + cb * 256 + lane * 8) * 2;
 #pragma unroll
                 for (int u = 0; u < NCH; ++u) { st_stream(kd + u * 512, kv[u]); st_stream(vd + u * 512, vv[u]); }
+                continue;
+            }
+            if (LOW2 && t == 2u) {
+                // asymmetric 2-bit: (max, -min) of K and of V reduced over the lanes of a head vector, (lo, hi) records,
+                // 16 bits of codes per lane and chunk
+                __half2 mk[NCH], mv[NCH];
+#pragma unroll
+                for (int u = 0; u < NCH; ++u) { mk[u] = max_negmin8(kv[u]); mv[u] = max_negmin8(vv[u]); }
+                const __half2 rk = group_absmax<LPV, NCH>(mk, lane), rv = group_absmax<LPV, NCH>(mv, lane);
+                __half loK, hiK, loV, hiV;
+                lohi_of(rk, loK, hiK); lohi_of(rv, loV, hiV);
+                const float invK = inv3_of(range_of(loK, hiK)), invV = inv3_of(range_of(loV, hiV));
+                const float lKf = __half2float(loK), lVf = __half2float(loV);
+                if (scale_writer) {
+                    const int head = (cb + my_chunk) * HPC + (int)(lane / LPV);
+                    __half2 *ks = reinterpret_cast<__half2 *>(lbase + lo.seg_off[8]) + (uint64_t)slot * g.Hkv;
+                    __half2 *vs = reinterpret_cast<__half2 *>(lbase + lo.seg_off[9]) + (uint64_t)slot * g.Hkv;
+                    ks[head] = __halves2half2(loK, hiK);
+                    vs[head] = __halves2half2(loV, hiV);
+                }
+                uint8_t *kd = lbase + lo.seg_off[4] + (uint64_t)slot * (row_elems / 4) + cb * 64 + lane * 2;
+                uint8_t *vd = lbase + lo.seg_off[5] + (uint64_t)slot * (row_elems / 4) + cb * 64 + lane * 2;
+#pragma unroll
+                for (int u = 0; u < NCH; ++u) {
+                    const int src = src_lane<LPV, NCH>(lane, u);
+                    const float ik = __shfl_sync(0xffffffffu, invK, src), iv = __shfl_sync(0xffffffffu, invV, src);
+                    const float lk = __shfl_sync(0xffffffffu, lKf, src), lv = __shfl_sync(0xffffffffu, lVf, src);
+                    st_stream2(kd + u * 64, (uint16_t)quant8_int2(kv[u], lk, ik));
+                    st_stream2(vd + u * 64, (uint16_t)quant8_int2(vv[u], lv, iv));
+                }
                 continue;
             }
             __half2 m[NCH];
@@ -285,7 +349,8 @@ static cudaError_t launch_pack_fast(const Geom &g, const Layout &lo, const __hal
                                     const uint4 *tile_base, cudaStream_t s)
 {
     dim3 grid(g.tiles, g.L, g.R);
-    pack_fast_kernel<D, NCH, 3><<<grid, 256, 0, s>>>(g, lo, K, V, tier_map, blob, blob_stride, tile_base);
+    if (g.low_code == 2) pack_fast_kernel<D, NCH, 2, true><<<grid, 256, 0, s>>>(g, lo, K, V, tier_map, blob, blob_stride, tile_base);
+    else pack_fast_kernel<D, NCH, 3, false><<<grid, 256, 0, s>>>(g, lo, K, V, tier_map, blob, blob_stride, tile_base);
     return cudaGetLastError();
 }
 

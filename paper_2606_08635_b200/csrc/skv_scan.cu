@@ -12,7 +12,7 @@ namespace skv {
 
 // counts of 16 / 8 / 4 in a tile, packed 3 x 21 bits into a u64 so one scan serves all three
 // (the host rejects n > 2^20, so no field can carry into the next).
-__device__ __forceinline__ unsigned long long tile_counts(const uint8_t *tier, int64_t n, int64_t tile)
+__device__ __forceinline__ unsigned long long tile_counts(const uint8_t *tier, int64_t n, int64_t tile, uint32_t low)
 {
     const int64_t j0 = tile * kTileTokens;
     uint32_t c16 = 0, c8 = 0, c4 = 0;
@@ -27,13 +27,13 @@ __device__ __forceinline__ unsigned long long tile_counts(const uint8_t *tier, i
 #pragma unroll
                 for (int b = 0; b < 4; ++b) {
                     const uint32_t t = (w[k] >> (8 * b)) & 0xFFu;
-                    c16 += (t == 16u); c8 += (t == 8u); c4 += (t == 4u);
+                    c16 += (t == 16u); c8 += (t == 8u); c4 += (t == low);
                 }
         }
     } else {
         for (int i = 0; i < kTileTokens && j0 + i < n; ++i) {
             const uint32_t t = tier[j0 + i];
-            c16 += (t == 16u); c8 += (t == 8u); c4 += (t == 4u);
+            c16 += (t == 16u); c8 += (t == 8u); c4 += (t == low);
         }
     }
     return (unsigned long long)c16 | ((unsigned long long)c8 << 21) | ((unsigned long long)c4 << 42);
@@ -71,7 +71,7 @@ tile_scan_kernel(Geom g, Layout lo, const uint8_t *__restrict__ tier_in /* pack:
     uint4 *out = tile_base + ((int64_t)r * g.L + l) * g.tiles;
     for (int64_t t0 = 0; t0 < g.tiles; t0 += blockDim.x) {
         const int64_t tile = t0 + tid;
-        const unsigned long long c = tile < g.tiles ? tile_counts(tier, n, tile) : 0ull;
+        const unsigned long long c = tile < g.tiles ? tile_counts(tier, n, tile, (uint32_t)g.low_code) : 0ull;
         const unsigned long long x = warp_incl_scan(c, lane);
         if (lane == 31) warp_tot[warp] = x;
         __syncthreads();

@@ -26,7 +26,8 @@ unpack_kernel(Geom g, Layout lo, const uint8_t *__restrict__ blob, uint64_t blob
     const uint32_t my_t = (j0 + lane < n) ? (uint32_t)tm[j0 + lane] : 0xFFu;
     const uint32_t m16 = __ballot_sync(0xffffffffu, my_t == 16u);
     const uint32_t m8 = __ballot_sync(0xffffffffu, my_t == 8u);
-    const uint32_t m4 = __ballot_sync(0xffffffffu, my_t == 4u);
+    const uint32_t low = (uint32_t)g.low_code;                       // 4: symmetric INT4, 2: asymmetric 2-bit (NEXT-4)
+    const uint32_t m4 = __ballot_sync(0xffffffffu, my_t == low);
     const uint4 base = tile_base[((int64_t)r * g.L + l) * g.tiles + tile];
 
     const uint8_t *lbase = rblob + lo.layer0_off + (uint64_t)l * lo.layer_stride;
@@ -43,7 +44,7 @@ unpack_kernel(Geom g, Layout lo, const uint8_t *__restrict__ blob, uint64_t blob
         uint32_t slot = 0;
         if (t == 16u) { slot = base.x + __popc(m16 & below); if (slot >= (uint32_t)g.n16) t = 0; }
         else if (t == 8u) { slot = base.y + __popc(m8 & below); if (slot >= (uint32_t)g.n8) t = 0; }
-        else if (t == 4u) { slot = base.z + __popc(m4 & below); if (slot >= (uint32_t)g.n4) t = 0; }
+        else if (t == low) { slot = base.z + __popc(m4 & below); if (slot >= (uint32_t)g.n4) t = 0; }
         else t = 0;
         if (t == 0u && g.patch) continue;                             // patch mode (skv_unpack_patch): keep what is there
 
@@ -92,6 +93,23 @@ unpack_kernel(Geom g, Layout lo, const uint8_t *__restrict__ blob, uint64_t blob
                     }
                 }
             }
+        } else if (t == 2u) {
+            const uint8_t *ks = lbase + lo.seg_off[4] + (uint64_t)slot * (row_elems / 4);
+            const uint8_t *vs = lbase + lo.seg_off[5] + (uint64_t)slot * (row_elems / 4);
+            const __half2 *ka = reinterpret_cast<const __half2 *>(lbase + lo.seg_off[8]) + (uint64_t)slot * g.Hkv;
+            const __half2 *va = reinterpret_cast<const __half2 *>(lbase + lo.seg_off[9]) + (uint64_t)slot * g.Hkv;
+            for (int c0 = 0; c0 < g.row_chunks; ++c0) {
+                const int e = c0 * 256 + lane * 8;
+                if (e < row_elems) {
+                    const int h = e / D, c = e % D;
+                    const __half2 rk = ka[h], rv = va[h];                // (lo, hi) records
+                    const uint32_t kw = ld_stream2(ks + e / 4), vw = ld_stream2(vs + e / 4);
+                    st_stream(krow + (int64_t)h * g.sh + c,
+                              dequant_int2(kw, step3_of(range_of(__low2half(rk), __high2half(rk))), __half2float(__low2half(rk))));
+                    st_stream(vrow + (int64_t)h * g.sh + c,
+                              dequant_int2(vw, step3_of(range_of(__low2half(rv), __high2half(rv))), __half2float(__low2half(rv))));
+                }
+            }
         } else if (t == 4u) {
             const uint8_t *ks = lbase + lo.seg_off[4] + (uint64_t)slot * (row_elems / 2);
             const uint8_t *vs = lbase + lo.seg_off[5] + (uint64_t)slot * (row_elems / 2);
@@ -135,7 +153,7 @@ unpack_kernel(Geom g, Layout lo, const uint8_t *__restrict__ blob, uint64_t blob
 // Fast path (row_elems % (256*NCH) == 0): fully unrolled; each lane loads the amax record of ONE
 // (chunk, head) for K and V, divides twice, and the scales are broadcast with 2*NCH shuffles.
 // ------------------------------------------------------------------------------------------------
-template <int D, int NCH, int MINB>
+template <int D, int NCH, int MINB, bool LOW2>
 __global__ void __launch_bounds__(256, MINB)
 unpack_fast_kernel(Geom g, Layout lo, const uint8_t *__restrict__ blob, uint64_t blob_stride,
                    __half *__restrict__ K, __half *__restrict__ V, const uint4 *__restrict__ tile_base)
@@ -153,7 +171,8 @@ unpack_fast_kernel(Geom g, Layout lo, const uint8_t *__restrict__ blob, uint64_t
     const uint32_t my_t = (j0 + lane < n) ? (uint32_t)tm[j0 + lane] : 0xFFu;
     const uint32_t m16 = __ballot_sync(0xffffffffu, my_t == 16u);
     const uint32_t m8 = __ballot_sync(0xffffffffu, my_t == 8u);
-    const uint32_t m4 = __ballot_sync(0xffffffffu, my_t == 4u);
+    constexpr uint32_t kLow = LOW2 ? 2u : 4u;
+    const uint32_t m4 = __ballot_sync(0xffffffffu, my_t == kLow);
     const uint4 base = tile_base[((int64_t)r * g.L + l) * g.tiles + tile];
 
     const uint8_t *lbase = rblob + lo.layer0_off + (uint64_t)l * lo.layer_stride;
@@ -173,7 +192,7 @@ unpack_fast_kernel(Geom g, Layout lo, const uint8_t *__restrict__ blob, uint64_t
         uint32_t slot = 0;
         if (t == 16u) { slot = base.x + __popc(m16 & below); if (slot >= (uint32_t)g.n16) t = 0; }
         else if (t == 8u) { slot = base.y + __popc(m8 & below); if (slot >= (uint32_t)g.n8) t = 0; }
-        else if (t == 4u) { slot = base.z + __popc(m4 & below); if (slot >= (uint32_t)g.n4) t = 0; }
+        else if (t == kLow) { slot = base.z + __popc(m4 & below); if (slot >= (uint32_t)g.n4) t = 0; }
         else t = 0;
         if (t == 0u && g.patch) continue;                             // patch mode (skv_unpack_patch): keep what is there
 
@@ -208,7 +227,27 @@ unpack_fast_kernel(Geom g, Layout lo, const uint8_t *__restrict__ blob, uint64_t
                     st_stream(krow + off, dequant_int8(kv[u], sk));
                     st_stream(vrow + off, dequant_int8(vv[u], sv));
                 }
-            } else if (t == 4u) {
+            } else if (LOW2 && t == 2u) {
+                const uint8_t *ks = lbase + lo.seg_off[4] + (uint64_t)slot * (row_elems / 4) + cb * 64 + lane * 2;
+                const uint8_t *vs = lbase + lo.seg_off[5] + (uint64_t)slot * (row_elems / 4) + cb * 64 + lane * 2;
+                const int head = (cb + my_chunk) * HPC + (int)(lane / LPV);
+                uint32_t kv[NCH], vv[NCH];
+#pragma unroll
+                for (int u = 0; u < NCH; ++u) { kv[u] = ld_stream2(ks + u * 64); vv[u] = ld_stream2(vs + u * 64); }
+                const __half2 rk = reinterpret_cast<const __half2 *>(lbase + lo.seg_off[8])[(uint64_t)slot * g.Hkv + head];
+                const __half2 rv = reinterpret_cast<const __half2 *>(lbase + lo.seg_off[9])[(uint64_t)slot * g.Hkv + head];
+                const float sK = step3_of(range_of(__low2half(rk), __high2half(rk))), lK = __half2float(__low2half(rk));
+                const float sV = step3_of(range_of(__low2half(rv), __high2half(rv))), lV = __half2float(__low2half(rv));
+#pragma unroll
+                for (int u = 0; u < NCH; ++u) {
+                    const int src = src_lane<LPV, NCH>(lane, u);
+                    const float sk = __shfl_sync(0xffffffffu, sK, src), sv = __shfl_sync(0xffffffffu, sV, src);
+                    const float lk = __shfl_sync(0xffffffffu, lK, src), lv = __shfl_sync(0xffffffffu, lV, src);
+                    const int64_t off = (int64_t)((cb + u) * HPC + lane_h) * g.sh;
+                    st_stream(krow + off, dequant_int2(kv[u], sk, lk));
+                    st_stream(vrow + off, dequant_int2(vv[u], sv, lv));
+                }
+            } else if (!LOW2 && t == 4u) {
                 const uint8_t *ks = lbase + lo.seg_off[4] + (uint64_t)slot * (row_elems / 2) + cb * 128 + lane * 4;
                 const uint8_t *vs = lbase + lo.seg_off[5] + (uint64_t)slot * (row_elems / 2) + cb * 128 + lane * 4;
                 const int head = (cb + my_chunk) * HPC + (int)(lane / LPV);
@@ -244,9 +283,13 @@ static cudaError_t launch_unpack_d(const Geom &g, const Layout &lo, const uint8_
 {
     dim3 grid(g.tiles, g.L, g.R);
     if ((g.Hkv * D) % 256 == 0) {
-        if (g.row_chunks % 4 == 0) unpack_fast_kernel<D, 4, 3><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tile_base);
-        else if (g.row_chunks % 2 == 0) unpack_fast_kernel<D, 2, 3><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tile_base);
-        else unpack_fast_kernel<D, 1, 3><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tile_base);
+        if (g.low_code == 2) {
+            if (g.row_chunks % 4 == 0) unpack_fast_kernel<D, 4, 3, true><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tile_base);
+            else if (g.row_chunks % 2 == 0) unpack_fast_kernel<D, 2, 3, true><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tile_base);
+            else unpack_fast_kernel<D, 1, 3, true><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tile_base);
+        } else if (g.row_chunks % 4 == 0) unpack_fast_kernel<D, 4, 3, false><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tile_base);
+        else if (g.row_chunks % 2 == 0) unpack_fast_kernel<D, 2, 3, false><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tile_base);
+        else unpack_fast_kernel<D, 1, 3, false><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tile_base);
     } else {
         unpack_kernel<D><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tile_base);
     }

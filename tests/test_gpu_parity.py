@@ -457,3 +457,53 @@ def test_long_sequences_beyond_the_shared_memory_selection_path(n, b, a4):
     case = Case(cfg, b, with_importance=False, importance_override=I)
     out = gpu_pipeline(case, run_importance=False)
     assert_bit_exact(case, out)
+
+
+@pytest.mark.parametrize("d,Hkv,Hq,n,b", [(128, 8, 32, 1000, 0.2), (128, 4, 8, 513, 0.125), (128, 2, 2, 300, 0.3),
+                                          (64, 3, 3, 257, 0.2), (256, 2, 4, 640, 0.15), (64, 8, 8, 96, 0.05),
+                                          (256, 1, 2, 129, 0.22)])
+def test_two_bit_low_tier_parity(d, Hkv, Hq, n, b):
+    """NEXT-4: blobs whose low tier is asymmetric 2-bit (allow_int4 = 2, budget in eighths): counts, tier map (code 2),
+    every blob byte and every dequantised element bit-exact against the oracle; fast kernels (row = 4, 2, 1 chunk
+    batches) and the generic ones (rows that are not a multiple of 256 elements)."""
+    cfg = skv_synth.Config("int2", L=2, Hq=Hq, Hkv=Hkv, d=d, n=n, w=8, R=2, n_sink=2, seed=51, allow_int4=2)
+    case = Case(cfg, b, with_importance=False)
+    assert case.counts.low_bits == 2 and any((t == 2).any() for t in case.tier)
+    out = gpu_pipeline(case, run_importance=False)
+    assert_bit_exact(case, out)
+    # error bound of the 2-bit tier on the dequantised cache: half a step of the vector's range
+    for r in range(case.R):
+        m = case.tier[r] == 2
+        X, Y = case.K[r].numpy().astype(np.float64), out["K2"][r].astype(np.float64)
+        rng_ = X.max(axis=-1, keepdims=True) - X.min(axis=-1, keepdims=True)
+        ok = np.abs(Y - X) <= rng_ / 6 * (1 + 1e-3) + np.abs(Y) * 2.0 ** -11 + 1e-12
+        assert ok[m].all()
+
+
+def test_two_bit_upgrade_to_int8_patch():
+    """NEXT-4 + NEXT-3: a 2-bit token upgraded to INT8 by an upgrade blob (the upgrade blob itself has no low tier)."""
+    dev = torch.device("cuda:0")
+    cfg = skv_synth.Config("int2up", L=2, Hq=4, Hkv=2, d=128, n=400, w=8, R=1, n_sink=2, seed=52, allow_int4=2)
+    case = Case(cfg, 0.15, with_importance=False)
+    out = gpu_pipeline(case, run_importance=False)
+    shape = case.shape()
+    ws = torch.empty(skv.skv_workspace_bytes(shape, cfg.w), dtype=torch.uint8, device=dev)
+    Kc, Vc = torch.from_numpy(out["K2"]).to(dev), torch.from_numpy(out["V2"]).to(dev)
+    tc = torch.from_numpy(out["tier"]).to(dev)
+    k = 25
+    up = np.zeros((1, cfg.L, cfg.n), np.uint8)
+    for l in range(cfg.L):
+        up[0, l, np.flatnonzero(case.tier[0][l] == 2)[:k]] = 8
+    uc = skv.skv_counts_from_populations(shape, 0, k, 0)
+    bb = skv.skv_blob_bytes(shape, uc)
+    ublob = torch.empty((bb,), dtype=torch.uint8, device=dev)
+    skv.skv_pack(shape, case.K.to(dev), case.V.to(dev), torch.from_numpy(up).to(dev), uc, ublob, ws)
+    skv.skv_unpack_patch(shape, ublob, bb, uc, Kc, Vc, tc, ws)
+    torch.cuda.synchronize()
+    oc = oracle.Counts(0, k, 0, cfg.n - k, uc.budget_q4, uc.spent_q4)
+    blob_or = oracle.pack(case.K[0].numpy(), case.V[0].numpy(), up[0], oc, True)
+    assert np.array_equal(ublob.cpu().numpy(), blob_or)
+    K_or, V_or, t_or = oracle.unpack_patch(blob_or, case.K2[0], case.V2[0], case.tier[0])
+    assert np.array_equal(Kc[0].cpu().numpy().view(np.uint16), K_or.view(np.uint16))
+    assert np.array_equal(Vc[0].cpu().numpy().view(np.uint16), V_or.view(np.uint16))
+    assert np.array_equal(tc[0].cpu().numpy(), t_or) and set(np.unique(t_or)) <= {16, 8, 2, 0}

@@ -38,7 +38,7 @@ def test_tier_counts_match_oracle_sweep():
         rngs = []
         for _r in range(int(rng.integers(0, 4))):
             a = int(rng.integers(0, n + 1)); e = int(rng.integers(a, n + 1)); rngs.append((a, e))
-        a4 = bool(rng.integers(0, 2))
+        a4 = int(rng.integers(0, 3))                      # 0 = 2-tier, 1 = INT4 low tier, 2 = 2-bit low tier (NEXT-4)
         shape = skv.make_shape(2, 4, 2, 128, n)
         pol = skv.make_policy(b, s, rngs, a4)
         try:
@@ -111,6 +111,15 @@ def test_blob_check_accepts_oracle_blob_and_rejects_corruption():
         assert ei.value.status == skv.SKV_ERR_BAD_BLOB, off
     with pytest.raises(skv.SkvError):
         skv.skv_blob_check(blob[:256].tobytes(), blob.size - 256)
+    # NEXT-4: a blob whose low tier is 2-bit (flags = 3, budget in eighths)
+    c2, prot = oracle.tier_counts(n, 0.2, 4, [], 2)
+    tier2 = oracle.assign(rng.random((L_, n)).astype(np.float32), prot, c2)
+    assert set(np.unique(tier2)) <= {16, 8, 2, 0} and (tier2 == 2).any()
+    blob2 = oracle.pack(K, V, tier2, c2, 2)
+    s2, cc2 = skv.skv_blob_check(blob2[:256].tobytes(), blob2.size)
+    assert cc2.as_tuple() == (c2.n16, c2.n8, c2.n4, c2.n0) and cc2.allow_int4 == 2
+    assert (cc2.budget_q4, cc2.spent_q4) == (c2.budget_q4, c2.spent_q4)
+    assert skv.skv_blob_bytes(s2_shape := skv.make_shape(L_, Hkv, Hkv, d, n), cc2) == blob2.size
 
 
 def test_workspace_covers_every_entry_point():

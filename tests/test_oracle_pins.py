@@ -612,3 +612,109 @@ def test_upgrade_patch_restores_exact_rows_and_touches_nothing_else():
     K3, V3, t3 = oracle.unpack_patch(oracle.pack(K, V, up_all, ac, True), K1, V1, t1)
     assert np.array_equal(K3.view(np.uint16), K.view(np.uint16)) and np.array_equal(V3.view(np.uint16), V.view(np.uint16))
     assert (t3 == 16).all()
+
+
+# ----------------------------------------------------------------------------------------------
+# NEXT-4: asymmetric 2-bit low tier
+# ----------------------------------------------------------------------------------------------
+def test_quantizer2_worked_examples_and_special_cases():
+    rows = read_golden(os.path.join(GOLD, "quantizer2_worked.txt"))
+    groups = {}
+    for name, x, code, ybits in rows:
+        groups.setdefault(name, []).append((float(x), int(code), int(ybits, 16)))
+    assert len(groups) == 3
+    for name, items in groups.items():
+        xs = [it[0] for it in items]
+        v = np.full(64, min(xs), np.float16)
+        v[:len(items)] = xs
+        lo, hi, q = oracle.quantize2_vector(v)
+        assert lo == int(np.float16(min(xs)).view(np.uint16)) and hi == int(np.float16(max(xs)).view(np.uint16)), name
+        assert q[:len(items)].tolist() == [it[1] for it in items], name
+        assert (q[len(items):] == 0).all()
+        y = oracle.dequantize2_vector(q, lo, hi)
+        assert y[:len(items)].view(np.uint16).tolist() == [it[2] for it in items], name
+    # constant vector: r = 0 -> codes 0, reconstruction exact; signed zeros are recorded as +0
+    c = np.full(64, -3.5, np.float16)
+    lo, hi, q = oracle.quantize2_vector(c)
+    assert lo == hi == int(np.float16(-3.5).view(np.uint16)) and (q == 0).all()
+    assert np.array_equal(oracle.dequantize2_vector(q, lo, hi), c)
+    z = np.zeros(64, np.float16); z[5] = -0.0
+    lo, hi, q = oracle.quantize2_vector(z)
+    assert lo == 0 and hi == 0 and (oracle.dequantize2_vector(q, lo, hi).view(np.uint16) == 0).all()
+    big = np.full(64, -65504.0, np.float16); big[1] = 65504.0
+    lo, hi, q = oracle.quantize2_vector(big)
+    assert q[0] == 0 and q[1] == 3
+    assert np.array_equal(oracle.dequantize2_vector(q, lo, hi), big)            # no overflow at the fp16 extremes
+
+
+def test_quantizer2_codes_are_exactly_rounded_and_error_is_half_a_step():
+    from fractions import Fraction
+    import math
+    rng = np.random.default_rng(12)
+    for _ in range(40):
+        v = (rng.standard_normal(128) * rng.uniform(0.01, 30) + rng.uniform(-5, 5)).astype(np.float16)
+        lo_b, hi_b, q = oracle.quantize2_vector(v)
+        lo = np.float32(np.uint16(lo_b).view(np.float16)); hi = np.float32(np.uint16(hi_b).view(np.float16))
+        assert float(lo) == float(v.min()) and float(hi) == float(v.max())
+        r = np.float32(hi - lo)
+        inv = np.float32(3.0) / r
+        for e, code in zip(v, q):
+            dx = np.float32(np.float32(e) - lo)
+            ex = Fraction(float(dx)) * Fraction(float(inv))
+            fl = math.floor(ex); fr = ex - fl
+            want = fl if fr < Fraction(1, 2) else fl + 1 if fr > Fraction(1, 2) else (fl if fl % 2 == 0 else fl + 1)
+            assert int(code) == max(0, min(3, want))
+        assert q.min() == 0 and q.max() == 3                                      # the extremes hit codes 0 and 3
+        step = float(r) / 3.0
+        y = oracle.dequantize2_vector(q, lo_b, hi_b).astype(np.float64)
+        ulp = np.spacing(np.abs(y).astype(np.float16)).astype(np.float64)
+        assert (np.abs(y - v.astype(np.float64)) <= step / 2 * (1 + 1e-3) + ulp / 2 + 1e-12).all()
+
+
+def test_tier_counts_two_bit_low_tier():
+    # c(2-bit) = 1/8: b = 1/8 -> everything 2-bit; b = 0.5 -> everything INT8; b = 5/16 -> half and half; b = 1 -> FP16
+    for b, want in ((0.125, (0, 0, 1000, 0)), (0.5, (0, 1000, 0, 0)), (0.3125, (0, 500, 500, 0)), (1.0, (1000, 0, 0, 0)),
+                    (0.75, (500, 500, 0, 0)), (0.0625, (0, 0, 500, 500))):
+        c, _ = oracle.tier_counts(1000, b, 0, [], 2)
+        assert (c.n16, c.n8, c.n4, c.n0) == want and c.low_bits == 2, (b, c)
+    rng = np.random.default_rng(2)
+    for _ in range(300):
+        n = int(rng.integers(8, 5000)); s = int(rng.integers(0, 5)); b = float(rng.uniform(0.02, 1.0))
+        try:
+            c, prot = oracle.tier_counts(n, b, s, [], 2)
+        except ValueError:
+            assert 8 * s > int(np.floor(8 * b * n + 1e-6))
+            continue
+        assert c.n16 + c.n8 + c.n4 + c.n0 == n and c.n16 >= s
+        assert c.spent_q4 == 8 * c.n16 + 4 * c.n8 + c.n4 <= c.budget_q4 == int(np.floor(8 * b * n + 1e-6))
+        if c.n16 < n:
+            assert c.budget_q4 - c.spent_q4 < 4                                   # less than the cheapest upgrade left over
+        assert sum(x > 0 for x in (c.n16 - int(prot.sum()), c.n8, c.n4, c.n0)) <= 2   # two adjacent tiers at most
+
+
+def test_two_bit_blob_layout_round_trip_and_hand_written_bytes():
+    L, n, Hkv, d = 1, 3, 1, 64
+    rows = [r for r in read_golden(os.path.join(GOLD, "quantizer2_worked.txt")) if r[0] == "Z1"]
+    K = np.zeros((L, n, Hkv, d), np.float16); V = np.zeros((L, n, Hkv, d), np.float16)
+    K[0, 0, 0, :] = np.arange(64) / 4.0                       # FP16 token
+    K[0, 1, 0, :] = -1.0; K[0, 1, 0, :len(rows)] = [float(r[1]) for r in rows]          # 2-bit token, Z1 vector
+    V[0, 1, 0, :] = 0.0; V[0, 1, 0, :2] = [0.75, 0.375]                                # Z2: codes 3, 2, 0, 0 ...
+    K[0, 2] = 5.0; V[0, 2] = -5.0                             # dropped
+    tier = np.array([[16, 2, 0]], np.uint8)
+    counts = oracle.Counts(1, 0, 1, 1, 9, 9, low_bits=2)
+    blob = oracle.pack(K, V, tier, counts, 2)
+    assert int.from_bytes(bytes(blob[40:44]), "little") == 3                          # flags: low tier allowed, 2-bit
+    seg = [int.from_bytes(bytes(blob[80 + 8 * i:88 + 8 * i]), "little") for i in range(10)]
+    # raw sizes: K16,V16 128; K8,V8 0; K2,V2 16 (64 codes / 4); SK8,SV8 0; SK2,SV2 4 -> offsets step by 256 where non-empty
+    assert seg == [0, 256, 512, 512, 512, 768, 1024, 1024, 1024, 1280]
+    base = 256 + 256
+    codes = [int(r[2]) for r in rows] + [0] * (64 - len(rows))
+    want_k = bytes((codes[4 * i] | codes[4 * i + 1] << 2 | codes[4 * i + 2] << 4 | codes[4 * i + 3] << 6) for i in range(16))
+    assert bytes(blob[base + 512:base + 528]) == want_k
+    assert bytes(blob[base + 768:base + 784]) == bytes([3 | 2 << 2]) + bytes(15)
+    assert bytes(blob[base + 1024:base + 1028]) == bytes([0x00, 0xBC, 0x00, 0x40])    # lo = -1 (0xBC00), hi = 2 (0x4000)
+    assert bytes(blob[base + 1280:base + 1284]) == bytes([0x00, 0x00, 0x00, 0x3A])    # lo = 0, hi = 0.75 (0x3A00)
+    K2, V2, t2 = oracle.unpack(blob, L, Hkv, d, n)
+    assert np.array_equal(t2, tier) and np.array_equal(K2[0, 0], K[0, 0]) and (K2[0, 2] == 0).all()
+    assert K2[0, 1, 0, :len(rows)].view(np.uint16).tolist() == [int(r[3], 16) for r in rows]
+    assert V2[0, 1, 0, :3].tolist() == [0.75, 0.5, 0.0]
