@@ -315,27 +315,31 @@ def run_e2e(cfg, b, R, dev, steps, warmup, chunk_layers=4, depth=3):
     import skv_synth
     L = cfg.L
     pin = dict(pin_memory=True)
-    hK = torch.empty((R, L, cfg.n, cfg.Hkv, cfg.d), dtype=torch.float16, **pin)
+    # pinned host footprint is bounded (N ranks share one host): two distinct requests in, a two-request ring out; the
+    # R requests of a step alternate between them -- the bytes copied per step are those of R requests
+    Rh = min(R, 2)
+    hK = torch.empty((Rh, L, cfg.n, cfg.Hkv, cfg.d), dtype=torch.float16, **pin)
     hV = torch.empty_like(hK, **pin)
-    hQ = torch.empty((R, L, cfg.Hq, cfg.w, cfg.d), dtype=torch.float16, **pin)
-    for r in range(R):
+    hQ = torch.empty((Rh, L, cfg.Hq, cfg.w, cfg.d), dtype=torch.float16, **pin)
+    for r in range(Rh):
         k, v = skv_synth.make_kv(cfg, r, device=dev)
         hK[r].copy_(k); hV[r].copy_(v); hQ[r].copy_(skv_synth.make_q(cfg, r, device=dev))
         del k, v
-    hKo = torch.empty((min(R, 2), L, cfg.n, cfg.Hkv, cfg.d), dtype=torch.float16, **pin)    # 2-request output ring
+    hKo = torch.empty((Rh, L, cfg.n, cfg.Hkv, cfg.d), dtype=torch.float16, **pin)
     hVo = torch.empty_like(hKo, **pin)
+    reqs = [dict(K=hK[r % Rh], V=hV[r % Rh], Q=hQ[r % Rh], Ko=hKo[r % Rh], Vo=hVo[r % Rh]) for r in range(R)]
     lpc = max(1, min(L, chunk_layers))
     pipe = LayerPipelinedTransfer(L, cfg.Hq, cfg.Hkv, cfg.d, cfg.n, cfg.w, b, cfg.n_sink, cfg.ranges, cfg.allow_int4,
                                   layers_per_chunk=lpc, depth=depth, device=dev)
     torch.cuda.synchronize()
     for _ in range(warmup):
-        pipe.run(hK, hV, hQ, hKo, hVo)
+        pipe.run_ragged(reqs)
     barrier()
     torch.cuda.synchronize()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
     for _ in range(steps):
-        pipe.run(hK, hV, hQ, hKo, hVo)
+        pipe.run_ragged(reqs)
     e1.record()
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1) / steps
