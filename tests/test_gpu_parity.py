@@ -507,3 +507,33 @@ def test_two_bit_upgrade_to_int8_patch():
     assert np.array_equal(Kc[0].cpu().numpy().view(np.uint16), K_or.view(np.uint16))
     assert np.array_equal(Vc[0].cpu().numpy().view(np.uint16), V_or.view(np.uint16))
     assert np.array_equal(tc[0].cpu().numpy(), t_or) and set(np.unique(t_or)) <= {16, 8, 2, 0}
+
+
+def test_results_are_bitwise_reproducible_run_to_run():
+    """No atomics and fixed reduction orders everywhere: two runs of the whole path on the same inputs agree bit for
+    bit (importance included), whatever the CTA scheduling."""
+    dev = torch.device("cuda:0")
+    cfg = C["C5"].scaled(L=2, n=8192, R=2)
+    K = torch.stack([skv_synth.make_kv(cfg, r)[0] for r in range(2)]).to(dev)
+    V = torch.stack([skv_synth.make_kv(cfg, r)[1] for r in range(2)]).to(dev)
+    Q = torch.stack([skv_synth.make_q(cfg, r) for r in range(2)]).to(dev)
+    shape = skv.make_shape(cfg.L, cfg.Hq, cfg.Hkv, cfg.d, cfg.n, 2)
+    pol = skv.make_policy(0.4, cfg.n_sink, cfg.ranges, cfg.allow_int4)
+    ws = torch.empty(skv.skv_workspace_bytes(shape, cfg.w), dtype=torch.uint8, device=dev)
+    runs = []
+    for _ in range(3):
+        ws.fill_(0xCD)                                                   # stale workspace contents must not matter
+        I = torch.empty((2, cfg.L, cfg.n), dtype=torch.float32, device=dev)
+        tier = torch.empty((2, cfg.L, cfg.n), dtype=torch.uint8, device=dev)
+        skv.skv_importance(shape, K, Q, cfg.w, I, ws)
+        counts = skv.skv_assign_tiers(shape, pol, I, tier, ws)
+        bb = skv.skv_blob_bytes(shape, counts)
+        blob = torch.empty((2 * bb,), dtype=torch.uint8, device=dev)
+        skv.skv_pack(shape, K, V, tier, counts, blob, ws)
+        Ko, Vo = torch.empty_like(K), torch.empty_like(V)
+        skv.skv_unpack(shape, blob, bb, counts, Ko, Vo, None, ws)
+        torch.cuda.synchronize()
+        runs.append((I, tier, blob, Ko, Vo))
+    for other in runs[1:]:
+        for a, b_ in zip(runs[0], other):
+            assert torch.equal(a.view(torch.uint8) if a.dtype != torch.uint8 else a, b_.view(torch.uint8) if b_.dtype != torch.uint8 else b_)
