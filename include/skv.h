@@ -144,6 +144,15 @@ int skv_assign_tiers(const skv_shape *shape, const skv_policy *policy, const flo
                      uint8_t *tier_map_dev, skv_counts *counts_out_host,
                      void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
 
+/* DEVICE.  The same selection with EXPLICIT tier populations instead of a budget (ablation policies of PAPER.md:271,
+ * :503 -- e.g. "Balanced", whose fractions the paper does not define; Random_Tier is skv_assign_tiers with random
+ * scores).  counts: from skv_counts_from_populations(); positions [0,n_sink) and the n_ranges half-open ranges (HOST)
+ * are FP16 and count towards n16 (SKV_ERR_BUDGET_INFEASIBLE if they exceed it).  The rest is ranked as in
+ * skv_assign_tiers: top n16-P -> 16, next n8 -> 8, next n4 -> low tier, rest -> 0. */
+int skv_assign_tiers_counts(const skv_shape *shape, const skv_counts *counts, int32_t n_sink, int32_t n_ranges,
+                            const int32_t *ranges, const float *importance_dev, uint8_t *tier_map_dev,
+                            void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
+
 /* DEVICE.  Writes n_requests blobs at blob_dev + r*skv_blob_bytes(); every byte of each blob is written
  * (pads zero) so blobs are memcmp-comparable.  blob_dev must be 256-B aligned.  `counts` must match the
  * tier map of every layer (maps produced by skv_assign_tiers always do); on a mismatch slots are clamped

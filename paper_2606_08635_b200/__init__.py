@@ -58,7 +58,7 @@ class skv_counts(C.Structure):
 
 EXPORTS = ("skv_tier_counts", "skv_blob_bytes", "skv_workspace_bytes", "skv_blob_check", "skv_importance",
            "skv_importance_kvnorm", "skv_assign_tiers", "skv_pack", "skv_unpack", "skv_unpack_patch",
-           "skv_counts_from_populations", "skv_strerror", "skv_version")
+           "skv_counts_from_populations", "skv_assign_tiers_counts", "skv_strerror", "skv_version")
 
 _lib = None
 
@@ -81,6 +81,7 @@ def lib():
         L.skv_importance.argtypes = [P(skv_shape), V, V, C.c_int32, C.c_int32, C.c_float, V, V, C.c_size_t, V]
         L.skv_importance_kvnorm.argtypes = [P(skv_shape), V, C.c_float, V, V, C.c_size_t, V]
         L.skv_assign_tiers.argtypes = [P(skv_shape), P(skv_policy), V, V, P(skv_counts), V, C.c_size_t, V]
+        L.skv_assign_tiers_counts.argtypes = [P(skv_shape), P(skv_counts), C.c_int32, C.c_int32, P(C.c_int32), V, V, V, C.c_size_t, V]
         L.skv_pack.argtypes = [P(skv_shape), V, V, V, P(skv_counts), V, C.c_size_t, V, C.c_size_t, V]
         L.skv_unpack.argtypes = [P(skv_shape), V, C.c_size_t, P(skv_counts), V, V, V, V, C.c_size_t, V]
         L.skv_unpack_patch.argtypes = L.skv_unpack.argtypes
@@ -235,3 +236,11 @@ def skv_counts_from_populations(shape, n16, n8=0, n4=0, allow_int4=True):
     _check(lib().skv_counts_from_populations(C.byref(shape), int(n16), int(n8), int(n4), _low_mode(allow_int4),
                                              C.byref(c)), "skv_counts_from_populations")
     return c
+
+
+def skv_assign_tiers_counts(shape, counts, importance, tier_map, workspace, n_sink=0, ranges=(), stream=None):
+    flat = [int(v) for r in ranges for v in r]
+    arr = (C.c_int32 * max(1, len(flat)))(*flat)
+    _check(lib().skv_assign_tiers_counts(C.byref(shape), C.byref(counts), int(n_sink), len(flat) // 2,
+                                         C.cast(arr, C.POINTER(C.c_int32)), _ptr(importance), _ptr(tier_map),
+                                         _ptr(workspace), _nbytes(workspace), _stream(stream)), "skv_assign_tiers_counts")

@@ -249,16 +249,9 @@ int skv_importance_kvnorm(const skv_shape *shape, const void *K_dev, float lambd
     return e == cudaSuccess ? SKV_OK : SKV_ERR_CUDA;
 }
 
-int skv_assign_tiers(const skv_shape *shape, const skv_policy *policy, const float *importance_dev,
-                     uint8_t *tier_map_dev, skv_counts *counts_out_host, void *ws, size_t ws_bytes, void *cuda_stream)
+static int assign_launch(const skv_shape *shape, const skv_counts &c, const std::vector<std::pair<int32_t, int32_t>> &prot,
+                         const float *importance_dev, uint8_t *tier_map_dev, void *ws, size_t ws_bytes, void *cuda_stream)
 {
-    int rc = check_dims_supported(shape);
-    if (rc) return rc;
-    if (!policy || !importance_dev || !tier_map_dev) return SKV_ERR_INVALID_ARG;
-    skv_counts c;
-    std::vector<std::pair<int32_t, int32_t>> prot;
-    rc = tier_counts_impl(shape, policy, &c, prot);
-    if (rc) return rc;
     if (prot.size() > 32) return SKV_ERR_UNSUPPORTED;    // more than 32 disjoint protected intervals
     const size_t key_bytes = (size_t)shape->n_requests * shape->n_layers * shape->n_tokens * sizeof(uint32_t);
     const bool need_ws = (size_t)shape->n_tokens * 4 > 200 * 1024;
@@ -269,9 +262,40 @@ int skv_assign_tiers(const skv_shape *shape, const skv_policy *policy, const flo
     for (size_t i = 0; i < prot.size(); ++i) { iv.lo[i] = prot[i].first; iv.hi[i] = prot[i].second; }
     const Geom g = make_geom(shape, &c);
     cudaError_t e = launch_assign(g, iv, importance_dev, tier_map_dev, (uint32_t *)ws, (cudaStream_t)cuda_stream);
-    if (e != cudaSuccess) return SKV_ERR_CUDA;
+    return e == cudaSuccess ? SKV_OK : SKV_ERR_CUDA;
+}
+
+int skv_assign_tiers(const skv_shape *shape, const skv_policy *policy, const float *importance_dev,
+                     uint8_t *tier_map_dev, skv_counts *counts_out_host, void *ws, size_t ws_bytes, void *cuda_stream)
+{
+    int rc = check_dims_supported(shape);
+    if (rc) return rc;
+    if (!policy || !importance_dev || !tier_map_dev) return SKV_ERR_INVALID_ARG;
+    skv_counts c;
+    std::vector<std::pair<int32_t, int32_t>> prot;
+    rc = tier_counts_impl(shape, policy, &c, prot);
+    if (rc) return rc;
+    rc = assign_launch(shape, c, prot, importance_dev, tier_map_dev, ws, ws_bytes, cuda_stream);
+    if (rc) return rc;
     if (counts_out_host) *counts_out_host = c;
     return SKV_OK;
+}
+
+int skv_assign_tiers_counts(const skv_shape *shape, const skv_counts *counts, int32_t n_sink, int32_t n_ranges,
+                            const int32_t *ranges, const float *importance_dev, uint8_t *tier_map_dev,
+                            void *ws, size_t ws_bytes, void *cuda_stream)
+{
+    int rc = check_dims_supported(shape);
+    if (rc) return rc;
+    if (!importance_dev || !tier_map_dev || !counts_ok(shape, counts)) return SKV_ERR_INVALID_ARG;
+    skv_policy pol;
+    memset(&pol, 0, sizeof(pol));
+    pol.budget = 1.0; pol.n_sink = n_sink; pol.n_ranges = n_ranges; pol.ranges = ranges;
+    std::vector<std::pair<int32_t, int32_t>> prot;
+    const int64_t P = merge_protected(shape, &pol, prot);
+    if (P < 0) return SKV_ERR_INVALID_ARG;
+    if (P > counts->n16) return SKV_ERR_BUDGET_INFEASIBLE;            // the protected positions are all FP16
+    return assign_launch(shape, *counts, prot, importance_dev, tier_map_dev, ws, ws_bytes, cuda_stream);
 }
 
 int skv_pack(const skv_shape *shape, const void *K_dev, const void *V_dev, const uint8_t *tier_map_dev,

@@ -537,3 +537,32 @@ def test_results_are_bitwise_reproducible_run_to_run():
     for other in runs[1:]:
         for a, b_ in zip(runs[0], other):
             assert torch.equal(a.view(torch.uint8) if a.dtype != torch.uint8 else a, b_.view(torch.uint8) if b_.dtype != torch.uint8 else b_)
+
+
+def test_assign_with_explicit_populations_balanced_and_random_tier():
+    """NEXT-1 ablation policies: 'Balanced' = equal thirds through explicit populations, and
+    Random_Tier = the budget's own counts with random scores; both against the oracle's sort."""
+    dev = torch.device("cuda:0")
+    L, n, s = 3, 3001, 4
+    shape = skv.make_shape(L, 4, 2, 64, n, 1)
+    ws = torch.empty(skv.skv_workspace_bytes(shape, 0), dtype=torch.uint8, device=dev)
+    rng = np.random.default_rng(8)
+    I = rng.random((L, n)).astype(np.float32)
+    m = n - s
+    n8 = n4 = m // 3
+    n16 = n - n8 - n4                                               # sinks + a third (+ remainder)
+    counts = skv.skv_counts_from_populations(shape, n16, n8, n4)
+    tier = torch.full((1, L, n), 0xEE, dtype=torch.uint8, device=dev)
+    skv.skv_assign_tiers_counts(shape, counts, torch.from_numpy(I)[None].to(dev), tier, ws, n_sink=s)
+    prot = np.zeros(n, np.uint8); prot[:s] = 1
+    want = oracle.assign(I, prot, oracle.Counts(n16, n8, n4, 0, counts.budget_q4, counts.spent_q4))
+    assert np.array_equal(tier.cpu().numpy()[0], want)
+    with pytest.raises(skv.SkvError):                               # protected positions alone exceed n16
+        skv.skv_assign_tiers_counts(shape, skv.skv_counts_from_populations(shape, 2, n - 2, 0),
+                                    torch.from_numpy(I)[None].to(dev), tier, ws, n_sink=s)
+    # Random_Tier: closed-form counts of b = 0.4, ranked by random numbers supplied by the caller
+    pol = skv.make_policy(0.4, s, (), True)
+    c = skv.skv_assign_tiers(shape, pol, torch.from_numpy(I)[None].to(dev), tier, ws)
+    oc, prot = oracle.tier_counts(n, 0.4, s, (), True)
+    assert c.as_tuple() == (oc.n16, oc.n8, oc.n4, oc.n0)
+    assert np.array_equal(tier.cpu().numpy()[0], oracle.assign(I, prot, oc))
