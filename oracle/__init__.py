@@ -25,6 +25,8 @@ def lib():
         _lib.orc_half_to_float.argtypes = [C.c_uint16]
         _lib.orc_float_to_half.restype = C.c_uint16
         _lib.orc_float_to_half.argtypes = [C.c_float]
+        _lib.orc_float_to_bf16.restype = C.c_uint16
+        _lib.orc_float_to_bf16.argtypes = [C.c_float]
         _lib.orc_blob_bytes.restype = C.c_uint64
         _lib.orc_blob_bytes_low.restype = C.c_uint64
         _lib.orc_max_threads.restype = C.c_int
@@ -89,26 +91,31 @@ def tier_counts(n, b, n_sink=0, ranges=(), allow_int4=True):
     return Counts(*[int(v) for v in out], low_bits=2 if _mode(allow_int4) == 2 else 4), prot
 
 
-def importance(K, Q, causal=True, lam=0.0):
+def _elems(x, bf16):
+    """fp16 caches travel as numpy float16; bfloat16 caches (numpy has no such type) as uint16 bit patterns."""
+    return _c(x, np.uint16 if bf16 else np.float16)
+
+
+def importance(K, Q, causal=True, lam=0.0, bf16=False):
     """O1.  K [L][n][Hkv][d] f16, Q [L][Hq][w][d] f16 -> I [L][n] f32."""
-    K = _c(K, np.float16)
-    Q = _c(Q, np.float16)
+    K = _elems(K, bf16)
+    Q = _elems(Q, bf16)
     L, n, Hkv, d = K.shape
     L2, Hq, w, d2 = Q.shape
     assert L == L2 and d == d2 and Hq % Hkv == 0 and 1 <= w <= n
     I = np.empty((L, n), dtype=np.float32)
-    lib().orc_importance(C.c_int32(L), C.c_int32(Hq), C.c_int32(Hkv), C.c_int32(d), C.c_int64(n),
-                         C.c_int32(w), C.c_int32(1 if causal else 0), C.c_double(float(lam)),
-                         _p(K), _p(Q), _p(I))
+    lib().orc_importance_dt(C.c_int32(L), C.c_int32(Hq), C.c_int32(Hkv), C.c_int32(d), C.c_int64(n),
+                            C.c_int32(w), C.c_int32(1 if causal else 0), C.c_double(float(lam)),
+                            _p(K), _p(Q), _p(I), C.c_int32(1 if bf16 else 0))
     return I
 
 
-def importance_kvnorm(K, lam=0.0):
-    K = _c(K, np.float16)
+def importance_kvnorm(K, lam=0.0, bf16=False):
+    K = _elems(K, bf16)
     L, n, Hkv, d = K.shape
     I = np.empty((L, n), dtype=np.float32)
-    lib().orc_importance_kvnorm(C.c_int32(L), C.c_int32(Hkv), C.c_int32(d), C.c_int64(n),
-                                C.c_double(float(lam)), _p(K), _p(I))
+    lib().orc_importance_kvnorm_dt(C.c_int32(L), C.c_int32(Hkv), C.c_int32(d), C.c_int64(n),
+                                   C.c_double(float(lam)), _p(K), _p(I), C.c_int32(1 if bf16 else 0))
     return I
 
 
@@ -129,26 +136,29 @@ def blob_bytes(L, Hkv, d, n, counts: Counts) -> int:
                                         C.c_int32(counts.low_bits)))
 
 
-def pack(K, V, tier, counts: Counts, allow_int4=True):
+def pack(K, V, tier, counts: Counts, allow_int4=True, bf16=False):
     """O4+O5.  Returns the SKV1 blob as uint8[total_bytes]."""
-    K = _c(K, np.float16)
-    V = _c(V, np.float16)
+    K = _elems(K, bf16)
+    V = _elems(V, bf16)
     tier = _c(tier, np.uint8)
     L, n, Hkv, d = K.shape
     assert V.shape == K.shape and tier.shape == (L, n)
     blob = np.empty(blob_bytes(L, Hkv, d, n, counts), dtype=np.uint8)
-    rc = lib().orc_pack(C.c_int32(L), C.c_int32(Hkv), C.c_int32(d), C.c_int64(n), _p(K), _p(V),
-                        _p(tier), counts.arr(), C.c_int32(2 if counts.low_bits == 2 else _mode(allow_int4)), _p(blob))
+    rc = lib().orc_pack_dt(C.c_int32(L), C.c_int32(Hkv), C.c_int32(d), C.c_int64(n), _p(K), _p(V),
+                           _p(tier), counts.arr(), C.c_int32(2 if counts.low_bits == 2 else _mode(allow_int4)), _p(blob),
+                           C.c_int32(1 if bf16 else 0))
     if rc != 0:
         raise ValueError(f"orc_pack rc={rc} (tier map does not match counts)")
     return blob
 
 
-def unpack(blob, L, Hkv, d, n):
-    """O6.  Returns (K, V, tier) dense."""
+def unpack(blob, L, Hkv, d, n, bf16=False):
+    """O6.  Returns (K, V, tier) dense (K, V as uint16 bit patterns when the blob holds bfloat16 elements)."""
     blob = _c(blob, np.uint8)
-    K = np.empty((L, n, Hkv, d), dtype=np.float16)
-    V = np.empty((L, n, Hkv, d), dtype=np.float16)
+    assert bool(blob[40] & 4) == bool(bf16), "element type of the blob (header flags bit2) differs from the request"
+    et = np.uint16 if bf16 else np.float16
+    K = np.empty((L, n, Hkv, d), dtype=et)
+    V = np.empty((L, n, Hkv, d), dtype=et)
     tier = np.empty((L, n), dtype=np.uint8)
     rc = lib().orc_unpack(_p(blob), C.c_uint64(blob.size), C.c_int32(L), C.c_int32(Hkv), C.c_int32(d),
                           C.c_int64(n), _p(K), _p(V), _p(tier))
@@ -161,8 +171,9 @@ def unpack_patch(blob, K, V, tier):
     """NEXT-3 cold-tier upgrade: applies an upgrade blob to COPIES of the dense cache K, V [L][n][Hkv][d] and of the
     tier map [L][n]; returns (K, V, tier)."""
     blob = _c(blob, np.uint8)
-    K = np.array(K, dtype=np.float16, order="C", copy=True)
-    V = np.array(V, dtype=np.float16, order="C", copy=True)
+    et = np.uint16 if (blob[40] & 4) else np.float16
+    K = np.array(K, dtype=et, order="C", copy=True)
+    V = np.array(V, dtype=et, order="C", copy=True)
     tier = np.array(tier, dtype=np.uint8, order="C", copy=True)
     L, n, Hkv, d = K.shape
     rc = lib().orc_unpack_patch(_p(blob), C.c_uint64(blob.size), C.c_int32(L), C.c_int32(Hkv), C.c_int32(d),
@@ -172,33 +183,48 @@ def unpack_patch(blob, K, V, tier):
     return K, V, tier
 
 
-def quantize2_vector(x):
+def quantize2_vector(x, bf16=False):
     """NEXT-4 asymmetric 2-bit quantizer on one vector.  x float16[d] -> (lo_bits, hi_bits, uint8[d] codes 0..3)."""
-    x = _c(x, np.float16)
+    x = _elems(x, bf16)
     q = np.empty(x.size, dtype=np.uint8)
     lo, hi = C.c_uint16(0), C.c_uint16(0)
-    lib().orc_quantize2_vector(_p(x), C.c_int32(x.size), C.byref(lo), C.byref(hi), _p(q))
+    lib().orc_quantize2_vector_dt(_p(x), C.c_int32(x.size), C.byref(lo), C.byref(hi), _p(q), C.c_int32(1 if bf16 else 0))
     return int(lo.value), int(hi.value), q
 
 
-def dequantize2_vector(q, lo_bits, hi_bits):
+def dequantize2_vector(q, lo_bits, hi_bits, bf16=False):
     q = _c(q, np.uint8)
-    y = np.empty(q.size, dtype=np.float16)
-    lib().orc_dequantize2_vector(_p(q), C.c_int32(q.size), C.c_uint16(int(lo_bits)), C.c_uint16(int(hi_bits)), _p(y))
+    y = np.empty(q.size, dtype=np.uint16 if bf16 else np.float16)
+    lib().orc_dequantize2_vector_dt(_p(q), C.c_int32(q.size), C.c_uint16(int(lo_bits)), C.c_uint16(int(hi_bits)), _p(y),
+                                    C.c_int32(1 if bf16 else 0))
     return y
 
 
-def quantize_vector(x, qmax):
-    """O4 on one vector.  x float16[d] -> (amax_bits, int8[d])."""
-    x = _c(x, np.float16)
+def bf16_to_float(bits):
+    """uint16 bit patterns -> float32 (exact)."""
+    return (np.asarray(bits, dtype=np.uint16).astype(np.uint32) << 16).view(np.float32)
+
+
+def float_to_bf16(x):
+    """float32 array -> bfloat16 bit patterns, round to nearest even (through the oracle's scalar routine)."""
+    x = np.ascontiguousarray(x, dtype=np.float32)
+    f = lib().orc_float_to_bf16
+    return np.array([f(C.c_float(float(v))) for v in x.ravel()], dtype=np.uint16).reshape(x.shape)
+
+
+def quantize_vector(x, qmax, bf16=False):
+    """O4 on one vector.  x float16[d] (or bfloat16 bits uint16[d]) -> (amax_bits, int8[d])."""
+    x = _elems(x, bf16)
     q = np.empty(x.size, dtype=np.int8)
     ab = C.c_uint16(0)
-    lib().orc_quantize_vector(_p(x), C.c_int32(x.size), C.c_int32(int(qmax)), C.byref(ab), _p(q))
+    lib().orc_quantize_vector_dt(_p(x), C.c_int32(x.size), C.c_int32(int(qmax)), C.byref(ab), _p(q),
+                                 C.c_int32(1 if bf16 else 0))
     return int(ab.value), q
 
 
-def dequantize_vector(q, qmax, amax_bits):
+def dequantize_vector(q, qmax, amax_bits, bf16=False):
     q = _c(q, np.int8)
-    y = np.empty(q.size, dtype=np.float16)
-    lib().orc_dequantize_vector(_p(q), C.c_int32(q.size), C.c_int32(int(qmax)), C.c_uint16(int(amax_bits)), _p(y))
+    y = np.empty(q.size, dtype=np.uint16 if bf16 else np.float16)
+    lib().orc_dequantize_vector_dt(_p(q), C.c_int32(q.size), C.c_int32(int(qmax)), C.c_uint16(int(amax_bits)), _p(y),
+                                   C.c_int32(1 if bf16 else 0))
     return y

@@ -80,6 +80,28 @@ uint16_t orc_float_to_half(float f)
     return (uint16_t)(sign | (exp << 10) | frac);
 }
 
+/* bfloat16 <-> binary32 (the other half of SURVEY NEXT-4; reading P20): bfloat16 is the upper half of a binary32. */
+float orc_bf16_to_float(uint16_t b)
+{
+    uint32_t u = (uint32_t)b << 16;
+    float f; memcpy(&f, &u, 4);
+    return f;
+}
+
+/* binary32 -> bfloat16, round to nearest, ties to even (finite on the path; a NaN stays a NaN). */
+uint16_t orc_float_to_bf16(float f)
+{
+    uint32_t u; memcpy(&u, &f, 4);
+    if (isnan(f)) return (uint16_t)((u >> 16) | 0x0040u);
+    const uint32_t lower = u & 0xFFFFu, upper = u >> 16;
+    if (lower > 0x8000u || (lower == 0x8000u && (upper & 1u))) return (uint16_t)(upper + 1u);   /* carries into the exponent = correct rounding */
+    return (uint16_t)upper;
+}
+
+/* element type of a cache: 0 = binary16 (the paper's s16 = 2 bytes FP16), 1 = bfloat16 */
+static float elem_to_float(uint16_t b, int32_t dtype) { return dtype ? orc_bf16_to_float(b) : orc_half_to_float(b); }
+static uint16_t float_to_elem(float f, int32_t dtype) { return dtype ? orc_float_to_bf16(f) : orc_float_to_half(f); }
+
 /* ------------------------------------------------------------------------ */
 /* O1. Importance  (Eq. 13; logits q^T k / sqrt(d) PAPER.md:109; */
 /*     Alg. 1 step 2 PAPER.md:239; readings P1, P2, P4 in DESIGN.md)          */
@@ -90,9 +112,9 @@ uint16_t orc_float_to_half(float f)
  * p = softmax(z);  A[l,j] = (1/(Hq*w)) sum_{h,i} p_{h,i,j};  I[l,j] = A[l,j] * exp(-lambda*(n-1-j)).
  * All in float64; result cast to float32 (RN).
  */
-void orc_importance(int32_t L, int32_t Hq, int32_t Hkv, int32_t d, int64_t n, int32_t w,
-                    int32_t causal, double lambda,
-                    const uint16_t *K, const uint16_t *Q, float *I)
+void orc_importance_dt(int32_t L, int32_t Hq, int32_t Hkv, int32_t d, int64_t n, int32_t w,
+                       int32_t causal, double lambda,
+                       const uint16_t *K, const uint16_t *Q, float *I, int32_t dtype)
 {
     const int32_t G = Hq / Hkv;
     const double inv_sqrt_d = 1.0 / sqrt((double)d);
@@ -104,14 +126,14 @@ void orc_importance(int32_t L, int32_t Hq, int32_t Hkv, int32_t d, int64_t n, in
         /* the layer's keys converted to double once (exact), [n][Hkv][d] */
         double *Kd = (double *)malloc((size_t)n * Hkv * d * sizeof(double));
         for (size_t e = 0; e < (size_t)n * Hkv * d; ++e)
-            Kd[e] = (double)orc_half_to_float(K[(size_t)l * n * Hkv * d + e]);
+            Kd[e] = (double)elem_to_float(K[(size_t)l * n * Hkv * d + e], dtype);
         for (int32_t h = 0; h < Hq; ++h) {
             const int32_t g = h / G;
             for (int32_t i = 0; i < w; ++i) {
                 const int64_t pos = n - w + i;
                 const int64_t last = causal ? pos : n - 1;      /* keys 0..last take part */
                 const uint16_t *q = Q + (((size_t)l * Hq + h) * w + i) * d;
-                for (int32_t c = 0; c < d; ++c) kq[c] = (double)orc_half_to_float(q[c]);
+                for (int32_t c = 0; c < d; ++c) kq[c] = (double)elem_to_float(q[c], dtype);
                 double zmax = -INFINITY;
                 for (int64_t j = 0; j <= last; ++j) {
                     const double *k = Kd + ((size_t)j * Hkv + g) * d;
@@ -132,6 +154,13 @@ void orc_importance(int32_t L, int32_t Hq, int32_t Hkv, int32_t d, int64_t n, in
         }
         free(A); free(z); free(kq); free(Kd);
     }
+}
+
+void orc_importance(int32_t L, int32_t Hq, int32_t Hkv, int32_t d, int64_t n, int32_t w,
+                    int32_t causal, double lambda,
+                    const uint16_t *K, const uint16_t *Q, float *I)
+{
+    orc_importance_dt(L, Hq, Hkv, d, n, w, causal, lambda, K, Q, I, 0);
 }
 
 /* ------------------------------------------------------------------------ */
@@ -329,6 +358,7 @@ static uint64_t get_u64(const uint8_t *p) { uint64_t v = 0; for (int i = 0; i < 
  * 11 + 24 = 35 significant bits, so binary64 holds it without rounding) and rounded ONCE, half to even
  * (reading P8 of DESIGN.md: a single rounding of the real product, not fl32 first and rint second).
  */
+/* |x| as fp16 or bf16 bits is monotone for finite values in either format */
 static uint16_t orc_amax_bits(const uint16_t *x, int32_t d)
 {
     uint16_t best = 0;                                   /* |x| as fp16 bits: monotone for finite values */
@@ -336,14 +366,15 @@ static uint16_t orc_amax_bits(const uint16_t *x, int32_t d)
     return best;
 }
 
-void orc_quantize_vector(const uint16_t *x, int32_t d, int32_t qmax, uint16_t *amax_out, int8_t *q)
+void orc_quantize_vector_dt(const uint16_t *x, int32_t d, int32_t qmax, uint16_t *amax_out, int8_t *q, int32_t dtype)
 {
     const uint16_t ab = orc_amax_bits(x, d);
-    const float amax = orc_half_to_float(ab);
+    const float amax = elem_to_float(ab, dtype);
     volatile float inv = 0.0f;                           /* volatile: force a rounded binary32 at each step */
     if (amax != 0.0f) inv = (float)qmax / amax;
+    if (!isfinite(inv)) inv = 0.0f;                      /* P20: only a bfloat16 amax < ~4e-37 gets here: all codes 0 */
     for (int32_t c = 0; c < d; ++c) {
-        const double t = (double)orc_half_to_float(x[c]) * (double)inv;   /* exact: 35 bits fit in 53 */
+        const double t = (double)elem_to_float(x[c], dtype) * (double)inv;   /* exact: <= 35 bits fit in 53 */
         double r = rint(t);                              /* FE_TONEAREST: ties to even */
         if (r > (double)qmax) r = (double)qmax;
         if (r < -(double)qmax) r = -(double)qmax;
@@ -352,16 +383,26 @@ void orc_quantize_vector(const uint16_t *x, int32_t d, int32_t qmax, uint16_t *a
     *amax_out = ab;
 }
 
-/* y = f16_rn(fl32(float(q) * scale)), scale = fl32(amax / qmax).  ("table lookup", PAPER.md:202) */
-void orc_dequantize_vector(const int8_t *q, int32_t d, int32_t qmax, uint16_t amax_bits, uint16_t *y)
+void orc_quantize_vector(const uint16_t *x, int32_t d, int32_t qmax, uint16_t *amax_out, int8_t *q)
 {
-    const float amax = orc_half_to_float(amax_bits);
+    orc_quantize_vector_dt(x, d, qmax, amax_out, q, 0);
+}
+
+/* y = f16_rn(fl32(float(q) * scale)), scale = fl32(amax / qmax).  ("table lookup", PAPER.md:202) */
+void orc_dequantize_vector_dt(const int8_t *q, int32_t d, int32_t qmax, uint16_t amax_bits, uint16_t *y, int32_t dtype)
+{
+    const float amax = elem_to_float(amax_bits, dtype);
     volatile float scale = 0.0f;
     if (amax != 0.0f) scale = amax / (float)qmax;
     for (int32_t c = 0; c < d; ++c) {
         volatile float v = (float)q[c] * scale;
-        y[c] = orc_float_to_half(v);
+        y[c] = float_to_elem(v, dtype);
     }
+}
+
+void orc_dequantize_vector(const int8_t *q, int32_t d, int32_t qmax, uint16_t amax_bits, uint16_t *y)
+{
+    orc_dequantize_vector_dt(q, d, qmax, amax_bits, y, 0);
 }
 
 /*
@@ -372,36 +413,47 @@ void orc_dequantize_vector(const int8_t *q, int32_t d, int32_t qmax, uint16_t am
  * (both 0 when r = 0).  q = clamp(rint(fl32(x - lo) * inv), 0, 3), the product exact and rounded once, half to even
  * (as P8).  y = f16_rn(fma(q, step, lo)), the fused multiply-add rounded once to binary32.
  */
-void orc_quantize2_vector(const uint16_t *x, int32_t d, uint16_t *lo_out, uint16_t *hi_out, uint8_t *q)
+void orc_quantize2_vector_dt(const uint16_t *x, int32_t d, uint16_t *lo_out, uint16_t *hi_out, uint8_t *q, int32_t dtype)
 {
-    float lo = orc_half_to_float(x[0]), hi = lo;
-    for (int32_t c = 1; c < d; ++c) { const float v = orc_half_to_float(x[c]); if (v < lo) lo = v; if (v > hi) hi = v; }
+    float lo = elem_to_float(x[0], dtype), hi = lo;
+    for (int32_t c = 1; c < d; ++c) { const float v = elem_to_float(x[c], dtype); if (v < lo) lo = v; if (v > hi) hi = v; }
     if (lo == 0.0f) lo = 0.0f * 0.0f;                    /* -0 -> +0 (0*0 = +0) */
     if (hi == 0.0f) hi = 0.0f * 0.0f;
     volatile float r = hi - lo;
     volatile float inv = 0.0f;
     if (r != 0.0f) inv = 3.0f / r;
+    if (!isfinite(inv)) inv = 0.0f;                      /* P20: bfloat16 ranges below ~1e-38 only */
     for (int32_t c = 0; c < d; ++c) {
-        volatile float dx = orc_half_to_float(x[c]) - lo;                    /* one binary32 rounding */
+        volatile float dx = elem_to_float(x[c], dtype) - lo;                 /* one binary32 rounding */
         double t = rint((double)dx * (double)inv);                           /* exact product, rounded once */
         if (t > 3.0) t = 3.0;
         if (t < 0.0) t = 0.0;
         q[c] = (uint8_t)t;
     }
-    *lo_out = orc_float_to_half(lo);                     /* exact: lo, hi are fp16 values */
-    *hi_out = orc_float_to_half(hi);
+    *lo_out = float_to_elem(lo, dtype);                  /* exact: lo, hi are element values */
+    *hi_out = float_to_elem(hi, dtype);
 }
 
-void orc_dequantize2_vector(const uint8_t *q, int32_t d, uint16_t lo_bits, uint16_t hi_bits, uint16_t *y)
+void orc_quantize2_vector(const uint16_t *x, int32_t d, uint16_t *lo_out, uint16_t *hi_out, uint8_t *q)
 {
-    const float lo = orc_half_to_float(lo_bits), hi = orc_half_to_float(hi_bits);
+    orc_quantize2_vector_dt(x, d, lo_out, hi_out, q, 0);
+}
+
+void orc_dequantize2_vector_dt(const uint8_t *q, int32_t d, uint16_t lo_bits, uint16_t hi_bits, uint16_t *y, int32_t dtype)
+{
+    const float lo = elem_to_float(lo_bits, dtype), hi = elem_to_float(hi_bits, dtype);
     volatile float r = hi - lo;
     volatile float step = 0.0f;
     if (r != 0.0f) step = r / 3.0f;
     for (int32_t c = 0; c < d; ++c) {
         volatile float v = fmaf((float)q[c], step, lo);                      /* correctly rounded fused multiply-add */
-        y[c] = orc_float_to_half(v);
+        y[c] = float_to_elem(v, dtype);
     }
+}
+
+void orc_dequantize2_vector(const uint8_t *q, int32_t d, uint16_t lo_bits, uint16_t hi_bits, uint16_t *y)
+{
+    orc_dequantize2_vector_dt(q, d, lo_bits, hi_bits, y, 0);
 }
 
 /* ------------------------------------------------------------------------ */
@@ -409,8 +461,8 @@ void orc_dequantize2_vector(const uint8_t *q, int32_t d, uint16_t lo_bits, uint1
 /* ------------------------------------------------------------------------ */
 /* counts6 = {n16,n8,n4,n0,Q,spent}; blob must hold orc_blob_bytes(); written completely
  * (every pad byte zero).  Returns 0, or -1 if a layer's tier map disagrees with counts. */
-int orc_pack(int32_t L, int32_t Hkv, int32_t d, int64_t n, const uint16_t *K, const uint16_t *V,
-             const uint8_t *tier, const int64_t counts6[6], int32_t allow_int4, uint8_t *blob)
+int orc_pack_dt(int32_t L, int32_t Hkv, int32_t d, int64_t n, const uint16_t *K, const uint16_t *V,
+                const uint8_t *tier, const int64_t counts6[6], int32_t allow_int4, uint8_t *blob, int32_t dtype)
 {
     const int low2 = (allow_int4 == 2);                  /* NEXT-4: the low tier is asymmetric 2-bit, tier code 2 */
     orc_layout_t lo; orc_layout_low(L, Hkv, d, n, counts6, low2 ? 2 : 4, &lo);
@@ -420,7 +472,8 @@ int orc_pack(int32_t L, int32_t Hkv, int32_t d, int64_t n, const uint16_t *K, co
     put_u32(blob + 16, (uint32_t)d); put_u32(blob + 20, (uint32_t)n);
     put_u32(blob + 24, (uint32_t)counts6[0]); put_u32(blob + 28, (uint32_t)counts6[1]);
     put_u32(blob + 32, (uint32_t)counts6[2]); put_u32(blob + 36, (uint32_t)counts6[3]);
-    put_u32(blob + 40, (allow_int4 ? 1u : 0u) | (low2 ? 2u : 0u)); put_u32(blob + 44, 0u);   /* flags: bit0 low tier allowed, bit1 it is 2-bit */
+    /* flags: bit0 low tier allowed, bit1 it is 2-bit, bit2 the elements (and the scale records) are bfloat16 */
+    put_u32(blob + 40, (allow_int4 ? 1u : 0u) | (low2 ? 2u : 0u) | (dtype ? 4u : 0u)); put_u32(blob + 44, 0u);
     put_u64(blob + 48, (uint64_t)counts6[4]);
     put_u64(blob + 56, lo.tier_map_off); put_u64(blob + 64, lo.layer0_off); put_u64(blob + 72, lo.layer_stride);
     for (int s = 0; s < 10; ++s) put_u64(blob + 80 + 8 * s, lo.seg_off[s]);
@@ -446,7 +499,7 @@ int orc_pack(int32_t L, int32_t Hkv, int32_t d, int64_t n, const uint16_t *K, co
                     uint8_t *sc  = base + lo.seg_off[6 + kv] + (size_t)slot8 * Hkv * 2;
                     for (int32_t h = 0; h < Hkv; ++h) {
                         uint16_t ab;
-                        orc_quantize_vector(src + (size_t)h * d, d, 127, &ab, q);
+                        orc_quantize_vector_dt(src + (size_t)h * d, d, 127, &ab, q, dtype);
                         for (int32_t c = 0; c < d; ++c) dst[(size_t)h * d + c] = (uint8_t)q[c];
                         sc[2 * h] = (uint8_t)ab; sc[2 * h + 1] = (uint8_t)(ab >> 8);
                     }
@@ -455,7 +508,7 @@ int orc_pack(int32_t L, int32_t Hkv, int32_t d, int64_t n, const uint16_t *K, co
                     uint8_t *sc  = base + lo.seg_off[8 + kv] + (size_t)slot4 * Hkv * 2;
                     for (int32_t h = 0; h < Hkv; ++h) {
                         uint16_t ab;
-                        orc_quantize_vector(src + (size_t)h * d, d, 7, &ab, q);
+                        orc_quantize_vector_dt(src + (size_t)h * d, d, 7, &ab, q, dtype);
                         for (int32_t c = 0; c < d; c += 2)   /* element 2i low nibble, 2i+1 high nibble */
                             dst[((size_t)h * d + c) / 2] = (uint8_t)((q[c] & 0xF) | ((q[c + 1] & 0xF) << 4));
                         sc[2 * h] = (uint8_t)ab; sc[2 * h + 1] = (uint8_t)(ab >> 8);
@@ -465,7 +518,7 @@ int orc_pack(int32_t L, int32_t Hkv, int32_t d, int64_t n, const uint16_t *K, co
                     uint8_t *sc  = base + lo.seg_off[8 + kv] + (size_t)slot4 * Hkv * 4;
                     for (int32_t h = 0; h < Hkv; ++h) {
                         uint16_t lb, hb;
-                        orc_quantize2_vector(src + (size_t)h * d, d, &lb, &hb, (uint8_t *)q);
+                        orc_quantize2_vector_dt(src + (size_t)h * d, d, &lb, &hb, (uint8_t *)q, dtype);
                         for (int32_t c = 0; c < d; c += 4)   /* element 4i+k in bits 2k..2k+1 of byte i */
                             dst[((size_t)h * d + c) / 4] = (uint8_t)((q[c] & 3) | ((q[c + 1] & 3) << 2) | ((q[c + 2] & 3) << 4) | ((q[c + 3] & 3) << 6));
                         sc[4 * h] = (uint8_t)lb; sc[4 * h + 1] = (uint8_t)(lb >> 8);
@@ -484,6 +537,12 @@ int orc_pack(int32_t L, int32_t Hkv, int32_t d, int64_t n, const uint16_t *K, co
     return bad ? -1 : 0;
 }
 
+int orc_pack(int32_t L, int32_t Hkv, int32_t d, int64_t n, const uint16_t *K, const uint16_t *V,
+             const uint8_t *tier, const int64_t counts6[6], int32_t allow_int4, uint8_t *blob)
+{
+    return orc_pack_dt(L, Hkv, d, n, K, V, tier, counts6, allow_int4, blob, 0);
+}
+
 /* ------------------------------------------------------------------------ */
 /* O6. Unpack (decode side; dropped -> +0.0 fill, reading P10) */
 /* ------------------------------------------------------------------------ */
@@ -498,8 +557,9 @@ static int orc_unpack_impl(const uint8_t *blob, uint64_t blob_bytes, int32_t L, 
     int64_t counts[4] = { get_u32(blob + 24), get_u32(blob + 28), get_u32(blob + 32), get_u32(blob + 36) };
     if (counts[0] + counts[1] + counts[2] + counts[3] != n) return -5;
     const uint32_t flags = get_u32(blob + 40);
-    if (flags & ~3u) return -5;
+    if (flags & ~7u) return -5;
     const int low2 = (flags & 2u) != 0;                  /* NEXT-4: the low tier is asymmetric 2-bit */
+    const int32_t dtype = (flags & 4u) ? 1 : 0;          /* NEXT-4: bfloat16 elements and records */
     orc_layout_t lo; orc_layout_low(L, Hkv, d, n, counts, low2 ? 2 : 4, &lo);
     if (get_u64(blob + 56) != lo.tier_map_off || get_u64(blob + 64) != lo.layer0_off ||
         get_u64(blob + 72) != lo.layer_stride || get_u64(blob + 160) != lo.total_bytes ||
@@ -528,7 +588,7 @@ static int orc_unpack_impl(const uint8_t *blob, uint64_t blob_bytes, int32_t L, 
                     const uint8_t *sc  = base + lo.seg_off[6 + kv] + (size_t)slot8 * Hkv * 2;
                     for (int32_t h = 0; h < Hkv; ++h) {
                         for (int32_t c = 0; c < d; ++c) q[c] = (int8_t)src[(size_t)h * d + c];
-                        orc_dequantize_vector(q, d, 127, (uint16_t)(sc[2 * h] | (sc[2 * h + 1] << 8)), dst + (size_t)h * d);
+                        orc_dequantize_vector_dt(q, d, 127, (uint16_t)(sc[2 * h] | (sc[2 * h + 1] << 8)), dst + (size_t)h * d, dtype);
                     }
                 } else if (t == 2 && low2) {
                     const uint8_t *src = base + lo.seg_off[4 + kv] + (size_t)slot4 * row / 4;
@@ -536,8 +596,8 @@ static int orc_unpack_impl(const uint8_t *blob, uint64_t blob_bytes, int32_t L, 
                     for (int32_t h = 0; h < Hkv; ++h) {
                         for (int32_t c = 0; c < d; ++c)
                             q[c] = (int8_t)((src[((size_t)h * d + c) / 4] >> (2 * (c & 3))) & 3);
-                        orc_dequantize2_vector((const uint8_t *)q, d, (uint16_t)(sc[4 * h] | (sc[4 * h + 1] << 8)),
-                                               (uint16_t)(sc[4 * h + 2] | (sc[4 * h + 3] << 8)), dst + (size_t)h * d);
+                        orc_dequantize2_vector_dt((const uint8_t *)q, d, (uint16_t)(sc[4 * h] | (sc[4 * h + 1] << 8)),
+                                                  (uint16_t)(sc[4 * h + 2] | (sc[4 * h + 3] << 8)), dst + (size_t)h * d, dtype);
                     }
                 } else if (t == 4 && !low2) {
                     const uint8_t *src = base + lo.seg_off[4 + kv] + (size_t)slot4 * row / 2;
@@ -548,7 +608,7 @@ static int orc_unpack_impl(const uint8_t *blob, uint64_t blob_bytes, int32_t L, 
                             int nib = (c & 1) ? (byte >> 4) : (byte & 0xF);
                             q[c] = (int8_t)(nib >= 8 ? nib - 16 : nib);      /* 4-bit two's complement */
                         }
-                        orc_dequantize_vector(q, d, 7, (uint16_t)(sc[2 * h] | (sc[2 * h + 1] << 8)), dst + (size_t)h * d);
+                        orc_dequantize_vector_dt(q, d, 7, (uint16_t)(sc[2 * h] | (sc[2 * h + 1] << 8)), dst + (size_t)h * d, dtype);
                     }
                 } else if (!patch) {
                     for (size_t e = 0; e < row; ++e) dst[e] = 0;             /* P10: dropped => +0.0 */
@@ -582,8 +642,8 @@ int orc_unpack_patch(const uint8_t *blob, uint64_t blob_bytes, int32_t L, int32_
 /* fallback").  Reading P15: A_j = mean over KV heads of the L2 norm of the  */
 /* key vector, normalised to sum 1 over j; then the same decay.  UNPINNED.   */
 /* ------------------------------------------------------------------------ */
-void orc_importance_kvnorm(int32_t L, int32_t Hkv, int32_t d, int64_t n, double lambda,
-                           const uint16_t *K, float *I)
+void orc_importance_kvnorm_dt(int32_t L, int32_t Hkv, int32_t d, int64_t n, double lambda,
+                              const uint16_t *K, float *I, int32_t dtype)
 {
 #pragma omp parallel for schedule(dynamic, 1)
     for (int32_t l = 0; l < L; ++l) {
@@ -594,7 +654,7 @@ void orc_importance_kvnorm(int32_t L, int32_t Hkv, int32_t d, int64_t n, double 
             for (int32_t g = 0; g < Hkv; ++g) {
                 const uint16_t *k = K + (((size_t)l * n + j) * Hkv + g) * d;
                 double ss = 0.0;
-                for (int32_t c = 0; c < d; ++c) { double v = (double)orc_half_to_float(k[c]); ss += v * v; }
+                for (int32_t c = 0; c < d; ++c) { double v = (double)elem_to_float(k[c], dtype); ss += v * v; }
                 acc += sqrt(ss);
             }
             A[j] = acc / (double)Hkv;
@@ -606,6 +666,12 @@ void orc_importance_kvnorm(int32_t L, int32_t Hkv, int32_t d, int64_t n, double 
         }
         free(A);
     }
+}
+
+void orc_importance_kvnorm(int32_t L, int32_t Hkv, int32_t d, int64_t n, double lambda,
+                           const uint16_t *K, float *I)
+{
+    orc_importance_kvnorm_dt(L, Hkv, d, n, lambda, K, I, 0);
 }
 
 int orc_max_threads(void)

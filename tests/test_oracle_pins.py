@@ -718,3 +718,84 @@ def test_two_bit_blob_layout_round_trip_and_hand_written_bytes():
     assert np.array_equal(t2, tier) and np.array_equal(K2[0, 0], K[0, 0]) and (K2[0, 2] == 0).all()
     assert K2[0, 1, 0, :len(rows)].view(np.uint16).tolist() == [int(r[3], 16) for r in rows]
     assert V2[0, 1, 0, :3].tolist() == [0.75, 0.5, 0.0]
+
+
+# ----------------------------------------------------------------------------------------------
+# NEXT-4: bfloat16 caches (reading P20)
+# ----------------------------------------------------------------------------------------------
+def _bf16_bits(t):
+    import torch
+    return t.to(torch.bfloat16).view(torch.int16).numpy().view(np.uint16)
+
+
+def test_bf16_conversions_against_torch():
+    import torch
+    allbits = np.arange(65536, dtype=np.uint16)
+    f = oracle.bf16_to_float(allbits)
+    want = torch.from_numpy(allbits.view(np.int16)).view(torch.bfloat16).float().numpy()
+    fin = np.isfinite(want)
+    assert np.array_equal(f[fin].view(np.uint32), want[fin].view(np.uint32))            # exhaustive, exact
+    rng = np.random.default_rng(7)
+    x = np.concatenate([rng.standard_normal(4000) * 10.0 ** rng.uniform(-30, 30, 4000),
+                        oracle.bf16_to_float(rng.integers(0, 0x7F00, 2000).astype(np.uint16)) * (1 + 2.0 ** -9),   # near ties
+                        [0.0, -0.0, 1.0, 3.3895313892515355e38]]).astype(np.float32)
+    got = oracle.float_to_bf16(x)
+    assert np.array_equal(got, _bf16_bits(torch.from_numpy(x)))                           # RNE, as torch rounds
+
+
+def test_bf16_quantizer_identities_and_error_bound():
+    from fractions import Fraction
+    import torch
+    rng = np.random.default_rng(13)
+    for qmax in (127, 7):
+        for _ in range(25):
+            xb = _bf16_bits(torch.from_numpy((rng.standard_normal(128) * rng.uniform(1e-3, 100)).astype(np.float32)))
+            x = oracle.bf16_to_float(xb).astype(np.float64)
+            ab, q = oracle.quantize_vector(xb, qmax, bf16=True)
+            amax = float(oracle.bf16_to_float(np.uint16(ab)))
+            assert amax == np.abs(x).max() and np.abs(q).max() == qmax
+            inv = np.float32(qmax) / np.float32(amax)
+            for e, code in zip(x[:32], q[:32]):                                           # exact rational rounding
+                assert int(code) == _exact_code(np.float32(e), inv, qmax)
+            scale = amax / qmax
+            assert np.abs(q * scale - x).max() <= scale / 2 * (1 + 1e-4)
+            y = oracle.bf16_to_float(oracle.dequantize_vector(q, qmax, ab, bf16=True)).astype(np.float64)
+            assert (np.abs(y - x) <= scale / 2 * (1 + 1e-4) + np.abs(y) * 2.0 ** -8 + 1e-30).all()
+    # P20: an amax so small that qmax/amax overflows binary32 -> all codes 0, record kept
+    tiny = np.full(64, 0x0001, np.uint16)                                                 # smallest bf16 subnormal, 9.2e-41
+    ab, q = oracle.quantize_vector(tiny, 127, bf16=True)
+    assert ab == 1 and (q == 0).all()
+    # 2-bit on bf16: extremes hit 0 and 3, constant vector exact
+    xb = _bf16_bits(torch.from_numpy(rng.standard_normal(64).astype(np.float32)))
+    lo, hi, q2 = oracle.quantize2_vector(xb, bf16=True)
+    x = oracle.bf16_to_float(xb)
+    assert float(oracle.bf16_to_float(np.uint16(lo))) == x.min() and float(oracle.bf16_to_float(np.uint16(hi))) == x.max()
+    assert q2.min() == 0 and q2.max() == 3
+    y = oracle.bf16_to_float(oracle.dequantize2_vector(q2, lo, hi, bf16=True)).astype(np.float64)
+    step = (float(x.max()) - float(x.min())) / 3
+    assert (np.abs(y - x.astype(np.float64)) <= step / 2 * (1 + 1e-3) + np.abs(y) * 2.0 ** -8).all()
+
+
+def test_bf16_blob_round_trip_and_fp16_tier_is_a_copy():
+    import torch
+    L, n, Hkv, d = 2, 40, 2, 64
+    rng = np.random.default_rng(14)
+    K = _bf16_bits(torch.from_numpy(rng.standard_normal((L, n, Hkv, d)).astype(np.float32)))
+    V = _bf16_bits(torch.from_numpy(rng.standard_normal((L, n, Hkv, d)).astype(np.float32)))
+    c, prot = oracle.tier_counts(n, 0.4, 2, [], True)
+    tier = oracle.assign(rng.random((L, n)).astype(np.float32), prot, c)
+    blob = oracle.pack(K, V, tier, c, True, bf16=True)
+    assert blob[40] == 5                                                                  # flags: low tier allowed | bf16
+    assert blob.size == oracle.blob_bytes(L, Hkv, d, n, c)                                 # same byte model as FP16 (2 B)
+    K2, V2, t2 = oracle.unpack(blob, L, Hkv, d, n, bf16=True)
+    assert np.array_equal(t2, tier) and np.array_equal(K2[tier == 16], K[tier == 16])
+    for l, j in ((0, 5), (1, 17), (1, 39)):
+        for h in range(Hkv):
+            t = int(tier[l, j])
+            if t in (8, 4):
+                ab, q = oracle.quantize_vector(K[l, j, h], 127 if t == 8 else 7, bf16=True)
+                assert np.array_equal(K2[l, j, h], oracle.dequantize_vector(q, 127 if t == 8 else 7, ab, bf16=True))
+    c1, _ = oracle.tier_counts(n, 1.0, 0, [], True)
+    b1 = oracle.pack(K, V, np.full((L, n), 16, np.uint8), c1, True, bf16=True)
+    K3, V3, _ = oracle.unpack(b1, L, Hkv, d, n, bf16=True)
+    assert np.array_equal(K3, K) and np.array_equal(V3, V)                                 # b = 1 identity
