@@ -300,6 +300,28 @@ def run_next_rows(prob, steps):
     out["two_bit_low_tier"] = {"budget": 0.2, "counts": list(c2.as_tuple()), "blob_bytes_per_request": bb2,
                                "ms_pack_plus_unpack": ms, "GBps": moved2 / (ms * 1e-3) / 1e9,
                                "GBps_of_fp16_kv": cfg.bytes_fp16 * R / (ms * 1e-3) / 1e9}
+    del blob2
+    # NEXT-4: bfloat16 caches (same values rounded to bf16), the headline policy (b of the run), pack + unpack
+    for r in range(R):
+        prob.Ko[r].copy_(prob.K[r].float().to(torch.bfloat16).view(torch.float16))     # Ko/Vo reused as bf16 inputs
+        prob.Vo[r].copy_(prob.V[r].float().to(torch.bfloat16).view(torch.float16))
+    shape_b = skv.make_shape(cfg.L, cfg.Hq, cfg.Hkv, cfg.d, cfg.n, R, dtype="bf16")
+    cb = skv.skv_assign_tiers(shape_b, prob.policy, prob.I, prob.tier, prob.ws)
+    bbb = skv.skv_blob_bytes(shape_b, cb)
+    blob3 = torch.empty((R, bbb), dtype=torch.uint8, device=prob.dev)
+    Kb, Vb = prob.Ko.clone(), prob.Vo.clone()
+    def once3():
+        skv.skv_pack(shape_b, Kb, Vb, prob.tier, cb, blob3, prob.ws)
+        skv.skv_unpack(shape_b, blob3, bbb, cb, prob.Ko, prob.Vo, prob.tier_out, prob.ws)
+    once3()
+    a.record()
+    for _ in range(steps):
+        once3()
+    b_.record(); torch.cuda.synchronize()
+    ms = a.elapsed_time(b_) / steps
+    moved3 = 2 * (cfg.bytes_fp16 * R + R * bbb + cfg.L * cfg.n * R)
+    out["bf16_caches"] = {"budget": prob.b, "ms_pack_plus_unpack": ms, "GBps": moved3 / (ms * 1e-3) / 1e9,
+                          "GBps_of_16bit_kv": cfg.bytes_fp16 * R / (ms * 1e-3) / 1e9}
     return out
 
 

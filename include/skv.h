@@ -27,6 +27,10 @@
  *   - Every entry returns SKV_OK (0) or a negative skv_status and launches nothing on error.
  *   - The library keeps no global state and is re-entrant.
  *   - fp16 = IEEE binary16.  K/V inputs must be finite (NaN/Inf is undefined behaviour).
+ *   - With skv_shape.dtype = SKV_BF16 every "fp16" below reads bfloat16 (caches, queries, amax / (lo, hi) records,
+ *     dequantised output); the byte model is unchanged (2 bytes per element).  Only difference in the arithmetic: a
+ *     quotient qmax/amax (or 3/r) that overflows binary32 -- possible only for a bfloat16 amax below ~4e-37 -- is
+ *     replaced by 0, i.e. such a vector gets all-zero codes (reading P20 of DESIGN.md).
  *
  * Tier codes (bits per element): 16 = FP16, 8 = INT8, 4 = INT4, 0 = dropped (c = 0).
  *
@@ -34,7 +38,7 @@
  * back at stride skv_blob_bytes(); the paper only says "mixed-precision payload"):
  *
  *   [0,256)  header: 0 u32 magic 0x31564B53 ("SKV1"), 4 u32 version = 1, 8 u32 L, 12 u32 Hkv, 16 u32 d_h,
- *            20 u32 n, 24 u32 n16, 28 u32 n8, 32 u32 n4, 36 u32 n0, 40 u32 flags (bit0 = allow_int4, bit1 = 2-bit low tier),
+ *            20 u32 n, 24 u32 n16, 28 u32 n8, 32 u32 n4, 36 u32 n0, 40 u32 flags (bit0 = allow_int4, bit1 = 2-bit low tier, bit2 = bfloat16),
  *            44 u32 0, 48 u64 budget in quarter-units, 56 u64 tier_map_off (= 256), 64 u64 layer0_off,
  *            72 u64 layer_stride, 80 u64 seg_off[10] (relative to the layer block), 160 u64 total_bytes,
  *            168..255 zero
@@ -89,7 +93,12 @@ typedef enum {
 typedef struct {
     int32_t n_layers, n_q_heads, n_kv_heads, head_dim, n_tokens, n_requests;
     int64_t stride_request, stride_layer, stride_token, stride_head;
+    int32_t dtype;            /* element type of K, V, Q and of the scale records: 0 = fp16 (SKV_F16, the paper's
+                                 cache), 1 = bfloat16 (SKV_BF16, NEXT-4); header flags bit2 */
+    int32_t reserved;         /* must be 0 */
 } skv_shape;
+#define SKV_F16 0
+#define SKV_BF16 1
 
 /* Transfer policy (PAPER.md:51-58 b; :216, :230 sinks; :25 protected positions; :234 allow_int4). */
 typedef struct {

@@ -35,7 +35,8 @@ class skv_shape(C.Structure):
     _fields_ = [("n_layers", C.c_int32), ("n_q_heads", C.c_int32), ("n_kv_heads", C.c_int32),
                 ("head_dim", C.c_int32), ("n_tokens", C.c_int32), ("n_requests", C.c_int32),
                 ("stride_request", C.c_int64), ("stride_layer", C.c_int64),
-                ("stride_token", C.c_int64), ("stride_head", C.c_int64)]
+                ("stride_token", C.c_int64), ("stride_head", C.c_int64),
+                ("dtype", C.c_int32), ("reserved", C.c_int32)]
 
 
 class skv_policy(C.Structure):
@@ -96,11 +97,15 @@ def lib():
 # ------------------------------------------------------------------------------------------------
 # marshalling helpers
 # ------------------------------------------------------------------------------------------------
+SKV_F16, SKV_BF16 = 0, 1
+
+
 def make_shape(n_layers, n_q_heads, n_kv_heads, head_dim, n_tokens, n_requests=1, layout="token_major",
-               strides=None):
+               strides=None, dtype="f16"):
     """skv_shape for a contiguous cache.  layout: "token_major" [R][L][n][Hkv][d] or "hf" [R][L][Hkv][n][d];
     or pass strides=(request, layer, token, head) in elements."""
     s = skv_shape(n_layers, n_q_heads, n_kv_heads, head_dim, n_tokens, n_requests)
+    s.dtype = SKV_BF16 if dtype in ("bf16", SKV_BF16) and dtype is not False else SKV_F16
     if strides is not None:
         s.stride_request, s.stride_layer, s.stride_token, s.stride_head = [int(x) for x in strides]
     elif layout == "token_major":

@@ -1,6 +1,8 @@
 // skv_codec.cuh -- device helpers shared by the pack and unpack kernels: streaming loads/stores, the
 // per-vector absmax machinery and the exact fp32 quantise / dequantise steps of include/skv.h.
 #pragma once
+#include <cuda_bf16.h>
+
 #include "skv_common.cuh"
 
 namespace skv {
@@ -37,14 +39,40 @@ __device__ __forceinline__ void st_stream(void *p, uint32_t v)
     asm volatile("st.global.L1::no_allocate.u32 [%0], %1;" :: "l"(p), "r"(v) : "memory");
 }
 
+// ------------------------------------------------------------------------------------------------
+// Element types of a cache: binary16 (the paper's FP16) or bfloat16 (reading P20).  The kernels are
+// templates on one of these traits; everything that differs between the two formats is an overload below.
+// ------------------------------------------------------------------------------------------------
+struct ElemF16  { using H = __half;        using H2 = __half2;        static constexpr bool kBf16 = false; };
+struct ElemBF16 { using H = __nv_bfloat16; using H2 = __nv_bfloat162; static constexpr bool kBf16 = true; };
+
 __device__ __forceinline__ uint32_t h2u(__half2 h) { return *reinterpret_cast<uint32_t *>(&h); }
-__device__ __forceinline__ __half2 u2h(uint32_t u) { return *reinterpret_cast<__half2 *>(&u); }
+__device__ __forceinline__ uint32_t h2u(__nv_bfloat162 h) { return *reinterpret_cast<uint32_t *>(&h); }
+template <class H2> __device__ __forceinline__ H2 as_pair(uint32_t u) { return *reinterpret_cast<H2 *>(&u); }
+__device__ __forceinline__ __half2 u2h(uint32_t u) { return as_pair<__half2>(u); }
+__device__ __forceinline__ __half lo_h(__half2 v) { return __low2half(v); }
+__device__ __forceinline__ __half hi_h(__half2 v) { return __high2half(v); }
+__device__ __forceinline__ __nv_bfloat16 lo_h(__nv_bfloat162 v) { return __low2bfloat16(v); }
+__device__ __forceinline__ __nv_bfloat16 hi_h(__nv_bfloat162 v) { return __high2bfloat16(v); }
+__device__ __forceinline__ __half2 pair_h(__half a, __half b) { return __halves2half2(a, b); }
+__device__ __forceinline__ __nv_bfloat162 pair_h(__nv_bfloat16 a, __nv_bfloat16 b) { return __halves2bfloat162(a, b); }
+__device__ __forceinline__ float to_f(__half a) { return __half2float(a); }
+__device__ __forceinline__ float to_f(__nv_bfloat16 a) { return __bfloat162float(a); }
+__device__ __forceinline__ float2 to_f2(__half2 a) { return __half22float2(a); }
+__device__ __forceinline__ float2 to_f2(__nv_bfloat162 a) { return __bfloat1622float2(a); }
+template <class E> __device__ __forceinline__ uint32_t from_f2(float a, float b);
+template <> __device__ __forceinline__ uint32_t from_f2<ElemF16>(float a, float b) { return h2u(__floats2half2_rn(a, b)); }
+template <> __device__ __forceinline__ uint32_t from_f2<ElemBF16>(float a, float b) { return h2u(__floats2bfloat162_rn(a, b)); }
+template <class H> __device__ __forceinline__ H zero_h() { unsigned short z = 0; return *reinterpret_cast<H *>(&z); }
 
 // |x| max of the 8 halves in a uint4 as one half
-__device__ __forceinline__ __half absmax8_scalar(const uint4 &v)
+template <class E>
+__device__ __forceinline__ typename E::H absmax8_scalar(const uint4 &v)
 {
-    const __half2 m = __hmax2(__hmax2(__habs2(u2h(v.x)), __habs2(u2h(v.y))), __hmax2(__habs2(u2h(v.z)), __habs2(u2h(v.w))));
-    return __hmax(__low2half(m), __high2half(m));
+    using H2 = typename E::H2;
+    const H2 m = __hmax2(__hmax2(__habs2(as_pair<H2>(v.x)), __habs2(as_pair<H2>(v.y))),
+                         __hmax2(__habs2(as_pair<H2>(v.z)), __habs2(as_pair<H2>(v.w))));
+    return __hmax(lo_h(m), hi_h(m));
 }
 
 // round-half-even of the EXACT product x*inv (include/skv.h) in one fused multiply-add with the 1.5*2^23 magic
@@ -64,19 +92,23 @@ __device__ __forceinline__ uint32_t pack4_bytes(uint32_t a, uint32_t b, uint32_t
 }
 
 // 8 fp16 -> 8 INT8 codes (two words)
+template <class E>
 __device__ __forceinline__ uint2 quant8_int8(const uint4 &v, float inv)
 {
-    const float2 a = __half22float2(u2h(v.x)), b = __half22float2(u2h(v.y));
-    const float2 c = __half22float2(u2h(v.z)), d = __half22float2(u2h(v.w));
+    using H2 = typename E::H2;
+    const float2 a = to_f2(as_pair<H2>(v.x)), b = to_f2(as_pair<H2>(v.y));
+    const float2 c = to_f2(as_pair<H2>(v.z)), d = to_f2(as_pair<H2>(v.w));
     return make_uint2(pack4_bytes(rne_code_bits(a.x, inv), rne_code_bits(a.y, inv), rne_code_bits(b.x, inv), rne_code_bits(b.y, inv)),
                       pack4_bytes(rne_code_bits(c.x, inv), rne_code_bits(c.y, inv), rne_code_bits(d.x, inv), rne_code_bits(d.y, inv)));
 }
 
 // 8 fp16 -> 8 INT4 codes (one word; element 2k in the low nibble of byte k)
+template <class E>
 __device__ __forceinline__ uint32_t quant8_int4(const uint4 &v, float inv)
 {
-    const float2 a = __half22float2(u2h(v.x)), b = __half22float2(u2h(v.y));
-    const float2 c = __half22float2(u2h(v.z)), d = __half22float2(u2h(v.w));
+    using H2 = typename E::H2;
+    const float2 a = to_f2(as_pair<H2>(v.x)), b = to_f2(as_pair<H2>(v.y));
+    const float2 c = to_f2(as_pair<H2>(v.z)), d = to_f2(as_pair<H2>(v.w));
     const uint32_t b0 = (rne_code_bits(a.x, inv) & 0xFu) | (rne_code_bits(a.y, inv) << 4);
     const uint32_t b1 = (rne_code_bits(b.x, inv) & 0xFu) | (rne_code_bits(b.y, inv) << 4);
     const uint32_t b2 = (rne_code_bits(c.x, inv) & 0xFu) | (rne_code_bits(c.y, inv) << 4);
@@ -105,40 +137,38 @@ __device__ __forceinline__ int src_lane(uint32_t lane, int u)
     if (NCH == 2) return base + u * (LPV / 2);
     return base;
 }
-template <int LPV, int NCH>
-__device__ __forceinline__ __half2 group_absmax(__half2 (&m)[NCH], uint32_t lane)
+template <int LPV, int NCH, class H2>
+__device__ __forceinline__ H2 group_absmax(H2 (&m)[NCH], uint32_t lane)
 {
-    __half2 v;
+    H2 v;
     int o = LPV / 2;
     if (NCH == 4) {
         const bool hi = (lane / (LPV / 2)) & 1;
-        const __half2 keep0 = hi ? m[2] : m[0], keep1 = hi ? m[3] : m[1];
-        const __half2 send0 = hi ? m[0] : m[2], send1 = hi ? m[1] : m[3];
-        const __half2 k0 = __hmax2(keep0, u2h(__shfl_xor_sync(0xffffffffu, h2u(send0), LPV / 2)));
-        const __half2 k1 = __hmax2(keep1, u2h(__shfl_xor_sync(0xffffffffu, h2u(send1), LPV / 2)));
+        const H2 keep0 = hi ? m[2] : m[0], keep1 = hi ? m[3] : m[1];
+        const H2 send0 = hi ? m[0] : m[2], send1 = hi ? m[1] : m[3];
+        const H2 k0 = __hmax2(keep0, as_pair<H2>(__shfl_xor_sync(0xffffffffu, h2u(send0), LPV / 2)));
+        const H2 k1 = __hmax2(keep1, as_pair<H2>(__shfl_xor_sync(0xffffffffu, h2u(send1), LPV / 2)));
         const bool hi2 = (lane / (LPV / 4)) & 1;
-        const __half2 keep = hi2 ? k1 : k0, send = hi2 ? k0 : k1;
-        v = __hmax2(keep, u2h(__shfl_xor_sync(0xffffffffu, h2u(send), LPV / 4)));
+        const H2 keep = hi2 ? k1 : k0, send = hi2 ? k0 : k1;
+        v = __hmax2(keep, as_pair<H2>(__shfl_xor_sync(0xffffffffu, h2u(send), LPV / 4)));
         o = LPV / 8;
     } else if (NCH == 2) {
         const bool hi = (lane / (LPV / 2)) & 1;
-        const __half2 keep = hi ? m[1] : m[0], send = hi ? m[0] : m[1];
-        v = __hmax2(keep, u2h(__shfl_xor_sync(0xffffffffu, h2u(send), LPV / 2)));
+        const H2 keep = hi ? m[1] : m[0], send = hi ? m[0] : m[1];
+        v = __hmax2(keep, as_pair<H2>(__shfl_xor_sync(0xffffffffu, h2u(send), LPV / 2)));
         o = LPV / 4;
     } else {
         v = m[0];
     }
 #pragma unroll
-    for (; o >= 1; o >>= 1) v = __hmax2(v, u2h(__shfl_xor_sync(0xffffffffu, h2u(v), o)));
+    for (; o >= 1; o >>= 1) v = __hmax2(v, as_pair<H2>(__shfl_xor_sync(0xffffffffu, h2u(v), o)));
     return v;
 }
 
 // ------------------------------------------------------------------------------------------------
 // dequantise: biased bytes -> f16_rn(fl32(float(q) * scale)); int->float through the 2^23 exponent trick
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t h2_bits(float a, float b) { return h2u(__floats2half2_rn(a, b)); }
-
-template <int BIAS>
+template <int BIAS, class E>
 __device__ __forceinline__ void dequant4(uint32_t w, float scale, uint32_t &o0, uint32_t &o1)
 {
     constexpr float kOff = 8388608.0f + (float)BIAS;                  // 2^23 + BIAS, exact
@@ -146,16 +176,18 @@ __device__ __forceinline__ void dequant4(uint32_t w, float scale, uint32_t &o0, 
     const float f1 = __fsub_rn(__uint_as_float(__byte_perm(w, 0x4B000000u, 0x7541)), kOff);
     const float f2 = __fsub_rn(__uint_as_float(__byte_perm(w, 0x4B000000u, 0x7542)), kOff);
     const float f3 = __fsub_rn(__uint_as_float(__byte_perm(w, 0x4B000000u, 0x7543)), kOff);
-    o0 = h2_bits(__fmul_rn(f0, scale), __fmul_rn(f1, scale));
-    o1 = h2_bits(__fmul_rn(f2, scale), __fmul_rn(f3, scale));
+    o0 = from_f2<E>(__fmul_rn(f0, scale), __fmul_rn(f1, scale));
+    o1 = from_f2<E>(__fmul_rn(f2, scale), __fmul_rn(f3, scale));
 }
+template <class E>
 __device__ __forceinline__ uint4 dequant_int8(uint2 w, float scale)
 {
     uint4 o;
-    dequant4<128>(w.x ^ 0x80808080u, scale, o.x, o.y);
-    dequant4<128>(w.y ^ 0x80808080u, scale, o.z, o.w);
+    dequant4<128, E>(w.x ^ 0x80808080u, scale, o.x, o.y);
+    dequant4<128, E>(w.y ^ 0x80808080u, scale, o.z, o.w);
     return o;
 }
+template <class E>
 __device__ __forceinline__ uint4 dequant_int4(uint32_t w, float scale)
 {
     w ^= 0x88888888u;                                   // every nibble becomes q+8
@@ -169,10 +201,10 @@ __device__ __forceinline__ uint4 dequant_int4(uint32_t w, float scale)
         f[2 * k + 1] = __fsub_rn(__uint_as_float(__byte_perm(odd, 0x4B000000u, 0x7540 + k)), kOff);
     }
     uint4 o;
-    o.x = h2_bits(__fmul_rn(f[0], scale), __fmul_rn(f[1], scale));
-    o.y = h2_bits(__fmul_rn(f[2], scale), __fmul_rn(f[3], scale));
-    o.z = h2_bits(__fmul_rn(f[4], scale), __fmul_rn(f[5], scale));
-    o.w = h2_bits(__fmul_rn(f[6], scale), __fmul_rn(f[7], scale));
+    o.x = from_f2<E>(__fmul_rn(f[0], scale), __fmul_rn(f[1], scale));
+    o.y = from_f2<E>(__fmul_rn(f[2], scale), __fmul_rn(f[3], scale));
+    o.z = from_f2<E>(__fmul_rn(f[4], scale), __fmul_rn(f[5], scale));
+    o.w = from_f2<E>(__fmul_rn(f[6], scale), __fmul_rn(f[7], scale));
     return o;
 }
 // ------------------------------------------------------------------------------------------------
@@ -189,33 +221,43 @@ __device__ __forceinline__ void st_stream2(void *p, uint16_t v)
     asm volatile("st.global.L1::no_allocate.u16 [%0], %1;" :: "l"(p), "h"(v) : "memory");
 }
 // (max, -min) of the 8 halves in a uint4: both halves of the result reduce with hmax2
-__device__ __forceinline__ __half2 max_negmin8(const uint4 &v)
+template <class E>
+__device__ __forceinline__ typename E::H2 max_negmin8(const uint4 &v)
 {
-    const __half2 a = u2h(v.x), b = u2h(v.y), c = u2h(v.z), d = u2h(v.w);
-    const __half2 mx = __hmax2(__hmax2(a, b), __hmax2(c, d));
-    const __half2 mn = __hmin2(__hmin2(a, b), __hmin2(c, d));
-    return __halves2half2(__hmax(__low2half(mx), __high2half(mx)), __hneg(__hmin(__low2half(mn), __high2half(mn))));
+    using H2 = typename E::H2;
+    const H2 a = as_pair<H2>(v.x), b = as_pair<H2>(v.y), c = as_pair<H2>(v.z), d = as_pair<H2>(v.w);
+    const H2 mx = __hmax2(__hmax2(a, b), __hmax2(c, d));
+    const H2 mn = __hmin2(__hmin2(a, b), __hmin2(c, d));
+    return pair_h(__hmax(lo_h(mx), hi_h(mx)), __hneg(__hmin(lo_h(mn), hi_h(mn))));
 }
 // canonical records from a reduced (max, -min): a zero of either sign is stored as +0
-__device__ __forceinline__ void lohi_of(__half2 m, __half &lo, __half &hi)
+template <class H2, class H>
+__device__ __forceinline__ void lohi_of(H2 m, H &lo, H &hi)
 {
-    hi = __low2half(m);
-    lo = __hneg(__high2half(m));
-    const __half z = __ushort_as_half((unsigned short)0);
+    hi = lo_h(m);
+    lo = __hneg(hi_h(m));
+    const H z = zero_h<H>();
     if (__heq(hi, z)) hi = z;
     if (__heq(lo, z)) lo = z;
 }
-__device__ __forceinline__ float range_of(__half lo, __half hi) { return __fsub_rn(__half2float(hi), __half2float(lo)); }
-__device__ __forceinline__ float inv3_of(float r) { return r != 0.0f ? __fdiv_rn(3.0f, r) : 0.0f; }
+template <class H> __device__ __forceinline__ float range_of(H lo, H hi) { return __fsub_rn(to_f(hi), to_f(lo)); }
+// 3/r; a bfloat16 range below ~1e-38 overflows the quotient: such vectors are coded as all-zero codes (P20)
+__device__ __forceinline__ float inv3_of(float r)
+{
+    const float q = r != 0.0f ? __fdiv_rn(3.0f, r) : 0.0f;
+    return (q <= 3.402823466e38f) ? q : 0.0f;
+}
 __device__ __forceinline__ float step3_of(float r) { return r != 0.0f ? __fdiv_rn(r, 3.0f) : 0.0f; }
 // 8 fp16 -> 8 two-bit codes (16 bits; element k in bits 2k..2k+1).  q_k = rint(fl32(x_k - lo) * inv), the product exact
 // and rounded once: the whole word is built in the mantissa of one float by a chain of fused multiply-adds,
 //     a <- fma(dx_k, inv, a)      adds q_k (a is an even integer in [2^23, 2^24), so the FMA's rounding is RNE of the product)
 //     a <- fma(a, 4, -3*M)        shifts the partial word two bits up (exact), M = 1.5 * 2^23
+template <class E>
 __device__ __forceinline__ uint32_t quant8_int2(const uint4 &v, float lo, float inv)
 {
-    const float2 p0 = __half22float2(u2h(v.x)), p1 = __half22float2(u2h(v.y));
-    const float2 p2 = __half22float2(u2h(v.z)), p3 = __half22float2(u2h(v.w));
+    using H2 = typename E::H2;
+    const float2 p0 = to_f2(as_pair<H2>(v.x)), p1 = to_f2(as_pair<H2>(v.y));
+    const float2 p2 = to_f2(as_pair<H2>(v.z)), p3 = to_f2(as_pair<H2>(v.w));
     const float x[8] = {p0.x, p0.y, p1.x, p1.y, p2.x, p2.y, p3.x, p3.y};
     float a = __fmaf_rn(__fsub_rn(x[7], lo), inv, 12582912.0f);
 #pragma unroll
@@ -226,6 +268,7 @@ __device__ __forceinline__ uint32_t quant8_int2(const uint4 &v, float lo, float 
     return __float_as_uint(a) & 0xFFFFu;
 }
 // 16 bits of two-bit codes -> 8 fp16: y = f16_rn(fma(q, step, lo))
+template <class E>
 __device__ __forceinline__ uint4 dequant_int2(uint32_t w, float step, float lo)
 {
     float f[8];
@@ -233,19 +276,27 @@ __device__ __forceinline__ uint4 dequant_int2(uint32_t w, float step, float lo)
     for (int k = 0; k < 8; ++k)                          // int -> float through the 2^23 exponent trick (exact)
         f[k] = __fmaf_rn(__fsub_rn(__uint_as_float(0x4B000000u | ((w >> (2 * k)) & 3u)), 8388608.0f), step, lo);
     uint4 o;
-    o.x = h2_bits(f[0], f[1]); o.y = h2_bits(f[2], f[3]); o.z = h2_bits(f[4], f[5]); o.w = h2_bits(f[6], f[7]);
+    o.x = from_f2<E>(f[0], f[1]); o.y = from_f2<E>(f[2], f[3]); o.z = from_f2<E>(f[4], f[5]); o.w = from_f2<E>(f[6], f[7]);
     return o;
 }
 
-__device__ __forceinline__ float scale_of(__half amax, float qmax)
+template <class H>
+__device__ __forceinline__ float scale_of(H amax, float qmax)
 {
-    const float af = __half2float(amax);
+    const float af = to_f(amax);
     return af != 0.0f ? __fdiv_rn(af, qmax) : 0.0f;
 }
+// qmax/amax; only a bfloat16 amax below ~4e-37 can overflow the quotient: such a vector gets all-zero codes (P20)
 __device__ __forceinline__ float inv_of(__half amax, float qmax)
 {
-    const float af = __half2float(amax);
+    const float af = to_f(amax);
     return af != 0.0f ? __fdiv_rn(qmax, af) : 0.0f;
+}
+__device__ __forceinline__ float inv_of(__nv_bfloat16 amax, float qmax)
+{
+    const float af = to_f(amax);
+    const float q = af != 0.0f ? __fdiv_rn(qmax, af) : 0.0f;
+    return (q <= 3.402823466e38f) ? q : 0.0f;
 }
 
 }  // namespace skv

@@ -26,6 +26,7 @@ struct Geom {
     int32_t tiles;               // ceil(n / kTileTokens)
     int32_t patch;               // unpack only: 1 = tokens the blob does not carry (tier 0) are left untouched
     int32_t low_code;            // tier code of the low tier: 4 (symmetric INT4) or 2 (asymmetric 2-bit, NEXT-4)
+    int32_t bf16;                // element type of the dense caches and of the scale records: 0 = fp16, 1 = bfloat16
 };
 
 constexpr int kTileTokens = 32;  // tokens per pack/unpack tile (one ballot word)

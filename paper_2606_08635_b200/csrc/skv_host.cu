@@ -43,6 +43,7 @@ static int check_dims_supported(const skv_shape *s)
     if (!dims_ok(s)) return SKV_ERR_INVALID_ARG;
     if (s->head_dim != 64 && s->head_dim != 128 && s->head_dim != 256) return SKV_ERR_UNSUPPORTED;
     if (s->n_tokens > (1 << 20)) return SKV_ERR_UNSUPPORTED;
+    if ((s->dtype != SKV_F16 && s->dtype != SKV_BF16) || s->reserved != 0) return SKV_ERR_INVALID_ARG;
     if (s->n_layers > 65535 || s->n_requests > 65535 || (int64_t)s->n_layers * s->n_requests > 65535) return SKV_ERR_UNSUPPORTED;
     return SKV_OK;
 }
@@ -68,6 +69,7 @@ static Geom make_geom(const skv_shape *s, const skv_counts *c)
     g.tiles = (g.n + kTileTokens - 1) / kTileTokens;
     g.patch = 0;
     g.low_code = (c && c->allow_int4 == 2) ? 2 : 4;
+    g.bf16 = s->dtype == SKV_BF16 ? 1 : 0;
     return g;
 }
 
@@ -194,7 +196,7 @@ int skv_blob_check(const void *header_host, size_t blob_bytes, skv_shape *shape_
     const uint32_t flags = get32(h + 40);
     if (L == 0 || Hkv == 0 || n == 0 || L > 65535u || n > (1u << 20) || Hkv > 65535u) return SKV_ERR_BAD_BLOB;
     if (D != 64 && D != 128 && D != 256) return SKV_ERR_BAD_BLOB;
-    if ((uint64_t)n16 + n8 + n4 + n0 != n || (flags & ~3u) || flags == 2u || get32(h + 44) != 0) return SKV_ERR_BAD_BLOB;
+    if ((uint64_t)n16 + n8 + n4 + n0 != n || (flags & ~7u) || (flags & 3u) == 2u || get32(h + 44) != 0) return SKV_ERR_BAD_BLOB;
     if (!(flags & 1u) && n4 != 0) return SKV_ERR_BAD_BLOB;
     const bool low2 = (flags & 2u) != 0;                    // bit1: the low tier is asymmetric 2-bit (budget in eighths)
     const Layout lo = make_layout((int)L, (int)Hkv, (int)D, n, n16, n8, n4, low2 ? 2 : 4);
@@ -210,6 +212,7 @@ int skv_blob_check(const void *header_host, size_t blob_bytes, skv_shape *shape_
         memset(shape_out, 0, sizeof(*shape_out));
         shape_out->n_layers = (int32_t)L; shape_out->n_kv_heads = (int32_t)Hkv; shape_out->head_dim = (int32_t)D;
         shape_out->n_tokens = (int32_t)n; shape_out->n_requests = 1;
+        shape_out->dtype = (flags & 4u) ? SKV_BF16 : SKV_F16;
     }
     if (counts_out) {
         counts_out->n16 = (int32_t)n16; counts_out->n8 = (int32_t)n8; counts_out->n4 = (int32_t)n4; counts_out->n0 = (int32_t)n0;
@@ -316,7 +319,7 @@ int skv_pack(const skv_shape *shape, const void *K_dev, const void *V_dev, const
     put32(h + 0, 0x31564B53u); put32(h + 4, 1u);
     put32(h + 8, (uint32_t)g.L); put32(h + 12, (uint32_t)g.Hkv); put32(h + 16, (uint32_t)g.D); put32(h + 20, (uint32_t)g.n);
     put32(h + 24, (uint32_t)g.n16); put32(h + 28, (uint32_t)g.n8); put32(h + 32, (uint32_t)g.n4); put32(h + 36, (uint32_t)g.n0);
-    put32(h + 40, (counts->allow_int4 ? 1u : 0u) | (counts->allow_int4 == 2 ? 2u : 0u));
+    put32(h + 40, (counts->allow_int4 ? 1u : 0u) | (counts->allow_int4 == 2 ? 2u : 0u) | (g.bf16 ? 4u : 0u));
     put64(h + 48, (uint64_t)counts->budget_q4);
     put64(h + 56, lo.tier_map_off); put64(h + 64, lo.layer0_off); put64(h + 72, lo.layer_stride);
     for (int s = 0; s < 10; ++s) put64(h + 80 + 8 * s, lo.seg_off[s]);

@@ -7,6 +7,8 @@
 // entry-point dispatch and the KV-norm fallback score of Alg. 1 step 2.
 #include <algorithm>
 
+#include <cuda_bf16.h>
+
 #include "skv_common.cuh"
 
 namespace skv {
@@ -47,10 +49,14 @@ kvnorm_kernel(Geom g, const __half *__restrict__ K, float *__restrict__ raw /*[R
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
             const int e = e0 + u * 256 + lane * 8;
-            const __half2 *h = reinterpret_cast<const __half2 *>(&v[u]);
+            const uint32_t wv[4] = {v[u].x, v[u].y, v[u].z, v[u].w};
             float2 s2 = make_float2(0.f, 0.f);
 #pragma unroll
-            for (int k = 0; k < 4; ++k) { const float2 f = __half22float2(h[k]); s2 = __ffma2_rn(f, f, s2); }
+            for (int k = 0; k < 4; ++k) {
+                const float2 f = g.bf16 ? __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162 *>(&wv[k]))
+                                        : __half22float2(*reinterpret_cast<const __half2 *>(&wv[k]));
+                s2 = __ffma2_rn(f, f, s2);
+            }
             float ss = s2.x + s2.y;
             for (int o = 1; o < lpv; o <<= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
             if ((lane % lpv) == 0 && e < row_elems) acc += sqrtf(ss);

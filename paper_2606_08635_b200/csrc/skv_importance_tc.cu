@@ -94,10 +94,10 @@ __device__ __forceinline__ uint64_t umma_desc(uint32_t smem_addr)
     return (uint64_t)((smem_addr & 0x3FFFFu) >> 4) | ((uint64_t)1 << 16) | ((uint64_t)(1024 >> 4) << 32) |
            ((uint64_t)1 << 46) | ((uint64_t)2 << 61);
 }
-// kind::f16 instruction descriptor: fp16 x fp16 -> fp32, both operands K-major.
-__device__ __forceinline__ uint32_t umma_idesc(int M, int N)
+// kind::f16 instruction descriptor: fp16 x fp16 (or bf16 x bf16: a_format / b_format = 1) -> fp32, both operands K-major.
+__device__ __forceinline__ uint32_t umma_idesc(int M, int N, int bf16)
 {
-    return (1u << 4) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
+    return (1u << 4) | (bf16 ? ((1u << 7) | (1u << 10)) : 0u) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
 }
 __device__ __forceinline__ void umma_f16(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate)
 {
@@ -290,7 +290,7 @@ imp_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ C
         // ===================== MMA issuer =====================
         if (lane == 0) {
             uint32_t kstage = 0, kphase = 0, qphase = 0, astage = 0, aphase = 0;
-            const uint32_t idesc = (PASS == 1) ? umma_idesc(128, kTileKeys) : umma_idesc(128, p.qrows);
+            const uint32_t idesc = (PASS == 1) ? umma_idesc(128, kTileKeys, p.g.bf16) : umma_idesc(128, p.qrows, p.g.bf16);
             for (int item = blockIdx.x; item < p.n_items; item += gridDim.x) {
                 const Item it = decode_item(p, item);
                 mbar_wait(qfull, qphase); qphase ^= 1;
@@ -617,14 +617,15 @@ cudaError_t launch_importance_tc(const Geom &g, const __half *K, const __half *Q
         p.kdim[d[i].which] = i + 1;
     }
     CUtensorMap tmK, tmQ;
-    if (encode(&tmK, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 5, const_cast<__half *>(K), kdims, kstr, kbox, ones,
+    const CUtensorMapDataType et = g.bf16 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT16;
+    if (encode(&tmK, et, 5, const_cast<__half *>(K), kdims, kstr, kbox, ones,
                CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
         return cudaErrorNotSupported;
     cuuint64_t qdims[3] = {(cuuint64_t)g.D, (cuuint64_t)M, (cuuint64_t)g.R * g.L * g.Hkv};
     cuuint64_t qstr[2] = {(cuuint64_t)g.D * 2, (cuuint64_t)M * g.D * 2};
     cuuint32_t qbox[3] = {64, (cuuint32_t)t.qrows, 1};
-    if (encode(&tmQ, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 3, const_cast<__half *>(Q), qdims, qstr, qbox, ones,
+    if (encode(&tmQ, et, 3, const_cast<__half *>(Q), qdims, qstr, qbox, ones,
                CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
         return cudaErrorNotSupported;

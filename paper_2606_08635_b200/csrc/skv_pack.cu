@@ -12,32 +12,29 @@
 namespace skv {
 
 // |x| max of the 8 halves in a uint4, as a half2 with the max in both halves' union (max(lo,hi) taken later)
-__device__ __forceinline__ __half2 absmax8(const uint4 &v)
+template <class E>
+__device__ __forceinline__ typename E::H2 absmax8(const uint4 &v)
 {
-    const __half2 a = __habs2(*reinterpret_cast<const __half2 *>(&v.x));
-    const __half2 b = __habs2(*reinterpret_cast<const __half2 *>(&v.y));
-    const __half2 c = __habs2(*reinterpret_cast<const __half2 *>(&v.z));
-    const __half2 d = __habs2(*reinterpret_cast<const __half2 *>(&v.w));
+    using H2 = typename E::H2;
+    const H2 a = __habs2(as_pair<H2>(v.x)), b = __habs2(as_pair<H2>(v.y));
+    const H2 c = __habs2(as_pair<H2>(v.z)), d = __habs2(as_pair<H2>(v.w));
     return __hmax2(__hmax2(a, b), __hmax2(c, d));
 }
 
-template <int D, int QMAX>
-__device__ __forceinline__ void quantize_chunk(const uint4 &v, uint32_t lane, __half &amax_out, uint32_t codes[8])
+template <int D, int QMAX, class E>
+__device__ __forceinline__ void quantize_chunk(const uint4 &v, uint32_t lane, typename E::H &amax_out, uint32_t codes[8])
 {
+    using H = typename E::H; using H2 = typename E::H2;
     constexpr int LPV = D / 8;                        // lanes per head vector
-    __half2 m2 = absmax8(v);
+    H2 m2 = absmax8<E>(v);
 #pragma unroll
-    for (int o = 1; o < LPV; o <<= 1) {
-        const uint32_t other = __shfl_xor_sync(0xffffffffu, *reinterpret_cast<uint32_t *>(&m2), o);
-        m2 = __hmax2(m2, *reinterpret_cast<const __half2 *>(&other));
-    }
-    const __half amax = __hmax(__low2half(m2), __high2half(m2));
-    const float af = __half2float(amax);
-    const float inv = af != 0.0f ? __fdiv_rn((float)QMAX, af) : 0.0f;
-    const __half2 *h = reinterpret_cast<const __half2 *>(&v);
+    for (int o = 1; o < LPV; o <<= 1) m2 = __hmax2(m2, as_pair<H2>(__shfl_xor_sync(0xffffffffu, h2u(m2), o)));
+    const H amax = __hmax(lo_h(m2), hi_h(m2));
+    const float inv = inv_of(amax, (float)QMAX);
+    const uint32_t w[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
-        const float2 f = __half22float2(h[k]);
+        const float2 f = to_f2(as_pair<H2>(w[k]));
         codes[2 * k] = rne_code_bits(f.x, inv);
         codes[2 * k + 1] = rne_code_bits(f.y, inv);
     }
@@ -45,12 +42,13 @@ __device__ __forceinline__ void quantize_chunk(const uint4 &v, uint32_t lane, __
     (void)lane;
 }
 
-template <int D>
+template <int D, class E>
 __global__ void __launch_bounds__(256)
 pack_kernel(Geom g, Layout lo, const __half *__restrict__ K, const __half *__restrict__ V,
             const uint8_t *__restrict__ tier_map, uint8_t *__restrict__ blob, uint64_t blob_stride,
             const uint4 *__restrict__ tile_base)
 {
+    using H = typename E::H; using H2 = typename E::H2;
     constexpr int LPV = D / 8;
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
     const int64_t tile = blockIdx.x;
@@ -106,8 +104,8 @@ pack_kernel(Geom g, Layout lo, const __half *__restrict__ K, const __half *__res
             if (slot >= (uint32_t)g.n8) continue;
             uint8_t *kd = lbase + lo.seg_off[2] + (uint64_t)slot * row_elems;
             uint8_t *vd = lbase + lo.seg_off[3] + (uint64_t)slot * row_elems;
-            __half *ks = reinterpret_cast<__half *>(lbase + lo.seg_off[6]) + (uint64_t)slot * g.Hkv;
-            __half *vs = reinterpret_cast<__half *>(lbase + lo.seg_off[7]) + (uint64_t)slot * g.Hkv;
+            H *ks = reinterpret_cast<H *>(lbase + lo.seg_off[6]) + (uint64_t)slot * g.Hkv;
+            H *vs = reinterpret_cast<H *>(lbase + lo.seg_off[7]) + (uint64_t)slot * g.Hkv;
             for (int c0 = 0; c0 < g.row_chunks; c0 += 4) {
                 uint4 kv[4], vv[4];
 #pragma unroll
@@ -124,9 +122,9 @@ pack_kernel(Geom g, Layout lo, const __half *__restrict__ K, const __half *__res
                 for (int u = 0; u < 4; ++u) {
                     if ((c0 + u) * 256 >= row_elems) break;            // warp-uniform
                     const int e = (c0 + u) * 256 + lane * 8;
-                    __half ak, av; uint32_t ck[8], cv[8];
-                    quantize_chunk<D, 127>(kv[u], lane, ak, ck);
-                    quantize_chunk<D, 127>(vv[u], lane, av, cv);
+                    H ak, av; uint32_t ck[8], cv[8];
+                    quantize_chunk<D, 127, E>(kv[u], lane, ak, ck);
+                    quantize_chunk<D, 127, E>(vv[u], lane, av, cv);
                     if (e < row_elems) {
                         st_stream(kd + e, make_uint2(pack4_bytes(ck[0], ck[1], ck[2], ck[3]), pack4_bytes(ck[4], ck[5], ck[6], ck[7])));
                         st_stream(vd + e, make_uint2(pack4_bytes(cv[0], cv[1], cv[2], cv[3]), pack4_bytes(cv[4], cv[5], cv[6], cv[7])));
@@ -139,8 +137,8 @@ pack_kernel(Geom g, Layout lo, const __half *__restrict__ K, const __half *__res
             if (slot >= (uint32_t)g.n4) continue;
             uint8_t *kd = lbase + lo.seg_off[4] + (uint64_t)slot * (row_elems / 4);
             uint8_t *vd = lbase + lo.seg_off[5] + (uint64_t)slot * (row_elems / 4);
-            __half2 *ks = reinterpret_cast<__half2 *>(lbase + lo.seg_off[8]) + (uint64_t)slot * g.Hkv;
-            __half2 *vs = reinterpret_cast<__half2 *>(lbase + lo.seg_off[9]) + (uint64_t)slot * g.Hkv;
+            H2 *ks = reinterpret_cast<H2 *>(lbase + lo.seg_off[8]) + (uint64_t)slot * g.Hkv;
+            H2 *vs = reinterpret_cast<H2 *>(lbase + lo.seg_off[9]) + (uint64_t)slot * g.Hkv;
             for (int c0 = 0; c0 < g.row_chunks; ++c0) {
                 const int e = c0 * 256 + lane * 8;
                 const bool in = e < row_elems;
@@ -151,18 +149,18 @@ pack_kernel(Geom g, Layout lo, const __half *__restrict__ K, const __half *__res
                     vv = ld_stream(vrow + (int64_t)h * g.sh + c);
                 }
                 // lanes past the row hold zeros: they sit in head-vector groups of their own (row_elems % D == 0)
-                __half2 mk = max_negmin8(kv), mv = max_negmin8(vv);
+                H2 mk = max_negmin8<E>(kv), mv = max_negmin8<E>(vv);
 #pragma unroll
                 for (int o = 1; o < LPV; o <<= 1) {
-                    mk = __hmax2(mk, u2h(__shfl_xor_sync(0xffffffffu, h2u(mk), o)));
-                    mv = __hmax2(mv, u2h(__shfl_xor_sync(0xffffffffu, h2u(mv), o)));
+                    mk = __hmax2(mk, as_pair<H2>(__shfl_xor_sync(0xffffffffu, h2u(mk), o)));
+                    mv = __hmax2(mv, as_pair<H2>(__shfl_xor_sync(0xffffffffu, h2u(mv), o)));
                 }
-                __half loK, hiK, loV, hiV;
+                H loK, hiK, loV, hiV;
                 lohi_of(mk, loK, hiK); lohi_of(mv, loV, hiV);
                 if (in) {
-                    st_stream2(kd + e / 4, (uint16_t)quant8_int2(kv, __half2float(loK), inv3_of(range_of(loK, hiK))));
-                    st_stream2(vd + e / 4, (uint16_t)quant8_int2(vv, __half2float(loV), inv3_of(range_of(loV, hiV))));
-                    if ((lane % LPV) == 0) { ks[e / D] = __halves2half2(loK, hiK); vs[e / D] = __halves2half2(loV, hiV); }
+                    st_stream2(kd + e / 4, (uint16_t)quant8_int2<E>(kv, to_f(loK), inv3_of(range_of(loK, hiK))));
+                    st_stream2(vd + e / 4, (uint16_t)quant8_int2<E>(vv, to_f(loV), inv3_of(range_of(loV, hiV))));
+                    if ((lane % LPV) == 0) { ks[e / D] = pair_h(loK, hiK); vs[e / D] = pair_h(loV, hiV); }
                 }
             }
         } else {
@@ -170,8 +168,8 @@ pack_kernel(Geom g, Layout lo, const __half *__restrict__ K, const __half *__res
             if (slot >= (uint32_t)g.n4) continue;
             uint8_t *kd = lbase + lo.seg_off[4] + (uint64_t)slot * (row_elems / 2);
             uint8_t *vd = lbase + lo.seg_off[5] + (uint64_t)slot * (row_elems / 2);
-            __half *ks = reinterpret_cast<__half *>(lbase + lo.seg_off[8]) + (uint64_t)slot * g.Hkv;
-            __half *vs = reinterpret_cast<__half *>(lbase + lo.seg_off[9]) + (uint64_t)slot * g.Hkv;
+            H *ks = reinterpret_cast<H *>(lbase + lo.seg_off[8]) + (uint64_t)slot * g.Hkv;
+            H *vs = reinterpret_cast<H *>(lbase + lo.seg_off[9]) + (uint64_t)slot * g.Hkv;
             for (int c0 = 0; c0 < g.row_chunks; c0 += 4) {
                 uint4 kv[4], vv[4];
 #pragma unroll
@@ -188,9 +186,9 @@ pack_kernel(Geom g, Layout lo, const __half *__restrict__ K, const __half *__res
                 for (int u = 0; u < 4; ++u) {
                     if ((c0 + u) * 256 >= row_elems) break;
                     const int e = (c0 + u) * 256 + lane * 8;
-                    __half ak, av; uint32_t ck[8], cv[8];
-                    quantize_chunk<D, 7>(kv[u], lane, ak, ck);
-                    quantize_chunk<D, 7>(vv[u], lane, av, cv);
+                    H ak, av; uint32_t ck[8], cv[8];
+                    quantize_chunk<D, 7, E>(kv[u], lane, ak, ck);
+                    quantize_chunk<D, 7, E>(vv[u], lane, av, cv);
                     if (e < row_elems) {
                         uint32_t kb[4], vb[4];
 #pragma unroll
@@ -215,12 +213,13 @@ pack_kernel(Geom g, Layout lo, const __half *__restrict__ K, const __half *__res
 // of 2*NCH*log2(LPV) shuffles and 2*NCH divisions; the reciprocals are then broadcast with 2*NCH shuffles.
 // ------------------------------------------------------------------------------------------------
 // LOW2 = false: the low tier is symmetric INT4 (tier code 4).  LOW2 = true (NEXT-4): asymmetric 2-bit (tier code 2).
-template <int D, int NCH, int MINB, bool LOW2>
+template <int D, int NCH, int MINB, bool LOW2, class E>
 __global__ void __launch_bounds__(256, MINB)
 pack_fast_kernel(Geom g, Layout lo, const __half *__restrict__ K, const __half *__restrict__ V,
                  const uint8_t *__restrict__ tier_map, uint8_t *__restrict__ blob, uint64_t blob_stride,
                  const uint4 *__restrict__ tile_base)
 {
+    using H = typename E::H; using H2 = typename E::H2;
     constexpr int LPV = D / 8;                 // lanes per head vector
     constexpr int HPC = 256 / D;               // head vectors per 256-element chunk
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -277,20 +276,20 @@ pack_fast_kernel(Geom g, Layout lo, const __half *__restrict__ K, const __half *
             if (LOW2 && t == 2u) {
                 // asymmetric 2-bit: (max, -min) of K and of V reduced over the lanes of a head vector, (lo, hi) records,
                 // 16 bits of codes per lane and chunk
-                __half2 mk[NCH], mv[NCH];
+                H2 mk[NCH], mv[NCH];
 #pragma unroll
-                for (int u = 0; u < NCH; ++u) { mk[u] = max_negmin8(kv[u]); mv[u] = max_negmin8(vv[u]); }
-                const __half2 rk = group_absmax<LPV, NCH>(mk, lane), rv = group_absmax<LPV, NCH>(mv, lane);
-                __half loK, hiK, loV, hiV;
+                for (int u = 0; u < NCH; ++u) { mk[u] = max_negmin8<E>(kv[u]); mv[u] = max_negmin8<E>(vv[u]); }
+                const H2 rk = group_absmax<LPV, NCH>(mk, lane), rv = group_absmax<LPV, NCH>(mv, lane);
+                H loK, hiK, loV, hiV;
                 lohi_of(rk, loK, hiK); lohi_of(rv, loV, hiV);
                 const float invK = inv3_of(range_of(loK, hiK)), invV = inv3_of(range_of(loV, hiV));
-                const float lKf = __half2float(loK), lVf = __half2float(loV);
+                const float lKf = to_f(loK), lVf = to_f(loV);
                 if (scale_writer) {
                     const int head = (cb + my_chunk) * HPC + (int)(lane / LPV);
-                    __half2 *ks = reinterpret_cast<__half2 *>(lbase + lo.seg_off[8]) + (uint64_t)slot * g.Hkv;
-                    __half2 *vs = reinterpret_cast<__half2 *>(lbase + lo.seg_off[9]) + (uint64_t)slot * g.Hkv;
-                    ks[head] = __halves2half2(loK, hiK);
-                    vs[head] = __halves2half2(loV, hiV);
+                    H2 *ks = reinterpret_cast<H2 *>(lbase + lo.seg_off[8]) + (uint64_t)slot * g.Hkv;
+                    H2 *vs = reinterpret_cast<H2 *>(lbase + lo.seg_off[9]) + (uint64_t)slot * g.Hkv;
+                    ks[head] = pair_h(loK, hiK);
+                    vs[head] = pair_h(loV, hiV);
                 }
                 uint8_t *kd = lbase + lo.seg_off[4] + (uint64_t)slot * (row_elems / 4) + cb * 64 + lane * 2;
                 uint8_t *vd = lbase + lo.seg_off[5] + (uint64_t)slot * (row_elems / 4) + cb * 64 + lane * 2;
@@ -299,24 +298,24 @@ pack_fast_kernel(Geom g, Layout lo, const __half *__restrict__ K, const __half *
                     const int src = src_lane<LPV, NCH>(lane, u);
                     const float ik = __shfl_sync(0xffffffffu, invK, src), iv = __shfl_sync(0xffffffffu, invV, src);
                     const float lk = __shfl_sync(0xffffffffu, lKf, src), lv = __shfl_sync(0xffffffffu, lVf, src);
-                    st_stream2(kd + u * 64, (uint16_t)quant8_int2(kv[u], lk, ik));
-                    st_stream2(vd + u * 64, (uint16_t)quant8_int2(vv[u], lv, iv));
+                    st_stream2(kd + u * 64, (uint16_t)quant8_int2<E>(kv[u], lk, ik));
+                    st_stream2(vd + u * 64, (uint16_t)quant8_int2<E>(vv[u], lv, iv));
                 }
                 continue;
             }
-            __half2 m[NCH];
+            H2 m[NCH];
 #pragma unroll
-            for (int u = 0; u < NCH; ++u) m[u] = __halves2half2(absmax8_scalar(kv[u]), absmax8_scalar(vv[u]));
-            const __half2 a2 = group_absmax<LPV, NCH>(m, lane);      // (K amax, V amax) of chunk cb + my_chunk
+            for (int u = 0; u < NCH; ++u) m[u] = pair_h(absmax8_scalar<E>(kv[u]), absmax8_scalar<E>(vv[u]));
+            const H2 a2 = group_absmax<LPV, NCH>(m, lane);      // (K amax, V amax) of chunk cb + my_chunk
             const bool is8 = (t == 8u);
             const float qmax = is8 ? 127.0f : 7.0f;
-            const float invK = inv_of(__low2half(a2), qmax), invV = inv_of(__high2half(a2), qmax);
+            const float invK = inv_of(lo_h(a2), qmax), invV = inv_of(hi_h(a2), qmax);
             if (scale_writer) {
                 const int head = (cb + my_chunk) * HPC + (int)(lane / LPV);
-                __half *ks = reinterpret_cast<__half *>(lbase + lo.seg_off[is8 ? 6 : 8]) + (uint64_t)slot * g.Hkv;
-                __half *vs = reinterpret_cast<__half *>(lbase + lo.seg_off[is8 ? 7 : 9]) + (uint64_t)slot * g.Hkv;
-                ks[head] = __low2half(a2);
-                vs[head] = __high2half(a2);
+                H *ks = reinterpret_cast<H *>(lbase + lo.seg_off[is8 ? 6 : 8]) + (uint64_t)slot * g.Hkv;
+                H *vs = reinterpret_cast<H *>(lbase + lo.seg_off[is8 ? 7 : 9]) + (uint64_t)slot * g.Hkv;
+                ks[head] = lo_h(a2);
+                vs[head] = hi_h(a2);
             }
             if (is8) {
                 uint8_t *kd = lbase + lo.seg_off[2] + (uint64_t)slot * row_elems + cb * 256 + lane * 8;
@@ -325,8 +324,8 @@ pack_fast_kernel(Geom g, Layout lo, const __half *__restrict__ K, const __half *
                 for (int u = 0; u < NCH; ++u) {
                     const int src = src_lane<LPV, NCH>(lane, u);
                     const float ik = __shfl_sync(0xffffffffu, invK, src), iv = __shfl_sync(0xffffffffu, invV, src);
-                    st_stream(kd + u * 256, quant8_int8(kv[u], ik));
-                    st_stream(vd + u * 256, quant8_int8(vv[u], iv));
+                    st_stream(kd + u * 256, quant8_int8<E>(kv[u], ik));
+                    st_stream(vd + u * 256, quant8_int8<E>(vv[u], iv));
                 }
             } else {
                 uint8_t *kd = lbase + lo.seg_off[4] + (uint64_t)slot * (row_elems / 2) + cb * 128 + lane * 4;
@@ -335,37 +334,37 @@ pack_fast_kernel(Geom g, Layout lo, const __half *__restrict__ K, const __half *
                 for (int u = 0; u < NCH; ++u) {
                     const int src = src_lane<LPV, NCH>(lane, u);
                     const float ik = __shfl_sync(0xffffffffu, invK, src), iv = __shfl_sync(0xffffffffu, invV, src);
-                    st_stream(kd + u * 128, quant8_int4(kv[u], ik));
-                    st_stream(vd + u * 128, quant8_int4(vv[u], iv));
+                    st_stream(kd + u * 128, quant8_int4<E>(kv[u], ik));
+                    st_stream(vd + u * 128, quant8_int4<E>(vv[u], iv));
                 }
             }
         }
     }
 }
 
-template <int D, int NCH>
+template <int D, int NCH, class E>
 static cudaError_t launch_pack_fast(const Geom &g, const Layout &lo, const __half *K, const __half *V,
                                     const uint8_t *tier_map, uint8_t *blob, uint64_t blob_stride,
                                     const uint4 *tile_base, cudaStream_t s)
 {
     dim3 grid(g.tiles, g.L, g.R);
-    if (g.low_code == 2) pack_fast_kernel<D, NCH, 2, true><<<grid, 256, 0, s>>>(g, lo, K, V, tier_map, blob, blob_stride, tile_base);
-    else pack_fast_kernel<D, NCH, 3, false><<<grid, 256, 0, s>>>(g, lo, K, V, tier_map, blob, blob_stride, tile_base);
+    if (g.low_code == 2) pack_fast_kernel<D, NCH, 2, true, E><<<grid, 256, 0, s>>>(g, lo, K, V, tier_map, blob, blob_stride, tile_base);
+    else pack_fast_kernel<D, NCH, 3, false, E><<<grid, 256, 0, s>>>(g, lo, K, V, tier_map, blob, blob_stride, tile_base);
     return cudaGetLastError();
 }
 
-template <int D>
+template <int D, class E>
 static cudaError_t launch_pack_d(const Geom &g, const Layout &lo, const __half *K, const __half *V,
                                  const uint8_t *tier_map, uint8_t *blob, uint64_t blob_stride,
                                  const uint4 *tile_base, cudaStream_t s)
 {
     if ((g.Hkv * D) % 256 == 0) {
-        if (g.row_chunks % 4 == 0) return launch_pack_fast<D, 4>(g, lo, K, V, tier_map, blob, blob_stride, tile_base, s);
-        if (g.row_chunks % 2 == 0) return launch_pack_fast<D, 2>(g, lo, K, V, tier_map, blob, blob_stride, tile_base, s);
-        return launch_pack_fast<D, 1>(g, lo, K, V, tier_map, blob, blob_stride, tile_base, s);
+        if (g.row_chunks % 4 == 0) return launch_pack_fast<D, 4, E>(g, lo, K, V, tier_map, blob, blob_stride, tile_base, s);
+        if (g.row_chunks % 2 == 0) return launch_pack_fast<D, 2, E>(g, lo, K, V, tier_map, blob, blob_stride, tile_base, s);
+        return launch_pack_fast<D, 1, E>(g, lo, K, V, tier_map, blob, blob_stride, tile_base, s);
     }
     dim3 grid(g.tiles, g.L, g.R);
-    pack_kernel<D><<<grid, 256, 0, s>>>(g, lo, K, V, tier_map, blob, blob_stride, tile_base);
+    pack_kernel<D, E><<<grid, 256, 0, s>>>(g, lo, K, V, tier_map, blob, blob_stride, tile_base);
     return cudaGetLastError();
 }
 
@@ -373,9 +372,12 @@ cudaError_t launch_pack(const Geom &g, const Layout &lo, const __half *K, const 
                         uint8_t *blob, uint64_t blob_stride, const uint4 *tile_base, cudaStream_t s)
 {
     switch (g.D) {
-    case 64:  return launch_pack_d<64>(g, lo, K, V, tier_map, blob, blob_stride, tile_base, s);
-    case 128: return launch_pack_d<128>(g, lo, K, V, tier_map, blob, blob_stride, tile_base, s);
-    case 256: return launch_pack_d<256>(g, lo, K, V, tier_map, blob, blob_stride, tile_base, s);
+    case 64: return g.bf16 ? launch_pack_d<64, ElemBF16>(g, lo, K, V, tier_map, blob, blob_stride, tile_base, s)
+                            : launch_pack_d<64, ElemF16>(g, lo, K, V, tier_map, blob, blob_stride, tile_base, s);
+    case 128: return g.bf16 ? launch_pack_d<128, ElemBF16>(g, lo, K, V, tier_map, blob, blob_stride, tile_base, s)
+                            : launch_pack_d<128, ElemF16>(g, lo, K, V, tier_map, blob, blob_stride, tile_base, s);
+    case 256: return g.bf16 ? launch_pack_d<256, ElemBF16>(g, lo, K, V, tier_map, blob, blob_stride, tile_base, s)
+                            : launch_pack_d<256, ElemF16>(g, lo, K, V, tier_map, blob, blob_stride, tile_base, s);
     default: return cudaErrorInvalidValue;
     }
 }

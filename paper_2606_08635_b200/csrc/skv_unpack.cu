@@ -10,11 +10,12 @@
 
 namespace skv {
 
-template <int D>
+template <int D, class E>
 __global__ void __launch_bounds__(256)
 unpack_kernel(Geom g, Layout lo, const uint8_t *__restrict__ blob, uint64_t blob_stride,
               __half *__restrict__ K, __half *__restrict__ V, const uint4 *__restrict__ tile_base)
 {
+    using H = typename E::H; using H2 = typename E::H2;
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
     const int64_t tile = blockIdx.x;
     const int l = blockIdx.y, r = blockIdx.z;
@@ -71,10 +72,10 @@ unpack_kernel(Geom g, Layout lo, const uint8_t *__restrict__ blob, uint64_t blob
         } else if (t == 8u) {
             const uint8_t *ks = lbase + lo.seg_off[2] + (uint64_t)slot * row_elems;
             const uint8_t *vs = lbase + lo.seg_off[3] + (uint64_t)slot * row_elems;
-            const __half *ka = reinterpret_cast<const __half *>(lbase + lo.seg_off[6]) + (uint64_t)slot * g.Hkv;
-            const __half *va = reinterpret_cast<const __half *>(lbase + lo.seg_off[7]) + (uint64_t)slot * g.Hkv;
+            const H *ka = reinterpret_cast<const H *>(lbase + lo.seg_off[6]) + (uint64_t)slot * g.Hkv;
+            const H *va = reinterpret_cast<const H *>(lbase + lo.seg_off[7]) + (uint64_t)slot * g.Hkv;
             for (int c0 = 0; c0 < g.row_chunks; c0 += 4) {
-                uint2 kv[4], vv[4]; __half ak[4], av[4];
+                uint2 kv[4], vv[4]; H ak[4], av[4];
 #pragma unroll
                 for (int u = 0; u < 4; ++u) {
                     const int e = (c0 + u) * 256 + lane * 8;
@@ -88,35 +89,35 @@ unpack_kernel(Geom g, Layout lo, const uint8_t *__restrict__ blob, uint64_t blob
                     const int e = (c0 + u) * 256 + lane * 8;
                     if (e < row_elems) {
                         const int h = e / D, c = e % D;
-                        st_stream(krow + (int64_t)h * g.sh + c, dequant_int8(kv[u], scale_of(ak[u], 127.0f)));
-                        st_stream(vrow + (int64_t)h * g.sh + c, dequant_int8(vv[u], scale_of(av[u], 127.0f)));
+                        st_stream(krow + (int64_t)h * g.sh + c, dequant_int8<E>(kv[u], scale_of(ak[u], 127.0f)));
+                        st_stream(vrow + (int64_t)h * g.sh + c, dequant_int8<E>(vv[u], scale_of(av[u], 127.0f)));
                     }
                 }
             }
         } else if (t == 2u) {
             const uint8_t *ks = lbase + lo.seg_off[4] + (uint64_t)slot * (row_elems / 4);
             const uint8_t *vs = lbase + lo.seg_off[5] + (uint64_t)slot * (row_elems / 4);
-            const __half2 *ka = reinterpret_cast<const __half2 *>(lbase + lo.seg_off[8]) + (uint64_t)slot * g.Hkv;
-            const __half2 *va = reinterpret_cast<const __half2 *>(lbase + lo.seg_off[9]) + (uint64_t)slot * g.Hkv;
+            const H2 *ka = reinterpret_cast<const H2 *>(lbase + lo.seg_off[8]) + (uint64_t)slot * g.Hkv;
+            const H2 *va = reinterpret_cast<const H2 *>(lbase + lo.seg_off[9]) + (uint64_t)slot * g.Hkv;
             for (int c0 = 0; c0 < g.row_chunks; ++c0) {
                 const int e = c0 * 256 + lane * 8;
                 if (e < row_elems) {
                     const int h = e / D, c = e % D;
-                    const __half2 rk = ka[h], rv = va[h];                // (lo, hi) records
+                    const H2 rk = ka[h], rv = va[h];                // (lo, hi) records
                     const uint32_t kw = ld_stream2(ks + e / 4), vw = ld_stream2(vs + e / 4);
                     st_stream(krow + (int64_t)h * g.sh + c,
-                              dequant_int2(kw, step3_of(range_of(__low2half(rk), __high2half(rk))), __half2float(__low2half(rk))));
+                              dequant_int2<E>(kw, step3_of(range_of(lo_h(rk), hi_h(rk))), to_f(lo_h(rk))));
                     st_stream(vrow + (int64_t)h * g.sh + c,
-                              dequant_int2(vw, step3_of(range_of(__low2half(rv), __high2half(rv))), __half2float(__low2half(rv))));
+                              dequant_int2<E>(vw, step3_of(range_of(lo_h(rv), hi_h(rv))), to_f(lo_h(rv))));
                 }
             }
         } else if (t == 4u) {
             const uint8_t *ks = lbase + lo.seg_off[4] + (uint64_t)slot * (row_elems / 2);
             const uint8_t *vs = lbase + lo.seg_off[5] + (uint64_t)slot * (row_elems / 2);
-            const __half *ka = reinterpret_cast<const __half *>(lbase + lo.seg_off[8]) + (uint64_t)slot * g.Hkv;
-            const __half *va = reinterpret_cast<const __half *>(lbase + lo.seg_off[9]) + (uint64_t)slot * g.Hkv;
+            const H *ka = reinterpret_cast<const H *>(lbase + lo.seg_off[8]) + (uint64_t)slot * g.Hkv;
+            const H *va = reinterpret_cast<const H *>(lbase + lo.seg_off[9]) + (uint64_t)slot * g.Hkv;
             for (int c0 = 0; c0 < g.row_chunks; c0 += 4) {
-                uint32_t kv[4], vv[4]; __half ak[4], av[4];
+                uint32_t kv[4], vv[4]; H ak[4], av[4];
 #pragma unroll
                 for (int u = 0; u < 4; ++u) {
                     const int e = (c0 + u) * 256 + lane * 8;
@@ -130,8 +131,8 @@ unpack_kernel(Geom g, Layout lo, const uint8_t *__restrict__ blob, uint64_t blob
                     const int e = (c0 + u) * 256 + lane * 8;
                     if (e < row_elems) {
                         const int h = e / D, c = e % D;
-                        st_stream(krow + (int64_t)h * g.sh + c, dequant_int4(kv[u], scale_of(ak[u], 7.0f)));
-                        st_stream(vrow + (int64_t)h * g.sh + c, dequant_int4(vv[u], scale_of(av[u], 7.0f)));
+                        st_stream(krow + (int64_t)h * g.sh + c, dequant_int4<E>(kv[u], scale_of(ak[u], 7.0f)));
+                        st_stream(vrow + (int64_t)h * g.sh + c, dequant_int4<E>(vv[u], scale_of(av[u], 7.0f)));
                     }
                 }
             }
@@ -153,11 +154,12 @@ unpack_kernel(Geom g, Layout lo, const uint8_t *__restrict__ blob, uint64_t blob
 // Fast path (row_elems % (256*NCH) == 0): fully unrolled; each lane loads the amax record of ONE
 // (chunk, head) for K and V, divides twice, and the scales are broadcast with 2*NCH shuffles.
 // ------------------------------------------------------------------------------------------------
-template <int D, int NCH, int MINB, bool LOW2>
+template <int D, int NCH, int MINB, bool LOW2, class E>
 __global__ void __launch_bounds__(256, MINB)
 unpack_fast_kernel(Geom g, Layout lo, const uint8_t *__restrict__ blob, uint64_t blob_stride,
                    __half *__restrict__ K, __half *__restrict__ V, const uint4 *__restrict__ tile_base)
 {
+    using H = typename E::H; using H2 = typename E::H2;
     constexpr int LPV = D / 8;
     constexpr int HPC = 256 / D;
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -216,16 +218,16 @@ unpack_fast_kernel(Geom g, Layout lo, const uint8_t *__restrict__ blob, uint64_t
                 uint2 kv[NCH], vv[NCH];
 #pragma unroll
                 for (int u = 0; u < NCH; ++u) { kv[u] = ld_stream8(ks + u * 256); vv[u] = ld_stream8(vs + u * 256); }
-                const __half ak = reinterpret_cast<const __half *>(lbase + lo.seg_off[6])[(uint64_t)slot * g.Hkv + head];
-                const __half av = reinterpret_cast<const __half *>(lbase + lo.seg_off[7])[(uint64_t)slot * g.Hkv + head];
+                const H ak = reinterpret_cast<const H *>(lbase + lo.seg_off[6])[(uint64_t)slot * g.Hkv + head];
+                const H av = reinterpret_cast<const H *>(lbase + lo.seg_off[7])[(uint64_t)slot * g.Hkv + head];
                 const float sK = scale_of(ak, 127.0f), sV = scale_of(av, 127.0f);
 #pragma unroll
                 for (int u = 0; u < NCH; ++u) {
                     const int src = src_lane<LPV, NCH>(lane, u);
                     const float sk = __shfl_sync(0xffffffffu, sK, src), sv = __shfl_sync(0xffffffffu, sV, src);
                     const int64_t off = (int64_t)((cb + u) * HPC + lane_h) * g.sh;
-                    st_stream(krow + off, dequant_int8(kv[u], sk));
-                    st_stream(vrow + off, dequant_int8(vv[u], sv));
+                    st_stream(krow + off, dequant_int8<E>(kv[u], sk));
+                    st_stream(vrow + off, dequant_int8<E>(vv[u], sv));
                 }
             } else if (LOW2 && t == 2u) {
                 const uint8_t *ks = lbase + lo.seg_off[4] + (uint64_t)slot * (row_elems / 4) + cb * 64 + lane * 2;
@@ -234,18 +236,18 @@ unpack_fast_kernel(Geom g, Layout lo, const uint8_t *__restrict__ blob, uint64_t
                 uint32_t kv[NCH], vv[NCH];
 #pragma unroll
                 for (int u = 0; u < NCH; ++u) { kv[u] = ld_stream2(ks + u * 64); vv[u] = ld_stream2(vs + u * 64); }
-                const __half2 rk = reinterpret_cast<const __half2 *>(lbase + lo.seg_off[8])[(uint64_t)slot * g.Hkv + head];
-                const __half2 rv = reinterpret_cast<const __half2 *>(lbase + lo.seg_off[9])[(uint64_t)slot * g.Hkv + head];
-                const float sK = step3_of(range_of(__low2half(rk), __high2half(rk))), lK = __half2float(__low2half(rk));
-                const float sV = step3_of(range_of(__low2half(rv), __high2half(rv))), lV = __half2float(__low2half(rv));
+                const H2 rk = reinterpret_cast<const H2 *>(lbase + lo.seg_off[8])[(uint64_t)slot * g.Hkv + head];
+                const H2 rv = reinterpret_cast<const H2 *>(lbase + lo.seg_off[9])[(uint64_t)slot * g.Hkv + head];
+                const float sK = step3_of(range_of(lo_h(rk), hi_h(rk))), lK = to_f(lo_h(rk));
+                const float sV = step3_of(range_of(lo_h(rv), hi_h(rv))), lV = to_f(lo_h(rv));
 #pragma unroll
                 for (int u = 0; u < NCH; ++u) {
                     const int src = src_lane<LPV, NCH>(lane, u);
                     const float sk = __shfl_sync(0xffffffffu, sK, src), sv = __shfl_sync(0xffffffffu, sV, src);
                     const float lk = __shfl_sync(0xffffffffu, lK, src), lv = __shfl_sync(0xffffffffu, lV, src);
                     const int64_t off = (int64_t)((cb + u) * HPC + lane_h) * g.sh;
-                    st_stream(krow + off, dequant_int2(kv[u], sk, lk));
-                    st_stream(vrow + off, dequant_int2(vv[u], sv, lv));
+                    st_stream(krow + off, dequant_int2<E>(kv[u], sk, lk));
+                    st_stream(vrow + off, dequant_int2<E>(vv[u], sv, lv));
                 }
             } else if (!LOW2 && t == 4u) {
                 const uint8_t *ks = lbase + lo.seg_off[4] + (uint64_t)slot * (row_elems / 2) + cb * 128 + lane * 4;
@@ -254,16 +256,16 @@ unpack_fast_kernel(Geom g, Layout lo, const uint8_t *__restrict__ blob, uint64_t
                 uint32_t kv[NCH], vv[NCH];
 #pragma unroll
                 for (int u = 0; u < NCH; ++u) { kv[u] = ld_stream4(ks + u * 128); vv[u] = ld_stream4(vs + u * 128); }
-                const __half ak = reinterpret_cast<const __half *>(lbase + lo.seg_off[8])[(uint64_t)slot * g.Hkv + head];
-                const __half av = reinterpret_cast<const __half *>(lbase + lo.seg_off[9])[(uint64_t)slot * g.Hkv + head];
+                const H ak = reinterpret_cast<const H *>(lbase + lo.seg_off[8])[(uint64_t)slot * g.Hkv + head];
+                const H av = reinterpret_cast<const H *>(lbase + lo.seg_off[9])[(uint64_t)slot * g.Hkv + head];
                 const float sK = scale_of(ak, 7.0f), sV = scale_of(av, 7.0f);
 #pragma unroll
                 for (int u = 0; u < NCH; ++u) {
                     const int src = src_lane<LPV, NCH>(lane, u);
                     const float sk = __shfl_sync(0xffffffffu, sK, src), sv = __shfl_sync(0xffffffffu, sV, src);
                     const int64_t off = (int64_t)((cb + u) * HPC + lane_h) * g.sh;
-                    st_stream(krow + off, dequant_int4(kv[u], sk));
-                    st_stream(vrow + off, dequant_int4(vv[u], sv));
+                    st_stream(krow + off, dequant_int4<E>(kv[u], sk));
+                    st_stream(vrow + off, dequant_int4<E>(vv[u], sv));
                 }
             } else {
                 const uint4 z = make_uint4(0, 0, 0, 0);
@@ -277,21 +279,21 @@ unpack_fast_kernel(Geom g, Layout lo, const uint8_t *__restrict__ blob, uint64_t
     }
 }
 
-template <int D>
+template <int D, class E>
 static cudaError_t launch_unpack_d(const Geom &g, const Layout &lo, const uint8_t *blob, uint64_t blob_stride,
                                    __half *K, __half *V, const uint4 *tile_base, cudaStream_t s)
 {
     dim3 grid(g.tiles, g.L, g.R);
     if ((g.Hkv * D) % 256 == 0) {
         if (g.low_code == 2) {
-            if (g.row_chunks % 4 == 0) unpack_fast_kernel<D, 4, 3, true><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tile_base);
-            else if (g.row_chunks % 2 == 0) unpack_fast_kernel<D, 2, 3, true><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tile_base);
-            else unpack_fast_kernel<D, 1, 3, true><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tile_base);
-        } else if (g.row_chunks % 4 == 0) unpack_fast_kernel<D, 4, 3, false><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tile_base);
-        else if (g.row_chunks % 2 == 0) unpack_fast_kernel<D, 2, 3, false><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tile_base);
-        else unpack_fast_kernel<D, 1, 3, false><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tile_base);
+            if (g.row_chunks % 4 == 0) unpack_fast_kernel<D, 4, 3, true, E><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tile_base);
+            else if (g.row_chunks % 2 == 0) unpack_fast_kernel<D, 2, 3, true, E><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tile_base);
+            else unpack_fast_kernel<D, 1, 3, true, E><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tile_base);
+        } else if (g.row_chunks % 4 == 0) unpack_fast_kernel<D, 4, 3, false, E><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tile_base);
+        else if (g.row_chunks % 2 == 0) unpack_fast_kernel<D, 2, 3, false, E><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tile_base);
+        else unpack_fast_kernel<D, 1, 3, false, E><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tile_base);
     } else {
-        unpack_kernel<D><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tile_base);
+        unpack_kernel<D, E><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tile_base);
     }
     return cudaGetLastError();
 }
@@ -300,9 +302,12 @@ cudaError_t launch_unpack(const Geom &g, const Layout &lo, const uint8_t *blob, 
                           __half *K, __half *V, const uint4 *tile_base, cudaStream_t s)
 {
     switch (g.D) {
-    case 64:  return launch_unpack_d<64>(g, lo, blob, blob_stride, K, V, tile_base, s);
-    case 128: return launch_unpack_d<128>(g, lo, blob, blob_stride, K, V, tile_base, s);
-    case 256: return launch_unpack_d<256>(g, lo, blob, blob_stride, K, V, tile_base, s);
+    case 64: return g.bf16 ? launch_unpack_d<64, ElemBF16>(g, lo, blob, blob_stride, K, V, tile_base, s)
+                            : launch_unpack_d<64, ElemF16>(g, lo, blob, blob_stride, K, V, tile_base, s);
+    case 128: return g.bf16 ? launch_unpack_d<128, ElemBF16>(g, lo, blob, blob_stride, K, V, tile_base, s)
+                            : launch_unpack_d<128, ElemF16>(g, lo, blob, blob_stride, K, V, tile_base, s);
+    case 256: return g.bf16 ? launch_unpack_d<256, ElemBF16>(g, lo, blob, blob_stride, K, V, tile_base, s)
+                            : launch_unpack_d<256, ElemF16>(g, lo, blob, blob_stride, K, V, tile_base, s);
     default: return cudaErrorInvalidValue;
     }
 }

@@ -566,3 +566,83 @@ def test_assign_with_explicit_populations_balanced_and_random_tier():
     oc, prot = oracle.tier_counts(n, 0.4, s, (), True)
     assert c.as_tuple() == (oc.n16, oc.n8, oc.n4, oc.n0)
     assert np.array_equal(tier.cpu().numpy()[0], oracle.assign(I, prot, oc))
+
+
+def _bf16_case(cfg, b, seed_req=0):
+    """bfloat16 inputs from the seeded fp32 draws of skv_synth (cast to bf16 instead of fp16), as uint16 bits."""
+    K, V = skv_synth.make_kv(cfg, seed_req)
+    Q = skv_synth.make_q(cfg, seed_req)
+    tb = lambda t: t.float().to(torch.bfloat16)
+    return tb(K), tb(V), tb(Q)
+
+
+def _bits(t):
+    return t.contiguous().view(torch.int16).cpu().numpy().view(np.uint16)
+
+
+@pytest.mark.parametrize("d,Hkv,Hq,n,b,a4", [(128, 8, 32, 1000, 0.4, 1), (128, 2, 4, 513, 0.3, 1), (64, 3, 3, 257, 0.5, 0),
+                                             (256, 2, 4, 640, 0.75, 1), (128, 4, 8, 300, 0.2, 2), (64, 8, 8, 96, 1.0, 1)])
+def test_bfloat16_caches_parity(d, Hkv, Hq, n, b, a4):
+    """NEXT-4 (reading P20): bfloat16 K, V, Q through the whole path -- importance within 1e-3 of the float64 oracle on
+    the same bf16 values; tier map, every blob byte (records are bf16, flags bit2) and the dequantised bf16 cache
+    bit-exact given the oracle's importance; skv_blob_check reports the element type."""
+    dev = torch.device("cuda:0")
+    cfg = skv_synth.Config("bf16", L=2, Hq=Hq, Hkv=Hkv, d=d, n=n, w=16, R=1, n_sink=2, seed=61, allow_int4=a4)
+    K, V, Q = _bf16_case(cfg, b)
+    Kb, Vb, Qb = _bits(K), _bits(V), _bits(Q)
+    I_or = oracle.importance(Kb, Qb, bf16=True)
+    counts, prot = oracle.tier_counts(n, b, cfg.n_sink, (), a4)
+    tier_or = oracle.assign(I_or, prot, counts)
+    blob_or = oracle.pack(Kb, Vb, tier_or, counts, a4, bf16=True)
+    K2_or, V2_or, _ = oracle.unpack(blob_or, cfg.L, Hkv, d, n, bf16=True)
+
+    shape = skv.make_shape(cfg.L, Hq, Hkv, d, n, 1, dtype="bf16")
+    pol = skv.make_policy(b, cfg.n_sink, (), a4)
+    ws = torch.empty(skv.skv_workspace_bytes(shape, cfg.w), dtype=torch.uint8, device=dev)
+    Kd, Vd, Qd = K[None].to(dev), V[None].to(dev), Q[None].to(dev)
+    I = torch.full((1, cfg.L, n), float("nan"), dtype=torch.float32, device=dev)
+    skv.skv_importance(shape, Kd, Qd, cfg.w, I, ws)
+    Ig = I[0].cpu().numpy().astype(np.float64)
+    assert np.all(np.abs(Ig - I_or) <= 1e-3 * I_or.astype(np.float64) + 1e-30)
+    tier = torch.full((1, cfg.L, n), 0xEE, dtype=torch.uint8, device=dev)
+    c = skv.skv_assign_tiers(shape, pol, torch.from_numpy(I_or)[None].to(dev), tier, ws)
+    assert c.as_tuple() == (counts.n16, counts.n8, counts.n4, counts.n0)
+    assert np.array_equal(tier[0].cpu().numpy(), tier_or)
+    bb = skv.skv_blob_bytes(shape, c)
+    blob = torch.full((bb,), 0xAB, dtype=torch.uint8, device=dev)
+    skv.skv_pack(shape, Kd, Vd, tier, c, blob, ws)
+    hb = blob.cpu().numpy()
+    assert np.array_equal(hb, blob_or)
+    hs, hc = skv.skv_blob_check(hb[:256].tobytes(), bb)
+    assert hs.dtype == skv.SKV_BF16 and hc.as_tuple() == c.as_tuple()
+    Ko = torch.full_like(Kd, float("nan")); Vo = torch.full_like(Vd, float("nan"))
+    skv.skv_unpack(shape, blob, bb, hc, Ko, Vo, None, ws)
+    torch.cuda.synchronize()
+    assert np.array_equal(_bits(Ko[0]), K2_or) and np.array_equal(_bits(Vo[0]), V2_or)
+    # KV-norm score on bf16 keys
+    skv.skv_importance_kvnorm(shape, Kd, I, ws)
+    want = oracle.importance_kvnorm(Kb, bf16=True).astype(np.float64)
+    assert np.all(np.abs(I[0].cpu().numpy() - want) <= 1e-3 * want + 1e-30)
+
+
+def test_bfloat16_vanishing_amax_gets_zero_codes():
+    """P20: a bf16 vector whose amax is so small that qmax/amax overflows binary32 is coded as zeros, on both sides."""
+    dev = torch.device("cuda:0")
+    L, n, Hkv, d = 1, 64, 2, 128
+    K = torch.zeros((L, n, Hkv, d), dtype=torch.bfloat16); V = torch.zeros_like(K)
+    K[0, :, 0, :] = 1e-39; K[0, :, 1, ::3] = -3e-40; V[0, :, 0, 5] = 1e-38; V[0, :, 1, :] = 0.5
+    tier_or = np.full((L, n), 8, np.uint8); tier_or[0, ::2] = 4; tier_or[0, 0] = 16
+    n16, n8, n4 = int((tier_or == 16).sum()), int((tier_or == 8).sum()), int((tier_or == 4).sum())
+    shape = skv.make_shape(L, 2, Hkv, d, n, 1, dtype="bf16")
+    c = skv.skv_counts_from_populations(shape, n16, n8, n4)
+    oc = oracle.Counts(n16, n8, n4, 0, c.budget_q4, c.spent_q4)
+    blob_or = oracle.pack(_bits(K), _bits(V), tier_or, oc, True, bf16=True)
+    ws = torch.empty(skv.skv_workspace_bytes(shape, 0), dtype=torch.uint8, device=dev)
+    bb = skv.skv_blob_bytes(shape, c)
+    blob = torch.empty((bb,), dtype=torch.uint8, device=dev)
+    skv.skv_pack(shape, K[None].to(dev), V[None].to(dev), torch.from_numpy(tier_or)[None].to(dev), c, blob, ws)
+    assert np.array_equal(blob.cpu().numpy(), blob_or)
+    Ko = torch.empty((1, L, n, Hkv, d), dtype=torch.bfloat16, device=dev); Vo = torch.empty_like(Ko)
+    skv.skv_unpack(shape, blob, bb, c, Ko, Vo, None, ws)
+    K2, V2, _ = oracle.unpack(blob_or, L, Hkv, d, n, bf16=True)
+    assert np.array_equal(_bits(Ko[0]), K2) and np.array_equal(_bits(Vo[0]), V2)
