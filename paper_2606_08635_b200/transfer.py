@@ -25,19 +25,21 @@ from . import (make_policy, make_shape, skv_assign_tiers, skv_blob_bytes, skv_bl
 
 class LayerPipelinedTransfer:
     def __init__(self, L, Hq, Hkv, d, n, w, budget, n_sink=0, ranges=(), allow_int4=True, layers_per_chunk=4,
-                 depth=3, device="cuda:0", causal=True, lam=0.0):
-        """n is the LARGEST token count any request will have (device slots are sized for it)."""
+                 depth=3, device="cuda:0", causal=True, lam=0.0, dtype="f16"):
+        """n is the LARGEST token count any request will have (device slots are sized for it).  dtype: "f16" | "bf16"
+        (element type of the host caches; they must be torch.float16 / torch.bfloat16 tensors accordingly)."""
         assert depth >= 2 and layers_per_chunk >= 1
         self.L, self.Hq, self.Hkv, self.d, self.n, self.w = L, Hq, Hkv, d, n, w
         self.Lc, self.depth, self.causal, self.lam = min(layers_per_chunk, L), depth, causal, lam
         self.dev = torch.device(device)
+        self.dtype = "bf16" if dtype in ("bf16", 1) else "f16"
         self._pol_args = (budget, n_sink, tuple(ranges), allow_int4)
         self.policy = make_policy(*self._pol_args)
         # chunks: full chunks of Lc layers and (if L % Lc) one ragged tail chunk
         self.chunks = [(l0, min(self.Lc, L - l0)) for l0 in range(0, L, self.Lc)]
         self._plans = {}
         bb_max = self._plan(n, self.Lc)[2]
-        dv, f16, u8 = self.dev, torch.float16, torch.uint8
+        dv, f16, u8 = self.dev, (torch.bfloat16 if self.dtype == "bf16" else torch.float16), torch.uint8
         mk = lambda numel, dt: [torch.empty((numel,), dtype=dt, device=dv) for _ in range(depth)]
         kv = self.Lc * n * Hkv * d
         self.dK, self.dV, self.dKo, self.dVo = mk(kv, f16), mk(kv, f16), mk(kv, f16), mk(kv, f16)
@@ -55,7 +57,7 @@ class LayerPipelinedTransfer:
         key = (n, lc)
         if key not in self._plans:
             assert self.w <= n <= self.n
-            s = make_shape(lc, self.Hq, self.Hkv, self.d, n, 1)
+            s = make_shape(lc, self.Hq, self.Hkv, self.d, n, 1, dtype=self.dtype)
             c = skv_tier_counts(s, self.policy)
             self._plans[key] = (s, c, skv_blob_bytes(s, c))
         return self._plans[key]

@@ -646,3 +646,22 @@ def test_bfloat16_vanishing_amax_gets_zero_codes():
     skv.skv_unpack(shape, blob, bb, c, Ko, Vo, None, ws)
     K2, V2, _ = oracle.unpack(blob_or, L, Hkv, d, n, bf16=True)
     assert np.array_equal(_bits(Ko[0]), K2) and np.array_equal(_bits(Vo[0]), V2)
+
+
+def test_layer_pipelined_transfer_bfloat16():
+    """The pipelined host round trip with bfloat16 caches: per-layer results equal the oracle's on the GPU's scores."""
+    from paper_2606_08635_b200.transfer import LayerPipelinedTransfer
+    cfg = C["C5"].scaled(L=3, n=777, R=1)
+    K, V, Q = _bf16_case(cfg, 0.4)
+    nan = lambda t: torch.full(t.shape, float("nan"), dtype=torch.bfloat16, pin_memory=True)
+    req = dict(K=K.pin_memory(), V=V.pin_memory(), Q=Q.pin_memory(), Ko=nan(K), Vo=nan(V),
+               I=torch.empty((3, cfg.n), dtype=torch.float32, pin_memory=True),
+               T=torch.empty((3, cfg.n), dtype=torch.uint8, pin_memory=True))
+    pipe = LayerPipelinedTransfer(3, cfg.Hq, cfg.Hkv, cfg.d, cfg.n, cfg.w, 0.4, cfg.n_sink, (), True, layers_per_chunk=2,
+                                  depth=2, dtype="bf16")
+    pipe.run_ragged([req])
+    counts, prot = oracle.tier_counts(cfg.n, 0.4, cfg.n_sink, (), True)
+    tier = oracle.assign(req["I"].numpy(), prot, counts)
+    assert np.array_equal(tier, req["T"].numpy())
+    K2, V2, _ = oracle.unpack(oracle.pack(_bits(K), _bits(V), tier, counts, True, bf16=True), 3, cfg.Hkv, cfg.d, cfg.n, bf16=True)
+    assert np.array_equal(_bits(req["Ko"]), K2) and np.array_equal(_bits(req["Vo"]), V2)
