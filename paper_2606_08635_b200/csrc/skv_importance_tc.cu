@@ -532,13 +532,19 @@ static TcPlan tc_plan(const Geom &g, int w)
     t.qrows = ((std::min(t.MB, M) + 63) / 64) * 64;
     t.halves = t.qrows > 128 ? 2 : 1;
     const long long triples = (long long)g.R * g.L * g.Hkv * t.RB;
-    long long want = (8LL * 148 + triples - 1) / triples;
-    if (want < 1) want = 1;
-    int ck = (int)((g.n + want - 1) / want);
-    ck = ((ck + 127) / 128) * 128;
-    if (ck < 1024) ck = 1024;
+    // Key chunk per work item: items are dealt round-robin to one persistent CTA per SM, so the cost of a candidate
+    // chunk size is (rounds of items) x (tiles per item + ~3 tiles of per-item overhead: Q load, pipeline fill and
+    // drain).  Candidates are multiples of 128 keys from 512 up; ties go to the larger chunk (fewer partials).
     const int npad = ((g.n + 127) / 128) * 128;
-    if (ck > npad) ck = npad;
+    constexpr long long kSMs = 148;                     // B200; also used by the host-only workspace query
+    int ck = npad;
+    long long best = -1;
+    for (int c = std::min(512, npad); c <= npad; c += 128) {
+        const long long chunks = (g.n + c - 1) / c;
+        const long long rounds = (triples * chunks + kSMs - 1) / kSMs;
+        const long long cost = rounds * (c / 128 + 3);
+        if (best < 0 || cost <= best) { best = cost; ck = c; }
+    }
     t.chunk_keys = ck;
     t.n_chunks = (g.n + ck - 1) / ck;
     t.pchunks = t.n_chunks * (t.halves == 1 ? 4 : 2);
