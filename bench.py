@@ -593,7 +593,7 @@ def main():
         "importance": {"ms": ms_imp, "useful_tflops": 2.0 * cfg.L * cfg.Hq * cfg.w * cfg.n * cfg.d * R / (ms_imp * 1e-3) / 1e12,
                        "executed_tflops": 4.0 * cfg.L * cfg.Hq * cfg.w * cfg.n * cfg.d * R / (ms_imp * 1e-3) / 1e12,
                        "note": "two-pass: the contraction and the exponentials run twice; bound by the MUFU ex2 / FMA / "
-                               "tensor pipe mix at d_h = 128 (profiles/r1_full_v3_ncu.md), not by the tensor pipe alone",
+                               "tensor pipe mix at d_h = 128 (profiles/r1_full_v4_ncu.md), not by the tensor pipe alone",
                        "tensor_peak_tflops": measured_tensor_peak()[0], "tensor_peak_source": measured_tensor_peak()[1],
                        "useful_frac_of_tensor_peak": 2.0 * cfg.L * cfg.Hq * cfg.w * cfg.n * cfg.d * R / (ms_imp * 1e-3) / 1e12 / measured_tensor_peak()[0],
                        "executed_frac_of_tensor_peak": 4.0 * cfg.L * cfg.Hq * cfg.w * cfg.n * cfg.d * R / (ms_imp * 1e-3) / 1e12 / measured_tensor_peak()[0]},
