@@ -348,7 +348,7 @@ static cudaError_t launch_pack_fast(const Geom &g, const Layout &lo, const __hal
                                     const uint4 *tile_base, cudaStream_t s)
 {
     dim3 grid(g.tiles, g.L, g.R);
-    if (g.low_code == 2) pack_fast_kernel<D, NCH, 2, true, E><<<grid, 256, 0, s>>>(g, lo, K, V, tier_map, blob, blob_stride, tile_base);
+    if (g.low_code == 2) pack_fast_kernel<D, NCH, 3, true, E><<<grid, 256, 0, s>>>(g, lo, K, V, tier_map, blob, blob_stride, tile_base);
     else pack_fast_kernel<D, NCH, 3, false, E><<<grid, 256, 0, s>>>(g, lo, K, V, tier_map, blob, blob_stride, tile_base);
     return cudaGetLastError();
 }
