@@ -171,7 +171,8 @@ int skv_pack(const skv_shape *shape, const void *K_dev, const void *V_dev, const
              void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
 
 /* DEVICE.  blob_dev holds n_requests blobs of blob_bytes each (as validated by skv_blob_check on the
- * host copy).  `shape` gives dims and OUTPUT strides.  Writes every element of K_out/V_out (dropped
+ * host copy).  `shape` gives dims, OUTPUT strides and the element type, which must be the one the header declares
+ * (skv_blob_check reports it in shape_out->dtype).  Writes every element of K_out/V_out (dropped
  * tokens -> +0.0) and, if tier_map_out_dev != NULL, the tier map u8 [R][L][n] (the validity mask). */
 int skv_unpack(const skv_shape *shape, const void *blob_dev, size_t blob_bytes, const skv_counts *counts,
                void *K_out_dev, void *V_out_dev, uint8_t *tier_map_out_dev,
