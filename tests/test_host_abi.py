@@ -91,6 +91,25 @@ def test_argument_errors():
     rc = L.skv_importance(C.byref(shape3), 256, 256, 8, 1, 0.0, 256, 256, 1 << 30, None)
     assert rc == skv.SKV_ERR_INVALID_ARG            # Hq % Hkv != 0
     assert skv.skv_strerror(skv.SKV_ERR_BAD_BLOB).startswith("malformed")
+    # the NEXT-row entry points validate the same way
+    rc = L.skv_unpack_patch(C.byref(shape), 0, 0, C.byref(c), 0, 0, None, 0, 0, None)
+    assert rc == skv.SKV_ERR_INVALID_ARG
+    rc = L.skv_unpack_patch(C.byref(shape), 256, 12345, C.byref(c), 256, 256, None, 256, 1 << 30, None)
+    assert rc == skv.SKV_ERR_BAD_BLOB               # blob_bytes disagrees with the layout of `counts`
+    shape_dt = skv.make_shape(2, 4, 2, 128, 100)
+    shape_dt.dtype = 7
+    rc = L.skv_pack(C.byref(shape_dt), 256, 256, 256, C.byref(c), 256, 1 << 30, 256, 1 << 30, None)
+    assert rc == skv.SKV_ERR_INVALID_ARG            # unknown element type
+    with pytest.raises(skv.SkvError):               # populations exceed n
+        skv.skv_counts_from_populations(shape, 60, 50, 0)
+    with pytest.raises(skv.SkvError):               # low tier populated but not allowed
+        skv.skv_counts_from_populations(shape, 1, 1, 5, allow_int4=False)
+    cp = skv.skv_counts_from_populations(shape, 10, 20, 30, allow_int4=2)
+    assert cp.as_tuple() == (10, 20, 30, 40) and cp.allow_int4 == 2 and cp.spent_q4 == 8 * 10 + 4 * 20 + 30
+    rc = L.skv_assign_tiers_counts(C.byref(shape), C.byref(cp), 11, 0, None, 256, 256, 0, 0, None)
+    assert rc == skv.SKV_ERR_BUDGET_INFEASIBLE      # 11 protected positions but only 10 FP16 slots
+    rc = L.skv_assign_tiers_counts(C.byref(shape), C.byref(cp), 2, 0, None, 0, 256, 0, 0, None)
+    assert rc == skv.SKV_ERR_INVALID_ARG            # null importance
 
 
 def test_blob_check_accepts_oracle_blob_and_rejects_corruption():
