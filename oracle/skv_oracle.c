@@ -28,10 +28,18 @@
  *   quantizer               : worked examples W1..W5 (hand-computed), error bound <= scale/2
  *   wire format             : W6 layout, hand-written blob, Eq. 1 byte identity
  *   pack/unpack             : b=1 identity round trip
+ *   quantizer rounding (P8) : cases that separate the single rounding of the exact product from the
+ *                             two-step rounding, re-derived with exact rational arithmetic
+ *   upgrade (NEXT-3)        : upgraded rows equal the original rows, everything else untouched, identity
+ *                             after upgrading every token
+ *   2-bit tier (NEXT-4)     : hand-worked examples Z1..Z3, exact-rational codes, half-a-step error bound,
+ *                             hand-written blob bytes; count ladder: closed-form identities only
+ *   bfloat16 (NEXT-4)       : conversions exhaustively against torch; quantizer identities and bounds
  * PARITY UNPINNED (conventions of this build with no external fixture):
  *   group size = one head vector, fp16 amax scale record, reciprocal multiply,
  *   nibble order, segment order/alignment, tie direction, causal default,
- *   mean normalisation, per-layer map.
+ *   mean normalisation, per-layer map; the KV-norm score's choice of norm (P15); the fractions of the
+ *   eighth-unit ladder of the 2-bit tier (P18: the paper prints none); the bf16 overflow rule (P20).
  */
 #include <math.h>
 #include <stdint.h>
