@@ -35,10 +35,13 @@
  *   2-bit tier (NEXT-4)     : hand-worked examples Z1..Z3, exact-rational codes, half-a-step error bound,
  *                             hand-written blob bytes; count ladder: closed-form identities only
  *   bfloat16 (NEXT-4)       : conversions exhaustively against torch; quantizer identities and bounds
+ *   KV-norm score (NEXT-1)  : hand-worked Pythagorean key vectors with integer norms and scores for lambda = 0, ln 2,
+ *                             0.005 (tests/golden/kvnorm_worked.txt); scaling, permutation, zero-layer and decay properties
  * PARITY UNPINNED (conventions of this build with no external fixture):
  *   group size = one head vector, fp16 amax scale record, reciprocal multiply,
  *   nibble order, segment order/alignment, tie direction, causal default,
- *   mean normalisation, per-layer map; the KV-norm score's choice of norm (P15); the fractions of the
+ *   mean normalisation, per-layer map; the KV-norm score's choice of the L2 norm (P15: a reading; its arithmetic is
+ *   pinned above); the fractions of the
  *   eighth-unit ladder of the 2-bit tier (P18: the paper prints none); the bf16 overflow rule (P20).
  */
 #include <math.h>
@@ -648,7 +651,8 @@ int orc_unpack_patch(const uint8_t *blob, uint64_t blob_bytes, int32_t L, int32_
 /* ------------------------------------------------------------------------ */
 /* NEXT-1: KV-norm fallback score ("or a KV-norm          */
 /* fallback").  Reading P15: A_j = mean over KV heads of the L2 norm of the  */
-/* key vector, normalised to sum 1 over j; then the same decay.  UNPINNED.   */
+/* key vector, normalised to sum 1 over j; then the same decay.  Pinned by   */
+/* tests/golden/kvnorm_worked.txt (the choice of the L2 norm is the reading). */
 /* ------------------------------------------------------------------------ */
 void orc_importance_kvnorm_dt(int32_t L, int32_t Hkv, int32_t d, int64_t n, double lambda,
                               const uint16_t *K, float *I, int32_t dtype)

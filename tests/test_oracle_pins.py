@@ -3,6 +3,7 @@
 None of these tests touches the CUDA path.  Each pin is chosen so that a plausible mistake in the
 oracle (dropped term, wrong sign/index, transposed operand, wrong rounding) fails it.
 """
+import math
 import os
 
 import numpy as np
@@ -566,12 +567,58 @@ def test_importance_matches_textbook_softmax(causal):
     assert np.allclose(I, A.numpy(), rtol=1e-6, atol=1e-12)
 
 
-def test_kvnorm_fallback_shape_and_normalisation():
-    K, _ = _rand_qk(2, 2, 2, 64, 33, 3, 14)
-    I = oracle.importance_kvnorm(K)
-    assert np.allclose(I.astype(np.float64).sum(axis=1), 1.0, atol=1e-6)
-    nrm = np.linalg.norm(K.astype(np.float64), axis=-1).mean(axis=-1)
-    assert np.allclose(I, nrm / nrm.sum(axis=1, keepdims=True), rtol=1e-6)
+def _kvnorm_golden(golden_dir):
+    rows = read_golden(os.path.join(golden_dir, "kvnorm_worked.txt"))
+    keys = [r for r in rows if r[0] == "key"]
+    n, Hkv, d = 1 + max(int(r[1]) for r in keys), 1 + max(int(r[2]) for r in keys), 4
+    K = np.zeros((1, n, Hkv, d), np.float16)
+    norms = np.zeros((n, Hkv))
+    for r in keys:
+        K[0, int(r[1]), int(r[2])] = [float(x) for x in r[3:7]]
+        norms[int(r[1]), int(r[2])] = float(r[7])
+    scores = {}
+    for r in rows:
+        if r[0] == "score":
+            scores.setdefault(r[1], {})[int(r[2])] = float(r[3])
+    return K, norms, scores
+
+
+def test_kvnorm_hand_worked_example(golden_dir):
+    """tests/golden/kvnorm_worked.txt: Pythagorean key vectors whose norms are integers, scores worked by hand for
+    lambda = 0, ln 2 (decay factors 1/8, 1/4, 1/2, 1) and 0.005 (Eq. 13)."""
+    K, norms, scores = _kvnorm_golden(golden_dir)
+    # the fixture's own norms are integers a reader can check: sum of squares of each row
+    assert np.array_equal((K.astype(np.float64) ** 2).sum(axis=-1)[0], norms ** 2)
+    for name, lam in (("0", 0.0), ("ln2", math.log(2.0)), ("0.005", 0.005)):
+        I = oracle.importance_kvnorm(K, lam=lam)[0].astype(np.float64)
+        want = np.array([scores[name][j] for j in range(K.shape[1])])
+        assert np.all(np.abs(I - want) <= 1e-7 * want), (name, I, want)          # float32 output: half an ulp = 6e-8
+        assert I[1] == 0.0                                                       # the zero token
+
+
+def test_kvnorm_scaling_permutation_and_normalisation_properties():
+    """Properties the definition fixes (no formula retyped): scaling one token's keys by c scales its UNNORMALISED
+    score by c (so every ratio to another token's score scales by c); permuting the KV heads or the elements inside a
+    head vector changes nothing; an all-zero layer falls back to the uniform 1/n; scores sum to 1 at lambda = 0."""
+    rng = np.random.default_rng(14)
+    L, n, Hkv, d = 2, 33, 3, 64
+    K = rng.standard_normal((L, n, Hkv, d)).astype(np.float16)
+    I0 = oracle.importance_kvnorm(K).astype(np.float64)
+    assert np.allclose(I0.sum(axis=1), 1.0, atol=1e-6)
+    t, c = 7, 4.0                                                                # power of two: exact in fp16
+    K2 = K.copy(); K2[:, t] *= np.float16(c)
+    I2 = oracle.importance_kvnorm(K2).astype(np.float64)
+    others = np.array([j for j in range(n) if j != t])
+    assert np.allclose(I2[:, t:t + 1] / I2[:, others], c * I0[:, t:t + 1] / I0[:, others], rtol=1e-5)
+    assert np.allclose(I2[:, others] / I2[:, others[:1]], I0[:, others] / I0[:, others[:1]], rtol=1e-5)
+    Kp = K[:, :, ::-1, :][:, :, :, rng.permutation(d)].copy()
+    assert np.allclose(oracle.importance_kvnorm(Kp), I0, rtol=2e-6)
+    Z = np.zeros((1, 5, 2, 64), np.float16)
+    assert np.allclose(oracle.importance_kvnorm(Z), 0.2, rtol=1e-7)
+    # decay closed form on top of any scores: I_j(lambda) / I_j(0) = exp(-lambda (n-1-j))
+    lam = 0.01
+    Il = oracle.importance_kvnorm(K, lam=lam).astype(np.float64)
+    assert np.allclose(Il / I0, np.exp(-lam * (n - 1 - np.arange(n)))[None, :], rtol=1e-6)
 
 
 # ----------------------------------------------------------------------------------------------
