@@ -25,7 +25,9 @@
  *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  All work is
  *     enqueued on that stream; no entry point synchronises the host.
  *   - Every entry returns SKV_OK (0) or a negative skv_status and launches nothing on error.
- *   - The library keeps no global state and is re-entrant.
+ *   - The library keeps no mutable global state and is re-entrant.  (Two process-wide constants are set idempotently:
+ *     the driver entry point of the tensor-map encoder is looked up once and cached, and kernels that need more than
+ *     48 KiB of dynamic shared memory always request the same fixed maximum.)
  *   - fp16 = IEEE binary16.  K/V inputs must be finite (NaN/Inf is undefined behaviour).
  *   - With skv_shape.dtype = SKV_BF16 every "fp16" below reads bfloat16 (caches, queries, amax / (lo, hi) records,
  *     dequantised output); the byte model is unchanged (2 bytes per element).  Only difference in the arithmetic: a
@@ -76,10 +78,15 @@ extern "C" {
 typedef enum {
     SKV_OK = 0,
     SKV_ERR_INVALID_ARG = -1,       /* null pointer, dims <= 0, Hq % Hkv != 0, window outside [1,n], b <= 0 or NaN,
-                                       range outside [0,n] or begin > end */
+                                       range outside [0,n] or begin > end; counts that do not add up to n, carry a
+                                       low tier without the allow_int4 flag, or spend more than their budget (such a
+                                       blob would fail skv_blob_check); an OUTPUT cache whose layer / request stride
+                                       is 0 with more than one layer / request (overlapping writes) */
     SKV_ERR_UNSUPPORTED = -2,       /* head_dim not in {64,128,256}; stride_token/stride_head/stride_layer/
-                                       stride_request not multiples of 8 elements; pointer not 16-B aligned;
-                                       n_tokens > 2^24 */
+                                       stride_request not multiples of 8 elements; pointer not 16-B aligned (blob:
+                                       256-B); n_tokens > 2^20 (the slot scan packs three 21-bit counters in a word);
+                                       n_layers * n_requests > 65535 (grid dimension of the per-layer kernels);
+                                       more than 32 disjoint protected intervals after merging sinks and ranges */
     SKV_ERR_BUDGET_INFEASIBLE = -3, /* protected tokens alone exceed the budget (4P > floor(4bn)) */
     SKV_ERR_BUFFER_TOO_SMALL = -4,  /* blob capacity or workspace */
     SKV_ERR_BAD_BLOB = -5,          /* skv_blob_check: magic / version / dims / offsets / total_bytes mismatch */
@@ -126,7 +133,8 @@ int skv_tier_counts(const skv_shape *shape, const skv_policy *policy, skv_counts
 size_t skv_blob_bytes(const skv_shape *shape, const skv_counts *counts);
 
 /* HOST only.  Workspace (DEVICE bytes) sufficient for any entry point on this shape with the given
- * observation window (pass window = 0 if skv_importance is not used). */
+ * observation window (pass window = 0 if skv_importance is not used).  0 on invalid arguments (dims <= 0; with
+ * window > 0 also Hq % Hkv != 0 or window > n) and on shapes skv_importance reports as unsupported. */
 size_t skv_workspace_bytes(const skv_shape *shape, int32_t window);
 
 /* HOST only.  Validates the first 256 bytes of a received blob (HOST memory) against blob_bytes and

@@ -165,7 +165,9 @@ cudaError_t launch_assign(const Geom &g, const Intervals &prot, const float *imp
     const int in_smem = need <= 200 * 1024;
     const size_t dyn = in_smem ? need : 0;
     if (dyn > 48 * 1024) {
-        cudaError_t e = cudaFuncSetAttribute(assign_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
+        // the attribute is per function and process-wide: always request the SAME maximum, so that concurrent callers
+        // with different n cannot lower each other's limit between the attribute call and the launch
+        cudaError_t e = cudaFuncSetAttribute(assign_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
         if (e != cudaSuccess) return e;
     }
     dim3 grid(g.L, g.R);

@@ -48,12 +48,16 @@ static int check_dims_supported(const skv_shape *s)
     return SKV_OK;
 }
 
-static int check_cache(const skv_shape *s, const void *K, const void *V)
+// is_output: the cache is written (skv_unpack / skv_unpack_patch), so a zero layer / request stride with more than one
+// layer / request would make the writes overlap; for inputs a zero stride is a harmless broadcast.
+static int check_cache(const skv_shape *s, const void *K, const void *V, bool is_output = false)
 {
     int rc = check_dims_supported(s);
     if (rc) return rc;
     if (!K || !V) return SKV_ERR_INVALID_ARG;
     if (s->stride_head <= 0 || s->stride_token <= 0 || s->stride_layer < 0 || s->stride_request < 0) return SKV_ERR_INVALID_ARG;
+    if (is_output && ((s->n_layers > 1 && s->stride_layer == 0) || (s->n_requests > 1 && s->stride_request == 0)))
+        return SKV_ERR_INVALID_ARG;
     if ((s->stride_head % 8) || (s->stride_token % 8) || (s->stride_layer % 8) || (s->stride_request % 8)) return SKV_ERR_UNSUPPORTED;
     if (((uintptr_t)K & 15) || ((uintptr_t)V & 15)) return SKV_ERR_UNSUPPORTED;
     return SKV_OK;
@@ -77,6 +81,16 @@ static bool counts_ok(const skv_shape *s, const skv_counts *c)
 {
     return c && c->n16 >= 0 && c->n8 >= 0 && c->n4 >= 0 && c->n0 >= 0 &&
            (int64_t)c->n16 + c->n8 + c->n4 + c->n0 == (int64_t)s->n_tokens;
+}
+
+// what skv_blob_check would refuse on the decode side: a low tier without the flag, or a budget the populations exceed
+static bool counts_wire_ok(const skv_shape *s, const skv_counts *c)
+{
+    if (!counts_ok(s, c) || c->allow_int4 < 0 || c->allow_int4 > 2 || c->reserved != 0) return false;
+    if (c->allow_int4 == 0 && c->n4 != 0) return false;
+    const int64_t unit = c->allow_int4 == 2 ? 8 : 4;
+    const int64_t spent = unit * c->n16 + (unit / 2) * c->n8 + c->n4;
+    return c->budget_q4 >= spent && c->budget_q4 <= unit * (int64_t)s->n_tokens;
 }
 
 static size_t scan_ws_bytes(const skv_shape *s)
@@ -181,7 +195,13 @@ size_t skv_workspace_bytes(const skv_shape *shape, int32_t window)
     size_t need = scan_ws_bytes(shape);
     need = std::max(need, (size_t)shape->n_requests * shape->n_layers * shape->n_tokens * sizeof(uint32_t));  // assign keys
     need = std::max(need, importance_ws_bytes(g, 0));
-    if (window > 0 && shape->n_q_heads > 0) need = std::max(need, importance_ws_bytes(g, window));
+    if (window > 0) {
+        // the importance plan divides by (Hq / Hkv) * window: refuse what skv_importance itself refuses
+        if (shape->n_q_heads <= 0 || shape->n_q_heads % shape->n_kv_heads || window > shape->n_tokens) return 0;
+        const size_t imp = importance_ws_bytes(g, window);
+        if (imp == 0) return 0;                                          // work decomposition does not fit 32-bit counters
+        need = std::max(need, imp);
+    }
     return (need + 255) & ~(size_t)255;
 }
 
@@ -233,7 +253,9 @@ int skv_importance(const skv_shape *shape, const void *K_dev, const void *Q_dev,
     if (!(lambda >= 0.0f)) return SKV_ERR_INVALID_ARG;
     if ((uintptr_t)Q_dev & 15) return SKV_ERR_UNSUPPORTED;
     const Geom g = make_geom(shape, nullptr);
-    if (ws_bytes < importance_ws_bytes(g, window)) return SKV_ERR_BUFFER_TOO_SMALL;
+    const size_t need = importance_ws_bytes(g, window);
+    if (need == 0) return SKV_ERR_UNSUPPORTED;                            // R*L*Hkv*key-chunk items overflow 32 bits
+    if (ws_bytes < need) return SKV_ERR_BUFFER_TOO_SMALL;
     cudaError_t e = launch_importance(g, (const __half *)K_dev, (const __half *)Q_dev, window, causal ? 1 : 0, lambda,
                                       importance_dev, ws, ws_bytes, (cudaStream_t)cuda_stream);
     return e == cudaSuccess ? SKV_OK : SKV_ERR_CUDA;
@@ -306,7 +328,7 @@ int skv_pack(const skv_shape *shape, const void *K_dev, const void *V_dev, const
 {
     int rc = check_cache(shape, K_dev, V_dev);
     if (rc) return rc;
-    if (!tier_map_dev || !blob_dev || !ws || !counts_ok(shape, counts)) return SKV_ERR_INVALID_ARG;
+    if (!tier_map_dev || !blob_dev || !ws || !counts_wire_ok(shape, counts)) return SKV_ERR_INVALID_ARG;
     if ((uintptr_t)blob_dev & 255) return SKV_ERR_UNSUPPORTED;
     const Geom g = make_geom(shape, counts);
     const Layout lo = make_layout(g.L, g.Hkv, g.D, g.n, g.n16, g.n8, g.n4, g.low_code);
@@ -337,9 +359,9 @@ static int unpack_impl(const skv_shape *shape, const void *blob_dev, size_t blob
                        void *K_out_dev, void *V_out_dev, uint8_t *tier_map_out_dev, void *ws, size_t ws_bytes,
                        void *cuda_stream, int patch)
 {
-    int rc = check_cache(shape, K_out_dev, V_out_dev);
+    int rc = check_cache(shape, K_out_dev, V_out_dev, true);
     if (rc) return rc;
-    if (!blob_dev || !ws || !counts_ok(shape, counts)) return SKV_ERR_INVALID_ARG;
+    if (!blob_dev || !ws || !counts_wire_ok(shape, counts)) return SKV_ERR_INVALID_ARG;
     if ((uintptr_t)blob_dev & 255) return SKV_ERR_UNSUPPORTED;
     Geom g = make_geom(shape, counts);
     g.patch = patch;

@@ -105,7 +105,8 @@ size_t importance_ws_bytes(const Geom &g, int window)
 {
     const size_t raw = (size_t)g.R * g.L * g.n * sizeof(float);                // kvnorm raw buffer
     if (window <= 0) return raw;
-    return std::max(raw, importance_tc_ws_bytes(g, window));
+    const size_t tc = importance_tc_ws_bytes(g, window);
+    return tc == 0 ? 0 : std::max(raw, tc);                             // 0: unsupported work decomposition
 }
 
 // There is one implementation (tcgen05 / TMEM / TMA); a driver that cannot encode the tensor maps is an error.

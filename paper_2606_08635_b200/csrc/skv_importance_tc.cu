@@ -549,7 +549,8 @@ static TcPlan tc_plan(const Geom &g, int w)
     t.n_chunks = (g.n + ck - 1) / ck;
     t.pchunks = t.n_chunks * (t.halves == 1 ? 4 : 2);
     t.S = g.Hkv * t.RB;
-    t.n_items = (int)(triples * t.n_chunks);
+    const long long items = triples * t.n_chunks;
+    t.n_items = items > 0x7FFFFFFFll ? -1 : (int)items;                 // -1: does not fit (reported as unsupported)
     const size_t rows = (size_t)g.R * g.L * g.Hq * w;
     t.partial_bytes = (rows * t.pchunks * sizeof(float2) + 255) & ~(size_t)255;
     t.lse_bytes = (rows * sizeof(float) + 255) & ~(size_t)255;
@@ -559,7 +560,9 @@ static TcPlan tc_plan(const Geom &g, int w)
 
 size_t importance_tc_ws_bytes(const Geom &g, int window)
 {
+    if (g.Hkv <= 0 || g.Hq < g.Hkv || g.Hq % g.Hkv || window <= 0) return 0;
     const TcPlan t = tc_plan(g, window);
+    if (t.n_items < 0) return 0;
     return t.partial_bytes + t.lse_bytes + t.apart_bytes;
 }
 

@@ -169,68 +169,82 @@ def test_foreign_tier_map_with_wrong_counts_is_memory_safe():
 
 
 @pytest.mark.slow
-def test_full_size_bench_config_sampled():
-    """BASELINE config C5 at full size (n = 32768, 32 layers, 8 KV heads), in the launch configuration
-    bench.py times (4 requests, token-major, b = 0.5): the oracle checks sampled layers of sampled requests
-    element by element; every other layer is checked through properties that hold at any size."""
+def test_full_size_c5_every_layer_every_request_every_budget():
+    """BASELINE config C5 at FULL size (n = 32768, 32 layers, 8 KV heads, 4 requests, token-major), in the launch
+    configuration bench.py times (one launch per stage for the whole batch), over the whole budget sweep
+    b in {0.3, 0.4, 0.5, 0.75, 1.0}.  GPU importance runs once (it does not depend on b).  Then, per budget and per
+    request, against the oracle on the SAME importance scores: the tier map of all 32 layers (oracle.assign), EVERY byte
+    of the request's blob (oracle.pack) and EVERY dequantised fp16 element of K and V (oracle.unpack).  The float64
+    oracle importance is compared on two layers per request (1e-3 relative, P13), and on those layers the end-to-end
+    tier maps (oracle scores -> oracle map vs GPU scores -> GPU map) agree on >= 99.9 % of the tokens that are not
+    near-ties (P14).  Requests are compared one at a time to bound host memory ("hard parts")."""
     cfg = C["C5"]
     dev = torch.device("cuda:0")
-    R, L = cfg.R, cfg.L
-    Kd = torch.empty((R, L, cfg.n, cfg.Hkv, cfg.d), dtype=torch.float16, device=dev)
+    R, L, n = cfg.R, cfg.L, cfg.n
+    Kd = torch.empty((R, L, n, cfg.Hkv, cfg.d), dtype=torch.float16, device=dev)
     Vd = torch.empty_like(Kd)
     Qd = torch.empty((R, L, cfg.Hq, cfg.w, cfg.d), dtype=torch.float16, device=dev)
     for r in range(R):
         Kd[r], Vd[r] = skv_synth.make_kv(cfg, r, device=dev)
         Qd[r] = skv_synth.make_q(cfg, r, device=dev)
-    shape = skv.make_shape(L, cfg.Hq, cfg.Hkv, cfg.d, cfg.n, R)
-    pol = skv.make_policy(0.5, cfg.n_sink, cfg.ranges, cfg.allow_int4)
+    shape = skv.make_shape(L, cfg.Hq, cfg.Hkv, cfg.d, n, R)
     ws = torch.empty(skv.skv_workspace_bytes(shape, cfg.w), dtype=torch.uint8, device=dev)
-    I = torch.empty((R, L, cfg.n), dtype=torch.float32, device=dev)
-    tier = torch.empty((R, L, cfg.n), dtype=torch.uint8, device=dev)
+    I = torch.full((R, L, n), float("nan"), dtype=torch.float32, device=dev)
     skv.skv_importance(shape, Kd, Qd, cfg.w, I, ws)
-    counts = skv.skv_assign_tiers(shape, pol, I, tier, ws)
-    bb = skv.skv_blob_bytes(shape, counts)
-    blob = torch.empty((R, bb), dtype=torch.uint8, device=dev)
-    skv.skv_pack(shape, Kd, Vd, tier, counts, blob, ws)
-    Ko = torch.empty_like(Kd); Vo = torch.empty_like(Vd); to = torch.empty_like(tier)
-    skv.skv_unpack(shape, blob, bb, counts, Ko, Vo, to, ws)
     torch.cuda.synchronize()
+    Ih = I.cpu().numpy()
+    assert np.isfinite(Ih).all() and np.allclose(Ih.astype(np.float64).sum(axis=2), 1.0, atol=1e-4)
 
-    oc, prot = oracle.tier_counts(cfg.n, 0.5, cfg.n_sink, cfg.ranges, cfg.allow_int4)
-    assert counts.as_tuple() == (oc.n16, oc.n8, oc.n4, oc.n0) and bb == oracle.blob_bytes(L, cfg.Hkv, cfg.d, cfg.n, oc)
-    # properties at full size: populations per layer, sinks FP16, importance sums to 1, FP16 rows identical,
-    # error bound on every quantised element
-    th = tier.cpu().numpy()
-    for t, want in ((16, oc.n16), (8, oc.n8), (4, oc.n4), (0, oc.n0)):
-        assert ((th == t).sum(axis=2) == want).all()
-    assert (th[:, :, :cfg.n_sink] == 16).all() and torch.equal(to, tier)
-    assert torch.allclose(I.double().sum(dim=2), torch.ones(R, L, dtype=torch.float64, device=dev), atol=1e-4)
-    m16 = (tier == 16)
-    assert torch.equal(Ko[m16], Kd[m16]) and torch.equal(Vo[m16], Vd[m16])
-    for X, Xo in ((Kd, Ko), (Vd, Vo)):
+    # float64 oracle importance on two layers per request (the oracle parallelises over layers)
+    sampled = {0: (0, 31), 1: (17, 5), 2: (9, 26), 3: (31, 12)}
+    I_or = {}
+    for r, layers in sampled.items():
+        Kh = torch.stack([Kd[r, l] for l in layers]).cpu().numpy()
+        Qh = torch.stack([Qd[r, l] for l in layers]).cpu().numpy()
+        Io = oracle.importance(Kh, Qh).astype(np.float64)
+        for i, l in enumerate(layers):
+            got = Ih[r, l].astype(np.float64)
+            assert np.all(np.abs(got - Io[i]) <= 1e-3 * Io[i] + 1e-30), (r, l, np.max(np.abs(got - Io[i]) / (Io[i] + 1e-30)))
+            I_or[(r, l)] = Io[i].astype(np.float32)
+
+    tier = torch.empty((R, L, n), dtype=torch.uint8, device=dev)
+    Ko = torch.empty_like(Kd); Vo = torch.empty_like(Vd); to = torch.empty_like(tier)
+    for b in cfg.budgets:
+        pol = skv.make_policy(b, cfg.n_sink, cfg.ranges, cfg.allow_int4)
+        tier.fill_(0xEE); Ko.fill_(float("nan")); Vo.fill_(float("nan")); to.fill_(0xEE)
+        counts = skv.skv_assign_tiers(shape, pol, I, tier, ws)
+        bb = skv.skv_blob_bytes(shape, counts)
+        blob = torch.full((R, bb), 0xAB, dtype=torch.uint8, device=dev)               # poisoned: every byte must be written
+        skv.skv_pack(shape, Kd, Vd, tier, counts, blob, ws)
+        skv.skv_unpack(shape, blob, bb, counts, Ko, Vo, to, ws)
+        torch.cuda.synchronize()
+        oc, prot = oracle.tier_counts(n, b, cfg.n_sink, cfg.ranges, cfg.allow_int4)
+        assert counts.as_tuple() == (oc.n16, oc.n8, oc.n4, oc.n0) and bb == oracle.blob_bytes(L, cfg.Hkv, cfg.d, n, oc)
+        assert torch.equal(to, tier)
         for r in range(R):
-            amax = X[r].float().abs().amax(dim=-1, keepdim=True)
-            qmax = torch.where(tier[r] == 8, 127.0, 7.0)[..., None, None]
-            bound = amax / qmax * 0.5 * (1 + 1e-4) + Xo[r].float().abs() * 2.0 ** -11 + 1e-12
-            ok = ((Xo[r].float() - X[r].float()).abs() <= bound) | (tier[r] == 16)[..., None, None]
-            assert bool(ok.all())
-    # sampled element-by-element parity against the oracle: (request, layer) pairs
-    for (r, l) in ((0, 0), (3, 31), (1, 17)):
-        Kh, Vh, Qh = Kd[r, l:l + 1].cpu().numpy(), Vd[r, l:l + 1].cpu().numpy(), Qd[r, l:l + 1].cpu().numpy()
-        Ih = I[r, l:l + 1].cpu().numpy()
-        t_or = oracle.assign(Ih, prot, oc)
-        assert np.array_equal(t_or, th[r, l:l + 1])                      # selection, identical importance
-        blob_or = oracle.pack(Kh, Vh, t_or, oc, cfg.allow_int4)          # a 1-layer blob: compare the layer block
-        lay0 = 256 + (cfg.n + 255) // 256 * 256
-        stride = (bb - (256 + (L * cfg.n + 255) // 256 * 256)) // L
-        off = 256 + (L * cfg.n + 255) // 256 * 256 + l * stride
-        assert np.array_equal(blob[r, off:off + stride].cpu().numpy(), blob_or[lay0:lay0 + stride])
-        K2, V2, _ = oracle.unpack(blob_or, 1, cfg.Hkv, cfg.d, cfg.n)
-        assert np.array_equal(Ko[r, l].cpu().numpy().view(np.uint16), K2[0].view(np.uint16))
-        assert np.array_equal(Vo[r, l].cpu().numpy().view(np.uint16), V2[0].view(np.uint16))
-        if (r, l) == (0, 0):                                             # float64 importance of one full layer
-            I_or = oracle.importance(Kh, Qh).astype(np.float64)
-            assert np.all(np.abs(Ih.astype(np.float64) - I_or) <= 1e-3 * I_or + 1e-30)
+            t_or = oracle.assign(Ih[r], prot, oc)                                     # all 32 layers, identical importance
+            assert np.array_equal(t_or, tier[r].cpu().numpy()), (b, r)
+            Kh, Vh = Kd[r].cpu().numpy(), Vd[r].cpu().numpy()
+            blob_or = oracle.pack(Kh, Vh, t_or, oc, cfg.allow_int4)
+            got = blob[r].cpu().numpy()
+            if not np.array_equal(got, blob_or):
+                bad = np.flatnonzero(got != blob_or)
+                raise AssertionError(f"b={b} request {r}: blob differs at {bad.size} bytes, first offsets {bad[:8]}")
+            del got
+            K2, V2, _ = oracle.unpack(blob_or, L, cfg.Hkv, cfg.d, n)
+            del blob_or
+            assert np.array_equal(Ko[r].cpu().numpy().view(np.uint16), K2.view(np.uint16)), (b, r)
+            assert np.array_equal(Vo[r].cpu().numpy().view(np.uint16), V2.view(np.uint16)), (b, r)
+            if b == 1.0:                                                              # identity round trip
+                assert np.array_equal(K2.view(np.uint16), Kh.view(np.uint16)) and np.array_equal(V2.view(np.uint16), Vh.view(np.uint16))
+            del K2, V2, Kh, Vh
+            # end to end on the layers with a float64 score: agreement outside near-ties (P14)
+            for l in sampled[r]:
+                t_e2e = oracle.assign(I_or[(r, l)][None], prot, oc)
+                nt = ~near_tie_mask(I_or[(r, l)][None].astype(np.float64), t_e2e)
+                agree = (t_e2e == t_or[l:l + 1])[nt].mean() if nt.any() else 1.0
+                assert agree >= 0.999, (b, r, l, agree)
+        del blob
 
 
 @pytest.mark.parametrize("L,lpc", [(5, 2), (3, 4)])

@@ -149,3 +149,40 @@ def test_workspace_covers_every_entry_point():
         assert ws >= R * L_ * ((n + 31) // 32) * 16          # tile prefix table of pack / unpack
         assert ws >= R * L_ * n * 4                           # selection keys when they do not fit shared memory
         assert ws >= R * L_ * Hq * w * 4                      # per-row log-sum-exp of the importance pass
+
+
+def test_limits_documented_in_the_header_are_the_ones_enforced():
+    """include/skv.h lists: n_tokens <= 2^20, n_layers * n_requests <= 65535, counts that a receiver would refuse,
+    zero output strides; the workspace query returns 0 instead of dividing by zero."""
+    import ctypes as C
+    L = skv.lib()
+    hdr = open(os.path.join(ROOT, "include", "skv.h")).read()
+    assert "n_tokens > 2^20" in hdr and "n_tokens > 2^24" not in hdr and "65535" in hdr
+    c0 = skv.skv_counts()
+    big = skv.make_shape(1, 2, 2, 128, (1 << 20) + 1)
+    ok = skv.make_shape(1, 2, 2, 128, 1 << 20)
+    pol = skv.make_policy(0.5)
+    assert L.skv_assign_tiers(C.byref(big), C.byref(pol), 256, 256, C.byref(c0), 256, 1 << 40, None) == skv.SKV_ERR_UNSUPPORTED
+    assert L.skv_tier_counts(C.byref(ok), C.byref(pol), C.byref(c0)) == skv.SKV_OK
+    grid = skv.make_shape(256, 2, 2, 128, 64, 256)                       # L * R = 65536
+    assert L.skv_assign_tiers(C.byref(grid), C.byref(pol), 256, 256, C.byref(c0), 256, 1 << 40, None) == skv.SKV_ERR_UNSUPPORTED
+    # workspace query: Hq < Hkv or Hq % Hkv != 0 with a window used to divide by zero
+    assert skv.skv_workspace_bytes(skv.make_shape(2, 2, 4, 128, 100), 8) == 0
+    assert skv.skv_workspace_bytes(skv.make_shape(2, 6, 4, 128, 100), 8) == 0
+    assert skv.skv_workspace_bytes(skv.make_shape(2, 4, 4, 128, 100), 101) == 0
+    assert skv.skv_workspace_bytes(skv.make_shape(2, 2, 4, 128, 100), 0) > 0
+    # counts a receiver would refuse are refused by the sender
+    shape = skv.make_shape(2, 4, 2, 128, 100)
+    good = skv.skv_counts_from_populations(shape, 10, 20, 30)
+    for mutate in (lambda c: setattr(c, "allow_int4", 0),               # low tier populated without the flag
+                   lambda c: setattr(c, "budget_q4", c.spent_q4 - 1),    # over budget
+                   lambda c: setattr(c, "budget_q4", 4 * 100 + 1),       # budget above all-FP16
+                   lambda c: setattr(c, "n0", c.n0 + 1),                 # populations do not add up
+                   lambda c: setattr(c, "allow_int4", 3)):
+        c = skv.skv_counts_from_populations(shape, 10, 20, 30)
+        mutate(c)
+        assert L.skv_pack(C.byref(shape), 256, 256, 256, C.byref(c), 256, 1 << 30, 256, 1 << 30, None) == skv.SKV_ERR_INVALID_ARG
+        assert L.skv_unpack(C.byref(shape), 256, 1 << 20, C.byref(c), 256, 256, None, 256, 1 << 30, None) == skv.SKV_ERR_INVALID_ARG
+    # overlapping output rows: layer stride 0 with two layers
+    zs = skv.make_shape(2, 4, 2, 128, 100, strides=(0, 0, 256, 128))
+    assert L.skv_unpack(C.byref(zs), 256, skv.skv_blob_bytes(shape, good), C.byref(good), 256, 256, None, 256, 1 << 30, None) == skv.SKV_ERR_INVALID_ARG
