@@ -209,6 +209,7 @@ def test_full_size_c5_every_layer_every_request_every_budget():
 
     tier = torch.empty((R, L, n), dtype=torch.uint8, device=dev)
     Ko = torch.empty_like(Kd); Vo = torch.empty_like(Vd); to = torch.empty_like(tier)
+    host_kv = [(Kd[r].cpu().numpy(), Vd[r].cpu().numpy()) for r in range(R)]          # 16 GiB of host memory, read 5 times
     for b in cfg.budgets:
         pol = skv.make_policy(b, cfg.n_sink, cfg.ranges, cfg.allow_int4)
         tier.fill_(0xEE); Ko.fill_(float("nan")); Vo.fill_(float("nan")); to.fill_(0xEE)
@@ -224,7 +225,7 @@ def test_full_size_c5_every_layer_every_request_every_budget():
         for r in range(R):
             t_or = oracle.assign(Ih[r], prot, oc)                                     # all 32 layers, identical importance
             assert np.array_equal(t_or, tier[r].cpu().numpy()), (b, r)
-            Kh, Vh = Kd[r].cpu().numpy(), Vd[r].cpu().numpy()
+            Kh, Vh = host_kv[r]
             blob_or = oracle.pack(Kh, Vh, t_or, oc, cfg.allow_int4)
             got = blob[r].cpu().numpy()
             if not np.array_equal(got, blob_or):
@@ -237,7 +238,7 @@ def test_full_size_c5_every_layer_every_request_every_budget():
             assert np.array_equal(Vo[r].cpu().numpy().view(np.uint16), V2.view(np.uint16)), (b, r)
             if b == 1.0:                                                              # identity round trip
                 assert np.array_equal(K2.view(np.uint16), Kh.view(np.uint16)) and np.array_equal(V2.view(np.uint16), Vh.view(np.uint16))
-            del K2, V2, Kh, Vh
+            del K2, V2
             # end to end on the layers with a float64 score: agreement outside near-ties (P14)
             for l in sampled[r]:
                 t_e2e = oracle.assign(I_or[(r, l)][None], prot, oc)
