@@ -1,21 +1,29 @@
 // skv_importance_tc.cu -- importance scores on the 5th-generation tensor cores (tcgen05 + TMEM + TMA).
 //
-// Same mathematics as skv_importance.cu (Eq. 13; logits PAPER.md:109), re-designed for sm_100a:
+// Eq. 13 with the logits of PAPER.md:109, designed for sm_100a:
 //   * one persistent, warp-specialised CTA per SM: warp 0 = TMA producer, warp 1 = MMA issuer (one elected
 //     thread) and TMEM owner, warps 2..17 = sixteen epilogue warps (four per scheduler, so that the MUFU pipe,
-//     which bounds this kernel at d_h = 128, always has an eligible warp);
-//   * a quarter of the exponentials is evaluated on the FMA pipe (round-to-nearest range reduction + degree-4
-//     minimax polynomial, 2.7e-6 relative) instead of MUFU.EX2, which lifts the 16 ex2/clk/SM ceiling;
+//     which bounds the arithmetic at d_h = 128, always has an eligible warp);
+//   * a quarter of the exponentials is evaluated on the FMA pipe (round-to-nearest range reduction + minimax
+//     polynomial: degree 4, 2.7e-6 relative, in pass 2; degree 3, 7.5e-5, for the row normaliser of pass 1)
+//     instead of MUFU.EX2, which lifts the 16 ex2/clk/SM ceiling;
 //   * operands land in shared memory by TMA (cp.async.bulk.tensor, 128-byte swizzle, mbarrier complete_tx)
-//     straight from the strided K cache and the Q window; accumulators live in TMEM (2 stages x 256 columns);
+//     straight from the strided K cache and the Q window; accumulators live in TMEM (2 stages x 256 columns, or
+//     4 x 128 when a tile needs no more than 128 columns);
 //   * pass 1 (rowstats): D[query row][key] = Q_blk K_tile^T, queries are TMEM lanes, so each epilogue thread owns
-//     one query row and keeps its online (max, sum 2^x) entirely in registers -- no shuffles;
+//     one query row and keeps its (reference exponent, sum 2^x) entirely in registers -- no shuffles;
 //   * pass 2 (colsum):  D[key][query row] = K_tile Q_blk^T, keys are TMEM lanes, so each thread owns one key and
 //     sums p = 2^(s - lse2[row]) over its columns in registers -- no shuffles, no atomics; the four column groups
 //     of a tile are added through shared memory in a fixed order, the per-(KV head, row block) partial sums go to a
 //     workspace and a small finish kernel adds them in a fixed order (deterministic) and applies 1/(Hq w) and the
-//     recency decay.
-// A work item is (request, layer, KV head, row block, key chunk); items are dealt round-robin to the CTAs.
+//     recency decay;
+//   * the epilogue pulls TMEM in 16-column chunks with one chunk in flight (the load of chunk c+1 is issued before
+//     the exponentials of chunk c), so the TMEM latency hides behind arithmetic.
+// Work decomposition (both passes): the unit is one 128-key tile of one (request, layer, KV head, row block); the
+// R*L*S*T units, tile index fastest, are cut into gridDim.x equal contiguous ranges, one per CTA ("stream-K"), so
+// every SM gets the same number of tiles (+-1) whatever the shape.  A CTA walks its range as segments (one
+// (request, layer, KV head, row block) and a run of its tiles); a row of T tiles cut by CTA boundaries yields one
+// partial (m, z) per piece in pass 1 and disjoint key ranges in pass 2.
 #include <cuda.h>
 #include <string.h>
 
@@ -31,21 +39,21 @@ constexpr int kEpiWarps = 16;
 constexpr int kEpiThreads = kEpiWarps * 32;
 constexpr int kThreads = 64 + kEpiThreads;   // warps: 0 TMA, 1 MMA/TMEM, 2..17 epilogue
 constexpr int kTileKeys = 128;
+constexpr int kRing = 8;                     // pass 2: depth of the column-group reduction ring (> accumulator stages)
 constexpr float kNegBig = -1.0e30f;
 
 struct Params {
     Geom g;
     int w, causal;
-    int chunk_keys, n_chunks;           // key chunk per work item
-    int RB, MB, qrows;                  // row blocks per KV head, rows per block, TMA box rows (multiple of 32)
+    int RB, MB, qrows;                  // row blocks per KV head, rows per block, TMA box rows (multiple of 64)
     int halves;                         // pass 1: 128-row MMA halves per row block (1 or 2)
-    int n_items;
+    int S, T;                           // S = Hkv*RB (KV head, row block) pairs per layer; T = 128-key tiles per row
+    long long U;                        // work units = R*L*S*T
+    int pmax;                           // pass 1: partial slots per query row = max pieces of a row * column groups
     int kdim[4];                        // position of (head, token, layer, request) in the K tensor map (1..4)
-    float2 *partial;                    // [rows][pchunks]
-    int pchunks;                        // n_chunks * (column groups per row in pass 1: 4 / halves)
+    float2 *partial;                    // [R*L*Hq*w][pmax]
     const float *lse2;                  // [R][L][Hq*w]
-    float *apart;                       // [R][L][S][n], S = Hkv*RB
-    int S;
+    float *apart;                       // [R][L][S][n]
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -177,7 +185,23 @@ __device__ __forceinline__ constexpr bool pair_on_fma(int pi)
          : SKV_EX2_FMA_PAIRS == 3 ? ((pi & 7) == 1 || (pi & 7) == 4 || (pi & 7) == 6)
          :                          (pi & 1) == 1;
 }
-template <int PI> __device__ __forceinline__ float2 ex2_pair(float2 x) { return pair_on_fma(PI) ? ex2_fma2(x) : ex2_mufu2(x); }
+// pass 2 has its own share (SKV_EX2_FMA_PAIRS_P2 of 8 pairs)
+#ifndef SKV_EX2_FMA_PAIRS_P2
+#define SKV_EX2_FMA_PAIRS_P2 SKV_EX2_FMA_PAIRS
+#endif
+__device__ __forceinline__ constexpr bool pair_on_fma2(int pi)
+{
+    return SKV_EX2_FMA_PAIRS_P2 == 0 ? false
+         : SKV_EX2_FMA_PAIRS_P2 == 1 ? (pi & 7) == 3
+         : SKV_EX2_FMA_PAIRS_P2 == 2 ? (pi & 3) == 1
+         : SKV_EX2_FMA_PAIRS_P2 == 3 ? ((pi & 7) == 1 || (pi & 7) == 4 || (pi & 7) == 6)
+         :                             (pi & 1) == 1;
+}
+#ifndef SKV_P1_DEG
+#define SKV_P1_DEG 3
+#endif
+// degree-3 minimax polynomial for 2^f on [-0.5, 0.5] (relative error 7.5e-5)
+constexpr float kP3c0 = 0.9999280571937561f, kP3c1 = 0.6932609677314758f, kP3c2 = 0.2426111251115799f, kP3c3 = 0.0551716685295105f;
 // sum of 2^(v*sc + add) over a 16-wide group, two packed accumulators
 template <int N>
 __device__ __forceinline__ void exp_accumulate(const float (&v)[N], float2 sc2, const float2 (&add2)[N / 2], float2 &accA, float2 &accB)
@@ -206,29 +230,316 @@ template <int D> struct Cfg {
     static constexpr int K_KB_STRIDE = kTileKeys * 128;
     static constexpr int K_BYTES = KB * K_KB_STRIDE;
     static constexpr int STAGES = (D == 64) ? 6 : (D == 128) ? 4 : 2;
-    static constexpr int RED_BYTES = 4 * 3 * kTileKeys * 4;            // pass 2: ring of 4 x [column groups 1..3][128 keys]
+    static constexpr int RED_BYTES = kRing * 3 * kTileKeys * 4;        // pass 2: ring of [column groups 1..3][128 keys]
     static constexpr int SMEM = 1024 + Q_BYTES + STAGES * K_BYTES + 256 * 4 * 2 + RED_BYTES + 256;
 };
 
-struct Item { int r, l, g, rb, chunk, gb; };
+// One segment of a CTA's unit range: tiles [t0, t1) of one (request, layer, KV head, row block).
+struct Seg { int r, l, g, rb, gb, t0, t1, piece; };
 
-__device__ __forceinline__ Item decode_item(const Params &p, int item)
+// CTA that owns unit u when U units are cut into G equal contiguous ranges [c*U/G, (c+1)*U/G)
+__host__ __device__ __forceinline__ long long cta_of_unit(long long u, long long U, long long G) { return ((u + 1) * G - 1) / U; }
+
+__device__ __forceinline__ Seg seg_at(const Params &p, long long u, long long end)
 {
-    Item it;
-    it.chunk = item % p.n_chunks;
-    int t = item / p.n_chunks;
-    const int GB = p.g.Hkv * p.RB;
-    it.gb = t % GB; t /= GB;
-    it.l = t % p.g.L; it.r = t / p.g.L;
-    it.g = it.gb / p.RB; it.rb = it.gb % p.RB;
-    return it;
+    Seg s;
+    const long long row = u / p.T;
+    s.t0 = (int)(u - row * p.T);
+    const long long left = end - u;
+    s.t1 = (left < (long long)(p.T - s.t0)) ? s.t0 + (int)left : p.T;
+    int t = (int)row;
+    s.gb = t % p.S; t /= p.S;
+    s.l = t % p.g.L; s.r = t / p.g.L;
+    s.g = s.gb / p.RB; s.rb = s.gb % p.RB;
+    s.piece = (int)((long long)blockIdx.x - cta_of_unit(row * p.T, p.U, gridDim.x));
+    return s;
 }
 
-template <int D, int PASS>
+// ---- epilogue building blocks -------------------------------------------------------------------------------
+// TMEM leaves in 16-column chunks with ONE chunk in flight: the load of chunk c+1 is issued before the exponentials
+// of chunk c run, so its latency hides behind ~100 instructions of arithmetic, and an accumulator stage goes back to
+// the MMA warp as soon as its last chunk has landed in registers (not after the arithmetic on it).
+__device__ __forceinline__ void tmem_ld16_issue(uint32_t taddr, uint32_t (&r)[16])
+{
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+        "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+          "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+        : "r"(taddr) : "memory");
+}
+// wait for the outstanding TMEM loads; the chunk's registers are threaded through the statement so that no use of
+// them can be scheduled above the wait
+__device__ __forceinline__ void tmem_wait_ld(uint32_t (&r)[16])
+{
+    asm volatile("tcgen05.wait::ld.sync.aligned;"
+                 : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]), "+r"(r[4]), "+r"(r[5]), "+r"(r[6]), "+r"(r[7]),
+                   "+r"(r[8]), "+r"(r[9]), "+r"(r[10]), "+r"(r[11]), "+r"(r[12]), "+r"(r[13]), "+r"(r[14]), "+r"(r[15])
+                 :: "memory");
+}
+
+// One tile = NCH chunks; b0 holds (or is about to receive) chunk 0.  chunk(regs, c) consumes a chunk, and the next
+// tile's first chunk is requested while the last chunk of this one is being consumed.  The caller hands the stage
+// back (release_stage) once it no longer needs TMEM: the MMA warp is a whole tile ahead, so a late release costs nothing.
+template <int NCH, int ACOLS, class ChunkFn>
+__device__ __forceinline__ void stream_tile(uint32_t (&b0)[16], uint32_t (&b1)[16], uint32_t base, bool more, uint32_t tfull,
+                                            uint32_t &astage, uint32_t &aphase, ChunkFn &&chunk)
+{
+    const uint32_t tile_addr = base + astage * ACOLS;
+#pragma unroll
+    for (int c = 0; c < NCH; ++c) {
+        uint32_t (&cur)[16] = (c & 1) ? b1 : b0;
+        uint32_t (&nxt)[16] = (c & 1) ? b0 : b1;
+        tmem_wait_ld(cur);
+        if (c == NCH - 1) {
+            if (++astage == 512 / ACOLS) { astage = 0; aphase ^= 1; }
+            if (more) {
+                mbar_wait(tfull + 8 * astage, aphase);
+                tc_fence_after();
+                tmem_ld16_issue(base + astage * ACOLS, nxt);
+            }
+        } else {
+            tmem_ld16_issue(tile_addr + 16 * (c + 1), nxt);
+        }
+        chunk(cur, c);
+    }
+}
+__device__ __forceinline__ void release_stage(uint32_t tempty, uint32_t stage, int lane)
+{
+    tc_fence_before();
+    __syncwarp();
+    if (lane == 0) mbar_arrive(tempty + 8 * stage);
+}
+
+// 2^x for a pair on the FMA pipe when x <= ~0 is known or watched by the caller: lower clamp only.  DEG = 4: 2.7e-6
+// relative; DEG = 3: 7.5e-5 relative (enough for the row normaliser of pass 1, which a 1e-3 contract divides by).
+template <int DEG>
+__device__ __forceinline__ float2 ex2_fma2_lo(float2 x)
+{
+    x.x = fmaxf(x.x, -125.0f);
+    x.y = fmaxf(x.y, -125.0f);
+    const float2 t = __fadd2_rn(x, make_float2(12582912.0f, 12582912.0f));
+    const float2 nf = __fadd2_rn(t, make_float2(-12582912.0f, -12582912.0f));
+    const float2 f = __ffma2_rn(nf, make_float2(-1.0f, -1.0f), x);
+    float2 q;
+    if (DEG == 4) {
+        q = __ffma2_rn(f, make_float2(0.009570102207362652f, 0.009570102207362652f), make_float2(0.05591785907745361f, 0.05591785907745361f));
+        q = __ffma2_rn(q, f, make_float2(0.240247443318367f, 0.240247443318367f));
+        q = __ffma2_rn(q, f, make_float2(0.6931217908859253f, 0.6931217908859253f));
+        q = __ffma2_rn(q, f, make_float2(0.9999992847442627f, 0.9999992847442627f));
+    } else {
+        q = __ffma2_rn(f, make_float2(kP3c3, kP3c3), make_float2(kP3c2, kP3c2));
+        q = __ffma2_rn(q, f, make_float2(kP3c1, kP3c1));
+        q = __ffma2_rn(q, f, make_float2(kP3c0, kP3c0));
+    }
+    return make_float2(__int_as_float(__float_as_int(q.x) + (__float_as_int(t.x) << 23)),
+                       __int_as_float(__float_as_int(q.y) + (__float_as_int(t.y) << 23)));
+}
+
+// pass 1, one work item: every epilogue thread owns one query row and 16*NCH key columns of each 128-key tile and
+// keeps the row's (reference exponent m, sum z of 2^(x - m)) in registers.  The reference exponent is lazy: it is
+// fixed by the first visible chunk of the row and only an overflow guard watches it afterwards (the row sum is
+// z * 2^m for ANY m, so no per-element max is needed); a tile that trips the guard is read again from TMEM and
+// folded in with the exact online-max update (the rare rescue path).
+template <int D, int NCH>
+__device__ __forceinline__ void rowstats_segment(const Params &p, const Seg &it, uint32_t tmem, uint32_t tfull, uint32_t tempty,
+                                                 uint32_t &astage, uint32_t &aphase, int quad, int grp, int lane,
+                                                 int64_t rowbase, int mrows)
+{
+    constexpr float sc = ScaleLog2<D>::value;
+    constexpr int NC = 16 * NCH;
+    constexpr int ACOLS = (NCH == 4) ? 256 : 128;             // accumulator stage: both 128-row halves, or one
+    const int key_beg = it.t0 * kTileKeys, key_end = min(p.g.n, it.t1 * kTileKeys);
+    const int n = p.g.n;
+    const int hsel = (NCH == 4) ? (grp & 1) : 0;
+    const int cg = (NCH == 4) ? (grp >> 1) : grp;
+    const int col0 = cg * NC;                                 // key offset inside the 128-key tile
+    const int row_in_blk = hsel * 128 + quad * 32 + lane;
+    const int row_g = it.rb * p.MB + row_in_blk;
+    const bool valid = row_in_blk < mrows;
+    const int lim = p.causal ? (n - p.w + (row_g % p.w)) : (n - 1);
+    // first key of the first tile that needs a mask (causal window or ragged tail); tiles before it take the fast path
+    const int mask_from = p.causal ? (n - p.w - kTileKeys + 2) : (n - kTileKeys + 1);
+    float m = kNegBig, z = 0.f;
+    const uint32_t base = tmem + ((uint32_t)(quad * 32) << 16) + hsel * 128 + col0;
+    uint32_t bA[16], bB[16];
+    if (key_beg < key_end) {
+        mbar_wait(tfull + 8 * astage, aphase);
+        tc_fence_after();
+        tmem_ld16_issue(base + astage * ACOLS, bA);
+    }
+    int k0 = key_beg;
+    for (; k0 < key_end && k0 < mask_from; k0 += kTileKeys) {             // ---- fast tiles
+        const uint32_t stage = astage;
+        float2 accA = make_float2(0.f, 0.f), accB = accA;
+        float xmax = kNegBig;                                             // largest exponent sent to the FMA pipe
+        stream_tile<NCH, ACOLS>(bA, bB, base, k0 + kTileKeys < key_end, tfull, astage, aphase,
+            [&](const uint32_t (&r)[16], int c) {
+#ifdef SKV_DBG_NOEXP
+                z += __uint_as_float(r[0]); return;
+#endif
+                if (c == 0 && m < 0.5f * kNegBig) {
+                    float tmax = kNegBig;
+#pragma unroll
+                    for (int i = 0; i < 16; ++i) tmax = fmaxf(tmax, __uint_as_float(r[i]));
+                    m = tmax * sc;
+                }
+                const float2 nm2 = make_float2(-m, -m), sc2 = make_float2(sc, sc);
+#pragma unroll
+                for (int pi = 0; pi < 8; ++pi) {
+                    const float2 x = __ffma2_rn(make_float2(__uint_as_float(r[2 * pi]), __uint_as_float(r[2 * pi + 1])), sc2, nm2);
+                    float2 e;
+                    if (pair_on_fma(pi)) { xmax = fmaxf(xmax, fmaxf(x.x, x.y)); e = ex2_fma2_lo<SKV_P1_DEG>(x); }
+                    else e = ex2_mufu2(x);
+                    if (pi & 1) accB = __fadd2_rn(accB, e); else accA = __fadd2_rn(accA, e);
+                }
+            });
+        const float2 s2 = __fadd2_rn(accA, accB);
+        const float a = s2.x + s2.y;
+        const bool ok = a < 1.0e30f && xmax < 127.0f;
+        if (__all_sync(0xffffffffu, ok)) {
+            z += a;
+            if (!(z < 1.0e30f)) { z *= 0x1p-80f; m += 80.0f; }
+        } else {
+            // a term overflowed in some row of this warp: the whole warp reads the tile again (tcgen05.ld is warp-
+            // collective) and the rows that tripped the guard redo it with the exact online-max update
+            float tmax = kNegBig;
+            for (int c = 0; c < NCH; ++c) {
+                float v[16];
+                tmem_ld16(base + stage * ACOLS + 16 * c, v);
+#pragma unroll
+                for (int i = 0; i < 16; ++i) tmax = fmaxf(tmax, v[i]);
+            }
+            const float mn = ok ? m : fmaxf(m, tmax * sc);
+            float acc = 0.f;
+            for (int c = 0; c < NCH; ++c) {
+                float v[16];
+                tmem_ld16(base + stage * ACOLS + 16 * c, v);
+#pragma unroll
+                for (int i = 0; i < 16; ++i) acc += ex2(fmaf(v[i], sc, -mn));
+            }
+            if (ok) { z += a; if (!(z < 1.0e30f)) { z *= 0x1p-80f; m += 80.0f; } }
+            else    { z = z * ex2(m - mn) + acc; m = mn; }
+        }
+        release_stage(tempty, stage, lane);
+    }
+    for (; k0 < key_end; k0 += kTileKeys) {                               // ---- masked tiles (the last ones of a layer)
+        const uint32_t stage = astage;
+        stream_tile<NCH, ACOLS>(bA, bB, base, k0 + kTileKeys < key_end, tfull, astage, aphase,
+            [&](const uint32_t (&r)[16], int c) {
+                const int j0 = k0 + col0 + 16 * c;
+                float tmax = kNegBig;
+#pragma unroll
+                for (int i = 0; i < 16; ++i) if (j0 + i <= lim) tmax = fmaxf(tmax, __uint_as_float(r[i]));
+                const float mn = fmaxf(m, tmax > 0.5f * kNegBig ? tmax * sc : kNegBig);
+                float acc = 0.f;
+#pragma unroll
+                for (int i = 0; i < 16; ++i) acc += (j0 + i <= lim) ? ex2(fmaf(__uint_as_float(r[i]), sc, -mn)) : 0.f;
+                z = z * ex2(m - mn) + acc;
+                m = mn;
+            });
+        release_stage(tempty, stage, lane);
+    }
+    if (valid) {
+        const int cs = (NCH == 4) ? 2 : 4;
+        p.partial[(rowbase + row_g) * p.pmax + it.piece * cs + cg] = make_float2(m, z);
+    }
+}
+
+// pass 2, one work item: keys are TMEM lanes, so every epilogue thread owns one key and 16*QC query columns of each
+// tile and sums p = 2^(s - lse2[column]) over them in registers; the four column groups of a tile are then added in a
+// fixed order through a 4-deep shared-memory ring.
+template <int D, int QC>
+__device__ __forceinline__ void colsum_segment(const Params &p, const Seg &it, uint32_t tmem, uint32_t tfull, uint32_t tempty, uint32_t redfull,
+                                               uint32_t &astage, uint32_t &aphase, uint32_t &rstage, uint32_t &rphase,
+                                               int quad, int grp, int lane, int mrows,
+                                               const float *sLse, const int *sLim, float *sRed, float *out)
+{
+    constexpr float sc = ScaleLog2<D>::value;
+    constexpr int qcols = 16 * QC;
+    constexpr int ACOLS = (QC >= 3) ? 256 : 128;                          // accumulator stage = the block's query rows
+    const int key_beg = it.t0 * kTileKeys, key_end = min(p.g.n, it.t1 * kTileKeys);
+    const int n = p.g.n;
+    const int cbeg = grp * qcols;
+    const bool cols_full = cbeg + qcols <= mrows;                         // no padding column in this warp's group
+    const int mask_from = p.causal ? (n - p.w - kTileKeys + 2) : n;       // first key of the first tile with masked logits
+    const uint32_t base = tmem + ((uint32_t)(quad * 32) << 16) + cbeg;
+    uint32_t bA[16], bB[16];
+    if (key_beg < key_end) {
+        mbar_wait(tfull + 8 * astage, aphase);
+        tc_fence_after();
+        tmem_ld16_issue(base + astage * ACOLS, bA);
+    }
+    bool par = false;                                                     // buffer holding chunk 0 of the tile (QC odd: alternates)
+    for (int k0 = key_beg; k0 < key_end; k0 += kTileKeys) {
+        const int j = k0 + quad * 32 + lane;
+        const uint32_t stage = astage;
+        const bool more = k0 + kTileKeys < key_end;
+        float mine;
+        if (cols_full && k0 < mask_from) {                                // ---- fast tile
+            float2 accA = make_float2(0.f, 0.f), accB = accA;
+            auto chunk = [&](const uint32_t (&r)[16], int c) {
+#ifdef SKV_DBG_NOEXP
+                accA.x += __uint_as_float(r[0]); return;
+#endif
+                const float4 *l4 = reinterpret_cast<const float4 *>(sLse + cbeg + 16 * c);
+                const float2 sc2 = make_float2(sc, sc);
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    const float4 L4 = l4[i];
+                    const float2 x0 = __ffma2_rn(make_float2(__uint_as_float(r[4 * i]), __uint_as_float(r[4 * i + 1])), sc2, make_float2(L4.x, L4.y));
+                    const float2 x1 = __ffma2_rn(make_float2(__uint_as_float(r[4 * i + 2]), __uint_as_float(r[4 * i + 3])), sc2, make_float2(L4.z, L4.w));
+                    accA = __fadd2_rn(accA, pair_on_fma2(2 * i) ? ex2_fma2_lo<4>(x0) : ex2_mufu2(x0));
+                    accB = __fadd2_rn(accB, pair_on_fma2(2 * i + 1) ? ex2_fma2_lo<4>(x1) : ex2_mufu2(x1));
+                }
+            };
+            if (!par) stream_tile<QC, ACOLS>(bA, bB, base, more, tfull, astage, aphase, chunk);
+            else      stream_tile<QC, ACOLS>(bB, bA, base, more, tfull, astage, aphase, chunk);
+            const float2 s2 = __fadd2_rn(accA, accB);
+            mine = s2.x + s2.y;
+        } else {                                                          // ---- masked tile or padded column group
+            float s0 = 0.f;
+            auto chunk = [&](const uint32_t (&r)[16], int c) {
+                const int cc = 16 * c;
+                if (cbeg + cc >= mrows) return;                           // warp-uniform: padding columns
+                const int *lim = sLim + cbeg + cc;
+#pragma unroll
+                for (int i = 0; i < 16; ++i)
+                    s0 += (j <= lim[i]) ? ex2(fmaf(__uint_as_float(r[i]), sc, sLse[cbeg + cc + i])) : 0.f;
+            };
+            if (!par) stream_tile<QC, ACOLS>(bA, bB, base, more, tfull, astage, aphase, chunk);
+            else      stream_tile<QC, ACOLS>(bB, bA, base, more, tfull, astage, aphase, chunk);
+            mine = s0;
+        }
+        if (QC & 1) par = !par;
+        release_stage(tempty, stage, lane);
+        // add the four column groups of this tile in a fixed order (deterministic): groups 1..3 drop their sums
+        // into a 4-deep shared-memory ring and arrive on its mbarrier (they never block); group 0 waits for the
+        // slot, adds and stores.  A warp is never more than (accumulator stages <= 4) tiles ahead of the slowest one
+        // (the MMA of tile i+stages needs every warp to have released tile i), so with kRing = 8 slots a slot is
+        // never overwritten before group 0 has read it.
+        float *red = sRed + rstage * (3 * kTileKeys);
+        if (grp != 0) {
+            red[(grp - 1) * kTileKeys + quad * 32 + lane] = mine;
+            __syncwarp();
+            if (lane == 0) mbar_arrive(redfull + 8 * rstage);
+        } else {
+            mbar_wait(redfull + 8 * rstage, rphase);
+            const int k = quad * 32 + lane;
+            if (j < n) out[j] = (mine + red[k]) + (red[kTileKeys + k] + red[2 * kTileKeys + k]);
+        }
+        if (++rstage == kRing) { rstage = 0; rphase ^= 1; }
+    }
+}
+
+// V: pass 1 = 16-key chunks per thread per tile (2 or 4); pass 2 = 16-query-column chunks per thread per tile (1..4)
+template <int D, int PASS, int V>
 __global__ void __launch_bounds__(kThreads, 1)
 imp_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmQ, const Params p)
 {
     using C = Cfg<D>;
+    constexpr int ACOLS = (PASS == 1) ? (V == 4 ? 256 : 128) : (V >= 3 ? 256 : 128);   // TMEM columns per accumulator stage
+    constexpr int ASTAGES = 512 / ACOLS;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;       // 1024-B aligned (128-B swizzle atoms)
     uint8_t *gbase = smem_raw + (sbase - smem_u32(smem_raw));
@@ -238,21 +549,22 @@ imp_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ C
     int *sLim = reinterpret_cast<int *>(sLse + 256);
     float *sRed = reinterpret_cast<float *>(sLim + 256);
     const uint32_t sBar = sK + C::STAGES * C::K_BYTES + 256 * 4 * 2 + C::RED_BYTES;
-    // barriers (8 bytes each): kfull[S], kempty[S], qfull, qempty, tfull[2], tempty[2]
+    // barriers (8 bytes each): kfull[S], kempty[S], qfull, qempty, tfull[4], tempty[4], redfull[kRing]
     const uint32_t kfull = sBar, kempty = sBar + 8 * C::STAGES;
     const uint32_t qfull = sBar + 16 * C::STAGES, qempty = qfull + 8;
-    const uint32_t tfull = qempty + 8, tempty = tfull + 16;
-    const uint32_t redfull = tempty + 16;                               // 4 barriers: column-group partials landed
-    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(gbase + (redfull + 32 - sbase));
+    const uint32_t tfull = qempty + 8, tempty = tfull + 32;
+    const uint32_t redfull = tempty + 32;                               // column-group partials of a tile have landed
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(gbase + (redfull + 8 * kRing - sbase));
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n = p.g.n;
+    const long long ubeg = (long long)blockIdx.x * p.U / gridDim.x, uend = (long long)(blockIdx.x + 1) * p.U / gridDim.x;
 
     if (warp == 0 && lane == 0) {
         for (int s = 0; s < C::STAGES; ++s) { mbar_init(kfull + 8 * s, 1); mbar_init(kempty + 8 * s, 1); }
         mbar_init(qfull, 1); mbar_init(qempty, 1);
-        for (int a = 0; a < 2; ++a) { mbar_init(tfull + 8 * a, 1); mbar_init(tempty + 8 * a, kEpiWarps); }
-        for (int a = 0; a < 4; ++a) mbar_init(redfull + 8 * a, kEpiWarps - 4);
+        for (int a = 0; a < 4; ++a) { mbar_init(tfull + 8 * a, 1); mbar_init(tempty + 8 * a, kEpiWarps); }
+        for (int a = 0; a < kRing; ++a) mbar_init(redfull + 8 * a, kEpiWarps - 4);
         fence_barrier_init();
     }
     if (warp == 1) {
@@ -268,18 +580,18 @@ imp_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ C
         // ===================== TMA producer =====================
         if (lane == 0) {
             uint32_t kstage = 0, kphase = 0, qphase = 0;
-            for (int item = blockIdx.x; item < p.n_items; item += gridDim.x) {
-                const Item it = decode_item(p, item);
+            for (long long u = ubeg; u < uend;) {
+                const Seg it = seg_at(p, u, uend);
+                u += it.t1 - it.t0;
                 mbar_wait(qempty, qphase ^ 1); qphase ^= 1;
                 mbar_expect_tx(qfull, (uint32_t)(p.qrows * D * 2));
                 for (int kb = 0; kb < C::KB; ++kb)
                     tma_load_3d(sQ + kb * C::Q_KB_STRIDE, &tmQ, qfull, kb * 64, it.rb * p.MB, (it.r * p.g.L + it.l) * p.g.Hkv + it.g);
-                const int key_beg = it.chunk * p.chunk_keys, key_end = min(n, key_beg + p.chunk_keys);
-                for (int k0 = key_beg; k0 < key_end; k0 += kTileKeys) {
+                for (int t = it.t0; t < it.t1; ++t) {
                     mbar_wait(kempty + 8 * kstage, kphase ^ 1);
                     mbar_expect_tx(kfull + 8 * kstage, (uint32_t)C::K_BYTES);
                     int c[5]; c[0] = 0;
-                    c[p.kdim[0]] = it.g; c[p.kdim[1]] = k0; c[p.kdim[2]] = it.l; c[p.kdim[3]] = it.r;
+                    c[p.kdim[0]] = it.g; c[p.kdim[1]] = t * kTileKeys; c[p.kdim[2]] = it.l; c[p.kdim[3]] = it.r;
                     for (int kb = 0; kb < C::KB; ++kb)
                         tma_load_5d(sK + kstage * C::K_BYTES + kb * C::K_KB_STRIDE, &tmK, kfull + 8 * kstage, kb * 64, c[1], c[2], c[3], c[4]);
                     if (++kstage == C::STAGES) { kstage = 0; kphase ^= 1; }
@@ -291,18 +603,22 @@ imp_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ C
         if (lane == 0) {
             uint32_t kstage = 0, kphase = 0, qphase = 0, astage = 0, aphase = 0;
             const uint32_t idesc = (PASS == 1) ? umma_idesc(128, kTileKeys, p.g.bf16) : umma_idesc(128, p.qrows, p.g.bf16);
-            for (int item = blockIdx.x; item < p.n_items; item += gridDim.x) {
-                const Item it = decode_item(p, item);
+            for (long long u = ubeg; u < uend;) {
+                const Seg it = seg_at(p, u, uend);
+                u += it.t1 - it.t0;
                 mbar_wait(qfull, qphase); qphase ^= 1;
-                const int key_beg = it.chunk * p.chunk_keys, key_end = min(n, key_beg + p.chunk_keys);
-                for (int k0 = key_beg; k0 < key_end; k0 += kTileKeys) {
+                for (int t = it.t0; t < it.t1; ++t) {
                     mbar_wait(tempty + 8 * astage, aphase ^ 1);
                     mbar_wait(kfull + 8 * kstage, kphase);
                     tc_fence_after();
                     const uint32_t kt = sK + kstage * C::K_BYTES;
-                    const uint32_t acc = tmem + astage * 256;
+                    const uint32_t acc = tmem + astage * ACOLS;
+#ifdef SKV_DBG_NOMMA
+                    if (false) {} else if (false)
+#endif
                     if (PASS == 1) {
-                        for (int hh = 0; hh < p.halves; ++hh)
+#pragma unroll
+                        for (int hh = 0; hh < (V == 4 ? 2 : 1); ++hh)
 #pragma unroll
                             for (int ks = 0; ks < D / 16; ++ks) {
                                 const uint32_t koff = (ks >> 2) * 1u, kin = (ks & 3) * 32u;
@@ -320,9 +636,9 @@ imp_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ C
                     umma_commit(kempty + 8 * kstage);          // smem stage free once these MMAs have read it
                     umma_commit(tfull + 8 * astage);           // accumulator ready for the epilogue
                     if (++kstage == C::STAGES) { kstage = 0; kphase ^= 1; }
-                    if (++astage == 2) { astage = 0; aphase ^= 1; }
+                    if (++astage == ASTAGES) { astage = 0; aphase ^= 1; }
                 }
-                umma_commit(qempty);                           // Q buffer free once every MMA of the item is done
+                umma_commit(qempty);                           // Q buffer free once every MMA of the segment is done
             }
         }
     } else {
@@ -330,86 +646,17 @@ imp_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ C
         // TMEM lane window of a warp is fixed by (warp id % 4); grp = which of the four warps on that window.
         const int e = warp - 2, quad = warp & 3, grp = e >> 2;
         const int etid = e * 32 + lane;                                   // 0..511 among the epilogue threads
-        constexpr float sc = ScaleLog2<D>::value;                         // log2(e)/sqrt(d)
         const int G = p.g.Hq / p.g.Hkv, M = G * p.w;
         uint32_t astage = 0, aphase = 0, rstage = 0, rphase = 0;
-        for (int item = blockIdx.x; item < p.n_items; item += gridDim.x) {
-            const Item it = decode_item(p, item);
-            const int key_beg = it.chunk * p.chunk_keys, key_end = min(n, key_beg + p.chunk_keys);
+        for (long long u = ubeg; u < uend;) {
+            const Seg it = seg_at(p, u, uend);
+            u += it.t1 - it.t0;
             const int64_t rowbase = ((int64_t)it.r * p.g.L + it.l) * p.g.Hq * p.w + (int64_t)it.g * M;
             const int mrows = min(p.MB, M - it.rb * p.MB);
             if (PASS == 1) {
-                // halves == 2: 2 row halves x 2 column groups of 64 keys; halves == 1: 4 column groups of 32 keys
-                const int hsel = (p.halves == 2) ? (grp & 1) : 0;
-                const int cg = (p.halves == 2) ? (grp >> 1) : grp;
-                const int ncols = (p.halves == 2) ? 64 : 32;
-                const int col0 = cg * ncols;                              // key offset inside the 128-key tile
-                const int row_in_blk = hsel * 128 + quad * 32 + lane;
-                const int row_g = it.rb * p.MB + row_in_blk;
-                const bool valid = row_in_blk < mrows;
-                const int lim = p.causal ? (n - p.w + (row_g % p.w)) : (n - 1);
-                float m = kNegBig, z = 0.f;
-                for (int k0 = key_beg; k0 < key_end; k0 += kTileKeys) {
-                    mbar_wait(tfull + 8 * astage, aphase);
-                    tc_fence_after();
-                    const bool need_mask = p.causal ? (k0 + kTileKeys - 1 > n - p.w) : (k0 + kTileKeys > n);
-                    const uint32_t taddr = tmem + ((uint32_t)(quad * 32) << 16) + astage * 256 + hsel * 128 + col0;
-                    for (int cc = 0; cc < ncols; cc += 32) {
-                        float v[32];
-                        tmem_ld32(taddr + cc, v);
-                        const int j0 = k0 + col0 + cc;
-                        float tmax = kNegBig;
-                        if (!need_mask) {
-                            // lazy reference exponent: m is fixed by the first visible group of the row and only an
-                            // overflow guard watches it afterwards (the row sum is z * 2^m for ANY m, so no per-
-                            // element max is needed); the exact online-max update below is the rare rescue path.
-                            if (m < 0.5f * kNegBig) {
-#pragma unroll
-                                for (int i = 0; i < 32; ++i) tmax = fmaxf(tmax, v[i]);
-                                m = tmax * sc;
-                            }
-                            float2 nm2[16];
-#pragma unroll
-                            for (int pi = 0; pi < 16; ++pi) nm2[pi] = make_float2(-m, -m);
-                            float2 accA = make_float2(0.f, 0.f), accB = accA;
-                            exp_accumulate<32>(v, make_float2(sc, sc), nm2, accA, accB);
-                            const float2 s2 = __fadd2_rn(accA, accB);
-                            const float a = s2.x + s2.y;
-                            if (a < 1.0e30f) {
-                                z += a;
-                                if (!(z < 1.0e30f)) { z *= 0x1p-80f; m += 80.0f; }
-                            } else {                                      // a term overflowed: redo the group exactly
-#pragma unroll
-                                for (int i = 0; i < 32; ++i) tmax = fmaxf(tmax, v[i]);
-                                const float mn = fmaxf(m, tmax * sc);
-                                float acc = 0.f;
-#pragma unroll
-                                for (int i = 0; i < 32; ++i) acc += ex2(fmaf(v[i], sc, -mn));
-                                z = z * ex2(m - mn) + acc;
-                                m = mn;
-                            }
-                        } else {
-#pragma unroll
-                            for (int i = 0; i < 32; ++i) if (j0 + i <= lim) tmax = fmaxf(tmax, v[i]);
-                            const float mn = fmaxf(m, tmax > 0.5f * kNegBig ? tmax * sc : kNegBig);
-                            float acc = 0.f;
-#pragma unroll
-                            for (int i = 0; i < 32; ++i) acc += (j0 + i <= lim) ? ex2(fmaf(v[i], sc, -mn)) : 0.f;
-                            z = z * ex2(m - mn) + acc;
-                            m = mn;
-                        }
-                    }
-                    tc_fence_before();
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive(tempty + 8 * astage);
-                    if (++astage == 2) { astage = 0; aphase ^= 1; }
-                }
-                if (valid) {
-                    const int cs = (p.halves == 2) ? 2 : 4;
-                    p.partial[(rowbase + row_g) * p.pchunks + it.chunk * cs + cg] = make_float2(m, z);
-                }
+                rowstats_segment<D, (PASS == 1 ? V : 2)>(p, it, tmem, tfull, tempty, astage, aphase, quad, grp, lane, rowbase, mrows);
             } else {
-                // per-item column tables: lse2 of the block's query rows and their causal limits
+                // per-segment column tables: lse2 of the block's query rows and their causal limits
                 epi_bar_sync();
                 for (int idx = etid; idx < p.qrows; idx += kEpiThreads) {
                     const bool ok = idx < mrows;
@@ -417,60 +664,8 @@ imp_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ C
                     sLim[idx] = ok ? (p.causal ? (n - p.w + ((it.rb * p.MB + idx) % p.w)) : (n - 1)) : -1;
                 }
                 epi_bar_sync();
-                const int qcols = p.qrows >> 2;                           // query columns per group: 16, 32, 48 or 64
-                const int cbeg = grp * qcols;
                 float *out = p.apart + (((int64_t)it.r * p.g.L + it.l) * p.S + it.gb) * (int64_t)n;
-                for (int k0 = key_beg; k0 < key_end; k0 += kTileKeys) {
-                    mbar_wait(tfull + 8 * astage, aphase);
-                    tc_fence_after();
-                    const int j = k0 + quad * 32 + lane;
-                    const bool tile_mask = p.causal && (k0 + kTileKeys - 1 > n - p.w);
-                    const uint32_t taddr = tmem + ((uint32_t)(quad * 32) << 16) + astage * 256 + cbeg;
-                    float2 accA = make_float2(0.f, 0.f), accB = accA;
-                    float s0 = 0.f;
-                    for (int cc = 0; cc < qcols; cc += 16) {
-                        if (cbeg + cc >= mrows) break;                    // warp-uniform: only padding columns left
-                        float v[16];
-                        tmem_ld16(taddr + cc, v);
-                        if (!tile_mask && cbeg + cc + 16 <= mrows) {
-                            const float4 *l4 = reinterpret_cast<const float4 *>(sLse + cbeg + cc);
-                            float2 nl2[8];
-#pragma unroll
-                            for (int i = 0; i < 4; ++i) {
-                                const float4 L4 = l4[i];
-                                nl2[2 * i] = make_float2(L4.x, L4.y);
-                                nl2[2 * i + 1] = make_float2(L4.z, L4.w);
-                            }
-                            exp_accumulate<16>(v, make_float2(sc, sc), nl2, accA, accB);
-                        } else {
-                            const int *lim = sLim + cbeg + cc;
-#pragma unroll
-                            for (int i = 0; i < 16; ++i)
-                                s0 += (j <= lim[i]) ? ex2(fmaf(v[i], sc, sLse[cbeg + cc + i])) : 0.f;
-                        }
-                    }
-                    const float2 s2 = __fadd2_rn(accA, accB);
-                    tc_fence_before();
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive(tempty + 8 * astage);
-                    if (++astage == 2) { astage = 0; aphase ^= 1; }
-                    // add the four column groups of this tile in a fixed order (deterministic): groups 1..3 drop
-                    // their sums into a 4-deep shared-memory ring and arrive on its mbarrier (they never block);
-                    // group 0 waits for the slot, adds and stores.  Ring depth 4 > the 2 TMEM stages any warp can
-                    // run ahead, so a slot is never overwritten before group 0 has read it.
-                    const float mine = (s2.x + s2.y) + s0;
-                    float *red = sRed + rstage * (3 * kTileKeys);
-                    if (grp != 0) {
-                        red[(grp - 1) * kTileKeys + quad * 32 + lane] = mine;
-                        __syncwarp();
-                        if (lane == 0) mbar_arrive(redfull + 8 * rstage);
-                    } else {
-                        mbar_wait(redfull + 8 * rstage, rphase);
-                        const int k = quad * 32 + lane;
-                        if (j < n) out[j] = (mine + red[k]) + (red[kTileKeys + k] + red[2 * kTileKeys + k]);
-                    }
-                    if (++rstage == 4) { rstage = 0; rphase ^= 1; }
-                }
+                colsum_segment<D, (PASS == 2 ? V : 1)>(p, it, tmem, tfull, tempty, redfull, astage, aphase, rstage, rphase, quad, grp, lane, mrows, sLse, sLim, sRed, out);
             }
         }
     }
@@ -515,9 +710,12 @@ static EncodeTiledFn get_encode_fn()
 }
 
 struct TcPlan {
-    int QROWS_MAX, RB, MB, qrows, halves, chunk_keys, n_chunks, pchunks, S, n_items;
+    int QROWS_MAX, RB, MB, qrows, halves, S, T, grid, pmax;
+    long long U;
     size_t partial_bytes, lse_bytes, apart_bytes;
 };
+
+constexpr int kPlanSMs = 148;                          // B200; the grid is planned on the host (the workspace query is host-only)
 
 static TcPlan tc_plan(const Geom &g, int w)
 {
@@ -531,28 +729,16 @@ static TcPlan tc_plan(const Geom &g, int w)
     t.MB = (t.RB == 1) ? M : mb;
     t.qrows = ((std::min(t.MB, M) + 63) / 64) * 64;
     t.halves = t.qrows > 128 ? 2 : 1;
-    const long long triples = (long long)g.R * g.L * g.Hkv * t.RB;
-    // Key chunk per work item: items are dealt round-robin to one persistent CTA per SM, so the cost of a candidate
-    // chunk size is (rounds of items) x (tiles per item + ~3 tiles of per-item overhead: Q load, pipeline fill and
-    // drain).  Candidates are multiples of 128 keys from 512 up; ties go to the larger chunk (fewer partials).
-    const int npad = ((g.n + 127) / 128) * 128;
-    constexpr long long kSMs = 148;                     // B200; also used by the host-only workspace query
-    int ck = npad;
-    long long best = -1;
-    for (int c = std::min(512, npad); c <= npad; c += 128) {
-        const long long chunks = (g.n + c - 1) / c;
-        const long long rounds = (triples * chunks + kSMs - 1) / kSMs;
-        const long long cost = rounds * (c / 128 + 3);
-        if (best < 0 || cost <= best) { best = cost; ck = c; }
-    }
-    t.chunk_keys = ck;
-    t.n_chunks = (g.n + ck - 1) / ck;
-    t.pchunks = t.n_chunks * (t.halves == 1 ? 4 : 2);
     t.S = g.Hkv * t.RB;
-    const long long items = triples * t.n_chunks;
-    t.n_items = items > 0x7FFFFFFFll ? -1 : (int)items;                 // -1: does not fit (reported as unsupported)
+    t.T = (g.n + tc::kTileKeys - 1) / tc::kTileKeys;
+    t.U = (long long)g.R * g.L * t.S * t.T;
+    t.grid = (int)std::min<long long>(t.U, kPlanSMs);
+    // a row of T tiles is cut by CTA boundaries into at most ceil(T / q) + 1 pieces, q = units per CTA (floor)
+    const long long q = std::max<long long>(1, t.U / t.grid);
+    const int pieces = (int)((t.T + q - 1) / q) + 1;
+    t.pmax = pieces * (t.halves == 1 ? 4 : 2);
     const size_t rows = (size_t)g.R * g.L * g.Hq * w;
-    t.partial_bytes = (rows * t.pchunks * sizeof(float2) + 255) & ~(size_t)255;
+    t.partial_bytes = (rows * t.pmax * sizeof(float2) + 255) & ~(size_t)255;
     t.lse_bytes = (rows * sizeof(float) + 255) & ~(size_t)255;
     t.apart_bytes = (size_t)g.R * g.L * t.S * g.n * sizeof(float);
     return t;
@@ -562,39 +748,57 @@ size_t importance_tc_ws_bytes(const Geom &g, int window)
 {
     if (g.Hkv <= 0 || g.Hq < g.Hkv || g.Hq % g.Hkv || window <= 0) return 0;
     const TcPlan t = tc_plan(g, window);
-    if (t.n_items < 0) return 0;
     return t.partial_bytes + t.lse_bytes + t.apart_bytes;
 }
 
-// lse2[row] = M + log2(sum_c z_c 2^(m_c - M)) over the row's partial (max, sum) pairs
-__global__ void imp_tc_combine_kernel(const float2 *__restrict__ partial, int n_chunks, int64_t rows, float *__restrict__ lse2)
+// lse2[row] = M + log2(sum_c z_c 2^(m_c - M)) over the partial (reference exponent, sum) pairs of the row's pieces
+__global__ void imp_tc_combine_kernel(tc::Params p, int grid, int cs, int64_t rows, float *__restrict__ lse2)
 {
     const int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (row >= rows) return;
-    const float2 *q = partial + row * n_chunks;
+    // which (request, layer, KV head, row block) the query row belongs to, hence how many CTAs shared its tiles
+    const int HW = p.g.Hq * p.w, M = (p.g.Hq / p.g.Hkv) * p.w;
+    const int rr = (int)(row % HW);
+    const long long rl = row / HW;
+    const int gb = (rr / M) * p.RB + (rr % M) / p.MB;
+    const long long first = (rl * p.S + gb) * (long long)p.T;
+    const int pieces = (int)(tc::cta_of_unit(first + p.T - 1, p.U, grid) - tc::cta_of_unit(first, p.U, grid)) + 1;
+    const float2 *q = p.partial + row * p.pmax;
+    const int cnt = pieces * cs;
     float m = tc::kNegBig;
-    for (int c = 0; c < n_chunks; ++c) m = fmaxf(m, q[c].x);
+    for (int c = 0; c < cnt; ++c) m = fmaxf(m, q[c].x);
     float z = 0.f;
-    for (int c = 0; c < n_chunks; ++c) z += q[c].y * exp2f(q[c].x - m);
+    for (int c = 0; c < cnt; ++c) z += q[c].y * exp2f(q[c].x - m);
     lse2[row] = m + log2f(z);
+}
+
+template <int D, int PASS, int V>
+static cudaError_t launch_pass(const CUtensorMap &tmK, const CUtensorMap &tmQ, const tc::Params &p, int grid, cudaStream_t s)
+{
+    using C = tc::Cfg<D>;
+    cudaError_t e = cudaFuncSetAttribute(tc::imp_tc_kernel<D, PASS, V>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM);
+    if (e != cudaSuccess) return e;
+    tc::imp_tc_kernel<D, PASS, V><<<grid, tc::kThreads, C::SMEM, s>>>(tmK, tmQ, p);
+    return cudaGetLastError();
 }
 
 template <int D>
 static cudaError_t launch_tc_t(const Geom &g, const CUtensorMap &tmK, const CUtensorMap &tmQ, tc::Params p, float lambda,
-                               float *importance, int sms, cudaStream_t s)
+                               float *importance, int grid, cudaStream_t s)
 {
-    using C = tc::Cfg<D>;
     cudaError_t e;
-    if ((e = cudaFuncSetAttribute(tc::imp_tc_kernel<D, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM)) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(tc::imp_tc_kernel<D, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM)) != cudaSuccess) return e;
-    const int grid = std::min(p.n_items, sms);
-    tc::imp_tc_kernel<D, 1><<<grid, tc::kThreads, C::SMEM, s>>>(tmK, tmQ, p);
-    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    e = (p.halves == 2) ? launch_pass<D, 1, 4>(tmK, tmQ, p, grid, s) : launch_pass<D, 1, 2>(tmK, tmQ, p, grid, s);
+    if (e != cudaSuccess) return e;
     const int64_t rows = (int64_t)g.R * g.L * g.Hq * p.w;
-    imp_tc_combine_kernel<<<(unsigned)((rows + 255) / 256), 256, 0, s>>>(p.partial, p.pchunks, rows, const_cast<float *>(p.lse2));
+    imp_tc_combine_kernel<<<(unsigned)((rows + 255) / 256), 256, 0, s>>>(p, grid, p.halves == 2 ? 2 : 4, rows, const_cast<float *>(p.lse2));
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
-    tc::imp_tc_kernel<D, 2><<<grid, tc::kThreads, C::SMEM, s>>>(tmK, tmQ, p);
-    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    switch (p.qrows >> 6) {
+    case 1:  e = launch_pass<D, 2, 1>(tmK, tmQ, p, grid, s); break;
+    case 2:  e = launch_pass<D, 2, 2>(tmK, tmQ, p, grid, s); break;
+    case 3:  e = launch_pass<D, 2, 3>(tmK, tmQ, p, grid, s); break;
+    default: e = launch_pass<D, 2, 4>(tmK, tmQ, p, grid, s); break;
+    }
+    if (e != cudaSuccess) return e;
     dim3 gf((g.n + 255) / 256, g.L, g.R);
     tc::imp_finish_kernel<<<gf, 256, 0, s>>>(g, p.w, lambda, p.S, p.apart, importance);
     return cudaGetLastError();
@@ -640,20 +844,21 @@ cudaError_t launch_importance_tc(const Geom &g, const __half *K, const __half *Q
         return cudaErrorNotSupported;
 
     p.g = g; p.w = window; p.causal = causal;
-    p.chunk_keys = t.chunk_keys; p.n_chunks = t.n_chunks; p.RB = t.RB; p.MB = t.MB; p.qrows = t.qrows;
-    p.halves = t.halves; p.n_items = t.n_items; p.pchunks = t.pchunks; p.S = t.S;
+    p.RB = t.RB; p.MB = t.MB; p.qrows = t.qrows; p.halves = t.halves;
+    p.S = t.S; p.T = t.T; p.U = t.U; p.pmax = t.pmax;
     uint8_t *w8 = reinterpret_cast<uint8_t *>(ws);
     p.partial = reinterpret_cast<float2 *>(w8);
     p.lse2 = reinterpret_cast<const float *>(w8 + t.partial_bytes);
     p.apart = reinterpret_cast<float *>(w8 + t.partial_bytes + t.lse_bytes);
 
-    int dev = 0, sms = 148;
+    int dev = 0, sms = kPlanSMs;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const int grid = std::min(t.grid, sms);             // fewer CTAs than planned only lengthens the pieces: pmax still holds
     switch (g.D) {
-    case 64:  return launch_tc_t<64>(g, tmK, tmQ, p, lambda, importance, sms, s);
-    case 128: return launch_tc_t<128>(g, tmK, tmQ, p, lambda, importance, sms, s);
-    case 256: return launch_tc_t<256>(g, tmK, tmQ, p, lambda, importance, sms, s);
+    case 64:  return launch_tc_t<64>(g, tmK, tmQ, p, lambda, importance, grid, s);
+    case 128: return launch_tc_t<128>(g, tmK, tmQ, p, lambda, importance, grid, s);
+    case 256: return launch_tc_t<256>(g, tmK, tmQ, p, lambda, importance, grid, s);
     default: return cudaErrorInvalidValue;
     }
 }
