@@ -4,9 +4,8 @@
 //   * one persistent, warp-specialised CTA per SM: warp 0 = TMA producer, warp 1 = MMA issuer (one elected
 //     thread) and TMEM owner, warps 2..17 = sixteen epilogue warps (four per scheduler, so that the MUFU pipe,
 //     which bounds the arithmetic at d_h = 128, always has an eligible warp);
-//   * a quarter of the exponentials is evaluated on the FMA pipe (round-to-nearest range reduction + minimax
-//     polynomial: degree 4, 2.7e-6 relative, in pass 2; degree 3, 7.5e-5, for the row normaliser of pass 1)
-//     instead of MUFU.EX2, which lifts the 16 ex2/clk/SM ceiling;
+//   * a quarter of the exponentials is evaluated on the FMA pipe (round-to-nearest range reduction + degree-4
+//     minimax polynomial, 2.7e-6 relative) instead of MUFU.EX2, which lifts the 16 ex2/clk/SM ceiling;
 //   * operands land in shared memory by TMA (cp.async.bulk.tensor, 128-byte swizzle, mbarrier complete_tx)
 //     straight from the strided K cache and the Q window; accumulators live in TMEM (2 stages x 256 columns, or
 //     4 x 128 when a tile needs no more than 128 columns);
@@ -15,8 +14,9 @@
 //   * pass 2 (colsum):  D[key][query row] = K_tile Q_blk^T, keys are TMEM lanes, so each thread owns one key and
 //     sums p = 2^(s - lse2[row]) over its columns in registers -- no shuffles, no atomics; the four column groups
 //     of a tile are added through shared memory in a fixed order, the per-(KV head, row block) partial sums go to a
-//     workspace and a small finish kernel adds them in a fixed order (deterministic) and applies 1/(Hq w) and the
-//     recency decay;
+//     workspace and the last phase adds them in a fixed order (deterministic) and applies 1/(Hq w) and the decay;
+//   * ONE cooperative launch runs pass 1 | lse2 per row | pass 2 | final sum, separated by grid-wide barriers, so
+//     TMEM, the mbarriers and the tensor maps are set up once and a 4 K-token request pays one launch, not four;
 //   * the epilogue pulls TMEM in 16-column chunks with one chunk in flight (the load of chunk c+1 is issued before
 //     the exponentials of chunk c), so the TMEM latency hides behind arithmetic.
 // Work decomposition (both passes): the unit is one 128-key tile of one (request, layer, KV head, row block); the
@@ -54,6 +54,7 @@ struct Params {
     float2 *partial;                    // [R*L*Hq*w][pmax]
     const float *lse2;                  // [R][L][Hq*w]
     float *apart;                       // [R][L][S][n]
+    unsigned int *gbar;                 // grid-barrier arrival counter (zeroed on the stream before the launch)
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -119,21 +120,6 @@ __device__ __forceinline__ void umma_commit(uint32_t bar)
 {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(bar) : "memory");
 }
-__device__ __forceinline__ void tmem_ld32(uint32_t taddr, float (&v)[32])
-{
-    uint32_t r[32];
-    asm volatile(
-        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
-        "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
-        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
-          "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]),
-          "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]),
-          "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
-        : "r"(taddr) : "memory");
-    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
-    for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
-}
 __device__ __forceinline__ void tmem_ld16(uint32_t taddr, float (&v)[16])
 {
     uint32_t r[16];
@@ -153,27 +139,8 @@ __device__ __forceinline__ float ex2(float x)
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
-// 2^x for a PAIR of values on the FMA/ALU pipes with the packed fp32 instructions of sm_100 (FFMA2 / FADD2):
-// n = rint(x) through the 1.5*2^23 constant, f = x - n in [-0.5, 0.5], degree-4 minimax polynomial for 2^f (max
-// relative error 2.7e-6), exponent patched in with one shift-add per value.  x is clamped to [-125, 128]: anything
-// below contributes < 2^-125 of the row's reference term, anything above yields a value the caller's overflow guard
-// (a < 1e30 is false for huge, Inf and NaN) rejects.  6 issue slots per value and no MUFU.
-__device__ __forceinline__ float2 ex2_fma2(float2 x)
-{
-    x.x = fminf(fmaxf(x.x, -125.0f), 128.0f);            // upper clamp: x >= 128 must come out as >= 2^127 / Inf / NaN
-    x.y = fminf(fmaxf(x.y, -125.0f), 128.0f);            // (never a wrapped exponent), so the overflow guard sees it
-    const float2 t = __fadd2_rn(x, make_float2(12582912.0f, 12582912.0f));
-    const float2 nf = __fadd2_rn(t, make_float2(-12582912.0f, -12582912.0f));
-    const float2 f = __ffma2_rn(nf, make_float2(-1.0f, -1.0f), x);
-    float2 q = __ffma2_rn(f, make_float2(0.009570102207362652f, 0.009570102207362652f), make_float2(0.05591785907745361f, 0.05591785907745361f));
-    q = __ffma2_rn(q, f, make_float2(0.240247443318367f, 0.240247443318367f));
-    q = __ffma2_rn(q, f, make_float2(0.6931217908859253f, 0.6931217908859253f));
-    q = __ffma2_rn(q, f, make_float2(0.9999992847442627f, 0.9999992847442627f));
-    return make_float2(__int_as_float(__float_as_int(q.x) + (__float_as_int(t.x) << 23)),
-                       __int_as_float(__float_as_int(q.y) + (__float_as_int(t.y) << 23)));
-}
 __device__ __forceinline__ float2 ex2_mufu2(float2 x) { return make_float2(ex2(x.x), ex2(x.y)); }
-// which of the 8 value pairs of a 16-wide group go to the FMA pipe (the rest to MUFU.EX2): kFmaPairs of 8
+// which of the 8 value pairs of a 16-value chunk go to the FMA pipe (the rest to MUFU.EX2): SKV_EX2_FMA_PAIRS of 8
 #ifndef SKV_EX2_FMA_PAIRS
 #define SKV_EX2_FMA_PAIRS 2
 #endif
@@ -184,34 +151,6 @@ __device__ __forceinline__ constexpr bool pair_on_fma(int pi)
          : SKV_EX2_FMA_PAIRS == 2 ? (pi & 3) == 1
          : SKV_EX2_FMA_PAIRS == 3 ? ((pi & 7) == 1 || (pi & 7) == 4 || (pi & 7) == 6)
          :                          (pi & 1) == 1;
-}
-// pass 2 has its own share (SKV_EX2_FMA_PAIRS_P2 of 8 pairs)
-#ifndef SKV_EX2_FMA_PAIRS_P2
-#define SKV_EX2_FMA_PAIRS_P2 SKV_EX2_FMA_PAIRS
-#endif
-__device__ __forceinline__ constexpr bool pair_on_fma2(int pi)
-{
-    return SKV_EX2_FMA_PAIRS_P2 == 0 ? false
-         : SKV_EX2_FMA_PAIRS_P2 == 1 ? (pi & 7) == 3
-         : SKV_EX2_FMA_PAIRS_P2 == 2 ? (pi & 3) == 1
-         : SKV_EX2_FMA_PAIRS_P2 == 3 ? ((pi & 7) == 1 || (pi & 7) == 4 || (pi & 7) == 6)
-         :                             (pi & 1) == 1;
-}
-#ifndef SKV_P1_DEG
-#define SKV_P1_DEG 3
-#endif
-// degree-3 minimax polynomial for 2^f on [-0.5, 0.5] (relative error 7.5e-5)
-constexpr float kP3c0 = 0.9999280571937561f, kP3c1 = 0.6932609677314758f, kP3c2 = 0.2426111251115799f, kP3c3 = 0.0551716685295105f;
-// sum of 2^(v*sc + add) over a 16-wide group, two packed accumulators
-template <int N>
-__device__ __forceinline__ void exp_accumulate(const float (&v)[N], float2 sc2, const float2 (&add2)[N / 2], float2 &accA, float2 &accB)
-{
-#pragma unroll
-    for (int pi = 0; pi < N / 2; ++pi) {
-        const float2 x = __ffma2_rn(make_float2(v[2 * pi], v[2 * pi + 1]), sc2, add2[pi]);
-        const float2 e = pair_on_fma(pi) ? ex2_fma2(x) : ex2_mufu2(x);
-        if (pi & 1) accB = __fadd2_rn(accB, e); else accA = __fadd2_rn(accA, e);
-    }
 }
 template <int D> struct ScaleLog2 {   // log2(e) / sqrt(D) as an immediate
     static constexpr float value = (D == 64) ? 0.18033688011112042f : (D == 128) ? 0.12751743082459868f : 0.09016844005556021f;
@@ -311,9 +250,11 @@ __device__ __forceinline__ void release_stage(uint32_t tempty, uint32_t stage, i
     if (lane == 0) mbar_arrive(tempty + 8 * stage);
 }
 
-// 2^x for a pair on the FMA pipe when x <= ~0 is known or watched by the caller: lower clamp only.  DEG = 4: 2.7e-6
-// relative; DEG = 3: 7.5e-5 relative (enough for the row normaliser of pass 1, which a 1e-3 contract divides by).
-template <int DEG>
+// 2^x for a PAIR of values on the FMA/ALU pipes with the packed fp32 instructions of sm_100 (FFMA2 / FADD2):
+// n = rint(x) through the 1.5*2^23 constant, f = x - n in [-0.5, 0.5], degree-4 minimax polynomial for 2^f (max
+// relative error 2.7e-6), exponent patched in with one shift-add per value.  Only the lower clamp is applied
+// (anything below -125 contributes < 2^-125 of the reference term); the caller knows x <= ~0 (pass 2) or watches
+// the largest exponent it sends here (pass 1), because x >= 128 would wrap the exponent field.
 __device__ __forceinline__ float2 ex2_fma2_lo(float2 x)
 {
     x.x = fmaxf(x.x, -125.0f);
@@ -321,17 +262,10 @@ __device__ __forceinline__ float2 ex2_fma2_lo(float2 x)
     const float2 t = __fadd2_rn(x, make_float2(12582912.0f, 12582912.0f));
     const float2 nf = __fadd2_rn(t, make_float2(-12582912.0f, -12582912.0f));
     const float2 f = __ffma2_rn(nf, make_float2(-1.0f, -1.0f), x);
-    float2 q;
-    if (DEG == 4) {
-        q = __ffma2_rn(f, make_float2(0.009570102207362652f, 0.009570102207362652f), make_float2(0.05591785907745361f, 0.05591785907745361f));
-        q = __ffma2_rn(q, f, make_float2(0.240247443318367f, 0.240247443318367f));
-        q = __ffma2_rn(q, f, make_float2(0.6931217908859253f, 0.6931217908859253f));
-        q = __ffma2_rn(q, f, make_float2(0.9999992847442627f, 0.9999992847442627f));
-    } else {
-        q = __ffma2_rn(f, make_float2(kP3c3, kP3c3), make_float2(kP3c2, kP3c2));
-        q = __ffma2_rn(q, f, make_float2(kP3c1, kP3c1));
-        q = __ffma2_rn(q, f, make_float2(kP3c0, kP3c0));
-    }
+    float2 q = __ffma2_rn(f, make_float2(0.009570102207362652f, 0.009570102207362652f), make_float2(0.05591785907745361f, 0.05591785907745361f));
+    q = __ffma2_rn(q, f, make_float2(0.240247443318367f, 0.240247443318367f));
+    q = __ffma2_rn(q, f, make_float2(0.6931217908859253f, 0.6931217908859253f));
+    q = __ffma2_rn(q, f, make_float2(0.9999992847442627f, 0.9999992847442627f));
     return make_float2(__int_as_float(__float_as_int(q.x) + (__float_as_int(t.x) << 23)),
                        __int_as_float(__float_as_int(q.y) + (__float_as_int(t.y) << 23)));
 }
@@ -375,9 +309,6 @@ __device__ __forceinline__ void rowstats_segment(const Params &p, const Seg &it,
         float xmax = kNegBig;                                             // largest exponent sent to the FMA pipe
         stream_tile<NCH, ACOLS>(bA, bB, base, k0 + kTileKeys < key_end, tfull, astage, aphase,
             [&](const uint32_t (&r)[16], int c) {
-#ifdef SKV_DBG_NOEXP
-                z += __uint_as_float(r[0]); return;
-#endif
                 if (c == 0 && m < 0.5f * kNegBig) {
                     float tmax = kNegBig;
 #pragma unroll
@@ -389,7 +320,7 @@ __device__ __forceinline__ void rowstats_segment(const Params &p, const Seg &it,
                 for (int pi = 0; pi < 8; ++pi) {
                     const float2 x = __ffma2_rn(make_float2(__uint_as_float(r[2 * pi]), __uint_as_float(r[2 * pi + 1])), sc2, nm2);
                     float2 e;
-                    if (pair_on_fma(pi)) { xmax = fmaxf(xmax, fmaxf(x.x, x.y)); e = ex2_fma2_lo<SKV_P1_DEG>(x); }
+                    if (pair_on_fma(pi)) { xmax = fmaxf(xmax, fmaxf(x.x, x.y)); e = ex2_fma2_lo(x); }
                     else e = ex2_mufu2(x);
                     if (pi & 1) accB = __fadd2_rn(accB, e); else accA = __fadd2_rn(accA, e);
                 }
@@ -479,9 +410,6 @@ __device__ __forceinline__ void colsum_segment(const Params &p, const Seg &it, u
         if (cols_full && k0 < mask_from) {                                // ---- fast tile
             float2 accA = make_float2(0.f, 0.f), accB = accA;
             auto chunk = [&](const uint32_t (&r)[16], int c) {
-#ifdef SKV_DBG_NOEXP
-                accA.x += __uint_as_float(r[0]); return;
-#endif
                 const float4 *l4 = reinterpret_cast<const float4 *>(sLse + cbeg + 16 * c);
                 const float2 sc2 = make_float2(sc, sc);
 #pragma unroll
@@ -489,8 +417,8 @@ __device__ __forceinline__ void colsum_segment(const Params &p, const Seg &it, u
                     const float4 L4 = l4[i];
                     const float2 x0 = __ffma2_rn(make_float2(__uint_as_float(r[4 * i]), __uint_as_float(r[4 * i + 1])), sc2, make_float2(L4.x, L4.y));
                     const float2 x1 = __ffma2_rn(make_float2(__uint_as_float(r[4 * i + 2]), __uint_as_float(r[4 * i + 3])), sc2, make_float2(L4.z, L4.w));
-                    accA = __fadd2_rn(accA, pair_on_fma2(2 * i) ? ex2_fma2_lo<4>(x0) : ex2_mufu2(x0));
-                    accB = __fadd2_rn(accB, pair_on_fma2(2 * i + 1) ? ex2_fma2_lo<4>(x1) : ex2_mufu2(x1));
+                    accA = __fadd2_rn(accA, pair_on_fma(2 * i) ? ex2_fma2_lo(x0) : ex2_mufu2(x0));
+                    accB = __fadd2_rn(accB, pair_on_fma(2 * i + 1) ? ex2_fma2_lo(x1) : ex2_mufu2(x1));
                 }
             };
             if (!par) stream_tile<QC, ACOLS>(bA, bB, base, more, tfull, astage, aphase, chunk);
@@ -532,39 +460,166 @@ __device__ __forceinline__ void colsum_segment(const Params &p, const Seg &it, u
     }
 }
 
-// V: pass 1 = 16-key chunks per thread per tile (2 or 4); pass 2 = 16-query-column chunks per thread per tile (1..4)
+// Shared-memory addresses and the pipeline cursors that survive from pass 1 to pass 2 (every barrier keeps counting
+// phases across the grid-wide barriers in between; all pipelines are empty at a pass boundary).
+struct Smem {
+    uint32_t sQ, sK, kfull, kempty, qfull, qempty, tfull, tempty, redfull;
+    float *sLse; int *sLim; float *sRed;
+};
+struct Cursors { uint32_t kstage, kphase, qphase, astage, aphase, rstage, rphase; };
+
+// One pass over this CTA's unit range.  V: pass 1 = 16-key chunks per thread per tile (2 or 4); pass 2 = 16-query-
+// column chunks per thread per tile (1..4).
 template <int D, int PASS, int V>
-__global__ void __launch_bounds__(kThreads, 1)
-imp_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmQ, const Params p)
+__device__ __forceinline__ void run_pass(const CUtensorMap *tmK, const CUtensorMap *tmQ, const Params &p, const Smem &sm,
+                                         uint32_t tmem, Cursors &cu, int warp, int lane)
 {
     using C = Cfg<D>;
     constexpr int ACOLS = (PASS == 1) ? (V == 4 ? 256 : 128) : (V >= 3 ? 256 : 128);   // TMEM columns per accumulator stage
     constexpr int ASTAGES = 512 / ACOLS;
+    const int n = p.g.n;
+    const long long ubeg = (long long)blockIdx.x * p.U / gridDim.x, uend = (long long)(blockIdx.x + 1) * p.U / gridDim.x;
+    if (warp == 0) {
+        // ===================== TMA producer =====================
+        if (lane == 0) {
+            for (long long u = ubeg; u < uend;) {
+                const Seg it = seg_at(p, u, uend);
+                u += it.t1 - it.t0;
+                mbar_wait(sm.qempty, cu.qphase ^ 1); cu.qphase ^= 1;
+                mbar_expect_tx(sm.qfull, (uint32_t)(p.qrows * D * 2));
+                for (int kb = 0; kb < C::KB; ++kb)
+                    tma_load_3d(sm.sQ + kb * C::Q_KB_STRIDE, tmQ, sm.qfull, kb * 64, it.rb * p.MB, (it.r * p.g.L + it.l) * p.g.Hkv + it.g);
+                for (int t = it.t0; t < it.t1; ++t) {
+                    mbar_wait(sm.kempty + 8 * cu.kstage, cu.kphase ^ 1);
+                    mbar_expect_tx(sm.kfull + 8 * cu.kstage, (uint32_t)C::K_BYTES);
+                    int c[5]; c[0] = 0;
+                    c[p.kdim[0]] = it.g; c[p.kdim[1]] = t * kTileKeys; c[p.kdim[2]] = it.l; c[p.kdim[3]] = it.r;
+                    for (int kb = 0; kb < C::KB; ++kb)
+                        tma_load_5d(sm.sK + cu.kstage * C::K_BYTES + kb * C::K_KB_STRIDE, tmK, sm.kfull + 8 * cu.kstage, kb * 64, c[1], c[2], c[3], c[4]);
+                    if (++cu.kstage == C::STAGES) { cu.kstage = 0; cu.kphase ^= 1; }
+                }
+            }
+        }
+        __syncwarp();          // lanes 1..31 wait here for the elected lane: the CTA-wide barriers that follow are warp-collective
+    } else if (warp == 1) {
+        // ===================== MMA issuer =====================
+        if (lane == 0) {
+            const uint32_t idesc = (PASS == 1) ? umma_idesc(128, kTileKeys, p.g.bf16) : umma_idesc(128, p.qrows, p.g.bf16);
+            for (long long u = ubeg; u < uend;) {
+                const Seg it = seg_at(p, u, uend);
+                u += it.t1 - it.t0;
+                mbar_wait(sm.qfull, cu.qphase); cu.qphase ^= 1;
+                for (int t = it.t0; t < it.t1; ++t) {
+                    mbar_wait(sm.tempty + 8 * cu.astage, cu.aphase ^ 1);
+                    mbar_wait(sm.kfull + 8 * cu.kstage, cu.kphase);
+                    tc_fence_after();
+                    const uint32_t kt = sm.sK + cu.kstage * C::K_BYTES;
+                    const uint32_t acc = tmem + cu.astage * ACOLS;
+                    if (PASS == 1) {
+#pragma unroll
+                        for (int hh = 0; hh < (V == 4 ? 2 : 1); ++hh)
+#pragma unroll
+                            for (int ks = 0; ks < D / 16; ++ks) {
+                                const uint32_t koff = (ks >> 2) * 1u, kin = (ks & 3) * 32u;
+                                umma_f16(acc + hh * 128, umma_desc(sm.sQ + koff * C::Q_KB_STRIDE + hh * (128 * 128) + kin),
+                                         umma_desc(kt + koff * C::K_KB_STRIDE + kin), idesc, ks > 0);
+                            }
+                    } else {
+#pragma unroll
+                        for (int ks = 0; ks < D / 16; ++ks) {
+                            const uint32_t koff = (ks >> 2) * 1u, kin = (ks & 3) * 32u;
+                            umma_f16(acc, umma_desc(kt + koff * C::K_KB_STRIDE + kin),
+                                     umma_desc(sm.sQ + koff * C::Q_KB_STRIDE + kin), idesc, ks > 0);
+                        }
+                    }
+                    umma_commit(sm.kempty + 8 * cu.kstage);    // smem stage free once these MMAs have read it
+                    umma_commit(sm.tfull + 8 * cu.astage);     // accumulator ready for the epilogue
+                    if (++cu.kstage == C::STAGES) { cu.kstage = 0; cu.kphase ^= 1; }
+                    if (++cu.astage == ASTAGES) { cu.astage = 0; cu.aphase ^= 1; }
+                }
+                umma_commit(sm.qempty);                        // Q buffer free once every MMA of the segment is done
+            }
+        }
+        __syncwarp();
+    } else {
+        // ===================== epilogue warps (2..17) =====================
+        // TMEM lane window of a warp is fixed by (warp id % 4); grp = which of the four warps on that window.
+        const int e = warp - 2, quad = warp & 3, grp = e >> 2;
+        const int etid = e * 32 + lane;                                   // 0..511 among the epilogue threads
+        const int G = p.g.Hq / p.g.Hkv, M = G * p.w;
+        for (long long u = ubeg; u < uend;) {
+            const Seg it = seg_at(p, u, uend);
+            u += it.t1 - it.t0;
+            const int64_t rowbase = ((int64_t)it.r * p.g.L + it.l) * p.g.Hq * p.w + (int64_t)it.g * M;
+            const int mrows = min(p.MB, M - it.rb * p.MB);
+            if (PASS == 1) {
+                rowstats_segment<D, (PASS == 1 ? V : 2)>(p, it, tmem, sm.tfull, sm.tempty, cu.astage, cu.aphase, quad, grp, lane, rowbase, mrows);
+            } else {
+                // per-segment column tables: lse2 of the block's query rows and their causal limits
+                epi_bar_sync();
+                for (int idx = etid; idx < p.qrows; idx += kEpiThreads) {
+                    const bool ok = idx < mrows;
+                    sm.sLse[idx] = ok ? -p.lse2[rowbase + it.rb * p.MB + idx] : 0.f;   // NEGATED lse2
+                    sm.sLim[idx] = ok ? (p.causal ? (n - p.w + ((it.rb * p.MB + idx) % p.w)) : (n - 1)) : -1;
+                }
+                epi_bar_sync();
+                float *out = p.apart + (((int64_t)it.r * p.g.L + it.l) * p.S + it.gb) * (int64_t)n;
+                colsum_segment<D, (PASS == 2 ? V : 1)>(p, it, tmem, sm.tfull, sm.tempty, sm.redfull, cu.astage, cu.aphase, cu.rstage, cu.rphase,
+                                                       quad, grp, lane, mrows, sm.sLse, sm.sLim, sm.sRed, out);
+            }
+        }
+    }
+}
+
+// The whole score in ONE cooperative launch of one persistent CTA per SM:
+//   pass 1 (row statistics)  | grid barrier |  lse2 per query row  | grid barrier |  pass 2 (column sums)  | grid
+//   barrier |  fixed-order sum over (KV head, row block), 1/(Hq w) and the recency decay.
+// TMEM, the mbarriers and the tensor-map fetch are set up once.  VA / VC: chunk counts of pass 1 / pass 2 (run_pass).
+// Grid-wide barrier of the persistent grid (every CTA is resident: cooperative launch).  The counter only grows:
+// the k-th barrier of the launch completes when it reaches k * gridDim.x.
+__device__ __forceinline__ void grid_barrier(unsigned int *counter, unsigned int target)
+{
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();                                                  // this CTA's global writes before the arrival
+        atomicAdd(counter, 1u);
+        unsigned int seen;
+        do {
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(counter) : "memory");
+        } while (seen < target);
+    }
+    __syncthreads();
+}
+
+template <int D, int VA, int VC>
+__global__ void __launch_bounds__(kThreads, 1)
+imp_fused_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmQ, const Params p,
+                 float lambda, float *__restrict__ importance)
+{
+    using C = Cfg<D>;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;       // 1024-B aligned (128-B swizzle atoms)
     uint8_t *gbase = smem_raw + (sbase - smem_u32(smem_raw));
-    const uint32_t sQ = sbase;
-    const uint32_t sK = sQ + C::Q_BYTES;
-    float *sLse = reinterpret_cast<float *>(gbase + C::Q_BYTES + C::STAGES * C::K_BYTES);
-    int *sLim = reinterpret_cast<int *>(sLse + 256);
-    float *sRed = reinterpret_cast<float *>(sLim + 256);
-    const uint32_t sBar = sK + C::STAGES * C::K_BYTES + 256 * 4 * 2 + C::RED_BYTES;
+    Smem sm;
+    sm.sQ = sbase;
+    sm.sK = sm.sQ + C::Q_BYTES;
+    sm.sLse = reinterpret_cast<float *>(gbase + C::Q_BYTES + C::STAGES * C::K_BYTES);
+    sm.sLim = reinterpret_cast<int *>(sm.sLse + 256);
+    sm.sRed = reinterpret_cast<float *>(sm.sLim + 256);
+    const uint32_t sBar = sm.sK + C::STAGES * C::K_BYTES + 256 * 4 * 2 + C::RED_BYTES;
     // barriers (8 bytes each): kfull[S], kempty[S], qfull, qempty, tfull[4], tempty[4], redfull[kRing]
-    const uint32_t kfull = sBar, kempty = sBar + 8 * C::STAGES;
-    const uint32_t qfull = sBar + 16 * C::STAGES, qempty = qfull + 8;
-    const uint32_t tfull = qempty + 8, tempty = tfull + 32;
-    const uint32_t redfull = tempty + 32;                               // column-group partials of a tile have landed
-    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(gbase + (redfull + 8 * kRing - sbase));
+    sm.kfull = sBar; sm.kempty = sBar + 8 * C::STAGES;
+    sm.qfull = sBar + 16 * C::STAGES; sm.qempty = sm.qfull + 8;
+    sm.tfull = sm.qempty + 8; sm.tempty = sm.tfull + 32;
+    sm.redfull = sm.tempty + 32;                                        // column-group partials of a tile have landed
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(gbase + (sm.redfull + 8 * kRing - sbase));
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int n = p.g.n;
-    const long long ubeg = (long long)blockIdx.x * p.U / gridDim.x, uend = (long long)(blockIdx.x + 1) * p.U / gridDim.x;
-
     if (warp == 0 && lane == 0) {
-        for (int s = 0; s < C::STAGES; ++s) { mbar_init(kfull + 8 * s, 1); mbar_init(kempty + 8 * s, 1); }
-        mbar_init(qfull, 1); mbar_init(qempty, 1);
-        for (int a = 0; a < 4; ++a) { mbar_init(tfull + 8 * a, 1); mbar_init(tempty + 8 * a, kEpiWarps); }
-        for (int a = 0; a < kRing; ++a) mbar_init(redfull + 8 * a, kEpiWarps - 4);
+        for (int s = 0; s < C::STAGES; ++s) { mbar_init(sm.kfull + 8 * s, 1); mbar_init(sm.kempty + 8 * s, 1); }
+        mbar_init(sm.qfull, 1); mbar_init(sm.qempty, 1);
+        for (int a = 0; a < 4; ++a) { mbar_init(sm.tfull + 8 * a, 1); mbar_init(sm.tempty + 8 * a, kEpiWarps); }
+        for (int a = 0; a < kRing; ++a) mbar_init(sm.redfull + 8 * a, kEpiWarps - 4);
         fence_barrier_init();
     }
     if (warp == 1) {
@@ -575,98 +630,45 @@ imp_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ C
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
+    Cursors cu = {0, 0, 0, 0, 0, 0, 0};
 
-    if (warp == 0) {
-        // ===================== TMA producer =====================
-        if (lane == 0) {
-            uint32_t kstage = 0, kphase = 0, qphase = 0;
-            for (long long u = ubeg; u < uend;) {
-                const Seg it = seg_at(p, u, uend);
-                u += it.t1 - it.t0;
-                mbar_wait(qempty, qphase ^ 1); qphase ^= 1;
-                mbar_expect_tx(qfull, (uint32_t)(p.qrows * D * 2));
-                for (int kb = 0; kb < C::KB; ++kb)
-                    tma_load_3d(sQ + kb * C::Q_KB_STRIDE, &tmQ, qfull, kb * 64, it.rb * p.MB, (it.r * p.g.L + it.l) * p.g.Hkv + it.g);
-                for (int t = it.t0; t < it.t1; ++t) {
-                    mbar_wait(kempty + 8 * kstage, kphase ^ 1);
-                    mbar_expect_tx(kfull + 8 * kstage, (uint32_t)C::K_BYTES);
-                    int c[5]; c[0] = 0;
-                    c[p.kdim[0]] = it.g; c[p.kdim[1]] = t * kTileKeys; c[p.kdim[2]] = it.l; c[p.kdim[3]] = it.r;
-                    for (int kb = 0; kb < C::KB; ++kb)
-                        tma_load_5d(sK + kstage * C::K_BYTES + kb * C::K_KB_STRIDE, &tmK, kfull + 8 * kstage, kb * 64, c[1], c[2], c[3], c[4]);
-                    if (++kstage == C::STAGES) { kstage = 0; kphase ^= 1; }
-                }
-            }
+    run_pass<D, 1, VA>(&tmK, &tmQ, p, sm, tmem, cu, warp, lane);
+    grid_barrier(p.gbar, gridDim.x);
+
+    {   // lse2[row] = m* + log2(sum_c z_c 2^(m_c - m*)) over the (reference exponent, sum) pairs of the row's pieces
+        const int64_t rows = (int64_t)p.g.R * p.g.L * p.g.Hq * p.w;
+        const int HW = p.g.Hq * p.w, M = (p.g.Hq / p.g.Hkv) * p.w;
+        constexpr int cs = (VA == 4) ? 2 : 4;
+        for (int64_t row = (int64_t)blockIdx.x * kThreads + threadIdx.x; row < rows; row += (int64_t)gridDim.x * kThreads) {
+            // which (request, layer, KV head, row block) the row belongs to, hence how many CTAs shared its tiles
+            const int rr = (int)(row % HW);
+            const long long rl = row / HW;
+            const int gb = (rr / M) * p.RB + (rr % M) / p.MB;
+            const long long first = (rl * p.S + gb) * (long long)p.T;
+            const int cnt = cs * ((int)(cta_of_unit(first + p.T - 1, p.U, gridDim.x) - cta_of_unit(first, p.U, gridDim.x)) + 1);
+            const float2 *q = p.partial + row * p.pmax;
+            float m = kNegBig;
+            for (int c = 0; c < cnt; ++c) m = fmaxf(m, q[c].x);
+            float z = 0.f;
+            for (int c = 0; c < cnt; ++c) z += q[c].y * exp2f(q[c].x - m);
+            const_cast<float *>(p.lse2)[row] = m + log2f(z);
         }
-    } else if (warp == 1) {
-        // ===================== MMA issuer =====================
-        if (lane == 0) {
-            uint32_t kstage = 0, kphase = 0, qphase = 0, astage = 0, aphase = 0;
-            const uint32_t idesc = (PASS == 1) ? umma_idesc(128, kTileKeys, p.g.bf16) : umma_idesc(128, p.qrows, p.g.bf16);
-            for (long long u = ubeg; u < uend;) {
-                const Seg it = seg_at(p, u, uend);
-                u += it.t1 - it.t0;
-                mbar_wait(qfull, qphase); qphase ^= 1;
-                for (int t = it.t0; t < it.t1; ++t) {
-                    mbar_wait(tempty + 8 * astage, aphase ^ 1);
-                    mbar_wait(kfull + 8 * kstage, kphase);
-                    tc_fence_after();
-                    const uint32_t kt = sK + kstage * C::K_BYTES;
-                    const uint32_t acc = tmem + astage * ACOLS;
-#ifdef SKV_DBG_NOMMA
-                    if (false) {} else if (false)
-#endif
-                    if (PASS == 1) {
-#pragma unroll
-                        for (int hh = 0; hh < (V == 4 ? 2 : 1); ++hh)
-#pragma unroll
-                            for (int ks = 0; ks < D / 16; ++ks) {
-                                const uint32_t koff = (ks >> 2) * 1u, kin = (ks & 3) * 32u;
-                                umma_f16(acc + hh * 128, umma_desc(sQ + koff * C::Q_KB_STRIDE + hh * (128 * 128) + kin),
-                                         umma_desc(kt + koff * C::K_KB_STRIDE + kin), idesc, ks > 0);
-                            }
-                    } else {
-#pragma unroll
-                        for (int ks = 0; ks < D / 16; ++ks) {
-                            const uint32_t koff = (ks >> 2) * 1u, kin = (ks & 3) * 32u;
-                            umma_f16(acc, umma_desc(kt + koff * C::K_KB_STRIDE + kin),
-                                     umma_desc(sQ + koff * C::Q_KB_STRIDE + kin), idesc, ks > 0);
-                        }
-                    }
-                    umma_commit(kempty + 8 * kstage);          // smem stage free once these MMAs have read it
-                    umma_commit(tfull + 8 * astage);           // accumulator ready for the epilogue
-                    if (++kstage == C::STAGES) { kstage = 0; kphase ^= 1; }
-                    if (++astage == ASTAGES) { astage = 0; aphase ^= 1; }
-                }
-                umma_commit(qempty);                           // Q buffer free once every MMA of the segment is done
-            }
-        }
-    } else {
-        // ===================== epilogue warps (2..17) =====================
-        // TMEM lane window of a warp is fixed by (warp id % 4); grp = which of the four warps on that window.
-        const int e = warp - 2, quad = warp & 3, grp = e >> 2;
-        const int etid = e * 32 + lane;                                   // 0..511 among the epilogue threads
-        const int G = p.g.Hq / p.g.Hkv, M = G * p.w;
-        uint32_t astage = 0, aphase = 0, rstage = 0, rphase = 0;
-        for (long long u = ubeg; u < uend;) {
-            const Seg it = seg_at(p, u, uend);
-            u += it.t1 - it.t0;
-            const int64_t rowbase = ((int64_t)it.r * p.g.L + it.l) * p.g.Hq * p.w + (int64_t)it.g * M;
-            const int mrows = min(p.MB, M - it.rb * p.MB);
-            if (PASS == 1) {
-                rowstats_segment<D, (PASS == 1 ? V : 2)>(p, it, tmem, tfull, tempty, astage, aphase, quad, grp, lane, rowbase, mrows);
-            } else {
-                // per-segment column tables: lse2 of the block's query rows and their causal limits
-                epi_bar_sync();
-                for (int idx = etid; idx < p.qrows; idx += kEpiThreads) {
-                    const bool ok = idx < mrows;
-                    sLse[idx] = ok ? -p.lse2[rowbase + it.rb * p.MB + idx] : 0.f;      // NEGATED lse2
-                    sLim[idx] = ok ? (p.causal ? (n - p.w + ((it.rb * p.MB + idx) % p.w)) : (n - 1)) : -1;
-                }
-                epi_bar_sync();
-                float *out = p.apart + (((int64_t)it.r * p.g.L + it.l) * p.S + it.gb) * (int64_t)n;
-                colsum_segment<D, (PASS == 2 ? V : 1)>(p, it, tmem, tfull, tempty, redfull, astage, aphase, rstage, rphase, quad, grp, lane, mrows, sLse, sLim, sRed, out);
-            }
+    }
+    grid_barrier(p.gbar, 2 * gridDim.x);
+
+    run_pass<D, 2, VC>(&tmK, &tmQ, p, sm, tmem, cu, warp, lane);
+    grid_barrier(p.gbar, 3 * gridDim.x);
+
+    {   // importance = (sum over (KV head, row block) partials in a fixed order) / (Hq w) * exp(-lambda (n-1-j))
+        const int64_t total = (int64_t)p.g.R * p.g.L * p.g.n;
+        const float norm = 1.0f / ((float)p.g.Hq * (float)p.w);
+        for (int64_t i = (int64_t)blockIdx.x * kThreads + threadIdx.x; i < total; i += (int64_t)gridDim.x * kThreads) {
+            const int64_t rl = i / p.g.n;
+            const int j = (int)(i - rl * p.g.n);
+            const float *a = p.apart + rl * p.S * (int64_t)p.g.n + j;
+            float sum = 0.f;
+            for (int s = 0; s < p.S; ++s) sum += a[(int64_t)s * p.g.n];
+            importance[i] = sum * norm * expf(-lambda * (float)(p.g.n - 1 - j));
         }
     }
     tc_fence_before();
@@ -675,19 +677,6 @@ imp_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ C
         tc_fence_after();
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" :: "r"(tmem) : "memory");
     }
-}
-
-__global__ void __launch_bounds__(256)
-imp_finish_kernel(Geom g, int w, float lambda, int S, const float *__restrict__ apart, float *__restrict__ importance)
-{
-    const int l = blockIdx.y, r = blockIdx.z;
-    const int j = blockIdx.x * 256 + threadIdx.x;
-    if (j >= g.n) return;
-    const float *a = apart + (((int64_t)r * g.L + l) * S) * (int64_t)g.n + j;
-    float sum = 0.f;
-    for (int s = 0; s < S; ++s) sum += a[(int64_t)s * g.n];            // fixed order: deterministic
-    const float norm = 1.0f / ((float)g.Hq * (float)w);
-    importance[((int64_t)r * g.L + l) * g.n + j] = sum * norm * expf(-lambda * (float)(g.n - 1 - j));
 }
 
 }  // namespace tc
@@ -712,7 +701,7 @@ static EncodeTiledFn get_encode_fn()
 struct TcPlan {
     int QROWS_MAX, RB, MB, qrows, halves, S, T, grid, pmax;
     long long U;
-    size_t partial_bytes, lse_bytes, apart_bytes;
+    size_t partial_bytes, lse_bytes, apart_bytes, bar_bytes;
 };
 
 constexpr int kPlanSMs = 148;                          // B200; the grid is planned on the host (the workspace query is host-only)
@@ -740,7 +729,8 @@ static TcPlan tc_plan(const Geom &g, int w)
     const size_t rows = (size_t)g.R * g.L * g.Hq * w;
     t.partial_bytes = (rows * t.pmax * sizeof(float2) + 255) & ~(size_t)255;
     t.lse_bytes = (rows * sizeof(float) + 255) & ~(size_t)255;
-    t.apart_bytes = (size_t)g.R * g.L * t.S * g.n * sizeof(float);
+    t.apart_bytes = ((size_t)g.R * g.L * t.S * g.n * sizeof(float) + 255) & ~(size_t)255;
+    t.bar_bytes = 256;
     return t;
 }
 
@@ -748,60 +738,32 @@ size_t importance_tc_ws_bytes(const Geom &g, int window)
 {
     if (g.Hkv <= 0 || g.Hq < g.Hkv || g.Hq % g.Hkv || window <= 0) return 0;
     const TcPlan t = tc_plan(g, window);
-    return t.partial_bytes + t.lse_bytes + t.apart_bytes;
+    return t.partial_bytes + t.lse_bytes + t.apart_bytes + t.bar_bytes;
 }
 
-// lse2[row] = M + log2(sum_c z_c 2^(m_c - M)) over the partial (reference exponent, sum) pairs of the row's pieces
-__global__ void imp_tc_combine_kernel(tc::Params p, int grid, int cs, int64_t rows, float *__restrict__ lse2)
-{
-    const int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (row >= rows) return;
-    // which (request, layer, KV head, row block) the query row belongs to, hence how many CTAs shared its tiles
-    const int HW = p.g.Hq * p.w, M = (p.g.Hq / p.g.Hkv) * p.w;
-    const int rr = (int)(row % HW);
-    const long long rl = row / HW;
-    const int gb = (rr / M) * p.RB + (rr % M) / p.MB;
-    const long long first = (rl * p.S + gb) * (long long)p.T;
-    const int pieces = (int)(tc::cta_of_unit(first + p.T - 1, p.U, grid) - tc::cta_of_unit(first, p.U, grid)) + 1;
-    const float2 *q = p.partial + row * p.pmax;
-    const int cnt = pieces * cs;
-    float m = tc::kNegBig;
-    for (int c = 0; c < cnt; ++c) m = fmaxf(m, q[c].x);
-    float z = 0.f;
-    for (int c = 0; c < cnt; ++c) z += q[c].y * exp2f(q[c].x - m);
-    lse2[row] = m + log2f(z);
-}
-
-template <int D, int PASS, int V>
-static cudaError_t launch_pass(const CUtensorMap &tmK, const CUtensorMap &tmQ, const tc::Params &p, int grid, cudaStream_t s)
+template <int D, int VA, int VC>
+static cudaError_t launch_fused(const CUtensorMap &tmK, const CUtensorMap &tmQ, const tc::Params &p, float lambda,
+                                float *importance, int grid, cudaStream_t s)
 {
     using C = tc::Cfg<D>;
-    cudaError_t e = cudaFuncSetAttribute(tc::imp_tc_kernel<D, PASS, V>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM);
+    cudaError_t e = cudaFuncSetAttribute(tc::imp_fused_kernel<D, VA, VC>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM);
     if (e != cudaSuccess) return e;
-    tc::imp_tc_kernel<D, PASS, V><<<grid, tc::kThreads, C::SMEM, s>>>(tmK, tmQ, p);
-    return cudaGetLastError();
+    void *args[] = {const_cast<CUtensorMap *>(&tmK), const_cast<CUtensorMap *>(&tmQ), const_cast<tc::Params *>(&p), &lambda, &importance};
+    // cooperative: the grid-wide barriers need every CTA resident (one per SM; the launch fails rather than deadlocks)
+    return cudaLaunchCooperativeKernel(reinterpret_cast<const void *>(tc::imp_fused_kernel<D, VA, VC>), dim3(grid), dim3(tc::kThreads),
+                                       args, C::SMEM, s);
 }
 
 template <int D>
-static cudaError_t launch_tc_t(const Geom &g, const CUtensorMap &tmK, const CUtensorMap &tmQ, tc::Params p, float lambda,
+static cudaError_t launch_tc_t(const CUtensorMap &tmK, const CUtensorMap &tmQ, const tc::Params &p, float lambda,
                                float *importance, int grid, cudaStream_t s)
 {
-    cudaError_t e;
-    e = (p.halves == 2) ? launch_pass<D, 1, 4>(tmK, tmQ, p, grid, s) : launch_pass<D, 1, 2>(tmK, tmQ, p, grid, s);
-    if (e != cudaSuccess) return e;
-    const int64_t rows = (int64_t)g.R * g.L * g.Hq * p.w;
-    imp_tc_combine_kernel<<<(unsigned)((rows + 255) / 256), 256, 0, s>>>(p, grid, p.halves == 2 ? 2 : 4, rows, const_cast<float *>(p.lse2));
-    if ((e = cudaGetLastError()) != cudaSuccess) return e;
-    switch (p.qrows >> 6) {
-    case 1:  e = launch_pass<D, 2, 1>(tmK, tmQ, p, grid, s); break;
-    case 2:  e = launch_pass<D, 2, 2>(tmK, tmQ, p, grid, s); break;
-    case 3:  e = launch_pass<D, 2, 3>(tmK, tmQ, p, grid, s); break;
-    default: e = launch_pass<D, 2, 4>(tmK, tmQ, p, grid, s); break;
+    switch (p.qrows >> 6) {          // 64-row quarters of the query block: 16-column chunks per thread in pass 2
+    case 1:  return launch_fused<D, 2, 1>(tmK, tmQ, p, lambda, importance, grid, s);
+    case 2:  return launch_fused<D, 2, 2>(tmK, tmQ, p, lambda, importance, grid, s);
+    case 3:  return launch_fused<D, 4, 3>(tmK, tmQ, p, lambda, importance, grid, s);
+    default: return launch_fused<D, 4, 4>(tmK, tmQ, p, lambda, importance, grid, s);
     }
-    if (e != cudaSuccess) return e;
-    dim3 gf((g.n + 255) / 256, g.L, g.R);
-    tc::imp_finish_kernel<<<gf, 256, 0, s>>>(g, p.w, lambda, p.S, p.apart, importance);
-    return cudaGetLastError();
 }
 
 // Returns cudaErrorNotSupported when the tensor maps cannot be built (reported as SKV_ERR_CUDA; there is no other path).
@@ -850,15 +812,17 @@ cudaError_t launch_importance_tc(const Geom &g, const __half *K, const __half *Q
     p.partial = reinterpret_cast<float2 *>(w8);
     p.lse2 = reinterpret_cast<const float *>(w8 + t.partial_bytes);
     p.apart = reinterpret_cast<float *>(w8 + t.partial_bytes + t.lse_bytes);
+    p.gbar = reinterpret_cast<unsigned int *>(w8 + t.partial_bytes + t.lse_bytes + t.apart_bytes);
+    if (cudaMemsetAsync(p.gbar, 0, sizeof(unsigned int), s) != cudaSuccess) return cudaGetLastError();
 
     int dev = 0, sms = kPlanSMs;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     const int grid = std::min(t.grid, sms);             // fewer CTAs than planned only lengthens the pieces: pmax still holds
     switch (g.D) {
-    case 64:  return launch_tc_t<64>(g, tmK, tmQ, p, lambda, importance, grid, s);
-    case 128: return launch_tc_t<128>(g, tmK, tmQ, p, lambda, importance, grid, s);
-    case 256: return launch_tc_t<256>(g, tmK, tmQ, p, lambda, importance, grid, s);
+    case 64:  return launch_tc_t<64>(tmK, tmQ, p, lambda, importance, grid, s);
+    case 128: return launch_tc_t<128>(tmK, tmQ, p, lambda, importance, grid, s);
+    case 256: return launch_tc_t<256>(tmK, tmQ, p, lambda, importance, grid, s);
     default: return cudaErrorInvalidValue;
     }
 }
