@@ -29,6 +29,7 @@ def lib():
         _lib.orc_float_to_bf16.argtypes = [C.c_float]
         _lib.orc_blob_bytes.restype = C.c_uint64
         _lib.orc_blob_bytes_low.restype = C.c_uint64
+        _lib.orc_blob_bytes_mode.restype = C.c_uint64
         _lib.orc_max_threads.restype = C.c_int
     return _lib
 
@@ -52,6 +53,7 @@ class Counts:
     budget_q4: int            # quarter-units; EIGHTH-units when low_bits == 2
     spent_q4: int
     low_bits: int = 4         # 4 = symmetric INT4 low tier (tier code 4); 2 = asymmetric 2-bit (tier code 2, NEXT-4)
+    mode: int = 0             # NEXT-4 bit flags: 1 = INT8 hot tier (P21), 2 = 2-bit tier in groups of 32 elements (P22)
 
     def arr(self):
         return (C.c_int64 * 6)(self.n16, self.n8, self.n4, self.n0, self.budget_q4, self.spent_q4)
@@ -78,17 +80,21 @@ def _mode(allow_int4):
     return 2 if (allow_int4 == 2 and allow_int4 is not True) else (1 if allow_int4 else 0)
 
 
-def tier_counts(n, b, n_sink=0, ranges=(), allow_int4=True):
+MODE_HOT_INT8 = 1      # P21: the hot tier ships INT8 (nothing at FP16; protected positions pinned to INT8)
+MODE_GROUP2 = 2        # P22: the 2-bit low tier is quantised in groups of 32 elements
+
+
+def tier_counts(n, b, n_sink=0, ranges=(), allow_int4=True, mode=0):
     """O2.  Returns (Counts, protected bitmap uint8[n]).  Raises ValueError on infeasible/invalid."""
     rng = np.asarray(ranges, dtype=np.int32).reshape(-1, 2)
     out = (C.c_int64 * 6)()
     prot = np.zeros(int(n), dtype=np.uint8)
-    rc = lib().orc_tier_counts(C.c_int64(int(n)), C.c_double(float(b)), C.c_int32(int(n_sink)),
-                               C.c_int32(len(rng)), _p(np.ascontiguousarray(rng)),
-                               C.c_int32(_mode(allow_int4)), out, _p(prot))
+    rc = lib().orc_tier_counts_mode(C.c_int64(int(n)), C.c_double(float(b)), C.c_int32(int(n_sink)),
+                                    C.c_int32(len(rng)), _p(np.ascontiguousarray(rng)),
+                                    C.c_int32(_mode(allow_int4)), C.c_int32(int(mode)), out, _p(prot))
     if rc != 0:
         raise ValueError(f"orc_tier_counts rc={rc}")
-    return Counts(*[int(v) for v in out], low_bits=2 if _mode(allow_int4) == 2 else 4), prot
+    return Counts(*[int(v) for v in out], low_bits=2 if _mode(allow_int4) == 2 else 4, mode=int(mode)), prot
 
 
 def _elems(x, bf16):
@@ -126,14 +132,15 @@ def assign(I, prot, counts: Counts):
     L, n = I.shape
     tier = np.empty((L, n), dtype=np.uint8)
     c4 = (C.c_int64 * 4)(counts.n16, counts.n8, counts.n4, counts.n0)
-    lib().orc_assign_low(C.c_int32(L), C.c_int64(n), _p(I), _p(prot), c4, C.c_int32(counts.low_bits), _p(tier))
+    lib().orc_assign_mode(C.c_int32(L), C.c_int64(n), _p(I), _p(prot), c4, C.c_int32(counts.low_bits),
+                          C.c_int32(counts.mode), _p(tier))
     return tier
 
 
 def blob_bytes(L, Hkv, d, n, counts: Counts) -> int:
     c4 = (C.c_int64 * 4)(counts.n16, counts.n8, counts.n4, counts.n0)
-    return int(lib().orc_blob_bytes_low(C.c_int32(L), C.c_int32(Hkv), C.c_int32(d), C.c_int64(n), c4,
-                                        C.c_int32(counts.low_bits)))
+    return int(lib().orc_blob_bytes_mode(C.c_int32(L), C.c_int32(Hkv), C.c_int32(d), C.c_int64(n), c4,
+                                         C.c_int32(counts.low_bits), C.c_int32(counts.mode)))
 
 
 def pack(K, V, tier, counts: Counts, allow_int4=True, bf16=False):
@@ -144,9 +151,9 @@ def pack(K, V, tier, counts: Counts, allow_int4=True, bf16=False):
     L, n, Hkv, d = K.shape
     assert V.shape == K.shape and tier.shape == (L, n)
     blob = np.empty(blob_bytes(L, Hkv, d, n, counts), dtype=np.uint8)
-    rc = lib().orc_pack_dt(C.c_int32(L), C.c_int32(Hkv), C.c_int32(d), C.c_int64(n), _p(K), _p(V),
-                           _p(tier), counts.arr(), C.c_int32(2 if counts.low_bits == 2 else _mode(allow_int4)), _p(blob),
-                           C.c_int32(1 if bf16 else 0))
+    rc = lib().orc_pack_mode(C.c_int32(L), C.c_int32(Hkv), C.c_int32(d), C.c_int64(n), _p(K), _p(V),
+                             _p(tier), counts.arr(), C.c_int32(2 if counts.low_bits == 2 else _mode(allow_int4)),
+                             C.c_int32(counts.mode), _p(blob), C.c_int32(1 if bf16 else 0))
     if rc != 0:
         raise ValueError(f"orc_pack rc={rc} (tier map does not match counts)")
     return blob

@@ -35,6 +35,14 @@
  *   2-bit tier (NEXT-4)     : hand-worked examples Z1..Z3, exact-rational codes, half-a-step error bound,
  *                             hand-written blob bytes; count ladder: closed-form identities only
  *   bfloat16 (NEXT-4)       : conversions exhaustively against torch; quantizer identities and bounds
+ *   INT8 hot tier (NEXT-4)  : tests/golden/hot_int8_counts.txt (the paper's worked fractions carry over below b = 1/2:
+ *                             Eq. 14; hand arithmetic for the protected and 2-bit rows),
+ *                             invariant sweep, O(n^2) brute-force ranking with the protected set pinned to INT8,
+ *                             empty FP16 segments, payload identity of Eq. 3
+ *   group-wise 2-bit (NEXT-4): tests/golden/group2_worked.txt (two groups on their own grids, hand-written code and
+ *                             record bytes, exact round trip, and the ungrouped result for contrast), per-group
+ *                             half-a-step error bound, record-segment closed form, reduction to the ungrouped
+ *                             quantiser when every group spans the same range
  *   KV-norm score (NEXT-1)  : hand-worked Pythagorean key vectors with integer norms and scores for lambda = 0, ln 2,
  *                             0.005 (tests/golden/kvnorm_worked.txt); scaling, permutation, zero-layer and decay properties
  * PARITY UNPINNED (conventions of this build with no external fixture):
@@ -42,7 +50,8 @@
  *   nibble order, segment order/alignment, tie direction, causal default,
  *   mean normalisation, per-layer map; the KV-norm score's choice of the L2 norm (P15: a reading; its arithmetic is
  *   pinned above); the fractions of the
- *   eighth-unit ladder of the 2-bit tier (P18: the paper prints none); the bf16 overflow rule (P20).
+ *   eighth-unit ladder of the 2-bit tier (P18: the paper prints none); the bf16 overflow rule (P20); that the INT8 hot
+ *   tier pins the protected set to INT8 and caps every budget above 1/2 at Uniform INT8 (P21); the group size 32 (P22).
  */
 #include <math.h>
 #include <stdint.h>
@@ -183,8 +192,12 @@ void orc_importance(int32_t L, int32_t Hq, int32_t Hkv, int32_t d, int64_t n, in
  * prot (nullable, [n]) receives the protected bitmap = [0,s) U ranges.
  * out = {n16, n8, n4, n0, Q, spent}.  Returns 0, -1 invalid argument, -3 infeasible.
  */
-int orc_tier_counts(int64_t n, double b, int32_t n_sink, int32_t n_ranges, const int32_t *ranges,
-                    int32_t allow_int4, int64_t out[6], uint8_t *prot)
+/* mode bit0 (NEXT-4, reading P21 of DESIGN.md; "the FP16 tier could be further compressed to INT8 (if
+ * the model is INT8-safe for high-importance tokens)"): the HOT tier ships INT8.  Nothing is sent at FP16 any more
+ * (n16 = 0), the protected set is pinned to -- and paid at -- INT8, and the greedy ladder of Eq. 14 runs over the two
+ * remaining costs 1/2 and 1/4 (1/2 and 1/8 with the 2-bit low tier); b >= 1/2 sends every token at INT8. */
+int orc_tier_counts_mode(int64_t n, double b, int32_t n_sink, int32_t n_ranges, const int32_t *ranges,
+                         int32_t allow_int4, int32_t mode, int64_t out[6], uint8_t *prot)
 {
     if (n <= 0 || !(b > 0.0) || n_sink < 0 || n_ranges < 0) return -1;
     if (b > 1.0) b = 1.0;
@@ -200,6 +213,23 @@ int orc_tier_counts(int64_t n, double b, int32_t n_sink, int32_t n_ranges, const
     for (int64_t j = 0; j < n; ++j) P += p[j];
     if (!prot) free(p);
 
+    if (mode & 1) {                              /* INT8 hot tier (P21) */
+        const int64_t unit = (allow_int4 == 2) ? 8 : 4;              /* eighths with the 2-bit low tier, else quarters */
+        const int64_t c8 = unit / 2;                                 /* cost of an INT8 token; a low-tier token costs 1 */
+        const int64_t Qh = (int64_t)floor((double)unit * b * (double)n + 1e-6);
+        const int64_t mh = n - P, Rh = Qh - c8 * P;                  /* budget left after paying INT8 for the protected set */
+        if (Rh < 0) return -3;
+        int64_t h8 = P, hl = 0, h0 = 0;
+        if (Rh >= c8 * mh) h8 = n;                                   /* b >= 1/2: everything INT8 */
+        else if (!allow_int4) { h8 = P + Rh / c8; h0 = n - h8; }     /* 2-tier: INT8 + drop */
+        else if (Rh >= mh) {                                         /* INT8 + low-tier mix (Eq. 14 with the costs above) */
+            const int64_t extra = (Rh - mh) / (c8 - 1);              /* each INT8 upgrade over the low tier costs c8 - 1 */
+            h8 = P + extra; hl = mh - extra;
+        } else { hl = Rh; h0 = mh - Rh; }                            /* low tier + drop */
+        out[0] = 0; out[1] = h8; out[2] = hl; out[3] = h0;
+        out[4] = Qh; out[5] = c8 * h8 + hl;
+        return 0;
+    }
     if (allow_int4 == 2) {
         /* NEXT-4 ("the INT4 tier could use KIVI-style asymmetric 2-bit quantization"): the low tier
          * costs c = 1/8, so the same greedy ladder runs in EIGHTH-units, 8 / 4 / 1 / 0 per token (reading P18). */
@@ -243,6 +273,12 @@ int orc_tier_counts(int64_t n, double b, int32_t n_sink, int32_t n_ranges, const
     return 0;
 }
 
+int orc_tier_counts(int64_t n, double b, int32_t n_sink, int32_t n_ranges, const int32_t *ranges,
+                    int32_t allow_int4, int64_t out[6], uint8_t *prot)
+{
+    return orc_tier_counts_mode(n, b, n_sink, n_ranges, ranges, allow_int4, 0, out, prot);
+}
+
 /* ------------------------------------------------------------------------ */
 /* O3. Selection (PAPER.md:216 "pinned before ranking", :240 Alg. 1 step 3, */
 /*     Prop. 1; tie-break reading P6)                           */
@@ -260,19 +296,22 @@ static int orc_item_cmp(const void *a, const void *b)
 }
 
 /* One layer: I[n], prot[n] -> tier[n]; counts = {n16,n8,n4,n0} from orc_tier_counts. */
+/* hot_code: the tier the protected positions are pinned to: 16, or 8 with the INT8 hot tier (P21; counts[0] = 0 then
+ * and the protected tokens are part of counts[1]). */
 static void orc_assign_layer_code(int64_t n, const float *I, const uint8_t *prot, const int64_t counts[4],
-                                  uint8_t low_code, uint8_t *tier)
+                                  uint8_t low_code, uint8_t hot_code, uint8_t *tier)
 {
     orc_item *it = (orc_item *)malloc((size_t)n * sizeof(orc_item));
     int64_t m = 0, P = 0;
     for (int64_t j = 0; j < n; ++j) {
-        if (prot[j]) { tier[j] = 16; ++P; continue; }
+        if (prot[j]) { tier[j] = hot_code; ++P; continue; }
         float key = I[j];
         if (!(key > 0.0f)) key = 0.0f;       /* NaN, negative, -0 -> +0 (lowest rank) */
         it[m].key = key; it[m].pos = j; ++m;
     }
     qsort(it, (size_t)m, sizeof(orc_item), orc_item_cmp);
-    const int64_t c16 = counts[0] - P, c8 = counts[1], c4 = counts[2];
+    const int64_t c16 = (hot_code == 16) ? counts[0] - P : 0;
+    const int64_t c8 = (hot_code == 16) ? counts[1] : counts[1] - P, c4 = counts[2];
     for (int64_t r = 0; r < m; ++r) {
         uint8_t t;
         if (r < c16) t = 16;
@@ -287,16 +326,23 @@ static void orc_assign_layer_code(int64_t n, const float *I, const uint8_t *prot
 void orc_assign_layer(int64_t n, const float *I, const uint8_t *prot, const int64_t counts[4],
                       uint8_t *tier)
 {
-    orc_assign_layer_code(n, I, prot, counts, 4, tier);
+    orc_assign_layer_code(n, I, prot, counts, 4, 16, tier);
 }
 
 /* low_bits: 4 = the low tier is symmetric INT4 (tier code 4); 2 = asymmetric 2-bit (tier code 2). */
-void orc_assign_low(int32_t L, int64_t n, const float *I, const uint8_t *prot, const int64_t counts[4],
-                    int32_t low_bits, uint8_t *tier)
+void orc_assign_mode(int32_t L, int64_t n, const float *I, const uint8_t *prot, const int64_t counts[4],
+                     int32_t low_bits, int32_t mode, uint8_t *tier)
 {
 #pragma omp parallel for schedule(dynamic, 1)
     for (int32_t l = 0; l < L; ++l)
-        orc_assign_layer_code(n, I + (size_t)l * n, prot, counts, (uint8_t)(low_bits == 2 ? 2 : 4), tier + (size_t)l * n);
+        orc_assign_layer_code(n, I + (size_t)l * n, prot, counts, (uint8_t)(low_bits == 2 ? 2 : 4),
+                              (uint8_t)((mode & 1) ? 8 : 16), tier + (size_t)l * n);
+}
+
+void orc_assign_low(int32_t L, int64_t n, const float *I, const uint8_t *prot, const int64_t counts[4],
+                    int32_t low_bits, uint8_t *tier)
+{
+    orc_assign_mode(L, n, I, prot, counts, low_bits, 0, tier);
 }
 
 void orc_assign(int32_t L, int64_t n, const float *I, const uint8_t *prot, const int64_t counts[4],
@@ -317,12 +363,17 @@ static uint64_t pad256(uint64_t x) { return (x + 255u) / 256u * 256u; }
 
 /* segment order: K16 V16 K8 V8 K4 V4 SK8 SV8 SK4 SV4.  With low_bits = 2 (NEXT-4) the low-tier segments hold four
  * 2-bit codes per byte and a (lo, hi) pair of fp16 records per head vector. */
-void orc_layout_low(int32_t L, int32_t Hkv, int32_t d, int64_t n, const int64_t counts[4], int32_t low_bits,
-                    orc_layout_t *lo)
+/* mode bit1 (NEXT-4, reading P22; "KIVI partitions keys and values into separate quantization groups"):
+ * the 2-bit low tier is quantised in GROUPS OF 32 consecutive elements of a head vector (token-local, so a token stays
+ * self-contained on the wire) and SK4 / SV4 hold one (lo, hi) pair per group: d/32 pairs per head vector. */
+#define ORC_GROUP2 32
+void orc_layout_mode(int32_t L, int32_t Hkv, int32_t d, int64_t n, const int64_t counts[4], int32_t low_bits,
+                     int32_t mode, orc_layout_t *lo)
 {
     const uint64_t n16 = (uint64_t)counts[0], n8 = (uint64_t)counts[1], n4 = (uint64_t)counts[2];
     const uint64_t H = (uint64_t)Hkv, D = (uint64_t)d;
-    const uint64_t cpb = (low_bits == 2) ? 4 : 2, rec = (low_bits == 2) ? 4 : 2;
+    const uint64_t cpb = (low_bits == 2) ? 4 : 2;
+    const uint64_t rec = (low_bits == 2) ? (((mode & 2) ? D / ORC_GROUP2 : 1) * 4) : 2;   /* record bytes per head vector */
     const uint64_t raw[10] = {
         n16 * H * D * 2, n16 * H * D * 2,      /* K16, V16 : f16            */
         n8 * H * D,      n8 * H * D,           /* K8,  V8  : i8             */
@@ -337,14 +388,26 @@ void orc_layout_low(int32_t L, int32_t Hkv, int32_t d, int64_t n, const int64_t 
     lo->total_bytes = lo->layer0_off + (uint64_t)L * lo->layer_stride;
 }
 
+void orc_layout_low(int32_t L, int32_t Hkv, int32_t d, int64_t n, const int64_t counts[4], int32_t low_bits,
+                    orc_layout_t *lo)
+{
+    orc_layout_mode(L, Hkv, d, n, counts, low_bits, 0, lo);
+}
+
 void orc_layout(int32_t L, int32_t Hkv, int32_t d, int64_t n, const int64_t counts[4], orc_layout_t *lo)
 {
     orc_layout_low(L, Hkv, d, n, counts, 4, lo);
 }
 
+uint64_t orc_blob_bytes_mode(int32_t L, int32_t Hkv, int32_t d, int64_t n, const int64_t counts[4], int32_t low_bits,
+                             int32_t mode)
+{
+    orc_layout_t lo; orc_layout_mode(L, Hkv, d, n, counts, low_bits, mode, &lo); return lo.total_bytes;
+}
+
 uint64_t orc_blob_bytes_low(int32_t L, int32_t Hkv, int32_t d, int64_t n, const int64_t counts[4], int32_t low_bits)
 {
-    orc_layout_t lo; orc_layout_low(L, Hkv, d, n, counts, low_bits, &lo); return lo.total_bytes;
+    return orc_blob_bytes_mode(L, Hkv, d, n, counts, low_bits, 0);
 }
 
 uint64_t orc_blob_bytes(int32_t L, int32_t Hkv, int32_t d, int64_t n, const int64_t counts[4])
@@ -472,19 +535,23 @@ void orc_dequantize2_vector(const uint8_t *q, int32_t d, uint16_t lo_bits, uint1
 /* ------------------------------------------------------------------------ */
 /* counts6 = {n16,n8,n4,n0,Q,spent}; blob must hold orc_blob_bytes(); written completely
  * (every pad byte zero).  Returns 0, or -1 if a layer's tier map disagrees with counts. */
-int orc_pack_dt(int32_t L, int32_t Hkv, int32_t d, int64_t n, const uint16_t *K, const uint16_t *V,
-                const uint8_t *tier, const int64_t counts6[6], int32_t allow_int4, uint8_t *blob, int32_t dtype)
+int orc_pack_mode(int32_t L, int32_t Hkv, int32_t d, int64_t n, const uint16_t *K, const uint16_t *V,
+                  const uint8_t *tier, const int64_t counts6[6], int32_t allow_int4, int32_t mode, uint8_t *blob, int32_t dtype)
 {
     const int low2 = (allow_int4 == 2);                  /* NEXT-4: the low tier is asymmetric 2-bit, tier code 2 */
-    orc_layout_t lo; orc_layout_low(L, Hkv, d, n, counts6, low2 ? 2 : 4, &lo);
+    const int32_t g2 = (low2 && (mode & 2)) ? ORC_GROUP2 : d;   /* elements per 2-bit quantisation group (P22) */
+    orc_layout_t lo; orc_layout_mode(L, Hkv, d, n, counts6, low2 ? 2 : 4, mode, &lo);
     memset(blob, 0, (size_t)lo.total_bytes);
     put_u32(blob + 0, 0x31564B53u);  put_u32(blob + 4, 1u);
     put_u32(blob + 8, (uint32_t)L);  put_u32(blob + 12, (uint32_t)Hkv);
     put_u32(blob + 16, (uint32_t)d); put_u32(blob + 20, (uint32_t)n);
     put_u32(blob + 24, (uint32_t)counts6[0]); put_u32(blob + 28, (uint32_t)counts6[1]);
     put_u32(blob + 32, (uint32_t)counts6[2]); put_u32(blob + 36, (uint32_t)counts6[3]);
-    /* flags: bit0 low tier allowed, bit1 it is 2-bit, bit2 the elements (and the scale records) are bfloat16 */
-    put_u32(blob + 40, (allow_int4 ? 1u : 0u) | (low2 ? 2u : 0u) | (dtype ? 4u : 0u)); put_u32(blob + 44, 0u);
+    /* flags: bit0 low tier allowed, bit1 it is 2-bit, bit2 the elements (and the scale records) are bfloat16,
+     * bit3 INT8 hot tier (P21), bit4 the 2-bit tier is quantised in groups of 32 elements (P22) */
+    put_u32(blob + 40, (allow_int4 ? 1u : 0u) | (low2 ? 2u : 0u) | (dtype ? 4u : 0u) | ((mode & 1) ? 8u : 0u) |
+                       ((low2 && (mode & 2)) ? 16u : 0u));
+    put_u32(blob + 44, 0u);
     put_u64(blob + 48, (uint64_t)counts6[4]);
     put_u64(blob + 56, lo.tier_map_off); put_u64(blob + 64, lo.layer0_off); put_u64(blob + 72, lo.layer_stride);
     for (int s = 0; s < 10; ++s) put_u64(blob + 80 + 8 * s, lo.seg_off[s]);
@@ -525,15 +592,16 @@ int orc_pack_dt(int32_t L, int32_t Hkv, int32_t d, int64_t n, const uint16_t *K,
                         sc[2 * h] = (uint8_t)ab; sc[2 * h + 1] = (uint8_t)(ab >> 8);
                     }
                 } else if (t == 2 && low2) {
+                    const size_t ng = row / (size_t)g2;  /* quantisation groups in the row: Hkv, or Hkv * d/32 (P22) */
                     uint8_t *dst = base + lo.seg_off[4 + kv] + (size_t)slot4 * row / 4;
-                    uint8_t *sc  = base + lo.seg_off[8 + kv] + (size_t)slot4 * Hkv * 4;
-                    for (int32_t h = 0; h < Hkv; ++h) {
+                    uint8_t *sc  = base + lo.seg_off[8 + kv] + (size_t)slot4 * ng * 4;
+                    for (size_t gi = 0; gi < ng; ++gi) {
                         uint16_t lb, hb;
-                        orc_quantize2_vector_dt(src + (size_t)h * d, d, &lb, &hb, (uint8_t *)q, dtype);
-                        for (int32_t c = 0; c < d; c += 4)   /* element 4i+k in bits 2k..2k+1 of byte i */
-                            dst[((size_t)h * d + c) / 4] = (uint8_t)((q[c] & 3) | ((q[c + 1] & 3) << 2) | ((q[c + 2] & 3) << 4) | ((q[c + 3] & 3) << 6));
-                        sc[4 * h] = (uint8_t)lb; sc[4 * h + 1] = (uint8_t)(lb >> 8);
-                        sc[4 * h + 2] = (uint8_t)hb; sc[4 * h + 3] = (uint8_t)(hb >> 8);
+                        orc_quantize2_vector_dt(src + gi * g2, g2, &lb, &hb, (uint8_t *)q, dtype);
+                        for (int32_t c = 0; c < g2; c += 4)  /* element 4i+k in bits 2k..2k+1 of byte i */
+                            dst[(gi * g2 + c) / 4] = (uint8_t)((q[c] & 3) | ((q[c + 1] & 3) << 2) | ((q[c + 2] & 3) << 4) | ((q[c + 3] & 3) << 6));
+                        sc[4 * gi] = (uint8_t)lb; sc[4 * gi + 1] = (uint8_t)(lb >> 8);
+                        sc[4 * gi + 2] = (uint8_t)hb; sc[4 * gi + 3] = (uint8_t)(hb >> 8);
                     }
                 }                                        /* t == 0: dropped, no bytes */
             }
@@ -546,6 +614,12 @@ int orc_pack_dt(int32_t L, int32_t Hkv, int32_t d, int64_t n, const uint16_t *K,
         }
     }
     return bad ? -1 : 0;
+}
+
+int orc_pack_dt(int32_t L, int32_t Hkv, int32_t d, int64_t n, const uint16_t *K, const uint16_t *V,
+                const uint8_t *tier, const int64_t counts6[6], int32_t allow_int4, uint8_t *blob, int32_t dtype)
+{
+    return orc_pack_mode(L, Hkv, d, n, K, V, tier, counts6, allow_int4, 0, blob, dtype);
 }
 
 int orc_pack(int32_t L, int32_t Hkv, int32_t d, int64_t n, const uint16_t *K, const uint16_t *V,
@@ -568,10 +642,14 @@ static int orc_unpack_impl(const uint8_t *blob, uint64_t blob_bytes, int32_t L, 
     int64_t counts[4] = { get_u32(blob + 24), get_u32(blob + 28), get_u32(blob + 32), get_u32(blob + 36) };
     if (counts[0] + counts[1] + counts[2] + counts[3] != n) return -5;
     const uint32_t flags = get_u32(blob + 40);
-    if (flags & ~7u) return -5;
+    if (flags & ~31u) return -5;
     const int low2 = (flags & 2u) != 0;                  /* NEXT-4: the low tier is asymmetric 2-bit */
     const int32_t dtype = (flags & 4u) ? 1 : 0;          /* NEXT-4: bfloat16 elements and records */
-    orc_layout_t lo; orc_layout_low(L, Hkv, d, n, counts, low2 ? 2 : 4, &lo);
+    if ((flags & 8u) && counts[0] != 0) return -5;       /* P21: with the INT8 hot tier nothing ships at FP16 */
+    if ((flags & 16u) && !low2) return -5;               /* P22: groups exist only in the 2-bit tier */
+    const int32_t mode = ((flags & 8u) ? 1 : 0) | ((flags & 16u) ? 2 : 0);
+    const int32_t g2 = (flags & 16u) ? ORC_GROUP2 : d;
+    orc_layout_t lo; orc_layout_mode(L, Hkv, d, n, counts, low2 ? 2 : 4, mode, &lo);
     if (get_u64(blob + 56) != lo.tier_map_off || get_u64(blob + 64) != lo.layer0_off ||
         get_u64(blob + 72) != lo.layer_stride || get_u64(blob + 160) != lo.total_bytes ||
         lo.total_bytes != blob_bytes) return -5;
@@ -602,13 +680,14 @@ static int orc_unpack_impl(const uint8_t *blob, uint64_t blob_bytes, int32_t L, 
                         orc_dequantize_vector_dt(q, d, 127, (uint16_t)(sc[2 * h] | (sc[2 * h + 1] << 8)), dst + (size_t)h * d, dtype);
                     }
                 } else if (t == 2 && low2) {
+                    const size_t ng = row / (size_t)g2;
                     const uint8_t *src = base + lo.seg_off[4 + kv] + (size_t)slot4 * row / 4;
-                    const uint8_t *sc  = base + lo.seg_off[8 + kv] + (size_t)slot4 * Hkv * 4;
-                    for (int32_t h = 0; h < Hkv; ++h) {
-                        for (int32_t c = 0; c < d; ++c)
-                            q[c] = (int8_t)((src[((size_t)h * d + c) / 4] >> (2 * (c & 3))) & 3);
-                        orc_dequantize2_vector_dt((const uint8_t *)q, d, (uint16_t)(sc[4 * h] | (sc[4 * h + 1] << 8)),
-                                                  (uint16_t)(sc[4 * h + 2] | (sc[4 * h + 3] << 8)), dst + (size_t)h * d, dtype);
+                    const uint8_t *sc  = base + lo.seg_off[8 + kv] + (size_t)slot4 * ng * 4;
+                    for (size_t gi = 0; gi < ng; ++gi) {
+                        for (int32_t c = 0; c < g2; ++c)
+                            q[c] = (int8_t)((src[(gi * g2 + c) / 4] >> (2 * (c & 3))) & 3);
+                        orc_dequantize2_vector_dt((const uint8_t *)q, g2, (uint16_t)(sc[4 * gi] | (sc[4 * gi + 1] << 8)),
+                                                  (uint16_t)(sc[4 * gi + 2] | (sc[4 * gi + 3] << 8)), dst + gi * g2, dtype);
                     }
                 } else if (t == 4 && !low2) {
                     const uint8_t *src = base + lo.seg_off[4 + kv] + (size_t)slot4 * row / 2;

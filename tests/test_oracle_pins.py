@@ -846,3 +846,170 @@ def test_bf16_blob_round_trip_and_fp16_tier_is_a_copy():
     b1 = oracle.pack(K, V, np.full((L, n), 16, np.uint8), c1, True, bf16=True)
     K3, V3, _ = oracle.unpack(b1, L, Hkv, d, n, bf16=True)
     assert np.array_equal(K3, K) and np.array_equal(V3, V)                                 # b = 1 identity
+
+
+# ----------------------------------------------------------------------------------------------
+# NEXT-4: INT8 hot tier (reading P21)
+# ----------------------------------------------------------------------------------------------
+def test_hot_int8_counts_golden_and_invariants():
+    for n, b, s, rb, re_, a4, n16, n8, n4, n0 in read_golden(os.path.join(GOLD, "hot_int8_counts.txt")):
+        ranges = [] if int(rb) == int(re_) else [(int(rb), int(re_))]
+        a = int(a4)
+        c, prot = oracle.tier_counts(int(n), float(b), int(s), ranges, a if a == 2 else bool(a), mode=oracle.MODE_HOT_INT8)
+        assert (c.n16, c.n8, c.n4, c.n0) == (int(n16), int(n8), int(n4), int(n0)), (n, b, s, a4, c)
+    rng = np.random.default_rng(21)
+    for _ in range(2000):
+        n = int(rng.integers(1, 5000)); s = int(rng.integers(0, min(n, 9))); b = float(rng.uniform(0.01, 1.2))
+        a4 = [False, True, 2][int(rng.integers(0, 3))]
+        unit = 8 if a4 == 2 else 4
+        try:
+            c, prot = oracle.tier_counts(n, b, s, [], a4, mode=oracle.MODE_HOT_INT8)
+        except ValueError:
+            assert (unit // 2) * s > int(np.floor(unit * min(b, 1.0) * n + 1e-6))       # the INT8 sinks alone do not fit
+            continue
+        P = int(prot.sum())
+        assert c.n16 == 0 and c.n8 >= P and c.n16 + c.n8 + c.n4 + c.n0 == n
+        assert c.budget_q4 == int(np.floor(unit * min(b, 1.0) * n + 1e-6))
+        assert c.spent_q4 == (unit // 2) * c.n8 + c.n4 <= c.budget_q4
+        if c.n8 < n:
+            assert c.budget_q4 - c.spent_q4 < max(1, unit // 2 - 1) or (not a4 and c.budget_q4 - c.spent_q4 < unit // 2)
+        if not a4:
+            assert c.n4 == 0
+        assert sum(x > 0 for x in (c.n8 - P, c.n4, c.n0)) <= 2                           # two adjacent tiers at most
+        # s = 0 and b <= 1/2: identical to the default ladder (Eq. 14 has no FP16 term there)
+        if s == 0 and b <= 0.5:
+            d, _ = oracle.tier_counts(n, b, 0, [], a4)
+            assert (d.n16, d.n8, d.n4, d.n0) == (c.n16, c.n8, c.n4, c.n0)
+
+
+def test_hot_int8_selection_brute_force_and_pinned_positions():
+    rng = np.random.default_rng(22)
+    for n, b, s, ranges, a4 in ((97, 0.3, 3, [(40, 47)], True), (200, 0.2, 4, [], True), (64, 0.4, 2, [(10, 12)], False),
+                                (130, 0.22, 5, [(100, 130)], 2)):
+        c, prot = oracle.tier_counts(n, b, s, ranges, a4, mode=oracle.MODE_HOT_INT8)
+        I = rng.random((2, n)).astype(np.float32)
+        I[0, :s] = 0.0                                                  # sinks with the lowest score still ship INT8
+        I[1, 7::9] = I[1, 5]                                            # ties
+        tier = oracle.assign(I, prot, c)
+        low = 2 if a4 == 2 else 4
+        for l in range(2):
+            free = np.flatnonzero(prot == 0)
+            key = np.where(I[l] > 0, I[l], 0.0)
+            rank = {int(j): sum(1 for k in free if key[k] > key[j] or (key[k] == key[j] and k < j)) for j in free}
+            P = int(prot.sum())
+            for j in range(n):
+                if prot[j]:
+                    want = 8
+                else:
+                    r = rank[j]
+                    want = 8 if r < c.n8 - P else low if r < c.n8 - P + c.n4 else 0
+                assert tier[l, j] == want, (n, l, j)
+            assert (tier[l] == 16).sum() == 0 and (tier[l] == 8).sum() == c.n8 and (tier[l] == low).sum() == c.n4
+
+
+def test_hot_int8_blob_has_no_fp16_segment_and_round_trips():
+    L, n, Hkv, d = 2, 40, 2, 64
+    rng = np.random.default_rng(23)
+    K = (rng.standard_normal((L, n, Hkv, d)) * 3).astype(np.float16); V = rng.standard_normal((L, n, Hkv, d)).astype(np.float16)
+    c, prot = oracle.tier_counts(n, 0.35, 4, [], True, mode=oracle.MODE_HOT_INT8)
+    tier = oracle.assign(rng.random((L, n)).astype(np.float32), prot, c)
+    assert (tier[:, :4] == 8).all()
+    blob = oracle.pack(K, V, tier, c, True)
+    assert int.from_bytes(bytes(blob[40:44]), "little") == 1 | 8                      # low tier allowed + INT8 hot tier
+    assert int.from_bytes(bytes(blob[24:28]), "little") == 0                          # n16
+    seg = [int.from_bytes(bytes(blob[80 + 8 * i:88 + 8 * i]), "little") for i in range(10)]
+    assert seg[0] == seg[1] == seg[2] == 0                                            # K16 and V16 occupy no bytes
+    # payload identity (Eq. 3 with c(8) = 1/2, c(4) = 1/4): code bytes = Bytes_FP16 * spent / (4 n)
+    code_bytes = 2 * L * Hkv * d * (c.n8 + c.n4 // 2 + (c.n4 % 2) * 0.5)
+    assert code_bytes == 2 * L * Hkv * d * n * 2 * c.spent_q4 / (4 * n)
+    K2, V2, t2 = oracle.unpack(blob, L, Hkv, d, n)
+    assert np.array_equal(t2, tier)
+    for l in range(L):
+        for j in range(n):
+            qm = {8: 127, 4: 7}.get(int(tier[l, j]))
+            for h in range(Hkv):
+                if qm is None:
+                    assert (K2[l, j, h] == 0).all()
+                else:
+                    ab, q = oracle.quantize_vector(K[l, j, h], qm)
+                    assert np.array_equal(K2[l, j, h].view(np.uint16), oracle.dequantize_vector(q, qm, ab).view(np.uint16))
+    # a blob that claims the INT8 hot tier but carries FP16 tokens is refused
+    bad = blob.copy(); bad[24] = 1; bad[28] -= 1
+    with pytest.raises(ValueError):
+        oracle.unpack(bad, L, Hkv, d, n)
+
+
+# ----------------------------------------------------------------------------------------------
+# NEXT-4: group-wise 2-bit low tier (reading P22)
+# ----------------------------------------------------------------------------------------------
+def test_group2_hand_worked_blob_and_what_grouping_buys():
+    rows = {r[0]: r for r in read_golden(os.path.join(GOLD, "group2_worked.txt"))}
+    L, n, Hkv, d = 1, 1, 1, 64
+    K = np.zeros((L, n, Hkv, d), np.float16)
+    K[0, 0, 0, :32] = np.tile([float(v) for v in rows["G0"][1:5]], 8)
+    K[0, 0, 0, 32:] = np.tile([float(v) for v in rows["G1"][1:5]], 8)
+    V = K[..., ::-1].copy()                                                           # groups swapped and reversed
+    tier = np.array([[2]], np.uint8)
+    cg = oracle.Counts(0, 0, 1, 0, 1, 1, low_bits=2, mode=oracle.MODE_GROUP2)
+    blob = oracle.pack(K, V, tier, cg, 2)
+    assert int.from_bytes(bytes(blob[40:44]), "little") == 1 | 2 | 16
+    seg = [int.from_bytes(bytes(blob[80 + 8 * i:88 + 8 * i]), "little") for i in range(10)]
+    # raw sizes: K2,V2 16 bytes of codes; SK2,SV2 two groups x 4 bytes = 8
+    assert seg == [0, 0, 0, 0, 0, 256, 512, 512, 512, 768]
+    base = 256 + 256
+    assert bytes(blob[base:base + 16]) == bytes([int(rows["G0"][7], 16)] * 8 + [int(rows["G1"][7], 16)] * 8)
+    rec = bytes(blob[base + 512:base + 520])
+    want = b"".join(int(rows[g][k], 16).to_bytes(2, "little") for g in ("G0", "G1") for k in (5, 6))
+    assert rec == want
+    # V: reversed pattern 6 2 -2 -6 | 3 2 1 0 -> codes 3 2 1 0 in both groups: 0b00011011 = 0x1B; records swapped
+    assert bytes(blob[base + 256:base + 272]) == bytes([0x1B] * 16)
+    assert bytes(blob[base + 768:base + 776]) == want[4:] + want[:4]
+    K2, V2, t2 = oracle.unpack(blob, L, Hkv, d, n)
+    assert np.array_equal(K2, K) and np.array_equal(V2, V)                            # every value sits on its group's grid
+    # the same vector without grouping: one (lo, hi) = (-6, 6) for all 64 values, group 0 collapses to the code of 2
+    cw = oracle.Counts(0, 0, 1, 0, 1, 1, low_bits=2)
+    blobw = oracle.pack(K, V, tier, cw, 2)
+    assert bytes(blobw[base:base + 8]) == bytes([int(rows["W"][7], 16)] * 8)
+    Kw, _, _ = oracle.unpack(blobw, L, Hkv, d, n)
+    assert (Kw[0, 0, 0, :32] == 2.0).all() and np.array_equal(Kw[0, 0, 0, 32:], K[0, 0, 0, 32:])
+
+
+def test_group2_layout_closed_form_error_bound_and_reduction_to_the_ungrouped_quantiser():
+    rng = np.random.default_rng(24)
+    pad = lambda x: (x + 255) // 256 * 256
+    for L, n, Hkv, d, n8, n2 in ((1, 9, 2, 64, 3, 4), (2, 33, 4, 128, 0, 33), (1, 17, 8, 256, 5, 7)):
+        cg = oracle.Counts(0, n8, n2, n - n8 - n2, 4 * n8 + n2, 4 * n8 + n2, low_bits=2, mode=oracle.MODE_GROUP2)
+        cw = oracle.Counts(0, n8, n2, n - n8 - n2, 4 * n8 + n2, 4 * n8 + n2, low_bits=2)
+        # only the record segments differ: d/32 (lo, hi) pairs per head vector instead of one
+        diff = L * 2 * (pad(n2 * Hkv * (d // 32) * 4) - pad(n2 * Hkv * 4))
+        assert oracle.blob_bytes(L, Hkv, d, n, cg) - oracle.blob_bytes(L, Hkv, d, n, cw) == diff
+        K = (rng.standard_normal((L, n, Hkv, d)) * rng.uniform(0.1, 20, (L, n, Hkv, 1))).astype(np.float16)
+        K[..., 5] *= 10                                                               # an outlier channel in group 0
+        V = rng.standard_normal((L, n, Hkv, d)).astype(np.float16)
+        tier = np.zeros((L, n), np.uint8); tier[:, :n8] = 8; tier[:, n8:n8 + n2] = 2
+        blob = oracle.pack(K, V, tier, cg, 2)
+        K2, V2, t2 = oracle.unpack(blob, L, Hkv, d, n)
+        assert np.array_equal(t2, tier)
+        X = K[:, n8:n8 + n2].astype(np.float64).reshape(L, n2, Hkv, d // 32, 32)
+        Y = K2[:, n8:n8 + n2].astype(np.float64).reshape(L, n2, Hkv, d // 32, 32)
+        step = (X.max(-1, keepdims=True) - X.min(-1, keepdims=True)) / 3.0               # per GROUP, from the definition
+        ulp = np.spacing(np.abs(Y).astype(np.float16)).astype(np.float64)
+        assert (np.abs(Y - X) <= step / 2 * (1 + 1e-3) + ulp / 2 + 1e-12).all()
+        # groups without the outlier are coded on their own, finer grid: their error is far below the ungrouped one
+        Kw, _, _ = oracle.unpack(oracle.pack(K, V, tier, cw, 2), L, Hkv, d, n)
+        eg = np.abs(Y - X)[..., 1:, :].mean(); ew = np.abs(Kw[:, n8:n8 + n2].astype(np.float64).reshape(X.shape) - X)[..., 1:, :].mean()
+        assert eg < 0.6 * ew
+    # special case that reduces to the ungrouped quantiser: every group of a vector spans the same (min, max)
+    L, n, Hkv, d = 1, 4, 2, 128
+    g = (rng.standard_normal((L, n, Hkv, 1, 32)) * 2).astype(np.float16)
+    K = np.tile(g, (1, 1, 1, d // 32, 1)).reshape(L, n, Hkv, d)
+    K = np.take_along_axis(K.reshape(L, n, Hkv, d // 32, 32), rng.permuted(np.tile(np.arange(32), (L, n, Hkv, d // 32, 1)), axis=-1), -1).reshape(L, n, Hkv, d)
+    tier = np.full((L, n), 2, np.uint8)
+    cg = oracle.Counts(0, 0, n, 0, n, n, low_bits=2, mode=oracle.MODE_GROUP2)
+    cw = oracle.Counts(0, 0, n, 0, n, n, low_bits=2)
+    bg, bw = oracle.pack(K, K, tier, cg, 2), oracle.pack(K, K, tier, cw, 2)
+    lay = lambda b: [int.from_bytes(bytes(b[80 + 8 * i:88 + 8 * i]), "little") for i in range(10)]
+    base = int.from_bytes(bytes(bg[64:72]), "little")
+    ncode = n * Hkv * d // 4
+    assert bytes(bg[base + lay(bg)[4]:base + lay(bg)[4] + ncode]) == bytes(bw[base + lay(bw)[4]:base + lay(bw)[4] + ncode])
+    assert np.array_equal(oracle.unpack(bg, L, Hkv, d, n)[0], oracle.unpack(bw, L, Hkv, d, n)[0])
