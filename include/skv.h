@@ -40,7 +40,8 @@
  * back at stride skv_blob_bytes(); the paper only says "mixed-precision payload"):
  *
  *   [0,256)  header: 0 u32 magic 0x31564B53 ("SKV1"), 4 u32 version = 1, 8 u32 L, 12 u32 Hkv, 16 u32 d_h,
- *            20 u32 n, 24 u32 n16, 28 u32 n8, 32 u32 n4, 36 u32 n0, 40 u32 flags (bit0 = allow_int4, bit1 = 2-bit low tier, bit2 = bfloat16),
+ *            20 u32 n, 24 u32 n16, 28 u32 n8, 32 u32 n4, 36 u32 n0, 40 u32 flags (bit0 = allow_int4, bit1 = 2-bit low tier,
+ *            bit2 = bfloat16, bit3 = INT8 hot tier, bit4 = 2-bit tier quantised in groups of 32 elements),
  *            44 u32 0, 48 u64 budget in quarter-units, 56 u64 tier_map_off (= 256), 64 u64 layer0_off,
  *            72 u64 layer_stride, 80 u64 seg_off[10] (relative to the layer block), 160 u64 total_bytes,
  *            168..255 zero
@@ -58,6 +59,20 @@
  * eighths).  Quantiser: lo = min x, hi = max x (a zero of either sign recorded as +0), r = fl32(hi - lo),
  * inv = fl32(3/r), step = fl32(r/3) (0 when r = 0); q = clamp(rint(fl32(x - lo) * inv), 0, 3), the product exact and
  * rounded once, half to even; y = f16_rn(fma(q, step, lo)).
+ *
+ * INT8 hot tier (NEXT-4; "the FP16 tier could be further compressed to INT8 (if the model is INT8-safe for high-
+ * importance tokens)"; reading P21 of DESIGN.md): with tier_mode bit0 (SKV_MODE_HOT_INT8) nothing ships
+ * at FP16.  n16 = 0, the protected positions are pinned to -- and paid at -- INT8 (tier code 8), and the greedy ladder
+ * of Eq. 14 runs over the costs 1/2 and 1/4 (1/2 and 1/8 with the 2-bit low tier): R = Q - 2P, m = n - P;
+ * R >= 2m: all INT8 (every b >= 1/2); m <= R < 2m: n8 = P + (R - m), n4 = 2m - R; R < m: n8 = P, n4 = R, rest dropped;
+ * 2-tier: n8 = P + floor(R/2), rest dropped.  Header flags bit3; K16 / V16 are empty.
+ *
+ * Group-wise 2-bit low tier (NEXT-4; "KIVI partitions keys and values into separate quantization groups",
+ * PAPER.md:583; reading P22): with tier_mode bit1 (SKV_MODE_GROUP2, needs allow_int4 = 2) the 2-bit quantiser above
+ * runs on every group of 32 consecutive elements of a head vector instead of on the whole vector (token-local, so a
+ * token stays self-contained on the wire); SK4 / SV4 hold d_h/32 (lo, hi) pairs per head vector, in element order.
+ * Header flags bit4.  The records cost 1 bit per element on top of the 2 bits of code (scale overhead outside b, as
+ * for every tier): a 2-bit token takes 3 bits per element on the wire instead of 2.25 (d_h = 128) or 2.125 (d_h = 256).
  *
  * Quantiser (one group = one head vector of d_h values; qmax = 127 / 7):
  *   amax = max|x| (an fp16 value, stored as the 2-byte scale record);
@@ -115,14 +130,17 @@ typedef struct {
     const int32_t *ranges;    /* HOST, n_ranges x [begin,end) half-open, forced FP16; read during the call only */
     int32_t allow_int4;       /* probe result: 1 = 3-tier, 0 = 2-tier FP16+INT8(+drop);
                                  2 = 3-tier whose low tier is asymmetric 2-bit (NEXT-4) */
+    int32_t tier_mode;        /* NEXT-4 bit flags, 0 = the paper's tiers: SKV_MODE_HOT_INT8, SKV_MODE_GROUP2 */
 } skv_policy;
+#define SKV_MODE_HOT_INT8 1   /* the hot tier ships INT8: no FP16 on the wire, protected positions pinned to INT8 (P21) */
+#define SKV_MODE_GROUP2 2     /* the 2-bit low tier is quantised in groups of 32 elements (P22); needs allow_int4 = 2 */
 
 /* Tier populations of ONE layer of ONE request (identical for every layer and request of a batch,
  * because n, b and the protected set are).  budget_q4 = floor(4bn + 1e-6), spent_q4 = 4n16+2n8+n4; with
  * allow_int4 = 2, n4 is the population of the 2-bit tier and both are in eighths: floor(8bn + 1e-6), 8n16+4n8+n4. */
 typedef struct {
     int32_t n16, n8, n4, n0;
-    int32_t allow_int4, reserved;
+    int32_t allow_int4, tier_mode;   /* tier_mode: the policy's NEXT-4 flags (0 = default); with SKV_MODE_HOT_INT8, n16 = 0 */
     int64_t budget_q4, spent_q4;
 } skv_counts;
 
@@ -164,7 +182,7 @@ int skv_assign_tiers(const skv_shape *shape, const skv_policy *policy, const flo
 /* DEVICE.  The same selection with EXPLICIT tier populations instead of a budget (ablation policies of PAPER.md:271,
  * :503 -- e.g. "Balanced", whose fractions the paper does not define; Random_Tier is skv_assign_tiers with random
  * scores).  counts: from skv_counts_from_populations(); positions [0,n_sink) and the n_ranges half-open ranges (HOST)
- * are FP16 and count towards n16 (SKV_ERR_BUDGET_INFEASIBLE if they exceed it).  The rest is ranked as in
+ * are FP16 and count towards n16 (INT8 and n8 with SKV_MODE_HOT_INT8; SKV_ERR_BUDGET_INFEASIBLE if they exceed it).  The rest is ranked as in
  * skv_assign_tiers: top n16-P -> 16, next n8 -> 8, next n4 -> low tier, rest -> 0. */
 int skv_assign_tiers_counts(const skv_shape *shape, const skv_counts *counts, int32_t n_sink, int32_t n_ranges,
                             const int32_t *ranges, const float *importance_dev, uint8_t *tier_map_dev,
@@ -201,7 +219,8 @@ int skv_unpack_patch(const skv_shape *shape, const void *blob_dev, size_t blob_b
 
 /* HOST only.  Counts for explicit tier populations (upgrade blobs, ablation policies): n0 = n - n16 - n8 - n4,
  * budget_q4 = spent_q4 = 4 n16 + 2 n8 + n4.  SKV_ERR_INVALID_ARG if the populations exceed n or n4 > 0 without
- * allow_int4. */
+ * allow_int4.  tier_mode of the result is 0; a caller that wants group-wise 2-bit codes or an INT8 hot tier (n16 = 0)
+ * sets counts_out->tier_mode itself. */
 int skv_counts_from_populations(const skv_shape *shape, int32_t n16, int32_t n8, int32_t n4, int32_t allow_int4,
                                 skv_counts *counts_out);
 

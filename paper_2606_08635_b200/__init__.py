@@ -41,12 +41,12 @@ class skv_shape(C.Structure):
 
 class skv_policy(C.Structure):
     _fields_ = [("budget", C.c_double), ("n_sink", C.c_int32), ("n_ranges", C.c_int32),
-                ("ranges", C.POINTER(C.c_int32)), ("allow_int4", C.c_int32)]
+                ("ranges", C.POINTER(C.c_int32)), ("allow_int4", C.c_int32), ("tier_mode", C.c_int32)]
 
 
 class skv_counts(C.Structure):
     _fields_ = [("n16", C.c_int32), ("n8", C.c_int32), ("n4", C.c_int32), ("n0", C.c_int32),
-                ("allow_int4", C.c_int32), ("reserved", C.c_int32),
+                ("allow_int4", C.c_int32), ("tier_mode", C.c_int32),
                 ("budget_q4", C.c_int64), ("spent_q4", C.c_int64)]
 
     def as_tuple(self):
@@ -54,7 +54,8 @@ class skv_counts(C.Structure):
 
     def __repr__(self):
         return (f"skv_counts(n16={self.n16}, n8={self.n8}, n4={self.n4}, n0={self.n0}, "
-                f"allow_int4={self.allow_int4}, budget_q4={self.budget_q4}, spent_q4={self.spent_q4})")
+                f"allow_int4={self.allow_int4}, tier_mode={self.tier_mode}, budget_q4={self.budget_q4}, "
+                f"spent_q4={self.spent_q4})")
 
 
 EXPORTS = ("skv_tier_counts", "skv_blob_bytes", "skv_workspace_bytes", "skv_blob_check", "skv_importance",
@@ -128,10 +129,14 @@ def _low_mode(allow_int4):
     return 2 if (allow_int4 == 2 and allow_int4 is not True) else (1 if allow_int4 else 0)
 
 
-def make_policy(budget, n_sink=0, ranges=(), allow_int4=True):
+SKV_MODE_HOT_INT8, SKV_MODE_GROUP2 = 1, 2      # skv_policy.tier_mode / skv_counts.tier_mode bit flags (NEXT-4)
+
+
+def make_policy(budget, n_sink=0, ranges=(), allow_int4=True, tier_mode=0):
     flat = [int(v) for r in ranges for v in r]
     arr = (C.c_int32 * max(1, len(flat)))(*flat)
-    p = skv_policy(float(budget), int(n_sink), len(flat) // 2, C.cast(arr, C.POINTER(C.c_int32)), _low_mode(allow_int4))
+    p = skv_policy(float(budget), int(n_sink), len(flat) // 2, C.cast(arr, C.POINTER(C.c_int32)), _low_mode(allow_int4),
+                   int(tier_mode))
     p._keepalive = arr
     return p
 

@@ -27,6 +27,7 @@ struct Geom {
     int32_t patch;               // unpack only: 1 = tokens the blob does not carry (tier 0) are left untouched
     int32_t low_code;            // tier code of the low tier: 4 (symmetric INT4) or 2 (asymmetric 2-bit, NEXT-4)
     int32_t bf16;                // element type of the dense caches and of the scale records: 0 = fp16, 1 = bfloat16
+    int32_t low_group;           // 2-bit low tier: 0 = one (lo, hi) record per head vector, 32 = one per 32 elements (P22)
 };
 
 constexpr int kTileTokens = 32;  // tokens per pack/unpack tile (one ballot word)
@@ -36,7 +37,7 @@ struct Header256 { uint32_t w[64]; };   // the 256-byte SKV1 header image, built
 static inline __host__ __device__ uint64_t pad256(uint64_t x) { return (x + 255ull) & ~255ull; }
 
 // host helpers (skv_host.cu)
-Layout make_layout(int L, int Hkv, int D, int64_t n, int64_t n16, int64_t n8, int64_t n4, int low_bits);
+Layout make_layout(int L, int Hkv, int D, int64_t n, int64_t n16, int64_t n8, int64_t n4, int low_bits, int low_group = 0);
 
 // launchers (one per .cu)
 cudaError_t launch_tile_scan_pack(const Geom &g, const Layout &lo, const uint8_t *tier_map, uint8_t *blob,

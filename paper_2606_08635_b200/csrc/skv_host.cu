@@ -13,11 +13,13 @@ namespace skv {
 
 // low_bits: 4 = the low tier holds symmetric INT4 codes (two per byte, one fp16 amax record per head vector);
 // 2 = asymmetric 2-bit codes (four per byte, an fp16 (lo, hi) pair per head vector) -- NEXT-4.
-Layout make_layout(int L, int Hkv, int D, int64_t n, int64_t n16, int64_t n8, int64_t n4, int low_bits)
+// low_group (2-bit tier only): 0 = one record per head vector, 32 = one per group of 32 elements (reading P22).
+Layout make_layout(int L, int Hkv, int D, int64_t n, int64_t n16, int64_t n8, int64_t n4, int low_bits, int low_group)
 {
     Layout lo;
     const uint64_t H = (uint64_t)Hkv, d = (uint64_t)D;
-    const uint64_t cpb = low_bits == 2 ? 4 : 2, rec = low_bits == 2 ? 4 : 2;
+    const uint64_t cpb = low_bits == 2 ? 4 : 2;
+    const uint64_t rec = low_bits == 2 ? (low_group ? d / (uint64_t)low_group : 1) * 4 : 2;     // record bytes per head vector
     const uint64_t raw[10] = {
         (uint64_t)n16 * H * d * 2, (uint64_t)n16 * H * d * 2,
         (uint64_t)n8 * H * d,      (uint64_t)n8 * H * d,
@@ -74,6 +76,7 @@ static Geom make_geom(const skv_shape *s, const skv_counts *c)
     g.patch = 0;
     g.low_code = (c && c->allow_int4 == 2) ? 2 : 4;
     g.bf16 = s->dtype == SKV_BF16 ? 1 : 0;
+    g.low_group = (c && c->allow_int4 == 2 && (c->tier_mode & SKV_MODE_GROUP2)) ? 32 : 0;
     return g;
 }
 
@@ -86,8 +89,10 @@ static bool counts_ok(const skv_shape *s, const skv_counts *c)
 // what skv_blob_check would refuse on the decode side: a low tier without the flag, or a budget the populations exceed
 static bool counts_wire_ok(const skv_shape *s, const skv_counts *c)
 {
-    if (!counts_ok(s, c) || c->allow_int4 < 0 || c->allow_int4 > 2 || c->reserved != 0) return false;
+    if (!counts_ok(s, c) || c->allow_int4 < 0 || c->allow_int4 > 2 || (c->tier_mode & ~3)) return false;
     if (c->allow_int4 == 0 && c->n4 != 0) return false;
+    if ((c->tier_mode & SKV_MODE_HOT_INT8) && c->n16 != 0) return false;        // INT8 hot tier: nothing ships at FP16
+    if ((c->tier_mode & SKV_MODE_GROUP2) && c->allow_int4 != 2) return false;   // groups exist only in the 2-bit tier
     const int64_t unit = c->allow_int4 == 2 ? 8 : 4;
     const int64_t spent = unit * c->n16 + (unit / 2) * c->n8 + c->n4;
     return c->budget_q4 >= spent && c->budget_q4 <= unit * (int64_t)s->n_tokens;
@@ -133,6 +138,23 @@ static int tier_counts_impl(const skv_shape *s, const skv_policy *p, skv_counts 
     if (P < 0) return SKV_ERR_INVALID_ARG;
     const int64_t n = s->n_tokens;
     if (p->allow_int4 != 0 && p->allow_int4 != 1 && p->allow_int4 != 2) return SKV_ERR_INVALID_ARG;
+    if ((p->tier_mode & ~3) || ((p->tier_mode & SKV_MODE_GROUP2) && p->allow_int4 != 2)) return SKV_ERR_INVALID_ARG;
+    if (p->tier_mode & SKV_MODE_HOT_INT8) {
+        // NEXT-4, reading P21: the hot tier ships INT8.  Costs c8 (INT8) and 1 (low tier) in quarter- or eighth-units.
+        const int64_t unit = p->allow_int4 == 2 ? 8 : 4, c8 = unit / 2;
+        const int64_t Q = (int64_t)floor((double)unit * b * (double)n + 1e-6);
+        const int64_t m = n - P, R = Q - c8 * P;
+        if (R < 0) return SKV_ERR_BUDGET_INFEASIBLE;
+        int64_t n8 = P, nl = 0, n0 = 0;
+        if (R >= c8 * m) n8 = n;
+        else if (!p->allow_int4) { n8 = P + R / c8; n0 = n - n8; }
+        else if (R >= m) { const int64_t up = (R - m) / (c8 - 1); n8 = P + up; nl = m - up; }
+        else { nl = R; n0 = m - R; }
+        c->n16 = 0; c->n8 = (int32_t)n8; c->n4 = (int32_t)nl; c->n0 = (int32_t)n0;
+        c->allow_int4 = p->allow_int4; c->tier_mode = p->tier_mode;
+        c->budget_q4 = Q; c->spent_q4 = c8 * n8 + nl;
+        return SKV_OK;
+    }
     if (p->allow_int4 == 2) {
         // NEXT-4: 2-bit low tier, c = 1/8 -> the same greedy ladder in EIGHTH-units, 8 / 4 / 1 / 0 per token
         const int64_t Q8 = (int64_t)floor(8.0 * b * (double)n + 1e-6);
@@ -144,7 +166,7 @@ static int tier_counts_impl(const skv_shape *s, const skv_policy *p, skv_counts 
         else if (R8 >= m8) { a8 = (R8 - m8) / 3; a2 = m8 - a8; }
         else { a2 = R8; a0 = m8 - R8; }
         c->n16 = (int32_t)a16; c->n8 = (int32_t)a8; c->n4 = (int32_t)a2; c->n0 = (int32_t)a0;
-        c->allow_int4 = 2; c->reserved = 0;
+        c->allow_int4 = 2; c->tier_mode = p->tier_mode;
         c->budget_q4 = Q8; c->spent_q4 = 8 * a16 + 4 * a8 + a2;
         return SKV_OK;
     }
@@ -159,7 +181,7 @@ static int tier_counts_impl(const skv_shape *s, const skv_policy *p, skv_counts 
         else { n4 = R; n0 = m - R; }
     } else { n8 = R / 2; n0 = m - n8; }
     c->n16 = (int32_t)n16; c->n8 = (int32_t)n8; c->n4 = (int32_t)n4; c->n0 = (int32_t)n0;
-    c->allow_int4 = p->allow_int4 ? 1 : 0; c->reserved = 0;
+    c->allow_int4 = p->allow_int4 ? 1 : 0; c->tier_mode = 0;
     c->budget_q4 = Q; c->spent_q4 = 4 * n16 + 2 * n8 + n4;
     return SKV_OK;
 }
@@ -184,8 +206,10 @@ int skv_tier_counts(const skv_shape *shape, const skv_policy *policy, skv_counts
 size_t skv_blob_bytes(const skv_shape *shape, const skv_counts *counts)
 {
     if (!dims_ok(shape) || !counts_ok(shape, counts)) return 0;
+    const bool low2 = counts->allow_int4 == 2;
     return (size_t)make_layout(shape->n_layers, shape->n_kv_heads, shape->head_dim, shape->n_tokens,
-                               counts->n16, counts->n8, counts->n4, counts->allow_int4 == 2 ? 2 : 4).total_bytes;
+                               counts->n16, counts->n8, counts->n4, low2 ? 2 : 4,
+                               (low2 && (counts->tier_mode & SKV_MODE_GROUP2)) ? 32 : 0).total_bytes;
 }
 
 size_t skv_workspace_bytes(const skv_shape *shape, int32_t window)
@@ -216,10 +240,12 @@ int skv_blob_check(const void *header_host, size_t blob_bytes, skv_shape *shape_
     const uint32_t flags = get32(h + 40);
     if (L == 0 || Hkv == 0 || n == 0 || L > 65535u || n > (1u << 20) || Hkv > 65535u) return SKV_ERR_BAD_BLOB;
     if (D != 64 && D != 128 && D != 256) return SKV_ERR_BAD_BLOB;
-    if ((uint64_t)n16 + n8 + n4 + n0 != n || (flags & ~7u) || (flags & 3u) == 2u || get32(h + 44) != 0) return SKV_ERR_BAD_BLOB;
+    if ((uint64_t)n16 + n8 + n4 + n0 != n || (flags & ~31u) || (flags & 3u) == 2u || get32(h + 44) != 0) return SKV_ERR_BAD_BLOB;
     if (!(flags & 1u) && n4 != 0) return SKV_ERR_BAD_BLOB;
     const bool low2 = (flags & 2u) != 0;                    // bit1: the low tier is asymmetric 2-bit (budget in eighths)
-    const Layout lo = make_layout((int)L, (int)Hkv, (int)D, n, n16, n8, n4, low2 ? 2 : 4);
+    if ((flags & 8u) && n16 != 0) return SKV_ERR_BAD_BLOB;  // bit3: INT8 hot tier, nothing ships at FP16
+    if ((flags & 16u) && !low2) return SKV_ERR_BAD_BLOB;    // bit4: 2-bit groups of 32 elements
+    const Layout lo = make_layout((int)L, (int)Hkv, (int)D, n, n16, n8, n4, low2 ? 2 : 4, (flags & 16u) ? 32 : 0);
     if (get64(h + 56) != lo.tier_map_off || get64(h + 64) != lo.layer0_off || get64(h + 72) != lo.layer_stride ||
         get64(h + 160) != lo.total_bytes || lo.total_bytes != blob_bytes) return SKV_ERR_BAD_BLOB;
     for (int s = 0; s < 10; ++s) if (get64(h + 80 + 8 * s) != lo.seg_off[s]) return SKV_ERR_BAD_BLOB;
@@ -236,7 +262,8 @@ int skv_blob_check(const void *header_host, size_t blob_bytes, skv_shape *shape_
     }
     if (counts_out) {
         counts_out->n16 = (int32_t)n16; counts_out->n8 = (int32_t)n8; counts_out->n4 = (int32_t)n4; counts_out->n0 = (int32_t)n0;
-        counts_out->allow_int4 = low2 ? 2 : (int32_t)(flags & 1u); counts_out->reserved = 0;
+        counts_out->allow_int4 = low2 ? 2 : (int32_t)(flags & 1u);
+        counts_out->tier_mode = ((flags & 8u) ? SKV_MODE_HOT_INT8 : 0) | ((flags & 16u) ? SKV_MODE_GROUP2 : 0);
         counts_out->budget_q4 = (int64_t)Q; counts_out->spent_q4 = (int64_t)spent;
     }
     return SKV_OK;
@@ -319,7 +346,9 @@ int skv_assign_tiers_counts(const skv_shape *shape, const skv_counts *counts, in
     std::vector<std::pair<int32_t, int32_t>> prot;
     const int64_t P = merge_protected(shape, &pol, prot);
     if (P < 0) return SKV_ERR_INVALID_ARG;
-    if (P > counts->n16) return SKV_ERR_BUDGET_INFEASIBLE;            // the protected positions are all FP16
+    // the protected positions all sit in the hot tier (FP16, or INT8 with SKV_MODE_HOT_INT8)
+    if (P > ((counts->tier_mode & SKV_MODE_HOT_INT8) ? counts->n8 : counts->n16)) return SKV_ERR_BUDGET_INFEASIBLE;
+    if ((counts->tier_mode & SKV_MODE_HOT_INT8) && counts->n16 != 0) return SKV_ERR_INVALID_ARG;
     return assign_launch(shape, *counts, prot, importance_dev, tier_map_dev, ws, ws_bytes, cuda_stream);
 }
 
@@ -331,7 +360,7 @@ int skv_pack(const skv_shape *shape, const void *K_dev, const void *V_dev, const
     if (!tier_map_dev || !blob_dev || !ws || !counts_wire_ok(shape, counts)) return SKV_ERR_INVALID_ARG;
     if ((uintptr_t)blob_dev & 255) return SKV_ERR_UNSUPPORTED;
     const Geom g = make_geom(shape, counts);
-    const Layout lo = make_layout(g.L, g.Hkv, g.D, g.n, g.n16, g.n8, g.n4, g.low_code);
+    const Layout lo = make_layout(g.L, g.Hkv, g.D, g.n, g.n16, g.n8, g.n4, g.low_code, g.low_group);
     if (blob_capacity < (size_t)lo.total_bytes * (size_t)g.R) return SKV_ERR_BUFFER_TOO_SMALL;
     if (ws_bytes < scan_ws_bytes(shape)) return SKV_ERR_BUFFER_TOO_SMALL;
 
@@ -341,7 +370,8 @@ int skv_pack(const skv_shape *shape, const void *K_dev, const void *V_dev, const
     put32(h + 0, 0x31564B53u); put32(h + 4, 1u);
     put32(h + 8, (uint32_t)g.L); put32(h + 12, (uint32_t)g.Hkv); put32(h + 16, (uint32_t)g.D); put32(h + 20, (uint32_t)g.n);
     put32(h + 24, (uint32_t)g.n16); put32(h + 28, (uint32_t)g.n8); put32(h + 32, (uint32_t)g.n4); put32(h + 36, (uint32_t)g.n0);
-    put32(h + 40, (counts->allow_int4 ? 1u : 0u) | (counts->allow_int4 == 2 ? 2u : 0u) | (g.bf16 ? 4u : 0u));
+    put32(h + 40, (counts->allow_int4 ? 1u : 0u) | (counts->allow_int4 == 2 ? 2u : 0u) | (g.bf16 ? 4u : 0u) |
+                  ((counts->tier_mode & SKV_MODE_HOT_INT8) ? 8u : 0u) | (g.low_group ? 16u : 0u));
     put64(h + 48, (uint64_t)counts->budget_q4);
     put64(h + 56, lo.tier_map_off); put64(h + 64, lo.layer0_off); put64(h + 72, lo.layer_stride);
     for (int s = 0; s < 10; ++s) put64(h + 80 + 8 * s, lo.seg_off[s]);
@@ -365,7 +395,7 @@ static int unpack_impl(const skv_shape *shape, const void *blob_dev, size_t blob
     if ((uintptr_t)blob_dev & 255) return SKV_ERR_UNSUPPORTED;
     Geom g = make_geom(shape, counts);
     g.patch = patch;
-    const Layout lo = make_layout(g.L, g.Hkv, g.D, g.n, g.n16, g.n8, g.n4, g.low_code);
+    const Layout lo = make_layout(g.L, g.Hkv, g.D, g.n, g.n16, g.n8, g.n4, g.low_code, g.low_group);
     if (blob_bytes != (size_t)lo.total_bytes) return SKV_ERR_BAD_BLOB;
     if (ws_bytes < scan_ws_bytes(shape)) return SKV_ERR_BUFFER_TOO_SMALL;
     cudaStream_t st = (cudaStream_t)cuda_stream;

@@ -137,8 +137,9 @@ pack_kernel(Geom g, Layout lo, const __half *__restrict__ K, const __half *__res
             if (slot >= (uint32_t)g.n4) continue;
             uint8_t *kd = lbase + lo.seg_off[4] + (uint64_t)slot * (row_elems / 4);
             uint8_t *vd = lbase + lo.seg_off[5] + (uint64_t)slot * (row_elems / 4);
-            H2 *ks = reinterpret_cast<H2 *>(lbase + lo.seg_off[8]) + (uint64_t)slot * g.Hkv;
-            H2 *vs = reinterpret_cast<H2 *>(lbase + lo.seg_off[9]) + (uint64_t)slot * g.Hkv;
+            const int recs = g.low_group ? row_elems / g.low_group : g.Hkv;          // (lo, hi) records per token row
+            H2 *ks = reinterpret_cast<H2 *>(lbase + lo.seg_off[8]) + (uint64_t)slot * recs;
+            H2 *vs = reinterpret_cast<H2 *>(lbase + lo.seg_off[9]) + (uint64_t)slot * recs;
             for (int c0 = 0; c0 < g.row_chunks; ++c0) {
                 const int e = c0 * 256 + lane * 8;
                 const bool in = e < row_elems;
@@ -149,9 +150,10 @@ pack_kernel(Geom g, Layout lo, const __half *__restrict__ K, const __half *__res
                     vv = ld_stream(vrow + (int64_t)h * g.sh + c);
                 }
                 // lanes past the row hold zeros: they sit in head-vector groups of their own (row_elems % D == 0)
+                // quantisation group: the head vector (LPV lanes), or 32 elements = 4 lanes (reading P22)
+                const int glanes = g.low_group ? g.low_group / 8 : LPV;
                 H2 mk = max_negmin8<E>(kv), mv = max_negmin8<E>(vv);
-#pragma unroll
-                for (int o = 1; o < LPV; o <<= 1) {
+                for (int o = 1; o < glanes; o <<= 1) {
                     mk = __hmax2(mk, as_pair<H2>(__shfl_xor_sync(0xffffffffu, h2u(mk), o)));
                     mv = __hmax2(mv, as_pair<H2>(__shfl_xor_sync(0xffffffffu, h2u(mv), o)));
                 }
@@ -160,7 +162,10 @@ pack_kernel(Geom g, Layout lo, const __half *__restrict__ K, const __half *__res
                 if (in) {
                     st_stream2(kd + e / 4, (uint16_t)quant8_int2<E>(kv, to_f(loK), inv3_of(range_of(loK, hiK))));
                     st_stream2(vd + e / 4, (uint16_t)quant8_int2<E>(vv, to_f(loV), inv3_of(range_of(loV, hiV))));
-                    if ((lane % LPV) == 0) { ks[e / D] = pair_h(loK, hiK); vs[e / D] = pair_h(loV, hiV); }
+                    if ((lane % glanes) == 0) {
+                        const int rec = g.low_group ? e / g.low_group : e / D;      // record index inside the token's row
+                        ks[rec] = pair_h(loK, hiK); vs[rec] = pair_h(loV, hiV);
+                    }
                 }
             }
         } else {
@@ -271,6 +276,29 @@ pack_fast_kernel(Geom g, Layout lo, const __half *__restrict__ K, const __half *
                 uint8_t *vd = lbase + lo.seg_off[1] + ((uint64_t)slot * row_elems + cb * 256 + lane * 8) * 2;
 #pragma unroll
                 for (int u = 0; u < NCH; ++u) { st_stream(kd + u * 512, kv[u]); st_stream(vd + u * 512, vv[u]); }
+                continue;
+            }
+            if (LOW2 && t == 2u && g.low_group) {
+                // group-wise 2-bit (reading P22): a group of 32 elements = 4 lanes; every lane ends up with its own
+                // group's (max, -min), so nothing is broadcast; one (lo, hi) record per group
+                uint8_t *kd = lbase + lo.seg_off[4] + (uint64_t)slot * (row_elems / 4) + cb * 64 + lane * 2;
+                uint8_t *vd = lbase + lo.seg_off[5] + (uint64_t)slot * (row_elems / 4) + cb * 64 + lane * 2;
+                H2 *ks = reinterpret_cast<H2 *>(lbase + lo.seg_off[8]) + (uint64_t)slot * (row_elems / 32) + cb * 8 + lane / 4;
+                H2 *vs = reinterpret_cast<H2 *>(lbase + lo.seg_off[9]) + (uint64_t)slot * (row_elems / 32) + cb * 8 + lane / 4;
+#pragma unroll
+                for (int u = 0; u < NCH; ++u) {
+                    H2 mk = max_negmin8<E>(kv[u]), mv = max_negmin8<E>(vv[u]);
+#pragma unroll
+                    for (int o = 1; o < 4; o <<= 1) {
+                        mk = __hmax2(mk, as_pair<H2>(__shfl_xor_sync(0xffffffffu, h2u(mk), o)));
+                        mv = __hmax2(mv, as_pair<H2>(__shfl_xor_sync(0xffffffffu, h2u(mv), o)));
+                    }
+                    H loK, hiK, loV, hiV;
+                    lohi_of(mk, loK, hiK); lohi_of(mv, loV, hiV);
+                    st_stream2(kd + u * 64, (uint16_t)quant8_int2<E>(kv[u], to_f(loK), inv3_of(range_of(loK, hiK))));
+                    st_stream2(vd + u * 64, (uint16_t)quant8_int2<E>(vv[u], to_f(loV), inv3_of(range_of(loV, hiV))));
+                    if ((lane & 3) == 0) { ks[u * 8] = pair_h(loK, hiK); vs[u * 8] = pair_h(loV, hiV); }
+                }
                 continue;
             }
             if (LOW2 && t == 2u) {

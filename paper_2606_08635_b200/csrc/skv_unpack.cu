@@ -97,13 +97,15 @@ unpack_kernel(Geom g, Layout lo, const uint8_t *__restrict__ blob, uint64_t blob
         } else if (t == 2u) {
             const uint8_t *ks = lbase + lo.seg_off[4] + (uint64_t)slot * (row_elems / 4);
             const uint8_t *vs = lbase + lo.seg_off[5] + (uint64_t)slot * (row_elems / 4);
-            const H2 *ka = reinterpret_cast<const H2 *>(lbase + lo.seg_off[8]) + (uint64_t)slot * g.Hkv;
-            const H2 *va = reinterpret_cast<const H2 *>(lbase + lo.seg_off[9]) + (uint64_t)slot * g.Hkv;
+            const int recs = g.low_group ? row_elems / g.low_group : g.Hkv;          // (lo, hi) records per token row
+            const H2 *ka = reinterpret_cast<const H2 *>(lbase + lo.seg_off[8]) + (uint64_t)slot * recs;
+            const H2 *va = reinterpret_cast<const H2 *>(lbase + lo.seg_off[9]) + (uint64_t)slot * recs;
             for (int c0 = 0; c0 < g.row_chunks; ++c0) {
                 const int e = c0 * 256 + lane * 8;
                 if (e < row_elems) {
                     const int h = e / D, c = e % D;
-                    const H2 rk = ka[h], rv = va[h];                // (lo, hi) records
+                    const int rec = g.low_group ? e / g.low_group : h;             // per head vector, or per 32 elements (P22)
+                    const H2 rk = ka[rec], rv = va[rec];            // (lo, hi) records
                     const uint32_t kw = ld_stream2(ks + e / 4), vw = ld_stream2(vs + e / 4);
                     st_stream(krow + (int64_t)h * g.sh + c,
                               dequant_int2<E>(kw, step3_of(range_of(lo_h(rk), hi_h(rk))), to_f(lo_h(rk))));
@@ -228,6 +230,24 @@ unpack_fast_kernel(Geom g, Layout lo, const uint8_t *__restrict__ blob, uint64_t
                     const int64_t off = (int64_t)((cb + u) * HPC + lane_h) * g.sh;
                     st_stream(krow + off, dequant_int8<E>(kv[u], sk));
                     st_stream(vrow + off, dequant_int8<E>(vv[u], sv));
+                }
+            } else if (LOW2 && t == 2u && g.low_group) {
+                // group-wise 2-bit (reading P22): the four lanes of a 32-element group read the same (lo, hi) record
+                const uint8_t *ks = lbase + lo.seg_off[4] + (uint64_t)slot * (row_elems / 4) + cb * 64 + lane * 2;
+                const uint8_t *vs = lbase + lo.seg_off[5] + (uint64_t)slot * (row_elems / 4) + cb * 64 + lane * 2;
+                const H2 *ka = reinterpret_cast<const H2 *>(lbase + lo.seg_off[8]) + (uint64_t)slot * (row_elems / 32) + cb * 8 + lane / 4;
+                const H2 *va = reinterpret_cast<const H2 *>(lbase + lo.seg_off[9]) + (uint64_t)slot * (row_elems / 32) + cb * 8 + lane / 4;
+                uint32_t kv[NCH], vv[NCH]; H2 rk[NCH], rv[NCH];
+#pragma unroll
+                for (int u = 0; u < NCH; ++u) {
+                    kv[u] = ld_stream2(ks + u * 64); vv[u] = ld_stream2(vs + u * 64);
+                    rk[u] = ka[u * 8]; rv[u] = va[u * 8];
+                }
+#pragma unroll
+                for (int u = 0; u < NCH; ++u) {
+                    const int64_t off = (int64_t)((cb + u) * HPC + lane_h) * g.sh;
+                    st_stream(krow + off, dequant_int2<E>(kv[u], step3_of(range_of(lo_h(rk[u]), hi_h(rk[u]))), to_f(lo_h(rk[u]))));
+                    st_stream(vrow + off, dequant_int2<E>(vv[u], step3_of(range_of(lo_h(rv[u]), hi_h(rv[u]))), to_f(lo_h(rv[u]))));
                 }
             } else if (LOW2 && t == 2u) {
                 const uint8_t *ks = lbase + lo.seg_off[4] + (uint64_t)slot * (row_elems / 4) + cb * 64 + lane * 2;

@@ -38,8 +38,9 @@ class Case:
     """One (config, budget) problem: inputs on host (numpy, canonical token-major) and oracle results."""
 
     def __init__(self, cfg, b, requests=None, layers=None, with_importance=True, causal=True, lam=0.0,
-                 importance_override=None):
+                 importance_override=None, tier_mode=0):
         self.cfg, self.b, self.causal, self.lam = cfg, b, causal, lam
+        self.tier_mode = tier_mode            # NEXT-4 flags: 1 = INT8 hot tier, 2 = group-wise 2-bit (same bits on both sides)
         R = cfg.R if requests is None else requests
         self.R = R
         Ks, Vs, Qs = [], [], []
@@ -49,7 +50,7 @@ class Case:
             Qs.append(skv_synth.make_q(cfg, r, layers=layers))
         self.K = torch.stack(Ks); self.V = torch.stack(Vs); self.Q = torch.stack(Qs)   # [R][L][n][Hkv][d]
         self.L = self.K.shape[1]
-        self.counts, self.prot = oracle.tier_counts(cfg.n, b, cfg.n_sink, cfg.ranges, cfg.allow_int4)
+        self.counts, self.prot = oracle.tier_counts(cfg.n, b, cfg.n_sink, cfg.ranges, cfg.allow_int4, mode=tier_mode)
         self.I, self.tier, self.blob, self.K2, self.V2 = [], [], [], [], []
         for r in range(R):
             if importance_override is not None:
@@ -70,7 +71,7 @@ class Case:
 
     def policy(self):
         c = self.cfg
-        return skv.make_policy(self.b, c.n_sink, c.ranges, c.allow_int4)
+        return skv.make_policy(self.b, c.n_sink, c.ranges, c.allow_int4, self.tier_mode)
 
 
 def gpu_pipeline(case, layout="token_major", use_oracle_importance=True, run_importance=True):
@@ -99,7 +100,7 @@ def gpu_pipeline(case, layout="token_major", use_oracle_importance=True, run_imp
     out["blob"] = blob.cpu().numpy().reshape(case.R, bb)
     # decode side: header check on the host copy, then unpack into a poisoned dense cache
     hs, hc = skv.skv_blob_check(out["blob"][0][:256].tobytes(), bb)
-    assert hc.as_tuple() == counts.as_tuple()
+    assert hc.as_tuple() == counts.as_tuple() and hc.tier_mode == counts.tier_mode == case.tier_mode
     Ko = torch.full_like(Kd, float("nan")); Vo = torch.full_like(Vd, float("nan"))
     tm_out = torch.full_like(tier, 0xEE)
     skv.skv_unpack(shape, blob, bb, hc, Ko, Vo, tm_out, ws)

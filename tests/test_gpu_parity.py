@@ -495,6 +495,78 @@ def test_two_bit_low_tier_parity(d, Hkv, Hq, n, b):
         assert ok[m].all()
 
 
+@pytest.mark.parametrize("d,Hkv,Hq,n,b,a4", [(128, 8, 32, 1000, 0.3, 1), (128, 4, 8, 513, 0.45, 1), (64, 3, 3, 257, 0.2, 1),
+                                             (256, 2, 4, 640, 0.3, 0), (128, 2, 2, 300, 0.7, 1), (64, 8, 8, 96, 0.15, 2),
+                                             (256, 1, 2, 129, 0.3, 2)])
+def test_int8_hot_tier_parity(d, Hkv, Hq, n, b, a4):
+    """NEXT-4 (reading P21): the hot tier ships INT8 -- counts (n16 = 0), tier map (sinks and the
+    protected range pinned to code 8), header flags bit3, every blob byte and every dequantised element bit-exact
+    against the oracle; 3-tier, 2-tier and 2-bit low tiers, fast and generic rows, b above 1/2 = Uniform INT8."""
+    cfg = skv_synth.Config("hot8", L=2, Hq=Hq, Hkv=Hkv, d=d, n=n, w=8, R=2, n_sink=3, ranges=((n - 9, n),), seed=71,
+                           allow_int4=a4)
+    case = Case(cfg, b, with_importance=False, tier_mode=skv.SKV_MODE_HOT_INT8)
+    assert case.counts.n16 == 0 and all((t[:, :3] == 8).all() and (t[:, n - 9:] == 8).all() for t in case.tier)
+    out = gpu_pipeline(case, run_importance=False)
+    assert_bit_exact(case, out)
+    assert all(int.from_bytes(bytes(bl[40:44]), "little") & 8 for bl in out["blob"])
+    if b >= 0.5:
+        assert all((t == 8).all() for t in out["tier"])
+
+
+@pytest.mark.parametrize("d,Hkv,Hq,n,b,mode", [(128, 8, 32, 1000, 0.2, 2), (128, 4, 8, 513, 0.125, 2), (128, 2, 2, 300, 0.3, 2),
+                                               (64, 3, 3, 257, 0.2, 2), (256, 2, 4, 640, 0.15, 3), (64, 8, 8, 96, 0.05, 2),
+                                               (256, 1, 2, 129, 0.22, 3)])
+def test_group_wise_two_bit_tier_parity(d, Hkv, Hq, n, b, mode):
+    """NEXT-4 (reading P22): the 2-bit low tier quantised in groups of 32 elements, one (lo, hi) record
+    per group -- every blob byte (codes and the d/32-times larger record segments) and every dequantised element
+    bit-exact against the oracle; fast kernels (4, 2, 1 chunk batches) and generic rows; mode 3 adds the INT8 hot tier."""
+    cfg = skv_synth.Config("grp2", L=2, Hq=Hq, Hkv=Hkv, d=d, n=n, w=8, R=2, n_sink=2, seed=81, allow_int4=2)
+    case = Case(cfg, b, with_importance=False, tier_mode=mode)
+    assert case.counts.low_bits == 2 and any((t == 2).any() for t in case.tier)
+    out = gpu_pipeline(case, run_importance=False)
+    assert_bit_exact(case, out)
+    assert all(int.from_bytes(bytes(bl[40:44]), "little") & 16 for bl in out["blob"])
+    # error bound per GROUP on the dequantised cache: half a step of the group's own range
+    for r in range(case.R):
+        m = case.tier[r] == 2
+        X = case.K[r].numpy().astype(np.float64).reshape(case.L, n, Hkv, d // 32, 32)
+        Y = out["K2"][r].astype(np.float64).reshape(X.shape)
+        rng_ = X.max(axis=-1, keepdims=True) - X.min(axis=-1, keepdims=True)
+        ok = np.abs(Y - X) <= rng_ / 6 * (1 + 1e-3) + np.abs(Y) * 2.0 ** -11 + 1e-12
+        assert ok[m].all()
+
+
+def test_next4_modes_with_bfloat16_caches():
+    """INT8 hot tier + group-wise 2-bit on bfloat16 caches (flags bits 1-4 all set): blob and dequantised cache bit-exact."""
+    dev = torch.device("cuda:0")
+    cfg = skv_synth.Config("bf16m", L=2, Hq=4, Hkv=2, d=128, n=300, w=16, R=1, n_sink=2, seed=91, allow_int4=2)
+    b, mode = 0.2, 3
+    K, V, Q = _bf16_case(cfg, b)
+    Kb, Vb = _bits(K), _bits(V)
+    counts, prot = oracle.tier_counts(cfg.n, b, cfg.n_sink, (), 2, mode=mode)
+    I = skv_synth.make_importance(cfg, 0).numpy()
+    tier_or = oracle.assign(I, prot, counts)
+    blob_or = oracle.pack(Kb, Vb, tier_or, counts, 2, bf16=True)
+    K2_or, V2_or, _ = oracle.unpack(blob_or, cfg.L, cfg.Hkv, cfg.d, cfg.n, bf16=True)
+    shape = skv.make_shape(cfg.L, cfg.Hq, cfg.Hkv, cfg.d, cfg.n, 1, dtype="bf16")
+    pol = skv.make_policy(b, cfg.n_sink, (), 2, tier_mode=mode)
+    ws = torch.empty(skv.skv_workspace_bytes(shape, 0), dtype=torch.uint8, device=dev)
+    Kd, Vd = K[None].to(dev), V[None].to(dev)
+    tier = torch.full((1, cfg.L, cfg.n), 0xEE, dtype=torch.uint8, device=dev)
+    c = skv.skv_assign_tiers(shape, pol, torch.from_numpy(I)[None].to(dev), tier, ws)
+    assert np.array_equal(tier[0].cpu().numpy(), tier_or) and c.tier_mode == mode
+    bb = skv.skv_blob_bytes(shape, c)
+    blob = torch.full((bb,), 0xAB, dtype=torch.uint8, device=dev)
+    skv.skv_pack(shape, Kd, Vd, tier, c, blob, ws)
+    hb = blob.cpu().numpy()
+    assert np.array_equal(hb, blob_or) and int.from_bytes(bytes(hb[40:44]), "little") == 31
+    hs, hc = skv.skv_blob_check(hb[:256].tobytes(), bb)
+    Ko = torch.full_like(Kd, float("nan")); Vo = torch.full_like(Vd, float("nan"))
+    skv.skv_unpack(shape, blob, bb, hc, Ko, Vo, None, ws)
+    torch.cuda.synchronize()
+    assert np.array_equal(_bits(Ko[0]), K2_or) and np.array_equal(_bits(Vo[0]), V2_or)
+
+
 def test_two_bit_upgrade_to_int8_patch():
     """NEXT-4 + NEXT-3: a 2-bit token upgraded to INT8 by an upgrade blob (the upgrade blob itself has no low tier)."""
     dev = torch.device("cuda:0")

@@ -54,6 +54,53 @@ def test_tier_counts_match_oracle_sweep():
         assert skv.skv_blob_bytes(shape, got) == oracle.blob_bytes(2, 2, 128, n, want)
 
 
+def test_tier_counts_next4_modes_match_oracle_sweep_and_header_flags():
+    """NEXT-4 tier modes (INT8 hot tier P21, group-wise 2-bit P22): closed-form counts and blob sizes against the oracle."""
+    rng = np.random.default_rng(5)
+    for _ in range(1500):
+        n = int(rng.integers(1, 6000))
+        b = float(rng.choice([rng.uniform(0.01, 1.3), rng.integers(1, 41) / 40.0]))
+        s = int(rng.integers(0, min(n, 9) + 1))
+        a4 = int(rng.integers(0, 3))
+        mode = int(rng.integers(1, 4)) if a4 == 2 else 1
+        rngs = [(int(a), int(a + rng.integers(0, n - a + 1))) for a in rng.integers(0, n + 1, size=int(rng.integers(0, 3)))]
+        shape = skv.make_shape(2, 4, 2, 128, n)
+        pol = skv.make_policy(b, s, rngs, a4, tier_mode=mode)
+        try:
+            want, _ = oracle.tier_counts(n, b, s, rngs, a4, mode=mode)
+        except ValueError:
+            with pytest.raises(skv.SkvError) as ei:
+                skv.skv_tier_counts(shape, pol)
+            assert ei.value.status == skv.SKV_ERR_BUDGET_INFEASIBLE
+            continue
+        got = skv.skv_tier_counts(shape, pol)
+        assert got.as_tuple() == (want.n16, want.n8, want.n4, want.n0) and got.tier_mode == mode
+        assert (got.budget_q4, got.spent_q4, got.allow_int4) == (want.budget_q4, want.spent_q4, a4)
+        assert skv.skv_blob_bytes(shape, got) == oracle.blob_bytes(2, 2, 128, n, want)
+    # group-wise records need the 2-bit tier; unknown mode bits are refused
+    shape = skv.make_shape(2, 4, 2, 128, 100)
+    for pol in (skv.make_policy(0.3, 0, (), 1, tier_mode=2), skv.make_policy(0.3, 0, (), 0, tier_mode=2),
+                skv.make_policy(0.3, 0, (), 2, tier_mode=4)):
+        with pytest.raises(skv.SkvError) as ei:
+            skv.skv_tier_counts(shape, pol)
+        assert ei.value.status == skv.SKV_ERR_INVALID_ARG
+    # skv_blob_check: an oracle-written blob with both flags is accepted and reports the mode; FP16 tokens under the
+    # INT8-hot-tier flag and groups without the 2-bit tier are refused
+    L, n, Hkv, d = 1, 24, 2, 64
+    c, prot = oracle.tier_counts(n, 0.2, 2, [], 2, mode=3)
+    K = np.random.default_rng(6).standard_normal((L, n, Hkv, d)).astype(np.float16)
+    tier = oracle.assign(np.random.default_rng(7).random((L, n)).astype(np.float32), prot, c)
+    blob = oracle.pack(K, K, tier, c, 2)
+    assert int.from_bytes(bytes(blob[40:44]), "little") == 1 | 2 | 8 | 16
+    hs, hc = skv.skv_blob_check(bytes(blob[:256]), blob.size)
+    assert hc.tier_mode == 3 and hc.allow_int4 == 2 and hc.as_tuple() == (0, c.n8, c.n4, c.n0)
+    for off, val in ((24, 1), (40, 1 | 8 | 16)):
+        bad = blob[:256].copy(); bad[off] = val
+        with pytest.raises(skv.SkvError) as ei:
+            skv.skv_blob_check(bytes(bad), blob.size)
+        assert ei.value.status == skv.SKV_ERR_BAD_BLOB
+
+
 def test_argument_errors():
     shape = skv.make_shape(2, 4, 2, 128, 100)
     for bad_b in (0.0, -1.0, float("nan")):
