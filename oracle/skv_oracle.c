@@ -486,6 +486,8 @@ void orc_dequantize_vector(const int8_t *q, int32_t d, int32_t qmax, uint16_t am
  * 2-byte records; a zero of either sign is stored as +0).  r = fl32(hi - lo), step = fl32(r / 3), inv = fl32(3 / r)
  * (both 0 when r = 0).  q = clamp(rint(fl32(x - lo) * inv), 0, 3), the product exact and rounded once, half to even
  * (as P8).  y = f16_rn(fma(q, step, lo)), the fused multiply-add rounded once to binary32.
+ * bfloat16 only (P20): a range r that overflows binary32 (finite elements more than 3.4e38 apart) gives inv = 3 / Inf = 0
+ * and step is taken as 0 as well: all codes 0, every element decodes to lo (finite), instead of fma(0, Inf, lo) = NaN.
  */
 void orc_quantize2_vector_dt(const uint16_t *x, int32_t d, uint16_t *lo_out, uint16_t *hi_out, uint8_t *q, int32_t dtype)
 {
@@ -519,6 +521,8 @@ void orc_dequantize2_vector_dt(const uint8_t *q, int32_t d, uint16_t lo_bits, ui
     volatile float r = hi - lo;
     volatile float step = 0.0f;
     if (r != 0.0f) step = r / 3.0f;
+    if (!isfinite(step)) step = 0.0f;                    /* P20: a bfloat16 range beyond FLT_MAX (hi - lo = +Inf); the encoder's
+                                                            3 / Inf = 0 gave all-zero codes, so every element decodes to lo */
     for (int32_t c = 0; c < d; ++c) {
         volatile float v = fmaf((float)q[c], step, lo);                      /* correctly rounded fused multiply-add */
         y[c] = float_to_elem(v, dtype);

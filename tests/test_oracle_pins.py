@@ -821,6 +821,21 @@ def test_bf16_quantizer_identities_and_error_bound():
     y = oracle.bf16_to_float(oracle.dequantize2_vector(q2, lo, hi, bf16=True)).astype(np.float64)
     step = (float(x.max()) - float(x.min())) / 3
     assert (np.abs(y - x.astype(np.float64)) <= step / 2 * (1 + 1e-3) + np.abs(y) * 2.0 ** -8).all()
+    # P20, the other end: finite bf16 elements more than FLT_MAX apart (hi - lo = +Inf in binary32).  Fixed by hand:
+    # inv = 3 / Inf = 0 -> every code 0; step is taken as 0 -> every element decodes to lo; nothing is NaN or Inf.
+    big = float(oracle.bf16_to_float(np.uint16(0x7F62)))                                  # 3.0e38 as bf16 (finite, < FLT_MAX)
+    assert 2.9e38 < big < 3.1e38
+    wide = np.array([0x7F62, 0xFF62] + [0x3F80] * 30, np.uint16)                          # +3e38, -3e38, 1.0 ...
+    lo, hi, q2 = oracle.quantize2_vector(wide, bf16=True)
+    assert lo == 0xFF62 and hi == 0x7F62 and (q2 == 0).all()
+    y = oracle.dequantize2_vector(q2, lo, hi, bf16=True)
+    assert (y == 0xFF62).all()
+    # one binade lower the range is finite again and the rule does not apply: extremes hit codes 0 and 3 and round-trip
+    half = np.array([0x7EE2, 0xFEE2] + [0x3F80] * 30, np.uint16)                          # +-1.5e38: range 3e38 is finite
+    lo, hi, q2 = oracle.quantize2_vector(half, bf16=True)
+    assert q2[0] == 3 and q2[1] == 0
+    y = oracle.dequantize2_vector(q2, lo, hi, bf16=True)
+    assert y[0] == 0x7EE2 and y[1] == 0xFEE2
 
 
 def test_bf16_blob_round_trip_and_fp16_tier_is_a_copy():
