@@ -500,6 +500,8 @@ void orc_quantize2_vector_dt(const uint16_t *x, int32_t d, uint16_t *lo_out, uin
     if (r != 0.0f) inv = 3.0f / r;
     if (!isfinite(inv)) inv = 0.0f;                      /* P20: bfloat16 ranges below ~1e-38 only */
     for (int32_t c = 0; c < d; ++c) {
+        if (inv == 0.0f) { q[c] = 0; continue; }                             /* r = 0, or (P20) r or 3/r overflowed: all codes 0
+                                                                                (x - lo may itself be +Inf there: Inf * 0 is no code) */
         volatile float dx = elem_to_float(x[c], dtype) - lo;                 /* one binary32 rounding */
         double t = rint((double)dx * (double)inv);                           /* exact product, rounded once */
         if (t > 3.0) t = 3.0;
