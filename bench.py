@@ -4,7 +4,9 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl skv|reference] [--workload C5] [--budget 0.5]
 
 A "step" is one pass of the whole hot path over one batch of synthetic requests:
-    skv_importance -> skv_assign_tiers -> skv_pack -> skv_unpack      (9 kernel launches)
+    skv_importance -> skv_assign_tiers -> skv_pack -> skv_unpack
+(6 kernel launches at C5: importance, assign, tile scan + pack, tile scan + unpack; 4 for n <= 8192 tokens, where the
+scan is fused into pack / unpack)
 `value` = FP16 KV bytes of the batch / (time in skv_pack + skv_unpack), inputs resident in HBM, timed with CUDA
 events on the launching stream.  `e2e` = the same bytes / the time of the whole path driven from pinned HOST
 buffers (H2D of K,V,Q; the pinned-host D2H+H2D hop of the blob that stands in for the network; D2H of the
@@ -45,6 +47,10 @@ def parse_args():
     ap.add_argument("--e2e-chunk-layers", type=int, default=4, help="layers per pipelined transfer chunk")
     ap.add_argument("--e2e-depth", type=int, default=3, help="device slots of the pipelined transfer")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
+    ap.add_argument("--l2-flush", default="auto", choices=["auto", "on", "off"],
+                    help="read a 512 MiB buffer between stages (outside the stage events) so that no stage finds its "
+                         "input in L2; auto = on for batches whose FP16 KV is below 2 GiB (C1-C4)")
+    ap.add_argument("--no-sweep", action="store_true", help="skip the C1-C4 / budget sweep reported under 'sweep'")
     return ap.parse_args()
 
 
@@ -66,28 +72,58 @@ def measured_peak():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
 
 
+TRAFFIC_FILE = "profiles/r2_traffic.csv"
+
+
 def ncu_traffic(workload, b, R, kernel):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` ("pack" | "unpack"), as captured by
-    `ncu --set full` and recorded in profiles/r1_traffic.csv (workload,budget,n_requests,kernel,dram_bytes);
-    None when no capture of this exact workload is on file."""
+    """(dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` ("pack" | "unpack"), provenance) as
+    captured by `ncu --set full` and RECORDED in profiles/r2_traffic.csv
+    (workload,budget,n_requests,kernel,dram_bytes,captured) -- not measured in this run; `captured` names the date
+    and source revision of the capture.  (None, None) when no capture of this exact workload is on file."""
     try:
-        with open(os.path.join(ROOT, "profiles", "r1_traffic.csv")) as f:
+        with open(os.path.join(ROOT, TRAFFIC_FILE)) as f:
             for ln in f:
                 fld = [x.strip() for x in ln.split(",")]
                 if len(fld) >= 5 and fld[0] == workload and fld[3] == kernel:
                     if abs(float(fld[1]) - b) < 1e-9 and int(fld[2]) == R:
-                        return float(fld[4])
+                        return float(fld[4]), (fld[5] if len(fld) > 5 else None)
     except Exception:
         pass
-    return None
+    return None, None
 
 
-def config_json(cfg, b, R, extra=None):
+L2_BYTES = 126 * 2**20
+FLUSH_BYTES = 512 * 2**20
+
+
+def want_flush(args, cfg, R):
+    if args.l2_flush == "auto":
+        return cfg.bytes_fp16 * R < 2 * 2**30
+    return args.l2_flush == "on"
+
+
+def l2_note(cfg, R, blob_bytes, flush):
+    """How the timed steps relate to the 126 MB L2, computed from the working set of one step."""
+    kv = cfg.bytes_fp16 * R
+    ws = 2 * kv + blob_bytes * R
+    if flush:
+        return (f"L2 flushed between stages: {FLUSH_BYTES >> 20} MiB read (clean lines) after every stage, outside the stage events "
+                f"(step working set {ws / 2**20:.0f} MiB, blob {blob_bytes * R / 2**20:.0f} MiB would otherwise be partly "
+                f"L2-resident between pack and unpack); ms_per_step = sum of the four stage times")
+    if blob_bytes * R < 4 * L2_BYTES:
+        return (f"no flush: step working set {ws / 2**20:.0f} MiB; the blob ({blob_bytes * R / 2**20:.0f} MiB) may be partly "
+                f"L2-resident when unpack reads it")
+    return (f"inputs larger than L2: every stage streams >= {min(kv, blob_bytes * R) / 2**20:.0f} MiB "
+            f"(> 30x the 126 MB L2) between two uses of a line; no flush needed")
+
+
+def config_json(cfg, b, R, extra=None, l2=None):
     c = {"workload": f"{cfg.name}: {cfg.L} layers, {cfg.Hq} q heads / {cfg.Hkv} KV heads, head_dim {cfg.d}, "
                      f"{cfg.n} tokens, batch of {R} requests, window {cfg.w}, b={b}, "
                      f"{'3-tier FP16/INT8/INT4' if cfg.allow_int4 else '2-tier FP16+INT8'}, {cfg.n_sink} sinks",
-         "budget": b, "n_requests": R, "bytes_fp16_per_request": cfg.bytes_fp16,
-         "l2": "inputs larger than L2 (batch working set >> 126 MB); no flush needed"}
+         "budget": b, "n_requests": R, "bytes_fp16_per_request": cfg.bytes_fp16}
+    if l2 is not None:
+        c["l2"] = l2
     if extra:
         c.update(extra)
     return c
@@ -198,7 +234,12 @@ def barrier():
 # the CUDA arm
 # ----------------------------------------------------------------------------------------------------
 STAGES = ("importance", "assign", "pack", "unpack")
-LAUNCHES_PER_STEP = 4 + 1 + 2 + 2     # imp_tc<1>, combine, imp_tc<2>, finish | assign | tile_scan, pack | tile_scan, unpack
+FUSE_MAX_TOKENS = 8192                # csrc/skv_common.cuh kFuseMaxTokens: up to here pack / unpack need no scan launch
+
+
+def launches_per_step(cfg):
+    """Kernels of libskv launched by one step: imp_fused_kernel | assign_kernel | [tile_scan,] pack | [tile_scan,] unpack."""
+    return 1 + 1 + (1 if cfg.n <= FUSE_MAX_TOKENS else 2) * 2
 
 
 class DeviceProblem:
@@ -221,30 +262,134 @@ class DeviceProblem:
         self.ws = torch.empty(skv.skv_workspace_bytes(self.shape, cfg.w), dtype=torch.uint8, device=dev)
         self.I = torch.empty((R, L, cfg.n), dtype=torch.float32, device=dev)
         self.tier = torch.empty((R, L, cfg.n), dtype=torch.uint8, device=dev)
-        self.blob = torch.empty((R, self.blob_bytes), dtype=torch.uint8, device=dev)
+        self.blob_flat = torch.empty((R * self.blob_bytes,), dtype=torch.uint8, device=dev)
+        self.blob = self.blob_flat.view(R, self.blob_bytes)
         self.Ko = torch.empty_like(self.K)
         self.Vo = torch.empty_like(self.V)
         self.tier_out = torch.empty_like(self.tier)
+        self.flush_buf = None
+
+    def set_budget(self, b):
+        """Same caches, another budget (the C5 b-sweep): new policy, counts and blob size; buffers are reused."""
+        import torch
+        skv = self.skv
+        self.b = b
+        self.policy = skv.make_policy(b, self.cfg.n_sink, self.cfg.ranges, self.cfg.allow_int4)
+        self.counts = skv.skv_tier_counts(self.shape, self.policy)
+        self.blob_bytes = skv.skv_blob_bytes(self.shape, self.counts)
+        if self.blob_flat.numel() < self.R * self.blob_bytes:
+            self.blob = self.blob_flat = None
+            self.blob_flat = torch.empty((self.R * self.blob_bytes,), dtype=torch.uint8, device=self.dev)
+        self.blob = self.blob_flat[:self.R * self.blob_bytes].view(self.R, self.blob_bytes)
+
+    def enable_flush(self):
+        import torch
+        self.flush_buf = torch.zeros(FLUSH_BYTES // 8, dtype=torch.int64, device=self.dev)
 
     def step(self, events=None):
+        """events: 8 CUDA events = (start, stop) of each of the four stages.  With an L2 flush enabled the flush runs
+        between a stage's stop event and the next stage's start event."""
         skv, s = self.skv, self
         rec = (lambda i: events[i].record()) if events is not None else (lambda i: None)
+        blob = s.blob
+        # the flush READS 512 MiB (a torch reduction, outside the stage events): the lines it leaves in L2 are clean, so
+        # the next stage does not pay for write-backs of somebody else's dirty lines
+        fl = (lambda: s.flush_buf.sum()) if s.flush_buf is not None else (lambda: None)
         rec(0)
         skv.skv_importance(s.shape, s.K, s.Q, s.cfg.w, s.I, s.ws)
-        rec(1)
+        rec(1); fl(); rec(2)
         skv.skv_assign_tiers(s.shape, s.policy, s.I, s.tier, s.ws)
-        rec(2)
-        skv.skv_pack(s.shape, s.K, s.V, s.tier, s.counts, s.blob, s.ws)
-        rec(3)
-        skv.skv_unpack(s.shape, s.blob, s.blob_bytes, s.counts, s.Ko, s.Vo, s.tier_out, s.ws)
-        rec(4)
+        rec(3); fl(); rec(4)
+        skv.skv_pack(s.shape, s.K, s.V, s.tier, s.counts, blob, s.ws)
+        rec(5); fl(); rec(6)
+        skv.skv_unpack(s.shape, blob, s.blob_bytes, s.counts, s.Ko, s.Vo, s.tier_out, s.ws)
+        rec(7); fl()
 
     def algorithmic_bytes(self):
-        """pack reads Bytes_FP16 + tier map, writes the blob; unpack the mirror."""
+        """pack reads the rows it ships (dropped tokens are never loaded) + the tier map and
+        writes the blob; unpack reads the blob and writes every row (dropped ones as zeros) + the tier map."""
         fp16 = self.cfg.bytes_fp16 * self.R
         blob = self.blob_bytes * self.R
         tm = self.cfg.L * self.cfg.n * self.R
-        return {"pack": fp16 + blob + tm, "unpack": blob + fp16 + tm}
+        c = self.counts
+        shipped = (c.n16 + c.n8 + c.n4) / float(self.cfg.n)
+        return {"pack": int(fp16 * shipped) + blob + tm, "unpack": blob + fp16 + tm}
+
+
+def time_problem(prob, K, W, flush, sampler=None, dev=None):
+    """W untimed warm-up steps, then K timed steps bracketed by barrier + synchronize; per-stage CUDA events on the
+    launching stream.  Returns per-stage mean / min ms and ms per step (event time of the K steps / K; with an L2
+    flush between stages: the sum of the stage means)."""
+    import torch
+    if flush and prob.flush_buf is None:
+        prob.enable_flush()
+    if not flush:
+        prob.flush_buf = None
+    for _ in range(W):
+        prob.step()
+    torch.cuda.synchronize()
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(8)] for _ in range(K)]
+    barrier()
+    torch.cuda.synchronize()
+    if sampler is not None:
+        sampler.start()
+        sampler.wait_first_sample()
+    t_wall0 = time.perf_counter()
+    t_abs0 = time.time()
+    for k in range(K):
+        prob.step(ev[k])
+    torch.cuda.synchronize()
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    clocks = sampler.stop(t_abs0, time.time()) if sampler is not None else None
+    stage_ms = [sum(ev[k][2 * i].elapsed_time(ev[k][2 * i + 1]) for k in range(K)) / K for i in range(4)]
+    stage_min = [min(ev[k][2 * i].elapsed_time(ev[k][2 * i + 1]) for k in range(K)) for i in range(4)]
+    ms_step = sum(stage_ms) if flush else ev[0][0].elapsed_time(ev[K - 1][7]) / K
+    return {"stage_ms": stage_ms, "stage_min": stage_min, "ms_step": ms_step, "clocks": clocks, "wall_s": t_wall}
+
+
+def sweep_row(prob, res, peak, flush):
+    cfg = prob.cfg
+    alg = prob.algorithmic_bytes()
+    imp, asg, pk, up = res["stage_ms"]
+    kv = cfg.bytes_fp16 * prob.R
+    return {"workload": cfg.name, "budget": prob.b, "n_requests": prob.R, "counts": list(prob.counts.as_tuple()),
+            "stages_ms": dict(zip(STAGES, res["stage_ms"])), "stages_ms_min": dict(zip(STAGES, res["stage_min"])),
+            "ms_per_step": res["ms_step"], "value": kv / ((pk + up) * 1e-3) / 1e9, "unit": UNIT,
+            "pack_frac_of_hbm_peak": alg["pack"] / (pk * 1e-3) / 1e9 / peak,
+            "unpack_frac_of_hbm_peak": alg["unpack"] / (up * 1e-3) / 1e9 / peak,
+            "pack_plus_unpack_frac_of_hbm_peak": (alg["pack"] + alg["unpack"]) / ((pk + up) * 1e-3) / 1e9 / peak,
+            "gpu_launches_per_step": launches_per_step(cfg),
+            "l2": l2_note(cfg, prob.R, prob.blob_bytes, flush)}
+
+
+def run_sweep(args, main_prob, dev, peak, steps):
+    """BASELINE.json's other configs and budgets through the same timing loop: C1-C4 at their
+    budgets with the L2 flushed between stages, and the remaining budgets of the C5 sweep on the main problem's caches."""
+    import skv_synth
+    rows = []
+    main_cfg, main_b = main_prob.cfg, main_prob.b
+    for name in ("C1", "C2", "C3", "C4", "C5"):
+        cfg = skv_synth.CONFIGS[name]
+        if cfg.name == main_cfg.name:
+            for b in cfg.budgets:
+                if abs(b - main_b) < 1e-9:
+                    continue
+                main_prob.set_budget(b)
+                fl = want_flush(args, cfg, main_prob.R)
+                rows.append(sweep_row(main_prob, time_problem(main_prob, steps, 3, fl), peak, fl))
+            main_prob.set_budget(main_b)
+            main_prob.flush_buf = None
+            continue
+        if cfg.bytes_fp16 * cfg.R > main_cfg.bytes_fp16 * main_prob.R:
+            continue                                         # never sweep anything larger than the main workload
+        prob = DeviceProblem(cfg, cfg.budgets[0], cfg.R, dev)
+        for b in cfg.budgets:
+            prob.set_budget(b)
+            fl = want_flush(args, cfg, cfg.R)
+            rows.append(sweep_row(prob, time_problem(prob, steps, 3, fl), peak, fl))
+        del prob
+    return rows
 
 
 def run_next_rows(prob, steps):
@@ -325,7 +470,7 @@ def run_next_rows(prob, steps):
     return out
 
 
-def run_e2e(cfg, b, R, dev, steps, warmup, chunk_layers=4, depth=3):
+def run_e2e(cfg, b, R, dev, steps, warmup, chunk_layers=4, depth=3, host_requests=2):
     """The whole path driven from pinned HOST buffers through the public API (paper_2606_08635_b200.transfer.
     LayerPipelinedTransfer: per layer chunk  H2D K,V,Q -> importance -> assign -> pack -> D2H blob -> skv_blob_check
     (host) -> H2D blob -> unpack -> D2H K,V,  chunks overlapped on three streams).  Also times, once each for
@@ -337,9 +482,10 @@ def run_e2e(cfg, b, R, dev, steps, warmup, chunk_layers=4, depth=3):
     import skv_synth
     L = cfg.L
     pin = dict(pin_memory=True)
-    # pinned host footprint is bounded (N ranks share one host): two distinct requests in, a two-request ring out; the
-    # R requests of a step alternate between them -- the bytes copied per step are those of R requests
-    Rh = min(R, 2)
+    # pinned host footprint is bounded: `host_requests` distinct requests in and as many out (2 on a single rank, 1 per
+    # rank under torchrun, where N ranks share one host's pinned memory); the R requests of a step cycle through them --
+    # the bytes copied per step are those of R requests
+    Rh = max(1, min(R, host_requests))
     hK = torch.empty((Rh, L, cfg.n, cfg.Hkv, cfg.d), dtype=torch.float16, **pin)
     hV = torch.empty_like(hK, **pin)
     hQ = torch.empty((Rh, L, cfg.Hq, cfg.w, cfg.d), dtype=torch.float16, **pin)
@@ -366,7 +512,8 @@ def run_e2e(cfg, b, R, dev, steps, warmup, chunk_layers=4, depth=3):
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1) / steps
     h2d_req, d2h_req = pipe.bytes_per_request()
-    out = {"ms_per_step": ms, "steps": steps, "h2d": R * h2d_req, "d2h": R * d2h_req, "layers_per_chunk": lpc, "depth": depth}
+    out = {"ms_per_step": ms, "steps": steps, "h2d": R * h2d_req, "d2h": R * d2h_req, "layers_per_chunk": lpc, "depth": depth,
+           "host_requests": Rh}
     del pipe
 
     # context 1: no overlap -- one request at a time, one stream, whole-request blobs
@@ -420,10 +567,27 @@ def run_e2e(cfg, b, R, dev, steps, warmup, chunk_layers=4, depth=3):
 # ----------------------------------------------------------------------------------------------------
 # the CPU oracle arm (cpu_baseline leg and --impl reference).  The ONLY place bench.py touches oracle/.
 # ----------------------------------------------------------------------------------------------------
+def cpu_model():
+    try:
+        with open("/proc/cpuinfo") as f:
+            for ln in f:
+                if ln.lower().startswith("model name"):
+                    return ln.split(":", 1)[1].strip()
+    except Exception:
+        pass
+    import platform
+    return platform.processor() or platform.machine()
+
+
 def oracle_sample(cfg, b, target_seconds):
-    """Times oracle pack + unpack (the metric's two stages) on a bounded sample of the workload: the first
-    `layers` layers of request 0 (same generator, same bytes as the CUDA arm's request 0 on the CPU generator).
-    Returns (GB/s of FP16 KV, cores, sample description, seconds)."""
+    """SURVEY.md 8(d) 'Oracle timing': the oracle as it stands on a bounded sample of the workload (the first layers of
+    request 0; same generator, same bytes as the CUDA arm's request 0 on the CPU generator), about `target_seconds` of
+    CPU work in total:
+      (b) pack + unpack with OpenMP over layers on every available core -- the headline `value`;
+      (a) pack + unpack single-threaded on ONE layer;
+      (c) importance (float64 triple loop) and assign (qsort) on a token-truncated slice of one layer, timed separately
+          (importance cost is linear in n; the report says what was timed and the per-layer extrapolation).
+    Returns the cpu_baseline dict."""
     import numpy as np
     import oracle
     import skv_synth
@@ -443,10 +607,28 @@ def oracle_sample(cfg, b, target_seconds):
         t2 = time.perf_counter()
         return sub.bytes_fp16, t1 - t0, t2 - t1
 
+    # (a) single thread, one layer
+    oracle.set_threads(1)
+    nb1, tp1, tu1 = run(1)
+    # (c) importance + assign, single layer, OpenMP as the oracle has it; importance on n_imp <= n tokens
+    oracle.set_threads(threads)
+    n_imp = int(min(cfg.n, 4096))
+    sub = cfg.scaled(L=1, n=n_imp, ranges=())
+    K1, _ = skv_synth.make_kv(sub, 0)
+    Q1 = skv_synth.make_q(sub, 0)
+    t0 = time.perf_counter()
+    oracle.importance(K1.numpy(), Q1.numpy())
+    t_imp = time.perf_counter() - t0
+    I1 = skv_synth.make_importance(cfg.scaled(L=1), 0).numpy()
+    t0 = time.perf_counter()
+    oracle.assign(I1, prot, counts)
+    t_asg = time.perf_counter() - t0
+    # (b) all cores, as many layers as the time target allows
+    budget_s = max(1.0, target_seconds - (tp1 + tu1) - t_imp - t_asg)
     layers = min(cfg.L, max(1, threads))
     nbytes, tp, tu = run(layers)
     per_layer = (tp + tu) / layers
-    want = int(min(cfg.L, max(layers, target_seconds / max(per_layer, 1e-9))))
+    want = int(min(cfg.L, max(layers, budget_s / max(per_layer, 1e-9))))
     if want >= threads:
         want = (want // threads) * threads
     if want > layers:
@@ -455,7 +637,17 @@ def oracle_sample(cfg, b, target_seconds):
     gbs = nbytes / (tp + tu) / 1e9
     sample = (f"oracle pack+unpack of {layers} of {cfg.L} layers of 1 request ({nbytes / 2**20:.0f} MiB FP16 KV), "
               f"tier map from a synthetic importance vector, OpenMP over layers")
-    return gbs, threads, sample, tp + tu, {"pack_s": tp, "unpack_s": tu}
+    return {"value": gbs, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample, "cpu_model": cpu_model(),
+            "seconds": tp + tu, "pack_s": tp, "unpack_s": tu,
+            "single_thread": {"value": nb1 / (tp1 + tu1) / 1e9, "unit": UNIT, "cores": 1, "pack_s": tp1, "unpack_s": tu1,
+                              "sample": f"oracle pack+unpack of 1 layer of 1 request ({nb1 / 2**20:.0f} MiB FP16 KV), 1 thread"},
+            "importance": {"seconds": t_imp, "cores": threads,
+                           "sample": f"oracle importance (float64) of 1 layer truncated to {n_imp} of {cfg.n} tokens, "
+                                     f"window {cfg.w}, {cfg.Hq} query heads, OpenMP as the oracle has it",
+                           "seconds_per_layer_extrapolated": t_imp * cfg.n / n_imp,
+                           "seconds_per_request_extrapolated": t_imp * cfg.n / n_imp * cfg.L},
+            "assign": {"seconds": t_asg, "cores": 1, "sample": f"oracle assign (qsort) of 1 layer of {cfg.n} tokens",
+                       "seconds_per_request_extrapolated": t_asg * cfg.L}}
 
 
 def run_reference(args, cfg, b, R):
@@ -502,8 +694,9 @@ def run_reference(args, cfg, b, R):
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * mean, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f16 -> i8/i4 codes (exact products, f32 scales)",
-            "data": "synthetic", "config": config_json(cfg, b, R),
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+            "data": "synthetic", "config": config_json(cfg, b, R, l2="CPU arm: not applicable"),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample,
+                             "cpu_model": cpu_model()},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -528,87 +721,85 @@ def main():
     lib()                                              # fail loudly if the CUDA library is missing
 
     prob = DeviceProblem(cfg, b, R, dev, rank)
-    for _ in range(max(args.warmup, 3)):
-        prob.step()
-    torch.cuda.synchronize()
+    flush = want_flush(args, cfg, R)
     K = args.steps
-    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(5)] for _ in range(K)]
+    W = max(args.warmup, 3)
     sampler = ClockSampler(local)
-    barrier()
-    torch.cuda.synchronize()
-    sampler.start()
-    sampler.wait_first_sample()
-    t_wall0 = time.perf_counter()
-    t_abs0 = time.time()
-    for k in range(K):
-        prob.step(ev[k])
-    torch.cuda.synchronize()
-    barrier()
-    t_wall = time.perf_counter() - t_wall0
-    clocks = sampler.stop(t_abs0, time.time())
-
-    total_ms = ev[0][0].elapsed_time(ev[K - 1][4])
-    stage_ms = [sum(ev[k][i].elapsed_time(ev[k][i + 1]) for k in range(K)) / K for i in range(4)]
-    stage_min = [min(ev[k][i].elapsed_time(ev[k][i + 1]) for k in range(K)) for i in range(4)]
+    res = time_problem(prob, K, W, flush, sampler=sampler, dev=dev)
+    clocks, t_wall = res["clocks"], res["wall_s"]
     bytes_local = cfg.bytes_fp16 * R
-    red, bytes_all = aggregate_over_ranks([total_ms / K] + stage_ms, bytes_local, device=dev)
+    red, bytes_all = aggregate_over_ranks([res["ms_step"]] + res["stage_ms"], bytes_local, device=dev)
     ms_step, (ms_imp, ms_asg, ms_pack, ms_unpack) = red[0], red[1:]
+    stage_min = res["stage_min"]
     value = bytes_all / ((ms_pack + ms_unpack) * 1e-3) / 1e9
+    peak, peak_src = measured_peak()
 
+    sweep = None
+    if not args.no_sweep and world == 1:
+        sweep = run_sweep(args, prob, dev, peak, min(K, 10))
     next_rows = None if args.no_next else run_next_rows(prob, min(K, 10))
     e2e = None
     if not args.no_e2e:
-        r = run_e2e(cfg, b, R, dev, steps=min(K, 3), warmup=1, chunk_layers=args.e2e_chunk_layers, depth=args.e2e_depth)
+        r = run_e2e(cfg, b, R, dev, steps=min(K, 3), warmup=1, chunk_layers=args.e2e_chunk_layers, depth=args.e2e_depth,
+                    host_requests=1 if world > 1 else 2)
         red2, _ = aggregate_over_ranks([r["ms_per_step"]], bytes_local, device=dev)
-        e2e = {"value": bytes_all / (red2[0] * 1e-3) / 1e9, "unit": "GB/s of FP16 KV, whole path from pinned host buffers",
+        e2e = {"value": bytes_all / (red2[0] * 1e-3) / 1e9, "unit": UNIT,
+               "what": "GB/s of FP16 KV through the whole path from pinned host buffers (H2D K,V,Q; D2H + H2D hop of the blob; D2H result)",
                "h2d_bytes_per_step": r["h2d"], "d2h_bytes_per_step": r["d2h"], "ms_per_step": red2[0], "steps": r["steps"],
                "ms_per_request": red2[0] / R, "pipeline": f"layer chunks of {r['layers_per_chunk']}, {r['depth']} slots, 3 streams",
+               "pinned_host_requests": r["host_requests"],
                "sequential_ms_per_request": r["sequential_ms_per_request"],
                "raw_fp16_hop_ms_per_request": r["raw_fp16_hop_ms_per_request"],
                "blob_hop_ms_per_request": r["blob_hop_ms_per_request"]}
 
     if rank != 0:
         return
-    peak, peak_src = measured_peak()
     alg = prob.algorithmic_bytes()
     dom = "pack" if ms_pack >= ms_unpack else "unpack"
     dom_ms = max(ms_pack, ms_unpack)
     achieved = alg[dom] / (dom_ms * 1e-3) / 1e9
-    traffic = ncu_traffic(args.workload, b, R, dom)
+    traffic, traffic_src = ncu_traffic(args.workload, b, R, dom)
+    imp_flop = 2.0 * cfg.L * cfg.Hq * cfg.w * cfg.n * cfg.d * R
+    tpeak, tpeak_src = measured_tensor_peak()
+    fused = cfg.n <= FUSE_MAX_TOKENS
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": max(args.warmup, 3),
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f16 -> i8/i4 codes (quantiser arithmetic in f32); importance f16 x f16 -> f32",
-        "data": "synthetic", "config": config_json(cfg, b, R),
+        "data": "synthetic", "config": config_json(cfg, b, R, l2=l2_note(cfg, R, prob.blob_bytes, flush)),
         "stages_ms": {"importance": ms_imp, "assign": ms_asg, "pack": ms_pack, "unpack": ms_unpack},
         "stages_ms_min": dict(zip(STAGES, stage_min)),
         "ms_per_request_on_gpu": ms_step / R,
         "frac_of_hbm_peak_pack_plus_unpack": (alg["pack"] + alg["unpack"]) / ((ms_pack + ms_unpack) * 1e-3) / 1e9 / peak,
-        "roofline": {"bound": "hbm", "kernel": dom + "_kernel (+ tile_scan, < 1 % of the stage)", "achieved": achieved,
+        "roofline": {"bound": "hbm",
+                     "kernel": f"{dom}_fast_kernel" + ("" if fused else " (+ tile_scan_kernel, < 1 % of the stage)"),
+                     "achieved": achieved,
                      "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": achieved / peak,
-                     "algorithmic_bytes_per_launch": alg[dom], "avg_launch_ms": dom_ms, "traffic": traffic,
+                     "algorithmic_bytes_per_launch": alg[dom], "avg_launch_ms": dom_ms,
+                     "traffic": traffic, "traffic_source": (f"recorded ncu --set full capture, {TRAFFIC_FILE}: {traffic_src}"
+                                                            if traffic is not None else None),
                      "other": {k: {"achieved": alg[k] / (m * 1e-3) / 1e9, "frac": alg[k] / (m * 1e-3) / 1e9 / peak}
                                for k, m in (("pack", ms_pack), ("unpack", ms_unpack))},
                      "frac_of_nominal_8TBs": achieved / 8000.0},
-        "importance": {"ms": ms_imp, "useful_tflops": 2.0 * cfg.L * cfg.Hq * cfg.w * cfg.n * cfg.d * R / (ms_imp * 1e-3) / 1e12,
-                       "executed_tflops": 4.0 * cfg.L * cfg.Hq * cfg.w * cfg.n * cfg.d * R / (ms_imp * 1e-3) / 1e12,
+        "importance": {"ms": ms_imp, "useful_tflops": imp_flop / (ms_imp * 1e-3) / 1e12,
+                       "executed_tflops": 2.0 * imp_flop / (ms_imp * 1e-3) / 1e12,
                        "note": "two-pass: the contraction and the exponentials run twice; bound by the MUFU ex2 / FMA / "
-                               "tensor pipe mix at d_h = 128 (profiles/r1_full_v4_ncu.md), not by the tensor pipe alone",
-                       "tensor_peak_tflops": measured_tensor_peak()[0], "tensor_peak_source": measured_tensor_peak()[1],
-                       "useful_frac_of_tensor_peak": 2.0 * cfg.L * cfg.Hq * cfg.w * cfg.n * cfg.d * R / (ms_imp * 1e-3) / 1e12 / measured_tensor_peak()[0],
-                       "executed_frac_of_tensor_peak": 4.0 * cfg.L * cfg.Hq * cfg.w * cfg.n * cfg.d * R / (ms_imp * 1e-3) / 1e12 / measured_tensor_peak()[0]},
-        "clocks": clocks, "gpu_launches": LAUNCHES_PER_STEP * K, "wall_s_timed_region": t_wall,
+                               "tensor pipe mix at d_h = 128 (profiles/r2_importance_ncu.md), not by the tensor pipe alone",
+                       "tensor_peak_tflops": tpeak, "tensor_peak_source": tpeak_src,
+                       "useful_frac_of_tensor_peak": imp_flop / (ms_imp * 1e-3) / 1e12 / tpeak,
+                       "executed_frac_of_tensor_peak": 2.0 * imp_flop / (ms_imp * 1e-3) / 1e12 / tpeak},
+        "clocks": clocks, "gpu_launches": launches_per_step(cfg) * K, "wall_s_timed_region": t_wall,
     }
+    if sweep is not None:
+        line["sweep"] = sweep
     if next_rows is not None:
         for v in next_rows.values():
             v["frac_of_hbm_peak"] = v["GBps"] / peak
         line["next_rows"] = next_rows
     if e2e is not None:
         line["e2e"] = e2e
-    if not args.no_cpu_baseline and world == 1:
-        gbs, threads, sample, secs, parts = oracle_sample(cfg, b, args.cpu_seconds)
-        line["cpu_baseline"] = {"value": gbs, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample,
-                                "seconds": secs, **parts}
+    if not args.no_cpu_baseline:
+        line["cpu_baseline"] = oracle_sample(cfg, b, args.cpu_seconds)        # rank 0 only (the other ranks returned above)
     print(json.dumps(line), flush=True)
 
 

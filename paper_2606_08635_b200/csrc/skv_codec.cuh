@@ -39,6 +39,58 @@ __device__ __forceinline__ void st_stream(void *p, uint32_t v)
     asm volatile("st.global.L1::no_allocate.u32 [%0], %1;" :: "l"(p), "r"(v) : "memory");
 }
 
+// Resident CTAs per SM the fast pack / unpack kernels are compiled for (register cap 65536 / (256 * value)).  A lane
+// keeps 2 * NCH 16-byte loads in flight, so short rows (NCH = 2 or 1: rows of 512 or 256 elements, e.g. 4 KV heads of 128)
+// need more resident warps than long ones to cover the HBM latency.
+#ifndef SKV_MINB_NCH2
+#define SKV_MINB_NCH2 4
+#endif
+#ifndef SKV_MINB_NCH1
+#define SKV_MINB_NCH1 5
+#endif
+template <int NCH> struct MinBlocks { static constexpr int value = (NCH >= 4) ? 3 : (NCH == 2) ? SKV_MINB_NCH2 : SKV_MINB_NCH1; };
+
+// ------------------------------------------------------------------------------------------------
+// Fused slot scan (short sequences, n <= kFuseMaxTokens): the whole CTA counts the FP16 / INT8 / low-tier bytes of
+// the layer's tier map below its own tile -- the same exclusive counts tile_scan_kernel would have left in
+// tile_base[tile] -- so that pack and unpack are ONE launch each.  Every thread returns the counts.  Contains CTA-wide
+// barriers: call it from CTA-uniform control flow.  sCnt: 16 words of shared memory.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint4 self_tile_base(const uint8_t *__restrict__ tm, int64_t tile, uint32_t low, uint32_t *sCnt)
+{
+    const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int64_t chunks = tile * (kTileTokens / 16);                 // 16-byte chunks below the tile
+    const uint32_t lowrep = low * 0x01010101u;
+    uint32_t a = 0 /* #16 | #8 << 16 */, b = 0 /* #low */;
+    if ((reinterpret_cast<uintptr_t>(tm) & 15) == 0) {
+        for (int64_t c = tid; c < chunks; c += blockDim.x) {
+            const uint4 v = reinterpret_cast<const uint4 *>(tm)[c];
+            const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                a += (uint32_t)(__popc(__vcmpeq4(w[k], 0x10101010u)) >> 3) + ((uint32_t)(__popc(__vcmpeq4(w[k], 0x08080808u)) >> 3) << 16);
+                b += (uint32_t)(__popc(__vcmpeq4(w[k], lowrep)) >> 3);
+            }
+        }
+    } else {
+        for (int64_t c = tid; c < chunks; c += blockDim.x)
+            for (int k = 0; k < 16; ++k) {
+                const uint32_t t = tm[c * 16 + k];
+                a += (t == 16u) + ((uint32_t)(t == 8u) << 16);
+                b += (t == low);
+            }
+    }
+    a = __reduce_add_sync(0xffffffffu, a);
+    b = __reduce_add_sync(0xffffffffu, b);
+    __syncthreads();                                                  // sCnt may still be read by a previous call
+    if (lane == 0) { sCnt[warp] = a; sCnt[8 + warp] = b; }
+    __syncthreads();
+    uint32_t sa = 0, sb = 0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { sa += sCnt[i]; sb += sCnt[8 + i]; }
+    return make_uint4(sa & 0xFFFFu, sa >> 16, sb, 0u);
+}
+
 // ------------------------------------------------------------------------------------------------
 // Element types of a cache: binary16 (the paper's FP16) or bfloat16 (reading P20).  The kernels are
 // templates on one of these traits; everything that differs between the two formats is an overload below.
@@ -247,7 +299,13 @@ __device__ __forceinline__ float inv3_of(float r)
     const float q = r != 0.0f ? __fdiv_rn(3.0f, r) : 0.0f;
     return (q <= 3.402823466e38f) ? q : 0.0f;
 }
-__device__ __forceinline__ float step3_of(float r) { return r != 0.0f ? __fdiv_rn(r, 3.0f) : 0.0f; }
+// r/3; a bfloat16 range beyond FLT_MAX (r = +Inf; the encoder's 3/Inf = 0 gave all-zero codes) takes step = 0, so the vector
+// decodes to lo instead of fma(0, Inf, lo) = NaN (P20)
+__device__ __forceinline__ float step3_of(float r)
+{
+    const float q = r != 0.0f ? __fdiv_rn(r, 3.0f) : 0.0f;
+    return (q <= 3.402823466e38f) ? q : 0.0f;
+}
 // 8 fp16 -> 8 two-bit codes (16 bits; element k in bits 2k..2k+1).  q_k = rint(fl32(x_k - lo) * inv), the product exact
 // and rounded once: the whole word is built in the mantissa of one float by a chain of fused multiply-adds,
 //     a <- fma(dx_k, inv, a)      adds q_k (a is an even integer in [2^23, 2^24), so the FMA's rounding is RNE of the product)
@@ -259,6 +317,9 @@ __device__ __forceinline__ uint32_t quant8_int2(const uint4 &v, float lo, float 
     const float2 p0 = to_f2(as_pair<H2>(v.x)), p1 = to_f2(as_pair<H2>(v.y));
     const float2 p2 = to_f2(as_pair<H2>(v.z)), p3 = to_f2(as_pair<H2>(v.w));
     const float x[8] = {p0.x, p0.y, p1.x, p1.y, p2.x, p2.y, p3.x, p3.y};
+    // inv = 0 (zero range, or a bfloat16 range / reciprocal beyond binary32, P20) means "all codes 0"; x - lo may be +Inf
+    // there, and Inf * 0 is no code, so the subtraction runs against 0 instead (x is finite: x * 0 = 0)
+    lo = (inv != 0.0f) ? lo : 0.0f;
     float a = __fmaf_rn(__fsub_rn(x[7], lo), inv, 12582912.0f);
 #pragma unroll
     for (int k = 6; k >= 0; --k) {

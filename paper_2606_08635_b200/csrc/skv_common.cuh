@@ -31,6 +31,17 @@ struct Geom {
 };
 
 constexpr int kTileTokens = 32;  // tokens per pack/unpack tile (one ballot word)
+#ifndef SKV_FUSE_MAX_TOKENS
+#define SKV_FUSE_MAX_TOKENS 8192
+#endif
+constexpr int kFuseMaxTokens = SKV_FUSE_MAX_TOKENS;   // up to this n a pack / unpack CTA counts the tiers below its tile itself (one launch)
+
+// Where a pack / unpack CTA gets its tiles and their slot bases from.
+//   tile_base != nullptr: from tile_scan_kernel (skv_scan.cu), [R][L][tiles]; nullptr = "fused": the CTA counts the
+//                         tier-map bytes below its tile itself and also writes the stage's metadata;
+//   live_count != nullptr: sparse blob -- only the live_count[r][l] tiles listed in tile_base[r][l][idx].w carry
+//                         tokens, and the grid strides over that list.
+struct TileSrc { const uint4 *tile_base; const uint32_t *live_count; };
 
 struct Header256 { uint32_t w[64]; };   // the 256-byte SKV1 header image, built on the host
 
@@ -41,25 +52,25 @@ Layout make_layout(int L, int Hkv, int D, int64_t n, int64_t n16, int64_t n8, in
 
 // launchers (one per .cu)
 cudaError_t launch_tile_scan_pack(const Geom &g, const Layout &lo, const uint8_t *tier_map, uint8_t *blob,
-                                  uint64_t blob_stride, const Header256 &hdr, uint4 *tile_base, cudaStream_t s);
+                                  uint64_t blob_stride, const Header256 &hdr, uint4 *tile_base, uint32_t *live_count,
+                                  cudaStream_t s);
+// grid_x: CTAs per (layer, request) -- the number of tiles, or fewer when the grid strides over a sparse live list
 cudaError_t launch_pack(const Geom &g, const Layout &lo, const __half *K, const __half *V, const uint8_t *tier_map,
-                        uint8_t *blob, uint64_t blob_stride, const uint4 *tile_base, cudaStream_t s);
+                        uint8_t *blob, uint64_t blob_stride, const Header256 &hdr, TileSrc ts, int grid_x, cudaStream_t s);
 cudaError_t launch_tile_scan_unpack(const Geom &g, const Layout &lo, const uint8_t *blob, uint64_t blob_stride,
-                                    uint8_t *tier_map_out, uint4 *tile_base, cudaStream_t s);
+                                    uint8_t *tier_map_out, uint4 *tile_base, uint32_t *live_count, cudaStream_t s);
 cudaError_t launch_unpack(const Geom &g, const Layout &lo, const uint8_t *blob, uint64_t blob_stride,
-                          __half *K, __half *V, const uint4 *tile_base, cudaStream_t s);
+                          __half *K, __half *V, uint8_t *tier_map_out, TileSrc ts, int grid_x, cudaStream_t s);
 
 struct Intervals { int32_t count; int32_t lo[32]; int32_t hi[32]; };   // merged protected ranges (incl. sinks)
 cudaError_t launch_assign(const Geom &g, const Intervals &prot, const float *importance, uint8_t *tier_map,
                           uint32_t *key_ws, cudaStream_t s);
 
-cudaError_t launch_importance(const Geom &g, const __half *K, const __half *Q, int window, int causal, float lambda,
-                              float *importance, void *ws, size_t ws_bytes, cudaStream_t s);
-size_t importance_ws_bytes(const Geom &g, int window);
 cudaError_t launch_importance_tc(const Geom &g, const __half *K, const __half *Q, int window, int causal, float lambda,
                                  float *importance, void *ws, cudaStream_t s);
-size_t importance_tc_ws_bytes(const Geom &g, int window);
-cudaError_t launch_importance_kvnorm(const Geom &g, const __half *K, float lambda, float *importance, float *ws,
+size_t importance_tc_ws_bytes(const Geom &g, int window);      // 0: the work decomposition does not fit
+cudaError_t launch_importance_kvnorm(const Geom &g, const __half *K, float lambda, float *importance, void *ws,
                                      cudaStream_t s);
+size_t kvnorm_ws_bytes(const Geom &g);
 
 }  // namespace skv

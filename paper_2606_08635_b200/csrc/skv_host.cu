@@ -98,10 +98,38 @@ static bool counts_wire_ok(const skv_shape *s, const skv_counts *c)
     return c->budget_q4 >= spent && c->budget_q4 <= unit * (int64_t)s->n_tokens;
 }
 
-static size_t scan_ws_bytes(const skv_shape *s)
+// workspace of pack / unpack: the tile prefix table uint4[R][L][tiles] (.w = the list of live tiles of a sparse blob),
+// then the live-tile counts u32[R][L]
+static size_t scan_table_bytes(const skv_shape *s)
 {
     const size_t tiles = ((size_t)s->n_tokens + kTileTokens - 1) / kTileTokens;
     return (size_t)s->n_requests * s->n_layers * tiles * sizeof(uint4);
+}
+static size_t scan_ws_bytes(const skv_shape *s)
+{
+    return scan_table_bytes(s) + (size_t)s->n_requests * s->n_layers * sizeof(uint32_t);
+}
+
+// How a pack / unpack stage is launched (skv_common.cuh: TileSrc).
+//   fused  (n <= kFuseMaxTokens): one launch, every CTA counts the tiers below its own tile;
+//   sparse (fewer than 1 token in 8 is shipped, no 2-bit tier, and empty tiles need no work: pack, unpack_patch): the scan emits the
+//          list of live tiles and the grid strides over it -- a cold-tier upgrade of 1024 tokens of a 32 K-token layer
+//          touches at most 1024 of its tiles, typically a few dozen;
+//   otherwise the scan kernel, then one CTA per tile.
+struct StagePlan { bool fused, sparse; int grid_x; };
+static StagePlan plan_stage(const Geom &g, bool empty_tiles_skippable)
+{
+    StagePlan p;
+    const int64_t shipped = (int64_t)g.n16 + g.n8 + g.n4;
+    p.sparse = empty_tiles_skippable && shipped * 8 <= (int64_t)g.n && g.tiles > 1 && g.low_code != 2;
+    p.fused = !p.sparse && g.n <= kFuseMaxTokens;
+    p.grid_x = g.tiles;
+    if (p.sparse) {
+        const int64_t live_max = std::max<int64_t>(1, std::min<int64_t>(g.tiles, shipped));
+        const int64_t want = std::max<int64_t>(1, 4096 / ((int64_t)g.L * g.R));      // ~9 waves of CTAs in total
+        p.grid_x = (int)std::min(live_max, want);
+    }
+    return p;
 }
 
 // merged, sorted protected intervals = [0,s) U ranges; returns P (their total size) or <0 on error
@@ -218,11 +246,11 @@ size_t skv_workspace_bytes(const skv_shape *shape, int32_t window)
     const Geom g = make_geom(shape, nullptr);
     size_t need = scan_ws_bytes(shape);
     need = std::max(need, (size_t)shape->n_requests * shape->n_layers * shape->n_tokens * sizeof(uint32_t));  // assign keys
-    need = std::max(need, importance_ws_bytes(g, 0));
+    need = std::max(need, kvnorm_ws_bytes(g));
     if (window > 0) {
         // the importance plan divides by (Hq / Hkv) * window: refuse what skv_importance itself refuses
         if (shape->n_q_heads <= 0 || shape->n_q_heads % shape->n_kv_heads || window > shape->n_tokens) return 0;
-        const size_t imp = importance_ws_bytes(g, window);
+        const size_t imp = importance_tc_ws_bytes(g, window);
         if (imp == 0) return 0;                                          // work decomposition does not fit 32-bit counters
         need = std::max(need, imp);
     }
@@ -280,11 +308,11 @@ int skv_importance(const skv_shape *shape, const void *K_dev, const void *Q_dev,
     if (!(lambda >= 0.0f)) return SKV_ERR_INVALID_ARG;
     if ((uintptr_t)Q_dev & 15) return SKV_ERR_UNSUPPORTED;
     const Geom g = make_geom(shape, nullptr);
-    const size_t need = importance_ws_bytes(g, window);
+    const size_t need = importance_tc_ws_bytes(g, window);
     if (need == 0) return SKV_ERR_UNSUPPORTED;                            // R*L*Hkv*key-chunk items overflow 32 bits
     if (ws_bytes < need) return SKV_ERR_BUFFER_TOO_SMALL;
-    cudaError_t e = launch_importance(g, (const __half *)K_dev, (const __half *)Q_dev, window, causal ? 1 : 0, lambda,
-                                      importance_dev, ws, ws_bytes, (cudaStream_t)cuda_stream);
+    cudaError_t e = launch_importance_tc(g, (const __half *)K_dev, (const __half *)Q_dev, window, causal ? 1 : 0, lambda,
+                                         importance_dev, ws, (cudaStream_t)cuda_stream);
     return e == cudaSuccess ? SKV_OK : SKV_ERR_CUDA;
 }
 
@@ -295,9 +323,8 @@ int skv_importance_kvnorm(const skv_shape *shape, const void *K_dev, float lambd
     if (rc) return rc;
     if (!importance_dev || !ws || !(lambda >= 0.0f)) return SKV_ERR_INVALID_ARG;
     const Geom g = make_geom(shape, nullptr);
-    if (ws_bytes < importance_ws_bytes(g, 0)) return SKV_ERR_BUFFER_TOO_SMALL;
-    cudaError_t e = launch_importance_kvnorm(g, (const __half *)K_dev, lambda, importance_dev, (float *)ws,
-                                             (cudaStream_t)cuda_stream);
+    if (ws_bytes < kvnorm_ws_bytes(g)) return SKV_ERR_BUFFER_TOO_SMALL;
+    cudaError_t e = launch_importance_kvnorm(g, (const __half *)K_dev, lambda, importance_dev, ws, (cudaStream_t)cuda_stream);
     return e == cudaSuccess ? SKV_OK : SKV_ERR_CUDA;
 }
 
@@ -378,10 +405,15 @@ int skv_pack(const skv_shape *shape, const void *K_dev, const void *V_dev, const
     put64(h + 160, lo.total_bytes);
 
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    cudaError_t e = launch_tile_scan_pack(g, lo, tier_map_dev, (uint8_t *)blob_dev, lo.total_bytes, hdr, (uint4 *)ws, st);
-    if (e != cudaSuccess) return SKV_ERR_CUDA;
-    e = launch_pack(g, lo, (const __half *)K_dev, (const __half *)V_dev, tier_map_dev, (uint8_t *)blob_dev,
-                    lo.total_bytes, (const uint4 *)ws, st);
+    const StagePlan plan = plan_stage(g, true);
+    uint32_t *live = plan.sparse ? reinterpret_cast<uint32_t *>((uint8_t *)ws + scan_table_bytes(shape)) : nullptr;
+    TileSrc ts = {plan.fused ? nullptr : (const uint4 *)ws, live};
+    if (!plan.fused) {
+        cudaError_t e = launch_tile_scan_pack(g, lo, tier_map_dev, (uint8_t *)blob_dev, lo.total_bytes, hdr, (uint4 *)ws, live, st);
+        if (e != cudaSuccess) return SKV_ERR_CUDA;
+    }
+    cudaError_t e = launch_pack(g, lo, (const __half *)K_dev, (const __half *)V_dev, tier_map_dev, (uint8_t *)blob_dev,
+                                lo.total_bytes, hdr, ts, plan.grid_x, st);
     return e == cudaSuccess ? SKV_OK : SKV_ERR_CUDA;
 }
 
@@ -399,10 +431,15 @@ static int unpack_impl(const skv_shape *shape, const void *blob_dev, size_t blob
     if (blob_bytes != (size_t)lo.total_bytes) return SKV_ERR_BAD_BLOB;
     if (ws_bytes < scan_ws_bytes(shape)) return SKV_ERR_BUFFER_TOO_SMALL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    cudaError_t e = launch_tile_scan_unpack(g, lo, (const uint8_t *)blob_dev, lo.total_bytes, tier_map_out_dev, (uint4 *)ws, st);
-    if (e != cudaSuccess) return SKV_ERR_CUDA;
-    e = launch_unpack(g, lo, (const uint8_t *)blob_dev, lo.total_bytes, (__half *)K_out_dev, (__half *)V_out_dev,
-                      (const uint4 *)ws, st);
+    const StagePlan plan = plan_stage(g, patch != 0);               // a full unpack writes zeros into the empty tiles too
+    uint32_t *live = plan.sparse ? reinterpret_cast<uint32_t *>((uint8_t *)ws + scan_table_bytes(shape)) : nullptr;
+    TileSrc ts = {plan.fused ? nullptr : (const uint4 *)ws, live};
+    if (!plan.fused) {
+        cudaError_t e = launch_tile_scan_unpack(g, lo, (const uint8_t *)blob_dev, lo.total_bytes, tier_map_out_dev, (uint4 *)ws, live, st);
+        if (e != cudaSuccess) return SKV_ERR_CUDA;
+    }
+    cudaError_t e = launch_unpack(g, lo, (const uint8_t *)blob_dev, lo.total_bytes, (__half *)K_out_dev, (__half *)V_out_dev,
+                                  tier_map_out_dev, ts, plan.grid_x, st);
     return e == cudaSuccess ? SKV_OK : SKV_ERR_CUDA;
 }
 

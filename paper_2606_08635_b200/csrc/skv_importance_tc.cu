@@ -55,7 +55,26 @@ struct Params {
     const float *lse2;                  // [R][L][Hq*w]
     float *apart;                       // [R][L][S][n]
     unsigned int *gbar;                 // grid-barrier arrival counter (zeroed on the stream before the launch)
+#ifdef SKV_IMP_TRACE
+    unsigned long long *trace;          // diagnostics build only (never shipped): timestamps, see _TRACE macros below
+#endif
 };
+
+// Diagnostics hooks.  The product build defines none of SKV_IMP_TRACE / SKV_DIAG_*: every macro below expands to nothing.
+// A trace build logs globaltimer stamps of the phase boundaries of every CTA ([grid][16]) and clock64 stamps of the
+// per-tile pipeline events of CTA 0 ([512][8]) into a buffer handed over with skv_debug_set_trace().
+#ifdef SKV_IMP_TRACE
+__device__ unsigned long long *g_trace_ptr;
+__device__ int g_ev_tile;     // tile counter of the one epilogue thread that logs (CTA 0, warp 2, lane 0)
+#define SKV_EPI_LOGGER (blockIdx.x == 0 && threadIdx.x == 64)
+#define SKV_TRACE(slot, who) do { if (who) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); p.trace[blockIdx.x * 16 + (slot)] = t_; } } while (0)
+#define SKV_TRACE_EV(tile, k, who) do { if (blockIdx.x == 0 && (tile) >= 0 && (tile) < 512 && (who)) g_trace_ptr[148 * 16 + (tile) * 8 + (k)] = (unsigned long long)clock64(); } while (0)
+#define SKV_TRACE_ONLY(x) x
+#else
+#define SKV_TRACE(slot, who)
+#define SKV_TRACE_EV(tile, k, who)
+#define SKV_TRACE_ONLY(x)
+#endif
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -78,6 +97,21 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
         "WAIT_%=:\n\t"
         "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
         "@p bra DONE_%=;\n\t"
+        "bra WAIT_%=;\n\t"
+        "DONE_%=:\n\t}"
+        :: "r"(bar), "r"(parity) : "memory");
+}
+// The same wait for the two single-thread control roles (TMA producer, MMA issuer): they run a whole tile ahead of the
+// epilogue, so a failed probe sleeps before the next one instead of competing with the epilogue warps of its scheduler
+// for issue slots.
+__device__ __forceinline__ void mbar_wait_ctrl(uint32_t bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\t"
+        "nanosleep.u32 64;\n\t"
         "bra WAIT_%=;\n\t"
         "DONE_%=:\n\t}"
         :: "r"(bar), "r"(parity) : "memory");
@@ -217,12 +251,22 @@ __device__ __forceinline__ void tmem_wait_ld(uint32_t (&r)[16])
                  :: "memory");
 }
 
-// One tile = NCH chunks; b0 holds (or is about to receive) chunk 0.  chunk(regs, c) consumes a chunk, and the next
-// tile's first chunk is requested while the last chunk of this one is being consumed.  The caller hands the stage
-// back (release_stage) once it no longer needs TMEM: the MMA warp is a whole tile ahead, so a late release costs nothing.
+__device__ __forceinline__ void release_stage(uint32_t tempty, uint32_t stage, int lane)
+{
+    tc_fence_before();
+    __syncwarp();
+    if (lane == 0) mbar_arrive(tempty + 8 * stage);
+}
+
+// One tile = NCH chunks; b0 holds (or is about to receive) chunk 0.  chunk(regs, c) consumes a chunk.  The accumulator
+// stage goes back to the MMA warp the moment the tile's LAST chunk has landed in registers -- before that chunk's
+// arithmetic and before the wait for the next tile -- because with two 256-column stages the MMA of tile i+2 can only
+// start then, and the chain  release -> MMA (~1400 clk) -> commit -> next tile visible  must fit inside the arithmetic
+// of ONE tile (measured with per-tile clock stamps: releasing after the arithmetic left the epilogue idle ~20 % of the
+// time).  Nothing may read the tile's TMEM after its last chunk is in registers (pass 1 rescues from registers).
 template <int NCH, int ACOLS, class ChunkFn>
 __device__ __forceinline__ void stream_tile(uint32_t (&b0)[16], uint32_t (&b1)[16], uint32_t base, bool more, uint32_t tfull,
-                                            uint32_t &astage, uint32_t &aphase, ChunkFn &&chunk)
+                                            uint32_t tempty, int lane, uint32_t &astage, uint32_t &aphase, ChunkFn &&chunk)
 {
     const uint32_t tile_addr = base + astage * ACOLS;
 #pragma unroll
@@ -231,9 +275,13 @@ __device__ __forceinline__ void stream_tile(uint32_t (&b0)[16], uint32_t (&b1)[1
         uint32_t (&nxt)[16] = (c & 1) ? b0 : b1;
         tmem_wait_ld(cur);
         if (c == NCH - 1) {
+            SKV_TRACE_EV(g_ev_tile, 4, SKV_EPI_LOGGER);          // last chunk of this tile has landed in registers
+            release_stage(tempty, astage, lane);
+            SKV_TRACE_EV(g_ev_tile, 6, SKV_EPI_LOGGER);          // stage handed back
             if (++astage == 512 / ACOLS) { astage = 0; aphase ^= 1; }
             if (more) {
                 mbar_wait(tfull + 8 * astage, aphase);
+                SKV_TRACE_EV(g_ev_tile + 1, 3, SKV_EPI_LOGGER);  // next tile's accumulator seen ready
                 tc_fence_after();
                 tmem_ld16_issue(base + astage * ACOLS, nxt);
             }
@@ -242,12 +290,6 @@ __device__ __forceinline__ void stream_tile(uint32_t (&b0)[16], uint32_t (&b1)[1
         }
         chunk(cur, c);
     }
-}
-__device__ __forceinline__ void release_stage(uint32_t tempty, uint32_t stage, int lane)
-{
-    tc_fence_before();
-    __syncwarp();
-    if (lane == 0) mbar_arrive(tempty + 8 * stage);
 }
 
 // 2^x for a PAIR of values on the FMA/ALU pipes with the packed fp32 instructions of sm_100 (FFMA2 / FADD2):
@@ -273,8 +315,8 @@ __device__ __forceinline__ float2 ex2_fma2_lo(float2 x)
 // pass 1, one work item: every epilogue thread owns one query row and 16*NCH key columns of each 128-key tile and
 // keeps the row's (reference exponent m, sum z of 2^(x - m)) in registers.  The reference exponent is lazy: it is
 // fixed by the first visible chunk of the row and only an overflow guard watches it afterwards (the row sum is
-// z * 2^m for ANY m, so no per-element max is needed); a tile that trips the guard is read again from TMEM and
-// folded in with the exact online-max update (the rare rescue path).
+// z * 2^m for ANY m, so no per-element max is needed); a chunk that trips the guard is redone, by the rows concerned
+// and from the 16 logits still in registers, with the exact online-max update (the rare rescue path).
 template <int D, int NCH>
 __device__ __forceinline__ void rowstats_segment(const Params &p, const Seg &it, uint32_t tmem, uint32_t tfull, uint32_t tempty,
                                                  uint32_t &astage, uint32_t &aphase, int quad, int grp, int lane,
@@ -304,10 +346,7 @@ __device__ __forceinline__ void rowstats_segment(const Params &p, const Seg &it,
     }
     int k0 = key_beg;
     for (; k0 < key_end && k0 < mask_from; k0 += kTileKeys) {             // ---- fast tiles
-        const uint32_t stage = astage;
-        float2 accA = make_float2(0.f, 0.f), accB = accA;
-        float xmax = kNegBig;                                             // largest exponent sent to the FMA pipe
-        stream_tile<NCH, ACOLS>(bA, bB, base, k0 + kTileKeys < key_end, tfull, astage, aphase,
+        stream_tile<NCH, ACOLS>(bA, bB, base, k0 + kTileKeys < key_end, tfull, tempty, lane, astage, aphase,
             [&](const uint32_t (&r)[16], int c) {
                 if (c == 0 && m < 0.5f * kNegBig) {
                     float tmax = kNegBig;
@@ -316,6 +355,8 @@ __device__ __forceinline__ void rowstats_segment(const Params &p, const Seg &it,
                     m = tmax * sc;
                 }
                 const float2 nm2 = make_float2(-m, -m), sc2 = make_float2(sc, sc);
+                float2 accA = make_float2(0.f, 0.f), accB = accA;
+                float xmax = kNegBig;                                     // largest exponent sent to the FMA pipe
 #pragma unroll
                 for (int pi = 0; pi < 8; ++pi) {
                     const float2 x = __ffma2_rn(make_float2(__uint_as_float(r[2 * pi]), __uint_as_float(r[2 * pi + 1])), sc2, nm2);
@@ -324,39 +365,30 @@ __device__ __forceinline__ void rowstats_segment(const Params &p, const Seg &it,
                     else e = ex2_mufu2(x);
                     if (pi & 1) accB = __fadd2_rn(accB, e); else accA = __fadd2_rn(accA, e);
                 }
+                const float2 s2 = __fadd2_rn(accA, accB);
+                const float a = s2.x + s2.y;
+                // overflow guard of the lazy reference exponent, per chunk and per row: a row whose chunk trips it redoes
+                // the chunk with the exact online-max update, from the 16 logits still in registers (no TMEM re-read)
+                if (a < 1.0e30f && xmax < 127.0f) {
+                    z += a;
+                    if (!(z < 1.0e30f)) { z *= 0x1p-80f; m += 80.0f; }
+                } else {
+                    float tmax = kNegBig;
+#pragma unroll
+                    for (int i = 0; i < 16; ++i) tmax = fmaxf(tmax, __uint_as_float(r[i]));
+                    const float mn = fmaxf(m, tmax * sc);
+                    float acc = 0.f;
+#pragma unroll
+                    for (int i = 0; i < 16; ++i) acc += ex2(fmaf(__uint_as_float(r[i]), sc, -mn));
+                    z = z * ex2(m - mn) + acc;
+                    m = mn;
+                }
             });
-        const float2 s2 = __fadd2_rn(accA, accB);
-        const float a = s2.x + s2.y;
-        const bool ok = a < 1.0e30f && xmax < 127.0f;
-        if (__all_sync(0xffffffffu, ok)) {
-            z += a;
-            if (!(z < 1.0e30f)) { z *= 0x1p-80f; m += 80.0f; }
-        } else {
-            // a term overflowed in some row of this warp: the whole warp reads the tile again (tcgen05.ld is warp-
-            // collective) and the rows that tripped the guard redo it with the exact online-max update
-            float tmax = kNegBig;
-            for (int c = 0; c < NCH; ++c) {
-                float v[16];
-                tmem_ld16(base + stage * ACOLS + 16 * c, v);
-#pragma unroll
-                for (int i = 0; i < 16; ++i) tmax = fmaxf(tmax, v[i]);
-            }
-            const float mn = ok ? m : fmaxf(m, tmax * sc);
-            float acc = 0.f;
-            for (int c = 0; c < NCH; ++c) {
-                float v[16];
-                tmem_ld16(base + stage * ACOLS + 16 * c, v);
-#pragma unroll
-                for (int i = 0; i < 16; ++i) acc += ex2(fmaf(v[i], sc, -mn));
-            }
-            if (ok) { z += a; if (!(z < 1.0e30f)) { z *= 0x1p-80f; m += 80.0f; } }
-            else    { z = z * ex2(m - mn) + acc; m = mn; }
-        }
-        release_stage(tempty, stage, lane);
+        SKV_TRACE_EV(g_ev_tile, 5, SKV_EPI_LOGGER);              // arithmetic of the tile done
+        SKV_TRACE_ONLY(if (SKV_EPI_LOGGER) ++g_ev_tile;)
     }
     for (; k0 < key_end; k0 += kTileKeys) {                               // ---- masked tiles (the last ones of a layer)
-        const uint32_t stage = astage;
-        stream_tile<NCH, ACOLS>(bA, bB, base, k0 + kTileKeys < key_end, tfull, astage, aphase,
+        stream_tile<NCH, ACOLS>(bA, bB, base, k0 + kTileKeys < key_end, tfull, tempty, lane, astage, aphase,
             [&](const uint32_t (&r)[16], int c) {
                 const int j0 = k0 + col0 + 16 * c;
                 float tmax = kNegBig;
@@ -369,7 +401,6 @@ __device__ __forceinline__ void rowstats_segment(const Params &p, const Seg &it,
                 z = z * ex2(m - mn) + acc;
                 m = mn;
             });
-        release_stage(tempty, stage, lane);
     }
     if (valid) {
         const int cs = (NCH == 4) ? 2 : 4;
@@ -404,7 +435,6 @@ __device__ __forceinline__ void colsum_segment(const Params &p, const Seg &it, u
     bool par = false;                                                     // buffer holding chunk 0 of the tile (QC odd: alternates)
     for (int k0 = key_beg; k0 < key_end; k0 += kTileKeys) {
         const int j = k0 + quad * 32 + lane;
-        const uint32_t stage = astage;
         const bool more = k0 + kTileKeys < key_end;
         float mine;
         if (cols_full && k0 < mask_from) {                                // ---- fast tile
@@ -421,8 +451,8 @@ __device__ __forceinline__ void colsum_segment(const Params &p, const Seg &it, u
                     accB = __fadd2_rn(accB, pair_on_fma(2 * i + 1) ? ex2_fma2_lo(x1) : ex2_mufu2(x1));
                 }
             };
-            if (!par) stream_tile<QC, ACOLS>(bA, bB, base, more, tfull, astage, aphase, chunk);
-            else      stream_tile<QC, ACOLS>(bB, bA, base, more, tfull, astage, aphase, chunk);
+            if (!par) stream_tile<QC, ACOLS>(bA, bB, base, more, tfull, tempty, lane, astage, aphase, chunk);
+            else      stream_tile<QC, ACOLS>(bB, bA, base, more, tfull, tempty, lane, astage, aphase, chunk);
             const float2 s2 = __fadd2_rn(accA, accB);
             mine = s2.x + s2.y;
         } else {                                                          // ---- masked tile or padded column group
@@ -435,17 +465,16 @@ __device__ __forceinline__ void colsum_segment(const Params &p, const Seg &it, u
                 for (int i = 0; i < 16; ++i)
                     s0 += (j <= lim[i]) ? ex2(fmaf(__uint_as_float(r[i]), sc, sLse[cbeg + cc + i])) : 0.f;
             };
-            if (!par) stream_tile<QC, ACOLS>(bA, bB, base, more, tfull, astage, aphase, chunk);
-            else      stream_tile<QC, ACOLS>(bB, bA, base, more, tfull, astage, aphase, chunk);
+            if (!par) stream_tile<QC, ACOLS>(bA, bB, base, more, tfull, tempty, lane, astage, aphase, chunk);
+            else      stream_tile<QC, ACOLS>(bB, bA, base, more, tfull, tempty, lane, astage, aphase, chunk);
             mine = s0;
         }
         if (QC & 1) par = !par;
-        release_stage(tempty, stage, lane);
         // add the four column groups of this tile in a fixed order (deterministic): groups 1..3 drop their sums
         // into a 4-deep shared-memory ring and arrive on its mbarrier (they never block); group 0 waits for the
         // slot, adds and stores.  A warp is never more than (accumulator stages <= 4) tiles ahead of the slowest one
-        // (the MMA of tile i+stages needs every warp to have released tile i), so with kRing = 8 slots a slot is
-        // never overwritten before group 0 has read it.
+        // (the MMA of tile i+stages needs every warp to have released tile i, which it does before the arithmetic of
+        // that tile's last chunk), so with kRing = 8 slots a slot is never overwritten before group 0 has read it.
         float *red = sRed + rstage * (3 * kTileKeys);
         if (grp != 0) {
             red[(grp - 1) * kTileKeys + quad * 32 + lane] = mine;
@@ -485,12 +514,12 @@ __device__ __forceinline__ void run_pass(const CUtensorMap *tmK, const CUtensorM
             for (long long u = ubeg; u < uend;) {
                 const Seg it = seg_at(p, u, uend);
                 u += it.t1 - it.t0;
-                mbar_wait(sm.qempty, cu.qphase ^ 1); cu.qphase ^= 1;
+                mbar_wait_ctrl(sm.qempty, cu.qphase ^ 1); cu.qphase ^= 1;
                 mbar_expect_tx(sm.qfull, (uint32_t)(p.qrows * D * 2));
                 for (int kb = 0; kb < C::KB; ++kb)
                     tma_load_3d(sm.sQ + kb * C::Q_KB_STRIDE, tmQ, sm.qfull, kb * 64, it.rb * p.MB, (it.r * p.g.L + it.l) * p.g.Hkv + it.g);
                 for (int t = it.t0; t < it.t1; ++t) {
-                    mbar_wait(sm.kempty + 8 * cu.kstage, cu.kphase ^ 1);
+                    mbar_wait_ctrl(sm.kempty + 8 * cu.kstage, cu.kphase ^ 1);
                     mbar_expect_tx(sm.kfull + 8 * cu.kstage, (uint32_t)C::K_BYTES);
                     int c[5]; c[0] = 0;
                     c[p.kdim[0]] = it.g; c[p.kdim[1]] = t * kTileKeys; c[p.kdim[2]] = it.l; c[p.kdim[3]] = it.r;
@@ -504,14 +533,17 @@ __device__ __forceinline__ void run_pass(const CUtensorMap *tmK, const CUtensorM
     } else if (warp == 1) {
         // ===================== MMA issuer =====================
         if (lane == 0) {
+            SKV_TRACE_ONLY(int ev_tile = 0;)
             const uint32_t idesc = (PASS == 1) ? umma_idesc(128, kTileKeys, p.g.bf16) : umma_idesc(128, p.qrows, p.g.bf16);
             for (long long u = ubeg; u < uend;) {
                 const Seg it = seg_at(p, u, uend);
                 u += it.t1 - it.t0;
-                mbar_wait(sm.qfull, cu.qphase); cu.qphase ^= 1;
+                mbar_wait_ctrl(sm.qfull, cu.qphase); cu.qphase ^= 1;
                 for (int t = it.t0; t < it.t1; ++t) {
-                    mbar_wait(sm.tempty + 8 * cu.astage, cu.aphase ^ 1);
-                    mbar_wait(sm.kfull + 8 * cu.kstage, cu.kphase);
+                    mbar_wait_ctrl(sm.tempty + 8 * cu.astage, cu.aphase ^ 1);
+                    SKV_TRACE_EV(ev_tile, 0, PASS == 1);
+                    mbar_wait_ctrl(sm.kfull + 8 * cu.kstage, cu.kphase);
+                    SKV_TRACE_EV(ev_tile, 1, PASS == 1);
                     tc_fence_after();
                     const uint32_t kt = sm.sK + cu.kstage * C::K_BYTES;
                     const uint32_t acc = tmem + cu.astage * ACOLS;
@@ -534,6 +566,8 @@ __device__ __forceinline__ void run_pass(const CUtensorMap *tmK, const CUtensorM
                     }
                     umma_commit(sm.kempty + 8 * cu.kstage);    // smem stage free once these MMAs have read it
                     umma_commit(sm.tfull + 8 * cu.astage);     // accumulator ready for the epilogue
+                    SKV_TRACE_EV(ev_tile, 2, PASS == 1);
+                    SKV_TRACE_ONLY(++ev_tile;)
                     if (++cu.kstage == C::STAGES) { cu.kstage = 0; cu.kphase ^= 1; }
                     if (++cu.astage == ASTAGES) { cu.astage = 0; cu.aphase ^= 1; }
                 }
@@ -631,9 +665,15 @@ imp_fused_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant_
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
     Cursors cu = {0, 0, 0, 0, 0, 0, 0};
+    SKV_TRACE_ONLY(if (SKV_EPI_LOGGER) g_ev_tile = 0;)
+    SKV_TRACE_ONLY(if (blockIdx.x == 0 && threadIdx.x == 0) g_trace_ptr = p.trace;)
+    SKV_TRACE_ONLY(__syncthreads();)
+    SKV_TRACE(0, threadIdx.x == 0);
 
     run_pass<D, 1, VA>(&tmK, &tmQ, p, sm, tmem, cu, warp, lane);
+    SKV_TRACE(1, threadIdx.x == kThreads - 1);
     grid_barrier(p.gbar, gridDim.x);
+    SKV_TRACE(2, threadIdx.x == 0);
 
     {   // lse2[row] = m* + log2(sum_c z_c 2^(m_c - m*)) over the (reference exponent, sum) pairs of the row's pieces
         const int64_t rows = (int64_t)p.g.R * p.g.L * p.g.Hq * p.w;
@@ -654,10 +694,14 @@ imp_fused_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant_
             const_cast<float *>(p.lse2)[row] = m + log2f(z);
         }
     }
+    SKV_TRACE(3, threadIdx.x == 0);
     grid_barrier(p.gbar, 2 * gridDim.x);
+    SKV_TRACE(4, threadIdx.x == 0);
 
     run_pass<D, 2, VC>(&tmK, &tmQ, p, sm, tmem, cu, warp, lane);
+    SKV_TRACE(5, threadIdx.x == kThreads - 1);
     grid_barrier(p.gbar, 3 * gridDim.x);
+    SKV_TRACE(6, threadIdx.x == 0);
 
     {   // importance = (sum over (KV head, row block) partials in a fixed order) / (Hq w) * exp(-lambda (n-1-j))
         const int64_t total = (int64_t)p.g.R * p.g.L * p.g.n;
@@ -671,6 +715,7 @@ imp_fused_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant_
             importance[i] = sum * norm * expf(-lambda * (float)(p.g.n - 1 - j));
         }
     }
+    SKV_TRACE(7, threadIdx.x == 0);
     tc_fence_before();
     __syncthreads();
     if (warp == 1) {
@@ -697,6 +742,11 @@ static EncodeTiledFn get_encode_fn()
         return nullptr;
     return (EncodeTiledFn)fn;
 }
+
+#ifdef SKV_IMP_TRACE
+static unsigned long long *g_host_trace = nullptr;      // diagnostics build only: device buffer of (148 * 16 + 512 * 8) u64
+extern "C" void skv_debug_set_trace(void *dev_ptr) { g_host_trace = reinterpret_cast<unsigned long long *>(dev_ptr); }
+#endif
 
 struct TcPlan {
     int QROWS_MAX, RB, MB, qrows, halves, S, T, grid, pmax;
@@ -814,6 +864,9 @@ cudaError_t launch_importance_tc(const Geom &g, const __half *K, const __half *Q
     p.apart = reinterpret_cast<float *>(w8 + t.partial_bytes + t.lse_bytes);
     p.gbar = reinterpret_cast<unsigned int *>(w8 + t.partial_bytes + t.lse_bytes + t.apart_bytes);
     if (cudaMemsetAsync(p.gbar, 0, sizeof(unsigned int), s) != cudaSuccess) return cudaGetLastError();
+#ifdef SKV_IMP_TRACE
+    p.trace = g_host_trace;
+#endif
 
     int dev = 0, sms = kPlanSMs;
     cudaGetDevice(&dev);

@@ -3,8 +3,10 @@
 // One warp per token, one CTA per 32-token tile of one (request, layer).  The warp reads the token's K
 // row and V row with 16-byte loads (8 fp16 per lane, coalesced; any 16-B aligned strides), reduces the
 // |x| max over the lanes of a head vector with shuffles, quantises in fp32 exactly as include/skv.h
-// specifies, and stores the codes at the token's slot (tile base from skv_scan.cu + in-tile rank from a
-// ballot).  All lanes of a warp share one tier => no divergence.  Dropped tokens are never loaded.
+// specifies, and stores the codes at the token's slot (tile base + in-tile rank from a ballot).  The tile
+// base comes from skv_scan.cu (long sequences) or is counted by the CTA itself (n <= kFuseMaxTokens: pack
+// is then ONE launch, metadata included); a sparse blob (cold-tier upgrade) is walked through the scan's
+// list of live tiles.  All lanes of a warp share one tier => no divergence.  Dropped tokens are never loaded.
 //
 // HBM-bound: reads Bytes_FP16, writes beta*Bytes_FP16.
 #include "skv_codec.cuh"
@@ -19,6 +21,26 @@ __device__ __forceinline__ typename E::H2 absmax8(const uint4 &v)
     const H2 a = __habs2(as_pair<H2>(v.x)), b = __habs2(as_pair<H2>(v.y));
     const H2 c = __habs2(as_pair<H2>(v.z)), d = __habs2(as_pair<H2>(v.w));
     return __hmax2(__hmax2(a, b), __hmax2(c, d));
+}
+
+// Fused launch (TileSrc::tile_base == nullptr): the blob metadata tile_scan_kernel would have written.  Every CTA copies
+// its 32 tier-map bytes; the CTA of tile 0 zeroes the pads of its layer's ten segments and, in layer 0, writes the
+// header and the pad behind the tier map.
+__device__ __forceinline__ void pack_metadata(const Geom &g, const Layout &lo, const Header256 &hdr, uint8_t *rblob,
+                                              int l, int64_t tile, int64_t j0, uint32_t my_t)
+{
+    const uint32_t tid = threadIdx.x;
+    if (tid < 32 && j0 + tid < g.n) rblob[lo.tier_map_off + (int64_t)l * g.n + j0 + tid] = (uint8_t)my_t;
+    if (tile != 0) return;
+    uint8_t *lbase = rblob + lo.layer0_off + (uint64_t)l * lo.layer_stride;
+    for (int s = 0; s < 10; ++s) {
+        const uint64_t beg = lo.seg_off[s] + lo.seg_raw[s], end = lo.seg_off[s] + pad256(lo.seg_raw[s]);
+        for (uint64_t o = beg + tid; o < end; o += blockDim.x) lbase[o] = 0;
+    }
+    if (l == 0) {
+        if (tid < 64) reinterpret_cast<uint32_t *>(rblob)[tid] = hdr.w[tid];
+        for (uint64_t o = lo.tier_map_off + (uint64_t)g.L * (uint64_t)g.n + tid; o < lo.layer0_off; o += blockDim.x) rblob[o] = 0;
+    }
 }
 
 template <int D, int QMAX, class E>
@@ -42,32 +64,40 @@ __device__ __forceinline__ void quantize_chunk(const uint4 &v, uint32_t lane, ty
     (void)lane;
 }
 
-template <int D, class E>
+template <int D, class E, bool SPARSE>
 __global__ void __launch_bounds__(256)
 pack_kernel(Geom g, Layout lo, const __half *__restrict__ K, const __half *__restrict__ V,
             const uint8_t *__restrict__ tier_map, uint8_t *__restrict__ blob, uint64_t blob_stride,
-            const uint4 *__restrict__ tile_base)
+            Header256 hdr, TileSrc ts)
 {
     using H = typename E::H; using H2 = typename E::H2;
     constexpr int LPV = D / 8;
+    __shared__ uint32_t sCnt[16];
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
-    const int64_t tile = blockIdx.x;
     const int l = blockIdx.y, r = blockIdx.z;
-    const int64_t n = g.n;
-    const int64_t j0 = tile * kTileTokens;
+    const int64_t n = g.n, rl = (int64_t)r * g.L + l;
+    const uint8_t *tm = tier_map + rl * n;
+    const uint32_t low = (uint32_t)g.low_code;                       // 4: symmetric INT4, 2: asymmetric 2-bit (NEXT-4)
+    uint8_t *rblob = blob + (uint64_t)r * blob_stride;
+    uint8_t *lbase = rblob + lo.layer0_off + (uint64_t)l * lo.layer_stride;
+    const int row_elems = g.Hkv * D;
+    const int64_t cache_off = (int64_t)r * g.sr + (int64_t)l * g.sl;
+    const uint32_t limit = SPARSE ? ts.live_count[rl] : (uint32_t)g.tiles;
+    uint32_t idx = blockIdx.x;
+    if (SPARSE && idx >= limit) return;
 
+#pragma unroll 1
+    do {
+    const int64_t tile = SPARSE ? (int64_t)ts.tile_base[rl * g.tiles + idx].w : (int64_t)idx;
+    const int64_t j0 = tile * kTileTokens;
     // tiers of the tile: lane i holds token j0+i
-    const uint8_t *tm = tier_map + ((int64_t)r * g.L + l) * n;
     const uint32_t my_t = (j0 + lane < n) ? (uint32_t)tm[j0 + lane] : 0xFFu;
     const uint32_t m16 = __ballot_sync(0xffffffffu, my_t == 16u);
     const uint32_t m8 = __ballot_sync(0xffffffffu, my_t == 8u);
-    const uint32_t low = (uint32_t)g.low_code;                       // 4: symmetric INT4, 2: asymmetric 2-bit (NEXT-4)
     const uint32_t m4 = __ballot_sync(0xffffffffu, my_t == low);
-    const uint4 base = tile_base[((int64_t)r * g.L + l) * g.tiles + tile];
-
-    uint8_t *lbase = blob + (uint64_t)r * blob_stride + lo.layer0_off + (uint64_t)l * lo.layer_stride;
-    const int row_elems = g.Hkv * D;
-    const int64_t cache_off = (int64_t)r * g.sr + (int64_t)l * g.sl;
+    uint4 base;
+    if (ts.tile_base) base = ts.tile_base[rl * g.tiles + tile];
+    else { base = self_tile_base(tm, tile, low, sCnt); pack_metadata(g, lo, hdr, rblob, l, tile, j0, my_t); }
 
     for (uint32_t i = warp; i < (uint32_t)kTileTokens; i += nwarps) {
         const uint32_t t = __shfl_sync(0xffffffffu, my_t, i);
@@ -209,6 +239,8 @@ pack_kernel(Geom g, Layout lo, const __half *__restrict__ K, const __half *__res
             }
         }
     }
+    idx += gridDim.x;
+    } while (SPARSE && idx < limit);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -218,36 +250,45 @@ pack_kernel(Geom g, Layout lo, const __half *__restrict__ K, const __half *__res
 // of 2*NCH*log2(LPV) shuffles and 2*NCH divisions; the reciprocals are then broadcast with 2*NCH shuffles.
 // ------------------------------------------------------------------------------------------------
 // LOW2 = false: the low tier is symmetric INT4 (tier code 4).  LOW2 = true (NEXT-4): asymmetric 2-bit (tier code 2).
-template <int D, int NCH, int MINB, bool LOW2, class E>
+// SPARSE: the grid strides over the scan's list of live tiles (TileSrc::live_count); otherwise one CTA per tile, no loop.
+template <int D, int NCH, int MINB, bool LOW2, class E, bool SPARSE>
 __global__ void __launch_bounds__(256, MINB)
 pack_fast_kernel(Geom g, Layout lo, const __half *__restrict__ K, const __half *__restrict__ V,
                  const uint8_t *__restrict__ tier_map, uint8_t *__restrict__ blob, uint64_t blob_stride,
-                 const uint4 *__restrict__ tile_base)
+                 Header256 hdr, TileSrc ts)
 {
     using H = typename E::H; using H2 = typename E::H2;
     constexpr int LPV = D / 8;                 // lanes per head vector
     constexpr int HPC = 256 / D;               // head vectors per 256-element chunk
-    const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int64_t tile = blockIdx.x;
-    const int l = blockIdx.y, r = blockIdx.z;
-    const int64_t n = g.n;
-    const int64_t j0 = tile * kTileTokens;
-
-    const uint8_t *tm = tier_map + ((int64_t)r * g.L + l) * n;
-    const uint32_t my_t = (j0 + lane < n) ? (uint32_t)tm[j0 + lane] : 0xFFu;
-    const uint32_t m16 = __ballot_sync(0xffffffffu, my_t == 16u);
-    const uint32_t m8 = __ballot_sync(0xffffffffu, my_t == 8u);
     constexpr uint32_t kLow = LOW2 ? 2u : 4u;
-    const uint32_t m4 = __ballot_sync(0xffffffffu, my_t == kLow);
-    const uint4 base = tile_base[((int64_t)r * g.L + l) * g.tiles + tile];
-
-    uint8_t *lbase = blob + (uint64_t)r * blob_stride + lo.layer0_off + (uint64_t)l * lo.layer_stride;
+    __shared__ uint32_t sCnt[16];
+    const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int l = blockIdx.y, r = blockIdx.z;
+    const int64_t n = g.n, rl = (int64_t)r * g.L + l;
+    const uint8_t *tm = tier_map + rl * n;
+    uint8_t *rblob = blob + (uint64_t)r * blob_stride;
+    uint8_t *lbase = rblob + lo.layer0_off + (uint64_t)l * lo.layer_stride;
     const int row_elems = g.Hkv * D;
     const __half *Kb = K + (int64_t)r * g.sr + (int64_t)l * g.sl;
     const __half *Vb = V + (int64_t)r * g.sr + (int64_t)l * g.sl;
     const int lane_h = (int)(lane * 8) / D, lane_c = (int)(lane * 8) % D;
     const int my_chunk = held_chunk<LPV, NCH>(lane);
     const bool scale_writer = (lane % (LPV / NCH)) == 0;
+    const uint32_t limit = SPARSE ? ts.live_count[rl] : (uint32_t)g.tiles;
+    uint32_t idx = blockIdx.x;
+    if (SPARSE && idx >= limit) return;
+
+#pragma unroll 1
+    do {
+    const int64_t tile = SPARSE ? (int64_t)ts.tile_base[rl * g.tiles + idx].w : (int64_t)idx;
+    const int64_t j0 = tile * kTileTokens;
+    const uint32_t my_t = (j0 + lane < n) ? (uint32_t)tm[j0 + lane] : 0xFFu;
+    const uint32_t m16 = __ballot_sync(0xffffffffu, my_t == 16u);
+    const uint32_t m8 = __ballot_sync(0xffffffffu, my_t == 8u);
+    const uint32_t m4 = __ballot_sync(0xffffffffu, my_t == kLow);
+    uint4 base;
+    if (ts.tile_base) base = ts.tile_base[rl * g.tiles + tile];
+    else { base = self_tile_base(tm, tile, kLow, sCnt); pack_metadata(g, lo, hdr, rblob, l, tile, j0, my_t); }
 
 #pragma unroll 1
     for (uint32_t i = warp; i < (uint32_t)kTileTokens; i += 8) {
@@ -368,44 +409,48 @@ pack_fast_kernel(Geom g, Layout lo, const __half *__restrict__ K, const __half *
             }
         }
     }
+    idx += gridDim.x;
+    } while (SPARSE && idx < limit);
 }
 
 template <int D, int NCH, class E>
 static cudaError_t launch_pack_fast(const Geom &g, const Layout &lo, const __half *K, const __half *V,
                                     const uint8_t *tier_map, uint8_t *blob, uint64_t blob_stride,
-                                    const uint4 *tile_base, cudaStream_t s)
+                                    const Header256 &hdr, TileSrc ts, dim3 grid, cudaStream_t s)
 {
-    dim3 grid(g.tiles, g.L, g.R);
-    if (g.low_code == 2) pack_fast_kernel<D, NCH, 3, true, E><<<grid, 256, 0, s>>>(g, lo, K, V, tier_map, blob, blob_stride, tile_base);
-    else pack_fast_kernel<D, NCH, 3, false, E><<<grid, 256, 0, s>>>(g, lo, K, V, tier_map, blob, blob_stride, tile_base);
+    // (a sparse launch never carries a 2-bit tier: skv_host.cu plan_stage)
+    if (g.low_code == 2) pack_fast_kernel<D, NCH, MinBlocks<NCH>::value, true, E, false><<<grid, 256, 0, s>>>(g, lo, K, V, tier_map, blob, blob_stride, hdr, ts);
+    else if (ts.live_count) pack_fast_kernel<D, NCH, MinBlocks<NCH>::value, false, E, true><<<grid, 256, 0, s>>>(g, lo, K, V, tier_map, blob, blob_stride, hdr, ts);
+    else pack_fast_kernel<D, NCH, MinBlocks<NCH>::value, false, E, false><<<grid, 256, 0, s>>>(g, lo, K, V, tier_map, blob, blob_stride, hdr, ts);
     return cudaGetLastError();
 }
 
 template <int D, class E>
 static cudaError_t launch_pack_d(const Geom &g, const Layout &lo, const __half *K, const __half *V,
                                  const uint8_t *tier_map, uint8_t *blob, uint64_t blob_stride,
-                                 const uint4 *tile_base, cudaStream_t s)
+                                 const Header256 &hdr, TileSrc ts, dim3 grid, cudaStream_t s)
 {
     if ((g.Hkv * D) % 256 == 0) {
-        if (g.row_chunks % 4 == 0) return launch_pack_fast<D, 4, E>(g, lo, K, V, tier_map, blob, blob_stride, tile_base, s);
-        if (g.row_chunks % 2 == 0) return launch_pack_fast<D, 2, E>(g, lo, K, V, tier_map, blob, blob_stride, tile_base, s);
-        return launch_pack_fast<D, 1, E>(g, lo, K, V, tier_map, blob, blob_stride, tile_base, s);
+        if (g.row_chunks % 4 == 0) return launch_pack_fast<D, 4, E>(g, lo, K, V, tier_map, blob, blob_stride, hdr, ts, grid, s);
+        if (g.row_chunks % 2 == 0) return launch_pack_fast<D, 2, E>(g, lo, K, V, tier_map, blob, blob_stride, hdr, ts, grid, s);
+        return launch_pack_fast<D, 1, E>(g, lo, K, V, tier_map, blob, blob_stride, hdr, ts, grid, s);
     }
-    dim3 grid(g.tiles, g.L, g.R);
-    pack_kernel<D, E><<<grid, 256, 0, s>>>(g, lo, K, V, tier_map, blob, blob_stride, tile_base);
+    if (ts.live_count) pack_kernel<D, E, true><<<grid, 256, 0, s>>>(g, lo, K, V, tier_map, blob, blob_stride, hdr, ts);
+    else pack_kernel<D, E, false><<<grid, 256, 0, s>>>(g, lo, K, V, tier_map, blob, blob_stride, hdr, ts);
     return cudaGetLastError();
 }
 
 cudaError_t launch_pack(const Geom &g, const Layout &lo, const __half *K, const __half *V, const uint8_t *tier_map,
-                        uint8_t *blob, uint64_t blob_stride, const uint4 *tile_base, cudaStream_t s)
+                        uint8_t *blob, uint64_t blob_stride, const Header256 &hdr, TileSrc ts, int grid_x, cudaStream_t s)
 {
+    const dim3 grid(grid_x, g.L, g.R);
     switch (g.D) {
-    case 64: return g.bf16 ? launch_pack_d<64, ElemBF16>(g, lo, K, V, tier_map, blob, blob_stride, tile_base, s)
-                            : launch_pack_d<64, ElemF16>(g, lo, K, V, tier_map, blob, blob_stride, tile_base, s);
-    case 128: return g.bf16 ? launch_pack_d<128, ElemBF16>(g, lo, K, V, tier_map, blob, blob_stride, tile_base, s)
-                            : launch_pack_d<128, ElemF16>(g, lo, K, V, tier_map, blob, blob_stride, tile_base, s);
-    case 256: return g.bf16 ? launch_pack_d<256, ElemBF16>(g, lo, K, V, tier_map, blob, blob_stride, tile_base, s)
-                            : launch_pack_d<256, ElemF16>(g, lo, K, V, tier_map, blob, blob_stride, tile_base, s);
+    case 64: return g.bf16 ? launch_pack_d<64, ElemBF16>(g, lo, K, V, tier_map, blob, blob_stride, hdr, ts, grid, s)
+                            : launch_pack_d<64, ElemF16>(g, lo, K, V, tier_map, blob, blob_stride, hdr, ts, grid, s);
+    case 128: return g.bf16 ? launch_pack_d<128, ElemBF16>(g, lo, K, V, tier_map, blob, blob_stride, hdr, ts, grid, s)
+                            : launch_pack_d<128, ElemF16>(g, lo, K, V, tier_map, blob, blob_stride, hdr, ts, grid, s);
+    case 256: return g.bf16 ? launch_pack_d<256, ElemBF16>(g, lo, K, V, tier_map, blob, blob_stride, hdr, ts, grid, s)
+                            : launch_pack_d<256, ElemF16>(g, lo, K, V, tier_map, blob, blob_stride, hdr, ts, grid, s);
     default: return cudaErrorInvalidValue;
     }
 }

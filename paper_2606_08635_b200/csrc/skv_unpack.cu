@@ -2,7 +2,9 @@
 // (table lookup) is needed at the decode worker").
 //
 // Mirror of skv_pack.cu: one warp per token, one CTA per 32-token tile of one (request, layer).  The slot
-// of a token is recomputed from the transmitted tier map (tile base from skv_scan.cu + ballot rank).
+// of a token is recomputed from the transmitted tier map (tile base + ballot rank; the tile base comes from
+// skv_scan.cu, or for n <= kFuseMaxTokens from the CTA's own count of the tier-map bytes below its tile, so
+// that unpack is one launch; skv_unpack_patch of a sparse upgrade blob walks the scan's list of live tiles).
 // INT8: 8-byte loads per lane -> 8 fp16 (one 16-byte store); INT4: 4-byte loads -> 8 fp16.  y = f16_rn(
 // fl32(float(q) * fl32(amax/qmax))); int->float goes through the 2^23 exponent trick (exact), so no I2F.
 // Dropped tokens are written as +0.0 (reading P10).  HBM-bound: reads beta*Bytes_FP16, writes Bytes_FP16.
@@ -10,30 +12,46 @@
 
 namespace skv {
 
-template <int D, class E>
+// Fused launch (TileSrc::tile_base == nullptr): the tier map the scan kernel would have copied out (the validity mask);
+// in patch mode only the tokens the blob carries change tier.
+__device__ __forceinline__ void unpack_metadata(const Geom &g, uint8_t *tier_out, int64_t rl, int64_t j0, uint32_t my_t)
+{
+    const uint32_t tid = threadIdx.x;
+    if (tier_out != nullptr && tid < 32 && j0 + tid < g.n && !(g.patch && my_t == 0u))
+        tier_out[rl * g.n + j0 + tid] = (uint8_t)my_t;
+}
+
+template <int D, class E, bool SPARSE>
 __global__ void __launch_bounds__(256)
 unpack_kernel(Geom g, Layout lo, const uint8_t *__restrict__ blob, uint64_t blob_stride,
-              __half *__restrict__ K, __half *__restrict__ V, const uint4 *__restrict__ tile_base)
+              __half *__restrict__ K, __half *__restrict__ V, uint8_t *__restrict__ tier_out, TileSrc ts)
 {
     using H = typename E::H; using H2 = typename E::H2;
+    __shared__ uint32_t sCnt[16];
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
-    const int64_t tile = blockIdx.x;
     const int l = blockIdx.y, r = blockIdx.z;
-    const int64_t n = g.n;
-    const int64_t j0 = tile * kTileTokens;
-
+    const int64_t n = g.n, rl = (int64_t)r * g.L + l;
     const uint8_t *rblob = blob + (uint64_t)r * blob_stride;
     const uint8_t *tm = rblob + lo.tier_map_off + (int64_t)l * n;
-    const uint32_t my_t = (j0 + lane < n) ? (uint32_t)tm[j0 + lane] : 0xFFu;
-    const uint32_t m16 = __ballot_sync(0xffffffffu, my_t == 16u);
-    const uint32_t m8 = __ballot_sync(0xffffffffu, my_t == 8u);
     const uint32_t low = (uint32_t)g.low_code;                       // 4: symmetric INT4, 2: asymmetric 2-bit (NEXT-4)
-    const uint32_t m4 = __ballot_sync(0xffffffffu, my_t == low);
-    const uint4 base = tile_base[((int64_t)r * g.L + l) * g.tiles + tile];
-
     const uint8_t *lbase = rblob + lo.layer0_off + (uint64_t)l * lo.layer_stride;
     const int row_elems = g.Hkv * D;
     const int64_t cache_off = (int64_t)r * g.sr + (int64_t)l * g.sl;
+    const uint32_t limit = SPARSE ? ts.live_count[rl] : (uint32_t)g.tiles;
+    uint32_t idx = blockIdx.x;
+    if (SPARSE && idx >= limit) return;
+
+#pragma unroll 1
+    do {
+    const int64_t tile = SPARSE ? (int64_t)ts.tile_base[rl * g.tiles + idx].w : (int64_t)idx;
+    const int64_t j0 = tile * kTileTokens;
+    const uint32_t my_t = (j0 + lane < n) ? (uint32_t)tm[j0 + lane] : 0xFFu;
+    const uint32_t m16 = __ballot_sync(0xffffffffu, my_t == 16u);
+    const uint32_t m8 = __ballot_sync(0xffffffffu, my_t == 8u);
+    const uint32_t m4 = __ballot_sync(0xffffffffu, my_t == low);
+    uint4 base;
+    if (ts.tile_base) base = ts.tile_base[rl * g.tiles + tile];
+    else { base = self_tile_base(tm, tile, low, sCnt); unpack_metadata(g, tier_out, rl, j0, my_t); }
 
     for (uint32_t i = warp; i < (uint32_t)kTileTokens; i += nwarps) {
         const int64_t j = j0 + i;
@@ -150,41 +168,51 @@ unpack_kernel(Geom g, Layout lo, const uint8_t *__restrict__ blob, uint64_t blob
             }
         }
     }
+    idx += gridDim.x;
+    } while (SPARSE && idx < limit);
 }
 
 // ------------------------------------------------------------------------------------------------
 // Fast path (row_elems % (256*NCH) == 0): fully unrolled; each lane loads the amax record of ONE
 // (chunk, head) for K and V, divides twice, and the scales are broadcast with 2*NCH shuffles.
 // ------------------------------------------------------------------------------------------------
-template <int D, int NCH, int MINB, bool LOW2, class E>
+// SPARSE: the grid strides over the scan's list of live tiles (patch mode only); otherwise one CTA per tile, no loop.
+template <int D, int NCH, int MINB, bool LOW2, class E, bool SPARSE>
 __global__ void __launch_bounds__(256, MINB)
 unpack_fast_kernel(Geom g, Layout lo, const uint8_t *__restrict__ blob, uint64_t blob_stride,
-                   __half *__restrict__ K, __half *__restrict__ V, const uint4 *__restrict__ tile_base)
+                   __half *__restrict__ K, __half *__restrict__ V, uint8_t *__restrict__ tier_out, TileSrc ts)
 {
     using H = typename E::H; using H2 = typename E::H2;
     constexpr int LPV = D / 8;
     constexpr int HPC = 256 / D;
+    constexpr uint32_t kLow = LOW2 ? 2u : 4u;
+    __shared__ uint32_t sCnt[16];
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int64_t tile = blockIdx.x;
     const int l = blockIdx.y, r = blockIdx.z;
-    const int64_t n = g.n;
-    const int64_t j0 = tile * kTileTokens;
-
+    const int64_t n = g.n, rl = (int64_t)r * g.L + l;
     const uint8_t *rblob = blob + (uint64_t)r * blob_stride;
     const uint8_t *tm = rblob + lo.tier_map_off + (int64_t)l * n;
-    const uint32_t my_t = (j0 + lane < n) ? (uint32_t)tm[j0 + lane] : 0xFFu;
-    const uint32_t m16 = __ballot_sync(0xffffffffu, my_t == 16u);
-    const uint32_t m8 = __ballot_sync(0xffffffffu, my_t == 8u);
-    constexpr uint32_t kLow = LOW2 ? 2u : 4u;
-    const uint32_t m4 = __ballot_sync(0xffffffffu, my_t == kLow);
-    const uint4 base = tile_base[((int64_t)r * g.L + l) * g.tiles + tile];
-
     const uint8_t *lbase = rblob + lo.layer0_off + (uint64_t)l * lo.layer_stride;
     const int row_elems = g.Hkv * D;
     __half *Kb = K + (int64_t)r * g.sr + (int64_t)l * g.sl;
     __half *Vb = V + (int64_t)r * g.sr + (int64_t)l * g.sl;
     const int lane_h = (int)(lane * 8) / D, lane_c = (int)(lane * 8) % D;
     const int my_chunk = held_chunk<LPV, NCH>(lane);
+    const uint32_t limit = SPARSE ? ts.live_count[rl] : (uint32_t)g.tiles;
+    uint32_t idx = blockIdx.x;
+    if (SPARSE && idx >= limit) return;
+
+#pragma unroll 1
+    do {
+    const int64_t tile = SPARSE ? (int64_t)ts.tile_base[rl * g.tiles + idx].w : (int64_t)idx;
+    const int64_t j0 = tile * kTileTokens;
+    const uint32_t my_t = (j0 + lane < n) ? (uint32_t)tm[j0 + lane] : 0xFFu;
+    const uint32_t m16 = __ballot_sync(0xffffffffu, my_t == 16u);
+    const uint32_t m8 = __ballot_sync(0xffffffffu, my_t == 8u);
+    const uint32_t m4 = __ballot_sync(0xffffffffu, my_t == kLow);
+    uint4 base;
+    if (ts.tile_base) base = ts.tile_base[rl * g.tiles + tile];
+    else { base = self_tile_base(tm, tile, kLow, sCnt); unpack_metadata(g, tier_out, rl, j0, my_t); }
 
     for (uint32_t i = warp; i < (uint32_t)kTileTokens; i += 8) {
         const int64_t j = j0 + i;
@@ -297,37 +325,45 @@ unpack_fast_kernel(Geom g, Layout lo, const uint8_t *__restrict__ blob, uint64_t
             }
         }
     }
+    idx += gridDim.x;
+    } while (SPARSE && idx < limit);
 }
 
 template <int D, class E>
 static cudaError_t launch_unpack_d(const Geom &g, const Layout &lo, const uint8_t *blob, uint64_t blob_stride,
-                                   __half *K, __half *V, const uint4 *tile_base, cudaStream_t s)
+                                   __half *K, __half *V, uint8_t *tier_out, TileSrc ts, dim3 grid, cudaStream_t s)
 {
-    dim3 grid(g.tiles, g.L, g.R);
     if ((g.Hkv * D) % 256 == 0) {
-        if (g.low_code == 2) {
-            if (g.row_chunks % 4 == 0) unpack_fast_kernel<D, 4, 3, true, E><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tile_base);
-            else if (g.row_chunks % 2 == 0) unpack_fast_kernel<D, 2, 3, true, E><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tile_base);
-            else unpack_fast_kernel<D, 1, 3, true, E><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tile_base);
-        } else if (g.row_chunks % 4 == 0) unpack_fast_kernel<D, 4, 3, false, E><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tile_base);
-        else if (g.row_chunks % 2 == 0) unpack_fast_kernel<D, 2, 3, false, E><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tile_base);
-        else unpack_fast_kernel<D, 1, 3, false, E><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tile_base);
+        // (a sparse launch never carries a 2-bit tier: skv_host.cu plan_stage)
+#define SKV_LAUNCH_UNPACK(NCH)                                                                                                        \
+        do {                                                                                                                          \
+            if (g.low_code == 2) unpack_fast_kernel<D, NCH, MinBlocks<NCH>::value, true, E, false><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tier_out, ts); \
+            else if (ts.live_count) unpack_fast_kernel<D, NCH, MinBlocks<NCH>::value, false, E, true><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tier_out, ts); \
+            else unpack_fast_kernel<D, NCH, MinBlocks<NCH>::value, false, E, false><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tier_out, ts); \
+        } while (0)
+        if (g.row_chunks % 4 == 0) SKV_LAUNCH_UNPACK(4);
+        else if (g.row_chunks % 2 == 0) SKV_LAUNCH_UNPACK(2);
+        else SKV_LAUNCH_UNPACK(1);
+#undef SKV_LAUNCH_UNPACK
+    } else if (ts.live_count) {
+        unpack_kernel<D, E, true><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tier_out, ts);
     } else {
-        unpack_kernel<D, E><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tile_base);
+        unpack_kernel<D, E, false><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tier_out, ts);
     }
     return cudaGetLastError();
 }
 
 cudaError_t launch_unpack(const Geom &g, const Layout &lo, const uint8_t *blob, uint64_t blob_stride,
-                          __half *K, __half *V, const uint4 *tile_base, cudaStream_t s)
+                          __half *K, __half *V, uint8_t *tier_out, TileSrc ts, int grid_x, cudaStream_t s)
 {
+    const dim3 grid(grid_x, g.L, g.R);
     switch (g.D) {
-    case 64: return g.bf16 ? launch_unpack_d<64, ElemBF16>(g, lo, blob, blob_stride, K, V, tile_base, s)
-                            : launch_unpack_d<64, ElemF16>(g, lo, blob, blob_stride, K, V, tile_base, s);
-    case 128: return g.bf16 ? launch_unpack_d<128, ElemBF16>(g, lo, blob, blob_stride, K, V, tile_base, s)
-                            : launch_unpack_d<128, ElemF16>(g, lo, blob, blob_stride, K, V, tile_base, s);
-    case 256: return g.bf16 ? launch_unpack_d<256, ElemBF16>(g, lo, blob, blob_stride, K, V, tile_base, s)
-                            : launch_unpack_d<256, ElemF16>(g, lo, blob, blob_stride, K, V, tile_base, s);
+    case 64: return g.bf16 ? launch_unpack_d<64, ElemBF16>(g, lo, blob, blob_stride, K, V, tier_out, ts, grid, s)
+                            : launch_unpack_d<64, ElemF16>(g, lo, blob, blob_stride, K, V, tier_out, ts, grid, s);
+    case 128: return g.bf16 ? launch_unpack_d<128, ElemBF16>(g, lo, blob, blob_stride, K, V, tier_out, ts, grid, s)
+                            : launch_unpack_d<128, ElemF16>(g, lo, blob, blob_stride, K, V, tier_out, ts, grid, s);
+    case 256: return g.bf16 ? launch_unpack_d<256, ElemBF16>(g, lo, blob, blob_stride, K, V, tier_out, ts, grid, s)
+                            : launch_unpack_d<256, ElemF16>(g, lo, blob, blob_stride, K, V, tier_out, ts, grid, s);
     default: return cudaErrorInvalidValue;
     }
 }

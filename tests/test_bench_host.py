@@ -1,0 +1,40 @@
+"""Host-side logic of bench.py that needs no GPU: the CPU-baseline legs SURVEY.md 8(d) asks for, the L2 labelling
+computed from the working set, the launch count per step and the algorithmic-byte model."""
+import os
+import sys
+import types
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+sys.path.insert(0, ROOT)
+
+import bench
+import skv_synth
+
+
+def test_cpu_baseline_has_every_leg_of_the_measurement_contract():
+    cfg = skv_synth.Config("tiny-bench", L=4, Hq=4, Hkv=2, d=64, n=512, w=8, R=1, seed=3)
+    cb = bench.oracle_sample(cfg, 0.5, target_seconds=1.0)
+    assert cb["kind"] == "oracle" and cb["unit"] == "GB/s" and cb["value"] > 0 and cb["cores"] >= 1
+    assert isinstance(cb["cpu_model"], str) and cb["cpu_model"]
+    st = cb["single_thread"]
+    assert st["cores"] == 1 and st["value"] > 0 and st["unit"] == "GB/s"
+    assert cb["importance"]["seconds"] > 0 and cb["importance"]["seconds_per_request_extrapolated"] > 0
+    assert cb["assign"]["seconds"] > 0
+    import oracle
+    assert oracle.max_threads() == cb["cores"]                       # the single-thread leg restored the thread count
+
+
+def test_l2_label_follows_the_working_set():
+    args = types.SimpleNamespace(l2_flush="auto")
+    C = skv_synth.CONFIGS
+    assert bench.want_flush(args, C["C2"], 1) and bench.want_flush(args, C["C4"], 1)
+    assert not bench.want_flush(args, C["C5"], 4)
+    assert "flushed" in bench.l2_note(C["C2"], 1, 119_000_000, True)
+    assert "partly" in bench.l2_note(C["C2"], 1, 119_000_000, False)
+    assert "larger than L2" in bench.l2_note(C["C5"], 4, 2_182_000_000, False)
+
+
+def test_launch_count_per_step():
+    C = skv_synth.CONFIGS
+    assert bench.launches_per_step(C["C2"]) == 4          # importance, assign, pack, unpack (scan fused, n = 4096)
+    assert bench.launches_per_step(C["C5"]) == 6          # + one tile scan each for pack and unpack (n = 32768)

@@ -735,6 +735,36 @@ def test_bfloat16_vanishing_amax_gets_zero_codes():
     assert np.array_equal(_bits(Ko[0]), K2) and np.array_equal(_bits(Vo[0]), V2)
 
 
+def test_bfloat16_two_bit_range_beyond_binary32_decodes_to_lo():
+    """P20, large end: finite bf16 elements more than FLT_MAX apart (hi - lo = +Inf) -> all codes 0, decode to lo; both
+    the per-head-vector and the group-wise 2-bit tier, against the oracle (nothing NaN)."""
+    dev = torch.device("cuda:0")
+    L, n, Hkv, d = 1, 96, 2, 128
+    g = torch.Generator().manual_seed(5)
+    K = torch.randn((L, n, Hkv, d), generator=g).to(torch.bfloat16); V = torch.randn((L, n, Hkv, d), generator=g).to(torch.bfloat16)
+    K[0, ::3, 0, 7] = 3e38; K[0, ::3, 0, 40] = -3e38; V[0, 1::4, 1, 100] = -3e38; V[0, 1::4, 1, 101] = 3.2e38
+    K[0, 5, 1, 0] = 1.5e38; K[0, 5, 1, 1] = -1.5e38                       # range 3e38: finite, the rule does not apply
+    tier_or = np.full((L, n), 2, np.uint8); tier_or[0, ::5] = 8; tier_or[0, 0] = 16
+    n16, n8, n4 = int((tier_or == 16).sum()), int((tier_or == 8).sum()), int((tier_or == 2).sum())
+    shape = skv.make_shape(L, 2, Hkv, d, n, 1, dtype="bf16")
+    for mode in (0, 2):
+        c = skv.skv_counts_from_populations(shape, n16, n8, n4, allow_int4=2)
+        c.tier_mode = mode
+        oc = oracle.Counts(n16, n8, n4, 0, c.budget_q4, c.spent_q4, low_bits=2, mode=mode)
+        blob_or = oracle.pack(_bits(K), _bits(V), tier_or, oc, 2, bf16=True)
+        ws = torch.empty(skv.skv_workspace_bytes(shape, 0), dtype=torch.uint8, device=dev)
+        bb = skv.skv_blob_bytes(shape, c)
+        assert bb == blob_or.size
+        blob = torch.empty((bb,), dtype=torch.uint8, device=dev)
+        skv.skv_pack(shape, K[None].to(dev), V[None].to(dev), torch.from_numpy(tier_or)[None].to(dev), c, blob, ws)
+        assert np.array_equal(blob.cpu().numpy(), blob_or)
+        Ko = torch.empty((1, L, n, Hkv, d), dtype=torch.bfloat16, device=dev); Vo = torch.empty_like(Ko)
+        skv.skv_unpack(shape, blob, bb, c, Ko, Vo, None, ws)
+        K2, V2, _ = oracle.unpack(blob_or, L, Hkv, d, n, bf16=True)
+        assert np.array_equal(_bits(Ko[0]), K2) and np.array_equal(_bits(Vo[0]), V2)
+        assert torch.isfinite(Ko.float()).all() and torch.isfinite(Vo.float()).all()
+
+
 def test_layer_pipelined_transfer_bfloat16():
     """The pipelined host round trip with bfloat16 caches: per-layer results equal the oracle's on the GPU's scores."""
     from paper_2606_08635_b200.transfer import LayerPipelinedTransfer
@@ -752,3 +782,110 @@ def test_layer_pipelined_transfer_bfloat16():
     assert np.array_equal(tier, req["T"].numpy())
     K2, V2, _ = oracle.unpack(oracle.pack(_bits(K), _bits(V), tier, counts, True, bf16=True), 3, cfg.Hkv, cfg.d, cfg.n, bf16=True)
     assert np.array_equal(_bits(req["Ko"]), K2) and np.array_equal(_bits(req["Vo"]), V2)
+
+
+@pytest.mark.parametrize("n,d,Hkv,Hq", [(8193, 128, 2, 4), (8200, 64, 3, 3), (8224, 256, 1, 2), (8192, 128, 4, 8), (8191, 64, 8, 8)])
+def test_sequences_around_the_fused_scan_limit(n, d, Hkv, Hq):
+    """n <= 8192: pack / unpack are one launch each (every CTA counts the tiers below its own tile and writes the
+    metadata); beyond it the scan kernel runs first.  Both sides of the limit, fast and generic rows, aligned and
+    unaligned tier maps -- same bytes as the oracle."""
+    cfg = skv_synth.Config(f"fuse_{n}_{d}", L=3, Hq=Hq, Hkv=Hkv, d=d, n=n, w=4, R=2, n_sink=3, seed=71, allow_int4=True)
+    case = Case(cfg, 0.37, with_importance=False)
+    out = gpu_pipeline(case, run_importance=False)
+    assert_bit_exact(case, out)
+
+
+def test_sparse_upgrade_blob_walks_the_live_tile_list():
+    """NEXT-3 at a size where the grid strides over the scan's list of live tiles (fewer CTAs than live tiles): an FP16
+    upgrade of 300 scattered tokens of 9000 per layer, 16 layers x 4 requests; blob and patched cache bit-exact."""
+    dev = torch.device("cuda:0")
+    cfg = skv_synth.Config("sparse_up", L=16, Hq=4, Hkv=2, d=128, n=9000, w=4, R=4, n_sink=2, seed=73, allow_int4=True)
+    case = Case(cfg, 0.3, with_importance=False)
+    out = gpu_pipeline(case, run_importance=False)
+    assert_bit_exact(case, out)
+    shape = case.shape()
+    ws = torch.empty(skv.skv_workspace_bytes(shape, 0), dtype=torch.uint8, device=dev)
+    Kd, Vd = case.K.to(dev), case.V.to(dev)
+    Kc, Vc = torch.from_numpy(out["K2"]).to(dev), torch.from_numpy(out["V2"]).to(dev)
+    tc = torch.from_numpy(out["tier"]).to(dev)
+    rng = np.random.default_rng(5)
+    k = 300
+    up = np.zeros((case.R, case.L, cfg.n), np.uint8)
+    for r in range(case.R):
+        for l in range(case.L):
+            up[r, l, rng.choice(np.flatnonzero(case.tier[r][l] != 16), size=k, replace=False)] = 16
+    uc = skv.skv_counts_from_populations(shape, k)
+    bb = skv.skv_blob_bytes(shape, uc)
+    ublob = torch.full((case.R * bb,), 0xAB, dtype=torch.uint8, device=dev)
+    skv.skv_pack(shape, Kd, Vd, torch.from_numpy(up).to(dev), uc, ublob, ws)
+    skv.skv_unpack_patch(shape, ublob, bb, uc, Kc, Vc, tc, ws)
+    torch.cuda.synchronize()
+    oc = oracle.Counts(k, 0, 0, cfg.n - k, uc.budget_q4, uc.spent_q4)
+    for r in range(case.R):
+        blob_or = oracle.pack(case.K[r].numpy(), case.V[r].numpy(), up[r], oc, True)
+        assert np.array_equal(ublob[r * bb:(r + 1) * bb].cpu().numpy(), blob_or)
+        K_or, V_or, t_or = oracle.unpack_patch(blob_or, case.K2[r], case.V2[r], case.tier[r])
+        assert np.array_equal(Kc[r].cpu().numpy().view(np.uint16), K_or.view(np.uint16))
+        assert np.array_equal(Vc[r].cpu().numpy().view(np.uint16), V_or.view(np.uint16))
+        assert np.array_equal(tc[r].cpu().numpy(), t_or)
+
+
+@pytest.mark.parametrize("name,n", [("C3", 1000), ("C5", 9000)])
+def test_whole_path_is_cuda_graph_capturable(name, n):
+    """The 'no host synchronisation, caller's stream only' promise of include/skv.h: importance -> assign -> pack ->
+    unpack captured into ONE CUDA graph on a side stream (fused and scan-first launch plans), replayed on fresh inputs
+    written into the captured buffers, bit-exact against the oracle both times."""
+    dev = torch.device("cuda:0")
+    cfg = C[name].scaled(L=2, n=n, R=2, ranges=())
+    shape = skv.make_shape(cfg.L, cfg.Hq, cfg.Hkv, cfg.d, cfg.n, cfg.R)
+    pol = skv.make_policy(0.4, cfg.n_sink, cfg.ranges, cfg.allow_int4)
+    counts = skv.skv_tier_counts(shape, pol)
+    bb = skv.skv_blob_bytes(shape, counts)
+    Kd = torch.empty((cfg.R, cfg.L, cfg.n, cfg.Hkv, cfg.d), dtype=torch.float16, device=dev)
+    Vd, Qd = torch.empty_like(Kd), torch.empty((cfg.R, cfg.L, cfg.Hq, cfg.w, cfg.d), dtype=torch.float16, device=dev)
+    ws = torch.empty(skv.skv_workspace_bytes(shape, cfg.w), dtype=torch.uint8, device=dev)
+    I = torch.empty((cfg.R, cfg.L, cfg.n), dtype=torch.float32, device=dev)
+    tier, tier_out = torch.empty(I.shape, dtype=torch.uint8, device=dev), torch.empty(I.shape, dtype=torch.uint8, device=dev)
+    blob = torch.empty((cfg.R * bb,), dtype=torch.uint8, device=dev)
+    Ko, Vo = torch.empty_like(Kd), torch.empty_like(Vd)
+
+    def path():
+        skv.skv_importance(shape, Kd, Qd, cfg.w, I, ws)
+        skv.skv_assign_tiers(shape, pol, I, tier, ws)
+        skv.skv_pack(shape, Kd, Vd, tier, counts, blob, ws)
+        skv.skv_unpack(shape, blob, bb, counts, Ko, Vo, tier_out, ws)
+
+    def load(seed_off):
+        ks, vs, qs = [], [], []
+        for r in range(cfg.R):
+            k, v = skv_synth.make_kv(cfg, r + seed_off); ks.append(k); vs.append(v); qs.append(skv_synth.make_q(cfg, r + seed_off))
+        Kh, Vh, Qh = torch.stack(ks), torch.stack(vs), torch.stack(qs)
+        Kd.copy_(Kh); Vd.copy_(Vh); Qd.copy_(Qh)
+        return Kh, Vh, Qh
+
+    Kh, Vh, Qh = load(0)
+    path()                                               # warm-up outside capture (function attributes, module load)
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.graph(graph, stream=side):
+        path()
+    for seed_off in (0, 10):
+        Kh, Vh, Qh = load(seed_off)
+        blob.fill_(0xAB); Ko.fill_(float("nan")); Vo.fill_(float("nan")); tier.fill_(0xEE); tier_out.fill_(0xEE)
+        graph.replay()
+        torch.cuda.synchronize()
+        Ig = I.cpu().numpy()
+        tg = tier.cpu().numpy()
+        for r in range(cfg.R):
+            I_or = oracle.importance(Kh[r].numpy(), Qh[r].numpy())
+            assert np.all(np.abs(Ig[r] - I_or) <= 1e-3 * I_or + 1e-30)
+            c_or, prot = oracle.tier_counts(cfg.n, 0.4, cfg.n_sink, cfg.ranges, cfg.allow_int4)
+            assert np.array_equal(tg[r], oracle.assign(Ig[r], prot, c_or))          # selection on the GPU's own scores
+            blob_or = oracle.pack(Kh[r].numpy(), Vh[r].numpy(), tg[r], c_or, cfg.allow_int4)
+            assert np.array_equal(blob[r * bb:(r + 1) * bb].cpu().numpy(), blob_or)
+            K2, V2, t2 = oracle.unpack(blob_or, cfg.L, cfg.Hkv, cfg.d, cfg.n)
+            assert np.array_equal(Ko[r].cpu().numpy().view(np.uint16), K2.view(np.uint16))
+            assert np.array_equal(Vo[r].cpu().numpy().view(np.uint16), V2.view(np.uint16))
+            assert np.array_equal(tier_out[r].cpu().numpy(), t2)

@@ -18,8 +18,11 @@ WORKER = textwrap.dedent("""
     bench.barrier()
     ms_local = [10.0 + 5.0 * rank, 1.0, 2.0 - rank, 3.0, 4.0 + rank]
     red, total = bench.aggregate_over_ranks(ms_local, 1000 * (rank + 1))
+    # the e2e leg: one time per rank (ms of a pipelined step from pinned host buffers), same reduction
+    red2, total2 = bench.aggregate_over_ranks([100.0 - 30.0 * rank], 1000 * (rank + 1))
+    e2e_value = total2 / (red2[0] * 1e-3) / 1e9
     bench.barrier()
-    print(json.dumps({"rank": rank, "world": world, "red": red, "bytes": total,
+    print(json.dumps({"rank": rank, "world": world, "red": red, "bytes": total, "red2": red2, "e2e_value": e2e_value,
                       "ids": bench.rank_request_ids(rank, 4)}), flush=True)
 """)
 
@@ -44,6 +47,8 @@ def test_two_rank_gloo_max_time_sum_bytes(tmp_path):
         assert d["world"] == 2
         assert d["red"] == [15.0, 1.0, 2.0, 3.0, 5.0]           # max over ranks, element by element
         assert d["bytes"] == 3000.0                               # sum over ranks (weak scaling)
+        assert d["red2"] == [100.0]                               # e2e: the slowest rank's step time ...
+        assert abs(d["e2e_value"] - 3000.0 / 0.1 / 1e9) < 1e-18   # ... under the bytes of all ranks
     assert outs[0]["ids"] == [0, 1, 2, 3] and outs[1]["ids"] == [4, 5, 6, 7]   # disjoint requests per rank
 
 
