@@ -41,14 +41,11 @@ __device__ __forceinline__ void st_stream(void *p, uint32_t v)
 
 // Resident CTAs per SM the fast pack / unpack kernels are compiled for (register cap 65536 / (256 * value)).  A lane
 // keeps 2 * NCH 16-byte loads in flight, so short rows (NCH = 2 or 1: rows of 512 or 256 elements, e.g. 4 KV heads of 128)
-// need more resident warps than long ones to cover the HBM latency.
-#ifndef SKV_MINB_NCH2
-#define SKV_MINB_NCH2 4
-#endif
-#ifndef SKV_MINB_NCH1
-#define SKV_MINB_NCH1 5
-#endif
-template <int NCH> struct MinBlocks { static constexpr int value = (NCH >= 4) ? 3 : (NCH == 2) ? SKV_MINB_NCH2 : SKV_MINB_NCH1; };
+// need more resident warps than long ones to cover the HBM latency (C2 pack: 0.75 -> 0.85 of the copy peak from 3 -> 5).
+// The 2-bit codec needs more registers: it stays at four.
+template <int NCH, bool LOW2> struct MinBlocks {
+    static constexpr int value = (NCH >= 4) ? 3 : LOW2 ? 4 : (NCH == 2) ? 5 : 6;
+};
 
 // ------------------------------------------------------------------------------------------------
 // Fused slot scan (short sequences, n <= kFuseMaxTokens): the whole CTA counts the FP16 / INT8 / low-tier bytes of
@@ -307,38 +304,43 @@ __device__ __forceinline__ float step3_of(float r)
     return (q <= 3.402823466e38f) ? q : 0.0f;
 }
 // 8 fp16 -> 8 two-bit codes (16 bits; element k in bits 2k..2k+1).  q_k = rint(fl32(x_k - lo) * inv), the product exact
-// and rounded once: the whole word is built in the mantissa of one float by a chain of fused multiply-adds,
+// and rounded once: the codes are built in the mantissas of ONE packed pair of floats (even elements in .x, odd ones
+// in .y) by a chain of packed fused multiply-adds (FFMA2 / FADD2: two elements per issue slot),
 //     a <- fma(dx_k, inv, a)      adds q_k (a is an even integer in [2^23, 2^24), so the FMA's rounding is RNE of the product)
-//     a <- fma(a, 4, -3*M)        shifts the partial word two bits up (exact), M = 1.5 * 2^23
+//     a <- fma(a, 16, -15*M)      shifts the partial word four bits up (exact), M = 1.5 * 2^23
+// which leaves q_0 q_2 q_4 q_6 at bits 0, 4, 8, 12 of a.x and q_1 q_3 q_5 q_7 likewise in a.y; two logic ops interleave them.
 template <class E>
 __device__ __forceinline__ uint32_t quant8_int2(const uint4 &v, float lo, float inv)
 {
     using H2 = typename E::H2;
-    const float2 p0 = to_f2(as_pair<H2>(v.x)), p1 = to_f2(as_pair<H2>(v.y));
-    const float2 p2 = to_f2(as_pair<H2>(v.z)), p3 = to_f2(as_pair<H2>(v.w));
-    const float x[8] = {p0.x, p0.y, p1.x, p1.y, p2.x, p2.y, p3.x, p3.y};
     // inv = 0 (zero range, or a bfloat16 range / reciprocal beyond binary32, P20) means "all codes 0"; x - lo may be +Inf
     // there, and Inf * 0 is no code, so the subtraction runs against 0 instead (x is finite: x * 0 = 0)
     lo = (inv != 0.0f) ? lo : 0.0f;
-    float a = __fmaf_rn(__fsub_rn(x[7], lo), inv, 12582912.0f);
-#pragma unroll
-    for (int k = 6; k >= 0; --k) {
-        a = __fmaf_rn(a, 4.0f, -37748736.0f);
-        a = __fmaf_rn(__fsub_rn(x[k], lo), inv, a);
-    }
-    return __float_as_uint(a) & 0xFFFFu;
+    const float2 nlo = make_float2(-lo, -lo), inv2 = make_float2(inv, inv);
+    const float2 sh = make_float2(16.0f, 16.0f), back = make_float2(-188743680.0f, -188743680.0f);     // -15 * 1.5 * 2^23
+    float2 a = __ffma2_rn(__fadd2_rn(to_f2(as_pair<H2>(v.w)), nlo), inv2, make_float2(12582912.0f, 12582912.0f));
+    a = __ffma2_rn(a, sh, back);
+    a = __ffma2_rn(__fadd2_rn(to_f2(as_pair<H2>(v.z)), nlo), inv2, a);
+    a = __ffma2_rn(a, sh, back);
+    a = __ffma2_rn(__fadd2_rn(to_f2(as_pair<H2>(v.y)), nlo), inv2, a);
+    a = __ffma2_rn(a, sh, back);
+    a = __ffma2_rn(__fadd2_rn(to_f2(as_pair<H2>(v.x)), nlo), inv2, a);
+    return (__float_as_uint(a.x) & 0x3333u) | ((__float_as_uint(a.y) & 0x3333u) << 2);
 }
-// 16 bits of two-bit codes -> 8 fp16: y = f16_rn(fma(q, step, lo))
+// 16 bits of two-bit codes -> 8 fp16: y = f16_rn(fma(q, step, lo)); int -> float through the 2^23 exponent trick (exact),
+// the subtraction and the fused multiply-add in packed form
 template <class E>
 __device__ __forceinline__ uint4 dequant_int2(uint32_t w, float step, float lo)
 {
-    float f[8];
+    const float2 off = make_float2(-8388608.0f, -8388608.0f), st2 = make_float2(step, step), lo2 = make_float2(lo, lo);
+    uint32_t o[4];
 #pragma unroll
-    for (int k = 0; k < 8; ++k)                          // int -> float through the 2^23 exponent trick (exact)
-        f[k] = __fmaf_rn(__fsub_rn(__uint_as_float(0x4B000000u | ((w >> (2 * k)) & 3u)), 8388608.0f), step, lo);
-    uint4 o;
-    o.x = from_f2<E>(f[0], f[1]); o.y = from_f2<E>(f[2], f[3]); o.z = from_f2<E>(f[4], f[5]); o.w = from_f2<E>(f[6], f[7]);
-    return o;
+    for (int k = 0; k < 4; ++k) {
+        const float2 f = make_float2(__uint_as_float(0x4B000000u | ((w >> (4 * k)) & 3u)), __uint_as_float(0x4B000000u | ((w >> (4 * k + 2)) & 3u)));
+        const float2 y = __ffma2_rn(__fadd2_rn(f, off), st2, lo2);
+        o[k] = from_f2<E>(y.x, y.y);
+    }
+    return make_uint4(o[0], o[1], o[2], o[3]);
 }
 
 template <class H>

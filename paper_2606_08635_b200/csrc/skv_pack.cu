@@ -419,9 +419,9 @@ static cudaError_t launch_pack_fast(const Geom &g, const Layout &lo, const __hal
                                     const Header256 &hdr, TileSrc ts, dim3 grid, cudaStream_t s)
 {
     // (a sparse launch never carries a 2-bit tier: skv_host.cu plan_stage)
-    if (g.low_code == 2) pack_fast_kernel<D, NCH, MinBlocks<NCH>::value, true, E, false><<<grid, 256, 0, s>>>(g, lo, K, V, tier_map, blob, blob_stride, hdr, ts);
-    else if (ts.live_count) pack_fast_kernel<D, NCH, MinBlocks<NCH>::value, false, E, true><<<grid, 256, 0, s>>>(g, lo, K, V, tier_map, blob, blob_stride, hdr, ts);
-    else pack_fast_kernel<D, NCH, MinBlocks<NCH>::value, false, E, false><<<grid, 256, 0, s>>>(g, lo, K, V, tier_map, blob, blob_stride, hdr, ts);
+    if (g.low_code == 2) pack_fast_kernel<D, NCH, MinBlocks<NCH, true>::value, true, E, false><<<grid, 256, 0, s>>>(g, lo, K, V, tier_map, blob, blob_stride, hdr, ts);
+    else if (ts.live_count) pack_fast_kernel<D, NCH, MinBlocks<NCH, false>::value, false, E, true><<<grid, 256, 0, s>>>(g, lo, K, V, tier_map, blob, blob_stride, hdr, ts);
+    else pack_fast_kernel<D, NCH, MinBlocks<NCH, false>::value, false, E, false><<<grid, 256, 0, s>>>(g, lo, K, V, tier_map, blob, blob_stride, hdr, ts);
     return cudaGetLastError();
 }
 

@@ -337,9 +337,9 @@ static cudaError_t launch_unpack_d(const Geom &g, const Layout &lo, const uint8_
         // (a sparse launch never carries a 2-bit tier: skv_host.cu plan_stage)
 #define SKV_LAUNCH_UNPACK(NCH)                                                                                                        \
         do {                                                                                                                          \
-            if (g.low_code == 2) unpack_fast_kernel<D, NCH, MinBlocks<NCH>::value, true, E, false><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tier_out, ts); \
-            else if (ts.live_count) unpack_fast_kernel<D, NCH, MinBlocks<NCH>::value, false, E, true><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tier_out, ts); \
-            else unpack_fast_kernel<D, NCH, MinBlocks<NCH>::value, false, E, false><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tier_out, ts); \
+            if (g.low_code == 2) unpack_fast_kernel<D, NCH, MinBlocks<NCH, true>::value, true, E, false><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tier_out, ts); \
+            else if (ts.live_count) unpack_fast_kernel<D, NCH, MinBlocks<NCH, false>::value, false, E, true><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tier_out, ts); \
+            else unpack_fast_kernel<D, NCH, MinBlocks<NCH, false>::value, false, E, false><<<grid, 256, 0, s>>>(g, lo, blob, blob_stride, K, V, tier_out, ts); \
         } while (0)
         if (g.row_chunks % 4 == 0) SKV_LAUNCH_UNPACK(4);
         else if (g.row_chunks % 2 == 0) SKV_LAUNCH_UNPACK(2);
