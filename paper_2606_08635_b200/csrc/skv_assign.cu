@@ -5,7 +5,8 @@
 // memory (global workspace when n*4 exceeds the shared-memory budget): protected positions get the
 // sentinel 0xFFFFFFFF (they outrank everything, so the top-n16 set contains them), every other token the
 // bits of its non-negative f32 score (NaN / negative / -0 -> 0), which order like the floats.
-// Three order statistics (ranks n16, n16+n8, n16+n8+n4) are found by an MSB-first 8-bit radix select;
+// Three order statistics (ranks n16, n16+n8, n16+n8+n4) are found together by ONE MSB-first 8-bit radix select of
+// four digit passes (thresholds that still share a key prefix share a histogram);
 // ties at a threshold are admitted in ascending position (a block scan of the "== threshold" flags),
 // which makes the result the unique stable ranking the oracle's sort produces.
 #include "skv_common.cuh"
@@ -21,29 +22,40 @@ __device__ __forceinline__ uint32_t sanitize_key(float x)
     return (x > 0.0f) ? __float_as_uint(x) : 0u;        // NaN compares false -> 0; -0, negatives -> 0
 }
 
-// K-th largest (1-based, 1 <= kth <= n) of keys[0..n): returns the key and the number of strictly greater keys.
-__device__ void radix_select(const uint32_t *keys, int n, uint32_t kth, uint32_t *hist /*256*/, uint32_t *bcast /*2*/,
-                             uint32_t &key_out, uint32_t &ngt_out)
+// The three order statistics (ranks kth[0] <= kth[1] <= kth[2], 1-based "K-th largest") of keys[0..n) in ONE sweep of
+// four MSB-first 8-bit digits.  At a given digit position the candidate sets of the thresholds are defined by their key
+// prefixes, which are pairwise equal or disjoint, so every key falls into at most one of (at most three) histograms;
+// thresholds that still share a prefix share a histogram.  act[k] = 0 marks a threshold that needs no selection (rank
+// 0 or >= n).  Returns, per active threshold, the key of rank kth[k] and the number of strictly greater keys.
+__device__ void radix_select3(const uint32_t *keys, int n, const uint32_t (&kth)[3], const bool (&act)[3],
+                              uint32_t (*hist)[256] /*[3][256]*/, uint32_t *bcast /*[6]*/, uint32_t (&key_out)[3], uint32_t (&ngt_out)[3])
 {
-    const uint32_t tid = threadIdx.x, lane = tid & 31;
-    uint32_t prefix = 0, mask = 0, remaining = kth;
+    const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    uint32_t prefix[3] = {0, 0, 0}, remaining[3] = {kth[0], kth[1], kth[2]}, mask = 0;
     for (int shift = 24; shift >= 0; shift -= 8) {
-        if (tid < 256) hist[tid] = 0;
+        if (tid < 768) (&hist[0][0])[tid] = 0;
         __syncthreads();
         for (int j0 = 0; j0 < n; j0 += blockDim.x) {
             const int j = j0 + tid;
-            const bool in = j < n && ((keys[j] & mask) == prefix);
-            const uint32_t digit = in ? (keys[j] >> shift) & 0xFFu : 0x100u;
-            // warp-aggregated histogram update: one atomic per distinct digit per warp
-            const uint32_t peers = __match_any_sync(0xffffffffu, digit);
-            if (in && lane == (uint32_t)(__ffs(peers) - 1)) atomicAdd(&hist[digit], __popc(peers));
+            uint32_t code = 0x400u;                                  // "no histogram"
+            if (j < n) {
+                const uint32_t key = keys[j], pk = key & mask;
+                const int grp = (act[0] && pk == prefix[0]) ? 0 : (act[1] && pk == prefix[1]) ? 1 : (act[2] && pk == prefix[2]) ? 2 : -1;
+                if (grp >= 0) code = ((uint32_t)grp << 8) | ((key >> shift) & 0xFFu);
+            }
+            // warp-aggregated histogram update: one atomic per distinct (histogram, digit) per warp
+            const uint32_t peers = __match_any_sync(0xffffffffu, code);
+            if (code != 0x400u && lane == (uint32_t)(__ffs(peers) - 1)) atomicAdd(&hist[code >> 8][code & 0xFFu], __popc(peers));
         }
         __syncthreads();
-        if (tid < 32) {
+        if (warp < 3 && act[warp]) {
+            const int k = (int)warp;
+            // the histogram of threshold k is the one of the first active threshold with the same prefix
+            const int src = (act[0] && prefix[0] == prefix[k]) ? 0 : (act[1] && prefix[1] == prefix[k]) ? 1 : k;
             // lane i owns bins [8i, 8i+8); suffix sums from the top digit down
             uint32_t loc[8], sum = 0;
 #pragma unroll
-            for (int b = 0; b < 8; ++b) { loc[b] = hist[lane * 8 + b]; sum += loc[b]; }
+            for (int b = 0; b < 8; ++b) { loc[b] = hist[src][lane * 8 + b]; sum += loc[b]; }
             uint32_t incl = sum;                          // inclusive suffix sum over lanes >= this lane
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
@@ -51,23 +63,22 @@ __device__ void radix_select(const uint32_t *keys, int n, uint32_t kth, uint32_t
                 if (lane + o < 32) incl += y;
             }
             const uint32_t above = incl - sum;            // keys in bins owned by higher lanes
-            const bool mine = above < remaining && remaining <= incl;
-            if (mine) {
+            if (above < remaining[k] && remaining[k] <= incl) {
                 uint32_t acc = above;
                 int b = 7;
-                for (; b >= 0; --b) { if (acc + loc[b] >= remaining) break; acc += loc[b]; }
-                bcast[0] = lane * 8 + b;                  // the digit of the K-th largest
-                bcast[1] = remaining - acc;               // its rank inside that bin
+                for (; b >= 0; --b) { if (acc + loc[b] >= remaining[k]) break; acc += loc[b]; }
+                bcast[2 * k] = lane * 8 + b;              // the digit of the K-th largest
+                bcast[2 * k + 1] = remaining[k] - acc;    // its rank inside that bin
             }
         }
         __syncthreads();
-        prefix |= bcast[0] << shift;
+#pragma unroll
+        for (int k = 0; k < 3; ++k)
+            if (act[k]) { prefix[k] |= bcast[2 * k] << shift; remaining[k] = bcast[2 * k + 1]; }
         mask |= 0xFFu << shift;
-        remaining = bcast[1];
-        __syncthreads();
     }
-    key_out = prefix;
-    ngt_out = kth - remaining;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) { key_out[k] = prefix[k]; ngt_out[k] = kth[k] - remaining[k]; }
 }
 
 __global__ void __launch_bounds__(kAssignThreads)
@@ -75,8 +86,8 @@ assign_kernel(Geom g, Intervals prot, const float *__restrict__ importance, uint
               uint32_t *__restrict__ key_ws, int keys_in_smem)
 {
     extern __shared__ uint32_t smem[];
-    __shared__ uint32_t hist[256];
-    __shared__ uint32_t bcast[2];
+    __shared__ uint32_t hist[3][256];
+    __shared__ uint32_t bcast[6];
     __shared__ uint32_t warp_tot[3][32];
     __shared__ Thresh th[3];
 
@@ -93,17 +104,20 @@ assign_kernel(Geom g, Intervals prot, const float *__restrict__ importance, uint
     __syncthreads();
 
     const uint32_t K[3] = {(uint32_t)g.n16, (uint32_t)(g.n16 + g.n8), (uint32_t)(g.n16 + g.n8 + g.n4)};
-    for (int k = 0; k < 3; ++k) {
-        uint32_t key = 0xFFFFFFFFu, ngt = 0, all = 0;
-        if (K[k] >= (uint32_t)n) all = 1;                 // every token passes this level
-        else if (K[k] > 0) radix_select(keys, n, K[k], hist, bcast, key, ngt);
-        else { key = 0xFFFFFFFFu; ngt = 0; }              // K = 0: nobody passes (rank test below fails)
-        if (tid == 0) { th[k].key = key; th[k].n_gt = ngt; th[k].pass_all = all; th[k].rank = K[k]; }
-        __syncthreads();
+    const bool act[3] = {K[0] > 0 && K[0] < (uint32_t)n, K[1] > 0 && K[1] < (uint32_t)n, K[2] > 0 && K[2] < (uint32_t)n};
+    uint32_t skey[3] = {0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu}, sngt[3] = {0, 0, 0};
+    if (act[0] || act[1] || act[2]) radix_select3(keys, n, K, act, hist, bcast, skey, sngt);
+    if (tid < 3) {
+        const int k = (int)tid;
+        // K >= n: every token passes this level; K = 0: nobody does (key 0xFFFFFFFF, rank test below fails)
+        th[k].key = act[k] ? skey[k] : 0xFFFFFFFFu; th[k].n_gt = act[k] ? sngt[k] : 0u;
+        th[k].pass_all = K[k] >= (uint32_t)n ? 1u : 0u; th[k].rank = K[k];
     }
+    __syncthreads();
 
     // position-ordered rank among equals: thread t owns the contiguous chunk [t*c, (t+1)*c)
-    const int c = (n + blockDim.x - 1) / blockDim.x;
+    // (an ODD chunk length keeps the 32 lanes of a warp on 32 different shared-memory banks)
+    const int c = ((n + blockDim.x - 1) / blockDim.x) | 1;
     const int beg = min(n, (int)tid * c), end = min(n, beg + c);
     uint32_t eq[3] = {0, 0, 0};
     for (int j = beg; j < end; ++j) {
