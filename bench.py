@@ -206,6 +206,44 @@ def dist_init(backend):
     return rank, local, world
 
 
+def numa_cpus_of_pci(domain, bus, device, sysfs="/sys/bus/pci/devices"):
+    """CPUs local to the PCI device (Linux sysfs `local_cpulist`, e.g. "0-15,32-47"), or None."""
+    path = os.path.join(sysfs, f"{domain:04x}:{bus:02x}:{device:02x}.0", "local_cpulist")
+    try:
+        with open(path) as f:
+            txt = f.read().strip()
+    except OSError:
+        return None
+    cpus = set()
+    for part in txt.split(","):
+        if not part:
+            continue
+        lo, _, hi = part.partition("-")
+        try:
+            cpus.update(range(int(lo), int(hi or lo) + 1))
+        except ValueError:
+            return None
+    return cpus or None
+
+
+def bind_rank_to_gpu_numa_node(local):
+    """Under torchrun (N ranks on one host) every rank pins host memory for the e2e leg: run the rank -- and so the
+    first touch of its pinned buffers -- on the CPUs of the NUMA node its GPU hangs off, so that eight ranks do not all
+    allocate on node 0 and cross the socket link on every copy.  Best effort: any failure leaves the affinity alone."""
+    try:
+        import torch
+        pr = torch.cuda.get_device_properties(local)
+        cpus = numa_cpus_of_pci(pr.pci_domain_id, pr.pci_bus_id, pr.pci_device_id)
+        if cpus:
+            allowed = cpus & os.sched_getaffinity(0)
+            if allowed:
+                os.sched_setaffinity(0, allowed)
+                return sorted(allowed)
+    except Exception:
+        pass
+    return None
+
+
 def aggregate_over_ranks(ms_local, bytes_local, device="cpu"):
     """max over ranks of the times, sum over ranks of the bytes (weak scaling).  ms_local: list of floats."""
     import torch
@@ -720,6 +758,7 @@ def main():
     from paper_2606_08635_b200 import lib
     lib()                                              # fail loudly if the CUDA library is missing
 
+    numa = bind_rank_to_gpu_numa_node(local) if world > 1 else None
     prob = DeviceProblem(cfg, b, R, dev, rank)
     flush = want_flush(args, cfg, R)
     K = args.steps
@@ -747,7 +786,7 @@ def main():
                "what": "GB/s of FP16 KV through the whole path from pinned host buffers (H2D K,V,Q; D2H + H2D hop of the blob; D2H result)",
                "h2d_bytes_per_step": r["h2d"], "d2h_bytes_per_step": r["d2h"], "ms_per_step": red2[0], "steps": r["steps"],
                "ms_per_request": red2[0] / R, "pipeline": f"layer chunks of {r['layers_per_chunk']}, {r['depth']} slots, 3 streams",
-               "pinned_host_requests": r["host_requests"],
+               "pinned_host_requests": r["host_requests"], "rank0_cpu_affinity": (len(numa) if numa else None),
                "sequential_ms_per_request": r["sequential_ms_per_request"],
                "raw_fp16_hop_ms_per_request": r["raw_fp16_hop_ms_per_request"],
                "blob_hop_ms_per_request": r["blob_hop_ms_per_request"]}

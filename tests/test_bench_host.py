@@ -38,3 +38,13 @@ def test_launch_count_per_step():
     C = skv_synth.CONFIGS
     assert bench.launches_per_step(C["C2"]) == 4          # importance, assign, pack, unpack (scan fused, n = 4096)
     assert bench.launches_per_step(C["C5"]) == 6          # + one tile scan each for pack and unpack (n = 32768)
+
+
+def test_numa_cpu_list_parsing(tmp_path):
+    d = tmp_path / "0000:1b:00.0"
+    d.mkdir()
+    (d / "local_cpulist").write_text("0-3,8,10-11\n")
+    assert bench.numa_cpus_of_pci(0, 0x1b, 0, sysfs=str(tmp_path)) == {0, 1, 2, 3, 8, 10, 11}
+    assert bench.numa_cpus_of_pci(0, 0x1c, 0, sysfs=str(tmp_path)) is None            # no such device: affinity left alone
+    (d / "local_cpulist").write_text("garbage")
+    assert bench.numa_cpus_of_pci(0, 0x1b, 0, sysfs=str(tmp_path)) is None
