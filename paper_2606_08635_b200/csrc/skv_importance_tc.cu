@@ -312,6 +312,44 @@ __device__ __forceinline__ float2 ex2_fma2_lo(float2 x)
                        __int_as_float(__float_as_int(q.y) + (__float_as_int(t.y) << 23)));
 }
 
+// pass 1, one 16-logit chunk of one query row: z += sum 2^(x*sc - m) over the first nvis logits (MASKED: the causal window /
+// ragged tail hides the rest; they are pushed to 2^-200, i.e. nothing, before the same packed pipeline as the unmasked
+// tiles -- the masked tiles are few, but with a scalar path for them the CTAs that own a row end reached the grid
+// barrier late: C2 94 -> 91 us).  Overflow guard of the lazy reference exponent per chunk and per row: a row whose chunk trips it redoes
+// the chunk with the exact online-max update, from the 16 logits still in registers (no TMEM re-read).
+template <bool MASKED>
+__device__ __forceinline__ void rowstats_chunk(const uint32_t (&r)[16], int nvis, float sc, float &m, float &z)
+{
+    const float2 nm2 = make_float2(-m, -m), sc2 = make_float2(sc, sc);
+    float2 accA = make_float2(0.f, 0.f), accB = accA;
+    float xmax = kNegBig;                                             // largest exponent sent to the FMA pipe
+#pragma unroll
+    for (int pi = 0; pi < 8; ++pi) {
+        float2 x = __ffma2_rn(make_float2(__uint_as_float(r[2 * pi]), __uint_as_float(r[2 * pi + 1])), sc2, nm2);
+        if (MASKED) { if (2 * pi >= nvis) x.x = -200.0f; if (2 * pi + 1 >= nvis) x.y = -200.0f; }
+        float2 e;
+        if (pair_on_fma(pi)) { xmax = fmaxf(xmax, fmaxf(x.x, x.y)); e = ex2_fma2_lo(x); }
+        else e = ex2_mufu2(x);
+        if (pi & 1) accB = __fadd2_rn(accB, e); else accA = __fadd2_rn(accA, e);
+    }
+    const float2 s2 = __fadd2_rn(accA, accB);
+    const float a = s2.x + s2.y;
+    if (a < 1.0e30f && xmax < 127.0f) {
+        z += a;
+        if (!(z < 1.0e30f)) { z *= 0x1p-80f; m += 80.0f; }
+    } else {
+        float tmax = kNegBig;
+#pragma unroll
+        for (int i = 0; i < 16; ++i) if (!MASKED || i < nvis) tmax = fmaxf(tmax, __uint_as_float(r[i]));
+        const float mn = fmaxf(m, tmax * sc);
+        float acc = 0.f;
+#pragma unroll
+        for (int i = 0; i < 16; ++i) acc += (!MASKED || i < nvis) ? ex2(fmaf(__uint_as_float(r[i]), sc, -mn)) : 0.f;
+        z = z * ex2(m - mn) + acc;
+        m = mn;
+    }
+}
+
 // pass 1, one work item: every epilogue thread owns one query row and 16*NCH key columns of each 128-key tile and
 // keeps the row's (reference exponent m, sum z of 2^(x - m)) in registers.  The reference exponent is lazy: it is
 // fixed by the first visible chunk of the row and only an overflow guard watches it afterwards (the row sum is
@@ -354,35 +392,7 @@ __device__ __forceinline__ void rowstats_segment(const Params &p, const Seg &it,
                     for (int i = 0; i < 16; ++i) tmax = fmaxf(tmax, __uint_as_float(r[i]));
                     m = tmax * sc;
                 }
-                const float2 nm2 = make_float2(-m, -m), sc2 = make_float2(sc, sc);
-                float2 accA = make_float2(0.f, 0.f), accB = accA;
-                float xmax = kNegBig;                                     // largest exponent sent to the FMA pipe
-#pragma unroll
-                for (int pi = 0; pi < 8; ++pi) {
-                    const float2 x = __ffma2_rn(make_float2(__uint_as_float(r[2 * pi]), __uint_as_float(r[2 * pi + 1])), sc2, nm2);
-                    float2 e;
-                    if (pair_on_fma(pi)) { xmax = fmaxf(xmax, fmaxf(x.x, x.y)); e = ex2_fma2_lo(x); }
-                    else e = ex2_mufu2(x);
-                    if (pi & 1) accB = __fadd2_rn(accB, e); else accA = __fadd2_rn(accA, e);
-                }
-                const float2 s2 = __fadd2_rn(accA, accB);
-                const float a = s2.x + s2.y;
-                // overflow guard of the lazy reference exponent, per chunk and per row: a row whose chunk trips it redoes
-                // the chunk with the exact online-max update, from the 16 logits still in registers (no TMEM re-read)
-                if (a < 1.0e30f && xmax < 127.0f) {
-                    z += a;
-                    if (!(z < 1.0e30f)) { z *= 0x1p-80f; m += 80.0f; }
-                } else {
-                    float tmax = kNegBig;
-#pragma unroll
-                    for (int i = 0; i < 16; ++i) tmax = fmaxf(tmax, __uint_as_float(r[i]));
-                    const float mn = fmaxf(m, tmax * sc);
-                    float acc = 0.f;
-#pragma unroll
-                    for (int i = 0; i < 16; ++i) acc += ex2(fmaf(__uint_as_float(r[i]), sc, -mn));
-                    z = z * ex2(m - mn) + acc;
-                    m = mn;
-                }
+                rowstats_chunk<false>(r, 16, sc, m, z);
             });
         SKV_TRACE_EV(g_ev_tile, 5, SKV_EPI_LOGGER);              // arithmetic of the tile done
         SKV_TRACE_ONLY(if (SKV_EPI_LOGGER) ++g_ev_tile;)
@@ -390,16 +400,15 @@ __device__ __forceinline__ void rowstats_segment(const Params &p, const Seg &it,
     for (; k0 < key_end; k0 += kTileKeys) {                               // ---- masked tiles (the last ones of a layer)
         stream_tile<NCH, ACOLS>(bA, bB, base, k0 + kTileKeys < key_end, tfull, tempty, lane, astage, aphase,
             [&](const uint32_t (&r)[16], int c) {
-                const int j0 = k0 + col0 + 16 * c;
-                float tmax = kNegBig;
+                const int nvis = lim - (k0 + col0 + 16 * c) + 1;          // visible logits of this chunk: <= 0 none, >= 16 all
+                if (nvis <= 0) return;                                    // (per row; nothing warp-collective in here)
+                if (m < 0.5f * kNegBig) {                                 // first visible chunk of the row fixes the reference
+                    float tmax = kNegBig;
 #pragma unroll
-                for (int i = 0; i < 16; ++i) if (j0 + i <= lim) tmax = fmaxf(tmax, __uint_as_float(r[i]));
-                const float mn = fmaxf(m, tmax > 0.5f * kNegBig ? tmax * sc : kNegBig);
-                float acc = 0.f;
-#pragma unroll
-                for (int i = 0; i < 16; ++i) acc += (j0 + i <= lim) ? ex2(fmaf(__uint_as_float(r[i]), sc, -mn)) : 0.f;
-                z = z * ex2(m - mn) + acc;
-                m = mn;
+                    for (int i = 0; i < 16; ++i) if (i < nvis) tmax = fmaxf(tmax, __uint_as_float(r[i]));
+                    m = tmax * sc;
+                }
+                rowstats_chunk<true>(r, nvis, sc, m, z);
             });
     }
     if (valid) {
@@ -456,18 +465,33 @@ __device__ __forceinline__ void colsum_segment(const Params &p, const Seg &it, u
             const float2 s2 = __fadd2_rn(accA, accB);
             mine = s2.x + s2.y;
         } else {                                                          // ---- masked tile or padded column group
-            float s0 = 0.f;
+            // the same packed pipeline; a logit the key may not see (causal window, padding column: limit -1) is pushed
+            // to 2^-200 first
+            float2 accA = make_float2(0.f, 0.f), accB = accA;
             auto chunk = [&](const uint32_t (&r)[16], int c) {
                 const int cc = 16 * c;
-                if (cbeg + cc >= mrows) return;                           // warp-uniform: padding columns
-                const int *lim = sLim + cbeg + cc;
+                if (cbeg + cc >= mrows) return;                           // warp-uniform: padding columns only
+                const float4 *l4 = reinterpret_cast<const float4 *>(sLse + cbeg + cc);
+                const int4 *m4 = reinterpret_cast<const int4 *>(sLim + cbeg + cc);
+                const float2 sc2 = make_float2(sc, sc);
 #pragma unroll
-                for (int i = 0; i < 16; ++i)
-                    s0 += (j <= lim[i]) ? ex2(fmaf(__uint_as_float(r[i]), sc, sLse[cbeg + cc + i])) : 0.f;
+                for (int i = 0; i < 4; ++i) {
+                    const float4 L4 = l4[i];
+                    const int4 M4 = m4[i];
+                    float2 x0 = __ffma2_rn(make_float2(__uint_as_float(r[4 * i]), __uint_as_float(r[4 * i + 1])), sc2, make_float2(L4.x, L4.y));
+                    float2 x1 = __ffma2_rn(make_float2(__uint_as_float(r[4 * i + 2]), __uint_as_float(r[4 * i + 3])), sc2, make_float2(L4.z, L4.w));
+                    if (j > M4.x) x0.x = -200.0f;
+                    if (j > M4.y) x0.y = -200.0f;
+                    if (j > M4.z) x1.x = -200.0f;
+                    if (j > M4.w) x1.y = -200.0f;
+                    accA = __fadd2_rn(accA, pair_on_fma(2 * i) ? ex2_fma2_lo(x0) : ex2_mufu2(x0));
+                    accB = __fadd2_rn(accB, pair_on_fma(2 * i + 1) ? ex2_fma2_lo(x1) : ex2_mufu2(x1));
+                }
             };
             if (!par) stream_tile<QC, ACOLS>(bA, bB, base, more, tfull, tempty, lane, astage, aphase, chunk);
             else      stream_tile<QC, ACOLS>(bB, bA, base, more, tfull, tempty, lane, astage, aphase, chunk);
-            mine = s0;
+            const float2 s2 = __fadd2_rn(accA, accB);
+            mine = s2.x + s2.y;
         }
         if (QC & 1) par = !par;
         // add the four column groups of this tile in a fixed order (deterministic): groups 1..3 drop their sums
