@@ -23,7 +23,10 @@
  *   - Every pointer is tagged HOST or DEVICE.  DEVICE pointers are plain CUDA device addresses
  *     (e.g. torch.Tensor.data_ptr()); the library never allocates, frees or keeps them.
  *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  All work is
- *     enqueued on that stream; no entry point synchronises the host.
+ *     enqueued on that stream; no entry point synchronises the host, so a sequence of calls can be captured into a
+ *     CUDA graph (tests: test_whole_path_is_cuda_graph_capturable).  Launches per call: skv_importance 1 (cooperative:
+ *     it needs the whole GPU, one CTA per SM) + one 4-byte memset node (the grid-barrier counter); skv_assign_tiers 1; skv_pack / skv_unpack 1 for
+ *     n_tokens <= 8192 and 2 (slot scan first) beyond or for sparse upgrade blobs; skv_importance_kvnorm 2.
  *   - Every entry returns SKV_OK (0) or a negative skv_status and launches nothing on error.
  *   - The library keeps no mutable global state and is re-entrant.  (Two process-wide constants are set idempotently:
  *     the driver entry point of the tensor-map encoder is looked up once and cached, and kernels that need more than

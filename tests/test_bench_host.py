@@ -48,3 +48,12 @@ def test_numa_cpu_list_parsing(tmp_path):
     assert bench.numa_cpus_of_pci(0, 0x1c, 0, sysfs=str(tmp_path)) is None            # no such device: affinity left alone
     (d / "local_cpulist").write_text("garbage")
     assert bench.numa_cpus_of_pci(0, 0x1b, 0, sysfs=str(tmp_path)) is None
+
+
+def test_recorded_ncu_traffic_is_on_file_for_the_bench_workload():
+    for kernel in ("pack", "unpack"):
+        traffic, source = bench.ncu_traffic("C5", 0.5, 4, kernel)
+        alg = 25_912_476_672                                               # algorithmic bytes of one launch
+        assert traffic is not None and abs(traffic - alg) / alg < 0.01     # no re-reads: DRAM traffic = algorithmic bytes
+        assert "rev" in source                                             # provenance of the capture travels with the number
+    assert bench.ncu_traffic("C5", 0.45, 4, "pack") == (None, None)        # no capture of that workload: null, not a guess
