@@ -386,6 +386,18 @@ def time_problem(prob, K, W, flush, sampler=None, dev=None):
     return {"stage_ms": stage_ms, "stage_min": stage_min, "ms_step": ms_step, "clocks": clocks, "wall_s": t_wall}
 
 
+def importance_lower_bound_ms(cfg, R, hbm_gbs, tensor_tflops, sm_count=148, sm_ghz=1.965, ex2_per_clk_sm=16.0):
+    """max of (K read once from HBM, the contraction twice at the sustained tensor peak, the exponentials
+    twice at 16 MUFU results per clock per SM at the maximum SM clock).  Returns (ms, which term binds)."""
+    k_bytes = cfg.bytes_fp16 * R / 2.0
+    flop = 2.0 * cfg.L * cfg.Hq * cfg.w * cfg.n * cfg.d * R
+    exps = 1.0 * cfg.L * cfg.Hq * cfg.w * cfg.n * R
+    terms = {"hbm (K once)": k_bytes / (hbm_gbs * 1e9), "tensor (2 passes)": 2.0 * flop / (tensor_tflops * 1e12),
+             "ex2 (2 passes)": 2.0 * exps / (sm_count * ex2_per_clk_sm * sm_ghz * 1e9)}
+    which = max(terms, key=terms.get)
+    return terms[which] * 1e3, which
+
+
 def sweep_row(prob, res, peak, flush):
     cfg = prob.cfg
     alg = prob.algorithmic_bytes()
@@ -398,6 +410,8 @@ def sweep_row(prob, res, peak, flush):
             "unpack_frac_of_hbm_peak": alg["unpack"] / (up * 1e-3) / 1e9 / peak,
             "pack_plus_unpack_frac_of_hbm_peak": (alg["pack"] + alg["unpack"]) / ((pk + up) * 1e-3) / 1e9 / peak,
             "gpu_launches_per_step": launches_per_step(cfg),
+            "importance_lower_bound_ms": importance_lower_bound_ms(cfg, prob.R, peak, measured_tensor_peak()[0])[0],
+            "importance_frac_of_lower_bound": importance_lower_bound_ms(cfg, prob.R, peak, measured_tensor_peak()[0])[0] / imp,
             "l2": l2_note(cfg, prob.R, prob.blob_bytes, flush)}
 
 
@@ -824,6 +838,9 @@ def main():
                        "executed_tflops": 2.0 * imp_flop / (ms_imp * 1e-3) / 1e12,
                        "note": "two-pass: the contraction and the exponentials run twice; bound by the MUFU ex2 / FMA / "
                                "tensor pipe mix at d_h = 128 (profiles/r2_importance_ncu.md), not by the tensor pipe alone",
+                       "lower_bound_ms": importance_lower_bound_ms(cfg, R, peak, tpeak)[0],
+                       "lower_bound_term": importance_lower_bound_ms(cfg, R, peak, tpeak)[1],
+                       "frac_of_lower_bound": importance_lower_bound_ms(cfg, R, peak, tpeak)[0] / ms_imp,
                        "tensor_peak_tflops": tpeak, "tensor_peak_source": tpeak_src,
                        "useful_frac_of_tensor_peak": imp_flop / (ms_imp * 1e-3) / 1e12 / tpeak,
                        "executed_frac_of_tensor_peak": 2.0 * imp_flop / (ms_imp * 1e-3) / 1e12 / tpeak},

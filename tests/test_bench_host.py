@@ -57,3 +57,13 @@ def test_recorded_ncu_traffic_is_on_file_for_the_bench_workload():
         assert traffic is not None and abs(traffic - alg) / alg < 0.01     # no re-reads: DRAM traffic = algorithmic bytes
         assert "rev" in source                                             # provenance of the capture travels with the number
     assert bench.ncu_traffic("C5", 0.45, 4, "pack") == (None, None)        # no capture of that workload: null, not a guess
+
+
+def test_importance_lower_bounds_match_the_survey_table():
+    C = skv_synth.CONFIGS
+    want = {"C2": 0.044, "C3": 0.058, "C4": 0.108, "C5": 0.92}              # SURVEY.md 8(d), ms per request
+    for name, ms in want.items():
+        got, which = bench.importance_lower_bound_ms(C[name], 1, 6523.0, 1413.0)
+        assert abs(got - ms) / ms < 0.04, (name, got, which)
+    assert bench.importance_lower_bound_ms(C["C4"], 1, 6523.0, 1413.0)[1].startswith("hbm")
+    assert bench.importance_lower_bound_ms(C["C5"], 1, 6523.0, 1413.0)[1].startswith("ex2")
