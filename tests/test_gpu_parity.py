@@ -11,7 +11,7 @@ import torch
 import oracle
 import paper_2606_08635_b200 as skv
 import skv_synth
-from parity_util import Case, assert_bit_exact, assert_importance_close, gpu_pipeline, near_tie_mask
+from parity_util import Case, assert_bit_exact, assert_importance_close, gpu_pipeline, near_tie_mask, to_layout
 
 pytestmark = pytest.mark.gpu
 
@@ -889,3 +889,34 @@ def test_whole_path_is_cuda_graph_capturable(name, n):
             assert np.array_equal(Ko[r].cpu().numpy().view(np.uint16), K2.view(np.uint16))
             assert np.array_equal(Vo[r].cpu().numpy().view(np.uint16), V2.view(np.uint16))
             assert np.array_equal(tier_out[r].cpu().numpy(), t2)
+
+
+@pytest.mark.parametrize("d,Hkv,n,R,layout,bf16,lam", [
+    (128, 8, 1000, 2, "token_major", False, 0.0),      # rows of 1024 elements: four 16-byte chunks per lane
+    (128, 4, 777, 1, "token_major", False, 0.01),      # 512 elements: two chunks; n not a multiple of 64
+    (256, 1, 130, 3, "token_major", False, 0.0),       # 256 elements: one chunk, one head vector per warp load
+    (64, 4, 4097, 1, "hf", False, 0.001),              # head-major strides, four head vectors per chunk
+    (64, 3, 257, 2, "token_major", False, 0.005),      # 192 elements: the generic kernel
+    (128, 8, 515, 1, "token_major", True, 0.005),      # bfloat16 keys
+    (256, 2, 64, 1, "hf", True, 0.0)])
+def test_kvnorm_score_shapes_layouts_and_dtypes(d, Hkv, n, R, layout, bf16, lam):
+    """NEXT-1 fallback score on every instantiation of the kernel (chunks per row, generic rows, strides, bfloat16, several
+    requests, ragged token counts) against the oracle, 1e-3 relative; plus: the score sums to 1 per layer at lambda = 0."""
+    dev = torch.device("cuda:0")
+    L = 3
+    g = torch.Generator().manual_seed(1000 * d + Hkv + n)
+    K = torch.randn((R, L, n, Hkv, d), generator=g) * (1.0 + 3.0 * torch.rand((R, L, n, 1, 1), generator=g))
+    K[0, 0, 5] = 0.0                                                       # a zero token scores 0
+    K = K.to(torch.bfloat16 if bf16 else torch.float16)
+    shape = skv.make_shape(L, Hkv, Hkv, d, n, R, layout=layout, dtype="bf16" if bf16 else "f16")
+    Kd = to_layout(K, layout).to(dev)
+    ws = torch.full((skv.skv_workspace_bytes(shape, 0),), 0xCD, dtype=torch.uint8, device=dev)      # stale workspace contents
+    I = torch.full((R, L, n), float("nan"), dtype=torch.float32, device=dev)
+    skv.skv_importance_kvnorm(shape, Kd, I, ws, lam=lam)
+    got = I.cpu().numpy().astype(np.float64)
+    for r in range(R):
+        want = oracle.importance_kvnorm(_bits(K[r]) if bf16 else K[r].numpy(), lam=lam, bf16=bf16).astype(np.float64)
+        assert np.all(np.abs(got[r] - want) <= 1e-3 * want + 1e-30), np.max(np.abs(got[r] - want) / (want + 1e-30))
+        assert got[r][0, 5] == 0.0 if r == 0 else True
+        if lam == 0.0:
+            assert np.allclose(got[r].sum(axis=1), 1.0, rtol=1e-5)
