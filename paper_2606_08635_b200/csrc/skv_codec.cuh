@@ -151,18 +151,32 @@ __device__ __forceinline__ uint2 quant8_int8(const uint4 &v, float inv)
                       pack4_bytes(rne_code_bits(c.x, inv), rne_code_bits(c.y, inv), rne_code_bits(d.x, inv), rne_code_bits(d.y, inv)));
 }
 
-// 8 fp16 -> 8 INT4 codes (one word; element 2k in the low nibble of byte k)
+// 8 fp16 -> 8 INT4 codes (one word; element 2k in the low nibble of byte k).  The codes are built in the mantissas of
+// packed float pairs by fused multiply-adds (FFMA2: two elements per issue slot):
+//     a <- fma(x_hi, inv, M)              M = 1.5 * 2^23;  a = M + q_hi, the FMA's single rounding is RNE(x * inv)
+//     a <- fma(a, 256, -255 * M)          exact: M + 256 q_hi   (255 M = 765 * 2^22 is a binary32 number)
+//     a <- fma(x_lo, inv, a)              a = M + q_lo + 256 q_hi   (a is an even integer in [2^23, 2^24) before each
+//                                         rounding step, so ties keep rounding to even)
+// with (x_lo, x_hi) = elements (e, e + 2) in the .x lane and (e + 1, e + 3) in the .y lane.  The codes are signed, so an
+// integer add of 0x0808 to the mantissa makes both fields unsigned (q + 8 in 1..15, no borrows between them); one
+// bit-select interleaves the two lanes into four nibbles, and q + 8 -> two's-complement nibble is an XOR with 8.
 template <class E>
 __device__ __forceinline__ uint32_t quant8_int4(const uint4 &v, float inv)
 {
     using H2 = typename E::H2;
-    const float2 a = to_f2(as_pair<H2>(v.x)), b = to_f2(as_pair<H2>(v.y));
-    const float2 c = to_f2(as_pair<H2>(v.z)), d = to_f2(as_pair<H2>(v.w));
-    const uint32_t b0 = (rne_code_bits(a.x, inv) & 0xFu) | (rne_code_bits(a.y, inv) << 4);
-    const uint32_t b1 = (rne_code_bits(b.x, inv) & 0xFu) | (rne_code_bits(b.y, inv) << 4);
-    const uint32_t b2 = (rne_code_bits(c.x, inv) & 0xFu) | (rne_code_bits(c.y, inv) << 4);
-    const uint32_t b3 = (rne_code_bits(d.x, inv) & 0xFu) | (rne_code_bits(d.y, inv) << 4);
-    return pack4_bytes(b0, b1, b2, b3);
+    const float2 inv2 = make_float2(inv, inv);
+    const float2 first = make_float2(12582912.0f, 12582912.0f);                       // M
+    const float2 sh = make_float2(256.0f, 256.0f), back = make_float2(-3208642560.0f, -3208642560.0f);   // -255 M
+    float2 a = __ffma2_rn(to_f2(as_pair<H2>(v.y)), inv2, first);                      // elements (2, 3)
+    float2 b = __ffma2_rn(to_f2(as_pair<H2>(v.w)), inv2, first);                      // elements (6, 7)
+    a = __ffma2_rn(a, sh, back);
+    b = __ffma2_rn(b, sh, back);
+    a = __ffma2_rn(to_f2(as_pair<H2>(v.x)), inv2, a);                                 // elements (0, 1)
+    b = __ffma2_rn(to_f2(as_pair<H2>(v.z)), inv2, b);                                 // elements (4, 5)
+    // .x holds nibbles 0 and 2 of a half-word (bits 0-3, 8-11), .y nibbles 1 and 3 once shifted up by 4
+    const uint32_t h0 = ((__float_as_uint(a.x) + 0x0808u) & 0x0F0Fu) | (((__float_as_uint(a.y) + 0x0808u) << 4) & 0xF0F0u);
+    const uint32_t h1 = ((__float_as_uint(b.x) + 0x0808u) & 0x0F0Fu) | (((__float_as_uint(b.y) + 0x0808u) << 4) & 0xF0F0u);
+    return __byte_perm(h0, h1, 0x5410) ^ 0x88888888u;
 }
 
 // ------------------------------------------------------------------------------------------------
