@@ -48,10 +48,14 @@ __device__ void radix_select3(const uint32_t *keys, int n, const uint32_t (&kth)
             if (code != 0x400u && lane == (uint32_t)(__ffs(peers) - 1)) atomicAdd(&hist[code >> 8][code & 0xFFu], __popc(peers));
         }
         __syncthreads();
-        if (warp < 3 && act[warp]) {
-            const int k = (int)warp;
+        // (registers, not indexable arrays: select with the warp-uniform k)
+        const int k = (int)warp;
+        const bool act_k = k == 0 ? act[0] : k == 1 ? act[1] : k == 2 ? act[2] : false;
+        if (act_k) {
+            const uint32_t prefix_k = k == 0 ? prefix[0] : k == 1 ? prefix[1] : prefix[2];
+            const uint32_t rem_k = k == 0 ? remaining[0] : k == 1 ? remaining[1] : remaining[2];
             // the histogram of threshold k is the one of the first active threshold with the same prefix
-            const int src = (act[0] && prefix[0] == prefix[k]) ? 0 : (act[1] && prefix[1] == prefix[k]) ? 1 : k;
+            const int src = (act[0] && prefix[0] == prefix_k) ? 0 : (act[1] && prefix[1] == prefix_k) ? 1 : k;
             // lane i owns bins [8i, 8i+8); suffix sums from the top digit down
             uint32_t loc[8], sum = 0;
 #pragma unroll
@@ -63,12 +67,15 @@ __device__ void radix_select3(const uint32_t *keys, int n, const uint32_t (&kth)
                 if (lane + o < 32) incl += y;
             }
             const uint32_t above = incl - sum;            // keys in bins owned by higher lanes
-            if (above < remaining[k] && remaining[k] <= incl) {
+            if (above < rem_k && rem_k <= incl) {
                 uint32_t acc = above;
                 int b = 7;
-                for (; b >= 0; --b) { if (acc + loc[b] >= remaining[k]) break; acc += loc[b]; }
+#pragma unroll
+                for (int bb = 7; bb >= 0; --bb) {         // highest bin whose suffix count reaches the rank
+                    if (b == bb) { if (acc + loc[bb] >= rem_k) break; acc += loc[bb]; b = bb - 1; }
+                }
                 bcast[2 * k] = lane * 8 + b;              // the digit of the K-th largest
-                bcast[2 * k + 1] = remaining[k] - acc;    // its rank inside that bin
+                bcast[2 * k + 1] = rem_k - acc;           // its rank inside that bin
             }
         }
         __syncthreads();
