@@ -18,7 +18,12 @@
 //   * ONE cooperative launch runs pass 1 | lse2 per row | pass 2 | final sum, separated by grid-wide barriers, so
 //     TMEM, the mbarriers and the tensor maps are set up once and a 4 K-token request pays one launch, not four;
 //   * the epilogue pulls TMEM in 16-column chunks with one chunk in flight (the load of chunk c+1 is issued before
-//     the exponentials of chunk c), so the TMEM latency hides behind arithmetic.
+//     the exponentials of chunk c), so the TMEM latency hides behind arithmetic, and hands an accumulator stage back
+//     the moment its last chunk is in registers: with two 256-column stages the chain release -> MMA -> commit would
+//     otherwise be serial with the arithmetic (profiles/r2_importance_ncu.md: measured with per-tile clock stamps).
+// What bounds it (same file): not TMEM (>= 670 B/clk/SM read, ~50 used), not the tensor pipe (64 clk per K = 16 step,
+// as measured alone), not HBM except at head_dim 256; the epilogue's ~69 instructions per 16 exponentials on four
+// in-order warps per scheduler, at the clock the 1 kW power cap leaves.
 // Work decomposition (both passes): the unit is one 128-key tile of one (request, layer, KV head, row block); the
 // R*L*S*T units, tile index fastest, are cut into gridDim.x equal contiguous ranges, one per CTA ("stream-K"), so
 // every SM gets the same number of tiles (+-1) whatever the shape.  A CTA walks its range as segments (one
