@@ -199,6 +199,9 @@ def dist_env():
 def dist_init(backend):
     import torch.distributed as dist
     rank, local, world = dist_env()
+    if backend == "nccl":
+        import torch
+        torch.cuda.set_device(local)                  # before the process group exists: NCCL binds to the current device
     if world > 1 and not dist.is_initialized():
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
         os.environ.setdefault("MASTER_PORT", "29511")
@@ -266,6 +269,15 @@ def barrier():
     import torch.distributed as dist
     if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
         dist.barrier()
+
+
+def dist_finish():
+    import torch.distributed as dist
+    if dist.is_available() and dist.is_initialized():
+        try:
+            dist.destroy_process_group()
+        except Exception:
+            pass
 
 
 # ----------------------------------------------------------------------------------------------------
@@ -806,6 +818,7 @@ def main():
                "blob_hop_ms_per_request": r["blob_hop_ms_per_request"]}
 
     if rank != 0:
+        dist_finish()
         return
     alg = prob.algorithmic_bytes()
     dom = "pack" if ms_pack >= ms_unpack else "unpack"
@@ -857,6 +870,7 @@ def main():
     if not args.no_cpu_baseline:
         line["cpu_baseline"] = oracle_sample(cfg, b, args.cpu_seconds)        # rank 0 only (the other ranks returned above)
     print(json.dumps(line), flush=True)
+    dist_finish()
 
 
 if __name__ == "__main__":
