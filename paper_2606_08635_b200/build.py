@@ -1,6 +1,10 @@
 """Build libskv.so (hand-written CUDA for sm_100a + the C ABI of include/skv.h) in-tree with nvcc.
 
-    python -m paper_2606_08635_b200.build [--force] [--verbose]
+    python -m paper_2606_08635_b200.build [--force] [--verbose] [--define NAME[=VALUE] ...]
+
+--define passes -DNAME[=VALUE] to nvcc: the diagnostics switches of csrc/skv_importance_tc.cu (SKV_DIAG_NOEXP,
+SKV_DIAG_NOTMA, SKV_EX2_FMA_PAIRS=k; profiles/r2_importance_ncu.md) -- such a library is for measurements only; rebuild
+without the switch afterwards.
 
 The shared library sits next to this file so that it travels with the repository snapshot; it links the
 CUDA runtime statically and needs no GPU to load (nvcc cross-compiles on a CPU-only box).
@@ -32,14 +36,15 @@ def _stale():
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force=False, verbose=False):
-    if not force and not _stale():
+def build(force=False, verbose=False, defines=()):
+    if not force and not defines and not _stale():
         return LIB
     objs = []
     procs = []
     for src in SOURCES:
         obj = os.path.join(CSRC, src.replace(".cu", ".o"))
-        cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", os.path.join(CSRC, src), "-o", obj]
+        cmd = ([_nvcc()] + NVCC_FLAGS + ["-D" + d for d in defines] + (["-Xptxas", "-v"] if verbose else []) +
+               ["-c", os.path.join(CSRC, src), "-o", obj])
         procs.append((src, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
         objs.append(obj)
     for src, p in procs:
@@ -55,4 +60,5 @@ def build(force=False, verbose=False):
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    _defs = [sys.argv[i + 1] for i, a in enumerate(sys.argv[:-1]) if a == "--define"]
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv, defines=_defs))
