@@ -410,6 +410,30 @@ def importance_lower_bound_ms(cfg, R, hbm_gbs, tensor_tflops, sm_count=148, sm_g
     return terms[which] * 1e3, which
 
 
+def graph_replay_ms(prob, reps=20):
+    """The whole path (importance -> assign -> pack -> unpack) captured once into a CUDA graph and replayed: the latency a
+    serving loop sees for one request batch, without host launch gaps and without an L2 flush (warm L2, stated so)."""
+    import torch
+    saved, prob.flush_buf = prob.flush_buf, None
+    try:
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=side):
+            prob.step()
+        for _ in range(3):
+            graph.replay()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps):
+            graph.replay()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps
+    finally:
+        prob.flush_buf = saved
+
+
 def sweep_row(prob, res, peak, flush):
     cfg = prob.cfg
     alg = prob.algorithmic_bytes()
@@ -451,7 +475,10 @@ def run_sweep(args, main_prob, dev, peak, steps):
         for b in cfg.budgets:
             prob.set_budget(b)
             fl = want_flush(args, cfg, cfg.R)
-            rows.append(sweep_row(prob, time_problem(prob, steps, 3, fl), peak, fl))
+            row = sweep_row(prob, time_problem(prob, steps, 3, fl), peak, fl)
+            row["cuda_graph_replay_ms_per_step"] = graph_replay_ms(prob)
+            row["cuda_graph_note"] = "whole path as ONE captured CUDA graph, back-to-back replays, L2 not flushed"
+            rows.append(row)
         del prob
     return rows
 
