@@ -140,15 +140,16 @@ __device__ __forceinline__ uint32_t pack4_bytes(uint32_t a, uint32_t b, uint32_t
     return __byte_perm(ab, cd, 0x5410);               // [a.b0, b.b0, c.b0, d.b0]
 }
 
-// 8 fp16 -> 8 INT8 codes (two words)
+// 8 fp16 -> 8 INT8 codes (two words): rne_code_bits on packed pairs (FFMA2: two elements per issue slot)
 template <class E>
 __device__ __forceinline__ uint2 quant8_int8(const uint4 &v, float inv)
 {
     using H2 = typename E::H2;
-    const float2 a = to_f2(as_pair<H2>(v.x)), b = to_f2(as_pair<H2>(v.y));
-    const float2 c = to_f2(as_pair<H2>(v.z)), d = to_f2(as_pair<H2>(v.w));
-    return make_uint2(pack4_bytes(rne_code_bits(a.x, inv), rne_code_bits(a.y, inv), rne_code_bits(b.x, inv), rne_code_bits(b.y, inv)),
-                      pack4_bytes(rne_code_bits(c.x, inv), rne_code_bits(c.y, inv), rne_code_bits(d.x, inv), rne_code_bits(d.y, inv)));
+    const float2 inv2 = make_float2(inv, inv), magic = make_float2(12582912.0f, 12582912.0f);
+    const float2 a = __ffma2_rn(to_f2(as_pair<H2>(v.x)), inv2, magic), b = __ffma2_rn(to_f2(as_pair<H2>(v.y)), inv2, magic);
+    const float2 c = __ffma2_rn(to_f2(as_pair<H2>(v.z)), inv2, magic), d = __ffma2_rn(to_f2(as_pair<H2>(v.w)), inv2, magic);
+    return make_uint2(pack4_bytes(__float_as_uint(a.x), __float_as_uint(a.y), __float_as_uint(b.x), __float_as_uint(b.y)),
+                      pack4_bytes(__float_as_uint(c.x), __float_as_uint(c.y), __float_as_uint(d.x), __float_as_uint(d.y)));
 }
 
 // 8 fp16 -> 8 INT4 codes (one word; element 2k in the low nibble of byte k).  The codes are built in the mantissas of
