@@ -235,13 +235,15 @@ __device__ __forceinline__ H2 group_absmax(H2 (&m)[NCH], uint32_t lane)
 template <int BIAS, class E>
 __device__ __forceinline__ void dequant4(uint32_t w, float scale, uint32_t &o0, uint32_t &o1)
 {
-    constexpr float kOff = 8388608.0f + (float)BIAS;                  // 2^23 + BIAS, exact
-    const float f0 = __fsub_rn(__uint_as_float(__byte_perm(w, 0x4B000000u, 0x7540)), kOff);
-    const float f1 = __fsub_rn(__uint_as_float(__byte_perm(w, 0x4B000000u, 0x7541)), kOff);
-    const float f2 = __fsub_rn(__uint_as_float(__byte_perm(w, 0x4B000000u, 0x7542)), kOff);
-    const float f3 = __fsub_rn(__uint_as_float(__byte_perm(w, 0x4B000000u, 0x7543)), kOff);
-    o0 = from_f2<E>(__fmul_rn(f0, scale), __fmul_rn(f1, scale));
-    o1 = from_f2<E>(__fmul_rn(f2, scale), __fmul_rn(f3, scale));
+    constexpr float kOff = -(8388608.0f + (float)BIAS);               // -(2^23 + BIAS), exact
+    const float2 off = make_float2(kOff, kOff), sc2 = make_float2(scale, scale);
+    // packed pairs (FADD2 / FMUL2: two elements per issue slot); per lane the same two roundings as fsub, fmul
+    const float2 a = __fmul2_rn(__fadd2_rn(make_float2(__uint_as_float(__byte_perm(w, 0x4B000000u, 0x7540)),
+                                                       __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7541))), off), sc2);
+    const float2 b = __fmul2_rn(__fadd2_rn(make_float2(__uint_as_float(__byte_perm(w, 0x4B000000u, 0x7542)),
+                                                       __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7543))), off), sc2);
+    o0 = from_f2<E>(a.x, a.y);
+    o1 = from_f2<E>(b.x, b.y);
 }
 template <class E>
 __device__ __forceinline__ uint4 dequant_int8(uint2 w, float scale)
@@ -257,19 +259,16 @@ __device__ __forceinline__ uint4 dequant_int4(uint32_t w, float scale)
     w ^= 0x88888888u;                                   // every nibble becomes q+8
     const uint32_t even = w & 0x0F0F0F0Fu;              // elements 0,2,4,6
     const uint32_t odd = (w >> 4) & 0x0F0F0F0Fu;        // elements 1,3,5,7
-    constexpr float kOff = 8388608.0f + 8.0f;
-    float f[8];
+    const float2 off = make_float2(-8388616.0f, -8388616.0f), sc2 = make_float2(scale, scale);      // -(2^23 + 8)
+    uint32_t o[4];
 #pragma unroll
-    for (int k = 0; k < 4; ++k) {
-        f[2 * k] = __fsub_rn(__uint_as_float(__byte_perm(even, 0x4B000000u, 0x7540 + k)), kOff);
-        f[2 * k + 1] = __fsub_rn(__uint_as_float(__byte_perm(odd, 0x4B000000u, 0x7540 + k)), kOff);
+    for (int k = 0; k < 4; ++k) {                        // elements 2k (even nibble of byte k) and 2k+1 (odd nibble), as a packed pair
+        const float2 f = make_float2(__uint_as_float(__byte_perm(even, 0x4B000000u, 0x7540 + k)),
+                                     __uint_as_float(__byte_perm(odd, 0x4B000000u, 0x7540 + k)));
+        const float2 y = __fmul2_rn(__fadd2_rn(f, off), sc2);
+        o[k] = from_f2<E>(y.x, y.y);
     }
-    uint4 o;
-    o.x = from_f2<E>(__fmul_rn(f[0], scale), __fmul_rn(f[1], scale));
-    o.y = from_f2<E>(__fmul_rn(f[2], scale), __fmul_rn(f[3], scale));
-    o.z = from_f2<E>(__fmul_rn(f[4], scale), __fmul_rn(f[5], scale));
-    o.w = from_f2<E>(__fmul_rn(f[6], scale), __fmul_rn(f[7], scale));
-    return o;
+    return make_uint4(o[0], o[1], o[2], o[3]);
 }
 // ------------------------------------------------------------------------------------------------
 // NEXT-4: asymmetric 2-bit low tier (include/skv.h "2-bit quantiser")
