@@ -920,3 +920,40 @@ def test_kvnorm_score_shapes_layouts_and_dtypes(d, Hkv, n, R, layout, bf16, lam)
         assert got[r][0, 5] == 0.0 if r == 0 else True
         if lam == 0.0:
             assert np.allclose(got[r].sum(axis=1), 1.0, rtol=1e-5)
+
+
+@pytest.mark.parametrize("n,k", [(1000, 400), (9000, 3000)])
+def test_dense_upgrade_blob_patch_in_fused_and_scan_first_plans(n, k):
+    """skv_unpack_patch with a blob that is NOT sparse (more than one token in eight upgraded): the fused one-launch plan
+    (n <= 8192) and the scan-first plan (n > 8192) in patch mode -- tokens the blob does not carry stay untouched, the
+    tier map changes only at the carried tokens; blob and patched cache bit-exact against the oracle."""
+    dev = torch.device("cuda:0")
+    cfg = skv_synth.Config(f"dense_up_{n}", L=2, Hq=4, Hkv=2, d=128, n=n, w=4, R=2, n_sink=2, seed=91, allow_int4=True)
+    case = Case(cfg, 0.3, with_importance=False)
+    out = gpu_pipeline(case, run_importance=False)
+    shape = case.shape()
+    ws = torch.empty(skv.skv_workspace_bytes(shape, 0), dtype=torch.uint8, device=dev)
+    Kd, Vd = case.K.to(dev), case.V.to(dev)
+    Kc, Vc = torch.from_numpy(out["K2"]).to(dev), torch.from_numpy(out["V2"]).to(dev)
+    tc = torch.from_numpy(out["tier"]).to(dev)
+    rng = np.random.default_rng(n)
+    up = np.zeros((case.R, case.L, n), np.uint8)
+    for r in range(case.R):
+        for l in range(case.L):
+            sel = rng.choice(np.flatnonzero(case.tier[r][l] != 16), size=k, replace=False)
+            up[r, l, sel[: k // 2]] = 16
+            up[r, l, sel[k // 2:]] = 8
+    uc = skv.skv_counts_from_populations(shape, k // 2, k - k // 2)
+    bb = skv.skv_blob_bytes(shape, uc)
+    ublob = torch.full((case.R * bb,), 0xAB, dtype=torch.uint8, device=dev)
+    skv.skv_pack(shape, Kd, Vd, torch.from_numpy(up).to(dev), uc, ublob, ws)
+    skv.skv_unpack_patch(shape, ublob, bb, uc, Kc, Vc, tc, ws)
+    torch.cuda.synchronize()
+    oc = oracle.Counts(k // 2, k - k // 2, 0, n - k, uc.budget_q4, uc.spent_q4)
+    for r in range(case.R):
+        blob_or = oracle.pack(case.K[r].numpy(), case.V[r].numpy(), up[r], oc, True)
+        assert np.array_equal(ublob[r * bb:(r + 1) * bb].cpu().numpy(), blob_or)
+        K_or, V_or, t_or = oracle.unpack_patch(blob_or, case.K2[r], case.V2[r], case.tier[r])
+        assert np.array_equal(Kc[r].cpu().numpy().view(np.uint16), K_or.view(np.uint16))
+        assert np.array_equal(Vc[r].cpu().numpy().view(np.uint16), V_or.view(np.uint16))
+        assert np.array_equal(tc[r].cpu().numpy(), t_or)
