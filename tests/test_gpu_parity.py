@@ -957,3 +957,47 @@ def test_dense_upgrade_blob_patch_in_fused_and_scan_first_plans(n, k):
         assert np.array_equal(Kc[r].cpu().numpy().view(np.uint16), K_or.view(np.uint16))
         assert np.array_equal(Vc[r].cpu().numpy().view(np.uint16), V_or.view(np.uint16))
         assert np.array_equal(tc[r].cpu().numpy(), t_or)
+
+
+@pytest.mark.parametrize("d,Hkv,Hq,n,b,a4,mode", [(128, 2, 4, 8300, 0.2, 2, 0), (128, 8, 8, 8200, 0.17, 2, 2),
+                                                  (64, 3, 3, 8193, 0.2, 2, 0), (128, 4, 8, 8300, 0.3, 1, 1)])
+def test_next4_tiers_beyond_the_fused_scan_limit(d, Hkv, Hq, n, b, a4, mode):
+    """The NEXT-4 tiers (2-bit, group-wise 2-bit, INT8 hot tier) through the scan-first launch plan (n > 8192): the short
+    cases of the other NEXT-4 tests all take the fused plan."""
+    cfg = skv_synth.Config("next4_long", L=2, Hq=Hq, Hkv=Hkv, d=d, n=n, w=4, R=1, n_sink=2, seed=93, allow_int4=a4)
+    case = Case(cfg, b, with_importance=False, tier_mode=mode)
+    out = gpu_pipeline(case, run_importance=False)
+    assert_bit_exact(case, out)
+
+
+@pytest.mark.parametrize("d,Hkv,n,L,R,k", [(64, 3, 1000, 3, 2, 40), (64, 3, 9000, 16, 4, 300), (256, 1, 2000, 2, 1, 100)])
+def test_sparse_upgrade_blob_generic_rows_and_short_rows(d, Hkv, n, L, R, k):
+    """The sparse plan (live-tile list) on the kernels the other sparse tests do not reach: rows that are not a multiple of
+    256 elements (generic pack / unpack, with and without grid striding) and one-chunk rows."""
+    dev = torch.device("cuda:0")
+    cfg = skv_synth.Config("sparse_gen", L=L, Hq=Hkv, Hkv=Hkv, d=d, n=n, w=4, R=R, n_sink=2, seed=95, allow_int4=True)
+    case = Case(cfg, 0.3, with_importance=False)
+    out = gpu_pipeline(case, run_importance=False)
+    shape = case.shape()
+    ws = torch.empty(skv.skv_workspace_bytes(shape, 0), dtype=torch.uint8, device=dev)
+    Kc, Vc = torch.from_numpy(out["K2"]).to(dev), torch.from_numpy(out["V2"]).to(dev)
+    tc = torch.from_numpy(out["tier"]).to(dev)
+    rng = np.random.default_rng(k)
+    up = np.zeros((R, L, n), np.uint8)
+    for r in range(R):
+        for l in range(L):
+            up[r, l, rng.choice(np.flatnonzero(case.tier[r][l] != 16), size=k, replace=False)] = 16
+    uc = skv.skv_counts_from_populations(shape, k)
+    bb = skv.skv_blob_bytes(shape, uc)
+    ublob = torch.full((R * bb,), 0xAB, dtype=torch.uint8, device=dev)
+    skv.skv_pack(shape, case.K.to(dev), case.V.to(dev), torch.from_numpy(up).to(dev), uc, ublob, ws)
+    skv.skv_unpack_patch(shape, ublob, bb, uc, Kc, Vc, tc, ws)
+    torch.cuda.synchronize()
+    oc = oracle.Counts(k, 0, 0, n - k, uc.budget_q4, uc.spent_q4)
+    for r in range(R):
+        blob_or = oracle.pack(case.K[r].numpy(), case.V[r].numpy(), up[r], oc, True)
+        assert np.array_equal(ublob[r * bb:(r + 1) * bb].cpu().numpy(), blob_or)
+        K_or, V_or, t_or = oracle.unpack_patch(blob_or, case.K2[r], case.V2[r], case.tier[r])
+        assert np.array_equal(Kc[r].cpu().numpy().view(np.uint16), K_or.view(np.uint16))
+        assert np.array_equal(Vc[r].cpu().numpy().view(np.uint16), V_or.view(np.uint16))
+        assert np.array_equal(tc[r].cpu().numpy(), t_or)
