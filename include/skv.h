@@ -108,7 +108,10 @@ typedef enum {
     SKV_ERR_BUDGET_INFEASIBLE = -3, /* protected tokens alone exceed the budget (4P > floor(4bn)) */
     SKV_ERR_BUFFER_TOO_SMALL = -4,  /* blob capacity or workspace */
     SKV_ERR_BAD_BLOB = -5,          /* skv_blob_check: magic / version / dims / offsets / total_bytes mismatch */
-    SKV_ERR_CUDA = -6               /* a CUDA runtime call or kernel launch failed */
+    SKV_ERR_CUDA = -6,              /* a CUDA runtime call or kernel launch failed */
+    SKV_ERR_NOALLOC_LIMIT = -7      /* skv_importance_kvnorm_noalloc only: the problem needs more scratch than the
+                                       SKV_NOALLOC_SCRATCH_BYTES built into the library; use skv_importance_kvnorm
+                                       with a workspace of your own, or split the batch */
 } skv_status;
 
 /* One batch of dense caches.  Strides are in ELEMENTS (fp16) and apply to both K and V; the head
@@ -174,6 +177,39 @@ int skv_importance(const skv_shape *shape, const void *K_dev, const void *Q_dev,
  * times the same decay.  importance_dev: f32 [R][L][n]. */
 int skv_importance_kvnorm(const skv_shape *shape, const void *K_dev, float lambda, float *importance_dev,
                           void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
+
+/* DEVICE.  skv_importance_kvnorm for a caller that cannot allocate device memory: same inputs, same output (bit for
+ * bit -- the same two kernels run), no workspace argument.
+ *
+ * For whom: code embedded in a serving engine (a prefill-side plug-in, a custom op written against the engine's C
+ * interface) that is handed the key cache and the output tensor and nothing else.  The engine's memory pool has
+ * already claimed the GPU's memory, so the plug-in's own cudaMalloc fails (or, on a hot loop, is forbidden because it
+ * stalls the whole device), and the pool is not reachable from C.  Such a caller cannot produce the `workspace_dev`
+ * the other entry points ask for.
+ *
+ * How: the scratch the two KV-norm kernels share -- one f32 per (request, layer, token) plus one f64 per 64 tokens --
+ * is a fixed SKV_NOALLOC_SCRATCH_BYTES (4.25 MiB) array inside the library image.  Every GPU that loads the library
+ * carries it from load to process exit.  The call performs no cudaMalloc / cudaFree and calls nothing that allocates.
+ *
+ * Limit: n_requests * n_layers * n_tokens <= 1 Mi scores is always enough room as long as n_tokens >= 64 per layer
+ * (precisely: 4*R*L*n rounded up to 256, plus 8*R*L*ceil(n/64), must not exceed SKV_NOALLOC_SCRATCH_BYTES) -- one
+ * 32-layer request of 32768 tokens, or four of 8192.  Anything larger returns SKV_ERR_NOALLOC_LIMIT and launches
+ * nothing.  Other argument errors are those of skv_importance_kvnorm.
+ *
+ * First call on each GPU: the entry point asks the CUDA runtime for the array's address on the device that is current
+ * at that moment (this may also be the moment the driver loads the library's device code), and caches it per device
+ * ordinal.  Make that first call during start-up -- with the right device current, and before any stream capture is
+ * begun -- so that later calls are kernel launches only.  The device that is current at every call must be the one
+ * `cuda_stream`, K_dev and importance_dev belong to.  At most 64 device ordinals (SKV_ERR_UNSUPPORTED beyond).
+ *
+ * Sharing: all calls on one GPU use the same array -- from every stream and every host thread.  Two calls whose
+ * kernels can be in flight at the same time (different streams without an event between them) overwrite each other's
+ * partial results and return garbage without any error; order them on one stream or with events.  Nothing needs to be
+ * cleared between calls: each call writes every scratch word it later reads, so the previous call's leftovers (of
+ * whatever shape) are never read. */
+#define SKV_NOALLOC_SCRATCH_BYTES (4352u * 1024u)
+int skv_importance_kvnorm_noalloc(const skv_shape *shape, const void *K_dev, float lambda, float *importance_dev,
+                                  void *cuda_stream);
 
 /* DEVICE.  importance_dev f32 [R][L][n] -> tier_map_dev u8 [R][L][n].  NaN / negative / -0 scores rank as
  * +0; equal scores are ranked by ascending position.  counts_out_host (HOST, nullable) receives the

@@ -7,7 +7,7 @@ the import of any entry point raises.
 
 Entry points mirror the C ABI one to one (see include/skv.h for semantics and citations):
     skv_tier_counts, skv_blob_bytes, skv_workspace_bytes, skv_blob_check,
-    skv_importance, skv_importance_kvnorm, skv_assign_tiers, skv_pack, skv_unpack, skv_unpack_patch,
+    skv_importance, skv_importance_kvnorm, skv_importance_kvnorm_noalloc, skv_assign_tiers, skv_pack, skv_unpack, skv_unpack_patch,
     skv_counts_from_populations, skv_strerror
 """
 import ctypes as C
@@ -23,6 +23,8 @@ SKV_ERR_BUDGET_INFEASIBLE = -3
 SKV_ERR_BUFFER_TOO_SMALL = -4
 SKV_ERR_BAD_BLOB = -5
 SKV_ERR_CUDA = -6
+SKV_ERR_NOALLOC_LIMIT = -7
+SKV_NOALLOC_SCRATCH_BYTES = 4352 * 1024
 
 
 class SkvError(RuntimeError):
@@ -60,7 +62,8 @@ class skv_counts(C.Structure):
 
 EXPORTS = ("skv_tier_counts", "skv_blob_bytes", "skv_workspace_bytes", "skv_blob_check", "skv_importance",
            "skv_importance_kvnorm", "skv_assign_tiers", "skv_pack", "skv_unpack", "skv_unpack_patch",
-           "skv_counts_from_populations", "skv_assign_tiers_counts", "skv_strerror", "skv_version")
+           "skv_counts_from_populations", "skv_assign_tiers_counts", "skv_strerror", "skv_version",
+           "skv_importance_kvnorm_noalloc")
 
 _lib = None
 
@@ -82,6 +85,7 @@ def lib():
         L.skv_blob_check.argtypes = [V, C.c_size_t, P(skv_shape), P(skv_counts)]
         L.skv_importance.argtypes = [P(skv_shape), V, V, C.c_int32, C.c_int32, C.c_float, V, V, C.c_size_t, V]
         L.skv_importance_kvnorm.argtypes = [P(skv_shape), V, C.c_float, V, V, C.c_size_t, V]
+        L.skv_importance_kvnorm_noalloc.argtypes = [P(skv_shape), V, C.c_float, V, V]
         L.skv_assign_tiers.argtypes = [P(skv_shape), P(skv_policy), V, V, P(skv_counts), V, C.c_size_t, V]
         L.skv_assign_tiers_counts.argtypes = [P(skv_shape), P(skv_counts), C.c_int32, C.c_int32, P(C.c_int32), V, V, V, C.c_size_t, V]
         L.skv_pack.argtypes = [P(skv_shape), V, V, V, P(skv_counts), V, C.c_size_t, V, C.c_size_t, V]
@@ -216,6 +220,16 @@ def skv_importance(shape, K, Q, window, importance, workspace, causal=True, lam=
 def skv_importance_kvnorm(shape, K, importance, workspace, lam=0.0, stream=None):
     _check(lib().skv_importance_kvnorm(C.byref(shape), _ptr(K), float(lam), _ptr(importance), _ptr(workspace),
                                        _nbytes(workspace), _stream(stream)), "skv_importance_kvnorm")
+
+
+def skv_importance_kvnorm_noalloc(shape, K, importance, lam=0.0, stream=None):
+    """skv_importance_kvnorm without a workspace: for callers that cannot allocate device memory (code inside an engine
+    whose pool owns the GPU's memory and that receives only the call's tensors).  The scratch is a fixed 4.25 MiB array
+    inside libskv.so, shared by every call on the GPU: raises SkvError(SKV_ERR_NOALLOC_LIMIT) beyond
+    R * L * n ~ 1 Mi scores, and calls that overlap on the GPU (different streams, no event between them) corrupt each
+    other.  The first call on each GPU looks the array up; make it at start-up.  See include/skv.h."""
+    _check(lib().skv_importance_kvnorm_noalloc(C.byref(shape), _ptr(K), float(lam), _ptr(importance), _stream(stream)),
+           "skv_importance_kvnorm_noalloc")
 
 
 def skv_assign_tiers(shape, policy, importance, tier_map, workspace, stream=None):

@@ -16,7 +16,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libskv.so")
-SOURCES = ["skv_host.cu", "skv_scan.cu", "skv_pack.cu", "skv_unpack.cu", "skv_assign.cu", "skv_kvnorm.cu", "skv_importance_tc.cu"]
+SOURCES = ["skv_host.cu", "skv_scan.cu", "skv_pack.cu", "skv_unpack.cu", "skv_assign.cu", "skv_kvnorm.cu", "skv_importance_tc.cu",
+           "skv_noalloc.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "--compiler-options", "-fPIC", "-cudart", "static"]
 

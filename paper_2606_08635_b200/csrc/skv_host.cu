@@ -481,6 +481,7 @@ const char *skv_strerror(int status)
     case SKV_ERR_BUFFER_TOO_SMALL: return "blob capacity or workspace too small";
     case SKV_ERR_BAD_BLOB: return "malformed SKV1 blob";
     case SKV_ERR_CUDA: return "CUDA runtime error";
+    case SKV_ERR_NOALLOC_LIMIT: return "problem exceeds the scratch built into the library (SKV_NOALLOC_SCRATCH_BYTES); pass a workspace to skv_importance_kvnorm instead";
     default: return "unknown status";
     }
 }
