@@ -2,9 +2,9 @@
 
     python -m paper_2606_08635_b200.build [--force] [--verbose] [--define NAME[=VALUE] ...]
 
---define passes -DNAME[=VALUE] to nvcc: the diagnostics switches of csrc/skv_importance_tc.cu (SKV_DIAG_NOEXP,
-SKV_DIAG_NOTMA, SKV_EX2_FMA_PAIRS=k; profiles/r2_importance_ncu.md) -- such a library is for measurements only; rebuild
-without the switch afterwards.
+--define passes -DNAME[=VALUE] to nvcc.  The switches that exist are SKV_EX2_FMA_PAIRS=k (csrc/skv_importance_tc.cu: how
+many of 8 exponential pairs run on the FMA pipe; profiles/r2_importance_ncu.md) and SKV_FUSE_MAX_TOKENS=n
+(csrc/skv_common.cuh) -- such a library is for measurements only; rebuild without the switch afterwards.
 
 The shared library sits next to this file so that it travels with the repository snapshot; it links the
 CUDA runtime statically and needs no GPU to load (nvcc cross-compiles on a CPU-only box).
