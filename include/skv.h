@@ -55,7 +55,7 @@
  *   Slot order inside a tier = ascending token position.  INT4 byte i holds element 2i in the low nibble
  *   and 2i+1 in the high nibble (4-bit two's complement).  Dropped tokens occupy no bytes.
  *
- * 2-bit low tier (NEXT-4; "the INT4 tier could use KIVI-style asymmetric 2-bit quantization", PAPER.md:623): with
+ * 2-bit low tier (NEXT-4; "the INT4 tier could use KIVI-style asymmetric 2-bit quantization", PAPER.md:583): with
  * allow_int4 = 2 the low tier of a blob is coded in 2 bits instead of 4.  Its tier code is 2, header flags = 3,
  * K4/V4 hold four codes per byte (element 4i+k in bits 2k..2k+1 of byte i), SK4/SV4 hold an fp16 (lo, hi) pair per
  * head vector, and the budget runs in EIGHTH-units (8 / 4 / 1 / 0 per token; budget_q4 and spent_q4 are then
@@ -64,14 +64,14 @@
  * rounded once, half to even; y = f16_rn(fma(q, step, lo)).
  *
  * INT8 hot tier (NEXT-4; "the FP16 tier could be further compressed to INT8 (if the model is INT8-safe for high-
- * importance tokens)", PAPER.md:623; reading P21 of DESIGN.md): with tier_mode bit0 (SKV_MODE_HOT_INT8) nothing ships
+ * importance tokens)", PAPER.md:583; reading P21 of DESIGN.md): with tier_mode bit0 (SKV_MODE_HOT_INT8) nothing ships
  * at FP16.  n16 = 0, the protected positions are pinned to -- and paid at -- INT8 (tier code 8), and the greedy ladder
  * of Eq. 14 runs over the costs 1/2 and 1/4 (1/2 and 1/8 with the 2-bit low tier): R = Q - 2P, m = n - P;
  * R >= 2m: all INT8 (every b >= 1/2); m <= R < 2m: n8 = P + (R - m), n4 = 2m - R; R < m: n8 = P, n4 = R, rest dropped;
  * 2-tier: n8 = P + floor(R/2), rest dropped.  Header flags bit3; K16 / V16 are empty.
  *
  * Group-wise 2-bit low tier (NEXT-4; "KIVI partitions keys and values into separate quantization groups",
- * PAPER.md:583; reading P22): with tier_mode bit1 (SKV_MODE_GROUP2, needs allow_int4 = 2) the 2-bit quantiser above
+ * PAPER.md:623; reading P22): with tier_mode bit1 (SKV_MODE_GROUP2, needs allow_int4 = 2) the 2-bit quantiser above
  * runs on every group of 32 consecutive elements of a head vector instead of on the whole vector (token-local, so a
  * token stays self-contained on the wire); SK4 / SV4 hold d_h/32 (lo, hi) pairs per head vector, in element order.
  * Header flags bit4.  The records cost 1 bit per element on top of the 2 bits of code (scale overhead outside b, as
@@ -101,8 +101,10 @@ typedef enum {
                                        blob would fail skv_blob_check); an OUTPUT cache whose layer / request stride
                                        is 0 with more than one layer / request (overlapping writes) */
     SKV_ERR_UNSUPPORTED = -2,       /* head_dim not in {64,128,256}; stride_token/stride_head/stride_layer/
-                                       stride_request not multiples of 8 elements; pointer not 16-B aligned (blob:
-                                       256-B); n_tokens > 2^20 (the slot scan packs three 21-bit counters in a word);
+                                       stride_request not multiples of 8 elements; pointer (cache, queries or
+                                       workspace) not 16-B aligned (blob: 256-B); skv_importance only: stride_layer = 0
+                                       with more than one layer or stride_request = 0 with more than one request (the
+                                       tensor map has no broadcast stride); n_tokens > 2^20 (the slot scan packs three 21-bit counters in a word);
                                        n_layers * n_requests > 65535 (grid dimension of the per-layer kernels);
                                        more than 32 disjoint protected intervals after merging sinks and ranges */
     SKV_ERR_BUDGET_INFEASIBLE = -3, /* protected tokens alone exceed the budget (4P > floor(4bn)) */
@@ -135,7 +137,7 @@ typedef struct {
     int32_t n_ranges;         /* number of protected ranges */
     const int32_t *ranges;    /* HOST, n_ranges x [begin,end) half-open, forced FP16; read during the call only */
     int32_t allow_int4;       /* probe result: 1 = 3-tier, 0 = 2-tier FP16+INT8(+drop);
-                                 2 = 3-tier whose low tier is asymmetric 2-bit (NEXT-4, PAPER.md:623) */
+                                 2 = 3-tier whose low tier is asymmetric 2-bit (NEXT-4, PAPER.md:583) */
     int32_t tier_mode;        /* NEXT-4 bit flags, 0 = the paper's tiers: SKV_MODE_HOT_INT8, SKV_MODE_GROUP2 */
 } skv_policy;
 #define SKV_MODE_HOT_INT8 1   /* the hot tier ships INT8: no FP16 on the wire, protected positions pinned to INT8 (P21) */
@@ -158,7 +160,9 @@ size_t skv_blob_bytes(const skv_shape *shape, const skv_counts *counts);
 
 /* HOST only.  Workspace (DEVICE bytes) sufficient for any entry point on this shape with the given
  * observation window (pass window = 0 if skv_importance is not used).  0 on invalid arguments (dims <= 0; with
- * window > 0 also Hq % Hkv != 0 or window > n) and on shapes skv_importance reports as unsupported. */
+ * window > 0 also Hq % Hkv != 0 or window > n) and on shapes skv_importance reports as unsupported (its work
+ * decomposition -- R*L*Hkv*row-blocks*key-tiles items, R*L*Hq*window query rows -- must fit 32-bit counters).
+ * The workspace passed to any entry point must be 16-byte aligned (SKV_ERR_UNSUPPORTED otherwise). */
 size_t skv_workspace_bytes(const skv_shape *shape, int32_t window);
 
 /* HOST only.  Validates the first 256 bytes of a received blob (HOST memory) against blob_bytes and

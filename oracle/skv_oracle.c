@@ -192,7 +192,7 @@ void orc_importance(int32_t L, int32_t Hq, int32_t Hkv, int32_t d, int64_t n, in
  * prot (nullable, [n]) receives the protected bitmap = [0,s) U ranges.
  * out = {n16, n8, n4, n0, Q, spent}.  Returns 0, -1 invalid argument, -3 infeasible.
  */
-/* mode bit0 (NEXT-4, reading P21 of DESIGN.md; PAPER.md:623 "the FP16 tier could be further compressed to INT8 (if
+/* mode bit0 (NEXT-4, reading P21 of DESIGN.md; PAPER.md:583 "the FP16 tier could be further compressed to INT8 (if
  * the model is INT8-safe for high-importance tokens)"): the HOT tier ships INT8.  Nothing is sent at FP16 any more
  * (n16 = 0), the protected set is pinned to -- and paid at -- INT8, and the greedy ladder of Eq. 14 runs over the two
  * remaining costs 1/2 and 1/4 (1/2 and 1/8 with the 2-bit low tier); b >= 1/2 sends every token at INT8. */
@@ -231,7 +231,7 @@ int orc_tier_counts_mode(int64_t n, double b, int32_t n_sink, int32_t n_ranges, 
         return 0;
     }
     if (allow_int4 == 2) {
-        /* NEXT-4 (PAPER.md:623: "the INT4 tier could use KIVI-style asymmetric 2-bit quantization"): the low tier
+        /* NEXT-4 (PAPER.md:583: "the INT4 tier could use KIVI-style asymmetric 2-bit quantization"): the low tier
          * costs c = 1/8, so the same greedy ladder runs in EIGHTH-units, 8 / 4 / 1 / 0 per token (reading P18). */
         const int64_t Q8 = (int64_t)floor(8.0 * b * (double)n + 1e-6);
         const int64_t m8 = n - P, R8 = Q8 - 8 * P;
@@ -363,7 +363,7 @@ static uint64_t pad256(uint64_t x) { return (x + 255u) / 256u * 256u; }
 
 /* segment order: K16 V16 K8 V8 K4 V4 SK8 SV8 SK4 SV4.  With low_bits = 2 (NEXT-4) the low-tier segments hold four
  * 2-bit codes per byte and a (lo, hi) pair of fp16 records per head vector. */
-/* mode bit1 (NEXT-4, reading P22; PAPER.md:583 "KIVI partitions keys and values into separate quantization groups"):
+/* mode bit1 (NEXT-4, reading P22; PAPER.md:623 "KIVI partitions keys and values into separate quantization groups"):
  * the 2-bit low tier is quantised in GROUPS OF 32 consecutive elements of a head vector (token-local, so a token stays
  * self-contained on the wire) and SK4 / SV4 hold one (lo, hi) pair per group: d/32 pairs per head vector. */
 #define ORC_GROUP2 32
@@ -481,7 +481,7 @@ void orc_dequantize_vector(const int8_t *q, int32_t d, int32_t qmax, uint16_t am
 
 /*
  * NEXT-4: asymmetric 2-bit quantizer for the low tier ("the INT4 tier could use KIVI-style asymmetric 2-bit
- * quantization instead of standard symmetric INT4", PAPER.md:623; reading P19 of DESIGN.md -- the paper gives no
+ * quantization instead of standard symmetric INT4", PAPER.md:583; reading P19 of DESIGN.md -- the paper gives no
  * arithmetic).  One group = one head vector.  lo = min x, hi = max x (fp16 values, stored losslessly as the two
  * 2-byte records; a zero of either sign is stored as +0).  r = fl32(hi - lo), step = fl32(r / 3), inv = fl32(3 / r)
  * (both 0 when r = 0).  q = clamp(rint(fl32(x - lo) * inv), 0, 3), the product exact and rounded once, half to even

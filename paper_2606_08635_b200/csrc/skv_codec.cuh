@@ -271,7 +271,7 @@ __device__ __forceinline__ uint4 dequant_int4(uint32_t w, float scale)
     return make_uint4(o[0], o[1], o[2], o[3]);
 }
 // ------------------------------------------------------------------------------------------------
-// NEXT-4: asymmetric 2-bit low tier (include/skv.h "2-bit quantiser"; PAPER.md:623)
+// NEXT-4: asymmetric 2-bit low tier (include/skv.h "2-bit quantiser"; PAPER.md:583)
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ uint16_t ld_stream2(const void *p)
 {

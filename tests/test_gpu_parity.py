@@ -499,7 +499,7 @@ def test_two_bit_low_tier_parity(d, Hkv, Hq, n, b):
                                              (256, 2, 4, 640, 0.3, 0), (128, 2, 2, 300, 0.7, 1), (64, 8, 8, 96, 0.15, 2),
                                              (256, 1, 2, 129, 0.3, 2)])
 def test_int8_hot_tier_parity(d, Hkv, Hq, n, b, a4):
-    """NEXT-4 (reading P21, PAPER.md:623): the hot tier ships INT8 -- counts (n16 = 0), tier map (sinks and the
+    """NEXT-4 (reading P21, PAPER.md:583): the hot tier ships INT8 -- counts (n16 = 0), tier map (sinks and the
     protected range pinned to code 8), header flags bit3, every blob byte and every dequantised element bit-exact
     against the oracle; 3-tier, 2-tier and 2-bit low tiers, fast and generic rows, b above 1/2 = Uniform INT8."""
     cfg = skv_synth.Config("hot8", L=2, Hq=Hq, Hkv=Hkv, d=d, n=n, w=8, R=2, n_sink=3, ranges=((n - 9, n),), seed=71,
@@ -517,7 +517,7 @@ def test_int8_hot_tier_parity(d, Hkv, Hq, n, b, a4):
                                                (64, 3, 3, 257, 0.2, 2), (256, 2, 4, 640, 0.15, 3), (64, 8, 8, 96, 0.05, 2),
                                                (256, 1, 2, 129, 0.22, 3)])
 def test_group_wise_two_bit_tier_parity(d, Hkv, Hq, n, b, mode):
-    """NEXT-4 (reading P22, PAPER.md:583): the 2-bit low tier quantised in groups of 32 elements, one (lo, hi) record
+    """NEXT-4 (reading P22, PAPER.md:623): the 2-bit low tier quantised in groups of 32 elements, one (lo, hi) record
     per group -- every blob byte (codes and the d/32-times larger record segments) and every dequantised element
     bit-exact against the oracle; fast kernels (4, 2, 1 chunk batches) and generic rows; mode 3 adds the INT8 hot tier."""
     cfg = skv_synth.Config("grp2", L=2, Hq=Hq, Hkv=Hkv, d=d, n=n, w=8, R=2, n_sink=2, seed=81, allow_int4=2)

@@ -662,7 +662,7 @@ def test_upgrade_patch_restores_exact_rows_and_touches_nothing_else():
 
 
 # ----------------------------------------------------------------------------------------------
-# NEXT-4: asymmetric 2-bit low tier (PAPER.md:623)
+# NEXT-4: asymmetric 2-bit low tier (PAPER.md:583)
 # ----------------------------------------------------------------------------------------------
 def test_quantizer2_worked_examples_and_special_cases():
     rows = read_golden(os.path.join(GOLD, "quantizer2_worked.txt"))
@@ -864,7 +864,7 @@ def test_bf16_blob_round_trip_and_fp16_tier_is_a_copy():
 
 
 # ----------------------------------------------------------------------------------------------
-# NEXT-4: INT8 hot tier (reading P21; PAPER.md:623)
+# NEXT-4: INT8 hot tier (reading P21; PAPER.md:583)
 # ----------------------------------------------------------------------------------------------
 def test_hot_int8_counts_golden_and_invariants():
     for n, b, s, rb, re_, a4, n16, n8, n4, n0 in read_golden(os.path.join(GOLD, "hot_int8_counts.txt")):
