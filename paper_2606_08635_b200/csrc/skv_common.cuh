@@ -35,6 +35,8 @@ constexpr int kTileTokens = 32;  // tokens per pack/unpack tile (one ballot word
 #define SKV_FUSE_MAX_TOKENS 8192
 #endif
 constexpr int kFuseMaxTokens = SKV_FUSE_MAX_TOKENS;   // up to this n a pack / unpack CTA counts the tiers below its tile itself (one launch)
+static_assert(kFuseMaxTokens >= kTileTokens && kFuseMaxTokens <= 65535,
+              "self_tile_base (skv_codec.cuh) packs two tier counts into the 16-bit halves of one word");
 
 // Where a pack / unpack CTA gets its tiles and their slot bases from.
 //   tile_base != nullptr: from tile_scan_kernel (skv_scan.cu), [R][L][tiles]; nullptr = "fused": the CTA counts the

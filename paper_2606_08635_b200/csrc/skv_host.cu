@@ -12,7 +12,7 @@
 namespace skv {
 
 // low_bits: 4 = the low tier holds symmetric INT4 codes (two per byte, one fp16 amax record per head vector);
-// 2 = asymmetric 2-bit codes (four per byte, an fp16 (lo, hi) pair per head vector) -- NEXT-4, PAPER.md:623.
+// 2 = asymmetric 2-bit codes (four per byte, an fp16 (lo, hi) pair per head vector) -- NEXT-4, PAPER.md:583.
 // low_group (2-bit tier only): 0 = one record per head vector, 32 = one per group of 32 elements (reading P22).
 Layout make_layout(int L, int Hkv, int D, int64_t n, int64_t n16, int64_t n8, int64_t n4, int low_bits, int low_group)
 {
@@ -64,6 +64,9 @@ static int check_cache(const skv_shape *s, const void *K, const void *V, bool is
     if (((uintptr_t)K & 15) || ((uintptr_t)V & 15)) return SKV_ERR_UNSUPPORTED;
     return SKV_OK;
 }
+
+// every workspace layout starts with 16-byte (uint4 / float2 / double) records: a misaligned base would fault in the kernel
+static bool ws_misaligned(const void *ws) { return ((uintptr_t)ws & 15) != 0; }
 
 static Geom make_geom(const skv_shape *s, const skv_counts *c)
 {
@@ -306,7 +309,10 @@ int skv_importance(const skv_shape *shape, const void *K_dev, const void *Q_dev,
     if (shape->n_q_heads <= 0 || shape->n_q_heads % shape->n_kv_heads) return SKV_ERR_INVALID_ARG;
     if (window < 1 || window > shape->n_tokens) return SKV_ERR_INVALID_ARG;
     if (!(lambda >= 0.0f)) return SKV_ERR_INVALID_ARG;
-    if ((uintptr_t)Q_dev & 15) return SKV_ERR_UNSUPPORTED;
+    if (((uintptr_t)Q_dev & 15) || ws_misaligned(ws)) return SKV_ERR_UNSUPPORTED;
+    // the K tensor map cannot express a broadcast (zero) stride over a dimension that has more than one entry
+    if ((shape->n_layers > 1 && shape->stride_layer == 0) || (shape->n_requests > 1 && shape->stride_request == 0))
+        return SKV_ERR_UNSUPPORTED;
     const Geom g = make_geom(shape, nullptr);
     const size_t need = importance_tc_ws_bytes(g, window);
     if (need == 0) return SKV_ERR_UNSUPPORTED;                            // R*L*Hkv*key-chunk items overflow 32 bits
@@ -322,6 +328,7 @@ int skv_importance_kvnorm(const skv_shape *shape, const void *K_dev, float lambd
     int rc = check_cache(shape, K_dev, K_dev);
     if (rc) return rc;
     if (!importance_dev || !ws || !(lambda >= 0.0f)) return SKV_ERR_INVALID_ARG;
+    if (ws_misaligned(ws)) return SKV_ERR_UNSUPPORTED;
     const Geom g = make_geom(shape, nullptr);
     if (ws_bytes < kvnorm_ws_bytes(g)) return SKV_ERR_BUFFER_TOO_SMALL;
     cudaError_t e = launch_importance_kvnorm(g, (const __half *)K_dev, lambda, importance_dev, ws, (cudaStream_t)cuda_stream);
@@ -335,6 +342,7 @@ static int assign_launch(const skv_shape *shape, const skv_counts &c, const std:
     const size_t key_bytes = (size_t)shape->n_requests * shape->n_layers * shape->n_tokens * sizeof(uint32_t);
     const bool need_ws = (size_t)shape->n_tokens * 4 > 200 * 1024;
     if (need_ws && (!ws || ws_bytes < key_bytes)) return SKV_ERR_BUFFER_TOO_SMALL;
+    if (ws && ws_misaligned(ws)) return SKV_ERR_UNSUPPORTED;
     Intervals iv;
     memset(&iv, 0, sizeof(iv));
     iv.count = (int32_t)prot.size();
@@ -385,7 +393,7 @@ int skv_pack(const skv_shape *shape, const void *K_dev, const void *V_dev, const
     int rc = check_cache(shape, K_dev, V_dev);
     if (rc) return rc;
     if (!tier_map_dev || !blob_dev || !ws || !counts_wire_ok(shape, counts)) return SKV_ERR_INVALID_ARG;
-    if ((uintptr_t)blob_dev & 255) return SKV_ERR_UNSUPPORTED;
+    if (((uintptr_t)blob_dev & 255) || ws_misaligned(ws)) return SKV_ERR_UNSUPPORTED;
     const Geom g = make_geom(shape, counts);
     const Layout lo = make_layout(g.L, g.Hkv, g.D, g.n, g.n16, g.n8, g.n4, g.low_code, g.low_group);
     if (blob_capacity < (size_t)lo.total_bytes * (size_t)g.R) return SKV_ERR_BUFFER_TOO_SMALL;
@@ -424,7 +432,7 @@ static int unpack_impl(const skv_shape *shape, const void *blob_dev, size_t blob
     int rc = check_cache(shape, K_out_dev, V_out_dev, true);
     if (rc) return rc;
     if (!blob_dev || !ws || !counts_wire_ok(shape, counts)) return SKV_ERR_INVALID_ARG;
-    if ((uintptr_t)blob_dev & 255) return SKV_ERR_UNSUPPORTED;
+    if (((uintptr_t)blob_dev & 255) || ws_misaligned(ws)) return SKV_ERR_UNSUPPORTED;
     Geom g = make_geom(shape, counts);
     g.patch = patch;
     const Layout lo = make_layout(g.L, g.Hkv, g.D, g.n, g.n16, g.n8, g.n4, g.low_code, g.low_group);

@@ -32,6 +32,8 @@
 #include <cuda.h>
 #include <string.h>
 
+#include <math.h>
+
 #include <algorithm>
 
 #include "skv_common.cuh"
@@ -60,26 +62,8 @@ struct Params {
     const float *lse2;                  // [R][L][Hq*w]
     float *apart;                       // [R][L][S][n]
     unsigned int *gbar;                 // grid-barrier arrival counter (zeroed on the stream before the launch)
-#ifdef SKV_IMP_TRACE
-    unsigned long long *trace;          // diagnostics build only (never shipped): timestamps, see _TRACE macros below
-#endif
 };
 
-// Diagnostics hooks.  The product build defines none of SKV_IMP_TRACE / SKV_DIAG_*: every macro below expands to nothing.
-// A trace build logs globaltimer stamps of the phase boundaries of every CTA ([grid][16]) and clock64 stamps of the
-// per-tile pipeline events of CTA 0 ([512][8]) into a buffer handed over with skv_debug_set_trace().
-#ifdef SKV_IMP_TRACE
-__device__ unsigned long long *g_trace_ptr;
-__device__ int g_ev_tile;     // tile counter of the one epilogue thread that logs (CTA 0, warp 2, lane 0)
-#define SKV_EPI_LOGGER (blockIdx.x == 0 && threadIdx.x == 64)
-#define SKV_TRACE(slot, who) do { if (who) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); p.trace[blockIdx.x * 16 + (slot)] = t_; } } while (0)
-#define SKV_TRACE_EV(tile, k, who) do { if (blockIdx.x == 0 && (tile) >= 0 && (tile) < 512 && (who)) g_trace_ptr[148 * 16 + (tile) * 8 + (k)] = (unsigned long long)clock64(); } while (0)
-#define SKV_TRACE_ONLY(x) x
-#else
-#define SKV_TRACE(slot, who)
-#define SKV_TRACE_EV(tile, k, who)
-#define SKV_TRACE_ONLY(x)
-#endif
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -280,13 +264,10 @@ __device__ __forceinline__ void stream_tile(uint32_t (&b0)[16], uint32_t (&b1)[1
         uint32_t (&nxt)[16] = (c & 1) ? b0 : b1;
         tmem_wait_ld(cur);
         if (c == NCH - 1) {
-            SKV_TRACE_EV(g_ev_tile, 4, SKV_EPI_LOGGER);          // last chunk of this tile has landed in registers
             release_stage(tempty, astage, lane);
-            SKV_TRACE_EV(g_ev_tile, 6, SKV_EPI_LOGGER);          // stage handed back
             if (++astage == 512 / ACOLS) { astage = 0; aphase ^= 1; }
             if (more) {
                 mbar_wait(tfull + 8 * astage, aphase);
-                SKV_TRACE_EV(g_ev_tile + 1, 3, SKV_EPI_LOGGER);  // next tile's accumulator seen ready
                 tc_fence_after();
                 tmem_ld16_issue(base + astage * ACOLS, nxt);
             }
@@ -399,8 +380,6 @@ __device__ __forceinline__ void rowstats_segment(const Params &p, const Seg &it,
                 }
                 rowstats_chunk<false>(r, 16, sc, m, z);
             });
-        SKV_TRACE_EV(g_ev_tile, 5, SKV_EPI_LOGGER);              // arithmetic of the tile done
-        SKV_TRACE_ONLY(if (SKV_EPI_LOGGER) ++g_ev_tile;)
     }
     for (; k0 < key_end; k0 += kTileKeys) {                               // ---- masked tiles (the last ones of a layer)
         stream_tile<NCH, ACOLS>(bA, bB, base, k0 + kTileKeys < key_end, tfull, tempty, lane, astage, aphase,
@@ -562,7 +541,6 @@ __device__ __forceinline__ void run_pass(const CUtensorMap *tmK, const CUtensorM
     } else if (warp == 1) {
         // ===================== MMA issuer =====================
         if (lane == 0) {
-            SKV_TRACE_ONLY(int ev_tile = 0;)
             const uint32_t idesc = (PASS == 1) ? umma_idesc(128, kTileKeys, p.g.bf16) : umma_idesc(128, p.qrows, p.g.bf16);
             for (long long u = ubeg; u < uend;) {
                 const Seg it = seg_at(p, u, uend);
@@ -570,9 +548,7 @@ __device__ __forceinline__ void run_pass(const CUtensorMap *tmK, const CUtensorM
                 mbar_wait_ctrl(sm.qfull, cu.qphase); cu.qphase ^= 1;
                 for (int t = it.t0; t < it.t1; ++t) {
                     mbar_wait_ctrl(sm.tempty + 8 * cu.astage, cu.aphase ^ 1);
-                    SKV_TRACE_EV(ev_tile, 0, PASS == 1);
                     mbar_wait_ctrl(sm.kfull + 8 * cu.kstage, cu.kphase);
-                    SKV_TRACE_EV(ev_tile, 1, PASS == 1);
                     tc_fence_after();
                     const uint32_t kt = sm.sK + cu.kstage * C::K_BYTES;
                     const uint32_t acc = tmem + cu.astage * ACOLS;
@@ -595,8 +571,6 @@ __device__ __forceinline__ void run_pass(const CUtensorMap *tmK, const CUtensorM
                     }
                     umma_commit(sm.kempty + 8 * cu.kstage);    // smem stage free once these MMAs have read it
                     umma_commit(sm.tfull + 8 * cu.astage);     // accumulator ready for the epilogue
-                    SKV_TRACE_EV(ev_tile, 2, PASS == 1);
-                    SKV_TRACE_ONLY(++ev_tile;)
                     if (++cu.kstage == C::STAGES) { cu.kstage = 0; cu.kphase ^= 1; }
                     if (++cu.astage == ASTAGES) { cu.astage = 0; cu.aphase ^= 1; }
                 }
@@ -694,15 +668,9 @@ imp_fused_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant_
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
     Cursors cu = {0, 0, 0, 0, 0, 0, 0};
-    SKV_TRACE_ONLY(if (SKV_EPI_LOGGER) g_ev_tile = 0;)
-    SKV_TRACE_ONLY(if (blockIdx.x == 0 && threadIdx.x == 0) g_trace_ptr = p.trace;)
-    SKV_TRACE_ONLY(__syncthreads();)
-    SKV_TRACE(0, threadIdx.x == 0);
 
     run_pass<D, 1, VA>(&tmK, &tmQ, p, sm, tmem, cu, warp, lane);
-    SKV_TRACE(1, threadIdx.x == kThreads - 1);
     grid_barrier(p.gbar, gridDim.x);
-    SKV_TRACE(2, threadIdx.x == 0);
 
     {   // lse2[row] = m* + log2(sum_c z_c 2^(m_c - m*)) over the (reference exponent, sum) pairs of the row's pieces
         const int64_t rows = (int64_t)p.g.R * p.g.L * p.g.Hq * p.w;
@@ -723,14 +691,10 @@ imp_fused_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant_
             const_cast<float *>(p.lse2)[row] = m + log2f(z);
         }
     }
-    SKV_TRACE(3, threadIdx.x == 0);
     grid_barrier(p.gbar, 2 * gridDim.x);
-    SKV_TRACE(4, threadIdx.x == 0);
 
     run_pass<D, 2, VC>(&tmK, &tmQ, p, sm, tmem, cu, warp, lane);
-    SKV_TRACE(5, threadIdx.x == kThreads - 1);
     grid_barrier(p.gbar, 3 * gridDim.x);
-    SKV_TRACE(6, threadIdx.x == 0);
 
     {   // importance = (sum over (KV head, row block) partials in a fixed order) / (Hq w) * exp(-lambda (n-1-j))
         const int64_t total = (int64_t)p.g.R * p.g.L * p.g.n;
@@ -744,7 +708,6 @@ imp_fused_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant_
             importance[i] = sum * norm * expf(-lambda * (float)(p.g.n - 1 - j));
         }
     }
-    SKV_TRACE(7, threadIdx.x == 0);
     tc_fence_before();
     __syncthreads();
     if (warp == 1) {
@@ -772,10 +735,6 @@ static EncodeTiledFn get_encode_fn()
     return (EncodeTiledFn)fn;
 }
 
-#ifdef SKV_IMP_TRACE
-static unsigned long long *g_host_trace = nullptr;      // diagnostics build only: device buffer of (148 * 16 + 512 * 8) u64
-extern "C" void skv_debug_set_trace(void *dev_ptr) { g_host_trace = reinterpret_cast<unsigned long long *>(dev_ptr); }
-#endif
 
 struct TcPlan {
     int QROWS_MAX, RB, MB, qrows, halves, S, T, grid, pmax;
@@ -816,7 +775,17 @@ static TcPlan tc_plan(const Geom &g, int w)
 size_t importance_tc_ws_bytes(const Geom &g, int window)
 {
     if (g.Hkv <= 0 || g.Hq < g.Hkv || g.Hq % g.Hkv || window <= 0) return 0;
+    // The kernel keeps work-item indices, tile rows and the TMA coordinate (r*L + l)*Hkv + g in 32-bit ints, and the
+    // byte counts below must not wrap: refuse (0) what does not fit.  Checked in double before any integer product.
+    const double M = (double)(g.Hq / g.Hkv) * (double)window;
+    const double RB = ceil(M / ((g.D == 256) ? 128.0 : 256.0));
+    const double T = ceil((double)g.n / (double)tc::kTileKeys);
+    const double U = (double)g.R * (double)g.L * (double)g.Hkv * RB * T;
+    const double rows = (double)g.R * (double)g.L * (double)g.Hq * (double)window;
+    if (U > 2147483647.0 || rows > 2147483647.0 || M > 2147483647.0) return 0;
+    if ((double)g.R * (double)g.L * (double)g.Hkv * RB * (double)g.n * 4.0 > 9.0e18) return 0;      // apart_bytes
     const TcPlan t = tc_plan(g, window);
+    if (rows * (double)t.pmax * 8.0 > 9.0e18) return 0;                                               // partial_bytes
     return t.partial_bytes + t.lse_bytes + t.apart_bytes + t.bar_bytes;
 }
 
@@ -893,9 +862,6 @@ cudaError_t launch_importance_tc(const Geom &g, const __half *K, const __half *Q
     p.apart = reinterpret_cast<float *>(w8 + t.partial_bytes + t.lse_bytes);
     p.gbar = reinterpret_cast<unsigned int *>(w8 + t.partial_bytes + t.lse_bytes + t.apart_bytes);
     if (cudaMemsetAsync(p.gbar, 0, sizeof(unsigned int), s) != cudaSuccess) return cudaGetLastError();
-#ifdef SKV_IMP_TRACE
-    p.trace = g_host_trace;
-#endif
 
     int dev = 0, sms = kPlanSMs;
     cudaGetDevice(&dev);

@@ -159,6 +159,41 @@ def test_argument_errors():
     assert rc == skv.SKV_ERR_INVALID_ARG            # null importance
 
 
+def test_workspace_alignment_broadcast_strides_and_importance_plan_limits():
+    """Round-2 review items: a workspace that is not 16-byte aligned, a zero (broadcast) layer / request stride handed to
+    skv_importance, and an importance work decomposition that does not fit 32-bit counters all come back as a status
+    code before anything is launched (no GPU needed)."""
+    import ctypes as C
+    L = skv.lib()
+    shape = skv.make_shape(2, 4, 2, 128, 100)
+    c = skv.skv_tier_counts(shape, skv.make_policy(0.5, 4))
+    big = 1 << 40
+    for ws in (256 + 8, 256 + 4, 257):
+        assert L.skv_pack(C.byref(shape), 256, 256, 256, C.byref(c), 256, big, ws, big, None) == skv.SKV_ERR_UNSUPPORTED
+        bb = skv.skv_blob_bytes(shape, c)
+        assert L.skv_unpack(C.byref(shape), 256, bb, C.byref(c), 256, 256, None, ws, big, None) == skv.SKV_ERR_UNSUPPORTED
+        assert L.skv_unpack_patch(C.byref(shape), 256, bb, C.byref(c), 256, 256, None, ws, big, None) == skv.SKV_ERR_UNSUPPORTED
+        assert L.skv_importance(C.byref(shape), 256, 256, 8, 1, 0.0, 256, ws, big, None) == skv.SKV_ERR_UNSUPPORTED
+        assert L.skv_importance_kvnorm(C.byref(shape), 256, 0.0, 256, ws, big, None) == skv.SKV_ERR_UNSUPPORTED
+        pol = skv.make_policy(0.5, 4)
+        assert L.skv_assign_tiers(C.byref(shape), C.byref(pol), 256, 256, None, ws, big, None) == skv.SKV_ERR_UNSUPPORTED
+    # broadcast strides: fine for the other readers of K, not expressible in the importance kernel's tensor map
+    for field in ("stride_layer", "stride_request"):
+        sb = skv.make_shape(2, 4, 2, 128, 100, 2)
+        setattr(sb, field, 0)
+        assert L.skv_importance(C.byref(sb), 256, 256, 8, 1, 0.0, 256, 256, big, None) == skv.SKV_ERR_UNSUPPORTED
+    one = skv.make_shape(1, 4, 2, 128, 100, 1)
+    one.stride_layer = one.stride_request = 0                       # a single layer / request: the stride is never used
+    assert skv.skv_workspace_bytes(one, 8) > 0
+    # 65535 layers x 8 KV heads x 8192 key tiles = 4.3e9 work items: more than a 32-bit counter holds
+    huge = skv.make_shape(65535, 8, 8, 128, 1 << 20, 1)
+    assert skv.skv_workspace_bytes(huge, 0) > 0
+    assert skv.skv_workspace_bytes(huge, 1) == 0
+    assert L.skv_importance(C.byref(huge), 256, 256, 1, 1, 0.0, 256, 256, big, None) == skv.SKV_ERR_UNSUPPORTED
+    ok = skv.make_shape(65535, 8, 8, 128, 1 << 14, 1)               # 65535 x 8 x 128 tiles = 6.7e7 items: fits
+    assert skv.skv_workspace_bytes(ok, 1) > 0
+
+
 def test_blob_check_accepts_oracle_blob_and_rejects_corruption():
     L_, n, Hkv, d = 2, 50, 2, 64
     rng = np.random.default_rng(1)
