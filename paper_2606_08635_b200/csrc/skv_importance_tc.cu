@@ -519,6 +519,7 @@ __device__ __forceinline__ void run_pass(const CUtensorMap *tmK, const CUtensorM
     if (warp == 0) {
         // ===================== TMA producer =====================
         if (lane == 0) {
+            const int kd0 = p.kdim[0], kd1 = p.kdim[1], kd2 = p.kdim[2];
             for (long long u = ubeg; u < uend;) {
                 const Seg it = seg_at(p, u, uend);
                 u += it.t1 - it.t0;
@@ -529,10 +530,13 @@ __device__ __forceinline__ void run_pass(const CUtensorMap *tmK, const CUtensorM
                 for (int t = it.t0; t < it.t1; ++t) {
                     mbar_wait_ctrl(sm.kempty + 8 * cu.kstage, cu.kphase ^ 1);
                     mbar_expect_tx(sm.kfull + 8 * cu.kstage, (uint32_t)C::K_BYTES);
-                    int c[5]; c[0] = 0;
-                    c[p.kdim[0]] = it.g; c[p.kdim[1]] = t * kTileKeys; c[p.kdim[2]] = it.l; c[p.kdim[3]] = it.r;
+                    // coordinate of tensor-map dimension i = the one of (head, token, layer, request) whose kdim is i;
+                    // selects, not an array indexed by kdim (that array lived in local memory: ~100 STL / LDL per kernel)
+                    const int tk = t * kTileKeys;
+                    auto coord = [&](int i) { return kd0 == i ? it.g : kd1 == i ? tk : kd2 == i ? it.l : it.r; };
+                    const int c1 = coord(1), c2 = coord(2), c3 = coord(3), c4 = coord(4);
                     for (int kb = 0; kb < C::KB; ++kb)
-                        tma_load_5d(sm.sK + cu.kstage * C::K_BYTES + kb * C::K_KB_STRIDE, tmK, sm.kfull + 8 * cu.kstage, kb * 64, c[1], c[2], c[3], c[4]);
+                        tma_load_5d(sm.sK + cu.kstage * C::K_BYTES + kb * C::K_KB_STRIDE, tmK, sm.kfull + 8 * cu.kstage, kb * 64, c1, c2, c3, c4);
                     if (++cu.kstage == C::STAGES) { cu.kstage = 0; cu.kphase ^= 1; }
                 }
             }
