@@ -72,21 +72,42 @@ def measured_peak():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
 
 
-TRAFFIC_FILE = "profiles/r2_traffic.csv"
+TRAFFIC_FILE = "profiles/r3_traffic.csv"
+CODEC_SOURCES = ("paper_2606_08635_b200/csrc/skv_pack.cu", "paper_2606_08635_b200/csrc/skv_unpack.cu",
+                 "paper_2606_08635_b200/csrc/skv_codec.cuh")
 
 
-def ncu_traffic(workload, b, R, kernel):
+def codec_sources_hash(root=None):
+    """`git hash-object` (sha1 of "blob <len>\0" + contents) of the three files that make the pack / unpack kernels,
+    first 10 hex digits each, joined by '+': the revision stamp of a recorded traffic row.  Computed with hashlib so
+    that it also works on the GPU box, where the snapshot has no .git."""
+    import hashlib
+    out = []
+    for rel in CODEC_SOURCES:
+        with open(os.path.join(root or ROOT, rel), "rb") as f:
+            data = f.read()
+        out.append(hashlib.sha1(b"blob %d\0" % len(data) + data).hexdigest()[:10])
+    return "+".join(out)
+
+
+def ncu_traffic(workload, b, R, kernel, path=None, root=None):
     """(dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` ("pack" | "unpack"), provenance) as
-    captured by `ncu --set full` and RECORDED in profiles/r2_traffic.csv
-    (workload,budget,n_requests,kernel,dram_bytes,captured) -- not measured in this run; `captured` names the date
-    and source revision of the capture.  (None, None) when no capture of this exact workload is on file."""
+    captured by `ncu --set full` and RECORDED in profiles/r3_traffic.csv
+    (workload,budget,n_requests,kernel,dram_bytes,codec_hash,captured) -- not measured in this run.  A row counts only
+    if its codec_hash equals codec_sources_hash() of the tree that is running: a capture of other kernel sources is
+    refused, (None, "stale: ...").  (None, None) when no capture of this exact workload is on file."""
     try:
-        with open(os.path.join(ROOT, TRAFFIC_FILE)) as f:
+        with open(path or os.path.join(ROOT, TRAFFIC_FILE)) as f:
             for ln in f:
-                fld = [x.strip() for x in ln.split(",")]
-                if len(fld) >= 5 and fld[0] == workload and fld[3] == kernel:
+                if ln.lstrip().startswith("#"):
+                    continue
+                fld = [x.strip() for x in ln.split(",", 6)]
+                if len(fld) >= 6 and fld[0] == workload and fld[3] == kernel:
                     if abs(float(fld[1]) - b) < 1e-9 and int(fld[2]) == R:
-                        return float(fld[4]), (fld[5] if len(fld) > 5 else None)
+                        have = codec_sources_hash(root)
+                        if fld[5] != have:
+                            return None, f"stale: the row was captured on codec sources {fld[5]}, the tree has {have}"
+                        return float(fld[4]), (fld[6] if len(fld) > 6 else None)
     except Exception:
         pass
     return None, None
@@ -117,13 +138,13 @@ def l2_note(cfg, R, blob_bytes, flush):
             f"(> 30x the 126 MB L2) between two uses of a line; no flush needed")
 
 
-def config_json(cfg, b, R, extra=None, l2=None):
+def config_json(cfg, b, R, extra=None):
+    """The workload, identical for both arms (the driver compares the two `config` objects): nothing arm-specific goes
+    in here -- the L2 note of a line is its sibling key `l2`."""
     c = {"workload": f"{cfg.name}: {cfg.L} layers, {cfg.Hq} q heads / {cfg.Hkv} KV heads, head_dim {cfg.d}, "
                      f"{cfg.n} tokens, batch of {R} requests, window {cfg.w}, b={b}, "
                      f"{'3-tier FP16/INT8/INT4' if cfg.allow_int4 else '2-tier FP16+INT8'}, {cfg.n_sink} sinks",
          "budget": b, "n_requests": R, "bytes_fp16_per_request": cfg.bytes_fp16}
-    if l2 is not None:
-        c["l2"] = l2
     if extra:
         c.update(extra)
     return c
@@ -484,8 +505,10 @@ def run_sweep(args, main_prob, dev, peak, steps):
 
 
 def run_next_rows(prob, steps):
-    """SURVEY.md 8(f) rows at the same workload, outside the timed step: NEXT-1 KV-norm fallback score (reads K once)
-    and NEXT-3 cold-tier upgrade (FP16 upgrade blob of 1024 tokens per layer: skv_pack + skv_unpack_patch)."""
+    """SURVEY.md 8(f) rows at the same workload, outside the timed step: NEXT-1 KV-norm fallback score (reads K once),
+    NEXT-3 cold-tier upgrade (FP16 upgrade blob of 1024 tokens per layer: skv_pack + skv_unpack_patch) and every NEXT-4
+    variant (2-bit low tier, group-wise 2-bit, INT8 hot tier, bfloat16 caches), each as pack + unpack on algorithmic
+    bytes (main() adds frac_of_hbm_peak)."""
     import torch
     skv, cfg, R = prob.skv, prob.cfg, prob.R
     ev = lambda: torch.cuda.Event(enable_timing=True)
@@ -537,6 +560,28 @@ def run_next_rows(prob, steps):
                                "ms_pack_plus_unpack": ms, "GBps": moved2 / (ms * 1e-3) / 1e9,
                                "GBps_of_fp16_kv": cfg.bytes_fp16 * R / (ms * 1e-3) / 1e9}
     del blob2
+    # NEXT-4: the group-wise 2-bit low tier (reading P22) at the same b = 0.2, and the INT8 hot tier
+    # (reading P21: nothing ships at FP16) at b = 0.4 (INT8 + low-tier mix; b >= 0.5 would be all INT8)
+    for key, bx, polx in (
+            ("group2_low_tier", 0.2, skv.make_policy(0.2, cfg.n_sink, cfg.ranges, 2, tier_mode=skv.SKV_MODE_GROUP2)),
+            ("hot_int8", 0.4, skv.make_policy(0.4, cfg.n_sink, cfg.ranges, cfg.allow_int4, tier_mode=skv.SKV_MODE_HOT_INT8))):
+        cx = skv.skv_assign_tiers(prob.shape, polx, prob.I, prob.tier, prob.ws)
+        bbx = skv.skv_blob_bytes(prob.shape, cx)
+        blobx = torch.empty((R, bbx), dtype=torch.uint8, device=prob.dev)
+        def oncex():
+            skv.skv_pack(prob.shape, prob.K, prob.V, prob.tier, cx, blobx, prob.ws)
+            skv.skv_unpack(prob.shape, blobx, bbx, cx, prob.Ko, prob.Vo, prob.tier_out, prob.ws)
+        oncex()
+        a.record()
+        for _ in range(steps):
+            oncex()
+        b_.record(); torch.cuda.synchronize()
+        ms = a.elapsed_time(b_) / steps
+        movedx = 2 * (cfg.bytes_fp16 * R + R * bbx + cfg.L * cfg.n * R)
+        out[key] = {"budget": bx, "counts": list(cx.as_tuple()), "blob_bytes_per_request": bbx,
+                    "ms_pack_plus_unpack": ms, "GBps": movedx / (ms * 1e-3) / 1e9,
+                    "GBps_of_fp16_kv": cfg.bytes_fp16 * R / (ms * 1e-3) / 1e9}
+        del blobx
     # NEXT-4: bfloat16 caches (same values rounded to bf16), the headline policy (b of the run), pack + unpack
     for r in range(R):
         prob.Ko[r].copy_(prob.K[r].float().to(torch.bfloat16).view(torch.float16))     # Ko/Vo reused as bf16 inputs
@@ -559,6 +604,56 @@ def run_next_rows(prob, steps):
     out["bf16_caches"] = {"budget": prob.b, "ms_pack_plus_unpack": ms, "GBps": moved3 / (ms * 1e-3) / 1e9,
                           "GBps_of_16bit_kv": cfg.bytes_fp16 * R / (ms * 1e-3) / 1e9}
     return out
+
+
+def pcie_duplex_ms(h2d_bytes, d2h_bytes, h_src, h_dst, dev, chunk=256 * 2**20, reps=3):
+    """The denominator of the e2e leg, measured in the same run: the time to move exactly `h2d_bytes` host -> device and
+    `d2h_bytes` device -> host, both directions at once on two streams, from / to the same pinned buffers, with no
+    kernel anywhere -- what the link alone would take for the step's traffic.  Copies go in `chunk`-byte pieces that
+    cycle through the pinned tensors `h_src` / `h_dst` and one device staging buffer per direction."""
+    import torch
+    srcs = [t.view(torch.uint8).reshape(-1) for t in h_src]
+    dsts = [t.view(torch.uint8).reshape(-1) for t in h_dst]
+    chunk = int(min(chunk, min(t.numel() for t in srcs + dsts)))
+    d_in = torch.empty((chunk,), dtype=torch.uint8, device=dev)
+    d_out = torch.zeros((chunk,), dtype=torch.uint8, device=dev)
+    s_in, s_out = torch.cuda.Stream(device=dev), torch.cuda.Stream(device=dev)
+
+    def pieces(total, bufs):
+        left, i = int(total), 0
+        while left > 0:
+            buf = bufs[i % len(bufs)]
+            per = buf.numel() // chunk
+            for k in range(per):
+                if left <= 0:
+                    break
+                m = min(chunk, left)
+                yield buf[k * chunk:k * chunk + m], m
+                left -= m
+            i += 1
+
+    def once():
+        with torch.cuda.stream(s_in):
+            for h, m in pieces(h2d_bytes, srcs):
+                d_in[:m].copy_(h, non_blocking=True)
+        with torch.cuda.stream(s_out):
+            for h, m in pieces(d2h_bytes, dsts):
+                h.copy_(d_out[:m], non_blocking=True)
+
+    once()
+    torch.cuda.synchronize()
+    best = float("inf")
+    for _ in range(reps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        cur = torch.cuda.current_stream()
+        e0.record(cur)
+        s_in.wait_event(e0); s_out.wait_event(e0)
+        once()
+        cur.wait_stream(s_in); cur.wait_stream(s_out)
+        e1.record(cur)
+        torch.cuda.synchronize()
+        best = min(best, e0.elapsed_time(e1))
+    return best
 
 
 def run_e2e(cfg, b, R, dev, steps, warmup, chunk_layers=4, depth=3, host_requests=2):
@@ -606,6 +701,7 @@ def run_e2e(cfg, b, R, dev, steps, warmup, chunk_layers=4, depth=3, host_request
     out = {"ms_per_step": ms, "steps": steps, "h2d": R * h2d_req, "d2h": R * d2h_req, "layers_per_chunk": lpc, "depth": depth,
            "host_requests": Rh}
     del pipe
+    out["pcie_duplex_ms"] = pcie_duplex_ms(R * h2d_req, R * d2h_req, (hK, hV), (hKo, hVo), dev)
 
     # context 1: no overlap -- one request at a time, one stream, whole-request blobs
     shape = skv.make_shape(L, cfg.Hq, cfg.Hkv, cfg.d, cfg.n, 1)
@@ -672,7 +768,8 @@ def cpu_model():
 
 def oracle_sample(cfg, b, target_seconds):
     """SURVEY.md 8(d) 'Oracle timing': the oracle as it stands on a bounded sample of the workload (the first layers of
-    request 0; same generator, same bytes as the CUDA arm's request 0 on the CPU generator), about `target_seconds` of
+    request 0, made by the CPU generator of skv_synth: the same distribution as the CUDA arm's device-generated request
+    0, not the same bytes -- the `sample` string says so), about `target_seconds` of
     CPU work in total:
       (b) pack + unpack with OpenMP over layers on every available core -- the headline `value`;
       (a) pack + unpack single-threaded on ONE layer;
@@ -727,7 +824,8 @@ def oracle_sample(cfg, b, target_seconds):
         nbytes, tp, tu = run(layers)
     gbs = nbytes / (tp + tu) / 1e9
     sample = (f"oracle pack+unpack of {layers} of {cfg.L} layers of 1 request ({nbytes / 2**20:.0f} MiB FP16 KV), "
-              f"tier map from a synthetic importance vector, OpenMP over layers")
+              f"tier map from a synthetic importance vector, OpenMP over layers; CPU-generator bytes (skv_synth on the host: "
+              f"the same distribution as the CUDA arm's device-generated request 0, not the same bytes)")
     return {"value": gbs, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample, "cpu_model": cpu_model(),
             "seconds": tp + tu, "pack_s": tp, "unpack_s": tu,
             "single_thread": {"value": nb1 / (tp1 + tu1) / 1e9, "unit": UNIT, "cores": 1, "pack_s": tp1, "unpack_s": tu1,
@@ -781,11 +879,11 @@ def run_reference(args, cfg, b, R):
     mean = sum(secs) / len(secs)
     value = nbytes / mean / 1e9
     sample = (f"oracle pack+unpack of {layers} of {cfg.L} layers of 1 request ({nbytes / 2**20:.0f} MiB FP16 KV) per step, "
-              f"tier map from a synthetic importance vector, OpenMP over layers")
+              f"tier map from a synthetic importance vector, OpenMP over layers; CPU-generator bytes (skv_synth on the host)")
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * mean, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f16 -> i8/i4 codes (exact products, f32 scales)",
-            "data": "synthetic", "config": config_json(cfg, b, R, l2="CPU arm: not applicable"),
+            "data": "synthetic", "config": config_json(cfg, b, R), "l2": "CPU arm: not applicable",
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample,
                              "cpu_model": cpu_model()},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -832,7 +930,7 @@ def main():
     next_rows = None if args.no_next else run_next_rows(prob, min(K, 10))
     e2e = None
     if not args.no_e2e:
-        r = run_e2e(cfg, b, R, dev, steps=min(K, 3), warmup=1, chunk_layers=args.e2e_chunk_layers, depth=args.e2e_depth,
+        r = run_e2e(cfg, b, R, dev, steps=min(K, 10), warmup=1, chunk_layers=args.e2e_chunk_layers, depth=args.e2e_depth,
                     host_requests=1 if world > 1 else 2)
         red2, _ = aggregate_over_ranks([r["ms_per_step"]], bytes_local, device=dev)
         e2e = {"value": bytes_all / (red2[0] * 1e-3) / 1e9, "unit": UNIT,
@@ -842,7 +940,11 @@ def main():
                "pinned_host_requests": r["host_requests"], "rank0_cpu_affinity": (len(numa) if numa else None),
                "sequential_ms_per_request": r["sequential_ms_per_request"],
                "raw_fp16_hop_ms_per_request": r["raw_fp16_hop_ms_per_request"],
-               "blob_hop_ms_per_request": r["blob_hop_ms_per_request"]}
+               "blob_hop_ms_per_request": r["blob_hop_ms_per_request"],
+               "pcie_duplex_ms": r["pcie_duplex_ms"], "frac_of_pcie": r["pcie_duplex_ms"] / red2[0],
+               "pcie_note": "pcie_duplex_ms = the step's H2D and D2H byte counts copied both ways at once from / to the same "
+                            "pinned buffers on two streams with no kernels, best of 3, this run, this rank; frac_of_pcie = "
+                            "that time / the e2e step time (1.0 = the path is hidden entirely behind the link)"}
 
     if rank != 0:
         dist_finish()
@@ -859,7 +961,7 @@ def main():
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f16 -> i8/i4 codes (quantiser arithmetic in f32); importance f16 x f16 -> f32",
-        "data": "synthetic", "config": config_json(cfg, b, R, l2=l2_note(cfg, R, prob.blob_bytes, flush)),
+        "data": "synthetic", "config": config_json(cfg, b, R), "l2": l2_note(cfg, R, prob.blob_bytes, flush),
         "stages_ms": {"importance": ms_imp, "assign": ms_asg, "pack": ms_pack, "unpack": ms_unpack},
         "stages_ms_min": dict(zip(STAGES, stage_min)),
         "ms_per_request_on_gpu": ms_step / R,
@@ -870,7 +972,7 @@ def main():
                      "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": achieved / peak,
                      "algorithmic_bytes_per_launch": alg[dom], "avg_launch_ms": dom_ms,
                      "traffic": traffic, "traffic_source": (f"recorded ncu --set full capture, {TRAFFIC_FILE}: {traffic_src}"
-                                                            if traffic is not None else None),
+                                                            if traffic is not None else traffic_src),
                      "other": {k: {"achieved": alg[k] / (m * 1e-3) / 1e9, "frac": alg[k] / (m * 1e-3) / 1e9 / peak}
                                for k, m in (("pack", ms_pack), ("unpack", ms_unpack))},
                      "frac_of_nominal_8TBs": achieved / 8000.0},

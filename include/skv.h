@@ -30,7 +30,9 @@
  *   - Every entry returns SKV_OK (0) or a negative skv_status and launches nothing on error.
  *   - The library keeps no mutable global state and is re-entrant.  (Two process-wide constants are set idempotently:
  *     the driver entry point of the tensor-map encoder is looked up once and cached, and kernels that need more than
- *     48 KiB of dynamic shared memory always request the same fixed maximum.)
+ *     48 KiB of dynamic shared memory always request the same fixed maximum.)  The one exception is
+ *     skv_importance_kvnorm_noalloc, the entry point for callers that cannot allocate: its scratch is a fixed array
+ *     inside the library that all its calls on a GPU share (see its declaration for the rules that follow from that).
  *   - fp16 = IEEE binary16.  K/V inputs must be finite (NaN/Inf is undefined behaviour).
  *   - With skv_shape.dtype = SKV_BF16 every "fp16" below reads bfloat16 (caches, queries, amax / (lo, hi) records,
  *     dequantised output); the byte model is unchanged (2 bytes per element).  Only difference in the arithmetic: a

@@ -57,6 +57,41 @@ def test_recorded_ncu_traffic_is_on_file_for_the_bench_workload():
         assert traffic is not None and abs(traffic - alg) / alg < 0.01     # no re-reads: DRAM traffic = algorithmic bytes
         assert "rev" in source                                             # provenance of the capture travels with the number
     assert bench.ncu_traffic("C5", 0.45, 4, "pack") == (None, None)        # no capture of that workload: null, not a guess
+    for w in ("C2", "C3", "C4"):                                           # the single-request configs of the sweep are on file too
+        for kernel in ("pack", "unpack"):
+            assert bench.ncu_traffic(w, 0.5, 1, kernel)[0] is not None, (w, kernel)
+
+
+def test_recorded_ncu_traffic_is_refused_when_the_kernel_sources_changed(tmp_path):
+    """A traffic row is stamped with `git hash-object` of the three files that make the pack / unpack kernels; bench.py
+    uses it only while those files are the ones that were profiled."""
+    import hashlib
+    import subprocess
+    have = bench.codec_sources_hash()
+    assert len(have.split("+")) == 3 and all(len(h) == 10 for h in have.split("+"))
+    try:                                                                   # the stamp really is git's blob hash
+        out = subprocess.run(["git", "hash-object", os.path.join(ROOT, bench.CODEC_SOURCES[0])], capture_output=True, text=True, check=True)
+        assert out.stdout.strip()[:10] == have.split("+")[0]
+    except (OSError, subprocess.CalledProcessError):
+        pass                                                               # no git on this box: the hashlib form stands alone
+    csv = tmp_path / "traffic.csv"
+    csv.write_text("# comment\n"
+                   f"C5,0.5,4,pack,100,{have},2026-01-01 rev abc (x<1; 2>)\n"
+                   "C5,0.5,4,unpack,200,0000000000+0000000000+0000000000,2026-01-01 rev old\n")
+    assert bench.ncu_traffic("C5", 0.5, 4, "pack", path=str(csv)) == (100.0, "2026-01-01 rev abc (x<1; 2>)")
+    traffic, why = bench.ncu_traffic("C5", 0.5, 4, "unpack", path=str(csv))
+    assert traffic is None and why.startswith("stale")
+    # the same good row is refused by a tree whose codec differs by one byte
+    root = tmp_path / "tree"
+    for rel in bench.CODEC_SOURCES:
+        dst = root / rel
+        dst.parent.mkdir(parents=True, exist_ok=True)
+        dst.write_bytes(open(os.path.join(ROOT, rel), "rb").read() + (b" " if rel.endswith("skv_codec.cuh") else b""))
+    traffic, why = bench.ncu_traffic("C5", 0.5, 4, "pack", path=str(csv), root=str(root))
+    assert traffic is None and why.startswith("stale")
+    # every row of the committed file carries the stamp of the committed sources
+    rows = [ln for ln in open(os.path.join(ROOT, bench.TRAFFIC_FILE)) if ln.strip() and not ln.startswith("#")]
+    assert len(rows) >= 8 and all(ln.split(",")[5] == have for ln in rows)
 
 
 def test_importance_lower_bounds_match_the_survey_table():
@@ -67,3 +102,14 @@ def test_importance_lower_bounds_match_the_survey_table():
         assert abs(got - ms) / ms < 0.04, (name, got, which)
     assert bench.importance_lower_bound_ms(C["C4"], 1, 6523.0, 1413.0)[1].startswith("hbm")
     assert bench.importance_lower_bound_ms(C["C5"], 1, 6523.0, 1413.0)[1].startswith("ex2")
+
+
+def test_both_arms_print_the_same_config_object():
+    """The driver compares `config` of the CUDA arm and of `--impl reference`: it holds the workload only (the note on
+    how the timed steps relate to L2 is a sibling key of the line), so the two are equal for equal arguments."""
+    C = skv_synth.CONFIGS
+    a = bench.config_json(C["C5"], 0.5, 4)
+    assert "l2" not in a and "workload" in a and a["n_requests"] == 4 and a["budget"] == 0.5
+    assert a == bench.config_json(C["C5"], 0.5, 4)
+    src = open(bench.__file__).read()
+    assert src.count('"config": config_json(cfg, b, R), "l2":') == 2        # the two lines: reference arm and CUDA arm
